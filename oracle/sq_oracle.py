@@ -1,0 +1,132 @@
+"""CPU fp64 ORACLE for the sq_score hot path.  TEST INFRASTRUCTURE ONLY.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` / `--impl reference`
+legs may import this file.  It shares no code with `paper_2604_07725_b200/` (the CUDA path) and
+never imports it.  It is deliberately plain and slow: every function is the *definition* of the
+quantity written out in fp64 (numpy / torch CPU ops), in the paper's notation, with no blocking,
+fusion, online update or reordering, so it can be checked against the paper by eye.
+
+What the path computes:
+
+  z[t,v]   = sum_j H[t,j] * W[v,j]                       LM-head logits (prefill-only scoring pass,
+                                                          PAPER.md:163, 199-203); bf16 inputs are widened
+                                                          to fp64 exactly, bf16*bf16 products are exact.
+  log p    = z - logsumexp_v z                           softmax at temperature 1, no bias (reading #5)
+  target_logprob[t] = log p[t, targets[t]]               "cross-model log-probabilities", PAPER.md:84
+  entropy[t]        = - sum_v p log p   (nats)           BASELINE.json north_star (not in the paper)
+  top-K_l log-probs, descending, ties by ascending index PAPER.md:149-158
+  conf[t] = c(i) = -(1/K_l) * sum_{j<=K_l} log p(v_j)    Eq. 3
+  C(tau)  = (1/|tau|) * sum_i c(i)                       Eq. 4 (left)
+  per-sequence mean target_logprob / mean entropy        BASELINE.json north_star
+  min over stride-1 full windows of length w'=min(w,L) of the window mean of c(i)
+                                                          BASELINE.json north_star (readings #9, #10)
+
+Pins (tests/test_oracle_pins.py, `-m "not gpu"`): every function below is pinned to closed forms,
+invariants or pure-Python brute force -- see the table in DESIGN.md "Oracle and its pins".
+No function here is "parity unpinned".
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+ORACLE_VERSION = 1
+
+
+def widen(x_bf16: torch.Tensor) -> torch.Tensor:
+    """bf16 -> fp64 (exact)."""
+    return x_bf16.to(torch.float64)
+
+
+def logits(H_rows: torch.Tensor, W64: torch.Tensor) -> np.ndarray:
+    """z[t,v] = sum_j H[t,j] * W[v,j] in fp64.  The library matmul is the step (a dgemm); its
+    summation order is irrelevant at the 1e-16 level because every product is exact in fp64."""
+    return (widen(H_rows) @ W64.T).numpy()
+
+
+def token_scores(H_rows: torch.Tensor, W64: torch.Tensor, targets_rows, k: int, extra: int = 1) -> dict:
+    """Per-token outputs for the given rows.  `W64 = widen(W)` is passed in so that callers can
+    convert the LM head once.  Returns k+extra top entries (the extra one lets the parity checker
+    see the gap below the k-th entry, reading #7); `conf` uses exactly the first k (Eq. 3)."""
+    z = logits(H_rows, W64)                                   # [n, V]
+    n, V = z.shape
+    tg = np.asarray(targets_rows, dtype=np.int64)
+    m = z.max(axis=1)                                         # two-pass logsumexp (not online)
+    s = np.exp(z - m[:, None]).sum(axis=1)
+    lse = m + np.log(s)
+    logp = z - lse[:, None]                                   # log p_theta(v | t_<i, Q)
+    valid = (tg >= 0) & (tg < V)                              # targets outside [0,V) = "no target"
+    target_logprob = np.where(valid, logp[np.arange(n), np.where(valid, tg, 0)], 0.0)
+    p = np.exp(logp)
+    plogp = np.where(p > 0.0, p * logp, 0.0)                  # 0 * log 0 := 0
+    entropy = -plogp.sum(axis=1)
+    kk = min(V, k + extra)
+    order = np.argsort(-logp, axis=1, kind="stable")[:, :kk]  # value desc, index asc on ties
+    topk_logprob = np.take_along_axis(logp, order, axis=1)
+    conf = -topk_logprob[:, :k].sum(axis=1) / k               # Eq. 3
+    return {"lse": lse, "target_logprob": target_logprob, "target_valid": valid, "entropy": entropy,
+            "topk_logprob": topk_logprob, "topk_index": order.astype(np.int64), "conf": conf,
+            "logp": logp}
+
+
+def window_min_mean(conf_seq: np.ndarray, window: int) -> float:
+    """min_j (1/w') * sum_{i=j}^{j+w'-1} conf[i], w' = min(window, L), j = 0..L-w' (stride 1, full
+    windows only; reading #9).  Direct re-summation of every window -- no prefix sums."""
+    L = len(conf_seq)
+    if L == 0:
+        return float("nan")
+    w = min(int(window), L)
+    best = np.inf
+    for j in range(0, L - w + 1):
+        best = min(best, float(np.sum(conf_seq[j:j + w], dtype=np.float64)) / w)
+    return best
+
+
+def sequence_scores(target_logprob, entropy, conf, cu_seqlens, window: int, target_valid=None) -> dict:
+    """Per-sequence varlen reductions over tokens [cu[b], cu[b+1]).  Means are arithmetic means
+    over the L tokens (Eq. 4 left for conf); the mean target log-prob counts only valid targets
+    (reading #11).  Empty sequences (and sequences with no valid target, for the log-prob mean)
+    give NaN."""
+    lp = np.asarray(target_logprob, dtype=np.float64)
+    en = np.asarray(entropy, dtype=np.float64)
+    cf = np.asarray(conf, dtype=np.float64)
+    cu = np.asarray(cu_seqlens, dtype=np.int64)
+    ok = np.ones(len(lp), dtype=bool) if target_valid is None else np.asarray(target_valid, dtype=bool)
+    B = len(cu) - 1
+    out = {key: np.full(B, np.nan) for key in
+           ("seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf")}
+    for b in range(B):
+        lo, hi = int(cu[b]), int(cu[b + 1])
+        L = hi - lo
+        if L <= 0:
+            continue
+        nvalid = int(ok[lo:hi].sum())
+        if nvalid > 0:
+            out["seq_mean_logprob"][b] = float(np.sum(lp[lo:hi][ok[lo:hi]])) / nvalid
+        out["seq_mean_entropy"][b] = float(np.sum(en[lo:hi])) / L
+        out["seq_mean_conf"][b] = float(np.sum(cf[lo:hi])) / L          # C(tau), Eq. 4
+        out["seq_min_window_conf"][b] = window_min_mean(cf[lo:hi], window)
+    return out
+
+
+def score(H: torch.Tensor, W: torch.Tensor, targets, cu_seqlens, k: int, window: int,
+          row_batch: int = 64) -> dict:
+    """Whole path on all rows (small cases): per-token scores, then per-sequence reductions."""
+    W64 = widen(W)
+    T = H.shape[0]
+    tg = np.asarray(targets, dtype=np.int64)
+    keys = ("lse", "target_logprob", "target_valid", "entropy", "topk_logprob", "topk_index", "conf")
+    parts = {key: [] for key in keys}
+    for r0 in range(0, T, row_batch):
+        r = token_scores(H[r0:r0 + row_batch], W64, tg[r0:r0 + row_batch], k)
+        for key in keys:
+            parts[key].append(r[key])
+    V = W.shape[0]
+    kk = min(V, k + 1)
+    tok = {key: (np.concatenate(parts[key]) if T > 0 else
+                 np.zeros((0, kk) if key.startswith("topk") else (0,)))
+           for key in keys}
+    seq = sequence_scores(tok["target_logprob"], tok["entropy"], tok["conf"], cu_seqlens, window,
+                          tok["target_valid"])
+    tok.update(seq)
+    return tok

@@ -1,0 +1,138 @@
+"""Seeded synthetic inputs for the sq_score hot path (shared by oracle tests, GPU tests and bench).
+
+This module holds NONE of the method's arithmetic: it only draws the random inputs
+(H, W, targets, cu_seqlens) with the shapes and value distributions BASELINE.json's `configs`
+name, following the recipe written out in DESIGN.md ("Input recipe").  Both the CPU oracle
+(`oracle/`) and the CUDA path (`paper_2604_07725_b200/`) consume its output as *data*.
+
+The inputs stand in for the paper's workloads -- populations of N candidate trajectories per
+problem scored by one prefill-only pass -- whose real trajectories
+and model weights are not available; only the public (d, V) shapes are borrowed.
+
+Draw order, one `torch.Generator` (CPU) per config:
+  lengths -> W (row chunks of 16384) -> targets -> planted mask -> g (row chunks of 8192).
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, replace
+from typing import Dict, Optional, Sequence
+
+import torch
+
+W_CHUNK_ROWS = 16384
+H_CHUNK_ROWS = 8192
+
+
+@dataclass(frozen=True)
+class Workload:
+    name: str
+    d: int                 # hidden size
+    V: int                 # vocabulary size
+    B: int                 # number of packed candidate sequences
+    len_lo: int            # lengths ~ U[len_lo, len_hi], inclusive ints
+    len_hi: int
+    k: int                 # K_l of Eq. 3
+    window: int            # sliding-window length w
+    w_std: float           # W ~ N(0, w_std^2)
+    planted_frac: float    # fraction of rows that get +planted_scale*W[target]
+    planted_scale: float
+    rmsnorm: bool          # H rows RMS-normalised (unit gain) before planting
+    seed: int
+    total_tokens: Optional[int] = None   # if set, lengths are redrawn until they sum to this
+
+
+# BASELINE.json `configs`, in order (index 2 = "qwen3_8b" is the graded target config).
+CONFIGS: Dict[str, Workload] = {
+    "tiny": Workload("tiny", d=64, V=1024, B=4, len_lo=32, len_hi=96, k=5, window=16,
+                     w_std=0.05, planted_frac=0.0, planted_scale=0.0, rmsnorm=False, seed=1001,
+                     total_tokens=256),
+    "qwen3_4b": Workload("qwen3_4b", d=2560, V=151936, B=8, len_lo=1024, len_hi=4096, k=20,
+                         window=2048, w_std=0.02, planted_frac=0.5, planted_scale=3.0,
+                         rmsnorm=True, seed=1002),
+    "qwen3_8b": Workload("qwen3_8b", d=4096, V=151936, B=16, len_lo=2048, len_hi=8192, k=20,
+                         window=2048, w_std=0.02, planted_frac=0.5, planted_scale=3.0,
+                         rmsnorm=True, seed=1003),
+    "gpt_oss": Workload("gpt_oss", d=2880, V=201088, B=32, len_lo=512, len_hi=4096, k=20,
+                        window=1024, w_std=0.02, planted_frac=0.3, planted_scale=3.0,
+                        rmsnorm=True, seed=1004),
+    "qwen3_32b": Workload("qwen3_32b", d=5120, V=151936, B=64, len_lo=1024, len_hi=16384, k=20,
+                          window=2048, w_std=0.02, planted_frac=0.5, planted_scale=3.0,
+                          rmsnorm=True, seed=1005),
+}
+CONFIG_ORDER = ["tiny", "qwen3_4b", "qwen3_8b", "gpt_oss", "qwen3_32b"]
+
+
+def custom(name: str = "custom", **kw) -> Workload:
+    """A workload with the same recipe but caller-chosen sizes (edge-case and stress tests)."""
+    base = Workload(name, d=64, V=1024, B=2, len_lo=8, len_hi=64, k=5, window=16, w_std=0.05,
+                    planted_frac=0.0, planted_scale=0.0, rmsnorm=False, seed=7)
+    return replace(base, **kw)
+
+
+def draw_lengths(wl: Workload, gen: torch.Generator) -> torch.Tensor:
+    """B integer lengths, U[len_lo, len_hi] inclusive.  With `total_tokens` set, the first B-1
+    are drawn and the last is the remainder; the draw is repeated (same generator, so still
+    seeded) until the remainder also lies in [len_lo, len_hi]."""
+    if wl.total_tokens is None:
+        return torch.randint(wl.len_lo, wl.len_hi + 1, (wl.B,), generator=gen, dtype=torch.int64)
+    while True:
+        head = torch.randint(wl.len_lo, wl.len_hi + 1, (wl.B - 1,), generator=gen, dtype=torch.int64)
+        last = wl.total_tokens - int(head.sum())
+        if wl.len_lo <= last <= wl.len_hi:
+            return torch.cat([head, torch.tensor([last], dtype=torch.int64)])
+
+
+def make_inputs(wl: Workload, lengths: Optional[Sequence[int]] = None) -> dict:
+    """Returns CPU tensors: H bf16 [T,d], W bf16 [V,d], targets int32 [T], cu_seqlens int32 [B+1],
+    planted bool [T], plus k, window and the workload itself.  `lengths` overrides the drawn
+    lengths (edge cases: empty sequences, L < window, ...); the generator still advances as usual."""
+    gen = torch.Generator(device="cpu")
+    gen.manual_seed(wl.seed)
+
+    drawn = draw_lengths(wl, gen)
+    lens = torch.tensor(list(lengths), dtype=torch.int64) if lengths is not None else drawn
+    cu = torch.zeros(len(lens) + 1, dtype=torch.int64)
+    cu[1:] = torch.cumsum(lens, 0)
+    T = int(cu[-1])
+
+    W = torch.empty(wl.V, wl.d, dtype=torch.bfloat16)
+    for r0 in range(0, wl.V, W_CHUNK_ROWS):
+        r1 = min(wl.V, r0 + W_CHUNK_ROWS)
+        W[r0:r1] = (torch.randn(r1 - r0, wl.d, generator=gen, dtype=torch.float32) * wl.w_std).to(torch.bfloat16)
+
+    targets = torch.randint(0, wl.V, (T,), generator=gen, dtype=torch.int64)
+    planted = torch.rand(T, generator=gen) < wl.planted_frac
+
+    H = torch.empty(T, wl.d, dtype=torch.bfloat16)
+    for r0 in range(0, T, H_CHUNK_ROWS):
+        r1 = min(T, r0 + H_CHUNK_ROWS)
+        g = torch.randn(r1 - r0, wl.d, generator=gen, dtype=torch.float32)
+        if wl.rmsnorm:
+            g = g / torch.sqrt((g * g).mean(dim=1, keepdim=True) + 1e-6)
+        p = planted[r0:r1]
+        if bool(p.any()):
+            rows = torch.nonzero(p).squeeze(1)
+            g[rows] += wl.planted_scale * W[targets[r0:r1][rows]].to(torch.float32)
+        H[r0:r1] = g.to(torch.bfloat16)
+
+    return {
+        "H": H, "W": W, "targets": targets.to(torch.int32), "cu_seqlens": cu.to(torch.int32),
+        "planted": planted, "k": wl.k, "window": wl.window, "workload": wl,
+        "T": T, "B": len(lens),
+    }
+
+
+def reduction_inputs(num_seqs: int, len_lo: int, len_hi: int, seed: int = 2001) -> dict:
+    """Per-token arrays shaped like kernel 1's outputs, for timing/testing the segmented
+    reduction alone at a size where HBM bandwidth is meaningful."""
+    gen = torch.Generator(device="cpu")
+    gen.manual_seed(seed)
+    lens = torch.randint(len_lo, len_hi + 1, (num_seqs,), generator=gen, dtype=torch.int64)
+    cu = torch.zeros(num_seqs + 1, dtype=torch.int64)
+    cu[1:] = torch.cumsum(lens, 0)
+    T = int(cu[-1])
+    target_logprob = -(torch.rand(T, generator=gen) * 12.0)
+    entropy = torch.rand(T, generator=gen) * 11.9
+    conf = 3.0 + torch.rand(T, generator=gen) * 12.0
+    return {"target_logprob": target_logprob.float(), "entropy": entropy.float(), "conf": conf.float(),
+            "cu_seqlens": cu.to(torch.int32), "T": T, "B": num_seqs}
