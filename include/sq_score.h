@@ -1,0 +1,164 @@
+/*
+ * sq_score.h -- C ABI of the B200-native fused LM-head scoring library (libsq_score.so).
+ *
+ * The hot path is the prefill-side token-scoring pass behind SQUEEZE EVOLVE's confidence-based
+ * routing (arxiv 2604.07725):
+ *   - per-token top-K_l confidence  c(i) = -(1/K_l) * sum_{j<=K_l} log p(v_j^(i) | t_<i, Q)     Eq. 3
+ *   - per-trajectory confidence     C(tau) = (1/|tau|) * sum_i c(i)                             Eq. 4
+ *   - "cross-model log-probabilities" of the trajectory tokens
+ *   - one prefill-only pass over the N batched candidates, reduced on the GPU so that only
+ *     scalars per trajectory leave the device
+ *   - entropy and the sliding-window minimum are defined by BASELINE.json `north_star`.
+ *
+ * Given final hidden states H[T,d] and an LM head W[V,d] (bf16, row-major = K-major) the library
+ * never materialises the [T,V] logits: kernel 1 fuses the vocabulary GEMM (tcgen05 / TMEM / TMA,
+ * sm_100a) with an online logsumexp, target-logit capture, entropy and streaming top-k; a merge
+ * kernel combines vocab-chunk partial states; kernel 2 does the per-sequence varlen reductions.
+ *
+ * Conventions
+ *   - every function returns 0 (SQ_OK) or a negative SQ_ERR_* code; nothing aborts or throws.
+ *   - `sq_score_run` / `sq_score_reduce` are ASYNCHRONOUS on `stream` (a cudaStream_t passed as
+ *     void*), do no host synchronisation and no allocation; all workspace is owned by the ctx and
+ *     sized at create from max_tokens / max_seqs / max_k.
+ *   - pointers marked DEVICE must be device memory on ctx's device; HOST pointers are host memory
+ *     (pinned for true async copies).  The library never frees or keeps caller buffers beyond the
+ *     work it enqueued.
+ *   - H and W: bf16, contiguous, 16-byte aligned, d % 8 == 0 (TMA 16-byte stride rule).
+ *   - cu_seqlens[0] = 0, non-decreasing, cu_seqlens[B] = T.  Device-side contents are trusted.
+ *   - targets[t] outside [0, V) means "no target": target_logprob[t] = 0 and the token is left out
+ *     of seq_mean_logprob (numerator and denominator).
+ *   - empty sequences give NaN aggregates; window' = min(window, L), stride 1, full windows only.
+ *   - one ctx per host thread / stream.  There is no CPU fallback: without a B200-class device
+ *     `sq_score_create` fails with SQ_ERR_CUDA / SQ_ERR_UNSUPPORTED.
+ */
+#ifndef SQ_SCORE_H_
+#define SQ_SCORE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SQ_OK                 0
+#define SQ_ERR_INVALID_ARG   -1   /* null pointer, size out of range, k > max_k, ...              */
+#define SQ_ERR_UNSUPPORTED   -2   /* shape or device the kernels do not cover (d % 8, not sm_100) */
+#define SQ_ERR_CUDA          -3   /* a CUDA runtime/driver call failed; see sq_score_last_error   */
+#define SQ_ERR_NOMEM         -4   /* workspace allocation failed                                  */
+
+#define SQ_MAX_K             32   /* largest K_l the streaming top-k supports                     */
+
+typedef struct sq_score_ctx sq_score_ctx;   /* opaque */
+
+/* Fixed per context (one scorer model = one LM head shape). */
+typedef struct {
+  int     device;       /* CUDA device ordinal                                                    */
+  int     d;            /* hidden size, d % 8 == 0                                                */
+  int     vocab;        /* V                                                                      */
+  int64_t max_tokens;   /* largest T of any run (sizes the partial-state workspace)               */
+  int     max_seqs;     /* largest B of any run                                                   */
+  int     max_k;        /* largest k of any run, 1..SQ_MAX_K                                      */
+  int     cta_group;    /* 0 = default (2: CTA pairs, UMMA M=256); 1 = single-CTA UMMA (M=128)    */
+  int     num_chunks;   /* 0 = planner's choice; >0 forces the number of vocab chunks per row     */
+  int     group_m;      /* 0 = default (8): token tiles that share a W stream through L2          */
+} sq_score_config;
+
+/* Output pointers of one run.  Per-token pointers may be NULL (= not wanted; the ctx keeps the
+ * 12 B/token kernel 2 needs in its own scratch).  Per-sequence pointers are required. */
+typedef struct {
+  float   *lse;                 /* DEVICE [T]   logsumexp_v z[t,v]                                */
+  float   *target_logprob;      /* DEVICE [T]   z[t,targets[t]] - lse[t]     */
+  float   *entropy;             /* DEVICE [T]   -sum_v p log p, nats                              */
+  float   *conf;                /* DEVICE [T]   c(i), Eq. 3    */
+  float   *topk_logprob;        /* DEVICE [T,k] row-major, descending                             */
+  int32_t *topk_index;          /* DEVICE [T,k] vocabulary ids of topk_logprob                    */
+  float   *seq_mean_logprob;    /* DEVICE [B]   mean target_logprob over valid targets            */
+  float   *seq_mean_entropy;    /* DEVICE [B]                                                     */
+  float   *seq_mean_conf;       /* DEVICE [B]   C(tau), Eq. 4    */
+  float   *seq_min_window_conf; /* DEVICE [B]   min over windows of the window-mean of c(i)       */
+} sq_score_outputs;
+
+/* How a run of T tokens is cut into work units (host logic, no GPU needed).       */
+typedef struct {
+  int cta_group;        /* 1 or 2                                                                 */
+  int rows_per_tile;    /* 128 * cta_group token rows per work unit                               */
+  int m_tiles;          /* ceil(T / rows_per_tile)                                                */
+  int num_vtiles;       /* ceil(V / 256)                                                          */
+  int num_k_blocks;     /* ceil(d / 64)                                                           */
+  int num_chunks;       /* vocab chunks per row (partial states merged by the finalize kernel)    */
+  int tiles_per_chunk;  /* vocab tiles swept by one work unit                                     */
+  int group_m;          /* consecutive units that share one W chunk                               */
+  int num_units;        /* m_tiles * num_chunks                                                   */
+  int num_clusters;     /* persistent grid size in clusters (= CTAs / cta_group)                  */
+  int topk_cap;         /* compiled top-k list capacity used for this k (8, 20 or 32)             */
+} sq_score_plan_t;
+
+/* Creates a context on cfg->device and allocates its workspace.
+ * Errors: INVALID_ARG (null, sizes <= 0, max_k out of range), UNSUPPORTED (d % 8 != 0, device is
+ * not compute capability 10.x), CUDA, NOMEM.  On error *out is NULL. */
+int sq_score_create(const sq_score_config *cfg, sq_score_ctx **out);
+
+/* Scores T = outputs->... tokens: enqueues kernel 1 (fused GEMM + statistics), the merge/finalize
+ * kernel and kernel 2 on `stream`.
+ *   H          DEVICE bf16 [T,d]       final hidden states; row t predicts targets[t] (the caller
+ *                                      does the next-token shift and packs only trajectory tokens)
+ *   W          DEVICE bf16 [V,d]       LM head
+ *   targets    DEVICE int32 [T]
+ *   cu_seqlens DEVICE int32 [B+1]
+ *   k          1..min(max_k, V)        K_l of Eq. 3
+ *   window     >= 1
+ * T == 0 or B == 0 is legal (nothing / NaNs are written).
+ * Errors: INVALID_ARG (null required pointer, T > max_tokens, B > max_seqs, k or window out of
+ * range, misaligned H/W), CUDA. */
+int sq_score_run(sq_score_ctx *ctx, const void *H, const void *W, const int32_t *targets,
+                 const int32_t *cu_seqlens, int num_tokens, int num_seqs, int k, int window,
+                 const sq_score_outputs *outputs, void *stream);
+
+/* End-to-end form with HOST inputs and HOST results: copies H, targets and cu_seqlens to ctx-owned
+ * device staging buffers, runs the same kernels, and copies the 4*B per-sequence scalars back
+ * (order: mean_logprob[B], mean_entropy[B], mean_conf[B], min_window_conf[B]).  W stays on the
+ * device (it is the resident model weight).  Asynchronous on `stream`; the caller synchronises
+ * the stream before reading seq_out_host.
+ * Errors: as sq_score_run. */
+int sq_score_run_host(sq_score_ctx *ctx, const void *H_host, const void *W_dev,
+                      const int32_t *targets_host, const int32_t *cu_seqlens_host,
+                      int num_tokens, int num_seqs, int k, int window,
+                      float *seq_out_host, void *stream);
+
+/* Kernel 2 alone: per-sequence varlen reductions of caller-provided per-token arrays.
+ *   target_logprob, entropy, conf  DEVICE float [T]
+ *   targets                        DEVICE int32 [T] or NULL (NULL = every target valid)
+ *   seq_* outputs                  DEVICE float [B]
+ * Errors: INVALID_ARG, CUDA. */
+int sq_score_reduce(sq_score_ctx *ctx, const float *target_logprob, const float *entropy,
+                    const float *conf, const int32_t *targets, const int32_t *cu_seqlens,
+                    int64_t num_tokens, int num_seqs, int window,
+                    float *seq_mean_logprob, float *seq_mean_entropy, float *seq_mean_conf,
+                    float *seq_min_window_conf, void *stream);
+
+/* Host-only: the work decomposition `sq_score_run` would use for T tokens and top-k `k` on a
+ * device with `num_sms` SMs (pass 0 for the ctx-independent default of 148).  `cfg` supplies d,
+ * vocab, cta_group, num_chunks, group_m.  Needs no GPU.  Errors: INVALID_ARG. */
+int sq_score_plan(const sq_score_config *cfg, int64_t num_tokens, int k, int num_sms,
+                  sq_score_plan_t *plan);
+
+/* Number of kernels this ctx has launched so far (bench.py's `gpu_launches`). */
+int64_t sq_score_launch_count(const sq_score_ctx *ctx);
+
+/* Frees the workspace.  NULL is a no-op.  Errors: CUDA. */
+int sq_score_destroy(sq_score_ctx *ctx);
+
+/* Message of the last error on this ctx (ctx-owned, valid until the next call on ctx); with
+ * ctx == NULL, the message of the last failed sq_score_create on this thread. */
+const char *sq_score_last_error(const sq_score_ctx *ctx);
+
+/* Static name of an SQ_ERR_* code. */
+const char *sq_score_error_string(int code);
+
+/* Library version, e.g. 100 = 0.1.0. */
+int sq_score_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SQ_SCORE_H_ */

@@ -1,0 +1,7 @@
+"""sq_score -- B200-native fused LM-head scoring (SQUEEZE EVOLVE confidence path, Eq. 3 / Eq. 4).
+
+Thin ctypes binding over the C ABI in include/sq_score.h.  Argument marshalling only: every step
+of the path runs in the CUDA kernels of csrc/.  There is no CPU fallback.
+"""
+from .binding import (SqScore, SqScoreError, plan, lib, version, shard_sequences,  # noqa: F401
+                      SQ_MAX_K, ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOMEM)

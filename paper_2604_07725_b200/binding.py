@@ -1,0 +1,192 @@
+"""ctypes binding with the same names as the C ABI (include/sq_score.h)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, List, Optional, Sequence
+
+from . import build as _build
+
+SQ_MAX_K = 32
+ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOMEM = -1, -2, -3, -4
+
+
+class sq_score_config(C.Structure):
+    _fields_ = [("device", C.c_int), ("d", C.c_int), ("vocab", C.c_int), ("max_tokens", C.c_int64),
+                ("max_seqs", C.c_int), ("max_k", C.c_int), ("cta_group", C.c_int), ("num_chunks", C.c_int),
+                ("group_m", C.c_int)]
+
+
+class sq_score_outputs(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in
+                ("lse", "target_logprob", "entropy", "conf", "topk_logprob", "topk_index",
+                 "seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf")]
+
+
+class sq_score_plan_t(C.Structure):
+    _fields_ = [(n, C.c_int) for n in
+                ("cta_group", "rows_per_tile", "m_tiles", "num_vtiles", "num_k_blocks", "num_chunks",
+                 "tiles_per_chunk", "group_m", "num_units", "num_clusters", "topk_cap")]
+
+
+class SqScoreError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__("sq_score error %d: %s" % (code, msg))
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Loads (building if stale) csrc/libsq_score.so.  Fails loudly if it cannot be built/loaded."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.is_stale():
+        try:
+            path = _build.build()
+        except Exception:
+            if not os.path.exists(path):
+                raise
+    L = C.CDLL(path)
+    L.sq_score_create.argtypes = [C.POINTER(sq_score_config), C.POINTER(C.c_void_p)]
+    L.sq_score_create.restype = C.c_int
+    L.sq_score_run.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                               C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
+    L.sq_score_run.restype = C.c_int
+    L.sq_score_run_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                    C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+    L.sq_score_run_host.restype = C.c_int
+    L.sq_score_reduce.argtypes = [C.c_void_p] + [C.c_void_p] * 5 + [C.c_int64, C.c_int, C.c_int] + [C.c_void_p] * 5
+    L.sq_score_reduce.restype = C.c_int
+    L.sq_score_plan.argtypes = [C.POINTER(sq_score_config), C.c_int64, C.c_int, C.c_int, C.POINTER(sq_score_plan_t)]
+    L.sq_score_plan.restype = C.c_int
+    L.sq_score_launch_count.argtypes = [C.c_void_p]
+    L.sq_score_launch_count.restype = C.c_int64
+    L.sq_score_destroy.argtypes = [C.c_void_p]
+    L.sq_score_destroy.restype = C.c_int
+    L.sq_score_last_error.argtypes = [C.c_void_p]
+    L.sq_score_last_error.restype = C.c_char_p
+    L.sq_score_error_string.argtypes = [C.c_int]
+    L.sq_score_error_string.restype = C.c_char_p
+    L.sq_score_version.argtypes = []
+    L.sq_score_version.restype = C.c_int
+    _lib = L
+    return L
+
+
+def version() -> int:
+    return lib().sq_score_version()
+
+
+def plan(d: int, vocab: int, num_tokens: int, k: int, num_sms: int = 0, cta_group: int = 0,
+         num_chunks: int = 0, group_m: int = 0) -> Dict[str, int]:
+    """sq_score_plan: host-only work decomposition (no GPU needed)."""
+    cfg = sq_score_config(0, d, vocab, max(1, num_tokens), 1, max(1, min(k, SQ_MAX_K)), cta_group, num_chunks, group_m)
+    out = sq_score_plan_t()
+    rc = lib().sq_score_plan(C.byref(cfg), num_tokens, k, num_sms, C.byref(out))
+    if rc != 0:
+        raise SqScoreError(rc, lib().sq_score_error_string(rc).decode())
+    return {n: getattr(out, n) for n, _ in sq_score_plan_t._fields_}
+
+
+def _ptr(t) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+class SqScore:
+    """sq_score_create / sq_score_run / sq_score_destroy on torch tensors (device memory + streams)."""
+
+    def __init__(self, d: int, vocab: int, max_tokens: int, max_seqs: int, max_k: int = 20, device: int = 0,
+                 cta_group: int = 0, num_chunks: int = 0, group_m: int = 0):
+        self._L = lib()
+        self.cfg = sq_score_config(device, d, vocab, max_tokens, max_seqs, max_k, cta_group, num_chunks, group_m)
+        h = C.c_void_p()
+        rc = self._L.sq_score_create(C.byref(self.cfg), C.byref(h))
+        if rc != 0:
+            raise SqScoreError(rc, self._L.sq_score_last_error(None).decode())
+        self._h = h
+        self.device = device
+
+    def _check(self, rc: int):
+        if rc != 0:
+            raise SqScoreError(rc, self._L.sq_score_last_error(self._h).decode())
+
+    @staticmethod
+    def _stream(stream) -> int:
+        import torch
+        s = stream if stream is not None else torch.cuda.current_stream()
+        return s.cuda_stream
+
+    def run(self, H, W, targets, cu_seqlens, k: int, window: int, stream=None, per_token: bool = True,
+            topk: bool = True, out: Optional[dict] = None) -> dict:
+        """sq_score_run.  Allocates (or reuses `out`) the output tensors; asynchronous on the stream."""
+        import torch
+        T, B = H.shape[0], cu_seqlens.shape[0] - 1
+        dev = H.device
+        if out is None:
+            out = {}
+            f = dict(dtype=torch.float32, device=dev)
+            if per_token:
+                for n in ("lse", "target_logprob", "entropy", "conf"):
+                    out[n] = torch.empty(T, **f)
+            if topk:
+                out["topk_logprob"] = torch.empty(T, k, **f)
+                out["topk_index"] = torch.empty(T, k, dtype=torch.int32, device=dev)
+            for n in ("seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf"):
+                out[n] = torch.empty(B, **f)
+        o = sq_score_outputs(*[_ptr(out.get(n)) for n, _ in sq_score_outputs._fields_])
+        self._check(self._L.sq_score_run(self._h, _ptr(H), _ptr(W), _ptr(targets), _ptr(cu_seqlens), T, B, k, window,
+                                         C.byref(o), self._stream(stream)))
+        return out
+
+    def run_host(self, H_host, W_dev, targets_host, cu_seqlens_host, k: int, window: int, seq_out_host, stream=None):
+        """sq_score_run_host: host inputs -> 4*B host floats (copies are inside the call)."""
+        T, B = H_host.shape[0], cu_seqlens_host.shape[0] - 1
+        self._check(self._L.sq_score_run_host(self._h, _ptr(H_host), _ptr(W_dev), _ptr(targets_host),
+                                              _ptr(cu_seqlens_host), T, B, k, window, _ptr(seq_out_host),
+                                              self._stream(stream)))
+        return seq_out_host
+
+    def reduce(self, target_logprob, entropy, conf, cu_seqlens, window: int, targets=None, stream=None) -> dict:
+        """sq_score_reduce: kernel 2 alone."""
+        import torch
+        B = cu_seqlens.shape[0] - 1
+        out = {n: torch.empty(B, dtype=torch.float32, device=conf.device)
+               for n in ("seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf")}
+        self._check(self._L.sq_score_reduce(self._h, _ptr(target_logprob), _ptr(entropy), _ptr(conf), _ptr(targets),
+                                            _ptr(cu_seqlens), conf.shape[0], B, window,
+                                            _ptr(out["seq_mean_logprob"]), _ptr(out["seq_mean_entropy"]),
+                                            _ptr(out["seq_mean_conf"]), _ptr(out["seq_min_window_conf"]),
+                                            self._stream(stream)))
+        return out
+
+    def launch_count(self) -> int:
+        return self._L.sq_score_launch_count(self._h)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.sq_score_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def shard_sequences(lengths: Sequence[int], world_size: int) -> List[List[int]]:
+    """Multi-GPU partition: whole sequences to ranks, longest first onto the
+    least-loaded rank (ties -> lowest rank).  No collective on the data path; W is replicated."""
+    loads = [0] * world_size
+    parts: List[List[int]] = [[] for _ in range(world_size)]
+    for i in sorted(range(len(lengths)), key=lambda i: (-int(lengths[i]), i)):
+        r = min(range(world_size), key=lambda r: (loads[r], r))
+        parts[r].append(i)
+        loads[r] += int(lengths[i])
+    for p in parts:
+        p.sort()
+    return parts

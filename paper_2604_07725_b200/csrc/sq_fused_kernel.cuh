@@ -1,0 +1,333 @@
+// sq_fused_kernel.cuh -- kernel 1: fused vocabulary GEMM + online softmax statistics (sm_100a).
+//
+// Steps a1..a5 of the hot path: logits tile Z = H_tile * W_tile^T by
+// tcgen05.mma into TMEM (never written to memory), then per row an online logsumexp (m, s), the
+// shifted entropy accumulator u = sum e^{z-m}(z-m), the target logit, and a streaming top-k list
+// -- the quantities Eq. 3 needs: log p(v_j) = z_(j) - lse.
+//
+// Persistent, warp-specialised:  warp 0 = TMA producer, warp 1 = MMA issuer, warp 2 = TMEM
+// allocator, warps 4..7 = statistics epilogue (thread = TMEM lane = token row).
+// Work unit = (token tile of 128*CG rows, vocab chunk of `tiles_per_chunk` 256-column tiles);
+// a unit's running state lives in registers and is written as a partial state at its end.
+#pragma once
+#include "sq_ptx.cuh"
+
+namespace sq {
+
+constexpr int BLOCK_M = 128;   // token rows per CTA = TMEM lanes
+constexpr int BLOCK_N = 256;   // vocabulary columns per tile = UMMA N
+constexpr int BLOCK_K = 64;    // bf16 per k-block: 128 B = one swizzle-128B row
+constexpr int UMMA_K = 16;
+constexpr int NUM_THREADS = 256;
+constexpr int EPI_WARP0 = 4;
+constexpr int TMEM_COLS = 512;  // two 256-column accumulator stages
+constexpr float NEG_BIG = -1.0e30f;
+constexpr float LOG2E = 1.4426950408889634f;
+
+template <int CG> struct FusedCfg {
+  static constexpr int A_BYTES = BLOCK_M * BLOCK_K * 2;                 // 16 KB
+  static constexpr int B_ROWS = BLOCK_N / CG;                           // W rows this CTA stages
+  static constexpr int B_BYTES = B_ROWS * BLOCK_K * 2;                  // 32 KB (CG=1) / 16 KB (CG=2)
+  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  static constexpr int STAGES = (CG == 1) ? 4 : 6;
+  static constexpr int BAR_BYTES = 256;
+  static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;  // +1024: manual alignment
+  static constexpr int UMMA_M = BLOCK_M * CG;
+};
+
+struct FusedParams {
+  int T, V, d;
+  int num_k_blocks;
+  int num_vtiles;
+  int tiles_per_chunk;
+  int num_chunks;
+  int m_tiles;
+  int group_m;
+  int num_units;
+  const int32_t* targets;   // [T]
+  float* part_m;            // [C][T]
+  float* part_s;            // [C][T]
+  float* part_u;            // [C][T]
+  float* part_topv;         // [C][CAP][T]
+  int32_t* part_topi;       // [C][CAP][T]
+  float* zt;                // [T] target logit (written by the chunk that owns the target column)
+};
+
+struct Unit { int m_tile; int chunk; };
+
+__device__ __forceinline__ Unit decode_unit(const FusedParams& p, int u) {
+  // units ordered [group of group_m token tiles][chunk][tile in group]: the group_m units that are
+  // handed out back to back sweep the same W chunk in near lockstep and share it through L2.
+  const int per_group = p.group_m * p.num_chunks;
+  const int g = u / per_group;
+  const int r = u - g * per_group;
+  const int first = g * p.group_m;
+  const int gsize = min(p.group_m, p.m_tiles - first);
+  Unit out;
+  out.chunk = r / gsize;
+  out.m_tile = first + (r - out.chunk * gsize);
+  return out;
+}
+
+// value of r[i] for a run-time i without local memory: a 5-level select tree.
+__device__ __forceinline__ float pick32(const float (&r)[32], int i) {
+  float a[16], b[8], c[4], d2[2];
+#pragma unroll
+  for (int j = 0; j < 16; ++j) a[j] = (i & 1) ? r[2 * j + 1] : r[2 * j];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) b[j] = (i & 2) ? a[2 * j + 1] : a[2 * j];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) c[j] = (i & 4) ? b[2 * j + 1] : b[2 * j];
+#pragma unroll
+  for (int j = 0; j < 2; ++j) d2[j] = (i & 8) ? c[2 * j + 1] : c[2 * j];
+  return (i & 16) ? d2[1] : d2[0];
+}
+
+// Sorted (descending) insertion of (z, idx) into a register-resident list; the last entry drops out.
+template <int CAP>
+__device__ __forceinline__ void topk_insert(float (&tv)[CAP], int (&ti)[CAP], float z, int idx) {
+#pragma unroll
+  for (int j = CAP - 1; j >= 1; --j) {
+    const bool above = z > tv[j - 1];   // z belongs above slot j-1: slot j takes slot j-1
+    const bool here = z > tv[j];
+    ti[j] = above ? ti[j - 1] : (here ? idx : ti[j]);
+    tv[j] = above ? tv[j - 1] : (here ? z : tv[j]);
+  }
+  if (z > tv[0]) { tv[0] = z; ti[0] = idx; }
+}
+
+// Per-row running state of one work unit.
+template <int CAP> struct RowState {
+  float m, s, u, zt;
+  float tv[CAP];
+  int ti[CAP];
+  __device__ __forceinline__ void reset() {
+    m = NEG_BIG; s = 0.f; u = 0.f; zt = 0.f;
+#pragma unroll
+    for (int j = 0; j < CAP; ++j) { tv[j] = NEG_BIG; ti[j] = -1; }
+  }
+};
+
+// Consumes 32 consecutive logits of one row (columns col0 .. col0+31).
+template <int CAP>
+__device__ __forceinline__ void consume32(RowState<CAP>& st, float (&r)[32], int col0, int V, int tgt) {
+  if (col0 + 32 > V) {   // ragged vocabulary tail: columns >= V hold TMA zero fill
+#pragma unroll
+    for (int i = 0; i < 32; ++i) r[i] = (col0 + i < V) ? r[i] : NEG_BIG;
+  }
+  float g0 = fmaxf(r[0], r[1]), g1 = fmaxf(r[2], r[3]);
+#pragma unroll
+  for (int i = 4; i < 32; i += 4) {
+    g0 = fmaxf(g0, fmaxf(r[i], r[i + 1]));
+    g1 = fmaxf(g1, fmaxf(r[i + 2], r[i + 3]));
+  }
+  const float gmax = fmaxf(g0, g1);
+  if (gmax > st.m) {   // new running maximum: rescale s and the shifted entropy sum
+    const float dm = st.m - gmax;
+    const float sc = ex2_approx(dm * LOG2E);
+    st.u = (st.u + dm * st.s) * sc;
+    st.s *= sc;
+    st.m = gmax;
+  }
+  const float m = st.m;
+  float s0 = 0.f, s1 = 0.f, u0 = 0.f, u1 = 0.f;
+#pragma unroll
+  for (int i = 0; i < 32; i += 2) {
+    const float t0 = r[i] - m, t1 = r[i + 1] - m;
+    const float e0 = ex2_approx(t0 * LOG2E), e1 = ex2_approx(t1 * LOG2E);
+    s0 += e0; s1 += e1;
+    u0 = fmaf(e0, t0, u0); u1 = fmaf(e1, t1, u1);
+  }
+  st.s += s0 + s1;
+  st.u += u0 + u1;
+
+  if ((unsigned)(tgt - col0) < 32u) st.zt = pick32(r, tgt - col0);   // a3: target logit
+
+  if (gmax > st.tv[CAP - 1]) {   // a5: some element of this row beats the current k-th best
+    uint32_t mask = 0;
+    const float thr = st.tv[CAP - 1];
+#pragma unroll
+    for (int i = 0; i < 32; ++i) mask |= (r[i] > thr) ? (1u << i) : 0u;
+    while (mask) {
+      const int i = __ffs(mask) - 1;
+      mask &= mask - 1;
+      const float z = pick32(r, i);
+      if (z > st.tv[CAP - 1]) topk_insert<CAP>(st.tv, st.ti, z, col0 + i);
+    }
+  }
+}
+
+template <int CG, int CAP>
+__global__ void __launch_bounds__(NUM_THREADS, 1)
+sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_constant__ CUtensorMap tmap_w,
+                      const FusedParams p) {
+  using Cfg = FusedCfg<CG>;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // swizzle-128B: 1024-B aligned tiles
+  const uint32_t bar_base = smem_base + Cfg::STAGES * Cfg::STAGE_BYTES;
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (Cfg::STAGES + s); };
+  auto tfull_bar = [&](int a) { return bar_base + 8u * (2 * Cfg::STAGES + a); };
+  auto tempty_bar = [&](int a) { return bar_base + 8u * (2 * Cfg::STAGES + 2 + a); };
+  const uint32_t tmem_slot = bar_base + 8u * (2 * Cfg::STAGES + 4);
+  auto smem_a = [&](int s) { return smem_base + s * Cfg::STAGE_BYTES; };
+  auto smem_b = [&](int s) { return smem_base + s * Cfg::STAGE_BYTES + Cfg::A_BYTES; };
+
+  const int warp = threadIdx.x >> 5;
+  const uint32_t lane = lane_id();
+  const uint32_t cta_rank = (CG == 2) ? cluster_ctarank() : 0u;
+  const bool leader = (cta_rank == 0);
+  const int cluster = (CG == 2) ? (int)cluster_id_x() : (int)blockIdx.x;
+  const int ncluster = (CG == 2) ? (int)num_clusters_x() : (int)gridDim.x;
+
+  if (warp == 0 && lane == 0) {
+    prefetch_tensormap(&tmap_h);
+    prefetch_tensormap(&tmap_w);
+  }
+  if (warp == 1 && lane == 0) {
+    for (int s = 0; s < Cfg::STAGES; ++s) {
+      mbar_init(full_bar(s), 1);
+      mbar_init(empty_bar(s), 1);
+    }
+    for (int a = 0; a < 2; ++a) {
+      mbar_init(tfull_bar(a), 1);
+      mbar_init(tempty_bar(a), 4 * CG);   // one elected lane per epilogue warp, both CTAs of a pair
+    }
+    fence_mbar_init();
+  }
+  if (warp == 2) {
+    tmem_alloc<CG>(tmem_slot, TMEM_COLS);
+    tmem_relinquish<CG>();
+  }
+  __syncwarp();
+  tc_fence_before();
+  if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
+  tc_fence_after();
+  uint32_t tmem_base;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+
+  const int rows_per_unit = BLOCK_M * CG;
+
+  if (warp == 0) {
+    // ===================================================================== TMA producer
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      const uint32_t stage_tx = Cfg::STAGE_BYTES * CG;   // the pair leader's barrier counts both CTAs' bytes
+      for (int u = cluster; u < p.num_units; u += ncluster) {
+        const Unit un = decode_unit(p, u);
+        const int row0 = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M;
+        const int vt0 = un.chunk * p.tiles_per_chunk;
+        const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
+        for (int vt = vt0; vt < vt1; ++vt) {
+          const int wrow0 = vt * BLOCK_N + (int)cta_rank * Cfg::B_ROWS;
+          for (int kb = 0; kb < p.num_k_blocks; ++kb) {
+            mbar_wait(empty_bar(stage), phase ^ 1u);
+            if constexpr (CG == 1) {
+              mbar_arrive_expect_tx(full_bar(stage), stage_tx);
+              tma_load_2d(smem_a(stage), &tmap_h, full_bar(stage), kb * BLOCK_K, row0);
+              tma_load_2d(smem_b(stage), &tmap_w, full_bar(stage), kb * BLOCK_K, wrow0);
+            } else {
+              const uint32_t bar = mapa(full_bar(stage), 0);
+              if (leader) mbar_arrive_expect_tx(full_bar(stage), stage_tx);
+              tma_load_2d_pair(smem_a(stage), &tmap_h, bar, kb * BLOCK_K, row0);
+              tma_load_2d_pair(smem_b(stage), &tmap_w, bar, kb * BLOCK_K, wrow0);
+            }
+            if (++stage == Cfg::STAGES) { stage = 0; phase ^= 1u; }
+          }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================================================================== MMA issuer (pair leader only)
+    if (leader && lane == 0) {
+      constexpr uint32_t idesc = make_idesc_bf16(Cfg::UMMA_M, BLOCK_N);
+      int stage = 0; uint32_t phase = 0;
+      uint32_t tile = 0;
+      for (int u = cluster; u < p.num_units; u += ncluster) {
+        const Unit un = decode_unit(p, u);
+        const int vt0 = un.chunk * p.tiles_per_chunk;
+        const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
+        for (int vt = vt0; vt < vt1; ++vt, ++tile) {
+          const uint32_t acc = tile & 1u;
+          mbar_wait(tempty_bar(acc), ((tile >> 1) & 1u) ^ 1u);   // epilogue drained this accumulator
+          tc_fence_after();
+          const uint32_t d_tmem = tmem_base + acc * BLOCK_N;
+          for (int kb = 0; kb < p.num_k_blocks; ++kb) {
+            mbar_wait(full_bar(stage), phase);
+            tc_fence_after();
+            const uint64_t adesc = make_smem_desc_sw128(smem_a(stage));
+            const uint64_t bdesc = make_smem_desc_sw128(smem_b(stage));
+#pragma unroll
+            for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
+              // +32 B per UMMA_K step inside the 128-B swizzle row: +2 in the (addr >> 4) field
+              umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+            }
+            umma_commit<CG>(empty_bar(stage));   // smem slot free once these MMAs retire
+            if (++stage == Cfg::STAGES) { stage = 0; phase ^= 1u; }
+          }
+          umma_commit<CG>(tfull_bar(acc));       // accumulator ready for the epilogue
+        }
+      }
+    }
+  } else if (warp >= EPI_WARP0) {
+    // ===================================================================== statistics epilogue
+    const int q = warp & 3;                       // TMEM lane quarter this warp may read
+    const int row_in_tile = q * 32 + (int)lane;
+    const uint32_t lane_addr = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
+    const uint32_t tempty_remote = (CG == 2) ? mapa(tempty_bar(0), 0) : tempty_bar(0);
+    RowState<CAP> st;
+    uint32_t tile = 0;
+    for (int u = cluster; u < p.num_units; u += ncluster) {
+      const Unit un = decode_unit(p, u);
+      const int row = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M + row_in_tile;
+      const int vt0 = un.chunk * p.tiles_per_chunk;
+      const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
+      const int tgt = (row < p.T) ? __ldg(p.targets + row) : -1;
+      st.reset();
+      for (int vt = vt0; vt < vt1; ++vt, ++tile) {
+        const uint32_t acc = tile & 1u;
+        mbar_wait(tfull_bar(acc), (tile >> 1) & 1u);
+        tc_fence_after();
+        const int colbase = vt * BLOCK_N;
+        const int ngroups = min(BLOCK_N, p.V - colbase + 31) >> 5;   // 32-column groups with a valid column
+        for (int g = 0; g < ngroups; ++g) {
+          float r[32];
+          tmem_ld_32x32(lane_addr + acc * BLOCK_N + g * 32, r);
+          tmem_ld_wait();
+          consume32<CAP>(st, r, colbase + g * 32, p.V, tgt);
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          if constexpr (CG == 2) mbar_arrive_cluster(tempty_remote + 8u * acc);
+          else mbar_arrive(tempty_bar(acc));
+        }
+      }
+      if (row < p.T) {
+        const size_t o = (size_t)un.chunk * p.T + row;
+        p.part_m[o] = st.m;
+        p.part_s[o] = st.s;
+        p.part_u[o] = st.u;
+#pragma unroll
+        for (int j = 0; j < CAP; ++j) {
+          const size_t oj = ((size_t)un.chunk * CAP + j) * p.T + row;
+          p.part_topv[oj] = st.tv[j];
+          p.part_topi[oj] = st.ti[j];
+        }
+        const int c0 = vt0 * BLOCK_N;
+        if (tgt >= c0 && tgt < min(vt1 * BLOCK_N, p.V)) p.zt[row] = st.zt;
+      }
+    }
+  }
+
+  // ----------------------------------------------------------------------- teardown
+  __syncwarp();
+  tc_fence_before();
+  if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
+  if (warp == 2) {
+    tc_fence_after();
+    tmem_dealloc<CG>(tmem_base, TMEM_COLS);
+  }
+}
+
+}  // namespace sq

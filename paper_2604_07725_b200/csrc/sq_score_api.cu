@@ -1,0 +1,427 @@
+// sq_score_api.cu -- C ABI of libsq_score.so (include/sq_score.h): context, planning, TMA tensor
+// maps and kernel launches.  No torch types, no CPU fallback.
+#include "../../include/sq_score.h"
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "sq_finalize_kernel.cuh"
+#include "sq_fused_kernel.cuh"
+#include "sq_reduce_kernel.cuh"
+
+#define SQ_VERSION 100
+
+struct sq_score_ctx {
+  sq_score_config cfg;
+  int num_sms = 0;
+  int cap_max = 0;          // top-k capacity the workspace is sized for
+  int chunks_max = 0;       // largest num_chunks the workspace holds
+  int64_t launches = 0;
+  char err[512] = {0};
+  // partial states
+  float* part_m = nullptr; float* part_s = nullptr; float* part_u = nullptr;
+  float* part_topv = nullptr; int32_t* part_topi = nullptr; float* zt = nullptr;
+  // per-token scratch (used when the caller passes NULL per-token outputs)
+  float* tok_lse = nullptr; float* tok_lp = nullptr; float* tok_ent = nullptr; float* tok_conf = nullptr;
+  // kernel 2 workspace
+  int* tile_base = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
+  // staging for sq_score_run_host
+  void* h_stage = nullptr; int32_t* tgt_stage = nullptr; int32_t* cu_stage = nullptr; float* seq_stage = nullptr;
+  // driver entry point for tensor-map encoding
+  void* encode_fn = nullptr;
+};
+
+static thread_local char g_create_err[512] = {0};
+
+static int set_err(sq_score_ctx* ctx, int code, const char* fmt, ...) {
+  char* dst = ctx ? ctx->err : g_create_err;
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(dst, 512, fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+#define SQ_CUDA(ctx, call)                                                                   \
+  do {                                                                                       \
+    cudaError_t e_ = (call);                                                                 \
+    if (e_ != cudaSuccess)                                                                   \
+      return set_err(ctx, SQ_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                     __FILE__, __LINE__);                                                    \
+  } while (0)
+
+static int topk_cap_for(int k) { return k <= 8 ? 8 : (k <= 20 ? 20 : 32); }
+static inline int64_t cdiv64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// ------------------------------------------------------------------------------------------ plan
+// Work decomposition.  A unit sweeps `tiles_per_chunk` vocab tiles for one
+// token tile; units are ordered [group of group_m token tiles][chunk][tile in group] and handed to
+// the persistent clusters round-robin, so ~num_clusters consecutive units are in flight: group_m
+// token strips (H stays in L2) x ~num_clusters/group_m chunks (each W tile is read from HBM once
+// per group and shared through L2 by the group_m units that sweep it in lockstep).
+static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, sq_score_plan_t* pl) {
+  if (!cfg || !pl || T < 0 || cfg->d <= 0 || cfg->vocab <= 0 || k < 1 || k > SQ_MAX_K) return SQ_ERR_INVALID_ARG;
+  if (num_sms <= 0) num_sms = 148;
+  const int cg = (cfg->cta_group == 1) ? 1 : 2;
+  memset(pl, 0, sizeof(*pl));
+  pl->cta_group = cg;
+  pl->rows_per_tile = 128 * cg;
+  pl->m_tiles = (int)cdiv64(T, pl->rows_per_tile);
+  pl->num_vtiles = (int)cdiv64(cfg->vocab, 256);
+  pl->num_k_blocks = (int)cdiv64(cfg->d, 64);
+  pl->num_clusters = std::max(1, num_sms / cg);
+  pl->group_m = cfg->group_m > 0 ? cfg->group_m : 8;
+  pl->topk_cap = topk_cap_for(k);
+  const int max_chunks = std::min(32, pl->num_vtiles);
+  int best_c = 1;
+  if (cfg->num_chunks > 0) {
+    best_c = std::min(cfg->num_chunks, max_chunks);
+  } else if (pl->m_tiles > 0) {
+    // enough chunks that group_m strips x chunks cover the grid, then minimise whole waves x unit length
+    const int gm = std::min(pl->group_m, pl->m_tiles);
+    const int c_lo = std::min(max_chunks, std::max(1, (int)cdiv64(pl->num_clusters, gm) - 1));
+    const int c_hi = std::min(max_chunks, std::max(c_lo, 16));
+    double best_cost = 1e300;
+    for (int c = c_lo; c <= c_hi; ++c) {
+      const int tpc = (int)cdiv64(pl->num_vtiles, c);
+      const int ce = (int)cdiv64(pl->num_vtiles, tpc);
+      const int64_t units = (int64_t)pl->m_tiles * ce;
+      const int64_t waves = cdiv64(units, pl->num_clusters);
+      const double cost = (double)waves * (tpc + 0.75);   // 0.75 tile-times of fill/drain per unit
+      if (cost < best_cost - 1e-9) { best_cost = cost; best_c = c; }
+    }
+  }
+  pl->tiles_per_chunk = (int)cdiv64(pl->num_vtiles, best_c);
+  pl->num_chunks = (int)cdiv64(pl->num_vtiles, pl->tiles_per_chunk);
+  pl->num_units = pl->m_tiles * pl->num_chunks;
+  return SQ_OK;
+}
+
+extern "C" int sq_score_plan(const sq_score_config* cfg, int64_t num_tokens, int k, int num_sms,
+                             sq_score_plan_t* plan) {
+  return make_plan(cfg, num_tokens, k, num_sms, plan);
+}
+
+extern "C" int sq_score_version(void) { return SQ_VERSION; }
+
+extern "C" const char* sq_score_error_string(int code) {
+  switch (code) {
+    case SQ_OK: return "SQ_OK";
+    case SQ_ERR_INVALID_ARG: return "SQ_ERR_INVALID_ARG";
+    case SQ_ERR_UNSUPPORTED: return "SQ_ERR_UNSUPPORTED";
+    case SQ_ERR_CUDA: return "SQ_ERR_CUDA";
+    case SQ_ERR_NOMEM: return "SQ_ERR_NOMEM";
+    default: return "SQ_ERR_UNKNOWN";
+  }
+}
+
+extern "C" const char* sq_score_last_error(const sq_score_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
+
+extern "C" int64_t sq_score_launch_count(const sq_score_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+// ------------------------------------------------------------------------------------------ create / destroy
+static int64_t ws_rows_for(const sq_score_config& cfg) {
+  const int64_t small_t = std::min<int64_t>(cfg.max_tokens, 16384);
+  int64_t rows = std::max<int64_t>(32 * small_t, 16 * cfg.max_tokens);
+  if (cfg.num_chunks > 0) rows = std::max<int64_t>(rows, (int64_t)std::min(cfg.num_chunks, 32) * cfg.max_tokens);
+  return rows;
+}
+
+extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
+  if (!ctx) return SQ_OK;
+  cudaSetDevice(ctx->cfg.device);
+  void* bufs[] = {ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
+                  ctx->tok_lse, ctx->tok_lp, ctx->tok_ent, ctx->tok_conf, ctx->tile_base, ctx->red_sum,
+                  ctx->red_min, ctx->h_stage, ctx->tgt_stage, ctx->cu_stage, ctx->seq_stage};
+  int rc = SQ_OK;
+  for (void* b : bufs)
+    if (b && cudaFree(b) != cudaSuccess) rc = SQ_ERR_CUDA;
+  delete ctx;
+  return rc;
+}
+
+template <typename T>
+static int ws_alloc(sq_score_ctx* ctx, T** p, int64_t count) {
+  if (count <= 0) count = 1;
+  cudaError_t e = cudaMalloc(reinterpret_cast<void**>(p), (size_t)count * sizeof(T));
+  if (e != cudaSuccess) {
+    *p = nullptr;
+    cudaGetLastError();
+    return set_err(ctx, e == cudaErrorMemoryAllocation ? SQ_ERR_NOMEM : SQ_ERR_CUDA,
+                   "workspace allocation of %lld bytes failed: %s", (long long)(count * (int64_t)sizeof(T)),
+                   cudaGetErrorString(e));
+  }
+  return SQ_OK;
+}
+
+extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
+  if (out) *out = nullptr;
+  if (!cfg || !out) return set_err(nullptr, SQ_ERR_INVALID_ARG, "null argument");
+  if (cfg->d <= 0 || cfg->vocab <= 0 || cfg->max_tokens <= 0 || cfg->max_seqs <= 0)
+    return set_err(nullptr, SQ_ERR_INVALID_ARG, "d, vocab, max_tokens and max_seqs must be positive");
+  if (cfg->max_k < 1 || cfg->max_k > SQ_MAX_K)
+    return set_err(nullptr, SQ_ERR_INVALID_ARG, "max_k must be in 1..%d", SQ_MAX_K);
+  if (cfg->cta_group < 0 || cfg->cta_group > 2 || cfg->num_chunks < 0 || cfg->group_m < 0)
+    return set_err(nullptr, SQ_ERR_INVALID_ARG, "cta_group must be 0, 1 or 2; num_chunks, group_m >= 0");
+  if (cfg->d % 8 != 0)
+    return set_err(nullptr, SQ_ERR_UNSUPPORTED, "d = %d is not a multiple of 8 (TMA needs 16-byte row strides)", cfg->d);
+  if (cfg->max_tokens >= (1LL << 31) - 4096)
+    return set_err(nullptr, SQ_ERR_UNSUPPORTED, "max_tokens must be below 2^31 - 4096");
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return set_err(nullptr, SQ_ERR_CUDA, "no CUDA device available: %s (this library has no CPU fallback)",
+                   e == cudaSuccess ? "device count is 0" : cudaGetErrorString(e));
+  }
+  if (cfg->device < 0 || cfg->device >= ndev) return set_err(nullptr, SQ_ERR_INVALID_ARG, "device %d out of range", cfg->device);
+  cudaDeviceProp prop;
+  SQ_CUDA(nullptr, cudaGetDeviceProperties(&prop, cfg->device));
+  if (prop.major != 10)
+    return set_err(nullptr, SQ_ERR_UNSUPPORTED, "device %d is sm_%d%d; the kernels are built for sm_100a only", cfg->device,
+                   prop.major, prop.minor);
+  SQ_CUDA(nullptr, cudaSetDevice(cfg->device));
+
+  sq_score_ctx* ctx = new (std::nothrow) sq_score_ctx();
+  if (!ctx) return set_err(nullptr, SQ_ERR_NOMEM, "host allocation failed");
+  ctx->cfg = *cfg;
+  ctx->num_sms = prop.multiProcessorCount;
+  ctx->cap_max = topk_cap_for(cfg->max_k);
+
+  cudaDriverEntryPointQueryResult qres;
+  e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ctx->encode_fn, cudaEnableDefault, &qres);
+  if (e != cudaSuccess || qres != cudaDriverEntryPointSuccess || !ctx->encode_fn) {
+    set_err(nullptr, SQ_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+    delete ctx;
+    return SQ_ERR_CUDA;
+  }
+
+  const int64_t rows = ws_rows_for(*cfg);
+  const int64_t T = cfg->max_tokens;
+  ctx->red_tiles_max = cdiv64(T, sq::RED_TILE) + cfg->max_seqs;
+  int rc = SQ_OK;
+  auto A = [&](int r) { if (rc == SQ_OK && r != SQ_OK) rc = r; };
+  A(ws_alloc(ctx, &ctx->part_m, rows));
+  A(ws_alloc(ctx, &ctx->part_s, rows));
+  A(ws_alloc(ctx, &ctx->part_u, rows));
+  A(ws_alloc(ctx, &ctx->part_topv, rows * ctx->cap_max));
+  A(ws_alloc(ctx, &ctx->part_topi, rows * ctx->cap_max));
+  A(ws_alloc(ctx, &ctx->zt, T));
+  A(ws_alloc(ctx, &ctx->tok_lse, T));
+  A(ws_alloc(ctx, &ctx->tok_lp, T));
+  A(ws_alloc(ctx, &ctx->tok_ent, T));
+  A(ws_alloc(ctx, &ctx->tok_conf, T));
+  A(ws_alloc(ctx, &ctx->tile_base, (int64_t)cfg->max_seqs + 1));
+  A(ws_alloc(ctx, &ctx->red_sum, ctx->red_tiles_max));
+  A(ws_alloc(ctx, &ctx->red_min, ctx->red_tiles_max));
+  A(ws_alloc(ctx, &ctx->seq_stage, 4 * (int64_t)cfg->max_seqs));
+  if (rc != SQ_OK) {
+    memcpy(g_create_err, ctx->err, sizeof(g_create_err));
+    sq_score_destroy(ctx);
+    return rc;
+  }
+  // opt in to the large dynamic shared memory of every fused-kernel instantiation
+#define SQ_SET_SMEM(CG, CAP)                                                                                   \
+  if (cudaFuncSetAttribute(sq::sq_fused_score_kernel<CG, CAP>, cudaFuncAttributeMaxDynamicSharedMemorySize,    \
+                           sq::FusedCfg<CG>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
+  SQ_SET_SMEM(1, 8) SQ_SET_SMEM(1, 20) SQ_SET_SMEM(1, 32) SQ_SET_SMEM(2, 8) SQ_SET_SMEM(2, 20) SQ_SET_SMEM(2, 32)
+#undef SQ_SET_SMEM
+  if (rc != SQ_OK) {
+    set_err(nullptr, rc, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize) failed: %s", cudaGetErrorString(cudaGetLastError()));
+    sq_score_destroy(ctx);
+    return rc;
+  }
+  *out = ctx;
+  return SQ_OK;
+}
+
+// ------------------------------------------------------------------------------------------ tensor maps
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// bf16 [rows, d] row-major -> boxes of {64 columns (128 B, swizzle-128B), box_rows rows}; out-of-range
+// rows and columns are zero filled.
+static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int d, int box_rows) {
+  const cuuint64_t dims[2] = {(cuuint64_t)d, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)d * 2};
+  const cuuint32_t box[2] = {(cuuint32_t)sq::BLOCK_K, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  CUresult r = reinterpret_cast<encode_tiled_fn>(ctx->encode_fn)(
+      map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return set_err(ctx, SQ_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+  return SQ_OK;
+}
+
+// ------------------------------------------------------------------------------------------ launches
+template <int CG, int CAP>
+static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CUtensorMap& th, const CUtensorMap& tw,
+                                const sq::FusedParams& fp, cudaStream_t st) {
+  const int clusters = std::min(pl.num_clusters, pl.num_units);
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3((unsigned)(clusters * CG));
+  lc.blockDim = dim3(sq::NUM_THREADS);
+  lc.dynamicSmemBytes = sq::FusedCfg<CG>::SMEM_BYTES;
+  lc.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = CG; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  lc.attrs = at;
+  lc.numAttrs = 1;
+  (void)num_sms;
+  return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP>, th, tw, fp);
+}
+
+static int launch_reduce(sq_score_ctx* ctx, const sq::ReduceParams& rp, cudaStream_t st) {
+  if (rp.B <= 0) return SQ_OK;
+  const int64_t tiles = cdiv64(rp.T, sq::RED_TILE) + rp.B;
+  sq::sq_reduce_tile_scan_kernel<<<1, 1024, 0, st>>>(rp);
+  if (rp.T > 0) sq::sq_reduce_tile_part_kernel<<<(unsigned)tiles, sq::RED_THREADS, 0, st>>>(rp);
+  sq::sq_reduce_seq_final_kernel<<<(unsigned)cdiv64(rp.B, 4), 128, 0, st>>>(rp);
+  ctx->launches += (rp.T > 0) ? 3 : 2;
+  SQ_CUDA(ctx, cudaGetLastError());
+  return SQ_OK;
+}
+
+extern "C" int sq_score_reduce(sq_score_ctx* ctx, const float* target_logprob, const float* entropy, const float* conf,
+                               const int32_t* targets, const int32_t* cu_seqlens, int64_t num_tokens, int num_seqs,
+                               int window, float* seq_mean_logprob, float* seq_mean_entropy, float* seq_mean_conf,
+                               float* seq_min_window_conf, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (num_tokens < 0 || num_seqs < 0 || window < 1) return set_err(ctx, SQ_ERR_INVALID_ARG, "T, B >= 0 and window >= 1 required");
+  if (num_tokens > ctx->cfg.max_tokens || num_seqs > ctx->cfg.max_seqs)
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "T = %lld / B = %d exceed max_tokens / max_seqs of this ctx", (long long)num_tokens, num_seqs);
+  if (num_seqs == 0) return SQ_OK;
+  if (!cu_seqlens || !seq_mean_logprob || !seq_mean_entropy || !seq_mean_conf || !seq_min_window_conf ||
+      (num_tokens > 0 && (!target_logprob || !entropy || !conf)))
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "null pointer argument");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  sq::ReduceParams rp = {};
+  rp.T = num_tokens; rp.B = num_seqs; rp.V = ctx->cfg.vocab; rp.window = window;
+  rp.lp = target_logprob; rp.ent = entropy; rp.conf = conf; rp.targets = targets; rp.cu = cu_seqlens;
+  rp.tile_base = ctx->tile_base; rp.part_sum = ctx->red_sum; rp.part_min = ctx->red_min;
+  rp.out_lp = seq_mean_logprob; rp.out_ent = seq_mean_entropy; rp.out_conf = seq_mean_conf; rp.out_min = seq_min_window_conf;
+  return launch_reduce(ctx, rp, static_cast<cudaStream_t>(stream));
+}
+
+extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, const int32_t* targets,
+                            const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k, int window,
+                            const sq_score_outputs* o, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (!o) return set_err(ctx, SQ_ERR_INVALID_ARG, "outputs is null");
+  const int T = num_tokens, B = num_seqs, V = ctx->cfg.vocab, d = ctx->cfg.d;
+  if (T < 0 || B < 0) return set_err(ctx, SQ_ERR_INVALID_ARG, "negative T or B");
+  if (T > ctx->cfg.max_tokens || B > ctx->cfg.max_seqs)
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "T = %d / B = %d exceed max_tokens / max_seqs of this ctx", T, B);
+  if (k < 1 || k > ctx->cfg.max_k || k > V) return set_err(ctx, SQ_ERR_INVALID_ARG, "k = %d outside 1..min(max_k, V)", k);
+  if (window < 1) return set_err(ctx, SQ_ERR_INVALID_ARG, "window must be >= 1");
+  if (B > 0 && (!cu_seqlens || !o->seq_mean_logprob || !o->seq_mean_entropy || !o->seq_mean_conf || !o->seq_min_window_conf))
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "cu_seqlens and the four per-sequence outputs are required");
+  if (T > 0 && (!H || !W || !targets)) return set_err(ctx, SQ_ERR_INVALID_ARG, "H, W and targets are required");
+  if (T > 0 && (((uintptr_t)H & 15) || ((uintptr_t)W & 15))) return set_err(ctx, SQ_ERR_INVALID_ARG, "H and W must be 16-byte aligned");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+
+  float* lse = o->lse ? o->lse : ctx->tok_lse;
+  float* lp = o->target_logprob ? o->target_logprob : ctx->tok_lp;
+  float* ent = o->entropy ? o->entropy : ctx->tok_ent;
+  float* conf = o->conf ? o->conf : ctx->tok_conf;
+
+  if (T > 0) {
+    sq_score_plan_t pl;
+    sq_score_config pc = ctx->cfg;
+    make_plan(&pc, T, k, ctx->num_sms, &pl);
+    const int64_t rows = ws_rows_for(ctx->cfg);
+    if ((int64_t)pl.num_chunks * T > rows) {   // workspace bound: fewer, longer chunks
+      pc.num_chunks = (int)std::max<int64_t>(1, rows / T);
+      make_plan(&pc, T, k, ctx->num_sms, &pl);
+    }
+    if (pl.topk_cap > ctx->cap_max) return set_err(ctx, SQ_ERR_INVALID_ARG, "k exceeds the ctx's max_k capacity");
+    CUtensorMap th, tw;
+    int rc = make_tmap(ctx, &th, H, T, d, sq::BLOCK_M);
+    if (rc != SQ_OK) return rc;
+    rc = make_tmap(ctx, &tw, W, V, d, sq::BLOCK_N / pl.cta_group);
+    if (rc != SQ_OK) return rc;
+
+    sq::FusedParams fp = {};
+    fp.T = T; fp.V = V; fp.d = d;
+    fp.num_k_blocks = pl.num_k_blocks; fp.num_vtiles = pl.num_vtiles; fp.tiles_per_chunk = pl.tiles_per_chunk;
+    fp.num_chunks = pl.num_chunks; fp.m_tiles = pl.m_tiles; fp.group_m = pl.group_m; fp.num_units = pl.num_units;
+    fp.targets = targets;
+    fp.part_m = ctx->part_m; fp.part_s = ctx->part_s; fp.part_u = ctx->part_u;
+    fp.part_topv = ctx->part_topv; fp.part_topi = ctx->part_topi; fp.zt = ctx->zt;
+    cudaError_t e;
+    const int sel = pl.cta_group * 100 + pl.topk_cap;
+    switch (sel) {
+      case 108: e = launch_fused<1, 8>(pl, ctx->num_sms, th, tw, fp, st); break;
+      case 120: e = launch_fused<1, 20>(pl, ctx->num_sms, th, tw, fp, st); break;
+      case 132: e = launch_fused<1, 32>(pl, ctx->num_sms, th, tw, fp, st); break;
+      case 208: e = launch_fused<2, 8>(pl, ctx->num_sms, th, tw, fp, st); break;
+      case 220: e = launch_fused<2, 20>(pl, ctx->num_sms, th, tw, fp, st); break;
+      default: e = launch_fused<2, 32>(pl, ctx->num_sms, th, tw, fp, st); break;
+    }
+    if (e != cudaSuccess) return set_err(ctx, SQ_ERR_CUDA, "fused kernel launch failed: %s", cudaGetErrorString(e));
+
+    sq::FinalizeParams fin = {};
+    fin.T = T; fin.V = V; fin.k = k; fin.cap = pl.topk_cap; fin.num_chunks = pl.num_chunks;
+    fin.targets = targets;
+    fin.part_m = ctx->part_m; fin.part_s = ctx->part_s; fin.part_u = ctx->part_u;
+    fin.part_topv = ctx->part_topv; fin.part_topi = ctx->part_topi; fin.zt = ctx->zt;
+    fin.lse = lse; fin.target_logprob = lp; fin.entropy = ent; fin.conf = conf;
+    fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
+    sq::sq_finalize_kernel<<<(unsigned)cdiv64(T, sq::FIN_WARPS), sq::FIN_WARPS * 32, 0, st>>>(fin);
+    ctx->launches += 2;
+    SQ_CUDA(ctx, cudaGetLastError());
+  }
+  if (B > 0) {
+    sq::ReduceParams rp = {};
+    rp.T = T; rp.B = B; rp.V = V; rp.window = window;
+    rp.lp = lp; rp.ent = ent; rp.conf = conf; rp.targets = targets; rp.cu = cu_seqlens;
+    rp.tile_base = ctx->tile_base; rp.part_sum = ctx->red_sum; rp.part_min = ctx->red_min;
+    rp.out_lp = o->seq_mean_logprob; rp.out_ent = o->seq_mean_entropy; rp.out_conf = o->seq_mean_conf;
+    rp.out_min = o->seq_min_window_conf;
+    return launch_reduce(ctx, rp, st);
+  }
+  return SQ_OK;
+}
+
+extern "C" int sq_score_run_host(sq_score_ctx* ctx, const void* H_host, const void* W_dev, const int32_t* targets_host,
+                                 const int32_t* cu_seqlens_host, int num_tokens, int num_seqs, int k, int window,
+                                 float* seq_out_host, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  const int T = num_tokens, B = num_seqs;
+  if (T < 0 || B < 0 || T > ctx->cfg.max_tokens || B > ctx->cfg.max_seqs)
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "T / B out of range for this ctx");
+  if ((T > 0 && (!H_host || !W_dev || !targets_host)) || (B > 0 && (!cu_seqlens_host || !seq_out_host)))
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "null pointer argument");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (!ctx->h_stage) {   // staging is allocated on first use: only callers of the host form pay for it
+    int rc = ws_alloc(ctx, reinterpret_cast<uint8_t**>(&ctx->h_stage), ctx->cfg.max_tokens * (int64_t)ctx->cfg.d * 2);
+    if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->tgt_stage, ctx->cfg.max_tokens);
+    if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->cu_stage, (int64_t)ctx->cfg.max_seqs + 1);
+    if (rc != SQ_OK) return rc;
+  }
+  if (T > 0) {
+    SQ_CUDA(ctx, cudaMemcpyAsync(ctx->h_stage, H_host, (size_t)T * ctx->cfg.d * 2, cudaMemcpyHostToDevice, st));
+    SQ_CUDA(ctx, cudaMemcpyAsync(ctx->tgt_stage, targets_host, (size_t)T * 4, cudaMemcpyHostToDevice, st));
+  }
+  if (B > 0) SQ_CUDA(ctx, cudaMemcpyAsync(ctx->cu_stage, cu_seqlens_host, (size_t)(B + 1) * 4, cudaMemcpyHostToDevice, st));
+  sq_score_outputs o = {};
+  o.seq_mean_logprob = ctx->seq_stage;
+  o.seq_mean_entropy = ctx->seq_stage + B;
+  o.seq_mean_conf = ctx->seq_stage + 2 * (size_t)B;
+  o.seq_min_window_conf = ctx->seq_stage + 3 * (size_t)B;
+  int rc = sq_score_run(ctx, ctx->h_stage, W_dev, ctx->tgt_stage, ctx->cu_stage, T, B, k, window, &o, stream);
+  if (rc != SQ_OK) return rc;
+  if (B > 0) SQ_CUDA(ctx, cudaMemcpyAsync(seq_out_host, ctx->seq_stage, (size_t)4 * B * sizeof(float), cudaMemcpyDeviceToHost, st));
+  return SQ_OK;
+}
