@@ -1,0 +1,350 @@
+#!/usr/bin/env python
+"""bench.py -- scored tokens/s of the fused LM-head scoring pass (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl ours|reference]
+
+A step is one pass of the whole hot path (kernel 1 fused GEMM+statistics, finalize/merge, kernel 2)
+over one synthetic packed batch.  At N=1 the workload is BASELINE.json configs[2] (`qwen3_8b`, the
+config the metric's 60 % target is quoted on).  With N>1 (torchrun) every rank scores its own
+batch of the same shape (sequences shard across GPUs, W replicated, no data-path collective):
+weak scaling.  One JSON line is printed by rank 0.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+import workloads
+
+METRIC = "scored tokens/s & % of dense BF16 tensor peak (fused LM-head logprob scoring)"
+UNIT = "tokens/s"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return {"hbm_gbs": p["hbm_gbs"], "bf16_tflops": p["bf16_tflops"],
+                "bf16_tflops_sustained": p.get("bf16_tflops_sustained", p["bf16_tflops"]), "source": "measured"}
+    # fallback stated in B200_PROFILING.md
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+            nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+            nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+            nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.05)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline / --impl reference): the oracle as it stands, on a bounded row sample
+# ------------------------------------------------------------------------------------------------
+def oracle_sample_rows(T: int, n: int, seed: int) -> np.ndarray:
+    rng = np.random.default_rng(seed)
+    return np.sort(rng.choice(T, size=min(n, T), replace=False))
+
+
+def time_oracle(inp: dict, budget_s: float, steps: int = 1, warmup: int = 0):
+    """Times oracle.token_scores + sequence_scores on a row sample sized for ~budget_s of CPU work
+    per step.  Returns (tokens/s, seconds per step, rows per step, threads)."""
+    from oracle import sq_oracle as O   # bench.py's cpu_baseline / reference leg may execute oracle/
+    wl = inp["workload"]
+    T = inp["T"]
+    W64 = O.widen(inp["W"])             # converting the LM head once is set-up, like loading weights
+    tg = inp["targets"].numpy()
+    probe = oracle_sample_rows(T, min(16, T), 7)
+    t0 = time.perf_counter()
+    O.token_scores(inp["H"][probe], W64, tg[probe], wl.k)
+    per_row = (time.perf_counter() - t0) / max(1, len(probe))
+    n = int(max(16, min(T, budget_s / max(per_row, 1e-6))))
+    n = min(n, 4096)
+    rows = oracle_sample_rows(T, n, 11)
+    times = []
+    for it in range(warmup + steps):
+        t0 = time.perf_counter()
+        conf = np.empty(len(rows)); lp = np.empty(len(rows)); en = np.empty(len(rows))
+        for r0 in range(0, len(rows), 64):
+            idx = rows[r0:r0 + 64]
+            r = O.token_scores(inp["H"][idx], W64, tg[idx], wl.k)
+            conf[r0:r0 + 64] = r["conf"]; lp[r0:r0 + 64] = r["target_logprob"]; en[r0:r0 + 64] = r["entropy"]
+        # the sample treated as one packed sequence for the per-sequence step
+        O.sequence_scores(lp, en, conf, [0, len(rows)], wl.window)
+        dt = time.perf_counter() - t0
+        if it >= warmup:
+            times.append(dt)
+    sec = float(np.mean(times))
+    return len(rows) / sec, sec, len(rows), torch.get_num_threads()
+
+
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    wl = workloads.CONFIGS[args.config]
+    inp = workloads.make_inputs(wl)
+    tps, sec, rows, threads = time_oracle(inp, budget_s=args.oracle_seconds, steps=args.steps, warmup=min(args.warmup, 1))
+    sample = "%d seeded rows of %s (T=%d) per step, fp64 oracle.token_scores + sequence_scores" % (rows, wl.name, inp["T"])
+    line = {
+        "impl": "reference", "metric": METRIC, "value": tps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "d": wl.d, "V": wl.V, "B": inp["B"], "T": inp["T"], "k": wl.k,
+                   "window": wl.window, "sample_rows_per_step": rows},
+        "cpu_baseline": {"value": tps, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": tps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import paper_2604_07725_b200 as sq
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the sq_score path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    use_dist = world > 1
+    if use_dist:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    peaks = load_peaks()
+    wl = workloads.CONFIGS[args.config]
+    if use_dist:   # weak scaling: every rank scores its own population of the same shape
+        from dataclasses import replace
+        wl_rank = replace(wl, seed=wl.seed + 100 * rank)
+    else:
+        wl_rank = wl
+    inp = workloads.make_inputs(wl_rank)
+    T, B, d, V = inp["T"], inp["B"], wl.d, wl.V
+
+    eng = sq.SqScore(d, V, max_tokens=T, max_seqs=B, max_k=wl.k, device=local,
+                     cta_group=args.cta_group, num_chunks=args.num_chunks, group_m=args.group_m)
+    pl = sq.plan(d, V, T, wl.k, num_sms=torch.cuda.get_device_properties(dev).multi_processor_count,
+                 cta_group=args.cta_group, num_chunks=args.num_chunks, group_m=args.group_m)
+    stream = torch.cuda.Stream(device=dev)
+    H = inp["H"].to(dev); W = inp["W"].to(dev)
+    tg = inp["targets"].to(dev); cu = inp["cu_seqlens"].to(dev)
+    H_pin = inp["H"].pin_memory(); tg_pin = inp["targets"].pin_memory(); cu_pin = inp["cu_seqlens"].pin_memory()
+    seq_pin = torch.empty(4 * B, dtype=torch.float32).pin_memory()
+    torch.cuda.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if use_dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------- device-resident timing (value) + live per-kernel timing (roofline)
+    out = None
+    eng.set_profiling(True)
+    with torch.cuda.stream(stream):
+        for _ in range(max(3, args.warmup)):
+            out = eng.run(H, W, tg, cu, wl.k, wl.window, stream=stream, out=out)
+        barrier()
+        sampler = ClockSampler(local)
+        sampler.start()
+        launches0 = eng.launch_count()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        fused_ms = []
+        e0.record(stream)
+        for _ in range(args.steps):
+            eng.run(H, W, tg, cu, wl.k, wl.window, stream=stream, out=out)
+            if args.per_step_kernel_times:
+                fused_ms.append(eng.kernel_times())
+        e1.record(stream)
+        barrier()
+        clocks = sampler.stop()
+        launches = eng.launch_count() - launches0
+        total_ms = e0.elapsed_time(e1)
+        if not fused_ms:
+            fused_ms.append(eng.kernel_times())   # the last timed step's kernels
+    ms_step = total_ms / args.steps
+
+    # ---------------- end to end through the C ABI with HOST buffers
+    with torch.cuda.stream(stream):
+        for _ in range(2):
+            eng.run_host(H_pin, W, tg_pin, cu_pin, wl.k, wl.window, seq_pin, stream=stream)
+            stream.synchronize()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            eng.run_host(H_pin, W, tg_pin, cu_pin, wl.k, wl.window, seq_pin, stream=stream)
+            stream.synchronize()       # the caller reads the scalars every step
+        e2e_s = (time.perf_counter() - t0) / args.e2e_steps
+    seq_dev = torch.cat([out[n] for n in ("seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf")])
+    e2e_ok = bool(torch.allclose(seq_dev.cpu(), seq_pin, rtol=1e-5, atol=1e-6, equal_nan=True))
+
+    # ---------------- max over ranks
+    t_loc = torch.tensor([ms_step, e2e_s * 1e3, float(T)], dtype=torch.float64, device=dev)
+    if use_dist:
+        tmax = t_loc.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        tsum = t_loc.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
+        ms_step, e2e_ms, tokens_all = float(tmax[0]), float(tmax[1]), float(tsum[2])
+    else:
+        e2e_ms, tokens_all = e2e_s * 1e3, float(T)
+    if rank != 0:
+        if use_dist:
+            dist.destroy_process_group()
+        return
+
+    value = tokens_all / (ms_step * 1e-3)
+    k1_ms = float(np.mean([x["fused_ms"] for x in fused_ms]))
+    fin_ms = float(np.mean([x["finalize_ms"] for x in fused_ms]))
+    red_ms = float(np.mean([x["reduce_ms"] for x in fused_ms]))
+    flops = 2.0 * T * V * d                                   # algorithmic FLOPs per launch of kernel 1
+    achieved = flops / (k1_ms * 1e-3) / 1e12
+    peak = peaks["bf16_tflops_sustained"]                     # kernel timed inside a long step
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic_%s.json" % wl.name)
+    if os.path.exists(tpath):
+        with open(tpath) as f:
+            traffic = json.load(f).get("dram_bytes_per_launch")
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16", "data": "synthetic",
+        "config": {"workload": wl.name, "d": d, "V": V, "B": B, "T": T, "k": wl.k, "window": wl.window,
+                   "parallelism": "dp%d (sequences sharded, W replicated)" % world,
+                   "l2": "inputs larger than L2 (H %.0f MB + W %.0f MB re-streamed every step)" % (T * d * 2 / 1e6, V * d * 2 / 1e6),
+                   "plan": pl},
+        "tflops": flops / (ms_step * 1e-3) / 1e12,
+        "pct_of_bf16_peak_burst": 100.0 * flops / (ms_step * 1e-3) / 1e12 / peaks["bf16_tflops"],
+        "roofline": {"bound": "tensor", "kernel": "sq_fused_score_kernel", "achieved": achieved, "peak": peak,
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                     "peak_kind": "bf16_tflops_sustained of %s (kernel timed inside a long step)" % peaks["source"],
+                     "frac_of_burst": achieved / peaks["bf16_tflops"], "peak_burst": peaks["bf16_tflops"],
+                     "kernel_ms": k1_ms, "algorithmic_flops_per_launch": flops},
+        "kernels_ms": {"fused": k1_ms, "finalize": fin_ms, "reduce": red_ms,
+                       "fused_per_step": [round(x["fused_ms"], 3) for x in fused_ms]},
+        "e2e": {"value": tokens_all / (e2e_ms * 1e-3), "unit": UNIT,
+                "h2d_bytes_per_step": T * d * 2 + T * 4 + (B + 1) * 4, "d2h_bytes_per_step": 4 * B * 4,
+                "ms_per_step": e2e_ms, "matches_device_path": e2e_ok, "api": "sq_score_run_host"},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    if args.matmul_ceiling:
+        # context only: cuBLAS on the same (T, V, d) in row chunks, logits materialised chunk by chunk
+        rows = 8192
+        buf = torch.empty(rows, V, dtype=torch.bfloat16, device=dev)
+        Wt = W.t()
+        def mm_pass():
+            for r0 in range(0, T, rows):
+                r1 = min(T, r0 + rows)
+                torch.matmul(H[r0:r1], Wt, out=buf[: r1 - r0])
+        for _ in range(2):
+            mm_pass()
+        torch.cuda.synchronize()
+        m0 = torch.cuda.Event(enable_timing=True); m1 = torch.cuda.Event(enable_timing=True)
+        m0.record()
+        for _ in range(args.steps):
+            mm_pass()
+        m1.record(); torch.cuda.synchronize()
+        mm_ms = m0.elapsed_time(m1) / args.steps
+        line["context_cublas_matmul"] = {"ms_per_pass": mm_ms, "tflops": flops / (mm_ms * 1e-3) / 1e12,
+                                         "note": "torch.matmul bf16 over the same T,V,d in 8192-row chunks; not part of the path"}
+        del buf
+    if world == 1 and not args.no_cpu_baseline:
+        tps, sec, rows, threads = time_oracle(inp, budget_s=args.oracle_seconds)
+        line["cpu_baseline"] = {"value": tps, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": "%d seeded rows of %s in %.1f s (fp64 oracle.token_scores + sequence_scores)" % (rows, wl.name, sec)}
+    print(json.dumps(line))
+    eng.close()
+    if use_dist:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="qwen3_8b", choices=list(workloads.CONFIGS))
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--oracle-seconds", type=float, default=None)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--per-step-kernel-times", action="store_true",
+                    help="read kernel 1's duration after every step (adds a host sync per step)")
+    ap.add_argument("--matmul-ceiling", action="store_true", help="also time torch.matmul on the same shapes (context)")
+    ap.add_argument("--cta-group", type=int, default=0)
+    ap.add_argument("--num-chunks", type=int, default=0)
+    ap.add_argument("--group-m", type=int, default=0)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if args.oracle_seconds is None:
+            args.oracle_seconds = max(1.0, 90.0 / (args.steps + 1))
+        run_reference(args)
+    else:
+        if args.oracle_seconds is None:
+            args.oracle_seconds = 15.0
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

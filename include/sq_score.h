@@ -142,6 +142,14 @@ int sq_score_reduce(sq_score_ctx *ctx, const float *target_logprob, const float 
 int sq_score_plan(const sq_score_config *cfg, int64_t num_tokens, int k, int num_sms,
                   sq_score_plan_t *plan);
 
+/* Per-kernel timing for the roofline report.  With profiling enabled, every sq_score_run with
+ * T > 0 and B > 0 records CUDA events on its stream around kernel 1 (fused GEMM + statistics), the
+ * finalize kernel and kernel 2.  sq_score_kernel_times blocks until the last profiled run finished
+ * and writes its three durations in milliseconds: ms3 = {fused, finalize, reduce}.
+ * Errors: INVALID_ARG (null, profiling off, no profiled run yet), CUDA. */
+int sq_score_set_profiling(sq_score_ctx *ctx, int enable);
+int sq_score_kernel_times(sq_score_ctx *ctx, float *ms3);
+
 /* Number of kernels this ctx has launched so far (bench.py's `gpu_launches`). */
 int64_t sq_score_launch_count(const sq_score_ctx *ctx);
 

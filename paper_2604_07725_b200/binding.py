@@ -63,6 +63,10 @@ def lib() -> C.CDLL:
     L.sq_score_reduce.restype = C.c_int
     L.sq_score_plan.argtypes = [C.POINTER(sq_score_config), C.c_int64, C.c_int, C.c_int, C.POINTER(sq_score_plan_t)]
     L.sq_score_plan.restype = C.c_int
+    L.sq_score_set_profiling.argtypes = [C.c_void_p, C.c_int]
+    L.sq_score_set_profiling.restype = C.c_int
+    L.sq_score_kernel_times.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
+    L.sq_score_kernel_times.restype = C.c_int
     L.sq_score_launch_count.argtypes = [C.c_void_p]
     L.sq_score_launch_count.restype = C.c_int64
     L.sq_score_destroy.argtypes = [C.c_void_p]
@@ -162,6 +166,15 @@ class SqScore:
                                             _ptr(out["seq_mean_conf"]), _ptr(out["seq_min_window_conf"]),
                                             self._stream(stream)))
         return out
+
+    def set_profiling(self, enable: bool):
+        self._check(self._L.sq_score_set_profiling(self._h, 1 if enable else 0))
+
+    def kernel_times(self) -> dict:
+        """sq_score_kernel_times: ms of the last profiled run's fused / finalize / reduce kernels."""
+        ms = (C.c_float * 3)()
+        self._check(self._L.sq_score_kernel_times(self._h, ms))
+        return {"fused_ms": ms[0], "finalize_ms": ms[1], "reduce_ms": ms[2]}
 
     def launch_count(self) -> int:
         return self._L.sq_score_launch_count(self._h)

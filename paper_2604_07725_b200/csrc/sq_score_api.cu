@@ -35,6 +35,9 @@ struct sq_score_ctx {
   void* h_stage = nullptr; int32_t* tgt_stage = nullptr; int32_t* cu_stage = nullptr; float* seq_stage = nullptr;
   // driver entry point for tensor-map encoding
   void* encode_fn = nullptr;
+  // optional per-kernel timing (sq_score_set_profiling): events around kernel 1, finalize, kernel 2
+  int profiling = 0; int ev_valid = 0;
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
 };
 
 static thread_local char g_create_err[512] = {0};
@@ -142,6 +145,8 @@ extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
   int rc = SQ_OK;
   for (void* b : bufs)
     if (b && cudaFree(b) != cudaSuccess) rc = SQ_ERR_CUDA;
+  for (cudaEvent_t e : ctx->ev)
+    if (e) cudaEventDestroy(e);
   delete ctx;
   return rc;
 }
@@ -359,6 +364,7 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
     fp.part_m = ctx->part_m; fp.part_s = ctx->part_s; fp.part_u = ctx->part_u;
     fp.part_topv = ctx->part_topv; fp.part_topi = ctx->part_topi; fp.zt = ctx->zt;
     cudaError_t e;
+    if (ctx->profiling) cudaEventRecord(ctx->ev[0], st);
     const int sel = pl.cta_group * 100 + pl.topk_cap;
     switch (sel) {
       case 108: e = launch_fused<1, 8>(pl, ctx->num_sms, th, tw, fp, st); break;
@@ -369,6 +375,7 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
       default: e = launch_fused<2, 32>(pl, ctx->num_sms, th, tw, fp, st); break;
     }
     if (e != cudaSuccess) return set_err(ctx, SQ_ERR_CUDA, "fused kernel launch failed: %s", cudaGetErrorString(e));
+    if (ctx->profiling) cudaEventRecord(ctx->ev[1], st);
 
     sq::FinalizeParams fin = {};
     fin.T = T; fin.V = V; fin.k = k; fin.cap = pl.topk_cap; fin.num_chunks = pl.num_chunks;
@@ -380,6 +387,7 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
     sq::sq_finalize_kernel<<<(unsigned)cdiv64(T, sq::FIN_WARPS), sq::FIN_WARPS * 32, 0, st>>>(fin);
     ctx->launches += 2;
     SQ_CUDA(ctx, cudaGetLastError());
+    if (ctx->profiling) cudaEventRecord(ctx->ev[2], st);
   }
   if (B > 0) {
     sq::ReduceParams rp = {};
@@ -388,8 +396,29 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
     rp.tile_base = ctx->tile_base; rp.part_sum = ctx->red_sum; rp.part_min = ctx->red_min;
     rp.out_lp = o->seq_mean_logprob; rp.out_ent = o->seq_mean_entropy; rp.out_conf = o->seq_mean_conf;
     rp.out_min = o->seq_min_window_conf;
-    return launch_reduce(ctx, rp, st);
+    const int rc = launch_reduce(ctx, rp, st);
+    if (rc != SQ_OK) return rc;
+    if (ctx->profiling && T > 0) { cudaEventRecord(ctx->ev[3], st); ctx->ev_valid = 1; }
   }
+  return SQ_OK;
+}
+
+extern "C" int sq_score_set_profiling(sq_score_ctx* ctx, int enable) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  if (enable)
+    for (auto& e : ctx->ev)
+      if (!e) SQ_CUDA(ctx, cudaEventCreate(&e));
+  ctx->profiling = enable ? 1 : 0;
+  ctx->ev_valid = 0;
+  return SQ_OK;
+}
+
+extern "C" int sq_score_kernel_times(sq_score_ctx* ctx, float* ms3) {
+  if (!ctx || !ms3) return SQ_ERR_INVALID_ARG;
+  if (!ctx->profiling || !ctx->ev_valid) return set_err(ctx, SQ_ERR_INVALID_ARG, "no profiled run recorded");
+  SQ_CUDA(ctx, cudaEventSynchronize(ctx->ev[3]));
+  for (int i = 0; i < 3; ++i) SQ_CUDA(ctx, cudaEventElapsedTime(&ms3[i], ctx->ev[i], ctx->ev[i + 1]));
   return SQ_OK;
 }
 
