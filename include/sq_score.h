@@ -60,7 +60,7 @@ typedef struct {
   int     max_k;        /* largest k of any run, 1..SQ_MAX_K                                      */
   int     cta_group;    /* 0 = default (2: CTA pairs, UMMA M=256); 1 = single-CTA UMMA (M=128)    */
   int     num_chunks;   /* 0 = planner's choice; >0 forces the number of vocab chunks per row     */
-  int     group_m;      /* 0 = default (8): token tiles that share a W stream through L2          */
+  int     group_m;      /* 0 = default (8): gang size = token tiles that share one W stream       */
 } sq_score_config;
 
 /* Output pointers of one run.  Per-token pointers may be NULL (= not wanted; the ctx keeps the
@@ -87,9 +87,11 @@ typedef struct {
   int num_k_blocks;     /* ceil(d / 64)                                                           */
   int num_chunks;       /* vocab chunks per row (partial states merged by the finalize kernel)    */
   int tiles_per_chunk;  /* vocab tiles swept by one work unit                                     */
-  int group_m;          /* consecutive units that share one W chunk                               */
+  int group_m;          /* gang size: clusters that sweep one W chunk together (<= m_tiles)       */
   int num_units;        /* m_tiles * num_chunks                                                   */
-  int num_clusters;     /* persistent grid size in clusters (= CTAs / cta_group)                  */
+  int num_clusters;     /* clusters the device can hold (= SMs / cta_group)                       */
+  int num_gangs;        /* num_clusters / group_m; the launch uses num_gangs * group_m clusters   */
+  int num_gang_units;   /* ceil(m_tiles / group_m) * num_chunks, dealt round-robin to the gangs   */
   int topk_cap;         /* compiled top-k list capacity used for this k (8, 20 or 32)             */
 } sq_score_plan_t;
 

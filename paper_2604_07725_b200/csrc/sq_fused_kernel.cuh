@@ -42,8 +42,10 @@ struct FusedParams {
   int tiles_per_chunk;
   int num_chunks;
   int m_tiles;
-  int group_m;
-  int num_units;
+  int group_m;              // gang size
+  int num_gangs;
+  int num_gang_units;       // ceil(m_tiles / group_m) * num_chunks
+  unsigned int* gang_ctr;   // [num_gangs], zeroed before the launch
   const int32_t* targets;   // [T]
   float* part_m;            // [C][T]
   float* part_s;            // [C][T]
@@ -51,22 +53,36 @@ struct FusedParams {
   float* part_topv;         // [C][CAP][T]
   int32_t* part_topi;       // [C][CAP][T]
   float* zt;                // [T] target logit (written by the chunk that owns the target column)
+  int debug_flags;          // experiments only (env SQ_SCORE_DEBUG): bit0 = epilogue skips the statistics
 };
 
 struct Unit { int m_tile; int chunk; };
 
-__device__ __forceinline__ Unit decode_unit(const FusedParams& p, int u) {
-  // units ordered [group of group_m token tiles][chunk][tile in group]: the group_m units that are
-  // handed out back to back sweep the same W chunk in near lockstep and share it through L2.
-  const int per_group = p.group_m * p.num_chunks;
-  const int g = u / per_group;
-  const int r = u - g * per_group;
-  const int first = g * p.group_m;
-  const int gsize = min(p.group_m, p.m_tiles - first);
-  Unit out;
-  out.chunk = r / gsize;
-  out.m_tile = first + (r - out.chunk * gsize);
-  return out;
+// Gang scheduling.  The persistent clusters are split into `num_gangs` gangs of `group_m` clusters.
+// A gang processes gang-units (group g of group_m consecutive token tiles, vocab chunk c) in the
+// order [g][c], round-robin over gangs; member j of the gang takes token tile g*group_m + j.  All
+// members sweep the same W chunk at the same time, so each W tile is fetched from HBM once per
+// gang-unit and served to the other members from L2; gangs working on the same g share its H strips.
+__device__ __forceinline__ bool decode_gang_unit(const FusedParams& p, int gu, int member, Unit& out) {
+  const int g = gu / p.num_chunks;
+  out.chunk = gu - g * p.num_chunks;
+  out.m_tile = g * p.group_m + member;
+  return out.m_tile < p.m_tiles;   // ragged last group: the surplus members idle for this gang-unit
+}
+
+// Producer-side gang barrier: keeps the members' W streams within L2 reach of one another.  The
+// counter only grows (zeroed by the host before the launch); epoch e completes at e * arrivals.
+__device__ __forceinline__ void gang_barrier(unsigned int* ctr, unsigned int target) {
+  __threadfence();
+  atomicAdd(ctr, 1u);
+  const long long t0 = clock64();
+  unsigned int v;
+  do {
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+    if (v >= target) break;
+    __nanosleep(64);
+    if (clock64() - t0 > 4000000000LL) __trap();
+  } while (true);
 }
 
 // value of r[i] for a run-time i without local memory: a 5-level select tree.
@@ -178,7 +194,9 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   const uint32_t cta_rank = (CG == 2) ? cluster_ctarank() : 0u;
   const bool leader = (cta_rank == 0);
   const int cluster = (CG == 2) ? (int)cluster_id_x() : (int)blockIdx.x;
-  const int ncluster = (CG == 2) ? (int)num_clusters_x() : (int)gridDim.x;
+  const int gang = cluster / p.group_m;
+  const int member = cluster - gang * p.group_m;
+  const int gu0 = (gang < p.num_gangs) ? gang : p.num_gang_units;   // surplus clusters idle
 
   if (warp == 0 && lane == 0) {
     prefetch_tensormap(&tmap_h);
@@ -213,8 +231,12 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       const uint32_t stage_tx = Cfg::STAGE_BYTES * CG;   // the pair leader's barrier counts both CTAs' bytes
-      for (int u = cluster; u < p.num_units; u += ncluster) {
-        const Unit un = decode_unit(p, u);
+      unsigned int epoch = 0;
+      for (int gu = gu0; gu < p.num_gang_units; gu += p.num_gangs) {
+        Unit un;
+        const bool active = decode_gang_unit(p, gu, member, un);
+        if (p.group_m > 1) gang_barrier(p.gang_ctr + gang, (++epoch) * (unsigned)(p.group_m * CG));
+        if (!active) continue;
         const int row0 = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M;
         const int vt0 = un.chunk * p.tiles_per_chunk;
         const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
@@ -243,8 +265,9 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
       constexpr uint32_t idesc = make_idesc_bf16(Cfg::UMMA_M, BLOCK_N);
       int stage = 0; uint32_t phase = 0;
       uint32_t tile = 0;
-      for (int u = cluster; u < p.num_units; u += ncluster) {
-        const Unit un = decode_unit(p, u);
+      for (int gu = gu0; gu < p.num_gang_units; gu += p.num_gangs) {
+        Unit un;
+        if (!decode_gang_unit(p, gu, member, un)) continue;
         const int vt0 = un.chunk * p.tiles_per_chunk;
         const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
         for (int vt = vt0; vt < vt1; ++vt, ++tile) {
@@ -277,8 +300,9 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
     const uint32_t tempty_remote = (CG == 2) ? mapa(tempty_bar(0), 0) : tempty_bar(0);
     RowState<CAP> st;
     uint32_t tile = 0;
-    for (int u = cluster; u < p.num_units; u += ncluster) {
-      const Unit un = decode_unit(p, u);
+    for (int gu = gu0; gu < p.num_gang_units; gu += p.num_gangs) {
+      Unit un;
+      if (!decode_gang_unit(p, gu, member, un)) continue;
       const int row = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M + row_in_tile;
       const int vt0 = un.chunk * p.tiles_per_chunk;
       const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
@@ -290,7 +314,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
         tc_fence_after();
         const int colbase = vt * BLOCK_N;
         const int ngroups = min(BLOCK_N, p.V - colbase + 31) >> 5;   // 32-column groups with a valid column
-        for (int g = 0; g < ngroups; ++g) {
+        for (int g = 0; g < ngroups && !(p.debug_flags & 1); ++g) {
           float r[32];
           tmem_ld_32x32(lane_addr + acc * BLOCK_N + g * 32, r);
           tmem_ld_wait();

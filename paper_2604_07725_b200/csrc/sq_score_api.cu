@@ -8,6 +8,7 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -27,6 +28,7 @@ struct sq_score_ctx {
   // partial states
   float* part_m = nullptr; float* part_s = nullptr; float* part_u = nullptr;
   float* part_topv = nullptr; int32_t* part_topi = nullptr; float* zt = nullptr;
+  unsigned int* gang_ctr = nullptr;
   // per-token scratch (used when the caller passes NULL per-token outputs)
   float* tok_lse = nullptr; float* tok_lp = nullptr; float* tok_ent = nullptr; float* tok_conf = nullptr;
   // kernel 2 workspace
@@ -36,7 +38,7 @@ struct sq_score_ctx {
   // driver entry point for tensor-map encoding
   void* encode_fn = nullptr;
   // optional per-kernel timing (sq_score_set_profiling): events around kernel 1, finalize, kernel 2
-  int profiling = 0; int ev_valid = 0;
+  int profiling = 0; int ev_valid = 0; int debug_flags = 0;
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
 };
 
@@ -79,30 +81,34 @@ static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, 
   pl->num_vtiles = (int)cdiv64(cfg->vocab, 256);
   pl->num_k_blocks = (int)cdiv64(cfg->d, 64);
   pl->num_clusters = std::max(1, num_sms / cg);
-  pl->group_m = cfg->group_m > 0 ? cfg->group_m : 8;
   pl->topk_cap = topk_cap_for(k);
+  // gang size: group_m clusters sweep one W chunk together (default 8), never more than there are
+  // token tiles or clusters
+  int G = cfg->group_m > 0 ? cfg->group_m : 8;
+  G = std::max(1, std::min(G, std::min(std::max(1, pl->m_tiles), pl->num_clusters)));
+  pl->group_m = G;
+  pl->num_gangs = pl->num_clusters / G;
+  const int groups = (int)cdiv64(pl->m_tiles, G);
   const int max_chunks = std::min(32, pl->num_vtiles);
   int best_c = 1;
   if (cfg->num_chunks > 0) {
     best_c = std::min(cfg->num_chunks, max_chunks);
   } else if (pl->m_tiles > 0) {
-    // enough chunks that group_m strips x chunks cover the grid, then minimise whole waves x unit length
-    const int gm = std::min(pl->group_m, pl->m_tiles);
-    const int c_lo = std::min(max_chunks, std::max(1, (int)cdiv64(pl->num_clusters, gm) - 1));
-    const int c_hi = std::min(max_chunks, std::max(c_lo, 16));
+    // minimise (rounds of gang-units per gang) x (unit length + fill/drain); ties -> fewer chunks
+    const int c_hi = std::min(max_chunks, (int64_t)groups * 16 < pl->num_gangs ? 32 : 16);
     double best_cost = 1e300;
-    for (int c = c_lo; c <= c_hi; ++c) {
+    for (int c = 1; c <= c_hi; ++c) {
       const int tpc = (int)cdiv64(pl->num_vtiles, c);
       const int ce = (int)cdiv64(pl->num_vtiles, tpc);
-      const int64_t units = (int64_t)pl->m_tiles * ce;
-      const int64_t waves = cdiv64(units, pl->num_clusters);
-      const double cost = (double)waves * (tpc + 0.75);   // 0.75 tile-times of fill/drain per unit
+      const int64_t rounds = cdiv64((int64_t)groups * ce, pl->num_gangs);
+      const double cost = (double)rounds * (tpc + 0.75);   // 0.75 tile-times of fill/drain per unit
       if (cost < best_cost - 1e-9) { best_cost = cost; best_c = c; }
     }
   }
   pl->tiles_per_chunk = (int)cdiv64(pl->num_vtiles, best_c);
   pl->num_chunks = (int)cdiv64(pl->num_vtiles, pl->tiles_per_chunk);
   pl->num_units = pl->m_tiles * pl->num_chunks;
+  pl->num_gang_units = groups * pl->num_chunks;
   return SQ_OK;
 }
 
@@ -139,7 +145,7 @@ static int64_t ws_rows_for(const sq_score_config& cfg) {
 extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
   if (!ctx) return SQ_OK;
   cudaSetDevice(ctx->cfg.device);
-  void* bufs[] = {ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
+  void* bufs[] = {ctx->gang_ctr, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
                   ctx->tok_lse, ctx->tok_lp, ctx->tok_ent, ctx->tok_conf, ctx->tile_base, ctx->red_sum,
                   ctx->red_min, ctx->h_stage, ctx->tgt_stage, ctx->cu_stage, ctx->seq_stage};
   int rc = SQ_OK;
@@ -198,6 +204,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   ctx->cfg = *cfg;
   ctx->num_sms = prop.multiProcessorCount;
   ctx->cap_max = topk_cap_for(cfg->max_k);
+  if (const char* dbg = getenv("SQ_SCORE_DEBUG")) ctx->debug_flags = atoi(dbg);
 
   cudaDriverEntryPointQueryResult qres;
   e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ctx->encode_fn, cudaEnableDefault, &qres);
@@ -218,6 +225,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   A(ws_alloc(ctx, &ctx->part_topv, rows * ctx->cap_max));
   A(ws_alloc(ctx, &ctx->part_topi, rows * ctx->cap_max));
   A(ws_alloc(ctx, &ctx->zt, T));
+  A(ws_alloc(ctx, &ctx->gang_ctr, 256));
   A(ws_alloc(ctx, &ctx->tok_lse, T));
   A(ws_alloc(ctx, &ctx->tok_lp, T));
   A(ws_alloc(ctx, &ctx->tok_ent, T));
@@ -270,7 +278,7 @@ static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int6
 template <int CG, int CAP>
 static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CUtensorMap& th, const CUtensorMap& tw,
                                 const sq::FusedParams& fp, cudaStream_t st) {
-  const int clusters = std::min(pl.num_clusters, pl.num_units);
+  const int clusters = pl.num_gangs * pl.group_m;   // every launched cluster belongs to a gang
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3((unsigned)(clusters * CG));
   lc.blockDim = dim3(sq::NUM_THREADS);
@@ -359,10 +367,13 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
     sq::FusedParams fp = {};
     fp.T = T; fp.V = V; fp.d = d;
     fp.num_k_blocks = pl.num_k_blocks; fp.num_vtiles = pl.num_vtiles; fp.tiles_per_chunk = pl.tiles_per_chunk;
-    fp.num_chunks = pl.num_chunks; fp.m_tiles = pl.m_tiles; fp.group_m = pl.group_m; fp.num_units = pl.num_units;
+    fp.num_chunks = pl.num_chunks; fp.m_tiles = pl.m_tiles; fp.group_m = pl.group_m;
+    fp.num_gangs = pl.num_gangs; fp.num_gang_units = pl.num_gang_units; fp.gang_ctr = ctx->gang_ctr;
+    SQ_CUDA(ctx, cudaMemsetAsync(ctx->gang_ctr, 0, 256 * sizeof(unsigned int), st));
     fp.targets = targets;
     fp.part_m = ctx->part_m; fp.part_s = ctx->part_s; fp.part_u = ctx->part_u;
     fp.part_topv = ctx->part_topv; fp.part_topi = ctx->part_topi; fp.zt = ctx->zt;
+    fp.debug_flags = ctx->debug_flags;
     cudaError_t e;
     if (ctx->profiling) cudaEventRecord(ctx->ev[0], st);
     const int sel = pl.cta_group * 100 + pl.topk_cap;
