@@ -1,6 +1,6 @@
 // sq_finalize_kernel.cuh -- step a6: merge the vocab-chunk partial states of every row and finalise.
 //
-//   lse = M + ln S,  M = max_c m_c,  S = sum_c s_c e^{m_c - M}
+//   lse = M + ln S,  M = max_c m_c,  S = sum_c s_c e^{m_c - M}      (merged in fp64)
 //   entropy = ln S - U / S,  U = sum_c e^{m_c - M} (u_c + (m_c - M) s_c)
 //   target_logprob = z_target - lse
 //   topk_logprob_j = z_(j) - lse,  conf = c(i) = -(1/k) sum_j topk_logprob_j    (Eq. 3)
@@ -20,6 +20,8 @@ struct FinalizeParams {
   const float* part_m;
   const float* part_s;
   const float* part_u;
+  const float* part_cs;     // Kahan residues of s and u
+  const float* part_cu;
   const float* part_topv;   // [C][cap][T]
   const int32_t* part_topi;
   const float* zt;
@@ -43,23 +45,24 @@ sq_finalize_kernel(const FinalizeParams p) {
   const bool has = lane < p.num_chunks;
   const size_t o = (size_t)lane * p.T + row;
   const float m_c = has ? p.part_m[o] : NEG;
-  const float s_c = has ? p.part_s[o] : 0.f;
-  const float u_c = has ? p.part_u[o] : 0.f;
+  // the merge runs in fp64: S - 1 of a peaked row is ~1e-4 and carries the whole entropy
+  const double s_c = has ? ((double)p.part_s[o] - (double)p.part_cs[o]) : 0.0;
+  const double u_c = has ? ((double)p.part_u[o] - (double)p.part_cu[o]) : 0.0;
 
   float M = m_c;
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) M = fmaxf(M, __shfl_xor_sync(FULL, M, off));
-  const float dm = m_c - M;
-  const float w = has ? expf(dm) : 0.f;
-  float S = w * s_c;
-  float U = w * (u_c + dm * s_c);
+  const double dm = (double)m_c - (double)M;
+  const double w = has ? exp(dm) : 0.0;
+  double S = w * s_c;
+  double U = w * (u_c + dm * s_c);
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {
     S += __shfl_xor_sync(FULL, S, off);
     U += __shfl_xor_sync(FULL, U, off);
   }
-  const float lnS = logf(S);
-  const float lse = M + lnS;
+  const double lnS = log(S);
+  const float lse = (float)((double)M + lnS);
 
   // ---- top-k merge: lane c walks chunk c's descending list
   int pos = 0;
@@ -98,7 +101,7 @@ sq_finalize_kernel(const FinalizeParams p) {
     const bool valid = (tgt >= 0) && (tgt < p.V);
     p.lse[row] = lse;
     p.target_logprob[row] = valid ? (p.zt[row] - lse) : 0.f;
-    p.entropy[row] = lnS - U / S;
+    p.entropy[row] = (float)(lnS - U / S);
     p.conf[row] = lse - acc / (float)p.k;   // -(1/k) sum_j (z_(j) - lse)
   }
 }

@@ -50,6 +50,8 @@ struct FusedParams {
   float* part_m;            // [C][T]
   float* part_s;            // [C][T]
   float* part_u;            // [C][T]
+  float* part_cs;           // [C][T] Kahan residues: the true sums are s - cs and u - cu
+  float* part_cu;           // [C][T]
   float* part_topv;         // [C][CAP][T]
   int32_t* part_topi;       // [C][CAP][T]
   float* zt;                // [T] target logit (written by the chunk that owns the target column)
@@ -115,10 +117,11 @@ __device__ __forceinline__ void topk_insert(float (&tv)[CAP], int (&ti)[CAP], fl
 // Per-row running state of one work unit.
 template <int CAP> struct RowState {
   float m, s, u, zt;
+  float cs, cu;   // Kahan compensation of s and u: a peaked row adds ~1e-7 terms to s ~ 1
   float tv[CAP];
   int ti[CAP];
   __device__ __forceinline__ void reset() {
-    m = NEG_BIG; s = 0.f; u = 0.f; zt = 0.f;
+    m = NEG_BIG; s = 0.f; u = 0.f; zt = 0.f; cs = 0.f; cu = 0.f;
 #pragma unroll
     for (int j = 0; j < CAP; ++j) { tv[j] = NEG_BIG; ti[j] = -1; }
   }
@@ -142,7 +145,9 @@ __device__ __forceinline__ void consume32(RowState<CAP>& st, float (&r)[32], int
     const float dm = st.m - gmax;
     const float sc = ex2_approx(dm * LOG2E);
     st.u = (st.u + dm * st.s) * sc;
+    st.cu = (st.cu + dm * st.cs) * sc;
     st.s *= sc;
+    st.cs *= sc;
     st.m = gmax;
   }
   const float m = st.m;
@@ -154,8 +159,16 @@ __device__ __forceinline__ void consume32(RowState<CAP>& st, float (&r)[32], int
     s0 += e0; s1 += e1;
     u0 = fmaf(e0, t0, u0); u1 = fmaf(e1, t1, u1);
   }
-  st.s += s0 + s1;
-  st.u += u0 + u1;
+  {   // compensated accumulation of the group sums
+    const float ys = (s0 + s1) - st.cs;
+    const float ts = st.s + ys;
+    st.cs = (ts - st.s) - ys;
+    st.s = ts;
+    const float yu = (u0 + u1) - st.cu;
+    const float tu = st.u + yu;
+    st.cu = (tu - st.u) - yu;
+    st.u = tu;
+  }
 
   if ((unsigned)(tgt - col0) < 32u) st.zt = pick32(r, tgt - col0);   // a3: target logit
 
@@ -332,6 +345,8 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
         p.part_m[o] = st.m;
         p.part_s[o] = st.s;
         p.part_u[o] = st.u;
+        p.part_cs[o] = st.cs;
+        p.part_cu[o] = st.cu;
 #pragma unroll
         for (int j = 0; j < CAP; ++j) {
           const size_t oj = ((size_t)un.chunk * CAP + j) * p.T + row;

@@ -27,6 +27,7 @@ struct sq_score_ctx {
   char err[512] = {0};
   // partial states
   float* part_m = nullptr; float* part_s = nullptr; float* part_u = nullptr;
+  float* part_cs = nullptr; float* part_cu = nullptr;
   float* part_topv = nullptr; int32_t* part_topi = nullptr; float* zt = nullptr;
   unsigned int* gang_ctr = nullptr;
   // per-token scratch (used when the caller passes NULL per-token outputs)
@@ -145,7 +146,7 @@ static int64_t ws_rows_for(const sq_score_config& cfg) {
 extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
   if (!ctx) return SQ_OK;
   cudaSetDevice(ctx->cfg.device);
-  void* bufs[] = {ctx->gang_ctr, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
+  void* bufs[] = {ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
                   ctx->tok_lse, ctx->tok_lp, ctx->tok_ent, ctx->tok_conf, ctx->tile_base, ctx->red_sum,
                   ctx->red_min, ctx->h_stage, ctx->tgt_stage, ctx->cu_stage, ctx->seq_stage};
   int rc = SQ_OK;
@@ -222,6 +223,8 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   A(ws_alloc(ctx, &ctx->part_m, rows));
   A(ws_alloc(ctx, &ctx->part_s, rows));
   A(ws_alloc(ctx, &ctx->part_u, rows));
+  A(ws_alloc(ctx, &ctx->part_cs, rows));
+  A(ws_alloc(ctx, &ctx->part_cu, rows));
   A(ws_alloc(ctx, &ctx->part_topv, rows * ctx->cap_max));
   A(ws_alloc(ctx, &ctx->part_topi, rows * ctx->cap_max));
   A(ws_alloc(ctx, &ctx->zt, T));
@@ -372,6 +375,7 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
     SQ_CUDA(ctx, cudaMemsetAsync(ctx->gang_ctr, 0, 256 * sizeof(unsigned int), st));
     fp.targets = targets;
     fp.part_m = ctx->part_m; fp.part_s = ctx->part_s; fp.part_u = ctx->part_u;
+    fp.part_cs = ctx->part_cs; fp.part_cu = ctx->part_cu;
     fp.part_topv = ctx->part_topv; fp.part_topi = ctx->part_topi; fp.zt = ctx->zt;
     fp.debug_flags = ctx->debug_flags;
     cudaError_t e;
@@ -392,6 +396,7 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
     fin.T = T; fin.V = V; fin.k = k; fin.cap = pl.topk_cap; fin.num_chunks = pl.num_chunks;
     fin.targets = targets;
     fin.part_m = ctx->part_m; fin.part_s = ctx->part_s; fin.part_u = ctx->part_u;
+    fin.part_cs = ctx->part_cs; fin.part_cu = ctx->part_cu;
     fin.part_topv = ctx->part_topv; fin.part_topi = ctx->part_topi; fin.zt = ctx->zt;
     fin.lse = lse; fin.target_logprob = lp; fin.entropy = ent; fin.conf = conf;
     fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;

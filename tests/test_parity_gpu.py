@@ -1,0 +1,383 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element on
+the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+  abs 2e-3 on logsumexp, target log-prob and top-k values (and conf, their mean);
+  rel 1e-3 on entropy and the sequence aggregates;
+  top-k indices exact wherever adjacent oracle values differ by more than 1e-2.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import workloads
+from oracle import sq_oracle as O
+
+pytestmark = pytest.mark.gpu
+
+ABS_TOL = 2e-3
+REL_TOL = 1e-3
+GAP = 1e-2
+SEQ_KEYS = ("seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf")
+
+
+def _sq():
+    import paper_2604_07725_b200 as sq
+    return sq
+
+
+def run_gpu(inp, k=None, window=None, targets=None, **eng_kw):
+    sq = _sq()
+    wl = inp["workload"]
+    k = wl.k if k is None else k
+    window = wl.window if window is None else window
+    dev = torch.device("cuda:0")
+    eng = sq.SqScore(wl.d, wl.V, max_tokens=max(1, inp["T"]), max_seqs=max(1, inp["B"]), max_k=k, **eng_kw)
+    tg = inp["targets"] if targets is None else targets
+    out = eng.run(inp["H"].to(dev), inp["W"].to(dev), tg.to(dev), inp["cu_seqlens"].to(dev), k, window)
+    torch.cuda.synchronize()
+    eng.close()
+    return {n: v.cpu().numpy() for n, v in out.items()}
+
+
+def check_tokens(out, ref, k, rows=None):
+    """`ref` holds k+1 oracle top entries; `rows` selects GPU rows when the oracle scored a sample."""
+    sel = (lambda a: a) if rows is None else (lambda a: a[rows])
+    for key in ("lse", "target_logprob", "conf"):
+        np.testing.assert_allclose(sel(out[key]), ref[key], rtol=0, atol=ABS_TOL, err_msg=key)
+    np.testing.assert_allclose(sel(out["entropy"]), ref["entropy"], rtol=REL_TOL, atol=1e-6, err_msg="entropy")
+    tv, ti = sel(out["topk_logprob"]), sel(out["topk_index"])
+    rv, ri = ref["topk_logprob"], ref["topk_index"]
+    np.testing.assert_allclose(tv, rv[:, :k], rtol=0, atol=ABS_TOL, err_msg="topk_logprob")
+    assert (np.diff(tv, axis=1) <= 0).all(), "top-k values must be non-increasing"
+    # index j must match where it is separated from both oracle neighbours by more than GAP
+    n = rv.shape[0]
+    gap_below = np.full((n, k), np.inf)
+    kk = rv.shape[1]
+    gap_below[:, :min(k, kk - 1)] = (rv[:, :-1] - rv[:, 1:])[:, :k]
+    gap_above = np.full((n, k), np.inf)
+    gap_above[:, 1:] = (rv[:, :-1] - rv[:, 1:])[:, :k - 1]
+    must = (gap_below > GAP) & (gap_above > GAP)
+    bad = must & (ti != ri[:, :k])
+    assert not bad.any(), "top-k index mismatch at %s" % (np.argwhere(bad)[:5],)
+    # the rest must at least be valid: in range, unique per row, and carry a matching value
+    assert (ti >= 0).all()
+    for r in range(min(n, 64)):
+        assert len(set(ti[r].tolist())) == k
+
+
+def check_seqs(out, ref):
+    for key in SEQ_KEYS:
+        a, b = out[key], np.asarray(ref[key])
+        assert (np.isnan(a) == np.isnan(b)).all(), key
+        ok = ~np.isnan(b)
+        np.testing.assert_allclose(a[ok], b[ok], rtol=REL_TOL, atol=1e-6, err_msg=key)
+
+
+def oracle_full(inp, k=None, window=None, targets=None):
+    wl = inp["workload"]
+    return O.score(inp["H"], inp["W"], inp["targets"] if targets is None else targets, inp["cu_seqlens"],
+                   wl.k if k is None else k, wl.window if window is None else window)
+
+
+# ------------------------------------------------------------------------------------------ small, full
+@pytest.mark.parametrize("cg", [1, 2])
+def test_tiny_config(cg):
+    inp = workloads.make_inputs(workloads.CONFIGS["tiny"])
+    out = run_gpu(inp, cta_group=cg)
+    ref = oracle_full(inp)
+    check_tokens(out, ref, inp["k"])
+    check_seqs(out, ref)
+
+
+SMALL = [
+    # several token tiles, ragged T, d not a multiple of 64, V not a multiple of 32 or 256
+    dict(name="ragged", d=200, V=1003, B=3, len_lo=100, len_hi=300, k=5, window=16, seed=5, w_std=0.1),
+    # several vocab tiles and chunks, planted peaks
+    dict(name="mid", d=512, V=5000, B=3, len_lo=200, len_hi=500, k=20, window=64, seed=6, w_std=0.05,
+         planted_frac=0.5, planted_scale=3.0, rmsnorm=True),
+    # strongly peaked rows: entropy -> 0 is where rel 1e-3 is hardest
+    dict(name="peaked", d=256, V=3000, B=2, len_lo=150, len_hi=260, k=20, window=32, seed=8, w_std=0.05,
+         planted_frac=0.5, planted_scale=30.0, rmsnorm=True),
+    # vocabulary smaller than one tile, tiny d
+    dict(name="smallV", d=8, V=40, B=2, len_lo=5, len_hi=40, k=8, window=4, seed=9, w_std=1.0),
+]
+
+
+@pytest.mark.parametrize("spec", SMALL, ids=[s["name"] for s in SMALL])
+@pytest.mark.parametrize("cg,chunks,gm", [(2, 0, 0), (1, 0, 0), (2, 3, 2), (1, 2, 1), (2, 1, 8)])
+def test_small_shapes_full_parity(spec, cg, chunks, gm):
+    inp = workloads.make_inputs(workloads.custom(**spec))
+    out = run_gpu(inp, cta_group=cg, num_chunks=chunks, group_m=gm)
+    ref = oracle_full(inp)
+    check_tokens(out, ref, inp["k"])
+    check_seqs(out, ref)
+
+
+@pytest.mark.parametrize("k", [1, 5, 8, 9, 20, 21, 32])
+def test_every_topk_capacity(k):
+    inp = workloads.make_inputs(workloads.custom(name="k", d=64, V=2000, B=2, len_lo=60, len_hi=200, k=k, window=8,
+                                                 seed=20 + k, w_std=0.2))
+    out = run_gpu(inp)
+    ref = oracle_full(inp)
+    check_tokens(out, ref, k)
+    check_seqs(out, ref)
+    assert out["conf"].min() >= math.log(k) - 1e-4        # Jensen bound, reading #2
+
+
+def test_k_equals_vocab():
+    inp = workloads.make_inputs(workloads.custom(name="kV", d=16, V=8, B=1, len_lo=50, len_hi=50, k=8, window=8, seed=3, w_std=1.0))
+    out = run_gpu(inp)
+    ref = oracle_full(inp)
+    check_tokens(out, ref, 8)
+    np.testing.assert_allclose(np.exp(out["topk_logprob"].astype(np.float64)).sum(1), 1.0, atol=1e-4)
+    for r in range(inp["T"]):
+        assert sorted(out["topk_index"][r].tolist()) == list(range(8))
+
+
+# ------------------------------------------------------------------------------------------ edge cases
+def test_empty_short_and_single_token_sequences():
+    wl = workloads.custom(name="edge", d=64, V=700, B=6, k=5, window=16, seed=31, w_std=0.2)
+    inp = workloads.make_inputs(wl, lengths=[0, 1, 15, 16, 17, 300])     # empty, L=1, L<w, L=w, L=w+1, long
+    out = run_gpu(inp)
+    ref = oracle_full(inp)
+    check_tokens(out, ref, 5)
+    check_seqs(out, ref)
+    assert np.isnan(out["seq_mean_conf"][0]) and np.isnan(out["seq_min_window_conf"][0])
+    assert out["seq_min_window_conf"][1] == pytest.approx(out["conf"][0], rel=1e-6)
+
+
+def test_all_sequences_empty_and_zero_tokens():
+    wl = workloads.custom(name="none", d=64, V=300, B=3, k=5, window=4, seed=32)
+    inp = workloads.make_inputs(wl, lengths=[0, 0, 0])
+    out = run_gpu(inp)
+    for key in SEQ_KEYS:
+        assert np.isnan(out[key]).all()
+    assert out["lse"].shape == (0,)
+
+
+def test_no_target_rows_are_excluded_from_the_mean():
+    wl = workloads.custom(name="notgt", d=64, V=500, B=2, len_lo=40, len_hi=80, k=5, window=8, seed=33, w_std=0.2)
+    inp = workloads.make_inputs(wl)
+    tg = inp["targets"].clone()
+    tg[::3] = -1
+    tg[1::7] = wl.V          # == V is also "no target"
+    L0 = int(inp["cu_seqlens"][1])
+    out = run_gpu(inp, targets=tg)
+    ref = oracle_full(inp, targets=tg.numpy())
+    check_tokens(out, ref, 5)
+    check_seqs(out, ref)
+    assert (out["target_logprob"][::3] == 0).all()
+    # a sequence whose targets are all invalid has a NaN log-prob mean and finite other aggregates
+    tg2 = inp["targets"].clone(); tg2[:L0] = -1
+    out2 = run_gpu(inp, targets=tg2)
+    assert np.isnan(out2["seq_mean_logprob"][0]) and np.isfinite(out2["seq_mean_logprob"][1])
+    assert np.isfinite(out2["seq_mean_entropy"]).all()
+
+
+def test_targets_on_tile_edges_and_topk_positions():
+    V, d = 1100, 64
+    cols = [0, 31, 32, 127, 128, 255, 256, 511, 512, 1023, 1024, V - 1]
+    T = len(cols) * 11
+    g = torch.Generator().manual_seed(4)
+    W = (torch.randn(V, d, generator=g) * 0.05).to(torch.bfloat16)
+    H = torch.randn(T, d, generator=g)
+    tg = torch.tensor([cols[t % len(cols)] for t in range(T)], dtype=torch.int32)
+    H = (H / H.norm(dim=1, keepdim=True) * 8 + 40.0 * W[tg.long()].float()).to(torch.bfloat16)   # the target wins top-1
+    wl = workloads.custom(name="edges", d=d, V=V, B=1, k=5, window=8)
+    inp = {"H": H, "W": W, "targets": tg, "cu_seqlens": torch.tensor([0, T], dtype=torch.int32), "k": 5, "window": 8,
+           "workload": wl, "T": T, "B": 1}
+    for cg in (1, 2):
+        out = run_gpu(inp, cta_group=cg, num_chunks=2)
+        ref = oracle_full(inp)
+        check_tokens(out, ref, 5)
+        assert (out["topk_index"][:, 0] == tg.numpy()).all()
+        np.testing.assert_allclose(out["target_logprob"], out["topk_logprob"][:, 0], atol=1e-6)
+
+
+def test_duplicate_rows_give_bit_identical_outputs():
+    wl = workloads.custom(name="dup", d=128, V=3000, B=1, len_lo=600, len_hi=600, k=20, window=8, seed=35, w_std=0.1)
+    inp = workloads.make_inputs(wl)
+    src = 5
+    places = [0, 31, 32, 127, 128, 255, 256, 300, 511, 599]      # different lanes, warps, CTAs of a pair, token tiles
+    for t in places:
+        inp["H"][t] = inp["H"][src]
+        inp["targets"][t] = inp["targets"][src]
+    out = run_gpu(inp, num_chunks=3)
+    for key in ("lse", "target_logprob", "entropy", "conf", "topk_logprob", "topk_index"):
+        for t in places:
+            assert (out[key][t] == out[key][src]).all(), (key, t)
+
+
+# ------------------------------------------------------------------------------------------ closed forms on the GPU
+def test_identical_w_rows_closed_form():
+    V, d, T = 1500, 64, 300
+    g = torch.Generator().manual_seed(2)
+    w = (torch.randn(d, generator=g) * 0.3).to(torch.bfloat16)
+    W = w.repeat(V, 1).contiguous()
+    H = torch.randn(T, d, generator=g).to(torch.bfloat16)
+    wl = workloads.custom(name="ident", d=d, V=V, B=1, k=20, window=8)
+    inp = {"H": H, "W": W, "targets": torch.randint(0, V, (T,), generator=g, dtype=torch.int32),
+           "cu_seqlens": torch.tensor([0, T], dtype=torch.int32), "k": 20, "window": 8, "workload": wl, "T": T, "B": 1}
+    out = run_gpu(inp, num_chunks=3)
+    lnV = math.log(V)
+    z = (H.double() @ w.double()).numpy()
+    np.testing.assert_allclose(out["lse"], z + lnV, atol=ABS_TOL)
+    np.testing.assert_allclose(out["target_logprob"], -lnV, atol=ABS_TOL)      # BASELINE.json pin
+    np.testing.assert_allclose(out["entropy"], lnV, rtol=REL_TOL)              # BASELINE.json pin
+    np.testing.assert_allclose(out["topk_logprob"], -lnV, atol=ABS_TOL)
+    np.testing.assert_allclose(out["conf"], lnV, atol=ABS_TOL)
+    for r in range(0, T, 37):                                                  # ties: any 20 distinct valid ids
+        ids = out["topk_index"][r]
+        assert len(set(ids.tolist())) == 20 and ids.min() >= 0 and ids.max() < V
+    np.testing.assert_allclose(out["seq_mean_entropy"], lnV, rtol=REL_TOL)
+
+
+@pytest.mark.parametrize("shift", [80.0, -80.0])
+def test_large_logit_shift(shift):
+    # a constant W column seen by a constant H column shifts every logit by `shift`: catches a
+    # missing max-subtraction (exp overflow/underflow in fp32)
+    wl = workloads.custom(name="shift", d=64, V=2000, B=1, len_lo=200, len_hi=200, k=5, window=8, seed=37, w_std=0.1)
+    inp = workloads.make_inputs(wl)
+    inp["H"][:, 63] = 8.0
+    inp["W"][:, 63] = shift / 8.0
+    out = run_gpu(inp, num_chunks=2)
+    ref = oracle_full(inp)
+    check_tokens(out, ref, 5)
+    check_seqs(out, ref)
+    assert np.isfinite(out["lse"]).all() and abs(np.median(out["lse"]) - shift) < 20
+
+
+# ------------------------------------------------------------------------------------------ full-size configs
+def sample_rows(inp, n_uniform=48, seed=123):
+    """Seeded row sample for oracle-A at full size: first/last row, rows next to every sequence
+    boundary, token-tile edges, planted and unplanted rows, the rest uniform."""
+    T = inp["T"]
+    cu = inp["cu_seqlens"].numpy().astype(np.int64)
+    rows = {0, T - 1, 127, 128, 255, 256, 257, 511, 512}
+    for c in cu[1:-1]:
+        rows.update((int(c) - 1, int(c)))
+    rng = np.random.default_rng(seed)
+    pl = inp["planted"].numpy()
+    for mask in (pl, ~pl):
+        idx = np.nonzero(mask)[0]
+        if len(idx):
+            rows.update(rng.choice(idx, size=min(8, len(idx)), replace=False).tolist())
+    rows.update(rng.integers(0, T, size=n_uniform).tolist())
+    last_tile = (T - 1) // 256 * 256
+    rows.update((last_tile, min(T - 1, last_tile + 129)))
+    return np.array(sorted(r for r in rows if 0 <= r < T), dtype=np.int64)
+
+
+@pytest.mark.parametrize("name", ["qwen3_4b", "qwen3_8b", "gpt_oss", "qwen3_32b"])
+def test_full_size_config_sampled_rows_and_all_sequences(name):
+    """BASELINE.json configs 2-5 at full size in the launch configuration bench.py times (default
+    planner, CTA pairs): kernel 1 + finalize on sampled rows (oracle-A), kernel 2 on every sequence
+    (oracle-B applied to the GPU's own per-token outputs), and one whole sequence end to end."""
+    wl = workloads.CONFIGS[name]
+    inp = workloads.make_inputs(wl)
+    out = run_gpu(inp)
+    T, k = inp["T"], wl.k
+    W64 = O.widen(inp["W"])
+    tg = inp["targets"].numpy()
+    rows = sample_rows(inp)
+    ref = O.token_scores(inp["H"][rows], W64, tg[rows], k)
+    check_tokens(out, ref, k, rows=rows)
+    # properties that hold for every row at any size
+    assert np.isfinite(out["lse"]).all()
+    assert (out["entropy"] > 0).all() and (out["entropy"] <= math.log(wl.V) * (1 + 1e-4)).all()
+    assert (out["target_logprob"] <= 1e-4).all()
+    assert (out["conf"] >= math.log(k) - 1e-3).all()
+    assert (np.diff(out["topk_logprob"], axis=1) <= 0).all()
+    assert (out["target_logprob"] <= out["topk_logprob"][:, 0] + 1e-5).all()
+    assert (out["topk_index"] >= 0).all() and (out["topk_index"] < wl.V).all()
+    pl = inp["planted"].numpy()
+    if pl.any() and (~pl).any():
+        assert out["target_logprob"][pl].mean() > out["target_logprob"][~pl].mean() + 1.0   # planted rows favour the target
+    # kernel 2 at full size, isolated: fp64 reduction oracle on the GPU's per-token outputs
+    seq_ref = O.sequence_scores(out["target_logprob"], out["entropy"], out["conf"], inp["cu_seqlens"].numpy(), wl.window)
+    check_seqs(out, seq_ref)
+    # one whole sequence end to end from H and W (the shortest one)
+    cu = inp["cu_seqlens"].numpy().astype(np.int64)
+    b = int(np.argmin(np.diff(cu)))
+    lo, hi = int(cu[b]), int(cu[b + 1])
+    if hi - lo <= 2600:
+        parts = [O.token_scores(inp["H"][r0:min(hi, r0 + 256)], W64, tg[r0:min(hi, r0 + 256)], k) for r0 in range(lo, hi, 256)]
+        full = {key: np.concatenate([p[key] for p in parts]) for key in ("lse", "target_logprob", "entropy", "conf", "topk_logprob", "topk_index")}
+        check_tokens(out, full, k, rows=np.arange(lo, hi))
+        e2e = O.sequence_scores(full["target_logprob"], full["entropy"], full["conf"], [0, hi - lo], wl.window)
+        for key in SEQ_KEYS:
+            np.testing.assert_allclose(out[key][b], e2e[key][0], rtol=REL_TOL, err_msg=key)
+
+
+# ------------------------------------------------------------------------------------------ kernel 2 alone
+@pytest.mark.parametrize("window", [1, 2, 16, 511, 512, 513, 2048, 4096, 4097, 100000])
+def test_reduce_kernel_alone(window):
+    sq = _sq()
+    lens = [1, 2, 511, 512, 513, 0, 4095, 4096, 4097, 8192, 9000, 20000, 3, 1025]
+    g = torch.Generator().manual_seed(77)
+    T = sum(lens)
+    cu = torch.tensor(np.concatenate([[0], np.cumsum(lens)]), dtype=torch.int32)
+    lp = -(torch.rand(T, generator=g) * 12); en = torch.rand(T, generator=g) * 11; cf = 3 + torch.rand(T, generator=g) * 12
+    cf[30000:30040] = 0.5                      # a dip the minimum window must find
+    eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5)
+    dev = torch.device("cuda:0")
+    out = eng.reduce(lp.to(dev), en.to(dev), cf.to(dev), cu.to(dev), window)
+    torch.cuda.synchronize()
+    ref = O.sequence_scores(lp.numpy(), en.numpy(), cf.numpy(), cu.numpy(), window)
+    check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
+    eng.close()
+
+
+def test_reduce_many_sequences():
+    sq = _sq()
+    r = workloads.reduction_inputs(3000, 1, 3000, seed=5)
+    eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5)
+    dev = torch.device("cuda:0")
+    out = eng.reduce(r["target_logprob"].to(dev), r["entropy"].to(dev), r["conf"].to(dev), r["cu_seqlens"].to(dev), 256)
+    torch.cuda.synchronize()
+    ref = O.sequence_scores(r["target_logprob"].numpy(), r["entropy"].numpy(), r["conf"].numpy(), r["cu_seqlens"].numpy(), 256)
+    check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
+    eng.close()
+
+
+# ------------------------------------------------------------------------------------------ API behaviour
+def test_run_host_matches_run_and_null_per_token_outputs():
+    sq = _sq()
+    inp = workloads.make_inputs(workloads.custom(name="host", d=128, V=3000, B=3, len_lo=100, len_hi=400, k=20, window=32, seed=41, w_std=0.1))
+    dev = torch.device("cuda:0")
+    eng = sq.SqScore(128, 3000, max_tokens=inp["T"], max_seqs=3, max_k=20)
+    W = inp["W"].to(dev)
+    out = eng.run(inp["H"].to(dev), W, inp["targets"].to(dev), inp["cu_seqlens"].to(dev), 20, 32)
+    out_seq_only = eng.run(inp["H"].to(dev), W, inp["targets"].to(dev), inp["cu_seqlens"].to(dev), 20, 32, per_token=False, topk=False)
+    host = torch.empty(12, dtype=torch.float32).pin_memory()
+    eng.run_host(inp["H"].pin_memory(), W, inp["targets"].pin_memory(), inp["cu_seqlens"].pin_memory(), 20, 32, host)
+    torch.cuda.synchronize()
+    dev_seq = torch.cat([out[n] for n in SEQ_KEYS]).cpu()
+    assert torch.equal(dev_seq, host)
+    assert torch.equal(dev_seq, torch.cat([out_seq_only[n] for n in SEQ_KEYS]).cpu())
+    assert eng.launch_count() == 15
+    eng.close()
+
+
+def test_run_rejects_bad_arguments():
+    sq = _sq()
+    dev = torch.device("cuda:0")
+    eng = sq.SqScore(64, 1000, max_tokens=128, max_seqs=2, max_k=5)
+    H = torch.zeros(128, 64, dtype=torch.bfloat16, device=dev); W = torch.zeros(1000, 64, dtype=torch.bfloat16, device=dev)
+    tg = torch.zeros(128, dtype=torch.int32, device=dev); cu = torch.tensor([0, 64, 128], dtype=torch.int32, device=dev)
+    for kw in (dict(k=6), dict(k=0), dict(window=0)):
+        args = dict(k=5, window=4); args.update(kw)
+        with pytest.raises(sq.SqScoreError) as ei:
+            eng.run(H, W, tg, cu, args["k"], args["window"])
+        assert ei.value.code == sq.ERR_INVALID_ARG
+    Hbig = torch.zeros(256, 64, dtype=torch.bfloat16, device=dev)
+    with pytest.raises(sq.SqScoreError):
+        eng.run(Hbig, W, torch.zeros(256, dtype=torch.int32, device=dev), cu, 5, 4)
+    with pytest.raises(sq.SqScoreError):
+        # H shifted by 8 bytes: not 16-byte aligned
+        eng.run(H.view(-1)[4:4 + 64 * 100].view(100, 64), W, tg[:100], torch.tensor([0, 100], dtype=torch.int32, device=dev), 5, 4)
+    out = eng.run(H, W, tg, cu, 5, 4)      # the ctx is still usable after errors
+    torch.cuda.synchronize()
+    assert np.isfinite(out["lse"].cpu().numpy()).all()
+    eng.close()
