@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -95,12 +96,20 @@ static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, 
   if (cfg->num_chunks > 0) {
     best_c = std::min(cfg->num_chunks, max_chunks);
   } else if (pl->m_tiles > 0) {
-    // minimise (rounds of gang-units per gang) x (unit length + fill/drain); ties -> fewer chunks
+    // The gangs in flight work on ceil(num_gangs / C) different token groups, i.e. about
+    // num_clusters / C token strips of rows_per_tile x d bf16 are re-read from L2 for every vocab
+    // tile.  Keep that hot set under ~40 MB of the 126 MB L2 (measured: beyond ~50 MB the strips
+    // start to miss and HBM traffic and power go up), then minimise
+    // (rounds of gang-units per gang) x (unit length + fill/drain); ties -> fewer chunks.
+    const double strip_mb = (double)pl->rows_per_tile * cfg->d * 2.0 / 1e6;
+    const int c_l2 = (int)std::ceil(pl->num_gangs * G * strip_mb / 40.0);
     const int c_hi = std::min(max_chunks, (int64_t)groups * 16 < pl->num_gangs ? 32 : 16);
+    const int c_lo = std::max(1, std::min(c_hi, c_l2));
     double best_cost = 1e300;
-    for (int c = 1; c <= c_hi; ++c) {
+    for (int c = c_lo; c <= c_hi; ++c) {
       const int tpc = (int)cdiv64(pl->num_vtiles, c);
       const int ce = (int)cdiv64(pl->num_vtiles, tpc);
+      if (ce < c_lo && c < c_hi) continue;   // rounding merged chunks below the L2 bound
       const int64_t rounds = cdiv64((int64_t)groups * ce, pl->num_gangs);
       const double cost = (double)rounds * (tpc + 0.75);   // 0.75 tile-times of fill/drain per unit
       if (cost < best_cost - 1e-9) { best_cost = cost; best_c = c; }

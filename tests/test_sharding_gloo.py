@@ -1,0 +1,62 @@
+"""world_size-2 gloo test (CPU) of the N>1 path's host logic: sequences are dealt to ranks, each
+rank scores its own packed sub-batch (here with the fp64 oracle standing in for the kernels -- the
+GPU is not available), and the all_gather puts the per-sequence scalars back in global order."""
+import os
+import socket
+
+import numpy as np
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+import workloads
+from oracle import sq_oracle as O
+from paper_2604_07725_b200 import sharding
+
+
+def _free_port():
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); p = s.getsockname()[1]; s.close(); return p
+
+
+def _worker(rank, world, port, ret):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    torch.set_num_threads(1)
+    wl = workloads.custom(name="shard", d=16, V=50, B=5, k=3, window=4, seed=17, w_std=0.5)
+    inp = workloads.make_inputs(wl, lengths=[9, 0, 30, 4, 17])
+    ids, local_cu, rows = sharding.local_batch(inp["cu_seqlens"], rank, world)
+    tok = O.score(inp["H"][rows], inp["W"], inp["targets"][rows].numpy(), local_cu.numpy(), wl.k, wl.window)
+    local = {k: torch.tensor(tok[k], dtype=torch.float32) for k in sharding.SEQ_KEYS}
+    out = sharding.gather_sequence_scores(local, ids, inp["B"], world)
+    if rank == 0:
+        ret.update({k: v.numpy() for k, v in out.items()})
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_rank_sharding_matches_single_rank():
+    world = 2
+    with mp.Manager() as mgr:
+        ret = mgr.dict()
+        mp.spawn(_worker, args=(world, _free_port(), ret), nprocs=world, join=True)
+        got = dict(ret)
+    wl = workloads.custom(name="shard", d=16, V=50, B=5, k=3, window=4, seed=17, w_std=0.5)
+    inp = workloads.make_inputs(wl, lengths=[9, 0, 30, 4, 17])
+    ref = O.score(inp["H"], inp["W"], inp["targets"].numpy(), inp["cu_seqlens"].numpy(), wl.k, wl.window)
+    for key in sharding.SEQ_KEYS:
+        a, b = got[key], ref[key]
+        assert (np.isnan(a) == np.isnan(b)).all()
+        np.testing.assert_allclose(a[~np.isnan(b)], b[~np.isnan(b)], rtol=1e-6)
+
+
+def test_local_batch_partitions_rows():
+    cu = torch.tensor([0, 9, 9, 39, 43, 60], dtype=torch.int32)
+    seen = []
+    for r in range(3):
+        ids, lcu, rows = sharding.local_batch(cu, r, 3)
+        assert int(lcu[-1]) == len(rows)
+        seen += rows.tolist()
+        for i, b in enumerate(ids):
+            assert int(lcu[i + 1] - lcu[i]) == int(cu[b + 1] - cu[b])
+    assert sorted(seen) == list(range(60))
