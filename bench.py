@@ -261,10 +261,12 @@ def run_ours(args):
     achieved = flops / (k1_ms * 1e-3) / 1e12
     peak = peaks["bf16_tflops_sustained"]                     # kernel timed inside a long step
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic_%s.json" % wl.name)
+    tpath = os.path.join(ROOT, "profiles", "traffic_%s.csv" % wl.name)   # from the committed ncu --set full summary
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get("dram_bytes_per_launch")
+            for ln in f:
+                if ln.startswith("sq_fused_score_kernel,"):
+                    traffic = float(ln.strip().split(",")[1])
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
