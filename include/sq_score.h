@@ -91,7 +91,10 @@ typedef struct {
   int num_units;        /* m_tiles * num_chunks                                                   */
   int num_clusters;     /* clusters the device can hold (= SMs / cta_group)                       */
   int num_gangs;        /* num_clusters / group_m; the launch uses num_gangs * group_m clusters   */
-  int num_gang_units;   /* ceil(m_tiles / group_m) * num_chunks, dealt round-robin to the gangs   */
+  int num_gang_units;   /* ceil(m_split / group_m) * num_chunks, dealt round-robin to the gangs   */
+  int m_split;          /* token tiles [0,m_split) -> gangs; [m_split,m_tiles) -> the smaller gang B */
+  int gang_b_size;      /* num_clusters - num_gangs * group_m clusters form gang B (0 = none)     */
+  int num_gang_units_b; /* ceil((m_tiles - m_split) / gang_b_size) * num_chunks; 0 = B not used   */
   int topk_cap;         /* compiled top-k list capacity used for this k (8, 20 or 32)             */
 } sq_score_plan_t;
 

@@ -26,7 +26,7 @@ class sq_score_outputs(C.Structure):
 class sq_score_plan_t(C.Structure):
     _fields_ = [(n, C.c_int) for n in
                 ("cta_group", "rows_per_tile", "m_tiles", "num_vtiles", "num_k_blocks", "num_chunks",
-                 "tiles_per_chunk", "group_m", "num_units", "num_clusters", "num_gangs", "num_gang_units", "topk_cap")]
+                 "tiles_per_chunk", "group_m", "num_units", "num_clusters", "num_gangs", "num_gang_units", "m_split", "gang_b_size", "num_gang_units_b", "topk_cap")]
 
 
 class SqScoreError(RuntimeError):

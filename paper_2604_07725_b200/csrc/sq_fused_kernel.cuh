@@ -44,7 +44,10 @@ struct FusedParams {
   int m_tiles;
   int group_m;              // gang size
   int num_gangs;
-  int num_gang_units;       // ceil(m_tiles / group_m) * num_chunks
+  int num_gang_units;       // ceil(m_split / group_m) * num_chunks (class A)
+  int m_split;              // token tiles [0, m_split) go to the class-A gangs, [m_split, m_tiles) to gang B
+  int gang_b_size;          // clusters left over after the class-A gangs form one smaller gang B (0 = none)
+  int num_gang_units_b;     // ceil((m_tiles - m_split) / gang_b_size) * num_chunks
   unsigned int* gang_ctr;   // [num_gangs], zeroed before the launch
   const int32_t* targets;   // [T]
   float* part_m;            // [C][T]
@@ -65,11 +68,38 @@ struct Unit { int m_tile; int chunk; };
 // order [g][c], round-robin over gangs; member j of the gang takes token tile g*group_m + j.  All
 // members sweep the same W chunk at the same time, so each W tile is fetched from HBM once per
 // gang-unit and served to the other members from L2; gangs working on the same g share its H strips.
-__device__ __forceinline__ bool decode_gang_unit(const FusedParams& p, int gu, int member, Unit& out) {
+// The num_clusters % group_m clusters that do not fill a gang form one smaller gang B with its own
+// slice of token tiles (sized by the planner so that both classes finish together).
+struct GangCtx {
+  int ctr;       // index of this gang's barrier counter
+  int member;    // position in the gang
+  int size;      // clusters in the gang
+  int m_base, m_end;        // token tiles this gang class owns
+  int gu0, gu_step, gu_end; // this gang's gang-units: gu0, gu0 + gu_step, ... < gu_end
+};
+__device__ __forceinline__ GangCtx make_gang_ctx(const FusedParams& p, int cluster) {
+  GangCtx g;
+  const int a_clusters = p.num_gangs * p.group_m;
+  if (cluster < a_clusters) {
+    g.ctr = cluster / p.group_m;
+    g.member = cluster - g.ctr * p.group_m;
+    g.size = p.group_m;
+    g.m_base = 0; g.m_end = p.m_split;
+    g.gu0 = g.ctr; g.gu_step = p.num_gangs; g.gu_end = p.num_gang_units;
+  } else {
+    g.ctr = p.num_gangs;
+    g.member = cluster - a_clusters;
+    g.size = p.gang_b_size;
+    g.m_base = p.m_split; g.m_end = p.m_tiles;
+    g.gu0 = 0; g.gu_step = 1; g.gu_end = p.num_gang_units_b;
+  }
+  return g;
+}
+__device__ __forceinline__ bool decode_gang_unit(const FusedParams& p, const GangCtx& gc, int gu, Unit& out) {
   const int g = gu / p.num_chunks;
   out.chunk = gu - g * p.num_chunks;
-  out.m_tile = g * p.group_m + member;
-  return out.m_tile < p.m_tiles;   // ragged last group: the surplus members idle for this gang-unit
+  out.m_tile = gc.m_base + g * gc.size + gc.member;
+  return out.m_tile < gc.m_end;   // ragged last group: the surplus members idle for this gang-unit
 }
 
 // Producer-side gang barrier: keeps the members' W streams within L2 reach of one another.  The
@@ -207,9 +237,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   const uint32_t cta_rank = (CG == 2) ? cluster_ctarank() : 0u;
   const bool leader = (cta_rank == 0);
   const int cluster = (CG == 2) ? (int)cluster_id_x() : (int)blockIdx.x;
-  const int gang = cluster / p.group_m;
-  const int member = cluster - gang * p.group_m;
-  const int gu0 = (gang < p.num_gangs) ? gang : p.num_gang_units;   // surplus clusters idle
+  const GangCtx gc = make_gang_ctx(p, cluster);
 
   if (warp == 0 && lane == 0) {
     prefetch_tensormap(&tmap_h);
@@ -245,10 +273,10 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
       int stage = 0; uint32_t phase = 0;
       const uint32_t stage_tx = Cfg::STAGE_BYTES * CG;   // the pair leader's barrier counts both CTAs' bytes
       unsigned int epoch = 0;
-      for (int gu = gu0; gu < p.num_gang_units; gu += p.num_gangs) {
+      for (int gu = gc.gu0; gu < gc.gu_end; gu += gc.gu_step) {
         Unit un;
-        const bool active = decode_gang_unit(p, gu, member, un);
-        if (p.group_m > 1) gang_barrier(p.gang_ctr + gang, (++epoch) * (unsigned)(p.group_m * CG));
+        const bool active = decode_gang_unit(p, gc, gu, un);
+        if (gc.size > 1) gang_barrier(p.gang_ctr + gc.ctr, (++epoch) * (unsigned)(gc.size * CG));
         if (!active) continue;
         const int row0 = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M;
         const int vt0 = un.chunk * p.tiles_per_chunk;
@@ -278,9 +306,9 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
       constexpr uint32_t idesc = make_idesc_bf16(Cfg::UMMA_M, BLOCK_N);
       int stage = 0; uint32_t phase = 0;
       uint32_t tile = 0;
-      for (int gu = gu0; gu < p.num_gang_units; gu += p.num_gangs) {
+      for (int gu = gc.gu0; gu < gc.gu_end; gu += gc.gu_step) {
         Unit un;
-        if (!decode_gang_unit(p, gu, member, un)) continue;
+        if (!decode_gang_unit(p, gc, gu, un)) continue;
         const int vt0 = un.chunk * p.tiles_per_chunk;
         const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
         for (int vt = vt0; vt < vt1; ++vt, ++tile) {
@@ -313,9 +341,9 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
     const uint32_t tempty_remote = (CG == 2) ? mapa(tempty_bar(0), 0) : tempty_bar(0);
     RowState<CAP> st;
     uint32_t tile = 0;
-    for (int gu = gu0; gu < p.num_gang_units; gu += p.num_gangs) {
+    for (int gu = gc.gu0; gu < gc.gu_end; gu += gc.gu_step) {
       Unit un;
-      if (!decode_gang_unit(p, gu, member, un)) continue;
+      if (!decode_gang_unit(p, gc, gu, un)) continue;
       const int row = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M + row_in_tile;
       const int vt0 = un.chunk * p.tiles_per_chunk;
       const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);

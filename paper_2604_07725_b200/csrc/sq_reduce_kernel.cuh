@@ -7,7 +7,7 @@
 //
 // HBM-bound (12 B/token).  Three launches:
 //   tile_scan : exclusive scan of ceil(L_b / TILE) -> tile_base[B+1]           (1 CTA)
-//   tile_part : one CTA per (sequence, tile of TILE tokens): coalesced partial sums and the minimum
+//   tile_part : one CTA per (sequence, tile of TILE = 8192 tokens): coalesced partial sums and the minimum
 //               window sum among the windows that START in the tile.  The window sums are
 //               S(j) = S(j0) + sum_{i=j0+1..j} (c[i+w'-1] - c[i-1]): S(j0) is summed directly and the
 //               differences are scanned per warp, so fp32 error does not grow with the sequence.
@@ -19,7 +19,14 @@
 
 namespace sq {
 
-constexpr int RED_TILE = 4096;        // tokens per CTA
+#ifndef SQ_RED_TILE
+#define SQ_RED_TILE 8192
+#endif
+#ifndef SQ_RED_UNROLL
+#define SQ_RED_UNROLL 8
+#endif
+constexpr int RED_TILE = SQ_RED_TILE;   // tokens per CTA
+constexpr int RED_UNROLL = SQ_RED_UNROLL;   // independent loads per array in flight per thread
 constexpr int RED_THREADS = 256;
 constexpr int RED_WARPS = RED_THREADS / 32;
 constexpr int RED_PER_WARP = RED_TILE / RED_WARPS;   // 512 window starts per warp
@@ -33,6 +40,7 @@ struct ReduceParams {
   const int32_t* targets;     // may be null: all valid
   const int32_t* cu;
   int* tile_base;             // [B+1]
+  int* tile_seq;              // [tiles] sequence that owns each tile (written by tile_scan)
   float4* part_sum;           // [tiles] (sum_lp, n_valid, sum_ent, sum_conf)
   float* part_min;            // [tiles] min window SUM among windows starting in the tile (+inf if none)
   float* out_lp; float* out_ent; float* out_conf; float* out_min;
@@ -70,7 +78,10 @@ __global__ void __launch_bounds__(1024) sq_reduce_tile_scan_kernel(const ReduceP
     __syncthreads();
     const int wbase = (threadIdx.x >> 5) ? warp_tot[(threadIdx.x >> 5) - 1] : 0;
     const int incl = carry_s + wbase + x;
-    if (b < p.B) p.tile_base[b + 1] = incl;
+    if (b < p.B) {
+      p.tile_base[b + 1] = incl;
+      for (int i = incl - n; i < incl; ++i) p.tile_seq[i] = b;   // n = ceil(L / 4096): a handful per sequence
+    }
     __syncthreads();
     if (threadIdx.x == 1023) carry_s = incl;
     __syncthreads();
@@ -88,28 +99,38 @@ __global__ void __launch_bounds__(RED_THREADS) sq_reduce_tile_part_kernel(const 
   const int tile = blockIdx.x;
   const int total_tiles = p.tile_base[p.B];
   if (tile >= total_tiles) return;
-  // sequence that owns this tile: largest b with tile_base[b] <= tile
-  int lo = 0, hi = p.B;
-  while (hi - lo > 1) {
-    const int mid = (lo + hi) >> 1;
-    if (p.tile_base[mid] <= tile) lo = mid; else hi = mid;
-  }
-  const int b = lo;
+  const int b = p.tile_seq[tile];
   const long long seq0 = p.cu[b];
   const int L = p.cu[b + 1] - p.cu[b];
   const int t_in = (tile - p.tile_base[b]) * RED_TILE;       // first token of the tile, in the sequence
   const int n_tok = min(RED_TILE, L - t_in);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
-  // ---- partial sums over the tile's tokens (coalesced)
+  // ---- partial sums over the tile's tokens (coalesced; 4 independent loads per array in flight)
   float a_lp = 0.f, a_n = 0.f, a_en = 0.f, a_cf = 0.f;
-  for (int i = threadIdx.x; i < n_tok; i += RED_THREADS) {
-    const long long t = seq0 + t_in + i;
-    bool valid = true;
-    if (p.targets) { const int tg = p.targets[t]; valid = (tg >= 0) && (tg < p.V); }
-    if (valid) { a_lp += p.lp[t]; a_n += 1.f; }
-    a_en += p.ent[t];
-    a_cf += p.conf[t];
+  {
+    const long long t0 = seq0 + t_in;
+    const float* lp = p.lp + t0; const float* en = p.ent + t0; const float* cf = p.conf + t0;
+    const int32_t* tg = p.targets ? p.targets + t0 : nullptr;
+    for (int i0 = 0; i0 < n_tok; i0 += RED_UNROLL * RED_THREADS) {
+      float vl[RED_UNROLL], ve[RED_UNROLL], vc[RED_UNROLL]; int vt[RED_UNROLL];
+#pragma unroll
+      for (int q = 0; q < RED_UNROLL; ++q) {
+        const int i = i0 + q * RED_THREADS + threadIdx.x;
+        const bool in = i < n_tok;
+        vl[q] = in ? __ldg(lp + i) : 0.f;
+        ve[q] = in ? __ldg(en + i) : 0.f;
+        vc[q] = in ? __ldg(cf + i) : 0.f;
+        vt[q] = in ? (tg ? __ldg(tg + i) : 0) : -1;
+      }
+#pragma unroll
+      for (int q = 0; q < RED_UNROLL; ++q) {
+        const bool valid = (vt[q] >= 0) && (vt[q] < p.V || !tg);
+        if (valid) { a_lp += vl[q]; a_n += 1.f; }
+        a_en += ve[q];
+        a_cf += vc[q];
+      }
+    }
   }
 
   // ---- sliding windows that start in this tile
@@ -128,13 +149,21 @@ __global__ void __launch_bounds__(RED_THREADS) sq_reduce_tile_part_kernel(const 
   float run = 0.f;                 // S(j) - S(first start of this warp's strip), inclusive
   float wmin = CUDART_INF_F;       // min over the strip of that relative sum
   const int s_begin = j0 + warp * RED_PER_WARP;
-  for (int r = 0; r < RED_PER_WARP; r += 32) {
-    const int j = s_begin + r + lane;
-    float dlt = 0.f;
-    const bool in = (j < j1);
+  float dl[RED_PER_WARP / 32];
+#pragma unroll
+  for (int r = 0; r < RED_PER_WARP / 32; ++r) {   // all difference loads first: 32 loads in flight per thread
+    const int j = s_begin + r * 32 + lane;
     // strip-relative: the first start of the strip contributes 0; later starts add c[j+w-1] - c[j-1]
-    if (in && j > s_begin) dlt = c[j + w - 1] - c[j - 1];
-    float x = dlt;
+    const bool ld = (j < j1) && (j > s_begin);
+    const float a = ld ? __ldg(c + j + w - 1) : 0.f;
+    const float bq = ld ? __ldg(c + j - 1) : 0.f;
+    dl[r] = a - bq;
+  }
+#pragma unroll
+  for (int r = 0; r < RED_PER_WARP / 32; ++r) {
+    const int j = s_begin + r * 32 + lane;
+    const bool in = (j < j1);
+    float x = dl[r];
 #pragma unroll
     for (int off = 1; off < 32; off <<= 1) {
       const float y = __shfl_up_sync(0xffffffffu, x, off);

@@ -34,7 +34,7 @@ struct sq_score_ctx {
   // per-token scratch (used when the caller passes NULL per-token outputs)
   float* tok_lse = nullptr; float* tok_lp = nullptr; float* tok_ent = nullptr; float* tok_conf = nullptr;
   // kernel 2 workspace
-  int* tile_base = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
+  int* tile_base = nullptr; int* tile_seq = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
   // staging for sq_score_run_host
   void* h_stage = nullptr; int32_t* tgt_stage = nullptr; int32_t* cu_stage = nullptr; float* seq_stage = nullptr;
   // driver entry point for tensor-map encoding
@@ -90,35 +90,50 @@ static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, 
   G = std::max(1, std::min(G, std::min(std::max(1, pl->m_tiles), pl->num_clusters)));
   pl->group_m = G;
   pl->num_gangs = pl->num_clusters / G;
-  const int groups = (int)cdiv64(pl->m_tiles, G);
+  const int GB = pl->num_clusters - pl->num_gangs * G;   // clusters left over: one smaller gang B
+  pl->gang_b_size = GB;
+  const int M = pl->m_tiles;
   const int max_chunks = std::min(32, pl->num_vtiles);
-  int best_c = 1;
-  if (cfg->num_chunks > 0) {
-    best_c = std::min(cfg->num_chunks, max_chunks);
-  } else if (pl->m_tiles > 0) {
+  // cost of a plan = the slower gang class, in tile-times: rounds x (unit length + fill/drain)
+  auto eval = [&](int c, int m_b, double* cost_out) {
+    const int tpc = (int)cdiv64(pl->num_vtiles, c);
+    const int ce = (int)cdiv64(pl->num_vtiles, tpc);
+    const int64_t rounds_a = cdiv64(cdiv64(M - m_b, G) * ce, pl->num_gangs);
+    const int64_t rounds_b = m_b > 0 ? cdiv64(m_b, GB) * ce : 0;
+    *cost_out = (double)std::max(rounds_a, rounds_b) * (tpc + 0.75);   // 0.75 tile-times of fill/drain per unit
+    return ce;
+  };
+  int best_c = 1, best_mb = 0;
+  if (M > 0) {
     // The gangs in flight work on ceil(num_gangs / C) different token groups, i.e. about
     // num_clusters / C token strips of rows_per_tile x d bf16 are re-read from L2 for every vocab
     // tile.  Keep that hot set under ~40 MB of the 126 MB L2 (measured: beyond ~50 MB the strips
-    // start to miss and HBM traffic and power go up), then minimise
-    // (rounds of gang-units per gang) x (unit length + fill/drain); ties -> fewer chunks.
+    // start to miss and HBM traffic and power go up), then minimise the cost above over the number
+    // of chunks and the number of token tiles handed to gang B; ties -> fewer chunks, smaller B.
     const double strip_mb = (double)pl->rows_per_tile * cfg->d * 2.0 / 1e6;
     const int c_l2 = (int)std::ceil(pl->num_gangs * G * strip_mb / 40.0);
-    const int c_hi = std::min(max_chunks, (int64_t)groups * 16 < pl->num_gangs ? 32 : 16);
-    const int c_lo = std::max(1, std::min(c_hi, c_l2));
+    int c_hi = std::min(max_chunks, cdiv64(M, G) * 16 < pl->num_gangs ? 32 : 16);
+    int c_lo = std::max(1, std::min(c_hi, c_l2));
+    if (cfg->num_chunks > 0) c_lo = c_hi = std::min(cfg->num_chunks, max_chunks);
+    const int mb_hi = GB > 0 ? std::min(M - 1, (int)(3.0 * M * GB / pl->num_clusters) + GB) : 0;
     double best_cost = 1e300;
     for (int c = c_lo; c <= c_hi; ++c) {
-      const int tpc = (int)cdiv64(pl->num_vtiles, c);
-      const int ce = (int)cdiv64(pl->num_vtiles, tpc);
-      if (ce < c_lo && c < c_hi) continue;   // rounding merged chunks below the L2 bound
-      const int64_t rounds = cdiv64((int64_t)groups * ce, pl->num_gangs);
-      const double cost = (double)rounds * (tpc + 0.75);   // 0.75 tile-times of fill/drain per unit
-      if (cost < best_cost - 1e-9) { best_cost = cost; best_c = c; }
+      for (int m_b = 0; m_b <= mb_hi; ++m_b) {
+        double cost;
+        const int ce = eval(c, m_b, &cost);
+        if (ce < c_lo && c < c_hi) break;   // rounding merged chunks below the L2 bound
+        if (cost < best_cost - 1e-9) { best_cost = cost; best_c = c; best_mb = m_b; }
+      }
     }
+  } else if (cfg->num_chunks > 0) {
+    best_c = std::min(cfg->num_chunks, max_chunks);
   }
   pl->tiles_per_chunk = (int)cdiv64(pl->num_vtiles, best_c);
   pl->num_chunks = (int)cdiv64(pl->num_vtiles, pl->tiles_per_chunk);
   pl->num_units = pl->m_tiles * pl->num_chunks;
-  pl->num_gang_units = groups * pl->num_chunks;
+  pl->m_split = M - best_mb;
+  pl->num_gang_units = (int)cdiv64(pl->m_split, G) * pl->num_chunks;
+  pl->num_gang_units_b = best_mb > 0 ? (int)cdiv64(best_mb, GB) * pl->num_chunks : 0;
   return SQ_OK;
 }
 
@@ -156,7 +171,7 @@ extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
   if (!ctx) return SQ_OK;
   cudaSetDevice(ctx->cfg.device);
   void* bufs[] = {ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
-                  ctx->tok_lse, ctx->tok_lp, ctx->tok_ent, ctx->tok_conf, ctx->tile_base, ctx->red_sum,
+                  ctx->tok_lse, ctx->tok_lp, ctx->tok_ent, ctx->tok_conf, ctx->tile_base, ctx->tile_seq, ctx->red_sum,
                   ctx->red_min, ctx->h_stage, ctx->tgt_stage, ctx->cu_stage, ctx->seq_stage};
   int rc = SQ_OK;
   for (void* b : bufs)
@@ -244,6 +259,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   A(ws_alloc(ctx, &ctx->tok_conf, T));
   A(ws_alloc(ctx, &ctx->tile_base, (int64_t)cfg->max_seqs + 1));
   A(ws_alloc(ctx, &ctx->red_sum, ctx->red_tiles_max));
+  A(ws_alloc(ctx, &ctx->tile_seq, ctx->red_tiles_max));
   A(ws_alloc(ctx, &ctx->red_min, ctx->red_tiles_max));
   A(ws_alloc(ctx, &ctx->seq_stage, 4 * (int64_t)cfg->max_seqs));
   if (rc != SQ_OK) {
@@ -290,7 +306,8 @@ static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int6
 template <int CG, int CAP>
 static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CUtensorMap& th, const CUtensorMap& tw,
                                 const sq::FusedParams& fp, cudaStream_t st) {
-  const int clusters = pl.num_gangs * pl.group_m;   // every launched cluster belongs to a gang
+  // every launched cluster belongs to a gang; gang B is launched only if it was given token tiles
+  const int clusters = pl.num_gangs * pl.group_m + (pl.num_gang_units_b > 0 ? pl.gang_b_size : 0);
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3((unsigned)(clusters * CG));
   lc.blockDim = dim3(sq::NUM_THREADS);
@@ -332,7 +349,7 @@ extern "C" int sq_score_reduce(sq_score_ctx* ctx, const float* target_logprob, c
   sq::ReduceParams rp = {};
   rp.T = num_tokens; rp.B = num_seqs; rp.V = ctx->cfg.vocab; rp.window = window;
   rp.lp = target_logprob; rp.ent = entropy; rp.conf = conf; rp.targets = targets; rp.cu = cu_seqlens;
-  rp.tile_base = ctx->tile_base; rp.part_sum = ctx->red_sum; rp.part_min = ctx->red_min;
+  rp.tile_base = ctx->tile_base; rp.tile_seq = ctx->tile_seq; rp.part_sum = ctx->red_sum; rp.part_min = ctx->red_min;
   rp.out_lp = seq_mean_logprob; rp.out_ent = seq_mean_entropy; rp.out_conf = seq_mean_conf; rp.out_min = seq_min_window_conf;
   return launch_reduce(ctx, rp, static_cast<cudaStream_t>(stream));
 }
@@ -381,6 +398,7 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
     fp.num_k_blocks = pl.num_k_blocks; fp.num_vtiles = pl.num_vtiles; fp.tiles_per_chunk = pl.tiles_per_chunk;
     fp.num_chunks = pl.num_chunks; fp.m_tiles = pl.m_tiles; fp.group_m = pl.group_m;
     fp.num_gangs = pl.num_gangs; fp.num_gang_units = pl.num_gang_units; fp.gang_ctr = ctx->gang_ctr;
+    fp.m_split = pl.m_split; fp.gang_b_size = pl.gang_b_size; fp.num_gang_units_b = pl.num_gang_units_b;
     SQ_CUDA(ctx, cudaMemsetAsync(ctx->gang_ctr, 0, 256 * sizeof(unsigned int), st));
     fp.targets = targets;
     fp.part_m = ctx->part_m; fp.part_s = ctx->part_s; fp.part_u = ctx->part_u;
@@ -418,7 +436,7 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
     sq::ReduceParams rp = {};
     rp.T = T; rp.B = B; rp.V = V; rp.window = window;
     rp.lp = lp; rp.ent = ent; rp.conf = conf; rp.targets = targets; rp.cu = cu_seqlens;
-    rp.tile_base = ctx->tile_base; rp.part_sum = ctx->red_sum; rp.part_min = ctx->red_min;
+    rp.tile_base = ctx->tile_base; rp.tile_seq = ctx->tile_seq; rp.part_sum = ctx->red_sum; rp.part_min = ctx->red_min;
     rp.out_lp = o->seq_mean_logprob; rp.out_ent = o->seq_mean_entropy; rp.out_conf = o->seq_mean_conf;
     rp.out_min = o->seq_min_window_conf;
     const int rc = launch_reduce(ctx, rp, st);

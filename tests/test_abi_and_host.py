@@ -88,29 +88,44 @@ def test_plan_covers_every_tile_exactly_once(name, cg):
     assert p["num_units"] == p["m_tiles"] * p["num_chunks"]
     assert p["num_clusters"] == 148 // cg
     assert p["topk_cap"] >= k
-    # replay the kernel's gang-unit decode: every (m_tile, chunk) pair is visited exactly once
+    # replay the kernel's gang-unit decode (class-A gangs + the smaller gang B): every
+    # (m_tile, chunk) pair is visited exactly once
     G, C, M = p["group_m"], p["num_chunks"], p["m_tiles"]
     assert 1 <= G <= max(1, min(M, p["num_clusters"]))
     assert p["num_gangs"] == p["num_clusters"] // G and p["num_gangs"] >= 1
-    assert p["num_gang_units"] == -(-M // G) * C
+    assert p["gang_b_size"] == p["num_clusters"] - p["num_gangs"] * G
+    assert 0 <= p["m_split"] <= M
+    assert p["num_gang_units"] == -(-p["m_split"] // G) * C
     seen = set()
     for gang in range(p["num_gangs"]):
         for gu in range(gang, p["num_gang_units"], p["num_gangs"]):
             g, c = divmod(gu, C)
             for member in range(G):
                 m = g * G + member
+                if m < p["m_split"]:
+                    assert (m, c) not in seen
+                    seen.add((m, c))
+    if p["m_split"] < M:
+        GB = p["gang_b_size"]
+        assert GB >= 1 and p["num_gang_units_b"] == -(-(M - p["m_split"]) // GB) * C
+        for gu in range(p["num_gang_units_b"]):
+            g, c = divmod(gu, C)
+            for member in range(GB):
+                m = p["m_split"] + g * GB + member
                 if m < M:
                     assert (m, c) not in seen
                     seen.add((m, c))
+    else:
+        assert p["num_gang_units_b"] == 0
     assert len(seen) == p["num_units"]
 
 
 def test_plan_wave_efficiency_on_target_config():
     d, V, T, k = CONFIG_SHAPES["qwen3_8b"]
     p = sq.plan(d, V, T, k, num_sms=148)
-    rounds = -(-p["num_gang_units"] // p["num_gangs"])
+    rounds = max(-(-p["num_gang_units"] // p["num_gangs"]), p["num_gang_units_b"])
     ideal = p["m_tiles"] * p["num_vtiles"] / p["num_clusters"]
-    assert ideal / (rounds * p["tiles_per_chunk"]) > 0.90    # < 10 % lost to gang/wave quantisation
+    assert ideal / (rounds * p["tiles_per_chunk"]) > 0.95    # < 5 % lost to gang/wave quantisation
 
 
 def test_plan_forced_chunks_and_edge_sizes():
