@@ -290,6 +290,29 @@ def run_ours(args):
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
+    if world == 1 and not args.no_reduce_standalone:
+        # kernel 2 alone on an input large enough for HBM bandwidth to mean something
+        r = workloads.reduction_inputs(4096, 1024, 16384, seed=2001)
+        eng2 = sq.SqScore(d, V, max_tokens=r["T"], max_seqs=r["B"], max_k=wl.k, device=local, reduce_only=True)
+        r_lp, r_en, r_cf, r_cu = (r[n].to(dev) for n in ("target_logprob", "entropy", "conf", "cu_seqlens"))
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                eng2.reduce(r_lp, r_en, r_cf, r_cu, wl.window, stream=stream)
+            r0 = torch.cuda.Event(enable_timing=True); r1 = torch.cuda.Event(enable_timing=True)
+            r0.record(stream)
+            for _ in range(20):
+                eng2.reduce(r_lp, r_en, r_cf, r_cu, wl.window, stream=stream)
+            r1.record(stream)
+            stream.synchronize()
+        r_ms = r0.elapsed_time(r1) / 20
+        r_bytes = 12.0 * r["T"] + 16.0 * r["B"]
+        line["reduce_standalone"] = {"bound": "hbm", "achieved": r_bytes / (r_ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                     "unit": "GB/s", "frac": r_bytes / (r_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                                     "ms": r_ms, "tokens": r["T"], "seqs": r["B"], "window": wl.window,
+                                     "algorithmic_bytes": r_bytes,
+                                     "note": "3 launches (tile_scan, tile_part, seq_final); 12 B/token read + 16 B/sequence written"}
+        eng2.close()
+        del r_lp, r_en, r_cf
     if args.matmul_ceiling:
         # context only: cuBLAS on the same (T, V, d) in row chunks, logits materialised chunk by chunk
         rows = 8192
@@ -311,6 +334,26 @@ def run_ours(args):
         line["context_cublas_matmul"] = {"ms_per_pass": mm_ms, "tflops": flops / (mm_ms * 1e-3) / 1e12,
                                          "note": "torch.matmul bf16 over the same T,V,d in 8192-row chunks; not part of the path"}
         del buf
+    if args.unfused_baseline:
+        # context only: what fusion buys -- the same outputs from library ops with the logits materialised
+        rows = 4096
+        Wt = W.t()
+        def unfused_pass():
+            for r0 in range(0, T, rows):
+                r1 = min(T, r0 + rows)
+                z = torch.matmul(H[r0:r1], Wt).float()
+                lsm = torch.log_softmax(z, dim=1)
+                tv, ti = torch.topk(lsm, wl.k, dim=1)
+                ent = -(lsm.exp() * lsm).sum(1)
+                tlp = lsm.gather(1, tg[r0:r1].long().unsqueeze(1))
+                del z, lsm
+        unfused_pass(); torch.cuda.synchronize()
+        u0 = torch.cuda.Event(enable_timing=True); u1 = torch.cuda.Event(enable_timing=True)
+        u0.record(); unfused_pass(); unfused_pass(); u1.record(); torch.cuda.synchronize()
+        u_ms = u0.elapsed_time(u1) / 2
+        line["context_unfused_torch"] = {"ms_per_pass": u_ms, "tokens_per_s": T / (u_ms * 1e-3),
+                                         "note": "torch matmul + log_softmax + topk + entropy + gather in 4096-row chunks "
+                                                 "(logits materialised); per-token outputs only; not part of the path"}
     if world == 1 and not args.no_cpu_baseline:
         tps, sec, rows, threads = time_oracle(inp, budget_s=args.oracle_seconds)
         line["cpu_baseline"] = {"value": tps, "unit": UNIT, "cores": threads, "kind": "oracle",
@@ -331,9 +374,11 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--oracle-seconds", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-reduce-standalone", action="store_true")
     ap.add_argument("--per-step-kernel-times", action="store_true",
                     help="read kernel 1's duration after every step (adds a host sync per step)")
     ap.add_argument("--matmul-ceiling", action="store_true", help="also time torch.matmul on the same shapes (context)")
+    ap.add_argument("--unfused-baseline", action="store_true", help="also time an unfused torch pipeline (context)")
     ap.add_argument("--cta-group", type=int, default=0)
     ap.add_argument("--num-chunks", type=int, default=0)
     ap.add_argument("--group-m", type=int, default=0)

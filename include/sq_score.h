@@ -48,6 +48,9 @@ extern "C" {
 
 #define SQ_MAX_K             32   /* largest K_l the streaming top-k supports                     */
 
+#define SQ_FLAG_REDUCE_ONLY   1   /* ctx serves sq_score_reduce only: no kernel-1 workspace is
+                                     allocated and sq_score_run / run_host return INVALID_ARG    */
+
 typedef struct sq_score_ctx sq_score_ctx;   /* opaque */
 
 /* Fixed per context (one scorer model = one LM head shape). */
@@ -61,6 +64,7 @@ typedef struct {
   int     cta_group;    /* 0 = default (2: CTA pairs, UMMA M=256); 1 = single-CTA UMMA (M=128)    */
   int     num_chunks;   /* 0 = planner's choice; >0 forces the number of vocab chunks per row     */
   int     group_m;      /* 0 = default (8): gang size = token tiles that share one W stream       */
+  int     flags;        /* SQ_FLAG_*                                                              */
 } sq_score_config;
 
 /* Output pointers of one run.  Per-token pointers may be NULL (= not wanted; the ctx keeps the

@@ -8,13 +8,14 @@ from typing import Dict, List, Optional, Sequence
 from . import build as _build
 
 SQ_MAX_K = 32
+FLAG_REDUCE_ONLY = 1
 ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOMEM = -1, -2, -3, -4
 
 
 class sq_score_config(C.Structure):
     _fields_ = [("device", C.c_int), ("d", C.c_int), ("vocab", C.c_int), ("max_tokens", C.c_int64),
                 ("max_seqs", C.c_int), ("max_k", C.c_int), ("cta_group", C.c_int), ("num_chunks", C.c_int),
-                ("group_m", C.c_int)]
+                ("group_m", C.c_int), ("flags", C.c_int)]
 
 
 class sq_score_outputs(C.Structure):
@@ -88,7 +89,7 @@ def version() -> int:
 def plan(d: int, vocab: int, num_tokens: int, k: int, num_sms: int = 0, cta_group: int = 0,
          num_chunks: int = 0, group_m: int = 0) -> Dict[str, int]:
     """sq_score_plan: host-only work decomposition (no GPU needed)."""
-    cfg = sq_score_config(0, d, vocab, max(1, num_tokens), 1, max(1, min(k, SQ_MAX_K)), cta_group, num_chunks, group_m)
+    cfg = sq_score_config(0, d, vocab, max(1, num_tokens), 1, max(1, min(k, SQ_MAX_K)), cta_group, num_chunks, group_m, 0)
     out = sq_score_plan_t()
     rc = lib().sq_score_plan(C.byref(cfg), num_tokens, k, num_sms, C.byref(out))
     if rc != 0:
@@ -104,9 +105,10 @@ class SqScore:
     """sq_score_create / sq_score_run / sq_score_destroy on torch tensors (device memory + streams)."""
 
     def __init__(self, d: int, vocab: int, max_tokens: int, max_seqs: int, max_k: int = 20, device: int = 0,
-                 cta_group: int = 0, num_chunks: int = 0, group_m: int = 0):
+                 cta_group: int = 0, num_chunks: int = 0, group_m: int = 0, reduce_only: bool = False):
         self._L = lib()
-        self.cfg = sq_score_config(device, d, vocab, max_tokens, max_seqs, max_k, cta_group, num_chunks, group_m)
+        self.cfg = sq_score_config(device, d, vocab, max_tokens, max_seqs, max_k, cta_group, num_chunks, group_m,
+                                   FLAG_REDUCE_ONLY if reduce_only else 0)
         h = C.c_void_p()
         rc = self._L.sq_score_create(C.byref(self.cfg), C.byref(h))
         if rc != 0:

@@ -203,7 +203,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
     return set_err(nullptr, SQ_ERR_INVALID_ARG, "d, vocab, max_tokens and max_seqs must be positive");
   if (cfg->max_k < 1 || cfg->max_k > SQ_MAX_K)
     return set_err(nullptr, SQ_ERR_INVALID_ARG, "max_k must be in 1..%d", SQ_MAX_K);
-  if (cfg->cta_group < 0 || cfg->cta_group > 2 || cfg->num_chunks < 0 || cfg->group_m < 0)
+  if (cfg->cta_group < 0 || cfg->cta_group > 2 || cfg->num_chunks < 0 || cfg->group_m < 0 || (cfg->flags & ~SQ_FLAG_REDUCE_ONLY))
     return set_err(nullptr, SQ_ERR_INVALID_ARG, "cta_group must be 0, 1 or 2; num_chunks, group_m >= 0");
   if (cfg->d % 8 != 0)
     return set_err(nullptr, SQ_ERR_UNSUPPORTED, "d = %d is not a multiple of 8 (TMA needs 16-byte row strides)", cfg->d);
@@ -239,7 +239,8 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
     return SQ_ERR_CUDA;
   }
 
-  const int64_t rows = ws_rows_for(*cfg);
+  const bool reduce_only = (cfg->flags & SQ_FLAG_REDUCE_ONLY) != 0;
+  const int64_t rows = reduce_only ? 1 : ws_rows_for(*cfg);
   const int64_t T = cfg->max_tokens;
   ctx->red_tiles_max = cdiv64(T, sq::RED_TILE) + cfg->max_seqs;
   int rc = SQ_OK;
@@ -251,12 +252,12 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   A(ws_alloc(ctx, &ctx->part_cu, rows));
   A(ws_alloc(ctx, &ctx->part_topv, rows * ctx->cap_max));
   A(ws_alloc(ctx, &ctx->part_topi, rows * ctx->cap_max));
-  A(ws_alloc(ctx, &ctx->zt, T));
+  A(ws_alloc(ctx, &ctx->zt, reduce_only ? 1 : T));
   A(ws_alloc(ctx, &ctx->gang_ctr, 256));
-  A(ws_alloc(ctx, &ctx->tok_lse, T));
-  A(ws_alloc(ctx, &ctx->tok_lp, T));
-  A(ws_alloc(ctx, &ctx->tok_ent, T));
-  A(ws_alloc(ctx, &ctx->tok_conf, T));
+  A(ws_alloc(ctx, &ctx->tok_lse, reduce_only ? 1 : T));
+  A(ws_alloc(ctx, &ctx->tok_lp, reduce_only ? 1 : T));
+  A(ws_alloc(ctx, &ctx->tok_ent, reduce_only ? 1 : T));
+  A(ws_alloc(ctx, &ctx->tok_conf, reduce_only ? 1 : T));
   A(ws_alloc(ctx, &ctx->tile_base, (int64_t)cfg->max_seqs + 1));
   A(ws_alloc(ctx, &ctx->red_sum, ctx->red_tiles_max));
   A(ws_alloc(ctx, &ctx->tile_seq, ctx->red_tiles_max));
@@ -359,6 +360,7 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
                             const sq_score_outputs* o, void* stream) {
   if (!ctx) return SQ_ERR_INVALID_ARG;
   if (!o) return set_err(ctx, SQ_ERR_INVALID_ARG, "outputs is null");
+  if (ctx->cfg.flags & SQ_FLAG_REDUCE_ONLY) return set_err(ctx, SQ_ERR_INVALID_ARG, "ctx was created with SQ_FLAG_REDUCE_ONLY");
   const int T = num_tokens, B = num_seqs, V = ctx->cfg.vocab, d = ctx->cfg.d;
   if (T < 0 || B < 0) return set_err(ctx, SQ_ERR_INVALID_ARG, "negative T or B");
   if (T > ctx->cfg.max_tokens || B > ctx->cfg.max_seqs)

@@ -54,9 +54,9 @@ def test_create_fails_loudly_without_gpu():
 def test_create_rejects_bad_config_before_touching_cuda():
     L = sq.lib()
     h = ctypes.c_void_p()
-    bad = [dict(d=0), dict(vocab=0), dict(max_tokens=0), dict(max_seqs=0), dict(max_k=0), dict(max_k=33), dict(cta_group=3)]
+    bad = [dict(d=0), dict(vocab=0), dict(max_tokens=0), dict(max_seqs=0), dict(max_k=0), dict(max_k=33), dict(cta_group=3), dict(flags=2)]
     for kw in bad:
-        base = dict(device=0, d=64, vocab=1024, max_tokens=256, max_seqs=4, max_k=5, cta_group=0, num_chunks=0, group_m=0)
+        base = dict(device=0, d=64, vocab=1024, max_tokens=256, max_seqs=4, max_k=5, cta_group=0, num_chunks=0, group_m=0, flags=0)
         base.update(kw)
         cfg = binding.sq_score_config(**base)
         assert L.sq_score_create(ctypes.byref(cfg), ctypes.byref(h)) == sq.ERR_INVALID_ARG, kw

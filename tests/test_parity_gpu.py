@@ -320,7 +320,7 @@ def test_reduce_kernel_alone(window):
     cu = torch.tensor(np.concatenate([[0], np.cumsum(lens)]), dtype=torch.int32)
     lp = -(torch.rand(T, generator=g) * 12); en = torch.rand(T, generator=g) * 11; cf = 3 + torch.rand(T, generator=g) * 12
     cf[30000:30040] = 0.5                      # a dip the minimum window must find
-    eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5)
+    eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
     dev = torch.device("cuda:0")
     out = eng.reduce(lp.to(dev), en.to(dev), cf.to(dev), cu.to(dev), window)
     torch.cuda.synchronize()
@@ -332,7 +332,7 @@ def test_reduce_kernel_alone(window):
 def test_reduce_many_sequences():
     sq = _sq()
     r = workloads.reduction_inputs(3000, 1, 3000, seed=5)
-    eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5)
+    eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True)
     dev = torch.device("cuda:0")
     out = eng.reduce(r["target_logprob"].to(dev), r["entropy"].to(dev), r["conf"].to(dev), r["cu_seqlens"].to(dev), 256)
     torch.cuda.synchronize()
