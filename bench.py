@@ -3,7 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl ours|reference]
 
-A step is one pass of the whole hot path (kernel 1 fused GEMM+statistics, finalize/merge, kernel 2)
+A step is one pass of the whole hot path (kernel 1 fused GEMM+statistics, finalize/merge, kernel 2: 5 launches)
 over one synthetic packed batch.  At N=1 the workload is BASELINE.json configs[2] (`qwen3_8b`, the
 config the metric's 60 % target is quoted on).  With N>1 (torchrun) every rank scores its own
 batch of the same shape (sequences shard across GPUs, W replicated, no data-path collective):

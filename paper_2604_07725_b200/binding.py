@@ -44,8 +44,8 @@ def lib() -> C.CDLL:
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.LIB
-    if _build.is_stale():
+    path = os.environ.get("SQ_SCORE_LIB") or _build.LIB   # SQ_SCORE_LIB: load another build of the same ABI (kernel A/B tests)
+    if path == _build.LIB and _build.is_stale():
         try:
             path = _build.build()
         except Exception:

@@ -29,7 +29,10 @@ template <int CG> struct FusedCfg {
   static constexpr int B_ROWS = BLOCK_N / CG;                           // W rows this CTA stages
   static constexpr int B_BYTES = B_ROWS * BLOCK_K * 2;                  // 32 KB (CG=1) / 16 KB (CG=2)
   static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
-  static constexpr int STAGES = (CG == 1) ? 4 : 6;
+#ifndef SQ_STAGES_PAIR
+#define SQ_STAGES_PAIR 6
+#endif
+  static constexpr int STAGES = (CG == 1) ? 4 : SQ_STAGES_PAIR;
   static constexpr int BAR_BYTES = 256;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;  // +1024: manual alignment
   static constexpr int UMMA_M = BLOCK_M * CG;

@@ -325,11 +325,29 @@ static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CU
 
 static int launch_reduce(sq_score_ctx* ctx, const sq::ReduceParams& rp, cudaStream_t st) {
   if (rp.B <= 0) return SQ_OK;
-  const int64_t tiles = cdiv64(rp.T, sq::RED_TILE) + rp.B;
+  const int64_t tiles = cdiv64(rp.T, sq::RED_TILE) + rp.B;   // upper bound on sum_b ceil(L_b / RED_TILE)
   sq::sq_reduce_tile_scan_kernel<<<1, 1024, 0, st>>>(rp);
-  if (rp.T > 0) sq::sq_reduce_tile_part_kernel<<<(unsigned)tiles, sq::RED_THREADS, 0, st>>>(rp);
-  sq::sq_reduce_seq_final_kernel<<<(unsigned)cdiv64(rp.B, 4), 128, 0, st>>>(rp);
-  ctx->launches += (rp.T > 0) ? 3 : 2;
+  ctx->launches += 1;
+  if (rp.T > 0) {
+    // programmatic dependent launch: tile_part's CTAs are scheduled while tile_scan drains and wait
+    // in cudaGridDependencySynchronize() for its results
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3((unsigned)tiles);
+    lc.blockDim = dim3(sq::RED_THREADS);
+    lc.dynamicSmemBytes = sq::RED_SMEM_BYTES;
+    lc.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    lc.attrs = at;
+    lc.numAttrs = 1;
+    SQ_CUDA(ctx, cudaLaunchKernelEx(&lc, sq::sq_reduce_tile_part_kernel, rp));
+    lc.gridDim = dim3((unsigned)cdiv64(rp.B, 4));
+    lc.blockDim = dim3(128);
+    lc.dynamicSmemBytes = 0;
+    SQ_CUDA(ctx, cudaLaunchKernelEx(&lc, sq::sq_reduce_seq_final_kernel, rp));
+    ctx->launches += 2;
+  }
   SQ_CUDA(ctx, cudaGetLastError());
   return SQ_OK;
 }
