@@ -27,10 +27,12 @@ No function here is "parity unpinned".
 """
 from __future__ import annotations
 
+import math
+
 import numpy as np
 import torch
 
-ORACLE_VERSION = 1
+ORACLE_VERSION = 2
 
 
 def widen(x_bf16: torch.Tensor) -> torch.Tensor:
@@ -130,3 +132,95 @@ def score(H: torch.Tensor, W: torch.Tensor, targets, cu_seqlens, k: int, window:
                           tok["target_valid"])
     tok.update(seq)
     return tok
+
+
+# ------------------------------------------------------------------------------------------------
+# Next row: group fitness, per-problem percentile threshold, routing,
+# fitness-weighted selection probabilities
+# ------------------------------------------------------------------------------------------------
+def group_confidence(seq_conf, group_members) -> np.ndarray:
+    """GC(g) = (1/K) * sum_{tau in g} C(tau) -- Eq. 4 (right), PAPER.md:160.  `group_members` is
+    [G, K] indices into seq_conf; K = |g| (reading #12)."""
+    c = np.asarray(seq_conf, dtype=np.float64)
+    gm = np.asarray(group_members, dtype=np.int64)
+    return c[gm].sum(axis=1) / gm.shape[1]
+
+
+def percentile_threshold(values, p: float) -> float:
+    """theta = Percentile_p(values) -- Eq. 6.  The paper does not say how to
+    interpolate; reading #13: linear interpolation between order statistics at rank p/100*(n-1)
+    (NumPy's default).  Empty input -> NaN."""
+    v = np.sort(np.asarray(values, dtype=np.float64))
+    n = len(v)
+    if n == 0:
+        return float("nan")
+    pos = (p / 100.0) * (n - 1)
+    lo = int(math.floor(pos))
+    hi = min(lo + 1, n - 1)
+    return float(v[lo] + (pos - lo) * (v[hi] - v[lo]))
+
+
+def route(seq_conf, group_members, group_offsets, p: float, lite_mask=None) -> dict:
+    """Per problem q (groups [off[q], off[q+1])): F(g) = GC(g); theta_q over the non-lite groups
+    (Eq. 6); mu(g,q) = Model 1 if GC(g) > theta_q ("easy", strict) else Model 2 (Eq. 7).
+    Codes: 0 = B_lite (given by `lite_mask`; the consensus test itself is on answer strings and is
+    out of scope), 1 = Model 1, 2 = Model 2."""
+    gc = group_confidence(seq_conf, group_members)
+    off = np.asarray(group_offsets, dtype=np.int64)
+    G = len(gc)
+    lite = np.zeros(G, dtype=bool) if lite_mask is None else np.asarray(lite_mask, dtype=bool)
+    theta = np.full(len(off) - 1, np.nan)
+    code = np.zeros(G, dtype=np.int32)
+    for q in range(len(off) - 1):
+        idx = np.arange(off[q], off[q + 1])
+        live = idx[~lite[idx]]
+        theta[q] = percentile_threshold(gc[live], p)
+        for g in live:
+            code[g] = 1 if gc[g] > theta[q] else 2
+    return {"group_fitness": gc, "theta": theta, "route": code}
+
+
+def route_decisions_fp32(seq_conf_f32, group_members, group_offsets, p: float, lite_mask=None) -> np.ndarray:
+    """The routing decision taken in the kernel's precision (fp32, same operation order: members
+    summed left to right then divided by K; theta = v[lo] + frac * (v[hi] - v[lo]) with separate
+    roundings).  A floating-point comparison decides an integer here, so the parity test compares
+    the GPU's codes with this, and GC / theta with the fp64 definitions above."""
+    f = np.float32
+    c = np.asarray(seq_conf_f32, dtype=np.float32)
+    gm = np.asarray(group_members, dtype=np.int64)
+    K = gm.shape[1]
+    gc = np.zeros(gm.shape[0], dtype=np.float32)
+    for j in range(K):
+        gc = (gc + c[gm[:, j]]).astype(np.float32)
+    gc = (gc / f(K)).astype(np.float32)
+    off = np.asarray(group_offsets, dtype=np.int64)
+    lite = np.zeros(len(gc), dtype=bool) if lite_mask is None else np.asarray(lite_mask, dtype=bool)
+    code = np.zeros(len(gc), dtype=np.int32)
+    for q in range(len(off) - 1):
+        idx = np.arange(off[q], off[q + 1])
+        live = idx[~lite[idx]]
+        if len(live) == 0:
+            continue
+        v = np.sort(gc[live])
+        n = len(v)
+        pos = f(f(p) / f(100.0)) * f(n - 1)
+        lo = int(np.floor(pos))
+        hi = min(lo + 1, n - 1)
+        frac = f(pos - f(lo))
+        theta = f(v[lo] + f(frac * f(v[hi] - v[lo])))
+        code[live] = np.where(gc[live] > theta, 1, 2)
+    return code
+
+
+def selection_probabilities(fitness, pop_offsets, zeta: float) -> np.ndarray:
+    """Fitness-weighted selection: candidate i of problem q is drawn with probability
+    exp(f_i / zeta) / sum_j exp(f_j / zeta) over the problem's population."""
+    fv = np.asarray(fitness, dtype=np.float64)
+    off = np.asarray(pop_offsets, dtype=np.int64)
+    out = np.zeros_like(fv)
+    for q in range(len(off) - 1):
+        x = fv[off[q]:off[q + 1]] / zeta
+        if len(x):
+            e = np.exp(x - x.max())
+            out[off[q]:off[q + 1]] = e / e.sum()
+    return out
