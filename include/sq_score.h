@@ -145,6 +145,28 @@ int sq_score_reduce(sq_score_ctx *ctx, const float *target_logprob, const float 
                     float *seq_mean_logprob, float *seq_mean_entropy, float *seq_mean_conf,
                     float *seq_min_window_conf, void *stream);
 
+/* Group fitness and routing on the device, one problem per CTA:
+ *   group_fitness[g] = GC(g) = (1/K) * sum_{j<K} seq_conf[group_members[g*K+j]]   Eq. 4 right
+ *   theta[q] = Percentile_p of GC over problem q's non-lite groups                Eq. 6
+ *              (linear interpolation at rank p/100*(n-1); NaN when every group is lite)
+ *   route[g] = 0 if lite_mask[g], else 1 (Model 1) if GC(g) > theta[q], else 2 (Model 2)   Eq. 7
+ *   seq_conf       DEVICE float [num_seqs]      C(tau), e.g. seq_mean_conf of sq_score_run
+ *   group_members  DEVICE int32 [num_groups*K]  indices into seq_conf (trusted, must be in range)
+ *   group_offsets  DEVICE int32 [num_problems+1] groups of problem q are [off[q], off[q+1])
+ *   lite_mask      DEVICE uint8 [num_groups] or NULL (the consensus test is on answer strings, not here)
+ *   max_groups_per_problem  host-side bound on off[q+1]-off[q], <= 1024
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, UNSUPPORTED (more than 1024 groups in a problem), CUDA. */
+int sq_score_route(sq_score_ctx *ctx, const float *seq_conf, int num_seqs, const int32_t *group_members,
+                   const int32_t *group_offsets, int num_problems, int num_groups, int group_size,
+                   int max_groups_per_problem, const uint8_t *lite_mask, float percentile,
+                   float *group_fitness, float *theta, int32_t *route, void *stream);
+
+/* Fitness-weighted selection probabilities: within each problem's population
+ * [pop_offsets[q], pop_offsets[q+1]),  prob[i] = exp(fitness[i]/zeta) / sum_j exp(fitness[j]/zeta).
+ * All pointers DEVICE; zeta > 0.  The draws themselves stay with the caller.  Errors: INVALID_ARG, CUDA. */
+int sq_score_select_prob(sq_score_ctx *ctx, const float *fitness, const int32_t *pop_offsets,
+                         int num_problems, float zeta, float *prob, void *stream);
+
 /* Host-only: the work decomposition `sq_score_run` would use for T tokens and top-k `k` on a
  * device with `num_sms` SMs (pass 0 for the ctx-independent default of 148).  `cfg` supplies d,
  * vocab, cta_group, num_chunks, group_m.  Needs no GPU.  Errors: INVALID_ARG. */

@@ -62,6 +62,11 @@ def lib() -> C.CDLL:
     L.sq_score_run_host.restype = C.c_int
     L.sq_score_reduce.argtypes = [C.c_void_p] + [C.c_void_p] * 5 + [C.c_int64, C.c_int, C.c_int] + [C.c_void_p] * 5
     L.sq_score_reduce.restype = C.c_int
+    L.sq_score_route.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int,
+                                 C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.sq_score_route.restype = C.c_int
+    L.sq_score_select_prob.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_float, C.c_void_p, C.c_void_p]
+    L.sq_score_select_prob.restype = C.c_int
     L.sq_score_plan.argtypes = [C.POINTER(sq_score_config), C.c_int64, C.c_int, C.c_int, C.POINTER(sq_score_plan_t)]
     L.sq_score_plan.restype = C.c_int
     L.sq_score_set_profiling.argtypes = [C.c_void_p, C.c_int]
@@ -168,6 +173,34 @@ class SqScore:
                                             _ptr(out["seq_mean_conf"]), _ptr(out["seq_min_window_conf"]),
                                             self._stream(stream)))
         return out
+
+    def route(self, seq_conf, group_members, group_offsets, percentile: float, lite_mask=None,
+              max_groups_per_problem: Optional[int] = None, stream=None) -> dict:
+        """sq_score_route: GC(g), per-problem percentile threshold and routing codes (0 lite / 1 Model 1 / 2 Model 2).
+        `group_members` is an int32 [G, K] tensor."""
+        import torch
+        G, K = group_members.shape
+        Q = group_offsets.shape[0] - 1
+        dev = seq_conf.device
+        if max_groups_per_problem is None:
+            off = group_offsets.cpu()
+            max_groups_per_problem = int((off[1:] - off[:-1]).max()) if Q > 0 else 0
+        out = {"group_fitness": torch.empty(G, dtype=torch.float32, device=dev),
+               "theta": torch.empty(Q, dtype=torch.float32, device=dev),
+               "route": torch.empty(G, dtype=torch.int32, device=dev)}
+        self._check(self._L.sq_score_route(self._h, _ptr(seq_conf), seq_conf.shape[0], _ptr(group_members), _ptr(group_offsets),
+                                           Q, G, K, max_groups_per_problem, _ptr(lite_mask), float(percentile),
+                                           _ptr(out["group_fitness"]), _ptr(out["theta"]), _ptr(out["route"]),
+                                           self._stream(stream)))
+        return out
+
+    def select_prob(self, fitness, pop_offsets, zeta: float, stream=None):
+        """sq_score_select_prob: softmax(fitness / zeta) within each problem's population."""
+        import torch
+        prob = torch.empty_like(fitness)
+        self._check(self._L.sq_score_select_prob(self._h, _ptr(fitness), _ptr(pop_offsets), pop_offsets.shape[0] - 1,
+                                                 float(zeta), _ptr(prob), self._stream(stream)))
+        return prob
 
     def set_profiling(self, enable: bool):
         self._check(self._L.sq_score_set_profiling(self._h, 1 if enable else 0))

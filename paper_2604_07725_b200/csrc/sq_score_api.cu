@@ -16,6 +16,7 @@
 #include "sq_finalize_kernel.cuh"
 #include "sq_fused_kernel.cuh"
 #include "sq_reduce_kernel.cuh"
+#include "sq_route_kernel.cuh"
 
 #define SQ_VERSION 100
 
@@ -515,5 +516,45 @@ extern "C" int sq_score_run_host(sq_score_ctx* ctx, const void* H_host, const vo
   int rc = sq_score_run(ctx, ctx->h_stage, W_dev, ctx->tgt_stage, ctx->cu_stage, T, B, k, window, &o, stream);
   if (rc != SQ_OK) return rc;
   if (B > 0) SQ_CUDA(ctx, cudaMemcpyAsync(seq_out_host, ctx->seq_stage, (size_t)4 * B * sizeof(float), cudaMemcpyDeviceToHost, st));
+  return SQ_OK;
+}
+
+// ------------------------------------------------------------------------------------------ routing (8(f)-1)
+extern "C" int sq_score_route(sq_score_ctx* ctx, const float* seq_conf, int num_seqs, const int32_t* group_members,
+                              const int32_t* group_offsets, int num_problems, int num_groups, int group_size,
+                              int max_groups_per_problem, const uint8_t* lite_mask, float percentile,
+                              float* group_fitness, float* theta, int32_t* route, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (num_problems < 0 || num_groups < 0 || num_seqs < 0 || group_size < 1 || max_groups_per_problem < 0)
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "negative size or group_size < 1");
+  if (!(percentile >= 0.f && percentile <= 100.f)) return set_err(ctx, SQ_ERR_INVALID_ARG, "percentile must be in [0, 100]");
+  if (max_groups_per_problem > sq::ROUTE_MAX_GROUPS)
+    return set_err(ctx, SQ_ERR_UNSUPPORTED, "at most %d groups per problem", sq::ROUTE_MAX_GROUPS);
+  if (num_problems == 0) return SQ_OK;
+  if (!group_offsets || !theta || (num_groups > 0 && (!seq_conf || !group_members || !group_fitness || !route)))
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "null pointer argument");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  sq::RouteParams rp = {};
+  rp.seq_conf = seq_conf; rp.group_members = group_members; rp.group_offsets = group_offsets; rp.lite_mask = lite_mask;
+  rp.K = group_size; rp.percentile = percentile;
+  rp.group_fitness = group_fitness; rp.theta = theta; rp.route = route;
+  sq::sq_route_kernel<<<(unsigned)num_problems, sq::ROUTE_THREADS, 0, static_cast<cudaStream_t>(stream)>>>(rp);
+  ctx->launches += 1;
+  SQ_CUDA(ctx, cudaGetLastError());
+  return SQ_OK;
+}
+
+extern "C" int sq_score_select_prob(sq_score_ctx* ctx, const float* fitness, const int32_t* pop_offsets, int num_problems,
+                                    float zeta, float* prob, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (num_problems < 0 || !(zeta > 0.f)) return set_err(ctx, SQ_ERR_INVALID_ARG, "num_problems >= 0 and zeta > 0 required");
+  if (num_problems == 0) return SQ_OK;
+  if (!fitness || !pop_offsets || !prob) return set_err(ctx, SQ_ERR_INVALID_ARG, "null pointer argument");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  sq::SelectParams sp = {};
+  sp.fitness = fitness; sp.pop_offsets = pop_offsets; sp.inv_zeta = 1.f / zeta; sp.prob = prob;
+  sq::sq_select_prob_kernel<<<(unsigned)num_problems, sq::ROUTE_THREADS, 0, static_cast<cudaStream_t>(stream)>>>(sp);
+  ctx->launches += 1;
+  SQ_CUDA(ctx, cudaGetLastError());
   return SQ_OK;
 }
