@@ -61,7 +61,8 @@ typedef struct {
   int64_t max_tokens;   /* largest T of any run (sizes the partial-state workspace)               */
   int     max_seqs;     /* largest B of any run                                                   */
   int     max_k;        /* largest k of any run, 1..SQ_MAX_K                                      */
-  int     cta_group;    /* 0 = default (2: CTA pairs, UMMA M=256); 1 = single-CTA UMMA (M=128)    */
+  int     cta_group;    /* 0 = default (CTA pairs, UMMA M=256; single CTA when T <= 128);
+                           1 = always single-CTA UMMA (M=128); 2 = always CTA pairs               */
   int     num_chunks;   /* 0 = planner's choice; >0 forces the number of vocab chunks per row     */
   int     group_m;      /* 0 = default (8): gang size = token tiles that share one W stream       */
   int     flags;        /* SQ_FLAG_*                                                              */

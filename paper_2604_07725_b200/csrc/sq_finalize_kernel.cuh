@@ -5,7 +5,7 @@
 //   target_logprob = z_target - lse
 //   topk_logprob_j = z_(j) - lse,  conf = c(i) = -(1/k) sum_j topk_logprob_j    (Eq. 3)
 //
-// One warp per token row; lane c holds chunk c's state (num_chunks <= 32).  The running max / sum /
+// One warp per token row; lane c holds the state of chunks c, c+32, ... (num_chunks <= 160).  The running max / sum /
 // entropy merge is a warp-shuffle reduction; the top-k merge is k rounds of a warp arg-max over the
 // heads of the per-chunk sorted lists (ties: larger value first, then smaller vocabulary id).
 #pragma once
@@ -34,6 +34,8 @@ struct FinalizeParams {
 };
 
 constexpr int FIN_WARPS = 8;
+constexpr int FIN_MAX_NL = 5;                      // lists per lane
+constexpr int FIN_MAX_CHUNKS = 32 * FIN_MAX_NL;    // 160 vocab chunks per row at most
 
 __global__ void __launch_bounds__(FIN_WARPS * 32)
 sq_finalize_kernel(const FinalizeParams p) {
@@ -42,20 +44,31 @@ sq_finalize_kernel(const FinalizeParams p) {
   if (row >= p.T) return;
   const unsigned FULL = 0xffffffffu;
   const float NEG = -1.0e30f;
-  const bool has = lane < p.num_chunks;
-  const size_t o = (size_t)lane * p.T + row;
-  const float m_c = has ? p.part_m[o] : NEG;
-  // the merge runs in fp64: S - 1 of a peaked row is ~1e-4 and carries the whole entropy
-  const double s_c = has ? ((double)p.part_s[o] - (double)p.part_cs[o]) : 0.0;
-  const double u_c = has ? ((double)p.part_u[o] - (double)p.part_cu[o]) : 0.0;
-
-  float M = m_c;
+  // lane owns chunks lane, lane + 32, ... (one per lane in the prefill-shaped plans, up to
+  // FIN_MAX_NL in the decode-shaped ones where every SM sweeps its own slice of the vocabulary)
+  float M = NEG;
+#pragma unroll
+  for (int i = 0; i < FIN_MAX_NL; ++i) {
+    const int c = lane + 32 * i;
+    if (c < p.num_chunks) M = fmaxf(M, p.part_m[(size_t)c * p.T + row]);
+  }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) M = fmaxf(M, __shfl_xor_sync(FULL, M, off));
-  const double dm = (double)m_c - (double)M;
-  const double w = has ? exp(dm) : 0.0;
-  double S = w * s_c;
-  double U = w * (u_c + dm * s_c);
+  // the merge runs in fp64: S - 1 of a peaked row is ~1e-4 and carries the whole entropy
+  double S = 0.0, U = 0.0;
+#pragma unroll
+  for (int i = 0; i < FIN_MAX_NL; ++i) {
+    const int c = lane + 32 * i;
+    if (c < p.num_chunks) {
+      const size_t o = (size_t)c * p.T + row;
+      const double s_c = (double)p.part_s[o] - (double)p.part_cs[o];
+      const double u_c = (double)p.part_u[o] - (double)p.part_cu[o];
+      const double dm = (double)p.part_m[o] - (double)M;
+      const double w = exp(dm);
+      S += w * s_c;
+      U += w * (u_c + dm * s_c);
+    }
+  }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {
     S += __shfl_xor_sync(FULL, S, off);
@@ -64,24 +77,31 @@ sq_finalize_kernel(const FinalizeParams p) {
   const double lnS = log(S);
   const float lse = (float)((double)M + lnS);
 
-  // ---- top-k merge: lane c walks chunk c's descending list
-  int pos = 0;
-  float hv = NEG; int hi = 0x7fffffff;
-  auto load_head = [&]() {
-    if (has && pos < p.cap) {
-      const size_t oj = ((size_t)lane * p.cap + pos) * p.T + row;
-      hv = p.part_topv[oj];
-      hi = p.part_topi[oj];
-      if (hi < 0) { hv = NEG; hi = 0x7fffffff; }   // unfilled slot
-    } else {
-      hv = NEG; hi = 0x7fffffff;
+  // ---- top-k merge: the lane walks its chunks' descending lists; hv/hi[i] = head of list i
+  int pos[FIN_MAX_NL];
+  float hv[FIN_MAX_NL];
+  int hi[FIN_MAX_NL];
+  auto load_head = [&](int i) -> void {
+    const int c = lane + 32 * i;
+    float v = NEG; int id = 0x7fffffff;
+    if (c < p.num_chunks && pos[i] < p.cap) {
+      const size_t oj = ((size_t)c * p.cap + pos[i]) * p.T + row;
+      v = p.part_topv[oj];
+      id = p.part_topi[oj];
+      if (id < 0) { v = NEG; id = 0x7fffffff; }   // unfilled slot
     }
+    hv[i] = v; hi[i] = id;
   };
-  load_head();
+#pragma unroll
+  for (int i = 0; i < FIN_MAX_NL; ++i) { pos[i] = 0; load_head(i); }
   float acc = 0.f;       // sum of the k best logits
   float my_v = 0.f; int my_i = 0;   // lane j keeps the j-th winner for a coalesced store
   for (int j = 0; j < p.k; ++j) {
-    float bv = hv; int bi = hi;
+    float lv = hv[0]; int li = hi[0];
+#pragma unroll
+    for (int i = 1; i < FIN_MAX_NL; ++i)
+      if (hv[i] > lv || (hv[i] == lv && hi[i] < li)) { lv = hv[i]; li = hi[i]; }
+    float bv = lv; int bi = li;
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
       const float ov = __shfl_xor_sync(FULL, bv, off);
@@ -90,7 +110,11 @@ sq_finalize_kernel(const FinalizeParams p) {
     }
     acc += bv;
     if (lane == j) { my_v = bv; my_i = bi; }
-    if (hi == bi && hv == bv) { ++pos; load_head(); }   // vocabulary ids are unique: exactly one lane advances
+    if (li == bi && lv == bv) {   // vocabulary ids are unique: exactly one list of one lane advances
+#pragma unroll
+      for (int i = 0; i < FIN_MAX_NL; ++i)
+        if (hi[i] == bi && hv[i] == bv) { ++pos[i]; load_head(i); }
+    }
   }
   if (lane < p.k) {
     if (p.topk_logprob) p.topk_logprob[(size_t)row * p.k + lane] = my_v - lse;

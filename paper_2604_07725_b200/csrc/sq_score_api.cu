@@ -76,7 +76,9 @@ static inline int64_t cdiv64(int64_t a, int64_t b) { return (a + b - 1) / b; }
 static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, sq_score_plan_t* pl) {
   if (!cfg || !pl || T < 0 || cfg->d <= 0 || cfg->vocab <= 0 || k < 1 || k > SQ_MAX_K) return SQ_ERR_INVALID_ARG;
   if (num_sms <= 0) num_sms = 148;
-  const int cg = (cfg->cta_group == 1) ? 1 : 2;
+  // default: CTA pairs (UMMA M = 256); a decode-shaped run of at most 128 rows fits one CTA's 128 TMEM
+  // lanes, so single-CTA UMMA (M = 128) halves the wasted MMA rows and lets all 148 SMs stream W
+  const int cg = (cfg->cta_group == 1) ? 1 : (cfg->cta_group == 2 ? 2 : ((T > 0 && T <= 128) ? 1 : 2));
   memset(pl, 0, sizeof(*pl));
   pl->cta_group = cg;
   pl->rows_per_tile = 128 * cg;
@@ -94,7 +96,7 @@ static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, 
   const int GB = pl->num_clusters - pl->num_gangs * G;   // clusters left over: one smaller gang B
   pl->gang_b_size = GB;
   const int M = pl->m_tiles;
-  const int max_chunks = std::min(32, pl->num_vtiles);
+  const int max_chunks = std::min((int)sq::FIN_MAX_CHUNKS, pl->num_vtiles);
   // cost of a plan = the slower gang class, in tile-times: rounds x (unit length + fill/drain)
   auto eval = [&](int c, int m_b, double* cost_out) {
     const int tpc = (int)cdiv64(pl->num_vtiles, c);
@@ -113,7 +115,10 @@ static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, 
     // of chunks and the number of token tiles handed to gang B; ties -> fewer chunks, smaller B.
     const double strip_mb = (double)pl->rows_per_tile * cfg->d * 2.0 / 1e6;
     const int c_l2 = (int)std::ceil(pl->num_gangs * G * strip_mb / 40.0);
-    int c_hi = std::min(max_chunks, cdiv64(M, G) * 16 < pl->num_gangs ? 32 : 16);
+    // decode-shaped runs (fewer token groups than gangs) split the vocabulary further so that every
+    // cluster streams its own slice of W: up to one chunk per gang
+    const int64_t groups = cdiv64(M, G);
+    int c_hi = std::min(max_chunks, groups * 16 < pl->num_gangs ? (int)cdiv64(pl->num_gangs, groups) : 16);
     int c_lo = std::max(1, std::min(c_hi, c_l2));
     if (cfg->num_chunks > 0) c_lo = c_hi = std::min(cfg->num_chunks, max_chunks);
     const int mb_hi = GB > 0 ? std::min(M - 1, (int)(3.0 * M * GB / pl->num_clusters) + GB) : 0;
@@ -162,9 +167,9 @@ extern "C" int64_t sq_score_launch_count(const sq_score_ctx* ctx) { return ctx ?
 
 // ------------------------------------------------------------------------------------------ create / destroy
 static int64_t ws_rows_for(const sq_score_config& cfg) {
-  const int64_t small_t = std::min<int64_t>(cfg.max_tokens, 16384);
-  int64_t rows = std::max<int64_t>(32 * small_t, 16 * cfg.max_tokens);
-  if (cfg.num_chunks > 0) rows = std::max<int64_t>(rows, (int64_t)std::min(cfg.num_chunks, 32) * cfg.max_tokens);
+  const int64_t small_t = std::min<int64_t>(cfg.max_tokens, 4096);
+  int64_t rows = std::max<int64_t>((int64_t)sq::FIN_MAX_CHUNKS * small_t, 16 * cfg.max_tokens);
+  if (cfg.num_chunks > 0) rows = std::max<int64_t>(rows, (int64_t)std::min(cfg.num_chunks, (int)sq::FIN_MAX_CHUNKS) * cfg.max_tokens);
   return rows;
 }
 

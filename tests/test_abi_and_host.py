@@ -81,7 +81,7 @@ def test_plan_covers_every_tile_exactly_once(name, cg):
     assert p["cta_group"] == cg and p["rows_per_tile"] == 128 * cg
     assert p["m_tiles"] == -(-T // (128 * cg))
     assert p["num_vtiles"] == -(-V // 256) and p["num_k_blocks"] == -(-d // 64)
-    assert 1 <= p["num_chunks"] <= 32
+    assert 1 <= p["num_chunks"] <= 160
     # chunks tile the vocabulary: no empty chunk, full coverage
     assert p["tiles_per_chunk"] * p["num_chunks"] >= p["num_vtiles"]
     assert p["tiles_per_chunk"] * (p["num_chunks"] - 1) < p["num_vtiles"]
@@ -126,6 +126,13 @@ def test_plan_wave_efficiency_on_target_config():
     rounds = max(-(-p["num_gang_units"] // p["num_gangs"]), p["num_gang_units_b"])
     ideal = p["m_tiles"] * p["num_vtiles"] / p["num_clusters"]
     assert ideal / (rounds * p["tiles_per_chunk"]) > 0.95    # < 5 % lost to gang/wave quantisation
+
+
+def test_plan_decode_shaped_defaults():
+    p = sq.plan(4096, 151936, 64, 20, num_sms=148)
+    assert p["cta_group"] == 1 and p["group_m"] == 1 and p["num_gangs"] == 148 and p["num_chunks"] > 100
+    p = sq.plan(4096, 151936, 256, 20, num_sms=148)
+    assert p["cta_group"] == 2 and p["num_gangs"] == 74 and 60 <= p["num_chunks"] <= 74
 
 
 def test_plan_forced_chunks_and_edge_sizes():

@@ -114,6 +114,21 @@ def test_small_shapes_full_parity(spec, cg, chunks, gm):
     check_seqs(out, ref)
 
 
+@pytest.mark.parametrize("T,cg", [(1, 2), (7, 1), (64, 2), (128, 1), (300, 2)])
+def test_decode_shaped_many_chunks(T, cg):
+    """Small T (self-confidence during decode): the planner gives every cluster its
+    own slice of the vocabulary (up to 160 chunks per row), merged by the finalize kernel."""
+    import paper_2604_07725_b200 as sq
+    wl = workloads.custom(name="decode", d=128, V=40000, B=1, len_lo=T, len_hi=T, k=20, window=4, seed=50 + T, w_std=0.1,
+                          planted_frac=0.5, planted_scale=3.0, rmsnorm=True)
+    inp = workloads.make_inputs(wl)
+    assert sq.plan(wl.d, wl.V, T, 20, 148, cta_group=cg)["num_chunks"] > (32 if T <= 256 else 16)
+    out = run_gpu(inp, cta_group=cg)
+    ref = oracle_full(inp)
+    check_tokens(out, ref, 20)
+    check_seqs(out, ref)
+
+
 @pytest.mark.parametrize("k", [1, 5, 8, 9, 20, 21, 32])
 def test_every_topk_capacity(k):
     inp = workloads.make_inputs(workloads.custom(name="k", d=64, V=2000, B=2, len_lo=60, len_hi=200, k=k, window=8,
