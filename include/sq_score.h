@@ -124,11 +124,15 @@ int sq_score_run(sq_score_ctx *ctx, const void *H, const void *W, const int32_t 
                  const int32_t *cu_seqlens, int num_tokens, int num_seqs, int k, int window,
                  const sq_score_outputs *outputs, void *stream);
 
-/* End-to-end form with HOST inputs and HOST results: copies H, targets and cu_seqlens to ctx-owned
- * device staging buffers, runs the same kernels, and copies the 4*B per-sequence scalars back
- * (order: mean_logprob[B], mean_entropy[B], mean_conf[B], min_window_conf[B]).  W stays on the
- * device (it is the resident model weight).  Asynchronous on `stream`; the caller synchronises
- * the stream before reading seq_out_host.
+/* End-to-end form with HOST inputs and HOST results: copies targets and cu_seqlens to ctx-owned
+ * device staging buffers, streams H in on a ctx-owned copy stream in blocks of rows (ascending, each
+ * block followed by an arrival flag) WHILE kernel 1 runs -- its producers wait for the flag of the
+ * rows they are about to load, so the transfer hides behind the GEMM -- runs the same kernels, and
+ * copies the 4*B per-sequence scalars back (order: mean_logprob[B], mean_entropy[B], mean_conf[B],
+ * min_window_conf[B]).  W stays on the device (it is the resident model weight).  Asynchronous on
+ * `stream` (which also waits for the copy stream); the caller synchronises `stream` before reading
+ * seq_out_host or reusing the host buffers.  Pinned host memory is needed for the overlap; pageable
+ * memory works but its copies are staged by the runtime.
  * Errors: as sq_score_run. */
 int sq_score_run_host(sq_score_ctx *ctx, const void *H_host, const void *W_dev,
                       const int32_t *targets_host, const int32_t *cu_seqlens_host,

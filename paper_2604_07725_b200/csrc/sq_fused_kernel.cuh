@@ -61,7 +61,10 @@ struct FusedParams {
   float* part_topv;         // [C][CAP][T]
   int32_t* part_topi;       // [C][CAP][T]
   float* zt;                // [T] target logit (written by the chunk that owns the target column)
-  int debug_flags;          // experiments only (env SQ_SCORE_DEBUG): bit0 = epilogue skips the statistics
+  const unsigned int* h_ready;   // null, or flags set as H arrives from the host (sq_score_run_host): flag f != 0
+  int flag_rows;                 //   <=> rows [0, (f+1) * flag_rows) of H are in device memory
+  int debug_flags;          // experiments only (env SQ_SCORE_DEBUG): bit0 = epilogue skips the statistics,
+                            // bit1 / bit2 = W / H boxes of half height (wrong results; L2->SM traffic probes)
 };
 
 struct Unit { int m_tile; int chunk; };
@@ -118,6 +121,20 @@ __device__ __forceinline__ void gang_barrier(unsigned int* ctr, unsigned int tar
     __nanosleep(64);
     if (clock64() - t0 > 4000000000LL) __trap();
   } while (true);
+}
+
+// H streams in from the host while the kernel runs (sq_score_run_host): rows arrive in ascending order and a copy
+// engine sets flag f once rows [0, (f+1) * flag_rows) have landed.  The producer polls before its first load of a unit.
+__device__ __forceinline__ void wait_rows_ready(const unsigned int* flag) {
+  const long long t0 = clock64();
+  unsigned int v;
+  do {
+    asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
+    if (v != 0u) break;
+    __nanosleep(200);
+    if (clock64() - t0 > 40000000000LL) __trap();
+  } while (true);
+  asm volatile("fence.proxy.async;" ::: "memory");   // the rows are read through the async proxy (TMA)
 }
 
 // value of r[i] for a run-time i without local memory: a 5-level select tree.
@@ -274,7 +291,9 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
     // ===================================================================== TMA producer
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      const uint32_t stage_tx = Cfg::STAGE_BYTES * CG;   // the pair leader's barrier counts both CTAs' bytes
+      uint32_t stage_tx = Cfg::STAGE_BYTES * CG;   // the pair leader's barrier counts both CTAs' bytes
+      if (p.debug_flags & 2) stage_tx -= (Cfg::B_BYTES / 2) * CG;   // experiment: W boxes of half height
+      if (p.debug_flags & 4) stage_tx -= (Cfg::A_BYTES / 2) * CG;   // experiment: H boxes of half height
       unsigned int epoch = 0;
       for (int gu = gc.gu0; gu < gc.gu_end; gu += gc.gu_step) {
         Unit un;
@@ -282,6 +301,8 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
         if (gc.size > 1) gang_barrier(p.gang_ctr + gc.ctr, (++epoch) * (unsigned)(gc.size * CG));
         if (!active) continue;
         const int row0 = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M;
+        if (p.h_ready != nullptr && row0 < p.T)
+          wait_rows_ready(p.h_ready + (min(row0 + BLOCK_M, p.T) - 1) / p.flag_rows);
         const int vt0 = un.chunk * p.tiles_per_chunk;
         const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
         for (int vt = vt0; vt < vt1; ++vt) {

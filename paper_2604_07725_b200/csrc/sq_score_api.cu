@@ -38,6 +38,9 @@ struct sq_score_ctx {
   int* tile_base = nullptr; int* tile_seq = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
   // staging for sq_score_run_host
   void* h_stage = nullptr; int32_t* tgt_stage = nullptr; int32_t* cu_stage = nullptr; float* seq_stage = nullptr;
+  // sq_score_run_host streams H in on its own copy stream while kernel 1 runs: one flag per block of rows
+  cudaStream_t copy_stream = nullptr; cudaEvent_t ev_fork = nullptr, ev_small = nullptr, ev_join = nullptr;
+  unsigned int* h_flags = nullptr; unsigned int* one_host = nullptr;
   // driver entry point for tensor-map encoding
   void* encode_fn = nullptr;
   // optional per-kernel timing (sq_score_set_profiling): events around kernel 1, finalize, kernel 2
@@ -184,6 +187,11 @@ extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
     if (b && cudaFree(b) != cudaSuccess) rc = SQ_ERR_CUDA;
   for (cudaEvent_t e : ctx->ev)
     if (e) cudaEventDestroy(e);
+  for (cudaEvent_t e : {ctx->ev_fork, ctx->ev_small, ctx->ev_join})
+    if (e) cudaEventDestroy(e);
+  if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+  if (ctx->h_flags && cudaFree(ctx->h_flags) != cudaSuccess) rc = SQ_ERR_CUDA;
+  if (ctx->one_host) cudaFreeHost(ctx->one_host);
   delete ctx;
   return rc;
 }
@@ -379,9 +387,10 @@ extern "C" int sq_score_reduce(sq_score_ctx* ctx, const float* target_logprob, c
   return launch_reduce(ctx, rp, static_cast<cudaStream_t>(stream));
 }
 
-extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, const int32_t* targets,
-                            const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k, int window,
-                            const sq_score_outputs* o, void* stream) {
+// h_ready / flag_rows: null / 0, or the arrival flags of an H that is still streaming in (sq_score_run_host)
+static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32_t* targets,
+                    const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k, int window,
+                    const sq_score_outputs* o, void* stream, const unsigned int* h_ready, int flag_rows) {
   if (!ctx) return SQ_ERR_INVALID_ARG;
   if (!o) return set_err(ctx, SQ_ERR_INVALID_ARG, "outputs is null");
   if (ctx->cfg.flags & SQ_FLAG_REDUCE_ONLY) return set_err(ctx, SQ_ERR_INVALID_ARG, "ctx was created with SQ_FLAG_REDUCE_ONLY");
@@ -414,9 +423,9 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
     }
     if (pl.topk_cap > ctx->cap_max) return set_err(ctx, SQ_ERR_INVALID_ARG, "k exceeds the ctx's max_k capacity");
     CUtensorMap th, tw;
-    int rc = make_tmap(ctx, &th, H, T, d, sq::BLOCK_M);
+    int rc = make_tmap(ctx, &th, H, T, d, (ctx->debug_flags & 4) ? sq::BLOCK_M / 2 : sq::BLOCK_M);
     if (rc != SQ_OK) return rc;
-    rc = make_tmap(ctx, &tw, W, V, d, sq::BLOCK_N / pl.cta_group);
+    rc = make_tmap(ctx, &tw, W, V, d, (sq::BLOCK_N / pl.cta_group) / ((ctx->debug_flags & 2) ? 2 : 1));
     if (rc != SQ_OK) return rc;
 
     sq::FusedParams fp = {};
@@ -431,6 +440,7 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
     fp.part_cs = ctx->part_cs; fp.part_cu = ctx->part_cu;
     fp.part_topv = ctx->part_topv; fp.part_topi = ctx->part_topi; fp.zt = ctx->zt;
     fp.debug_flags = ctx->debug_flags;
+    fp.h_ready = h_ready; fp.flag_rows = flag_rows;
     cudaError_t e;
     if (ctx->profiling) cudaEventRecord(ctx->ev[0], st);
     const int sel = pl.cta_group * 100 + pl.topk_cap;
@@ -472,6 +482,12 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
   return SQ_OK;
 }
 
+extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, const int32_t* targets,
+                            const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k, int window,
+                            const sq_score_outputs* o, void* stream) {
+  return run_impl(ctx, H, W, targets, cu_seqlens, num_tokens, num_seqs, k, window, o, stream, nullptr, 0);
+}
+
 extern "C" int sq_score_set_profiling(sq_score_ctx* ctx, int enable) {
   if (!ctx) return SQ_ERR_INVALID_ARG;
   SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
@@ -491,6 +507,9 @@ extern "C" int sq_score_kernel_times(sq_score_ctx* ctx, float* ms3) {
   return SQ_OK;
 }
 
+constexpr int HOST_FLAG_ROWS_MIN = 2048;   // rows of H per arrival flag (doubled until a run needs at most ...
+constexpr int HOST_FLAGS_PER_RUN = 256;    // ... this many flags)
+
 extern "C" int sq_score_run_host(sq_score_ctx* ctx, const void* H_host, const void* W_dev, const int32_t* targets_host,
                                  const int32_t* cu_seqlens_host, int num_tokens, int num_seqs, int k, int window,
                                  float* seq_out_host, void* stream) {
@@ -500,25 +519,55 @@ extern "C" int sq_score_run_host(sq_score_ctx* ctx, const void* H_host, const vo
     return set_err(ctx, SQ_ERR_INVALID_ARG, "T / B out of range for this ctx");
   if ((T > 0 && (!H_host || !W_dev || !targets_host)) || (B > 0 && (!cu_seqlens_host || !seq_out_host)))
     return set_err(ctx, SQ_ERR_INVALID_ARG, "null pointer argument");
+  if (ctx->cfg.flags & SQ_FLAG_REDUCE_ONLY) return set_err(ctx, SQ_ERR_INVALID_ARG, "ctx was created with SQ_FLAG_REDUCE_ONLY");
+  if (k < 1 || k > ctx->cfg.max_k || k > ctx->cfg.vocab || window < 1)   // before any copy is enqueued
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "k = %d outside 1..min(max_k, V) or window = %d < 1", k, window);
   SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (!ctx->h_stage) {   // staging is allocated on first use: only callers of the host form pay for it
     int rc = ws_alloc(ctx, reinterpret_cast<uint8_t**>(&ctx->h_stage), ctx->cfg.max_tokens * (int64_t)ctx->cfg.d * 2);
     if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->tgt_stage, ctx->cfg.max_tokens);
     if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->cu_stage, (int64_t)ctx->cfg.max_seqs + 1);
+    if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->h_flags, HOST_FLAGS_PER_RUN);
     if (rc != SQ_OK) return rc;
+    SQ_CUDA(ctx, cudaHostAlloc(reinterpret_cast<void**>(&ctx->one_host), sizeof(unsigned int), cudaHostAllocDefault));
+    *ctx->one_host = 1u;
+    SQ_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+    SQ_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
+    SQ_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_small, cudaEventDisableTiming));
+    SQ_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming));
   }
-  if (T > 0) {
-    SQ_CUDA(ctx, cudaMemcpyAsync(ctx->h_stage, H_host, (size_t)T * ctx->cfg.d * 2, cudaMemcpyHostToDevice, st));
-    SQ_CUDA(ctx, cudaMemcpyAsync(ctx->tgt_stage, targets_host, (size_t)T * 4, cudaMemcpyHostToDevice, st));
+  // H streams in on the ctx's copy stream in blocks of `flag_rows` rows, ascending, each followed by a 4-byte
+  // copy that raises the block's flag; kernel 1 starts as soon as targets and cu_seqlens are in and its producers
+  // wait for the flag of the rows they are about to load, so the transfer hides behind the GEMM.
+  int flag_rows = HOST_FLAG_ROWS_MIN;
+  while (cdiv64(T, flag_rows) > HOST_FLAGS_PER_RUN) flag_rows *= 2;
+  const int nflags = (int)cdiv64(T, flag_rows);
+  cudaStream_t cs = ctx->copy_stream;
+  if (T > 0) SQ_CUDA(ctx, cudaMemsetAsync(ctx->h_flags, 0, (size_t)nflags * sizeof(unsigned int), st));
+  SQ_CUDA(ctx, cudaEventRecord(ctx->ev_fork, st));         // staging buffers are free once earlier work on `st` is done
+  SQ_CUDA(ctx, cudaStreamWaitEvent(cs, ctx->ev_fork, 0));
+  if (T > 0) SQ_CUDA(ctx, cudaMemcpyAsync(ctx->tgt_stage, targets_host, (size_t)T * 4, cudaMemcpyHostToDevice, cs));
+  if (B > 0) SQ_CUDA(ctx, cudaMemcpyAsync(ctx->cu_stage, cu_seqlens_host, (size_t)(B + 1) * 4, cudaMemcpyHostToDevice, cs));
+  SQ_CUDA(ctx, cudaEventRecord(ctx->ev_small, cs));
+  const size_t row_bytes = (size_t)ctx->cfg.d * 2;
+  for (int f = 0; f < nflags; ++f) {
+    const int64_t r0 = (int64_t)f * flag_rows, r1 = std::min<int64_t>(T, r0 + flag_rows);
+    SQ_CUDA(ctx, cudaMemcpyAsync(static_cast<uint8_t*>(ctx->h_stage) + r0 * row_bytes,
+                                 static_cast<const uint8_t*>(H_host) + r0 * row_bytes, (size_t)(r1 - r0) * row_bytes,
+                                 cudaMemcpyHostToDevice, cs));
+    SQ_CUDA(ctx, cudaMemcpyAsync(ctx->h_flags + f, ctx->one_host, sizeof(unsigned int), cudaMemcpyHostToDevice, cs));
   }
-  if (B > 0) SQ_CUDA(ctx, cudaMemcpyAsync(ctx->cu_stage, cu_seqlens_host, (size_t)(B + 1) * 4, cudaMemcpyHostToDevice, st));
+  SQ_CUDA(ctx, cudaEventRecord(ctx->ev_join, cs));
+  SQ_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_small, 0));
   sq_score_outputs o = {};
   o.seq_mean_logprob = ctx->seq_stage;
   o.seq_mean_entropy = ctx->seq_stage + B;
   o.seq_mean_conf = ctx->seq_stage + 2 * (size_t)B;
   o.seq_min_window_conf = ctx->seq_stage + 3 * (size_t)B;
-  int rc = sq_score_run(ctx, ctx->h_stage, W_dev, ctx->tgt_stage, ctx->cu_stage, T, B, k, window, &o, stream);
+  int rc = run_impl(ctx, ctx->h_stage, W_dev, ctx->tgt_stage, ctx->cu_stage, T, B, k, window, &o, stream,
+                    T > 0 ? ctx->h_flags : nullptr, flag_rows);
+  SQ_CUDA(ctx, cudaStreamWaitEvent(st, ctx->ev_join, 0));   // also on the error path: `st` never runs ahead of the copies
   if (rc != SQ_OK) return rc;
   if (B > 0) SQ_CUDA(ctx, cudaMemcpyAsync(seq_out_host, ctx->seq_stage, (size_t)4 * B * sizeof(float), cudaMemcpyDeviceToHost, st));
   return SQ_OK;
