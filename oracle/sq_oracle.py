@@ -32,7 +32,7 @@ import math
 import numpy as np
 import torch
 
-ORACLE_VERSION = 2
+ORACLE_VERSION = 3
 
 
 def widen(x_bf16: torch.Tensor) -> torch.Tensor:
@@ -224,3 +224,50 @@ def selection_probabilities(fitness, pop_offsets, zeta: float) -> np.ndarray:
             e = np.exp(x - x.max())
             out[off[q]:off[q + 1]] = e / e.sum()
     return out
+
+
+# ------------------------------------------------------------------------------------------------
+# Next row: the step before the path -- gather the positions whose next-token
+# distribution is wanted and apply the scorer's final RMSNorm, giving the H the scoring pass consumes
+# ------------------------------------------------------------------------------------------------
+def trajectory_positions(query_lens, traj_lens):
+    """Packed prefill of B candidates, candidate b occupying query_lens[b] query tokens followed by
+    traj_lens[b] trajectory tokens.  Token i of the trajectory (i = 1..|tau|) is scored by
+    log p(. | t_<i, Q) (Eq. 3), i.e. by the hidden state of the position just before
+    it (reading #3); only the |tau| trajectory tokens are averaged (Eq. 4; reading #4).
+    Returns (pos, cu_seqlens): pos[t] = row of the packed hidden states that predicts scored token t.
+    A candidate with an empty query has no state that predicts its first token: ValueError."""
+    pos, cu, base = [], [0], 0
+    for q, L in zip(query_lens, traj_lens):
+        q, L = int(q), int(L)
+        if q < 1 and L > 0:
+            raise ValueError("a trajectory needs at least one query token before it")
+        first = base + q               # packed index of trajectory token 1
+        for i in range(L):
+            pos.append(first + i - 1)  # the state of the previous position predicts token i
+        cu.append(cu[-1] + L)
+        base += q + L
+    return np.asarray(pos, dtype=np.int64), np.asarray(cu, dtype=np.int64)
+
+
+def prepare_hidden(X: torch.Tensor, pos, gain: torch.Tensor, eps: float) -> np.ndarray:
+    """h[t,:] = x / sqrt(mean_j x_j^2 + eps) * gain with x = X[pos[t],:] -- the RMSNorm that closes the
+    model families whose (d, V) the configs borrow; the paper does not describe the scorer's
+    internals (reading #20: all arithmetic before ONE rounding to bf16).  fp64 throughout;
+    returns the unrounded fp64 rows [T, d]."""
+    x = widen(X)[torch.as_tensor(np.asarray(pos, dtype=np.int64))].numpy()
+    g = widen(gain).numpy()
+    ms = (x * x).sum(axis=1) / x.shape[1]
+    return x / np.sqrt(ms + eps)[:, None] * g[None, :]
+
+
+def round_to_bf16(h64: np.ndarray) -> torch.Tensor:
+    """Nearest-even rounding fp64 -> bf16 (one rounding; torch's conversion is the library step)."""
+    return torch.from_numpy(np.ascontiguousarray(h64)).to(torch.bfloat16)
+
+
+def bf16_half_ulp(h64: np.ndarray) -> np.ndarray:
+    """Half a bf16 unit in the last place at |h| (8 significand bits; subnormals below 2^-126)."""
+    a = np.abs(h64)
+    e = np.floor(np.log2(np.maximum(a, 2.0 ** -126)))
+    return 0.5 * 2.0 ** (e - 7)

@@ -136,3 +136,34 @@ def reduction_inputs(num_seqs: int, len_lo: int, len_hi: int, seed: int = 2001) 
     conf = 3.0 + torch.rand(T, generator=gen) * 12.0
     return {"target_logprob": target_logprob.float(), "entropy": entropy.float(), "conf": conf.float(),
             "cu_seqlens": cu.to(torch.int32), "T": T, "B": num_seqs}
+
+
+def prepare_inputs(wl: Workload, query_lo: int = 64, query_hi: int = 512, lengths: Optional[Sequence[int]] = None,
+                   query_lens: Optional[Sequence[int]] = None) -> dict:
+    """Inputs for the step before the path: the scorer's last-layer output X for a
+    packed prefill of B candidates (query tokens followed by trajectory tokens), the final-norm gain
+    and an LM head.  X rows are N(0,1) times a per-row scale drawn log-uniformly in [0.5, 8] (so the
+    normalisation matters), gain ~ 1 + 0.1*N(0,1); W and targets as in `make_inputs`.  Draw order:
+    trajectory lengths -> query lengths -> W -> targets -> gain -> row scales -> X (row chunks)."""
+    gen = torch.Generator(device="cpu")
+    gen.manual_seed(wl.seed + 500000)
+    drawn = draw_lengths(wl, gen)
+    lens = torch.tensor(list(lengths), dtype=torch.int64) if lengths is not None else drawn
+    qdrawn = torch.randint(query_lo, query_hi + 1, (len(drawn),), generator=gen, dtype=torch.int64)
+    qlens = torch.tensor(list(query_lens), dtype=torch.int64) if query_lens is not None else qdrawn[:len(lens)]
+    N = int(lens.sum() + qlens.sum())
+    T = int(lens.sum())
+    W = torch.empty(wl.V, wl.d, dtype=torch.bfloat16)
+    for r0 in range(0, wl.V, W_CHUNK_ROWS):
+        r1 = min(wl.V, r0 + W_CHUNK_ROWS)
+        W[r0:r1] = (torch.randn(r1 - r0, wl.d, generator=gen, dtype=torch.float32) * wl.w_std).to(torch.bfloat16)
+    targets = torch.randint(0, wl.V, (T,), generator=gen, dtype=torch.int64)
+    gain = (1.0 + 0.1 * torch.randn(wl.d, generator=gen, dtype=torch.float32)).to(torch.bfloat16)
+    scale = torch.exp(torch.rand(N, generator=gen) * (torch.log(torch.tensor(8.0)) - torch.log(torch.tensor(0.5)))
+                      + torch.log(torch.tensor(0.5)))
+    X = torch.empty(N, wl.d, dtype=torch.bfloat16)
+    for r0 in range(0, N, H_CHUNK_ROWS):
+        r1 = min(N, r0 + H_CHUNK_ROWS)
+        X[r0:r1] = (torch.randn(r1 - r0, wl.d, generator=gen, dtype=torch.float32) * scale[r0:r1, None]).to(torch.bfloat16)
+    return {"X": X, "W": W, "gain": gain, "targets": targets.to(torch.int32), "traj_lens": lens, "query_lens": qlens,
+            "eps": 1e-6, "k": wl.k, "window": wl.window, "workload": wl, "N": N, "T": T, "B": len(lens)}
