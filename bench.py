@@ -313,6 +313,33 @@ def run_ours(args):
                                      "note": "3 launches (tile_scan, tile_part, seq_final); 12 B/token read + 16 B/sequence written"}
         eng2.close()
         del r_lp, r_en, r_cf
+    if world == 1 and not args.no_prepare_standalone:
+        # the step before the path: gather + final RMSNorm of the same T rows out of a packed prefill
+        # that also holds query tokens; HBM-bound: 2*d bytes read + 2*d written + 4 (pos) per row
+        gen = torch.Generator(device=dev); gen.manual_seed(4242)
+        n_src = T + 256 * B
+        Xs = torch.randn(n_src, d, generator=gen, device=dev, dtype=torch.float32).to(torch.bfloat16)
+        gain = (1 + 0.1 * torch.randn(d, generator=gen, device=dev)).to(torch.bfloat16)
+        pos_l, _ = sq.trajectory_positions([256] * B, (inp["cu_seqlens"][1:] - inp["cu_seqlens"][:-1]).tolist())
+        pos_d = torch.tensor(pos_l, dtype=torch.int32, device=dev)
+        Hs = torch.empty(T, d, dtype=torch.bfloat16, device=dev)
+        with torch.cuda.stream(stream):
+            for _ in range(3):
+                eng.prepare(Xs, pos_d, gain, 1e-6, out=Hs, stream=stream)
+            p0 = torch.cuda.Event(enable_timing=True); p1 = torch.cuda.Event(enable_timing=True)
+            p0.record(stream)
+            for _ in range(20):
+                eng.prepare(Xs, pos_d, gain, 1e-6, out=Hs, stream=stream)
+            p1.record(stream)
+            stream.synchronize()
+        p_ms = p0.elapsed_time(p1) / 20
+        p_bytes = T * (4.0 * d + 4.0)
+        line["prepare_standalone"] = {"bound": "hbm", "achieved": p_bytes / (p_ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                      "unit": "GB/s", "frac": p_bytes / (p_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "ms": p_ms,
+                                      "rows": T, "src_rows": n_src, "algorithmic_bytes": p_bytes,
+                                      "note": "sq_score_prepare: gather + RMSNorm, 2d B read + 2d B written + 4 B per row; "
+                                              "input and output (2 x %.0f MB) exceed L2" % (T * d * 2 / 1e6)}
+        del Xs, Hs
     if args.matmul_ceiling:
         # context only: cuBLAS on the same (T, V, d) in row chunks, logits materialised chunk by chunk
         rows = 8192
@@ -375,6 +402,7 @@ def main():
     ap.add_argument("--oracle-seconds", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-reduce-standalone", action="store_true")
+    ap.add_argument("--no-prepare-standalone", action="store_true")
     ap.add_argument("--per-step-kernel-times", action="store_true",
                     help="read kernel 1's duration after every step (adds a host sync per step)")
     ap.add_argument("--matmul-ceiling", action="store_true", help="also time torch.matmul on the same shapes (context)")

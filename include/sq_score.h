@@ -150,6 +150,28 @@ int sq_score_reduce(sq_score_ctx *ctx, const float *target_logprob, const float 
                     float *seq_mean_logprob, float *seq_mean_entropy, float *seq_mean_conf,
                     float *seq_min_window_conf, void *stream);
 
+/* The step before the path: gathers the hidden states that predict the scored
+ * tokens and applies the scorer's final RMSNorm,
+ *     H_out[t,:] = bf16( x / sqrt(mean_j x_j^2 + eps) * gain ),  x = X[pos[t],:]
+ * Token i of a trajectory is scored by log p(. | t_<i, Q) (Eq. 3), i.e. by the state of the
+ * position before it, and only trajectory tokens are averaged (Eq. 4): `pos` carries that
+ * shift and packing.  fp32 arithmetic, one rounding to bf16.
+ *   X      DEVICE bf16 [num_rows, d]   last-layer output of the packed prefill (before the final norm)
+ *   pos    DEVICE int32 [T] rows of X (trusted; clamped into range), or NULL = identity (T <= num_rows)
+ *   gain   DEVICE bf16 [d]             RMSNorm weight
+ *   H_out  DEVICE bf16 [T, d]          16-byte aligned like X and gain; may alias X only when pos == NULL
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA. */
+int sq_score_prepare(sq_score_ctx *ctx, const void *X, int num_rows, const int32_t *pos, int num_tokens,
+                     const void *gain, float eps, void *H_out, void *stream);
+
+/* sq_score_prepare into a ctx-owned H buffer ([max_tokens, d] bf16, allocated on first use) followed by
+ * sq_score_run on it: the library takes the last layer's output and the position list directly.
+ * Errors: as sq_score_prepare and sq_score_run, NOMEM. */
+int sq_score_run_x(sq_score_ctx *ctx, const void *X, int num_rows, const int32_t *pos, const void *gain,
+                   float eps, const void *W, const int32_t *targets, const int32_t *cu_seqlens,
+                   int num_tokens, int num_seqs, int k, int window, const sq_score_outputs *outputs,
+                   void *stream);
+
 /* Group fitness and routing on the device, one problem per CTA:
  *   group_fitness[g] = GC(g) = (1/K) * sum_{j<K} seq_conf[group_members[g*K+j]]   Eq. 4 right
  *   theta[q] = Percentile_p of GC over problem q's non-lite groups                Eq. 6

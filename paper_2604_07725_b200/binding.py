@@ -67,6 +67,11 @@ def lib() -> C.CDLL:
     L.sq_score_route.restype = C.c_int
     L.sq_score_select_prob.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_float, C.c_void_p, C.c_void_p]
     L.sq_score_select_prob.restype = C.c_int
+    L.sq_score_prepare.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p]
+    L.sq_score_prepare.restype = C.c_int
+    L.sq_score_run_x.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p,
+                                 C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
+    L.sq_score_run_x.restype = C.c_int
     L.sq_score_plan.argtypes = [C.POINTER(sq_score_config), C.c_int64, C.c_int, C.c_int, C.POINTER(sq_score_plan_t)]
     L.sq_score_plan.restype = C.c_int
     L.sq_score_set_profiling.argtypes = [C.c_void_p, C.c_int]
@@ -138,19 +143,46 @@ class SqScore:
         T, B = H.shape[0], cu_seqlens.shape[0] - 1
         dev = H.device
         if out is None:
-            out = {}
-            f = dict(dtype=torch.float32, device=dev)
-            if per_token:
-                for n in ("lse", "target_logprob", "entropy", "conf"):
-                    out[n] = torch.empty(T, **f)
-            if topk:
-                out["topk_logprob"] = torch.empty(T, k, **f)
-                out["topk_index"] = torch.empty(T, k, dtype=torch.int32, device=dev)
-            for n in ("seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf"):
-                out[n] = torch.empty(B, **f)
+            out = self._alloc_out(T, B, k, dev, per_token, topk)
         o = sq_score_outputs(*[_ptr(out.get(n)) for n, _ in sq_score_outputs._fields_])
         self._check(self._L.sq_score_run(self._h, _ptr(H), _ptr(W), _ptr(targets), _ptr(cu_seqlens), T, B, k, window,
                                          C.byref(o), self._stream(stream)))
+        return out
+
+    def _alloc_out(self, T, B, k, dev, per_token, topk):
+        import torch
+        out = {}
+        f = dict(dtype=torch.float32, device=dev)
+        if per_token:
+            for n in ("lse", "target_logprob", "entropy", "conf"):
+                out[n] = torch.empty(T, **f)
+        if topk:
+            out["topk_logprob"] = torch.empty(T, k, **f)
+            out["topk_index"] = torch.empty(T, k, dtype=torch.int32, device=dev)
+        for n in ("seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf"):
+            out[n] = torch.empty(B, **f)
+        return out
+
+    def prepare(self, X, pos, gain, eps: float, out=None, stream=None):
+        """sq_score_prepare: H[t] = bf16(RMSNorm(X[pos[t]]) * gain); pos None = identity."""
+        import torch
+        T = X.shape[0] if pos is None else pos.shape[0]
+        if out is None:
+            out = torch.empty(T, X.shape[1], dtype=torch.bfloat16, device=X.device)
+        self._check(self._L.sq_score_prepare(self._h, _ptr(X), X.shape[0], _ptr(pos), T, _ptr(gain), float(eps), _ptr(out),
+                                             self._stream(stream)))
+        return out
+
+    def run_x(self, X, pos, gain, eps: float, W, targets, cu_seqlens, k: int, window: int, stream=None,
+              per_token: bool = True, topk: bool = True, out: Optional[dict] = None) -> dict:
+        """sq_score_run_x: prepare (gather + final RMSNorm) into the ctx's H buffer, then sq_score_run."""
+        T = X.shape[0] if pos is None else pos.shape[0]
+        B = cu_seqlens.shape[0] - 1
+        if out is None:
+            out = self._alloc_out(T, B, k, X.device, per_token, topk)
+        o = sq_score_outputs(*[_ptr(out.get(n)) for n, _ in sq_score_outputs._fields_])
+        self._check(self._L.sq_score_run_x(self._h, _ptr(X), X.shape[0], _ptr(pos), _ptr(gain), float(eps), _ptr(W), _ptr(targets),
+                                           _ptr(cu_seqlens), T, B, k, window, C.byref(o), self._stream(stream)))
         return out
 
     def run_host(self, H_host, W_dev, targets_host, cu_seqlens_host, k: int, window: int, seq_out_host, stream=None):
@@ -238,3 +270,21 @@ def shard_sequences(lengths: Sequence[int], world_size: int) -> List[List[int]]:
     for p in parts:
         p.sort()
     return parts
+
+
+def trajectory_positions(query_lens: Sequence[int], traj_lens: Sequence[int]):
+    """Host-side index arithmetic for sq_score_prepare / run_x: for a packed prefill where candidate b is
+    query_lens[b] query tokens followed by traj_lens[b] trajectory tokens, returns (pos, cu_seqlens) as
+    int32 lists -- pos[t] is the packed row whose hidden state predicts scored token t (the position
+    before it), cu_seqlens delimits the trajectories."""
+    pos: List[int] = []
+    cu = [0]
+    base = 0
+    for q, n in zip(query_lens, traj_lens):
+        q, n = int(q), int(n)
+        if n > 0 and q < 1:
+            raise ValueError("a trajectory needs at least one query token before it")
+        pos.extend(range(base + q - 1, base + q - 1 + n))
+        cu.append(cu[-1] + n)
+        base += q + n
+    return pos, cu

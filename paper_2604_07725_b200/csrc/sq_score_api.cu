@@ -15,6 +15,7 @@
 
 #include "sq_finalize_kernel.cuh"
 #include "sq_fused_kernel.cuh"
+#include "sq_prepare_kernel.cuh"
 #include "sq_reduce_kernel.cuh"
 #include "sq_route_kernel.cuh"
 
@@ -507,6 +508,49 @@ extern "C" int sq_score_kernel_times(sq_score_ctx* ctx, float* ms3) {
   return SQ_OK;
 }
 
+// H staging [max_tokens, d] bf16, allocated on first use: the landing buffer of sq_score_run_host and the output of the
+// prepare step inside sq_score_run_x
+static int ensure_h_stage(sq_score_ctx* ctx) {
+  if (ctx->h_stage) return SQ_OK;
+  return ws_alloc(ctx, reinterpret_cast<uint8_t**>(&ctx->h_stage), ctx->cfg.max_tokens * (int64_t)ctx->cfg.d * 2);
+}
+
+// ------------------------------------------------------------------------------------------ prepare (8(f)-2)
+extern "C" int sq_score_prepare(sq_score_ctx* ctx, const void* X, int num_rows, const int32_t* pos, int num_tokens,
+                                const void* gain, float eps, void* H_out, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (num_rows < 0 || num_tokens < 0 || !(eps >= 0.f)) return set_err(ctx, SQ_ERR_INVALID_ARG, "negative size or eps");
+  if (num_tokens == 0) return SQ_OK;
+  if (!X || !gain || !H_out || num_rows == 0) return set_err(ctx, SQ_ERR_INVALID_ARG, "null pointer argument or no source rows");
+  if (!pos && num_tokens > num_rows) return set_err(ctx, SQ_ERR_INVALID_ARG, "pos is null (identity) but T > num_rows");
+  if (((uintptr_t)X & 15) || ((uintptr_t)gain & 15) || ((uintptr_t)H_out & 15))
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "X, gain and H_out must be 16-byte aligned");
+  if (pos && H_out == X) return set_err(ctx, SQ_ERR_INVALID_ARG, "in-place operation needs pos == NULL");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  sq::PrepareParams pp = {};
+  pp.X = static_cast<const uint4*>(X); pp.pos = pos; pp.gain = static_cast<const uint4*>(gain);
+  pp.H = static_cast<uint4*>(H_out); pp.T = num_tokens; pp.N = num_rows; pp.d = ctx->cfg.d; pp.eps = eps;
+  const int64_t ctas = std::min<int64_t>(cdiv64(num_tokens, sq::PREP_WARPS), (int64_t)ctx->num_sms * 8);
+  sq::sq_prepare_kernel<<<(unsigned)ctas, sq::PREP_WARPS * 32, 0, static_cast<cudaStream_t>(stream)>>>(pp);
+  ctx->launches += 1;
+  SQ_CUDA(ctx, cudaGetLastError());
+  return SQ_OK;
+}
+
+extern "C" int sq_score_run_x(sq_score_ctx* ctx, const void* X, int num_rows, const int32_t* pos, const void* gain, float eps,
+                              const void* W, const int32_t* targets, const int32_t* cu_seqlens, int num_tokens, int num_seqs,
+                              int k, int window, const sq_score_outputs* outputs, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (ctx->cfg.flags & SQ_FLAG_REDUCE_ONLY) return set_err(ctx, SQ_ERR_INVALID_ARG, "ctx was created with SQ_FLAG_REDUCE_ONLY");
+  if (num_tokens < 0 || num_tokens > ctx->cfg.max_tokens) return set_err(ctx, SQ_ERR_INVALID_ARG, "T out of range for this ctx");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  int rc = ensure_h_stage(ctx);
+  if (rc != SQ_OK) return rc;
+  rc = sq_score_prepare(ctx, X, num_rows, pos, num_tokens, gain, eps, ctx->h_stage, stream);
+  if (rc != SQ_OK) return rc;
+  return run_impl(ctx, ctx->h_stage, W, targets, cu_seqlens, num_tokens, num_seqs, k, window, outputs, stream, nullptr, 0);
+}
+
 constexpr int HOST_FLAG_ROWS_MIN = 2048;   // rows of H per arrival flag (doubled until a run needs at most ...
 constexpr int HOST_FLAGS_PER_RUN = 256;    // ... this many flags)
 
@@ -524,8 +568,8 @@ extern "C" int sq_score_run_host(sq_score_ctx* ctx, const void* H_host, const vo
     return set_err(ctx, SQ_ERR_INVALID_ARG, "k = %d outside 1..min(max_k, V) or window = %d < 1", k, window);
   SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  if (!ctx->h_stage) {   // staging is allocated on first use: only callers of the host form pay for it
-    int rc = ws_alloc(ctx, reinterpret_cast<uint8_t**>(&ctx->h_stage), ctx->cfg.max_tokens * (int64_t)ctx->cfg.d * 2);
+  if (!ctx->copy_stream) {   // staging is allocated on first use: only callers of the host form pay for it
+    int rc = ensure_h_stage(ctx);
     if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->tgt_stage, ctx->cfg.max_tokens);
     if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->cu_stage, (int64_t)ctx->cfg.max_seqs + 1);
     if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->h_flags, HOST_FLAGS_PER_RUN);
