@@ -340,6 +340,32 @@ def run_ours(args):
                                       "note": "sq_score_prepare: gather + RMSNorm, 2d B read + 2d B written + 4 B per row; "
                                               "input and output (2 x %.0f MB) exceed L2" % (T * d * 2 / 1e6)}
         del Xs, Hs
+    if world == 1 and not args.no_decode_standalone:
+        # decode-shaped run (self-confidence of a decode batch): T = 64 rows against the
+        # same LM head -- every SM streams its own slice of W once, so the bound is HBM: V*d*2 bytes per pass
+        Td = 64
+        eng3 = sq.SqScore(d, V, max_tokens=Td, max_seqs=4, max_k=wl.k, device=local)
+        Hd = H[:Td].contiguous(); tgd = tg[:Td].contiguous()
+        cud = torch.tensor([0, 16, 32, 48, 64], dtype=torch.int32, device=dev)
+        with torch.cuda.stream(stream):
+            od = None
+            for _ in range(3):
+                od = eng3.run(Hd, W, tgd, cud, wl.k, 16, stream=stream, out=od)
+            d0 = torch.cuda.Event(enable_timing=True); d1 = torch.cuda.Event(enable_timing=True)
+            d0.record(stream)
+            for _ in range(20):
+                eng3.run(Hd, W, tgd, cud, wl.k, 16, stream=stream, out=od)
+            d1.record(stream)
+            stream.synchronize()
+        d_ms = d0.elapsed_time(d1) / 20
+        d_bytes = 2.0 * V * d + 2.0 * Td * d + Td * (4 + 16 + 8 * wl.k)
+        line["decode_standalone"] = {"bound": "hbm", "achieved": d_bytes / (d_ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
+                                     "unit": "GB/s", "frac": d_bytes / (d_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "ms": d_ms,
+                                     "rows": Td, "tokens_per_s": Td / (d_ms * 1e-3), "algorithmic_bytes": d_bytes,
+                                     "plan": sq.plan(d, V, Td, wl.k, num_sms=torch.cuda.get_device_properties(dev).multi_processor_count),
+                                     "note": "whole path (5 launches) on a decode batch of 64 rows; W (%.0f MB) exceeds L2 and is "
+                                             "streamed once per pass" % (V * d * 2 / 1e6)}
+        eng3.close()
     if args.matmul_ceiling:
         # context only: cuBLAS on the same (T, V, d) in row chunks, logits materialised chunk by chunk
         rows = 8192
@@ -403,6 +429,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-reduce-standalone", action="store_true")
     ap.add_argument("--no-prepare-standalone", action="store_true")
+    ap.add_argument("--no-decode-standalone", action="store_true")
     ap.add_argument("--per-step-kernel-times", action="store_true",
                     help="read kernel 1's duration after every step (adds a host sync per step)")
     ap.add_argument("--matmul-ceiling", action="store_true", help="also time torch.matmul on the same shapes (context)")

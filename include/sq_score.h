@@ -64,7 +64,7 @@ typedef struct {
   int     cta_group;    /* 0 = default (CTA pairs, UMMA M=256; single CTA when T <= 128);
                            1 = always single-CTA UMMA (M=128); 2 = always CTA pairs               */
   int     num_chunks;   /* 0 = planner's choice; >0 forces the number of vocab chunks per row     */
-  int     group_m;      /* 0 = default (8): gang size = token tiles that share one W stream       */
+  int     group_m;      /* 0 = default (12): gang size = token tiles that share one W stream       */
   int     flags;        /* SQ_FLAG_*                                                              */
 } sq_score_config;
 
