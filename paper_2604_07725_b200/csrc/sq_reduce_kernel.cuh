@@ -7,16 +7,20 @@
 //
 // HBM-bound (12 B/token).  Three launches, the 2nd and 3rd with programmatic stream serialization so that
 // their launch latency overlaps the kernel before them:
-//   tile_scan : exclusive scan of ceil(L_b / TILE) -> tile_base[B+1], tile -> sequence map, NaNs for
-//               empty sequences                                                  (1 CTA)
-//   tile_part : one CTA per (sequence, tile of TILE = 8192 tokens): coalesced partial sums and the minimum
-//               window sum among the windows that START in the tile.  The window sums are
-//               S(j) = S(j0) + sum_{i=j0+1..j} (c[i+w'-1] - c[i-1]): S(j0) is summed directly and the
-//               differences are parked in shared memory and scanned (32 per thread + one block scan),
-//               so fp32 error does not grow with the sequence.
+//   tile_scan : tile i of a sequence covers the block of TILE = 8192 tokens that starts at (s0 & ~3) + i*TILE of the
+//               packed arrays (s0 = the sequence's first token), so every tile's 16-byte vectors are aligned and only
+//               a sequence's last tile is ragged.  Exclusive scan of the tiles per sequence -> tile_base[B+1],
+//               tile -> sequence map, NaNs for empty sequences                   (1 CTA)
+//   tile_part : one CTA per tile: partial sums from 16-byte loads, and the minimum window sum among the windows
+//               that START in the tile.  The window sums are S(j) = S(ja) + sum_{m=ja..j-1} (c[m+w'] - c[m]):
+//               S(ja) for the tile's first token is summed directly; the differences are formed in registers
+//               (c[m] is the vector just loaded for the sums, c[m+w'] two aligned vectors funnelled by w' mod 4),
+//               parked in shared memory and scanned (32 per thread from 16-byte shared loads + one block scan),
+//               so fp32 error does not grow with the sequence.  The first version of this kernel issued 58
+//               instructions per token (scalar loads, 64-bit address arithmetic and a bounds check per element)
+//               and was issue-bound at 62 % of HBM bandwidth; this one issues ~10.
 //   seq_final : one warp per sequence folds its tiles' partials in fixed order (fp64 accumulators):
-//               deterministic, no float atomics.  (Folding in the tile CTA that finishes last was
-//               measured slower: the fence + atomic tail keeps every CTA's registers 2 us longer.)
+//               deterministic, no float atomics.
 #pragma once
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -27,18 +31,20 @@ namespace sq {
 #ifndef SQ_RED_TILE
 #define SQ_RED_TILE 8192
 #endif
-#ifndef SQ_RED_UNROLL
-#define SQ_RED_UNROLL 8
+#ifndef SQ_RED_NB
+#define SQ_RED_NB 2
 #endif
-constexpr int RED_TILE = SQ_RED_TILE;   // tokens per CTA
-constexpr int RED_UNROLL = SQ_RED_UNROLL;   // independent loads per array in flight per thread
+constexpr int RED_TILE = SQ_RED_TILE;     // tokens per tile = per CTA
 constexpr int RED_THREADS = 256;
 constexpr int RED_WARPS = RED_THREADS / 32;
-constexpr int RED_SMEM_BYTES = (RED_TILE + RED_TILE / 32 + 32) * 4;   // padded difference array
+constexpr int RED_PER_THREAD = RED_TILE / RED_THREADS;            // 32 consecutive differences per thread
+constexpr int RED_CHUNKS = RED_TILE / 4 / RED_THREADS;            // 16-byte vectors per thread and array: 8
+constexpr int RED_SMEM_BYTES = (RED_TILE + RED_TILE / 8) * 4;     // 4 pad floats per 32: 16-byte shared loads stay conflict-free
 
 struct ReduceParams {
   long long T;
   int B, V, window;
+  int vec;                    // 1: lp / ent / conf / targets are 16-byte aligned (vector loads); 0: scalar loads
   const float* lp;
   const float* ent;
   const float* conf;
@@ -51,16 +57,19 @@ struct ReduceParams {
   float* out_lp; float* out_ent; float* out_conf; float* out_min;
 };
 
+// tiles of the sequence [s0, s1): blocks of RED_TILE tokens from its 4-aligned start
+__device__ __forceinline__ int red_tiles_of(int s0, int s1) {
+  return s1 > s0 ? (s1 - (s0 & ~3) + RED_TILE - 1) / RED_TILE : 0;
+}
+
 __global__ void __launch_bounds__(1024) sq_reduce_tile_scan_kernel(const ReduceParams p) {
   __shared__ int warp_tot[32];
   // thread t owns the `per` consecutive sequences [t*per, (t+1)*per): one block scan in total
   const int per = (p.B + 1023) / 1024;
   const int b_lo = threadIdx.x * per, b_hi = min(p.B, b_lo + per);
   int mine = 0;
-  for (int b = b_lo; b < b_hi; ++b) {
-    const int L = p.cu[b + 1] - p.cu[b];
-    mine += L > 0 ? (L + RED_TILE - 1) / RED_TILE : 0;
-  }
+#pragma unroll 4
+  for (int b = b_lo; b < b_hi; ++b) mine += red_tiles_of(p.cu[b], p.cu[b + 1]);
   int x = mine;
 #pragma unroll
   for (int off = 1; off < 32; off <<= 1) {
@@ -82,9 +91,8 @@ __global__ void __launch_bounds__(1024) sq_reduce_tile_scan_kernel(const ReduceP
   int base = ((threadIdx.x >> 5) ? warp_tot[(threadIdx.x >> 5) - 1] : 0) + x - mine;   // exclusive prefix
   if (threadIdx.x == 0) p.tile_base[0] = 0;
   for (int b = b_lo; b < b_hi; ++b) {
-    const int L = p.cu[b + 1] - p.cu[b];
-    const int n = L > 0 ? (L + RED_TILE - 1) / RED_TILE : 0;
-    for (int i = 0; i < n; ++i) p.tile_seq[base + i] = b;   // n = ceil(L / RED_TILE): a handful per sequence
+    const int n = red_tiles_of(p.cu[b], p.cu[b + 1]);
+    for (int i = 0; i < n; ++i) p.tile_seq[base + i] = b;   // a handful per sequence
     base += n;
     p.tile_base[b + 1] = base;
     if (n == 0) {   // empty sequence: no tile CTA will ever visit it
@@ -100,91 +108,141 @@ __device__ __forceinline__ float warp_sum(float v) {
   return v;
 }
 
-// Partial sums of one tile: FULL = all RED_TILE tokens present (no bounds checks), HAS_TG = targets given.
-template <bool FULL, bool HAS_TG>
-__device__ __forceinline__ void tile_sums(const ReduceParams& p, long long t0, int n_tok, float& a_lp, float& a_n,
-                                          float& a_en, float& a_cf) {
-  const float* lp = p.lp + t0; const float* en = p.ent + t0; const float* cf = p.conf + t0;
-  const int32_t* tg = HAS_TG ? p.targets + t0 : nullptr;
-  for (int i0 = 0; i0 < (FULL ? RED_TILE : n_tok); i0 += RED_UNROLL * RED_THREADS) {
-    float vl[RED_UNROLL], ve[RED_UNROLL], vc[RED_UNROLL]; int vt[RED_UNROLL];
-#pragma unroll
-    for (int q = 0; q < RED_UNROLL; ++q) {   // all loads of the batch first: 3-4 x RED_UNROLL in flight per thread
-      const int i = i0 + q * RED_THREADS + threadIdx.x;
-      const bool in = FULL || (i < n_tok);
-      vl[q] = in ? __ldg(lp + i) : 0.f;
-      ve[q] = in ? __ldg(en + i) : 0.f;
-      vc[q] = in ? __ldg(cf + i) : 0.f;
-      if (HAS_TG) vt[q] = in ? __ldg(tg + i) : -1; else vt[q] = in ? 0 : -1;
-    }
-#pragma unroll
-    for (int q = 0; q < RED_UNROLL; ++q) {
-      const bool valid = HAS_TG ? ((unsigned)vt[q] < (unsigned)p.V) : (vt[q] >= 0);
-      a_lp += valid ? vl[q] : 0.f;
-      a_n += valid ? 1.f : 0.f;
-      a_en += ve[q];
-      a_cf += vc[q];
-    }
+__device__ __forceinline__ int red_pad(int u) { return u + ((u >> 5) << 2); }   // float index of difference u
+
+// c[e0+w .. e0+w+3] from the two aligned vectors that hold it (e0 % 4 == 0): q0 starts at e0 + (w & ~3).
+__device__ __forceinline__ float4 red_funnel(const float4& q0, const float4& q1, int s) {
+  switch (s) {
+    case 0: return q0;
+    case 1: return make_float4(q0.y, q0.z, q0.w, q1.x);
+    case 2: return make_float4(q0.z, q0.w, q1.x, q1.y);
+    default: return make_float4(q0.w, q1.x, q1.y, q1.z);
   }
 }
 
-__device__ __forceinline__ int red_pad(int i) { return i + (i >> 5); }   // conflict-free 32-float runs per thread
-
+template <bool HAS_TG>
 __global__ void __launch_bounds__(RED_THREADS) sq_reduce_tile_part_kernel(const ReduceParams p) {
-  extern __shared__ float s_d[];                 // window-sum differences of the tile, padded
+  extern __shared__ __align__(16) float s_d[];   // window-sum differences of the block, padded
   __shared__ float sh[RED_WARPS][8];
   cudaGridDependencySynchronize();               // launched with programmatic serialization behind tile_scan
   const int tile = blockIdx.x;
-  const int total_tiles = p.tile_base[p.B];
-  if (tile >= total_tiles) return;
+  if (tile >= p.tile_base[p.B]) return;
   const int b = p.tile_seq[tile];
-  const long long seq0 = p.cu[b];
-  const int L = p.cu[b + 1] - p.cu[b];
-  const int t_in = (tile - p.tile_base[b]) * RED_TILE;       // first token of the tile, in the sequence
-  const int n_tok = min(RED_TILE, L - t_in);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-
-  // ---- partial sums over the tile's tokens (coalesced)
-  float a_lp = 0.f, a_n = 0.f, a_en = 0.f, a_cf = 0.f;
-  if (n_tok == RED_TILE) {
-    if (p.targets) tile_sums<true, true>(p, seq0 + t_in, n_tok, a_lp, a_n, a_en, a_cf);
-    else tile_sums<true, false>(p, seq0 + t_in, n_tok, a_lp, a_n, a_en, a_cf);
-  } else {
-    if (p.targets) tile_sums<false, true>(p, seq0 + t_in, n_tok, a_lp, a_n, a_en, a_cf);
-    else tile_sums<false, false>(p, seq0 + t_in, n_tok, a_lp, a_n, a_en, a_cf);
-  }
-
-  // ---- sliding windows that start in this tile: S(j) = S(j0) + sum_{i=j0+1..j} (c[i+w-1] - c[i-1])
+  const int s0 = p.cu[b], s1 = p.cu[b + 1];
+  const int L = s1 - s0;
+  const int blk0 = (s0 & ~3) + (tile - p.tile_base[b]) * RED_TILE;         // first token of this tile's block, 4-aligned
+  const int g0 = max(s0, blk0), g1 = min(s1, blk0 + RED_TILE);             // the tile's tokens, absolute
   const int w = min(p.window, L);
   const int n_win = L - w + 1;
-  const int j0 = t_in;
-  const int j1 = min(t_in + RED_TILE, n_win);   // window starts [j0, j1)
-  const float* c = p.conf + seq0;
-  float a_s0 = 0.f;
-  if (j0 < j1) {
-    for (int i = threadIdx.x; i < w; i += RED_THREADS) a_s0 += __ldg(c + j0 + i);   // S(j0), summed directly
-    // differences, loaded coalesced and parked in shared memory (D[j0] = 0)
-#pragma unroll 8
-    for (int r = 0; r < RED_TILE / RED_THREADS; ++r) {
-      const int i = r * RED_THREADS + threadIdx.x;
-      const int j = j0 + i;
-      float dlt = 0.f;
-      if (j < j1 && i > 0) dlt = __ldg(c + j + w - 1) - __ldg(c + j - 1);
-      s_d[red_pad(i)] = dlt;
+  const int ta = g0 - s0;                         // first window start owned by the tile (in-sequence index)
+  const int jend = min(g1 - s0, n_win);           // owned starts: [ta, jend)
+  const bool has_start = ta < jend;
+  const int d1 = has_start ? s0 + jend - 1 : g0;  // differences c[e+w] - c[e] are formed for e in [g0, d1)
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int sh4 = w & ~3, sft = w & 3;
+
+  float a_lp = 0.f, a_n = 0.f, a_en = 0.f, a_cf = 0.f;
+  // the same for a chunk on the ragged edge of the tile, of the difference range or of the arrays: scalar loads
+  auto edge_chunk = [&](int e0) -> float4 {
+    float d[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int e = e0 + k;
+      const bool in = e >= g0 && e < g1;
+      const float cfk = in ? __ldg(p.conf + e) : 0.f;
+      const float vl = in ? __ldg(p.lp + e) : 0.f;
+      a_en += in ? __ldg(p.ent + e) : 0.f;
+      a_cf += cfk;
+      const bool valid = in && (!HAS_TG || (unsigned)__ldg(p.targets + e) < (unsigned)p.V);
+      a_lp += valid ? vl : 0.f;
+      a_n += valid ? 1.f : 0.f;
+      d[k] = (in && e < d1) ? __ldg(p.conf + e + w) - cfk : 0.f;
+    }
+    return make_float4(d[0], d[1], d[2], d[3]);
+  };
+  constexpr int ROW = 4 * RED_THREADS;            // tokens one pass of the CTA covers
+  constexpr int NB = SQ_RED_NB;                           // rows per batch: up to 5 * NB 16-byte loads in flight per thread
+  // CTA-uniform row classes: 2 = inside the tile and inside the difference range (look-ahead inside the arrays),
+  // 1 = inside the tile, past the difference range (the last w'-1 tokens of a sequence), 0 = ragged or empty
+  auto row_class = [&](int r0) -> int {
+    if (!p.vec || r0 < g0 || r0 + ROW > g1) return 0;
+    if (r0 >= d1) return 1;
+    return (r0 + ROW <= d1 && (long long)r0 + ROW + sh4 + 4 <= p.T) ? 2 : 0;
+  };
+#pragma unroll 1
+  for (int rb = 0; rb < RED_CHUNKS; rb += NB) {
+    int cls[NB];
+    float4 vl[NB], ve[NB], vc[NB], q0[NB], q1[NB];
+    int4 vt[NB];
+    const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int i = 0; i < NB; ++i) {                // every load of the batch first
+      const int e0 = blk0 + (rb + i) * ROW + 4 * threadIdx.x;
+      cls[i] = row_class(blk0 + (rb + i) * ROW);
+      vl[i] = cls[i] ? __ldg(reinterpret_cast<const float4*>(p.lp + e0)) : z4;
+      ve[i] = cls[i] ? __ldg(reinterpret_cast<const float4*>(p.ent + e0)) : z4;
+      vc[i] = cls[i] ? __ldg(reinterpret_cast<const float4*>(p.conf + e0)) : z4;
+      if (HAS_TG) vt[i] = cls[i] ? __ldg(reinterpret_cast<const int4*>(p.targets + e0)) : make_int4(-1, -1, -1, -1);
+      q0[i] = (cls[i] == 2) ? __ldg(reinterpret_cast<const float4*>(p.conf + e0 + sh4)) : z4;
+      // the vector after q0 is the next lane's q0: only lane 31 has to load it
+      q1[i] = (cls[i] == 2 && sft && lane == 31) ? __ldg(reinterpret_cast<const float4*>(p.conf + e0 + sh4 + 4)) : z4;
+    }
+#pragma unroll
+    for (int i = 0; i < NB; ++i) {
+      const int c = (rb + i) * RED_THREADS + threadIdx.x;
+      float4 dv = z4;
+      if (cls[i]) {
+        a_en += (ve[i].x + ve[i].y) + (ve[i].z + ve[i].w);
+        a_cf += (vc[i].x + vc[i].y) + (vc[i].z + vc[i].w);
+        if (HAS_TG) {
+          const bool k0 = (unsigned)vt[i].x < (unsigned)p.V, k1 = (unsigned)vt[i].y < (unsigned)p.V;
+          const bool k2 = (unsigned)vt[i].z < (unsigned)p.V, k3 = (unsigned)vt[i].w < (unsigned)p.V;
+          a_lp += ((k0 ? vl[i].x : 0.f) + (k1 ? vl[i].y : 0.f)) + ((k2 ? vl[i].z : 0.f) + (k3 ? vl[i].w : 0.f));
+          a_n += (float)((int)k0 + (int)k1 + (int)k2 + (int)k3);
+        } else {
+          a_lp += (vl[i].x + vl[i].y) + (vl[i].z + vl[i].w);
+          a_n += 4.f;
+        }
+        if (cls[i] == 2) {
+          if (sft) {                              // CTA-uniform
+            const float nx = __shfl_down_sync(0xffffffffu, q0[i].x, 1);
+            const float ny = __shfl_down_sync(0xffffffffu, q0[i].y, 1);
+            const float nz = __shfl_down_sync(0xffffffffu, q0[i].z, 1);
+            if (lane != 31) q1[i] = make_float4(nx, ny, nz, 0.f);
+          }
+          const float4 ah = red_funnel(q0[i], q1[i], sft);
+          dv = make_float4(ah.x - vc[i].x, ah.y - vc[i].y, ah.z - vc[i].z, ah.w - vc[i].w);
+        }
+      } else {
+        const int row0 = blk0 + (rb + i) * ROW;
+        if (row0 + ROW > g0 && row0 < g1) dv = edge_chunk(blk0 + 4 * c);
+      }
+      *reinterpret_cast<float4*>(s_d + red_pad(4 * c)) = dv;
     }
   }
+  float a_s0 = 0.f;                               // S(ta), summed directly
+  if (has_start)
+    for (int i = threadIdx.x; i < w; i += RED_THREADS) a_s0 += __ldg(p.conf + g0 + i);
   a_lp = warp_sum(a_lp); a_n = warp_sum(a_n); a_en = warp_sum(a_en); a_cf = warp_sum(a_cf); a_s0 = warp_sum(a_s0);
   __syncthreads();
 
-  // each thread scans its 32 consecutive window starts, then one block scan of the 256 totals
-  constexpr int PER_THREAD = RED_TILE / RED_THREADS;
+  // each thread scans its 32 consecutive differences, then one block scan of the 256 totals
+  const int uv0 = g0 - blk0, uv1 = d1 - blk0;     // differences that stand for a window start: u in [uv0, uv1)
+  const int ub = threadIdx.x * RED_PER_THREAD;
   float run = 0.f, tmin = CUDART_INF_F;
-  if (j0 < j1) {
-    const int base = threadIdx.x * PER_THREAD;
+  if (ub < uv1 && ub + RED_PER_THREAD > uv0) {
+    const float4* q = reinterpret_cast<const float4*>(s_d + red_pad(ub));
+    const bool full = ub >= uv0 && ub + RED_PER_THREAD <= uv1;
 #pragma unroll
-    for (int i = 0; i < PER_THREAD; ++i) {
-      run += s_d[red_pad(base + i)];
-      if (j0 + base + i < j1) tmin = fminf(tmin, run);
+    for (int i = 0; i < RED_PER_THREAD / 4; ++i) {
+      const float4 v = q[i];
+      const float x[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        run += x[k];
+        const int u = ub + 4 * i + k;
+        if (full || (u >= uv0 && u < uv1)) tmin = fminf(tmin, run);
+      }
     }
   }
   float incl = run;                               // inclusive scan of the thread totals
@@ -197,20 +255,20 @@ __global__ void __launch_bounds__(RED_THREADS) sq_reduce_tile_part_kernel(const 
   if (lane == 0) { sh[warp][0] = a_lp; sh[warp][1] = a_n; sh[warp][2] = a_en; sh[warp][3] = a_cf; sh[warp][6] = a_s0; }
   __syncthreads();
   float woff = 0.f;
-  for (int q = 0; q < warp; ++q) woff += sh[q][5];
+  for (int qq = 0; qq < warp; ++qq) woff += sh[qq][5];
   float wmin = tmin + (woff + incl - run);        // +inf stays +inf for threads without a window
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) wmin = fminf(wmin, __shfl_xor_sync(0xffffffffu, wmin, off));
   if (lane == 0) sh[warp][4] = wmin;
   __syncthreads();
   if (threadIdx.x == 0) {
-    float s_lp = 0.f, s_n = 0.f, s_en = 0.f, s_cf = 0.f, s0 = 0.f, best = CUDART_INF_F;
-    for (int q = 0; q < RED_WARPS; ++q) {        // fixed order: deterministic
-      s_lp += sh[q][0]; s_n += sh[q][1]; s_en += sh[q][2]; s_cf += sh[q][3]; s0 += sh[q][6];
-      best = fminf(best, sh[q][4]);
+    float s_lp = 0.f, s_n = 0.f, s_en = 0.f, s_cf = 0.f, sa = 0.f, best = 0.f;   // 0: the start ta itself
+    for (int qq = 0; qq < RED_WARPS; ++qq) {      // fixed order: deterministic
+      s_lp += sh[qq][0]; s_n += sh[qq][1]; s_en += sh[qq][2]; s_cf += sh[qq][3]; sa += sh[qq][6];
+      best = fminf(best, sh[qq][4]);
     }
     p.part_sum[tile] = make_float4(s_lp, s_n, s_en, s_cf);
-    p.part_min[tile] = s0 + best;
+    p.part_min[tile] = has_start ? sa + best : CUDART_INF_F;
   }
 }
 

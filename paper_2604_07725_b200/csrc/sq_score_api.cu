@@ -224,8 +224,8 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
     return set_err(nullptr, SQ_ERR_INVALID_ARG, "cta_group must be 0, 1 or 2; num_chunks, group_m >= 0");
   if (cfg->d % 8 != 0)
     return set_err(nullptr, SQ_ERR_UNSUPPORTED, "d = %d is not a multiple of 8 (TMA needs 16-byte row strides)", cfg->d);
-  if (cfg->max_tokens >= (1LL << 31) - 4096)
-    return set_err(nullptr, SQ_ERR_UNSUPPORTED, "max_tokens must be below 2^31 - 4096");
+  if (cfg->max_tokens >= (1LL << 31) - 16384)
+    return set_err(nullptr, SQ_ERR_UNSUPPORTED, "max_tokens must be below 2^31 - 16384");
   int ndev = 0;
   cudaError_t e = cudaGetDeviceCount(&ndev);
   if (e != cudaSuccess || ndev == 0) {
@@ -259,7 +259,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   const bool reduce_only = (cfg->flags & SQ_FLAG_REDUCE_ONLY) != 0;
   const int64_t rows = reduce_only ? 1 : ws_rows_for(*cfg);
   const int64_t T = cfg->max_tokens;
-  ctx->red_tiles_max = cdiv64(T, sq::RED_TILE) + cfg->max_seqs;
+  ctx->red_tiles_max = cdiv64(T, sq::RED_TILE) + 2 * (int64_t)cfg->max_seqs + 1;
   int rc = SQ_OK;
   auto A = [&](int r) { if (rc == SQ_OK && r != SQ_OK) rc = r; };
   A(ws_alloc(ctx, &ctx->part_m, rows));
@@ -340,9 +340,11 @@ static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CU
   return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP>, th, tw, fp);
 }
 
-static int launch_reduce(sq_score_ctx* ctx, const sq::ReduceParams& rp, cudaStream_t st) {
+static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t st) {
   if (rp.B <= 0) return SQ_OK;
-  const int64_t tiles = cdiv64(rp.T, sq::RED_TILE) + rp.B;   // upper bound on sum_b ceil(L_b / RED_TILE)
+  // 16-byte loads need 16-byte aligned arrays (tiles start on multiples of 4 tokens)
+  rp.vec = ((((uintptr_t)rp.lp | (uintptr_t)rp.ent | (uintptr_t)rp.conf | (uintptr_t)rp.targets) & 15) == 0) ? 1 : 0;
+  const int64_t tiles = cdiv64(rp.T, sq::RED_TILE) + 2 * (int64_t)rp.B;   // upper bound on sum_b ceil((L_b + 3) / RED_TILE)
   sq::sq_reduce_tile_scan_kernel<<<1, 1024, 0, st>>>(rp);
   ctx->launches += 1;
   if (rp.T > 0) {
@@ -358,7 +360,8 @@ static int launch_reduce(sq_score_ctx* ctx, const sq::ReduceParams& rp, cudaStre
     at[0].val.programmaticStreamSerializationAllowed = 1;
     lc.attrs = at;
     lc.numAttrs = 1;
-    SQ_CUDA(ctx, cudaLaunchKernelEx(&lc, sq::sq_reduce_tile_part_kernel, rp));
+    if (rp.targets) SQ_CUDA(ctx, cudaLaunchKernelEx(&lc, sq::sq_reduce_tile_part_kernel<true>, rp));
+    else SQ_CUDA(ctx, cudaLaunchKernelEx(&lc, sq::sq_reduce_tile_part_kernel<false>, rp));
     lc.gridDim = dim3((unsigned)cdiv64(rp.B, 4));
     lc.blockDim = dim3(128);
     lc.dynamicSmemBytes = 0;

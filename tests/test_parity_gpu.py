@@ -344,6 +344,37 @@ def test_reduce_kernel_alone(window):
     eng.close()
 
 
+@pytest.mark.parametrize("offset", [0, 1, 3])
+@pytest.mark.parametrize("with_targets", [False, True])
+def test_reduce_alignment_targets_and_array_end(offset, with_targets):
+    """Kernel 2's 16-byte-load path against its scalar path: arrays that start `offset` floats into an allocation
+    (unaligned -> scalar loads), a total length that is not a multiple of 4 (the last vector would cross the end of
+    the arrays), sequences that start and end inside a block, windows with every residue mod 4, invalid targets."""
+    sq = _sq()
+    lens = [5, 8190, 3, 8193, 16384, 1, 0, 12289, 4094, 7]          # T = 49165, odd
+    T = sum(lens)
+    g = torch.Generator().manual_seed(78 + offset)
+    cu = torch.tensor(np.concatenate([[0], np.cumsum(lens)]), dtype=torch.int32)
+    lp = -(torch.rand(T, generator=g) * 12); en = torch.rand(T, generator=g) * 11; cf = 3 + torch.rand(T, generator=g) * 12
+    cf[T - 600:T - 560] = 0.25                                       # a dip close to the end of the arrays
+    tg = torch.randint(0, 1000, (T,), generator=g, dtype=torch.int32)
+    tg[torch.rand(T, generator=g) < 0.2] = -1
+    tg[8195:8195 + 8193] = 5000                                      # a whole sequence without a valid target
+    dev = torch.device("cuda:0")
+    def place(x):                                                    # the same values at an `offset`-element misalignment
+        buf = torch.empty(T + 8, dtype=x.dtype, device=dev)
+        buf[offset:offset + T] = x.to(dev)
+        return buf[offset:offset + T]
+    eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
+    valid = ((tg >= 0) & (tg < 1000)).numpy() if with_targets else None
+    for window in (1, 6, 2047, 2048, 2049, 2050, 8192, 8195, 30000):
+        out = eng.reduce(place(lp), place(en), place(cf), cu.to(dev), window, targets=place(tg) if with_targets else None)
+        torch.cuda.synchronize()
+        ref = O.sequence_scores(lp.numpy(), en.numpy(), cf.numpy(), cu.numpy(), window, target_valid=valid)
+        check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
+    eng.close()
+
+
 def test_reduce_many_sequences():
     sq = _sq()
     r = workloads.reduction_inputs(3000, 1, 3000, seed=5)
