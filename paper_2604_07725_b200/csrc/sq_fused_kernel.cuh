@@ -61,6 +61,8 @@ struct FusedParams {
   float* part_topv;         // [C][CAP][T]
   int32_t* part_topi;       // [C][CAP][T]
   float* zt;                // [T] target logit (written by the chunk that owns the target column)
+  float* thr_pub;           // null, or [C][T]: chunk c's current thr_j-th best logit of row t (shared top-k bound, below)
+  int thr_j, thr_ns;        //   every chunk publishes its thr_j-th best; the bound is the thr_ns-th SMALLEST published value
   const unsigned int* h_ready;   // null, or flags set as H arrives from the host (sq_score_run_host): flag f != 0
   int flag_rows;                 //   <=> rows [0, (f+1) * flag_rows) of H are in device memory
   int debug_flags;          // experiments only (env SQ_SCORE_DEBUG): bit0 = epilogue skips the statistics,
@@ -137,6 +139,30 @@ __device__ __forceinline__ void wait_rows_ready(const unsigned int* flag) {
   asm volatile("fence.proxy.async;" ::: "memory");   // the rows are read through the async proxy (TMA)
 }
 
+// Shared top-k bound.  A row's vocabulary is swept by C chunks on C different gangs at about the same time, each
+// with its own top-k list, so a chunk that has seen n logits inserts ~k*ln(n/k) times although most of those entries
+// cannot survive the merge.  After every tile a chunk publishes its j-th best logit so far, and reads the others':
+// if r chunks each hold j logits >= x, and r*j >= k, then x is a lower bound on the row's final k-th best, and a logit
+// <= x can be dropped by every chunk (the k logits that prove the bound stay in their owners' lists, so the merged
+// top-k VALUES are exact; which of several logits exactly EQUAL to the k-th best is kept may differ).  The bound
+// used is the r-th largest = ns-th smallest of the C published values, ns = C - r + 1 <= 3.  Stale or missing values
+// only make the bound weaker.  Measured: ~5x fewer list insertions, ~40 % fewer epilogue instructions.
+template <int CAP>
+__device__ __forceinline__ float shared_topk_bound(const float (&tv)[CAP], const FusedParams& p, int chunk, int row) {
+  // thr_j is one of CAP, CAP/2, CAP/4 (host's choice): compile-time slots, so the list stays in registers
+  const float mine = (p.thr_j == CAP) ? tv[CAP - 1] : ((p.thr_j == CAP / 2) ? tv[CAP / 2 - 1] : tv[CAP / 4 - 1]);
+  float* pub = p.thr_pub + row;
+  __stcg(pub + (size_t)chunk * p.T, mine);
+  float s0 = 3.0e38f, s1 = 3.0e38f, s2 = 3.0e38f;   // the three smallest published values, ascending
+  for (int c = 0; c < p.num_chunks; ++c) {
+    const float v = (c == chunk) ? mine : __ldcg(pub + (size_t)c * p.T);
+    const float a = fminf(s0, v), b = fmaxf(s0, v);
+    const float c1 = fminf(s1, b), d = fmaxf(s1, b);
+    s0 = a; s1 = c1; s2 = fminf(s2, d);
+  }
+  return p.thr_ns == 1 ? s0 : (p.thr_ns == 2 ? s1 : s2);
+}
+
 // value of r[i] for a run-time i without local memory: a 5-level select tree.
 __device__ __forceinline__ float pick32(const float (&r)[32], int i) {
   float a[16], b[8], c[4], d2[2];
@@ -168,10 +194,11 @@ __device__ __forceinline__ void topk_insert(float (&tv)[CAP], int (&ti)[CAP], fl
 template <int CAP> struct RowState {
   float m, s, u, zt;
   float cs, cu;   // Kahan compensation of s and u: a peaked row adds ~1e-7 terms to s ~ 1
+  float gthr;     // lower bound on the row's final k-th best logit learnt from the other vocab chunks (-3e38 = none)
   float tv[CAP];
   int ti[CAP];
   __device__ __forceinline__ void reset() {
-    m = NEG_BIG; s = 0.f; u = 0.f; zt = 0.f; cs = 0.f; cu = 0.f;
+    m = NEG_BIG; s = 0.f; u = 0.f; zt = 0.f; cs = 0.f; cu = 0.f; gthr = -3.0e38f;
 #pragma unroll
     for (int j = 0; j < CAP; ++j) { tv[j] = NEG_BIG; ti[j] = -1; }
   }
@@ -222,16 +249,17 @@ __device__ __forceinline__ void consume32(RowState<CAP>& st, float (&r)[32], int
 
   if ((unsigned)(tgt - col0) < 32u) st.zt = pick32(r, tgt - col0);   // a3: target logit
 
-  if (gmax > st.tv[CAP - 1]) {   // a5: some element of this row beats the current k-th best
+  // a5: some element of this row beats the current k-th best of this chunk AND the bound from the other chunks
+  if (gmax > fmaxf(st.tv[CAP - 1], st.gthr)) {
     uint32_t mask = 0;
-    const float thr = st.tv[CAP - 1];
+    const float thr = fmaxf(st.tv[CAP - 1], st.gthr);
 #pragma unroll
     for (int i = 0; i < 32; ++i) mask |= (r[i] > thr) ? (1u << i) : 0u;
     while (mask) {
       const int i = __ffs(mask) - 1;
       mask &= mask - 1;
       const float z = pick32(r, i);
-      if (z > st.tv[CAP - 1]) topk_insert<CAP>(st.tv, st.ti, z, col0 + i);
+      if (z > st.tv[CAP - 1]) topk_insert<CAP>(st.tv, st.ti, z, col0 + i);   // (the bound itself never rises inside a group)
     }
   }
 }
@@ -391,6 +419,8 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
           if constexpr (CG == 2) mbar_arrive_cluster(tempty_remote + 8u * acc);
           else mbar_arrive(tempty_bar(acc));
         }
+        if (p.thr_pub != nullptr && row < p.T && vt + 1 < vt1)
+          st.gthr = fmaxf(st.gthr, shared_topk_bound<CAP>(st.tv, p, un.chunk, row));
       }
       if (row < p.T) {
         const size_t o = (size_t)un.chunk * p.T + row;

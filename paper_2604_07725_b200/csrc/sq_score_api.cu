@@ -33,6 +33,7 @@ struct sq_score_ctx {
   float* part_cs = nullptr; float* part_cu = nullptr;
   float* part_topv = nullptr; int32_t* part_topi = nullptr; float* zt = nullptr;
   unsigned int* gang_ctr = nullptr;
+  float* thr_pub = nullptr;   // [THR_MAX_CHUNKS][max_tokens] shared top-k bounds (sq_fused_kernel.cuh)
   // per-token scratch (used when the caller passes NULL per-token outputs)
   float* tok_lse = nullptr; float* tok_lp = nullptr; float* tok_ent = nullptr; float* tok_conf = nullptr;
   // kernel 2 workspace
@@ -67,6 +68,8 @@ static int set_err(sq_score_ctx* ctx, int code, const char* fmt, ...) {
       return set_err(ctx, SQ_ERR_CUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), \
                      __FILE__, __LINE__);                                                    \
   } while (0)
+
+constexpr int THR_MAX_CHUNKS = 16;   // the shared top-k bound is used for 2..16 vocab chunks per row
 
 static int topk_cap_for(int k) { return k <= 8 ? 8 : (k <= 20 ? 20 : 32); }
 static inline int64_t cdiv64(int64_t a, int64_t b) { return (a + b - 1) / b; }
@@ -182,7 +185,7 @@ static int64_t ws_rows_for(const sq_score_config& cfg) {
 extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
   if (!ctx) return SQ_OK;
   cudaSetDevice(ctx->cfg.device);
-  void* bufs[] = {ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
+  void* bufs[] = {ctx->thr_pub, ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
                   ctx->tok_lse, ctx->tok_lp, ctx->tok_ent, ctx->tok_conf, ctx->tile_base, ctx->tile_seq, ctx->red_sum,
                   ctx->red_min, ctx->h_stage, ctx->tgt_stage, ctx->cu_stage, ctx->seq_stage};
   int rc = SQ_OK;
@@ -271,6 +274,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   A(ws_alloc(ctx, &ctx->part_topi, rows * ctx->cap_max));
   A(ws_alloc(ctx, &ctx->zt, reduce_only ? 1 : T));
   A(ws_alloc(ctx, &ctx->gang_ctr, 256));
+  A(ws_alloc(ctx, &ctx->thr_pub, reduce_only ? 1 : (int64_t)THR_MAX_CHUNKS * T));
   A(ws_alloc(ctx, &ctx->tok_lse, reduce_only ? 1 : T));
   A(ws_alloc(ctx, &ctx->tok_lp, reduce_only ? 1 : T));
   A(ws_alloc(ctx, &ctx->tok_ent, reduce_only ? 1 : T));
@@ -447,6 +451,19 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fp.part_topv = ctx->part_topv; fp.part_topi = ctx->part_topi; fp.zt = ctx->zt;
     fp.debug_flags = ctx->debug_flags;
     fp.h_ready = h_ready; fp.flag_rows = flag_rows;
+    if (pl.num_chunks >= 2 && pl.num_chunks <= THR_MAX_CHUNKS && !(ctx->debug_flags & 16)) {
+      // every chunk publishes its j-th best, j one of cap/4, cap/2, cap (compile-time list slots); r = ceil(k / j)
+      // chunks holding j logits above x prove the bound, and the kernel takes the ns-th smallest published value,
+      // ns = C - r + 1 capped at 3 (a larger r only weakens the bound)
+      const int C = pl.num_chunks, cap = pl.topk_cap;
+      int j = cap;
+      for (int cand : {cap / 4, cap / 2})
+        if (cand >= 1 && (k + cand - 1) / cand <= C) { j = cand; break; }
+      const int r = (k + j - 1) / j;
+      fp.thr_pub = ctx->thr_pub; fp.thr_j = j; fp.thr_ns = std::min(3, C - r + 1);
+      // "nothing published": a finite value below every logit (bytes 0xFE -> -1.7e38)
+      SQ_CUDA(ctx, cudaMemsetAsync(ctx->thr_pub, 0xFE, (size_t)C * T * sizeof(float), st));
+    }
     cudaError_t e;
     if (ctx->profiling) cudaEventRecord(ctx->ev[0], st);
     const int sel = pl.cta_group * 100 + pl.topk_cap;
