@@ -37,6 +37,8 @@ constexpr int FIN_WARPS = 8;
 constexpr int FIN_MAX_NL = 5;                      // lists per lane
 constexpr int FIN_MAX_CHUNKS = 32 * FIN_MAX_NL;    // 160 vocab chunks per row at most
 
+// NL = lists (vocab chunks) per lane: 1 for the prefill-shaped plans (num_chunks <= 32), FIN_MAX_NL otherwise
+template <int NL>
 __global__ void __launch_bounds__(FIN_WARPS * 32)
 sq_finalize_kernel(const FinalizeParams p) {
   const int lane = threadIdx.x & 31;
@@ -45,10 +47,10 @@ sq_finalize_kernel(const FinalizeParams p) {
   const unsigned FULL = 0xffffffffu;
   const float NEG = -1.0e30f;
   // lane owns chunks lane, lane + 32, ... (one per lane in the prefill-shaped plans, up to
-  // FIN_MAX_NL in the decode-shaped ones where every SM sweeps its own slice of the vocabulary)
+  // NL in the decode-shaped ones where every SM sweeps its own slice of the vocabulary)
   float M = NEG;
 #pragma unroll
-  for (int i = 0; i < FIN_MAX_NL; ++i) {
+  for (int i = 0; i < NL; ++i) {
     const int c = lane + 32 * i;
     if (c < p.num_chunks) M = fmaxf(M, p.part_m[(size_t)c * p.T + row]);
   }
@@ -57,7 +59,7 @@ sq_finalize_kernel(const FinalizeParams p) {
   // the merge runs in fp64: S - 1 of a peaked row is ~1e-4 and carries the whole entropy
   double S = 0.0, U = 0.0;
 #pragma unroll
-  for (int i = 0; i < FIN_MAX_NL; ++i) {
+  for (int i = 0; i < NL; ++i) {
     const int c = lane + 32 * i;
     if (c < p.num_chunks) {
       const size_t o = (size_t)c * p.T + row;
@@ -77,29 +79,29 @@ sq_finalize_kernel(const FinalizeParams p) {
   const double lnS = log(S);
   const float lse = (float)((double)M + lnS);
 
-  // ---- top-k merge: the lane walks its chunks' descending lists; hv/hi[i] = head of list i
-  int pos[FIN_MAX_NL];
-  float hv[FIN_MAX_NL];
-  int hi[FIN_MAX_NL];
-  auto load_head = [&](int i) -> void {
+  // ---- top-k merge: the lane walks its chunks' descending lists; hv/hi[i] = head of list i, nv/ni[i] = the entry
+  // behind it, loaded one pop ahead so that its latency hides behind the next round's shuffles
+  int pos[NL];
+  float hv[NL], nv[NL];
+  int hi[NL], ni[NL];
+  auto load_at = [&](int i, int at, float& v, int& id) -> void {
     const int c = lane + 32 * i;
-    float v = NEG; int id = 0x7fffffff;
-    if (c < p.num_chunks && pos[i] < p.cap) {
-      const size_t oj = ((size_t)c * p.cap + pos[i]) * p.T + row;
+    v = NEG; id = 0x7fffffff;
+    if (c < p.num_chunks && at < p.cap) {
+      const size_t oj = ((size_t)c * p.cap + at) * p.T + row;
       v = p.part_topv[oj];
       id = p.part_topi[oj];
       if (id < 0) { v = NEG; id = 0x7fffffff; }   // unfilled slot
     }
-    hv[i] = v; hi[i] = id;
   };
 #pragma unroll
-  for (int i = 0; i < FIN_MAX_NL; ++i) { pos[i] = 0; load_head(i); }
+  for (int i = 0; i < NL; ++i) { pos[i] = 0; load_at(i, 0, hv[i], hi[i]); load_at(i, 1, nv[i], ni[i]); }
   float acc = 0.f;       // sum of the k best logits
   float my_v = 0.f; int my_i = 0;   // lane j keeps the j-th winner for a coalesced store
   for (int j = 0; j < p.k; ++j) {
     float lv = hv[0]; int li = hi[0];
 #pragma unroll
-    for (int i = 1; i < FIN_MAX_NL; ++i)
+    for (int i = 1; i < NL; ++i)
       if (hv[i] > lv || (hv[i] == lv && hi[i] < li)) { lv = hv[i]; li = hi[i]; }
     float bv = lv; int bi = li;
 #pragma unroll
@@ -112,8 +114,8 @@ sq_finalize_kernel(const FinalizeParams p) {
     if (lane == j) { my_v = bv; my_i = bi; }
     if (li == bi && lv == bv) {   // vocabulary ids are unique: exactly one list of one lane advances
 #pragma unroll
-      for (int i = 0; i < FIN_MAX_NL; ++i)
-        if (hi[i] == bi && hv[i] == bv) { ++pos[i]; load_head(i); }
+      for (int i = 0; i < NL; ++i)
+        if (hi[i] == bi && hv[i] == bv) { ++pos[i]; hv[i] = nv[i]; hi[i] = ni[i]; load_at(i, pos[i] + 1, nv[i], ni[i]); }
     }
   }
   if (lane < p.k) {

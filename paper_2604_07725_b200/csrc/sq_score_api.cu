@@ -486,7 +486,8 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fin.part_topv = ctx->part_topv; fin.part_topi = ctx->part_topi; fin.zt = ctx->zt;
     fin.lse = lse; fin.target_logprob = lp; fin.entropy = ent; fin.conf = conf;
     fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
-    sq::sq_finalize_kernel<<<(unsigned)cdiv64(T, sq::FIN_WARPS), sq::FIN_WARPS * 32, 0, st>>>(fin);
+    if (pl.num_chunks <= 32) sq::sq_finalize_kernel<1><<<(unsigned)cdiv64(T, sq::FIN_WARPS), sq::FIN_WARPS * 32, 0, st>>>(fin);
+    else sq::sq_finalize_kernel<sq::FIN_MAX_NL><<<(unsigned)cdiv64(T, sq::FIN_WARPS), sq::FIN_WARPS * 32, 0, st>>>(fin);
     ctx->launches += 2;
     SQ_CUDA(ctx, cudaGetLastError());
     if (ctx->profiling) cudaEventRecord(ctx->ev[2], st);
