@@ -172,6 +172,34 @@ int sq_score_run_x(sq_score_ctx *ctx, const void *X, int num_rows, const int32_t
                    int num_tokens, int num_seqs, int k, int window, const sq_score_outputs *outputs,
                    void *stream);
 
+/* Vocab-parallel scoring: the LM head is split by rows over R shards (the tensor-
+ * parallel layout of a served scorer); every shard scores the same H against its rows and produces ONE merged partial
+ * state per token; the states are exchanged (one all-gather, e.g. ncclAllGather / torch.distributed) and merged by the
+ * same associative operator that merges vocab chunks inside a GPU, followed by kernel 2.
+ *
+ * Packed state of one shard, 4-byte words, (6 + 2*cap) * T of them with cap = 8 / 20 / 32 for k <= 8 / 20 / 32:
+ *   m[T] s[T] u[T] cs[T] cu[T]  running max, sum exp(z-m), sum exp(z-m)(z-m), and the residues of s and u
+ *                               (true value = s - cs: the merged sums keep their fp64 precision)
+ *   topv[cap][T] topi[cap][T]   the shard's k best logits (descending) and their GLOBAL vocabulary ids, -1 = empty
+ *   zt[T]                       the target's logit, meaningful on the shard that owns its row
+ * sq_score_shard_state_bytes: size of that buffer (host-only; -1 on bad arguments). */
+int64_t sq_score_shard_state_bytes(int64_t num_tokens, int k);
+
+/* One shard: ctx was created with vocab = the shard's row count; W_shard holds rows [vocab_offset, vocab_offset +
+ * vocab) of the LM head; targets are GLOBAL ids.  Runs kernel 1 and the merge kernel in EMIT mode, writes state_out
+ * (DEVICE, sq_score_shard_state_bytes(T, k) bytes).  k <= min(max_k, shard vocab).  Asynchronous on `stream`.
+ * Errors: as sq_score_run. */
+int sq_score_run_shard(sq_score_ctx *ctx, const void *H, const void *W_shard, int vocab_offset,
+                       const int32_t *targets, int num_tokens, int k, void *state_out, void *stream);
+
+/* Merge of num_shards (1..32) packed states laid out back to back in `states` (DEVICE; the all-gather's output),
+ * then the per-token finalisation and kernel 2 -- the same outputs as sq_score_run on the whole LM head.
+ *   vocab_starts  HOST int32 [num_shards+1]: shard r owns ids [vocab_starts[r], vocab_starts[r+1]); the last entry is V
+ * Any ctx of the right max_tokens / max_seqs / max_k can merge.  Errors: INVALID_ARG, CUDA. */
+int sq_score_merge_shards(sq_score_ctx *ctx, const void *states, int num_shards, const int32_t *vocab_starts,
+                          const int32_t *targets, const int32_t *cu_seqlens, int num_tokens, int num_seqs,
+                          int k, int window, const sq_score_outputs *outputs, void *stream);
+
 /* Group fitness and routing on the device, one problem per CTA:
  *   group_fitness[g] = GC(g) = (1/K) * sum_{j<K} seq_conf[group_members[g*K+j]]   Eq. 4 right
  *   theta[q] = Percentile_p of GC over problem q's non-lite groups                Eq. 6

@@ -72,6 +72,13 @@ def lib() -> C.CDLL:
     L.sq_score_run_x.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p,
                                  C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
     L.sq_score_run_x.restype = C.c_int
+    L.sq_score_shard_state_bytes.argtypes = [C.c_int64, C.c_int]
+    L.sq_score_shard_state_bytes.restype = C.c_int64
+    L.sq_score_run_shard.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+    L.sq_score_run_shard.restype = C.c_int
+    L.sq_score_merge_shards.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_int32), C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                        C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
+    L.sq_score_merge_shards.restype = C.c_int
     L.sq_score_plan.argtypes = [C.POINTER(sq_score_config), C.c_int64, C.c_int, C.c_int, C.POINTER(sq_score_plan_t)]
     L.sq_score_plan.restype = C.c_int
     L.sq_score_set_profiling.argtypes = [C.c_void_p, C.c_int]
@@ -105,6 +112,34 @@ def plan(d: int, vocab: int, num_tokens: int, k: int, num_sms: int = 0, cta_grou
     if rc != 0:
         raise SqScoreError(rc, lib().sq_score_error_string(rc).decode())
     return {n: getattr(out, n) for n, _ in sq_score_plan_t._fields_}
+
+
+def shard_state_bytes(num_tokens: int, k: int) -> int:
+    """sq_score_shard_state_bytes (host-only)."""
+    n = lib().sq_score_shard_state_bytes(num_tokens, k)
+    if n < 0:
+        raise SqScoreError(ERR_INVALID_ARG, "bad num_tokens / k")
+    return n
+
+
+def neutral_shard_state(num_tokens: int, k: int, device):
+    """The packed state of a shard that owns no vocabulary rows: the merge operator's neutral element."""
+    import torch
+    T = num_tokens
+    cap = (shard_state_bytes(T, k) // 4 // max(T, 1) - 6) // 2 if T else 0
+    st = torch.zeros(shard_state_bytes(T, k) // 4, dtype=torch.float32, device=device)
+    st[:T] = -1.0e30                                      # m
+    st[5 * T:(5 + cap) * T] = -1.0e30                     # topv
+    st[(5 + cap) * T:(5 + 2 * cap) * T] = torch.full((cap * T,), -1, dtype=torch.int32, device=device).view(torch.float32)   # topi
+    return st
+
+
+def shard_vocab(vocab: int, world_size: int, multiple: int = 256) -> List[int]:
+    """Row split of the LM head for vocab-parallel scoring: world_size contiguous shards, sizes a multiple of
+    `multiple` rows (one vocab tile) except the last, as equal as that allows.  Returns the world_size + 1 starts."""
+    tiles = -(-vocab // multiple)
+    starts = [min(vocab, (tiles * r // world_size) * multiple) for r in range(world_size)]
+    return starts + [vocab]
 
 
 def _ptr(t) -> Optional[int]:
@@ -183,6 +218,30 @@ class SqScore:
         o = sq_score_outputs(*[_ptr(out.get(n)) for n, _ in sq_score_outputs._fields_])
         self._check(self._L.sq_score_run_x(self._h, _ptr(X), X.shape[0], _ptr(pos), _ptr(gain), float(eps), _ptr(W), _ptr(targets),
                                            _ptr(cu_seqlens), T, B, k, window, C.byref(o), self._stream(stream)))
+        return out
+
+    def run_shard(self, H, W_shard, vocab_offset: int, targets, k: int, out=None, stream=None):
+        """sq_score_run_shard: this ctx's shard of the LM head -> packed partial state (a float32 tensor of
+        shard_state_bytes(T, k) / 4 words; ids inside are int32 bit patterns)."""
+        import torch
+        T = H.shape[0]
+        if out is None:
+            out = torch.empty(shard_state_bytes(T, k) // 4, dtype=torch.float32, device=H.device)
+        self._check(self._L.sq_score_run_shard(self._h, _ptr(H), _ptr(W_shard), int(vocab_offset), _ptr(targets), T, k, _ptr(out),
+                                               self._stream(stream)))
+        return out
+
+    def merge_shards(self, states, vocab_starts: Sequence[int], targets, cu_seqlens, k: int, window: int, stream=None,
+                     per_token: bool = True, topk: bool = True, out: Optional[dict] = None) -> dict:
+        """sq_score_merge_shards: `states` is the [R, words] tensor the all-gather produced."""
+        R = len(vocab_starts) - 1
+        T, B = targets.shape[0], cu_seqlens.shape[0] - 1
+        if out is None:
+            out = self._alloc_out(T, B, k, targets.device, per_token, topk)
+        o = sq_score_outputs(*[_ptr(out.get(n)) for n, _ in sq_score_outputs._fields_])
+        vs = (C.c_int32 * (R + 1))(*[int(v) for v in vocab_starts])
+        self._check(self._L.sq_score_merge_shards(self._h, _ptr(states), R, vs, _ptr(targets), _ptr(cu_seqlens), T, B, k, window,
+                                                  C.byref(o), self._stream(stream)))
         return out
 
     def run_host(self, H_host, W_dev, targets_host, cu_seqlens_host, k: int, window: int, seq_out_host, stream=None):

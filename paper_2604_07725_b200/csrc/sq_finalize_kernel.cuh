@@ -16,6 +16,17 @@ namespace sq {
 
 struct FinalizeParams {
   int T, V, k, cap, num_chunks;
+  // Partial states may come from several vocab-parallel shards ("ranks"): chunk c lives in rank c / chunks_per_rank,
+  // whose arrays start rank_stride 4-byte words after the previous rank's (one packed state buffer per rank, gathered
+  // back to back).  One rank: chunks_per_rank = num_chunks, rank_stride = 0.
+  int chunks_per_rank;
+  long long rank_stride;
+  int num_ranks;
+  int vstart[33];           // ranks > 1: rank r owns vocabulary ids [vstart[r], vstart[r+1]) -- whose zt is the target's
+  // EMIT mode (sq_score_run_shard): instead of finalising, write the merged state as ONE chunk in the same format
+  float* out_m; float* out_s; float* out_u; float* out_cs; float* out_cu;   // [T]
+  float* out_topv; int32_t* out_topi;                                        // [cap][T]
+  float* out_zt;                                                             // [T]
   const int32_t* targets;
   const float* part_m;
   const float* part_s;
@@ -37,8 +48,10 @@ constexpr int FIN_WARPS = 8;
 constexpr int FIN_MAX_NL = 5;                      // lists per lane
 constexpr int FIN_MAX_CHUNKS = 32 * FIN_MAX_NL;    // 160 vocab chunks per row at most
 
-// NL = lists (vocab chunks) per lane: 1 for the prefill-shaped plans (num_chunks <= 32), FIN_MAX_NL otherwise
-template <int NL>
+// NL = lists (vocab chunks) per lane: 1 for the prefill-shaped plans (num_chunks <= 32), FIN_MAX_NL otherwise.
+// EMIT = write the merged state of this shard (m, s, u with their residues, k-entry list, target logit) for the
+// vocab-parallel exchange instead of the final per-token outputs.
+template <int NL, bool EMIT>
 __global__ void __launch_bounds__(FIN_WARPS * 32)
 sq_finalize_kernel(const FinalizeParams p) {
   const int lane = threadIdx.x & 31;
@@ -48,11 +61,19 @@ sq_finalize_kernel(const FinalizeParams p) {
   const float NEG = -1.0e30f;
   // lane owns chunks lane, lane + 32, ... (one per lane in the prefill-shaped plans, up to
   // NL in the decode-shaped ones where every SM sweeps its own slice of the vocabulary)
+  size_t base1[NL], basek[NL];   // word offsets of this lane's chunks: scalar arrays / first list entry
+#pragma unroll
+  for (int i = 0; i < NL; ++i) {
+    const int c = lane + 32 * i;
+    const int r = c / p.chunks_per_rank, cl = c - r * p.chunks_per_rank;
+    base1[i] = (size_t)r * p.rank_stride + (size_t)cl * p.T + row;
+    basek[i] = (size_t)r * p.rank_stride + (size_t)cl * p.cap * p.T + row;
+  }
   float M = NEG;
 #pragma unroll
   for (int i = 0; i < NL; ++i) {
     const int c = lane + 32 * i;
-    if (c < p.num_chunks) M = fmaxf(M, p.part_m[(size_t)c * p.T + row]);
+    if (c < p.num_chunks) M = fmaxf(M, p.part_m[base1[i]]);
   }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) M = fmaxf(M, __shfl_xor_sync(FULL, M, off));
@@ -62,7 +83,7 @@ sq_finalize_kernel(const FinalizeParams p) {
   for (int i = 0; i < NL; ++i) {
     const int c = lane + 32 * i;
     if (c < p.num_chunks) {
-      const size_t o = (size_t)c * p.T + row;
+      const size_t o = base1[i];
       const double s_c = (double)p.part_s[o] - (double)p.part_cs[o];
       const double u_c = (double)p.part_u[o] - (double)p.part_cu[o];
       const double dm = (double)p.part_m[o] - (double)M;
@@ -88,7 +109,7 @@ sq_finalize_kernel(const FinalizeParams p) {
     const int c = lane + 32 * i;
     v = NEG; id = 0x7fffffff;
     if (c < p.num_chunks && at < p.cap) {
-      const size_t oj = ((size_t)c * p.cap + at) * p.T + row;
+      const size_t oj = basek[i] + (size_t)at * p.T;
       v = p.part_topv[oj];
       id = p.part_topi[oj];
       if (id < 0) { v = NEG; id = 0x7fffffff; }   // unfilled slot
@@ -118,6 +139,21 @@ sq_finalize_kernel(const FinalizeParams p) {
         if (hi[i] == bi && hv[i] == bv) { ++pos[i]; hv[i] = nv[i]; hi[i] = ni[i]; load_at(i, pos[i] + 1, nv[i], ni[i]); }
     }
   }
+  if (EMIT) {
+    // the shard's merged state, one chunk: s and u keep their fp64 precision as value + residue (true = s - cs)
+    if (lane < p.cap) {
+      p.out_topv[(size_t)lane * p.T + row] = lane < p.k ? my_v : NEG;
+      p.out_topi[(size_t)lane * p.T + row] = (lane < p.k && my_v > NEG) ? my_i : -1;
+    }
+    if (lane == 0) {
+      const float s_hi = (float)S, u_hi = (float)U;
+      p.out_m[row] = M;
+      p.out_s[row] = s_hi; p.out_cs[row] = (float)((double)s_hi - S);
+      p.out_u[row] = u_hi; p.out_cu[row] = (float)((double)u_hi - U);
+      p.out_zt[row] = p.zt[row];                 // meaningful only on the shard that owns the target's column
+    }
+    return;
+  }
   if (lane < p.k) {
     if (p.topk_logprob) p.topk_logprob[(size_t)row * p.k + lane] = my_v - lse;
     if (p.topk_index) p.topk_index[(size_t)row * p.k + lane] = my_i;
@@ -125,8 +161,14 @@ sq_finalize_kernel(const FinalizeParams p) {
   if (lane == 0) {
     const int tgt = p.targets[row];
     const bool valid = (tgt >= 0) && (tgt < p.V);
+    size_t zo = row;
+    if (p.num_ranks > 1 && valid) {
+      int r = 0;
+      while (r + 1 < p.num_ranks && tgt >= p.vstart[r + 1]) ++r;
+      zo += (size_t)r * p.rank_stride;
+    }
     p.lse[row] = lse;
-    p.target_logprob[row] = valid ? (p.zt[row] - lse) : 0.f;
+    p.target_logprob[row] = valid ? (p.zt[zo] - lse) : 0.f;
     p.entropy[row] = (float)(lnS - U / S);
     p.conf[row] = lse - acc / (float)p.k;   // -(1/k) sum_j (z_(j) - lse)
   }

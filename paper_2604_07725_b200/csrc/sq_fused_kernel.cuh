@@ -65,6 +65,8 @@ struct FusedParams {
   int thr_j, thr_ns;        //   every chunk publishes its thr_j-th best; the bound is the thr_ns-th SMALLEST published value
   const unsigned int* h_ready;   // null, or flags set as H arrives from the host (sq_score_run_host): flag f != 0
   int flag_rows;                 //   <=> rows [0, (f+1) * flag_rows) of H are in device memory
+  int vocab_offset;         // W is rows [vocab_offset, vocab_offset + V) of a larger LM head (vocab-parallel shard):
+                            // targets and the reported vocabulary ids are global, columns local
   int debug_flags;          // experiments only (env SQ_SCORE_DEBUG): bit0 = epilogue skips the statistics,
                             // bit1 / bit2 = W / H boxes of half height (wrong results; L2->SM traffic probes)
 };
@@ -399,7 +401,8 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
       const int row = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M + row_in_tile;
       const int vt0 = un.chunk * p.tiles_per_chunk;
       const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
-      const int tgt = (row < p.T) ? __ldg(p.targets + row) : -1;
+      int tgt = (row < p.T) ? __ldg(p.targets + row) : -1;
+      tgt = (tgt >= p.vocab_offset) ? tgt - p.vocab_offset : -1;   // local column, or out of range
       st.reset();
       for (int vt = vt0; vt < vt1; ++vt, ++tile) {
         const uint32_t acc = tile & 1u;
@@ -433,7 +436,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
         for (int j = 0; j < CAP; ++j) {
           const size_t oj = ((size_t)un.chunk * CAP + j) * p.T + row;
           p.part_topv[oj] = st.tv[j];
-          p.part_topi[oj] = st.ti[j];
+          p.part_topi[oj] = st.ti[j] < 0 ? -1 : st.ti[j] + p.vocab_offset;
         }
         const int c0 = vt0 * BLOCK_N;
         if (tgt >= c0 && tgt < min(vt1 * BLOCK_N, p.V)) p.zt[row] = st.zt;

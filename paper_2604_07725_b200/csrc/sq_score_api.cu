@@ -397,19 +397,39 @@ extern "C" int sq_score_reduce(sq_score_ctx* ctx, const float* target_logprob, c
   return launch_reduce(ctx, rp, static_cast<cudaStream_t>(stream));
 }
 
+// Packed partial state of one vocab-parallel shard, in 4-byte words (the exchange unit of sq_score_run_shard /
+// sq_score_merge_shards): m[T] s[T] u[T] cs[T] cu[T] topv[cap][T] topi[cap][T] zt[T] -- one chunk in the layout the
+// finalize kernel merges.
+static int64_t shard_state_words(int64_t T, int cap) { return (6 + 2 * (int64_t)cap) * T; }
+static void set_state_pointers(sq::FinalizeParams& f, float* base, int64_t T, int cap, bool as_output) {
+  float* m = base; float* s_ = base + T; float* u = base + 2 * T; float* cs = base + 3 * T; float* cu = base + 4 * T;
+  float* tv = base + 5 * T; int32_t* ti = reinterpret_cast<int32_t*>(base + (5 + (int64_t)cap) * T);
+  float* zt = base + (5 + 2 * (int64_t)cap) * T;
+  if (as_output) {
+    f.out_m = m; f.out_s = s_; f.out_u = u; f.out_cs = cs; f.out_cu = cu; f.out_topv = tv; f.out_topi = ti; f.out_zt = zt;
+  } else {
+    f.part_m = m; f.part_s = s_; f.part_u = u; f.part_cs = cs; f.part_cu = cu; f.part_topv = tv; f.part_topi = ti; f.zt = zt;
+  }
+}
+
 // h_ready / flag_rows: null / 0, or the arrival flags of an H that is still streaming in (sq_score_run_host)
 static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32_t* targets,
                     const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k, int window,
-                    const sq_score_outputs* o, void* stream, const unsigned int* h_ready, int flag_rows) {
+                    const sq_score_outputs* o, void* stream, const unsigned int* h_ready, int flag_rows,
+                    int vocab_offset = 0, float* shard_state = nullptr) {
   if (!ctx) return SQ_ERR_INVALID_ARG;
-  if (!o) return set_err(ctx, SQ_ERR_INVALID_ARG, "outputs is null");
+  if (!o && !shard_state) return set_err(ctx, SQ_ERR_INVALID_ARG, "outputs is null");
+  static const sq_score_outputs no_outputs = {};
+  if (!o) o = &no_outputs;
   if (ctx->cfg.flags & SQ_FLAG_REDUCE_ONLY) return set_err(ctx, SQ_ERR_INVALID_ARG, "ctx was created with SQ_FLAG_REDUCE_ONLY");
-  const int T = num_tokens, B = num_seqs, V = ctx->cfg.vocab, d = ctx->cfg.d;
+  const int T = num_tokens, V = ctx->cfg.vocab, d = ctx->cfg.d;
+  int B = num_seqs;
   if (T < 0 || B < 0) return set_err(ctx, SQ_ERR_INVALID_ARG, "negative T or B");
   if (T > ctx->cfg.max_tokens || B > ctx->cfg.max_seqs)
     return set_err(ctx, SQ_ERR_INVALID_ARG, "T = %d / B = %d exceed max_tokens / max_seqs of this ctx", T, B);
   if (k < 1 || k > ctx->cfg.max_k || k > V) return set_err(ctx, SQ_ERR_INVALID_ARG, "k = %d outside 1..min(max_k, V)", k);
   if (window < 1) return set_err(ctx, SQ_ERR_INVALID_ARG, "window must be >= 1");
+  if (shard_state) B = 0;   // a shard run stops at the merged partial state
   if (B > 0 && (!cu_seqlens || !o->seq_mean_logprob || !o->seq_mean_entropy || !o->seq_mean_conf || !o->seq_min_window_conf))
     return set_err(ctx, SQ_ERR_INVALID_ARG, "cu_seqlens and the four per-sequence outputs are required");
   if (T > 0 && (!H || !W || !targets)) return set_err(ctx, SQ_ERR_INVALID_ARG, "H, W and targets are required");
@@ -450,6 +470,7 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fp.part_cs = ctx->part_cs; fp.part_cu = ctx->part_cu;
     fp.part_topv = ctx->part_topv; fp.part_topi = ctx->part_topi; fp.zt = ctx->zt;
     fp.debug_flags = ctx->debug_flags;
+    fp.vocab_offset = vocab_offset;
     fp.h_ready = h_ready; fp.flag_rows = flag_rows;
     if (pl.num_chunks >= 2 && pl.num_chunks <= THR_MAX_CHUNKS && !(ctx->debug_flags & 16)) {
       // every chunk publishes its j-th best, j one of cap/4, cap/2, cap (compile-time list slots); r = ceil(k / j)
@@ -486,8 +507,17 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fin.part_topv = ctx->part_topv; fin.part_topi = ctx->part_topi; fin.zt = ctx->zt;
     fin.lse = lse; fin.target_logprob = lp; fin.entropy = ent; fin.conf = conf;
     fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
-    if (pl.num_chunks <= 32) sq::sq_finalize_kernel<1><<<(unsigned)cdiv64(T, sq::FIN_WARPS), sq::FIN_WARPS * 32, 0, st>>>(fin);
-    else sq::sq_finalize_kernel<sq::FIN_MAX_NL><<<(unsigned)cdiv64(T, sq::FIN_WARPS), sq::FIN_WARPS * 32, 0, st>>>(fin);
+    fin.chunks_per_rank = pl.num_chunks; fin.rank_stride = 0; fin.num_ranks = 1;
+    const dim3 fgrid((unsigned)cdiv64(T, sq::FIN_WARPS)), fblock(sq::FIN_WARPS * 32);
+    if (shard_state) {   // vocab-parallel shard: the merged state goes out in the packed exchange layout
+      set_state_pointers(fin, shard_state, T, pl.topk_cap, /*as_output=*/true);
+      if (pl.num_chunks <= 32) sq::sq_finalize_kernel<1, true><<<fgrid, fblock, 0, st>>>(fin);
+      else sq::sq_finalize_kernel<sq::FIN_MAX_NL, true><<<fgrid, fblock, 0, st>>>(fin);
+    } else if (pl.num_chunks <= 32) {
+      sq::sq_finalize_kernel<1, false><<<fgrid, fblock, 0, st>>>(fin);
+    } else {
+      sq::sq_finalize_kernel<sq::FIN_MAX_NL, false><<<fgrid, fblock, 0, st>>>(fin);
+    }
     ctx->launches += 2;
     SQ_CUDA(ctx, cudaGetLastError());
     if (ctx->profiling) cudaEventRecord(ctx->ev[2], st);
@@ -510,6 +540,73 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
                             const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k, int window,
                             const sq_score_outputs* o, void* stream) {
   return run_impl(ctx, H, W, targets, cu_seqlens, num_tokens, num_seqs, k, window, o, stream, nullptr, 0);
+}
+
+// ------------------------------------------------------------------------------------------ vocab-parallel (8(f)-4)
+extern "C" int64_t sq_score_shard_state_bytes(int64_t num_tokens, int k) {
+  if (num_tokens < 0 || k < 1 || k > SQ_MAX_K) return -1;
+  return shard_state_words(num_tokens, topk_cap_for(k)) * 4;
+}
+
+extern "C" int sq_score_run_shard(sq_score_ctx* ctx, const void* H, const void* W_shard, int vocab_offset,
+                                  const int32_t* targets, int num_tokens, int k, void* state_out, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (vocab_offset < 0) return set_err(ctx, SQ_ERR_INVALID_ARG, "vocab_offset must be >= 0");
+  if (num_tokens > 0 && !state_out) return set_err(ctx, SQ_ERR_INVALID_ARG, "state_out is null");
+  if (num_tokens == 0) return SQ_OK;
+  return run_impl(ctx, H, W_shard, targets, nullptr, num_tokens, 0, k, 1, nullptr, stream, nullptr, 0, vocab_offset,
+                  static_cast<float*>(state_out));
+}
+
+extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int num_shards, const int32_t* vocab_starts,
+                                     const int32_t* targets, const int32_t* cu_seqlens, int num_tokens, int num_seqs,
+                                     int k, int window, const sq_score_outputs* o, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (!o) return set_err(ctx, SQ_ERR_INVALID_ARG, "outputs is null");
+  if (ctx->cfg.flags & SQ_FLAG_REDUCE_ONLY) return set_err(ctx, SQ_ERR_INVALID_ARG, "ctx was created with SQ_FLAG_REDUCE_ONLY");
+  const int T = num_tokens, B = num_seqs;
+  if (T < 0 || B < 0 || T > ctx->cfg.max_tokens || B > ctx->cfg.max_seqs)
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "T / B out of range for this ctx");
+  if (num_shards < 1 || num_shards > 32 || !vocab_starts) return set_err(ctx, SQ_ERR_INVALID_ARG, "1..32 shards with their vocabulary starts required");
+  for (int r = 0; r < num_shards; ++r)
+    if (vocab_starts[r] < 0 || vocab_starts[r + 1] < vocab_starts[r]) return set_err(ctx, SQ_ERR_INVALID_ARG, "vocab_starts must be non-decreasing from >= 0");
+  const int Vg = vocab_starts[num_shards];
+  if (k < 1 || k > ctx->cfg.max_k || k > Vg) return set_err(ctx, SQ_ERR_INVALID_ARG, "k = %d outside 1..min(max_k, V)", k);
+  if (window < 1) return set_err(ctx, SQ_ERR_INVALID_ARG, "window must be >= 1");
+  if (B > 0 && (!cu_seqlens || !o->seq_mean_logprob || !o->seq_mean_entropy || !o->seq_mean_conf || !o->seq_min_window_conf))
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "cu_seqlens and the four per-sequence outputs are required");
+  if (T > 0 && (!states || !targets)) return set_err(ctx, SQ_ERR_INVALID_ARG, "states and targets are required");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  float* lse = o->lse ? o->lse : ctx->tok_lse;
+  float* lp = o->target_logprob ? o->target_logprob : ctx->tok_lp;
+  float* ent = o->entropy ? o->entropy : ctx->tok_ent;
+  float* conf = o->conf ? o->conf : ctx->tok_conf;
+  if (T > 0) {
+    const int cap = topk_cap_for(k);
+    sq::FinalizeParams fin = {};
+    fin.T = T; fin.V = Vg; fin.k = k; fin.cap = cap; fin.num_chunks = num_shards;
+    fin.chunks_per_rank = 1; fin.rank_stride = shard_state_words(T, cap); fin.num_ranks = num_shards;
+    for (int r = 0; r <= num_shards; ++r) fin.vstart[r] = vocab_starts[r];
+    fin.targets = targets;
+    set_state_pointers(fin, const_cast<float*>(static_cast<const float*>(states)), T, cap, /*as_output=*/false);
+    fin.lse = lse; fin.target_logprob = lp; fin.entropy = ent; fin.conf = conf;
+    fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
+    sq::sq_finalize_kernel<1, false><<<(unsigned)cdiv64(T, sq::FIN_WARPS), sq::FIN_WARPS * 32, 0, st>>>(fin);
+    ctx->launches += 1;
+    SQ_CUDA(ctx, cudaGetLastError());
+  }
+  if (B > 0) {
+    sq::ReduceParams rp = {};
+    rp.T = T; rp.B = B; rp.V = Vg; rp.window = window;
+    rp.lp = lp; rp.ent = ent; rp.conf = conf; rp.targets = targets; rp.cu = cu_seqlens;
+    rp.tile_base = ctx->tile_base; rp.tile_seq = ctx->tile_seq; rp.part_sum = ctx->red_sum; rp.part_min = ctx->red_min;
+    rp.out_lp = o->seq_mean_logprob; rp.out_ent = o->seq_mean_entropy; rp.out_conf = o->seq_mean_conf;
+    rp.out_min = o->seq_min_window_conf;
+    const int rc = launch_reduce(ctx, rp, st);
+    if (rc != SQ_OK) return rc;
+  }
+  return SQ_OK;
 }
 
 extern "C" int sq_score_set_profiling(sq_score_ctx* ctx, int enable) {

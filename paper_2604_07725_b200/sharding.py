@@ -51,3 +51,30 @@ def gather_sequence_scores(local: dict, seq_ids: Sequence[int], num_seqs: int, w
                 for j, key in enumerate(SEQ_KEYS):
                     out[key][b] = g[r, 1 + j]
     return out
+
+
+def score_vocab_parallel(eng, H, W_shard, vocab_starts: Sequence[int], rank: int, targets, cu_seqlens, k: int, window: int,
+                         group=None, stream=None) -> dict:
+    """Vocab-parallel scoring on one rank: this rank's shard of the LM head -> packed partial
+    state, ONE all_gather of the states (NCCL over NVLink on GPUs), then the associative merge + kernel 2 on every
+    rank.  `eng` was created with vocab = the largest shard; every rank passes the same H, targets and cu_seqlens."""
+    import torch.distributed as dist
+    world = len(vocab_starts) - 1
+    if vocab_starts[rank + 1] > vocab_starts[rank]:
+        state = eng.run_shard(H, W_shard, vocab_starts[rank], targets, k, stream=stream)
+    else:                                                  # more ranks than vocab tiles: this rank owns no rows
+        from .binding import neutral_shard_state
+        state = neutral_shard_state(H.shape[0], k, H.device)
+    states = gather_shard_states(state, world, group=group, stream=stream)
+    return eng.merge_shards(states, vocab_starts, targets, cu_seqlens, k, window, stream=stream)
+
+
+def gather_shard_states(state: torch.Tensor, world_size: int, group=None, stream=None) -> torch.Tensor:
+    """The one collective of the vocab-parallel path: all_gather of the packed states, rank-major -- shard r's state
+    starts r * words into the result, which is what sq_score_merge_shards reads."""
+    import torch.distributed as dist
+    flat = torch.empty(world_size * state.numel(), dtype=state.dtype, device=state.device)
+    if stream is not None:
+        stream.synchronize()   # the collective runs on its own stream
+    dist.all_gather_into_tensor(flat, state, group=group)
+    return flat.view(world_size, state.numel())

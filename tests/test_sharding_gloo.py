@@ -60,3 +60,39 @@ def test_local_batch_partitions_rows():
         for i, b in enumerate(ids):
             assert int(lcu[i + 1] - lcu[i]) == int(cu[b + 1] - cu[b])
     assert sorted(seen) == list(range(60))
+
+
+# ---------------------------------------------------------------------------------- vocab-parallel exchange (8(f)-4)
+def test_shard_vocab_partition():
+    import paper_2604_07725_b200 as sq
+    for V, R in [(151936, 8), (201088, 4), (1003, 3), (100, 4), (256, 1), (257, 2)]:
+        st = sq.shard_vocab(V, R)
+        assert len(st) == R + 1 and st[0] == 0 and st[-1] == V and all(a <= b for a, b in zip(st, st[1:]))
+        assert all(s % 256 == 0 for s in st[:-1])                       # shards start on vocab-tile boundaries
+        sizes = [b - a for a, b in zip(st, st[1:])]
+        assert max(sizes) - min(s for s in sizes[:-1] or sizes) <= 2 * 256 or V < 256 * R
+
+
+def _vp_worker(rank, world, port, words, ret):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    state = torch.full((words,), float(rank + 1)) + torch.arange(words) * 1e-3      # this rank's packed state
+    ret[rank] = sharding.gather_shard_states(state, world).clone()                  # the ONE collective of the path
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_vocab_parallel_state_exchange_layout():
+    """The merge kernel reads shard r's state at word offset r * words: the gathered tensor must be rank-major."""
+    import paper_2604_07725_b200 as sq
+    words = sq.shard_state_bytes(7, 5) // 4
+    assert words == (6 + 16) * 7
+    with mp.Manager() as mgr:
+        ret = mgr.dict()
+        mp.spawn(_vp_worker, args=(2, _free_port(), words, ret), nprocs=2, join=True)
+        got = dict(ret)
+    for r in range(2):
+        g = got[r]
+        assert g.shape == (2, words) and g.is_contiguous()
+        assert torch.allclose(g[0], torch.full((words,), 1.0) + torch.arange(words) * 1e-3)
+        assert torch.allclose(g[1], torch.full((words,), 2.0) + torch.arange(words) * 1e-3)
