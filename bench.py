@@ -366,6 +366,41 @@ def run_ours(args):
                                      "note": "whole path (5 launches) on a decode batch of 64 rows; W (%.0f MB) exceeds L2 and is "
                                              "streamed once per pass" % (V * d * 2 / 1e6)}
         eng3.close()
+    if world == 1 and not args.no_vocab_parallel:
+        # one rank's share of a vocab-parallel (tensor-parallel LM head) deployment over R = 8 GPUs, emulated on this GPU:
+        # kernel 1 + merge on shard 0 (V/8 rows), then the merge of 8 gathered states + kernel 2.  The exchange itself
+        # (one all-gather of R x state bytes) is not timed here: there is one GPU.
+        R = 8
+        vs = sq.shard_vocab(V, R)
+        eng4 = sq.SqScore(d, vs[1] - vs[0], max_tokens=T, max_seqs=B, max_k=wl.k, device=local)
+        W0 = W[vs[0]:vs[1]]
+        with torch.cuda.stream(stream):
+            st0 = None
+            for _ in range(2):
+                st0 = eng4.run_shard(H, W0, vs[0], tg, wl.k, out=st0, stream=stream)
+            states = st0.unsqueeze(0).repeat(R, 1).contiguous()
+            om = None
+            for _ in range(2):
+                om = eng4.merge_shards(states, vs, tg, cu, wl.k, wl.window, stream=stream, out=om)
+            v0 = torch.cuda.Event(enable_timing=True); v1 = torch.cuda.Event(enable_timing=True); v2 = torch.cuda.Event(enable_timing=True)
+            v0.record(stream)
+            for _ in range(5):
+                eng4.run_shard(H, W0, vs[0], tg, wl.k, out=st0, stream=stream)
+            v1.record(stream)
+            for _ in range(5):
+                eng4.merge_shards(states, vs, tg, cu, wl.k, wl.window, stream=stream, out=om)
+            v2.record(stream)
+            stream.synchronize()
+        sh_ms, mg_ms = v0.elapsed_time(v1) / 5, v1.elapsed_time(v2) / 5
+        sh_flops = 2.0 * T * (vs[1] - vs[0]) * d
+        line["vocab_parallel_rank"] = {"shards": R, "shard_rows": vs[1] - vs[0], "run_shard_ms": sh_ms, "merge_shards_ms": mg_ms,
+                                       "run_shard_tflops": sh_flops / (sh_ms * 1e-3) / 1e12,
+                                       "state_bytes_per_rank": sq.shard_state_bytes(T, wl.k),
+                                       "tokens_per_s_per_rank_compute": T / ((sh_ms + mg_ms) * 1e-3),
+                                       "note": "emulated on one GPU: shard 0 of 8 + merge of 8 states; the all-gather of 8 x state "
+                                               "bytes (NVLink) is not included"}
+        eng4.close()
+        del states, st0
     if args.matmul_ceiling:
         # context only: cuBLAS on the same (T, V, d) in row chunks, logits materialised chunk by chunk
         rows = 8192
@@ -430,6 +465,7 @@ def main():
     ap.add_argument("--no-reduce-standalone", action="store_true")
     ap.add_argument("--no-prepare-standalone", action="store_true")
     ap.add_argument("--no-decode-standalone", action="store_true")
+    ap.add_argument("--no-vocab-parallel", action="store_true")
     ap.add_argument("--per-step-kernel-times", action="store_true",
                     help="read kernel 1's duration after every step (adds a host sync per step)")
     ap.add_argument("--matmul-ceiling", action="store_true", help="also time torch.matmul on the same shapes (context)")
