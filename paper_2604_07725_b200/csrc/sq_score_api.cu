@@ -248,6 +248,8 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   if (!ctx) return set_err(nullptr, SQ_ERR_NOMEM, "host allocation failed");
   ctx->cfg = *cfg;
   ctx->num_sms = prop.multiProcessorCount;
+  if (const char* lim = getenv("SQ_SCORE_MAX_SMS"))   // experiments only: plan for fewer SMs
+    if (atoi(lim) >= 2 && atoi(lim) < ctx->num_sms) ctx->num_sms = atoi(lim);
   ctx->cap_max = topk_cap_for(cfg->max_k);
   if (const char* dbg = getenv("SQ_SCORE_DEBUG")) ctx->debug_flags = atoi(dbg);
 
