@@ -54,6 +54,7 @@ constexpr int FIN_MAX_CHUNKS = 32 * FIN_MAX_NL;    // 160 vocab chunks per row a
 template <int NL, bool EMIT>
 __global__ void __launch_bounds__(FIN_WARPS * 32)
 sq_finalize_kernel(const FinalizeParams p) {
+  cudaGridDependencySynchronize();   // launched with programmatic serialization behind kernel 1 (or stand-alone: no-op)
   const int lane = threadIdx.x & 31;
   const int row = blockIdx.x * FIN_WARPS + (threadIdx.x >> 5);
   if (row >= p.T) return;

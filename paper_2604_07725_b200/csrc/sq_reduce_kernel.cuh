@@ -66,6 +66,7 @@ __device__ __forceinline__ int red_tiles_of(int s0, int s1) {
 
 __global__ void __launch_bounds__(1024) sq_reduce_tile_scan_kernel(const ReduceParams p) {
   __shared__ int warp_tot[32];
+  cudaGridDependencySynchronize();   // programmatic serialization behind the finalize kernel (stand-alone: no-op)
   // thread t owns the `per` consecutive sequences [t*per, (t+1)*per): one block scan in total
   const int per = (p.B + 1023) / 1024;
   const int b_lo = threadIdx.x * per, b_hi = min(p.B, b_lo + per);

@@ -346,12 +346,25 @@ static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CU
   return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP>, th, tw, fp);
 }
 
+// Launch with programmatic stream serialization: the kernel is scheduled while its predecessor drains and waits in
+// cudaGridDependencySynchronize() for its results.
+template <typename K, typename P>
+static cudaError_t launch_pdl(K kernel, dim3 grid, dim3 block, size_t smem, cudaStream_t st, const P& params) {
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = grid; lc.blockDim = block; lc.dynamicSmemBytes = smem; lc.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at; lc.numAttrs = 1;
+  return cudaLaunchKernelEx(&lc, kernel, params);
+}
+
 static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t st) {
   if (rp.B <= 0) return SQ_OK;
   // 16-byte loads need 16-byte aligned arrays (tiles start on multiples of 4 tokens)
   rp.vec = ((((uintptr_t)rp.lp | (uintptr_t)rp.ent | (uintptr_t)rp.conf | (uintptr_t)rp.targets) & 15) == 0) ? 1 : 0;
   const int64_t tiles = cdiv64(rp.T, sq::RED_TILE) + 2 * (int64_t)rp.B;   // upper bound on sum_b ceil((L_b + 3) / RED_TILE)
-  sq::sq_reduce_tile_scan_kernel<<<1, 1024, 0, st>>>(rp);
+  SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_tile_scan_kernel, dim3(1), dim3(1024), 0, st, rp));
   ctx->launches += 1;
   if (rp.T > 0) {
     // programmatic dependent launch: tile_part's CTAs are scheduled while tile_scan drains and wait
@@ -513,12 +526,12 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     const dim3 fgrid((unsigned)cdiv64(T, sq::FIN_WARPS)), fblock(sq::FIN_WARPS * 32);
     if (shard_state) {   // vocab-parallel shard: the merged state goes out in the packed exchange layout
       set_state_pointers(fin, shard_state, T, pl.topk_cap, /*as_output=*/true);
-      if (pl.num_chunks <= 32) sq::sq_finalize_kernel<1, true><<<fgrid, fblock, 0, st>>>(fin);
-      else sq::sq_finalize_kernel<sq::FIN_MAX_NL, true><<<fgrid, fblock, 0, st>>>(fin);
+      if (pl.num_chunks <= 32) SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, true>, fgrid, fblock, 0, st, fin));
+      else SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<sq::FIN_MAX_NL, true>, fgrid, fblock, 0, st, fin));
     } else if (pl.num_chunks <= 32) {
-      sq::sq_finalize_kernel<1, false><<<fgrid, fblock, 0, st>>>(fin);
+      SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, false>, fgrid, fblock, 0, st, fin));
     } else {
-      sq::sq_finalize_kernel<sq::FIN_MAX_NL, false><<<fgrid, fblock, 0, st>>>(fin);
+      SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<sq::FIN_MAX_NL, false>, fgrid, fblock, 0, st, fin));
     }
     ctx->launches += 2;
     SQ_CUDA(ctx, cudaGetLastError());
@@ -594,7 +607,7 @@ extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int 
     set_state_pointers(fin, const_cast<float*>(static_cast<const float*>(states)), T, cap, /*as_output=*/false);
     fin.lse = lse; fin.target_logprob = lp; fin.entropy = ent; fin.conf = conf;
     fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
-    sq::sq_finalize_kernel<1, false><<<(unsigned)cdiv64(T, sq::FIN_WARPS), sq::FIN_WARPS * 32, 0, st>>>(fin);
+    SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, false>, dim3((unsigned)cdiv64(T, sq::FIN_WARPS)), dim3(sq::FIN_WARPS * 32), 0, st, fin));
     ctx->launches += 1;
     SQ_CUDA(ctx, cudaGetLastError());
   }
