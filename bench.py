@@ -3,7 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl ours|reference]
 
-A step is one pass of the whole hot path (kernel 1 fused GEMM+statistics, finalize/merge, kernel 2: 5 launches)
+A step is one pass of the whole hot path (kernel 1 fused GEMM+statistics, finalize/merge, kernel 2: 3 launches)
 over one synthetic packed batch.  At N=1 the workload is BASELINE.json configs[2] (`qwen3_8b`, the
 config the metric's 60 % target is quoted on).  With N>1 (torchrun) every rank scores its own
 batch of the same shape (sequences shard across GPUs, W replicated, no data-path collective):
@@ -310,7 +310,7 @@ def run_ours(args):
                                      "unit": "GB/s", "frac": r_bytes / (r_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                                      "ms": r_ms, "tokens": r["T"], "seqs": r["B"], "window": wl.window,
                                      "algorithmic_bytes": r_bytes,
-                                     "note": "3 launches (tile_scan, tile_part, seq_final); 12 B/token read + 16 B/sequence written"}
+                                     "note": "3 launches (tile_scan, tile_part, seq_final) at this size; 12 B/token read + 16 B/sequence written"}
         eng2.close()
         del r_lp, r_en, r_cf
     if world == 1 and not args.no_prepare_standalone:
@@ -363,7 +363,7 @@ def run_ours(args):
                                      "unit": "GB/s", "frac": d_bytes / (d_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "ms": d_ms,
                                      "rows": Td, "tokens_per_s": Td / (d_ms * 1e-3), "algorithmic_bytes": d_bytes,
                                      "plan": sq.plan(d, V, Td, wl.k, num_sms=torch.cuda.get_device_properties(dev).multi_processor_count),
-                                     "note": "whole path (5 launches) on a decode batch of 64 rows; W (%.0f MB) exceeds L2 and is "
+                                     "note": "whole path (3 launches) on a decode batch of 64 rows; W (%.0f MB) exceeds L2 and is "
                                              "streamed once per pass" % (V * d * 2 / 1e6)}
         eng3.close()
     if world == 1 and not args.no_vocab_parallel:

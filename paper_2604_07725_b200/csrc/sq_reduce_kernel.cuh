@@ -57,6 +57,7 @@ struct ReduceParams {
   float4* part_sum;           // [tiles] (sum_lp, n_valid, sum_ent, sum_conf)
   float* part_min;            // [tiles] min window SUM among windows starting in the tile (+inf if none)
   float* out_lp; float* out_ent; float* out_conf; float* out_min;
+  int* seq_done;              // [B] tiles of each sequence finished so far (single-launch form; all zero between runs)
 };
 
 // tiles of the sequence [s0, s1): blocks of RED_TILE tokens from its 4-aligned start
@@ -123,17 +124,14 @@ __device__ __forceinline__ float4 red_funnel(const float4& q0, const float4& q1,
   }
 }
 
+// One tile: partial sums and the minimum window sum among the windows that start in it (see the header comment).
+// `tile_in_seq` = index of the tile inside sequence b, `tile` = its slot in part_sum / part_min.  Ends with thread 0
+// writing the two partials; callers synchronise before reusing s_d / sh.
 template <bool HAS_TG>
-__global__ void __launch_bounds__(RED_THREADS) sq_reduce_tile_part_kernel(const ReduceParams p) {
-  extern __shared__ __align__(16) float s_d[];   // window-sum differences of the block, padded
-  __shared__ float sh[RED_WARPS][8];
-  cudaGridDependencySynchronize();               // launched with programmatic serialization behind tile_scan
-  const int tile = blockIdx.x;
-  if (tile >= p.tile_base[p.B]) return;
-  const int b = p.tile_seq[tile];
+__device__ __forceinline__ void red_tile_body(const ReduceParams& p, float* s_d, float (*sh)[8], int b, int tile_in_seq, int tile) {
   const int s0 = p.cu[b], s1 = p.cu[b + 1];
   const int L = s1 - s0;
-  const int blk0 = (s0 & ~3) + (tile - p.tile_base[b]) * RED_TILE;         // first token of this tile's block, 4-aligned
+  const int blk0 = (s0 & ~3) + tile_in_seq * RED_TILE;                     // first token of this tile's block, 4-aligned
   const int g0 = max(s0, blk0), g1 = min(s1, blk0 + RED_TILE);             // the tile's tokens, absolute
   const int w = min(p.window, L);
   const int n_win = L - w + 1;
@@ -275,20 +273,25 @@ __global__ void __launch_bounds__(RED_THREADS) sq_reduce_tile_part_kernel(const 
   }
 }
 
-__global__ void __launch_bounds__(128) sq_reduce_seq_final_kernel(const ReduceParams p) {
-  cudaGridDependencySynchronize();               // launched with programmatic serialization behind tile_part
-  const int b = blockIdx.x * 4 + (threadIdx.x >> 5);
-  const int lane = threadIdx.x & 31;
-  if (b >= p.B) return;
-  const int L = p.cu[b + 1] - p.cu[b];
-  if (L <= 0) return;                            // tile_scan already wrote the NaNs
-  const int t0 = p.tile_base[b], t1 = p.tile_base[b + 1];
+template <bool HAS_TG>
+__global__ void __launch_bounds__(RED_THREADS) sq_reduce_tile_part_kernel(const ReduceParams p) {
+  extern __shared__ __align__(16) float s_d[];   // window-sum differences of the block, padded
+  __shared__ float sh[RED_WARPS][8];
+  cudaGridDependencySynchronize();               // launched with programmatic serialization behind tile_scan
+  const int tile = blockIdx.x;
+  if (tile >= p.tile_base[p.B]) return;
+  const int b = p.tile_seq[tile];
+  red_tile_body<HAS_TG>(p, s_d, sh, b, tile - p.tile_base[b], tile);
+}
+
+// Fold of one sequence's tile partials [t0, t1) by one warp, fixed order, fp64 accumulators.
+__device__ __forceinline__ void red_fold_sequence(const ReduceParams& p, int b, int L, int t0, int t1, int lane) {
   double s_lp = 0.0, s_n = 0.0, s_en = 0.0, s_cf = 0.0;
   float best = CUDART_INF_F;
-  for (int t = t0 + lane; t < t1; t += 32) {     // fixed order: deterministic
-    const float4 v = p.part_sum[t];
+  for (int t = t0 + lane; t < t1; t += 32) {
+    const float4 v = __ldcg(p.part_sum + t);
     s_lp += v.x; s_n += v.y; s_en += v.z; s_cf += v.w;
-    best = fminf(best, p.part_min[t]);
+    best = fminf(best, __ldcg(p.part_min + t));
   }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {
@@ -304,6 +307,86 @@ __global__ void __launch_bounds__(128) sq_reduce_seq_final_kernel(const ReducePa
     p.out_ent[b] = (float)(s_en / (double)L);
     p.out_conf[b] = (float)(s_cf / (double)L);
     p.out_min[b] = best / (float)w;
+  }
+}
+
+__global__ void __launch_bounds__(128) sq_reduce_seq_final_kernel(const ReduceParams p) {
+  cudaGridDependencySynchronize();               // launched with programmatic serialization behind tile_part
+  const int b = blockIdx.x * 4 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (b >= p.B) return;
+  const int L = p.cu[b + 1] - p.cu[b];
+  if (L <= 0) return;                            // tile_scan already wrote the NaNs
+  red_fold_sequence(p, b, L, p.tile_base[b], p.tile_base[b + 1], lane);
+}
+
+// Single-launch form (B <= RED_FUSED_MAX_SEQS): every CTA rebuilds the tile table in shared memory (a block scan over
+// the B sequence lengths: 16 KB of L2-resident cu_seqlens at B = 4096, ~2 us, instead of a one-CTA launch), takes
+// tiles round-robin, and the CTA that finishes a sequence's LAST tile folds that sequence's partials in fixed order
+// (fence + atomic counter, reset by the folder, so the counters are all zero again when the kernel ends).  Used when
+// the whole problem is one wave of CTAs (the scoring pipeline: a few dozen tiles), where it replaces three
+// latency-bound launches by one; on large inputs the three-launch form is 2x faster (a persistent CTA pays fence +
+// atomic + barriers per tile in series) and is kept.  Results are bit-identical to the three-launch form.
+constexpr int RED_FUSED_MAX_SEQS = 12287;   // (B + 1) ints of shared memory next to the difference array
+
+template <bool HAS_TG>
+__global__ void __launch_bounds__(RED_THREADS) sq_reduce_fused_kernel(const ReduceParams p) {
+  extern __shared__ __align__(16) float s_d[];
+  __shared__ float sh[RED_WARPS][8];
+  __shared__ int s_warp[RED_WARPS];
+  __shared__ int s_carry, s_last;
+  int* tb = reinterpret_cast<int*>(s_d + RED_SMEM_BYTES / 4);   // [B+1] exclusive scan of the tiles per sequence
+  cudaGridDependencySynchronize();
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) s_carry = 0;
+  __syncthreads();
+  for (int base = 0; base < p.B; base += RED_THREADS) {
+    const int b = base + threadIdx.x;
+    const int n = b < p.B ? red_tiles_of(__ldg(p.cu + b), __ldg(p.cu + b + 1)) : 0;
+    int x = n;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      const int y = __shfl_up_sync(0xffffffffu, x, off);
+      if (lane >= off) x += y;
+    }
+    if (lane == 31) s_warp[warp] = x;
+    __syncthreads();
+    int woff = s_carry;
+    for (int q = 0; q < warp; ++q) woff += s_warp[q];
+    if (b < p.B) {
+      tb[b] = woff + x - n;
+      if (n == 0 && (b % gridDim.x) == blockIdx.x) {   // empty sequence: exactly one CTA writes its NaNs
+        const float nan = CUDART_NAN_F;
+        p.out_lp[b] = nan; p.out_ent[b] = nan; p.out_conf[b] = nan; p.out_min[b] = nan;
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x == RED_THREADS - 1) s_carry = woff + x;
+    __syncthreads();
+  }
+  const int total = s_carry;
+  if (threadIdx.x == 0) tb[p.B] = total;
+  __syncthreads();
+  for (int tile = blockIdx.x; tile < total; tile += gridDim.x) {
+    int lo = 0, hi = p.B - 1;                     // the sequence b with tb[b] <= tile < tb[b+1]
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (tb[mid] <= tile) lo = mid; else hi = mid - 1;
+    }
+    const int b = lo;
+    red_tile_body<HAS_TG>(p, s_d, sh, b, tile - tb[b], tile);
+    if (threadIdx.x == 0) {
+      __threadfence();                            // the partials above are visible before the count
+      const int done = atomicAdd(p.seq_done + b, 1) + 1;
+      s_last = (done == tb[b + 1] - tb[b]) ? 1 : 0;
+    }
+    __syncthreads();
+    if (s_last && warp == 0) {
+      __threadfence();
+      red_fold_sequence(p, b, __ldg(p.cu + b + 1) - __ldg(p.cu + b), tb[b], tb[b + 1], lane);
+      if (lane == 0) p.seq_done[b] = 0;
+    }
+    __syncthreads();                              // s_d / sh / s_last are reused by the next tile
   }
 }
 

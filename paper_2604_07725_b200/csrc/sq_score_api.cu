@@ -37,6 +37,7 @@ struct sq_score_ctx {
   // per-token scratch (used when the caller passes NULL per-token outputs)
   float* tok_lse = nullptr; float* tok_lp = nullptr; float* tok_ent = nullptr; float* tok_conf = nullptr;
   // kernel 2 workspace
+  int* seq_done = nullptr;   // [max_seqs] per-sequence tile counters of the single-launch reduction (zero between runs)
   int* tile_base = nullptr; int* tile_seq = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
   // staging for sq_score_run_host
   void* h_stage = nullptr; int32_t* tgt_stage = nullptr; int32_t* cu_stage = nullptr; float* seq_stage = nullptr;
@@ -185,7 +186,7 @@ static int64_t ws_rows_for(const sq_score_config& cfg) {
 extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
   if (!ctx) return SQ_OK;
   cudaSetDevice(ctx->cfg.device);
-  void* bufs[] = {ctx->thr_pub, ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
+  void* bufs[] = {ctx->seq_done, ctx->thr_pub, ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
                   ctx->tok_lse, ctx->tok_lp, ctx->tok_ent, ctx->tok_conf, ctx->tile_base, ctx->tile_seq, ctx->red_sum,
                   ctx->red_min, ctx->h_stage, ctx->tgt_stage, ctx->cu_stage, ctx->seq_stage};
   int rc = SQ_OK;
@@ -282,6 +283,8 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   A(ws_alloc(ctx, &ctx->tok_ent, reduce_only ? 1 : T));
   A(ws_alloc(ctx, &ctx->tok_conf, reduce_only ? 1 : T));
   A(ws_alloc(ctx, &ctx->tile_base, (int64_t)cfg->max_seqs + 1));
+  A(ws_alloc(ctx, &ctx->seq_done, (int64_t)cfg->max_seqs));
+  if (rc == SQ_OK && cudaMemset(ctx->seq_done, 0, (size_t)cfg->max_seqs * sizeof(int)) != cudaSuccess) rc = SQ_ERR_CUDA;
   A(ws_alloc(ctx, &ctx->red_sum, ctx->red_tiles_max));
   A(ws_alloc(ctx, &ctx->tile_seq, ctx->red_tiles_max));
   A(ws_alloc(ctx, &ctx->red_min, ctx->red_tiles_max));
@@ -297,6 +300,9 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
                            sq::FusedCfg<CG>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
   SQ_SET_SMEM(1, 8) SQ_SET_SMEM(1, 20) SQ_SET_SMEM(1, 32) SQ_SET_SMEM(2, 8) SQ_SET_SMEM(2, 20) SQ_SET_SMEM(2, 32)
 #undef SQ_SET_SMEM
+  for (const void* f : {(const void*)sq::sq_reduce_fused_kernel<true>, (const void*)sq::sq_reduce_fused_kernel<false>})
+    if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             sq::RED_SMEM_BYTES + (sq::RED_FUSED_MAX_SEQS + 1) * (int)sizeof(int)) != cudaSuccess) rc = SQ_ERR_CUDA;
   if (rc != SQ_OK) {
     set_err(nullptr, rc, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize) failed: %s", cudaGetErrorString(cudaGetLastError()));
     sq_score_destroy(ctx);
@@ -364,6 +370,23 @@ static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t s
   // 16-byte loads need 16-byte aligned arrays (tiles start on multiples of 4 tokens)
   rp.vec = ((((uintptr_t)rp.lp | (uintptr_t)rp.ent | (uintptr_t)rp.conf | (uintptr_t)rp.targets) & 15) == 0) ? 1 : 0;
   const int64_t tiles = cdiv64(rp.T, sq::RED_TILE) + 2 * (int64_t)rp.B;   // upper bound on sum_b ceil((L_b + 3) / RED_TILE)
+  // Single launch (sq_reduce_kernel.cuh) when the whole problem is one wave of CTAs -- the scoring pipeline's case, a few
+  // dozen tiles, where the three launches are pure latency (20 -> 8 us).  On large inputs the three-launch form is 2x
+  // faster (measured 0.099 vs 0.218 ms on 3.6e7 tokens: a persistent CTA pays the fence + atomic + barriers per tile in
+  // series), so it stays.  SQ_SCORE_DEBUG bit 5 / bit 6 force the three-launch / single-launch form (tests).
+  const size_t fused_smem = sq::RED_SMEM_BYTES + (size_t)(rp.B + 1) * sizeof(int);
+  const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(6, (size_t)(220 * 1024) / (fused_smem + 1024)));
+  const bool one_wave = tiles <= (int64_t)ctx->num_sms * per_sm && rp.B <= 2048;
+  if (rp.B <= sq::RED_FUSED_MAX_SEQS && !(ctx->debug_flags & 32) && (one_wave || (ctx->debug_flags & 64))) {
+    rp.seq_done = ctx->seq_done;
+    const size_t smem = fused_smem;
+    const dim3 grid((unsigned)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)ctx->num_sms * per_sm)));
+    if (rp.targets) SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_fused_kernel<true>, grid, dim3(sq::RED_THREADS), smem, st, rp));
+    else SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_fused_kernel<false>, grid, dim3(sq::RED_THREADS), smem, st, rp));
+    ctx->launches += 1;
+    SQ_CUDA(ctx, cudaGetLastError());
+    return SQ_OK;
+  }
   SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_tile_scan_kernel, dim3(1), dim3(1024), 0, st, rp));
   ctx->launches += 1;
   if (rp.T > 0) {

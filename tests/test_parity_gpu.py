@@ -326,6 +326,32 @@ def test_full_size_config_sampled_rows_and_all_sequences(name):
 
 
 # ------------------------------------------------------------------------------------------ kernel 2 alone
+def _reduce_both_forms(sq, make_engine, call):
+    """Kernel 2 forced into its single-launch form (SQ_SCORE_DEBUG bit 6) and into its three-launch form (bit 5): the
+    two must agree bit for bit; returns the single-launch outputs."""
+    import os
+    outs = []
+    for dbg in ("64", "32"):
+        os.environ["SQ_SCORE_DEBUG"] = dbg
+        try:
+            eng = make_engine()
+        finally:
+            os.environ.pop("SQ_SCORE_DEBUG", None)
+        n0 = eng.launch_count()
+        o = call(eng)
+        torch.cuda.synchronize()
+        assert eng.launch_count() - n0 == (1 if dbg == "64" else 3)
+        outs.append({n: v.cpu().numpy() for n, v in o.items()})
+        o2 = call(eng)                                   # a second run on the same ctx: the per-sequence counters were reset
+        torch.cuda.synchronize()
+        for n in o:
+            np.testing.assert_array_equal(outs[-1][n], o2[n].cpu().numpy())
+        eng.close()
+    for n in outs[0]:
+        np.testing.assert_array_equal(outs[0][n], outs[1][n])
+    return outs[0]
+
+
 @pytest.mark.parametrize("window", [1, 2, 16, 511, 512, 513, 2048, 4096, 4097, 100000])
 def test_reduce_kernel_alone(window):
     sq = _sq()
@@ -335,13 +361,12 @@ def test_reduce_kernel_alone(window):
     cu = torch.tensor(np.concatenate([[0], np.cumsum(lens)]), dtype=torch.int32)
     lp = -(torch.rand(T, generator=g) * 12); en = torch.rand(T, generator=g) * 11; cf = 3 + torch.rand(T, generator=g) * 12
     cf[30000:30040] = 0.5                      # a dip the minimum window must find
-    eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
     dev = torch.device("cuda:0")
-    out = eng.reduce(lp.to(dev), en.to(dev), cf.to(dev), cu.to(dev), window)
-    torch.cuda.synchronize()
+    a = [x.to(dev) for x in (lp, en, cf, cu)]
+    out = _reduce_both_forms(sq, lambda: sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True),
+                             lambda eng: eng.reduce(a[0], a[1], a[2], a[3], window))
     ref = O.sequence_scores(lp.numpy(), en.numpy(), cf.numpy(), cu.numpy(), window)
-    check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
-    eng.close()
+    check_seqs(out, ref)
 
 
 @pytest.mark.parametrize("offset", [0, 1, 3])
@@ -378,11 +403,24 @@ def test_reduce_alignment_targets_and_array_end(offset, with_targets):
 def test_reduce_many_sequences():
     sq = _sq()
     r = workloads.reduction_inputs(3000, 1, 3000, seed=5)
-    eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True)
     dev = torch.device("cuda:0")
-    out = eng.reduce(r["target_logprob"].to(dev), r["entropy"].to(dev), r["conf"].to(dev), r["cu_seqlens"].to(dev), 256)
-    torch.cuda.synchronize()
+    a = [r[n].to(dev) for n in ("target_logprob", "entropy", "conf", "cu_seqlens")]
+    out = _reduce_both_forms(sq, lambda: sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True),
+                             lambda eng: eng.reduce(a[0], a[1], a[2], a[3], 256))
     ref = O.sequence_scores(r["target_logprob"].numpy(), r["entropy"].numpy(), r["conf"].numpy(), r["cu_seqlens"].numpy(), 256)
+    check_seqs(out, ref)
+
+
+def test_reduce_more_sequences_than_the_single_launch_form_holds():
+    """B = 13 000 > 12 287: the tile table no longer fits in shared memory and the three-launch form runs."""
+    sq = _sq()
+    r = workloads.reduction_inputs(13000, 0, 40, seed=6)
+    dev = torch.device("cuda:0")
+    eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True)
+    out = eng.reduce(r["target_logprob"].to(dev), r["entropy"].to(dev), r["conf"].to(dev), r["cu_seqlens"].to(dev), 7)
+    torch.cuda.synchronize()
+    assert eng.launch_count() == 3
+    ref = O.sequence_scores(r["target_logprob"].numpy(), r["entropy"].numpy(), r["conf"].numpy(), r["cu_seqlens"].numpy(), 7)
     check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
     eng.close()
 
@@ -402,7 +440,7 @@ def test_run_host_matches_run_and_null_per_token_outputs():
     dev_seq = torch.cat([out[n] for n in SEQ_KEYS]).cpu()
     assert torch.equal(dev_seq, host)
     assert torch.equal(dev_seq, torch.cat([out_seq_only[n] for n in SEQ_KEYS]).cpu())
-    assert eng.launch_count() == 15
+    assert eng.launch_count() == 9      # kernel 1, finalize, kernel 2 (single launch) per run
     eng.close()
 
 
