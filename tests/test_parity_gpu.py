@@ -444,6 +444,32 @@ def test_run_host_matches_run_and_null_per_token_outputs():
     eng.close()
 
 
+@pytest.mark.parametrize("T", [2048 * 3 + 17, 2048 * 256 + 5000])
+def test_run_host_streams_h_in_blocks(T):
+    """sq_score_run_host with several arrival flags (and, for the large T, blocks of 4096 rows because a run uses at
+    most 256 flags): H lands while kernel 1 runs; the result must be bit-equal to the device-resident path, twice in a
+    row on the same ctx (the staging buffers and flags are reused)."""
+    sq = _sq()
+    B = 7
+    wl = workloads.custom(name="host_blocks", d=64, V=700, B=B, len_lo=1, len_hi=2, k=5, window=64, seed=43, w_std=0.2)
+    base = T // B
+    lens = [base] * (B - 1) + [T - base * (B - 1)]
+    inp = workloads.make_inputs(wl, lengths=lens)
+    dev = torch.device("cuda:0")
+    eng = sq.SqScore(wl.d, wl.V, max_tokens=T, max_seqs=B, max_k=5)
+    W = inp["W"].to(dev)
+    out = eng.run(inp["H"].to(dev), W, inp["targets"].to(dev), inp["cu_seqlens"].to(dev), 5, 64, per_token=False, topk=False)
+    torch.cuda.synchronize()
+    dev_seq = torch.cat([out[n] for n in SEQ_KEYS]).cpu()
+    Hp, tp, cp = inp["H"].pin_memory(), inp["targets"].pin_memory(), inp["cu_seqlens"].pin_memory()
+    for _ in range(2):
+        host = torch.full((4 * B,), float("nan")).pin_memory()
+        eng.run_host(Hp, W, tp, cp, 5, 64, host)
+        torch.cuda.synchronize()
+        assert torch.equal(dev_seq, host)
+    eng.close()
+
+
 def test_run_rejects_bad_arguments():
     sq = _sq()
     dev = torch.device("cuda:0")
