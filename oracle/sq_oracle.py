@@ -32,7 +32,7 @@ import math
 import numpy as np
 import torch
 
-ORACLE_VERSION = 3
+ORACLE_VERSION = 4
 
 
 def widen(x_bf16: torch.Tensor) -> torch.Tensor:
@@ -271,3 +271,62 @@ def bf16_half_ulp(h64: np.ndarray) -> np.ndarray:
     a = np.abs(h64)
     e = np.floor(np.log2(np.maximum(a, 2.0 ** -126)))
     return 0.5 * 2.0 ** (e - 7)
+
+
+# ------------------------------------------------------------------------------------------------
+# Next row (SURVEY section 8(f)-4, FP8 variant): e4m3 quantisation with per-row / per-tensor scales.
+# The codes are a quantised representation decided by floating point, so the decision is taken in the
+# kernel's precision (fp32) and operation order: inv = 448 / amax; y = x * inv; clamp; round to nearest
+# even e4m3.  Everything after it (the scoring of the dequantised operands) is the fp64 path above.
+# ------------------------------------------------------------------------------------------------
+E4M3_MAX = 448.0
+
+
+def e4m3_values() -> np.ndarray:
+    """The 256 e4m3 ("fn": no infinities, S.1111.111 = NaN) code points as fp64, by their definition:
+    sign, 4 exponent bits (bias 7), 3 mantissa bits; exponent 0 = subnormal (mantissa / 8 * 2^-6)."""
+    vals = np.empty(256)
+    for c in range(256):
+        sgn = -1.0 if c & 0x80 else 1.0
+        e, m = (c >> 3) & 0xF, c & 0x7
+        if e == 0xF and m == 0x7:
+            vals[c] = np.nan
+        elif e == 0:
+            vals[c] = sgn * (m / 8.0) * 2.0 ** -6
+        else:
+            vals[c] = sgn * (1.0 + m / 8.0) * 2.0 ** (e - 7)
+    return vals
+
+
+def round_to_e4m3(y: np.ndarray) -> np.ndarray:
+    """Codes of the e4m3 values nearest to y (|y| <= 448), ties to the even mantissa.  Written as a search
+    over the 127 non-negative code points -- the definition of rounding to nearest -- not a bit trick."""
+    pos = e4m3_values()[:127]                     # codes 0 .. 126 = 0 .. 448 ascending
+    a = np.abs(np.asarray(y, dtype=np.float64))
+    hi = np.searchsorted(pos, a, side="left").clip(1, 126)
+    lo = hi - 1
+    dlo, dhi = a - pos[lo], pos[hi] - a
+    pick_hi = (dhi < dlo) | ((dhi == dlo) & (hi % 2 == 0))   # even code = even mantissa
+    code = np.where(pick_hi, hi, lo).astype(np.uint8)
+    code = np.where(a == 0, 0, code).astype(np.uint8)
+    return np.where(np.signbit(y), code | 0x80, code).astype(np.uint8)
+
+
+def quantize_fp8(X: torch.Tensor, per_tensor: bool):
+    """(codes uint8 [rows, d], scales float32 [rows] or [1]) with x ~= e4m3_values()[code] * scale."""
+    x = X.to(torch.float32).numpy()
+    amax = np.abs(x).max() if per_tensor else np.abs(x).max(axis=1)
+    amax = np.asarray(amax, dtype=np.float32).reshape(-1)
+    ok = amax > 0
+    scale = np.where(ok, (amax / np.float32(E4M3_MAX)).astype(np.float32), np.float32(1)).astype(np.float32)
+    inv = np.where(ok, (np.float32(E4M3_MAX) / np.where(ok, amax, np.float32(1))).astype(np.float32), np.float32(1)).astype(np.float32)
+    y = (x * (inv[0] if per_tensor else inv[:, None])).astype(np.float32)
+    y = np.clip(y, -E4M3_MAX, E4M3_MAX)
+    return round_to_e4m3(y), scale
+
+
+def dequantize_fp8(codes: np.ndarray, scale: np.ndarray) -> torch.Tensor:
+    """fp64 tensor codes * scale (exact: an e4m3 value times an fp32 scale fits fp64)."""
+    v = e4m3_values()[codes]
+    s = np.asarray(scale, dtype=np.float64)
+    return torch.from_numpy(v * (s[0] if s.size == 1 else s[:, None]))

@@ -79,6 +79,11 @@ def lib() -> C.CDLL:
     L.sq_score_merge_shards.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_int32), C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                         C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
     L.sq_score_merge_shards.restype = C.c_int
+    L.sq_score_quantize_fp8.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.sq_score_quantize_fp8.restype = C.c_int
+    L.sq_score_run_fp8.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                   C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
+    L.sq_score_run_fp8.restype = C.c_int
     L.sq_score_plan.argtypes = [C.POINTER(sq_score_config), C.c_int64, C.c_int, C.c_int, C.POINTER(sq_score_plan_t)]
     L.sq_score_plan.restype = C.c_int
     L.sq_score_set_profiling.argtypes = [C.c_void_p, C.c_int]
@@ -242,6 +247,27 @@ class SqScore:
         vs = (C.c_int32 * (R + 1))(*[int(v) for v in vocab_starts])
         self._check(self._L.sq_score_merge_shards(self._h, _ptr(states), R, vs, _ptr(targets), _ptr(cu_seqlens), T, B, k, window,
                                                   C.byref(o), self._stream(stream)))
+        return out
+
+    def quantize_fp8(self, X, per_tensor: bool, stream=None):
+        """sq_score_quantize_fp8: bf16 [rows, d] -> (uint8 e4m3 codes [rows, d], float32 scales [rows] or [1])."""
+        import torch
+        rows = X.shape[0]
+        q = torch.empty(rows, X.shape[1], dtype=torch.uint8, device=X.device)
+        scale = torch.empty(1 if per_tensor else rows, dtype=torch.float32, device=X.device)
+        self._check(self._L.sq_score_quantize_fp8(self._h, _ptr(X), rows, 1 if per_tensor else 0, _ptr(q), _ptr(scale),
+                                                  self._stream(stream)))
+        return q, scale
+
+    def run_fp8(self, Hq, h_scale, Wq, w_scale, targets, cu_seqlens, k: int, window: int, stream=None, per_token: bool = True,
+                topk: bool = True, out: Optional[dict] = None) -> dict:
+        """sq_score_run_fp8: the scoring pass on e4m3 operands with per-token / per-tensor scales."""
+        T, B = Hq.shape[0], cu_seqlens.shape[0] - 1
+        if out is None:
+            out = self._alloc_out(T, B, k, Hq.device, per_token, topk)
+        o = sq_score_outputs(*[_ptr(out.get(n)) for n, _ in sq_score_outputs._fields_])
+        self._check(self._L.sq_score_run_fp8(self._h, _ptr(Hq), _ptr(h_scale), _ptr(Wq), _ptr(w_scale), _ptr(targets), _ptr(cu_seqlens),
+                                             T, B, k, window, C.byref(o), self._stream(stream)))
         return out
 
     def run_host(self, H_host, W_dev, targets_host, cu_seqlens_host, k: int, window: int, seq_out_host, stream=None):

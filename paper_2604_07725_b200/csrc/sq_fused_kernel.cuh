@@ -16,13 +16,14 @@ namespace sq {
 
 constexpr int BLOCK_M = 128;   // token rows per CTA = TMEM lanes
 constexpr int BLOCK_N = 256;   // vocabulary columns per tile = UMMA N
-constexpr int BLOCK_K = 64;    // bf16 per k-block: 128 B = one swizzle-128B row
-constexpr int UMMA_K = 16;
+constexpr int BLOCK_K = 64;    // bf16 per k-block: 128 B = one swizzle-128B row (e4m3: 128 elements, BLOCK_K_F8)
+constexpr int UMMA_K = 16;     // K per MMA instruction: 32 bytes of each operand row (e4m3: 32 elements)
+constexpr int BLOCK_K_F8 = 128;
 constexpr int NUM_THREADS = 256;
 constexpr int EPI_WARP0 = 4;
 constexpr int TMEM_COLS = 512;  // two 256-column accumulator stages
 constexpr float NEG_BIG = -1.0e30f;
-constexpr float LOG2E = 1.4426950408889634f;
+constexpr float LOG2E_F = 1.4426950408889634f;   // consume32 takes log2(e) times the row's dequantisation scale (1 for bf16)
 
 template <int CG> struct FusedCfg {
   static constexpr int A_BYTES = BLOCK_M * BLOCK_K * 2;                 // 16 KB
@@ -65,6 +66,8 @@ struct FusedParams {
   int thr_j, thr_ns;        //   every chunk publishes its thr_j-th best; the bound is the thr_ns-th SMALLEST published value
   const unsigned int* h_ready;   // null, or flags set as H arrives from the host (sq_score_run_host): flag f != 0
   int flag_rows;                 //   <=> rows [0, (f+1) * flag_rows) of H are in device memory
+  const float* h_scale;     // FP8 variant: H = Hq * h_scale[row], W = Wq * (*w_scale) with Hq, Wq e4m3 (per-row / per-tensor
+  const float* w_scale;     //   scales, DEVICE); null in the bf16 path
   int vocab_offset;         // W is rows [vocab_offset, vocab_offset + V) of a larger LM head (vocab-parallel shard):
                             // targets and the reported vocabulary ids are global, columns local
   int debug_flags;          // experiments only (env SQ_SCORE_DEBUG): bit0 = epilogue skips the statistics,
@@ -208,7 +211,7 @@ template <int CAP> struct RowState {
 
 // Consumes 32 consecutive logits of one row (columns col0 .. col0+31).
 template <int CAP>
-__device__ __forceinline__ void consume32(RowState<CAP>& st, float (&r)[32], int col0, int V, int tgt) {
+__device__ __forceinline__ void consume32(RowState<CAP>& st, float (&r)[32], int col0, int V, int tgt, const float LOG2E) {
   if (col0 + 32 > V) {   // ragged vocabulary tail: columns >= V hold TMA zero fill
 #pragma unroll
     for (int i = 0; i < 32; ++i) r[i] = (col0 + i < V) ? r[i] : NEG_BIG;
@@ -266,7 +269,11 @@ __device__ __forceinline__ void consume32(RowState<CAP>& st, float (&r)[32], int
   }
 }
 
-template <int CG, int CAP>
+// F8: operands are e4m3 bytes (tcgen05 kind::f8f6f4, 128 elements per 128-byte k-block row); the accumulator is
+// Hq.Wq^T and the epilogue works in those units with log2(e) * h_scale[row] * w_scale folded into the exponent's
+// multiplier, so the dequantisation costs no instruction per logit; m, u, the list values and the target logit are
+// scaled once per row when the partial state is written.
+template <int CG, int CAP, bool F8 = false>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_constant__ CUtensorMap tmap_w,
                       const FusedParams p) {
@@ -316,6 +323,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
   const int rows_per_unit = BLOCK_M * CG;
+  constexpr int BK = F8 ? BLOCK_K_F8 : BLOCK_K;   // elements per k-block (128 bytes of every operand row)
 
   if (warp == 0) {
     // ===================================================================== TMA producer
@@ -341,13 +349,13 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
             mbar_wait(empty_bar(stage), phase ^ 1u);
             if constexpr (CG == 1) {
               mbar_arrive_expect_tx(full_bar(stage), stage_tx);
-              tma_load_2d(smem_a(stage), &tmap_h, full_bar(stage), kb * BLOCK_K, row0);
-              tma_load_2d(smem_b(stage), &tmap_w, full_bar(stage), kb * BLOCK_K, wrow0);
+              tma_load_2d(smem_a(stage), &tmap_h, full_bar(stage), kb * BK, row0);
+              tma_load_2d(smem_b(stage), &tmap_w, full_bar(stage), kb * BK, wrow0);
             } else {
               const uint32_t bar = mapa(full_bar(stage), 0);
               if (leader) mbar_arrive_expect_tx(full_bar(stage), stage_tx);
-              tma_load_2d_pair(smem_a(stage), &tmap_h, bar, kb * BLOCK_K, row0);
-              tma_load_2d_pair(smem_b(stage), &tmap_w, bar, kb * BLOCK_K, wrow0);
+              tma_load_2d_pair(smem_a(stage), &tmap_h, bar, kb * BK, row0);
+              tma_load_2d_pair(smem_b(stage), &tmap_w, bar, kb * BK, wrow0);
             }
             if (++stage == Cfg::STAGES) { stage = 0; phase ^= 1u; }
           }
@@ -357,7 +365,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   } else if (warp == 1) {
     // ===================================================================== MMA issuer (pair leader only)
     if (leader && lane == 0) {
-      constexpr uint32_t idesc = make_idesc_bf16(Cfg::UMMA_M, BLOCK_N);
+      constexpr uint32_t idesc = F8 ? make_idesc_e4m3(Cfg::UMMA_M, BLOCK_N) : make_idesc_bf16(Cfg::UMMA_M, BLOCK_N);
       int stage = 0; uint32_t phase = 0;
       uint32_t tile = 0;
       for (int gu = gc.gu0; gu < gc.gu_end; gu += gc.gu_step) {
@@ -378,7 +386,8 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
 #pragma unroll
             for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
               // +32 B per UMMA_K step inside the 128-B swizzle row: +2 in the (addr >> 4) field
-              umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+              if constexpr (F8) umma_f8<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+              else umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
             }
             umma_commit<CG>(empty_bar(stage));   // smem slot free once these MMAs retire
             if (++stage == Cfg::STAGES) { stage = 0; phase ^= 1u; }
@@ -404,6 +413,9 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
       int tgt = (row < p.T) ? __ldg(p.targets + row) : -1;
       tgt = (tgt >= p.vocab_offset) ? tgt - p.vocab_offset : -1;   // local column, or out of range
       st.reset();
+      float deq = 1.f;                             // F8: accumulator units -> logits for this row
+      if constexpr (F8) deq = ((row < p.T) ? __ldg(p.h_scale + row) : 1.f) * __ldg(p.w_scale);
+      const float l2e = F8 ? LOG2E_F * deq : LOG2E_F;
       for (int vt = vt0; vt < vt1; ++vt, ++tile) {
         const uint32_t acc = tile & 1u;
         mbar_wait(tfull_bar(acc), (tile >> 1) & 1u);
@@ -414,7 +426,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
           float r[32];
           tmem_ld_32x32(lane_addr + acc * BLOCK_N + g * 32, r);
           tmem_ld_wait();
-          consume32<CAP>(st, r, colbase + g * 32, p.V, tgt);
+          consume32<CAP>(st, r, colbase + g * 32, p.V, tgt, l2e);
         }
         tc_fence_before();
         __syncwarp();
@@ -427,19 +439,19 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
       }
       if (row < p.T) {
         const size_t o = (size_t)un.chunk * p.T + row;
-        p.part_m[o] = st.m;
+        p.part_m[o] = st.m * deq;                  // deq == 1 in the bf16 path: exact
         p.part_s[o] = st.s;
-        p.part_u[o] = st.u;
+        p.part_u[o] = st.u * deq;
         p.part_cs[o] = st.cs;
-        p.part_cu[o] = st.cu;
+        p.part_cu[o] = st.cu * deq;
 #pragma unroll
         for (int j = 0; j < CAP; ++j) {
           const size_t oj = ((size_t)un.chunk * CAP + j) * p.T + row;
-          p.part_topv[oj] = st.tv[j];
+          p.part_topv[oj] = st.tv[j] * deq;
           p.part_topi[oj] = st.ti[j] < 0 ? -1 : st.ti[j] + p.vocab_offset;
         }
         const int c0 = vt0 * BLOCK_N;
-        if (tgt >= c0 && tgt < min(vt1 * BLOCK_N, p.V)) p.zt[row] = st.zt;
+        if (tgt >= c0 && tgt < min(vt1 * BLOCK_N, p.V)) p.zt[row] = st.zt * deq;
       }
     }
   }

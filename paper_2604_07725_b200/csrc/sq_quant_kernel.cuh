@@ -1,0 +1,96 @@
+// sq_quant_kernel.cuh -- e4m3 quantisation for the FP8 variant of the scoring pass.
+//
+//   q[r, j] = e4m3_rn_sat( x[r, j] * (448 / amax) ),   scale = amax / 448,   x ~= q * scale
+//
+// amax is taken per row (H: one scale per token, applied for free in kernel 1's epilogue) or over the whole tensor
+// (W: one scale for the LM head, so that no per-column multiply is needed per logit).  fp32 arithmetic with _rn
+// intrinsics in a fixed order (inv = 448 / amax; y = x * inv; clamp; convert), mirrored operation by operation by the
+// oracle, so the bytes are bit-identical.  amax == 0 gives scale 1 and all-zero codes.  HBM-bound: 2 B read + 1 B
+// written per element (per-tensor mode reads the tensor twice: amax pass, then quantise).
+#pragma once
+#include <cuda_fp8.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace sq {
+
+constexpr int QUANT_WARPS = 8;
+constexpr float E4M3_MAX = 448.0f;
+
+struct QuantParams {
+  const uint4* X;        // bf16 [rows, d] as 16-byte vectors (8 elements)
+  uint2* Q;              // e4m3 [rows, d] as 8-byte vectors (8 elements)
+  float* scale;          // per-row: [rows] written; per-tensor: [1] written by sq_quant_scale_kernel, read here
+  unsigned int* amax_bits;   // per-tensor: running max of |x| as fp32 bits (non-negative floats order like uints)
+  long long rows;
+  int d;
+  int per_tensor;
+};
+
+__device__ __forceinline__ void q_unpack8(const uint4& v, float (&f)[8]) {
+  const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    f[2 * i] = __uint_as_float(w[i] << 16);
+    f[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+  }
+}
+__device__ __forceinline__ float q_amax8(const uint4& v) {
+  float f[8];
+  q_unpack8(v, f);
+  float m = 0.f;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) m = fmaxf(m, fabsf(f[i]));
+  return m;
+}
+__device__ __forceinline__ uint32_t q_code(float x, float inv) {
+  const float y = fminf(fmaxf(__fmul_rn(x, inv), -E4M3_MAX), E4M3_MAX);
+  return (uint32_t)__nv_cvt_float_to_fp8(y, __NV_SATFINITE, __NV_E4M3);
+}
+__device__ __forceinline__ uint2 q_pack8(const uint4& v, float inv) {
+  float f[8];
+  q_unpack8(v, f);
+  uint2 o;
+  o.x = q_code(f[0], inv) | (q_code(f[1], inv) << 8) | (q_code(f[2], inv) << 16) | (q_code(f[3], inv) << 24);
+  o.y = q_code(f[4], inv) | (q_code(f[5], inv) << 8) | (q_code(f[6], inv) << 16) | (q_code(f[7], inv) << 24);
+  return o;
+}
+
+// per-tensor pass 1: amax over everything
+__global__ void __launch_bounds__(256) sq_quant_amax_kernel(const QuantParams p) {
+  const long long nvec = p.rows * (p.d >> 3);
+  float m = 0.f;
+  for (long long v = (long long)blockIdx.x * 256 + threadIdx.x; v < nvec; v += (long long)gridDim.x * 256) m = fmaxf(m, q_amax8(p.X[v]));
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, off));
+  if ((threadIdx.x & 31) == 0) atomicMax(p.amax_bits, __float_as_uint(m));
+}
+// per-tensor pass 1b: the scale from the amax
+__global__ void sq_quant_scale_kernel(const QuantParams p) {
+  const float amax = __uint_as_float(*p.amax_bits);
+  p.scale[0] = amax > 0.f ? __fdiv_rn(amax, E4M3_MAX) : 1.f;
+}
+
+// quantise: one warp per row (per-row mode computes the row's amax first; the row is re-read from L1/L2)
+__global__ void __launch_bounds__(QUANT_WARPS * 32) sq_quant_rows_kernel(const QuantParams p) {
+  const int lane = threadIdx.x & 31;
+  const int nvec = p.d >> 3;
+  float amax_t = 0.f;
+  if (p.per_tensor) amax_t = __uint_as_float(*p.amax_bits);
+  for (long long r = (long long)blockIdx.x * QUANT_WARPS + (threadIdx.x >> 5); r < p.rows; r += (long long)gridDim.x * QUANT_WARPS) {
+    const uint4* x = p.X + r * nvec;
+    float amax = amax_t;
+    if (!p.per_tensor) {
+      amax = 0.f;
+      for (int v = lane; v < nvec; v += 32) amax = fmaxf(amax, q_amax8(x[v]));
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, off));
+      if (lane == 0) p.scale[r] = amax > 0.f ? __fdiv_rn(amax, E4M3_MAX) : 1.f;
+    }
+    const float inv = amax > 0.f ? __fdiv_rn(E4M3_MAX, amax) : 1.f;
+    uint2* q = p.Q + r * nvec;
+    for (int v = lane; v < nvec; v += 32) q[v] = q_pack8(x[v], inv);
+  }
+}
+
+}  // namespace sq

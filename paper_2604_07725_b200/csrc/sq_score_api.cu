@@ -16,6 +16,7 @@
 #include "sq_finalize_kernel.cuh"
 #include "sq_fused_kernel.cuh"
 #include "sq_prepare_kernel.cuh"
+#include "sq_quant_kernel.cuh"
 #include "sq_reduce_kernel.cuh"
 #include "sq_route_kernel.cuh"
 
@@ -37,6 +38,7 @@ struct sq_score_ctx {
   // per-token scratch (used when the caller passes NULL per-token outputs)
   float* tok_lse = nullptr; float* tok_lp = nullptr; float* tok_ent = nullptr; float* tok_conf = nullptr;
   // kernel 2 workspace
+  unsigned int* amax_bits = nullptr;   // per-tensor amax of sq_score_quantize_fp8
   int* seq_done = nullptr;   // [max_seqs] per-sequence tile counters of the single-launch reduction (zero between runs)
   int* tile_base = nullptr; int* tile_seq = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
   // staging for sq_score_run_host
@@ -186,7 +188,7 @@ static int64_t ws_rows_for(const sq_score_config& cfg) {
 extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
   if (!ctx) return SQ_OK;
   cudaSetDevice(ctx->cfg.device);
-  void* bufs[] = {ctx->seq_done, ctx->thr_pub, ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
+  void* bufs[] = {ctx->amax_bits, ctx->seq_done, ctx->thr_pub, ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
                   ctx->tok_lse, ctx->tok_lp, ctx->tok_ent, ctx->tok_conf, ctx->tile_base, ctx->tile_seq, ctx->red_sum,
                   ctx->red_min, ctx->h_stage, ctx->tgt_stage, ctx->cu_stage, ctx->seq_stage};
   int rc = SQ_OK;
@@ -283,6 +285,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   A(ws_alloc(ctx, &ctx->tok_ent, reduce_only ? 1 : T));
   A(ws_alloc(ctx, &ctx->tok_conf, reduce_only ? 1 : T));
   A(ws_alloc(ctx, &ctx->tile_base, (int64_t)cfg->max_seqs + 1));
+  A(ws_alloc(ctx, &ctx->amax_bits, 1));
   A(ws_alloc(ctx, &ctx->seq_done, (int64_t)cfg->max_seqs));
   if (rc == SQ_OK && cudaMemset(ctx->seq_done, 0, (size_t)cfg->max_seqs * sizeof(int)) != cudaSuccess) rc = SQ_ERR_CUDA;
   A(ws_alloc(ctx, &ctx->red_sum, ctx->red_tiles_max));
@@ -300,6 +303,11 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
                            sq::FusedCfg<CG>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
   SQ_SET_SMEM(1, 8) SQ_SET_SMEM(1, 20) SQ_SET_SMEM(1, 32) SQ_SET_SMEM(2, 8) SQ_SET_SMEM(2, 20) SQ_SET_SMEM(2, 32)
 #undef SQ_SET_SMEM
+#define SQ_SET_SMEM8(CG, CAP)                                                                                      \
+  if (cudaFuncSetAttribute(sq::sq_fused_score_kernel<CG, CAP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+                           sq::FusedCfg<CG>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
+  SQ_SET_SMEM8(1, 8) SQ_SET_SMEM8(1, 20) SQ_SET_SMEM8(1, 32) SQ_SET_SMEM8(2, 8) SQ_SET_SMEM8(2, 20) SQ_SET_SMEM8(2, 32)
+#undef SQ_SET_SMEM8
   for (const void* f : {(const void*)sq::sq_reduce_fused_kernel<true>, (const void*)sq::sq_reduce_fused_kernel<false>})
     if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              sq::RED_SMEM_BYTES + (sq::RED_FUSED_MAX_SEQS + 1) * (int)sizeof(int)) != cudaSuccess) rc = SQ_ERR_CUDA;
@@ -319,13 +327,13 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
 
 // bf16 [rows, d] row-major -> boxes of {64 columns (128 B, swizzle-128B), box_rows rows}; out-of-range
 // rows and columns are zero filled.
-static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int d, int box_rows) {
+static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int d, int box_rows, bool f8 = false) {
   const cuuint64_t dims[2] = {(cuuint64_t)d, (cuuint64_t)rows};
-  const cuuint64_t strides[1] = {(cuuint64_t)d * 2};
-  const cuuint32_t box[2] = {(cuuint32_t)sq::BLOCK_K, (cuuint32_t)box_rows};
+  const cuuint64_t strides[1] = {(cuuint64_t)d * (f8 ? 1 : 2)};
+  const cuuint32_t box[2] = {(cuuint32_t)(f8 ? sq::BLOCK_K_F8 : sq::BLOCK_K), (cuuint32_t)box_rows};   // 128 bytes wide
   const cuuint32_t estr[2] = {1, 1};
   CUresult r = reinterpret_cast<encode_tiled_fn>(ctx->encode_fn)(
-      map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+      map, f8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return set_err(ctx, SQ_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
@@ -333,7 +341,7 @@ static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int6
 }
 
 // ------------------------------------------------------------------------------------------ launches
-template <int CG, int CAP>
+template <int CG, int CAP, bool F8 = false>
 static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CUtensorMap& th, const CUtensorMap& tw,
                                 const sq::FusedParams& fp, cudaStream_t st) {
   // every launched cluster belongs to a gang; gang B is launched only if it was given token tiles
@@ -349,7 +357,7 @@ static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CU
   lc.attrs = at;
   lc.numAttrs = 1;
   (void)num_sms;
-  return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP>, th, tw, fp);
+  return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP, F8>, th, tw, fp);
 }
 
 // Launch with programmatic stream serialization: the kernel is scheduled while its predecessor drains and waits in
@@ -454,7 +462,8 @@ static void set_state_pointers(sq::FinalizeParams& f, float* base, int64_t T, in
 static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32_t* targets,
                     const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k, int window,
                     const sq_score_outputs* o, void* stream, const unsigned int* h_ready, int flag_rows,
-                    int vocab_offset = 0, float* shard_state = nullptr) {
+                    int vocab_offset = 0, float* shard_state = nullptr, const float* h_scale = nullptr,
+                    const float* w_scale = nullptr) {
   if (!ctx) return SQ_ERR_INVALID_ARG;
   if (!o && !shard_state) return set_err(ctx, SQ_ERR_INVALID_ARG, "outputs is null");
   static const sq_score_outputs no_outputs = {};
@@ -481,8 +490,10 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
   float* conf = o->conf ? o->conf : ctx->tok_conf;
 
   if (T > 0) {
+    const bool f8 = h_scale != nullptr;
     sq_score_plan_t pl;
     sq_score_config pc = ctx->cfg;
+    if (f8) pc.d = (d + 1) / 2;   // an e4m3 k-block is 128 elements: the plan sees half as many k-blocks
     make_plan(&pc, T, k, ctx->num_sms, &pl);
     const int64_t rows = ws_rows_for(ctx->cfg);
     if ((int64_t)pl.num_chunks * T > rows) {   // workspace bound: fewer, longer chunks
@@ -491,9 +502,10 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     }
     if (pl.topk_cap > ctx->cap_max) return set_err(ctx, SQ_ERR_INVALID_ARG, "k exceeds the ctx's max_k capacity");
     CUtensorMap th, tw;
-    int rc = make_tmap(ctx, &th, H, T, d, (ctx->debug_flags & 4) ? sq::BLOCK_M / 2 : sq::BLOCK_M);
+    if (f8 && d % 16 != 0) return set_err(ctx, SQ_ERR_UNSUPPORTED, "the FP8 variant needs d %% 16 == 0 (TMA 16-byte row strides)");
+    int rc = make_tmap(ctx, &th, H, T, d, (ctx->debug_flags & 4) ? sq::BLOCK_M / 2 : sq::BLOCK_M, f8);
     if (rc != SQ_OK) return rc;
-    rc = make_tmap(ctx, &tw, W, V, d, (sq::BLOCK_N / pl.cta_group) / ((ctx->debug_flags & 2) ? 2 : 1));
+    rc = make_tmap(ctx, &tw, W, V, d, (sq::BLOCK_N / pl.cta_group) / ((ctx->debug_flags & 2) ? 2 : 1), f8);
     if (rc != SQ_OK) return rc;
 
     sq::FusedParams fp = {};
@@ -509,6 +521,7 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fp.part_topv = ctx->part_topv; fp.part_topi = ctx->part_topi; fp.zt = ctx->zt;
     fp.debug_flags = ctx->debug_flags;
     fp.vocab_offset = vocab_offset;
+    fp.h_scale = h_scale; fp.w_scale = w_scale;
     fp.h_ready = h_ready; fp.flag_rows = flag_rows;
     if (pl.num_chunks >= 2 && pl.num_chunks <= THR_MAX_CHUNKS && !(ctx->debug_flags & 16)) {
       // every chunk publishes its j-th best, j one of cap/4, cap/2, cap (compile-time list slots); r = ceil(k / j)
@@ -525,8 +538,14 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     }
     cudaError_t e;
     if (ctx->profiling) cudaEventRecord(ctx->ev[0], st);
-    const int sel = pl.cta_group * 100 + pl.topk_cap;
+    const int sel = pl.cta_group * 100 + pl.topk_cap + (f8 ? 1000 : 0);
     switch (sel) {
+      case 1108: e = launch_fused<1, 8, true>(pl, ctx->num_sms, th, tw, fp, st); break;
+      case 1120: e = launch_fused<1, 20, true>(pl, ctx->num_sms, th, tw, fp, st); break;
+      case 1132: e = launch_fused<1, 32, true>(pl, ctx->num_sms, th, tw, fp, st); break;
+      case 1208: e = launch_fused<2, 8, true>(pl, ctx->num_sms, th, tw, fp, st); break;
+      case 1220: e = launch_fused<2, 20, true>(pl, ctx->num_sms, th, tw, fp, st); break;
+      case 1232: e = launch_fused<2, 32, true>(pl, ctx->num_sms, th, tw, fp, st); break;
       case 108: e = launch_fused<1, 8>(pl, ctx->num_sms, th, tw, fp, st); break;
       case 120: e = launch_fused<1, 20>(pl, ctx->num_sms, th, tw, fp, st); break;
       case 132: e = launch_fused<1, 32>(pl, ctx->num_sms, th, tw, fp, st); break;
@@ -578,6 +597,41 @@ extern "C" int sq_score_run(sq_score_ctx* ctx, const void* H, const void* W, con
                             const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k, int window,
                             const sq_score_outputs* o, void* stream) {
   return run_impl(ctx, H, W, targets, cu_seqlens, num_tokens, num_seqs, k, window, o, stream, nullptr, 0);
+}
+
+// ------------------------------------------------------------------------------------------ FP8 variant (8(f)-4)
+extern "C" int sq_score_quantize_fp8(sq_score_ctx* ctx, const void* X, int64_t num_rows, int per_tensor, void* q_out,
+                                     float* scale_out, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (num_rows < 0) return set_err(ctx, SQ_ERR_INVALID_ARG, "negative row count");
+  if (num_rows == 0) return SQ_OK;
+  if (!X || !q_out || !scale_out) return set_err(ctx, SQ_ERR_INVALID_ARG, "null pointer argument");
+  if (((uintptr_t)X & 15) || ((uintptr_t)q_out & 7)) return set_err(ctx, SQ_ERR_INVALID_ARG, "X must be 16-byte and q_out 8-byte aligned");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  sq::QuantParams qp = {};
+  qp.X = static_cast<const uint4*>(X); qp.Q = static_cast<uint2*>(q_out); qp.scale = scale_out;
+  qp.amax_bits = ctx->amax_bits; qp.rows = num_rows; qp.d = ctx->cfg.d; qp.per_tensor = per_tensor ? 1 : 0;
+  const unsigned ctas = (unsigned)std::min<int64_t>(cdiv64(num_rows, sq::QUANT_WARPS), (int64_t)ctx->num_sms * 8);
+  if (per_tensor) {
+    SQ_CUDA(ctx, cudaMemsetAsync(ctx->amax_bits, 0, sizeof(unsigned int), st));
+    sq::sq_quant_amax_kernel<<<(unsigned)ctx->num_sms * 8, 256, 0, st>>>(qp);
+    sq::sq_quant_scale_kernel<<<1, 1, 0, st>>>(qp);
+    ctx->launches += 2;
+  }
+  sq::sq_quant_rows_kernel<<<ctas, sq::QUANT_WARPS * 32, 0, st>>>(qp);
+  ctx->launches += 1;
+  SQ_CUDA(ctx, cudaGetLastError());
+  return SQ_OK;
+}
+
+extern "C" int sq_score_run_fp8(sq_score_ctx* ctx, const void* Hq, const float* h_scale, const void* Wq, const float* w_scale,
+                                const int32_t* targets, const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k,
+                                int window, const sq_score_outputs* outputs, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (num_tokens > 0 && (!h_scale || !w_scale)) return set_err(ctx, SQ_ERR_INVALID_ARG, "h_scale and w_scale are required");
+  return run_impl(ctx, Hq, Wq, targets, cu_seqlens, num_tokens, num_seqs, k, window, outputs, stream, nullptr, 0, 0, nullptr,
+                  h_scale, w_scale);
 }
 
 // ------------------------------------------------------------------------------------------ vocab-parallel (8(f)-4)
