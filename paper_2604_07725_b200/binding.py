@@ -249,12 +249,16 @@ class SqScore:
                                                   C.byref(o), self._stream(stream)))
         return out
 
-    def quantize_fp8(self, X, per_tensor: bool, stream=None):
-        """sq_score_quantize_fp8: bf16 [rows, d] -> (uint8 e4m3 codes [rows, d], float32 scales [rows] or [1])."""
+    def quantize_fp8(self, X, per_tensor: bool, stream=None, out=None):
+        """sq_score_quantize_fp8: bf16 [rows, d] -> (uint8 e4m3 codes [rows, d], float32 scales [rows] or [1]);
+        `out` = (codes, scales) reuses the tensors of an earlier call."""
         import torch
         rows = X.shape[0]
-        q = torch.empty(rows, X.shape[1], dtype=torch.uint8, device=X.device)
-        scale = torch.empty(1 if per_tensor else rows, dtype=torch.float32, device=X.device)
+        if out is not None:
+            q, scale = out
+        else:
+            q = torch.empty(rows, X.shape[1], dtype=torch.uint8, device=X.device)
+            scale = torch.empty(1 if per_tensor else rows, dtype=torch.float32, device=X.device)
         self._check(self._L.sq_score_quantize_fp8(self._h, _ptr(X), rows, 1 if per_tensor else 0, _ptr(q), _ptr(scale),
                                                   self._stream(stream)))
         return q, scale

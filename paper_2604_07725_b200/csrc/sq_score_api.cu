@@ -619,7 +619,14 @@ extern "C" int sq_score_quantize_fp8(sq_score_ctx* ctx, const void* X, int64_t n
     sq::sq_quant_scale_kernel<<<1, 1, 0, st>>>(qp);
     ctx->launches += 2;
   }
-  sq::sq_quant_rows_kernel<<<ctas, sq::QUANT_WARPS * 32, 0, st>>>(qp);
+  const unsigned ctas_reg = (unsigned)std::min<int64_t>(cdiv64(num_rows, sq::QUANT_REG_WARPS), (int64_t)ctx->num_sms * 8);
+  const int nv = (int)cdiv64(qp.d, 256);
+  if (nv <= 4) sq::sq_quant_rows_reg_kernel<4><<<ctas_reg, sq::QUANT_REG_WARPS * 32, 0, st>>>(qp);
+  else if (nv <= 8) sq::sq_quant_rows_reg_kernel<8><<<ctas_reg, sq::QUANT_REG_WARPS * 32, 0, st>>>(qp);
+  else if (nv <= 12) sq::sq_quant_rows_reg_kernel<12><<<ctas_reg, sq::QUANT_REG_WARPS * 32, 0, st>>>(qp);
+  else if (nv <= 16) sq::sq_quant_rows_reg_kernel<16><<<ctas_reg, sq::QUANT_REG_WARPS * 32, 0, st>>>(qp);
+  else if (nv <= 24) sq::sq_quant_rows_reg_kernel<24><<<ctas_reg, sq::QUANT_REG_WARPS * 32, 0, st>>>(qp);
+  else sq::sq_quant_rows_kernel<<<ctas, sq::QUANT_WARPS * 32, 0, st>>>(qp);   // d > 6144
   ctx->launches += 1;
   SQ_CUDA(ctx, cudaGetLastError());
   return SQ_OK;
