@@ -51,13 +51,19 @@ constexpr int FIN_MAX_CHUNKS = 32 * FIN_MAX_NL;    // 160 vocab chunks per row a
 // NL = lists (vocab chunks) per lane: 1 for the prefill-shaped plans (num_chunks <= 32), FIN_MAX_NL otherwise.
 // EMIT = write the merged state of this shard (m, s, u with their residues, k-entry list, target logit) for the
 // vocab-parallel exchange instead of the final per-token outputs.
-template <int NL, bool EMIT>
+// LPR = lanes per row: 32 (one warp per row), or 8 when there are at most 8 chunks (the large prefill plans: 6), so
+// that a warp merges four rows at once and the k rounds of arg-max shuffles are shared by four times as many rows.
+template <int NL, bool EMIT, int LPR = 32>
 __global__ void __launch_bounds__(FIN_WARPS * 32)
 sq_finalize_kernel(const FinalizeParams p) {
+  static_assert(LPR == 32 || (LPR == 8 && NL == 1), "8 lanes per row needs one list per lane");
   cudaGridDependencySynchronize();   // launched with programmatic serialization behind kernel 1 (or stand-alone: no-op)
-  const int lane = threadIdx.x & 31;
-  const int row = blockIdx.x * FIN_WARPS + (threadIdx.x >> 5);
-  if (row >= p.T) return;
+  constexpr int RPW = 32 / LPR;      // rows per warp
+  const int lane = (threadIdx.x & 31) % LPR;   // position inside the row's lane group = chunk index (+ 32 i)
+  const int row_raw = (blockIdx.x * FIN_WARPS + (threadIdx.x >> 5)) * RPW + (threadIdx.x & 31) / LPR;
+  if ((blockIdx.x * FIN_WARPS + (threadIdx.x >> 5)) * RPW >= p.T) return;   // the whole warp is past the end
+  const bool live = row_raw < p.T;   // lanes of a dead row still take part in the shuffles, on row T-1's data
+  const int row = live ? row_raw : p.T - 1;
   const unsigned FULL = 0xffffffffu;
   const float NEG = -1.0e30f;
   // lane owns chunks lane, lane + 32, ... (one per lane in the prefill-shaped plans, up to
@@ -77,7 +83,7 @@ sq_finalize_kernel(const FinalizeParams p) {
     if (c < p.num_chunks) M = fmaxf(M, p.part_m[base1[i]]);
   }
 #pragma unroll
-  for (int off = 16; off > 0; off >>= 1) M = fmaxf(M, __shfl_xor_sync(FULL, M, off));
+  for (int off = LPR / 2; off > 0; off >>= 1) M = fmaxf(M, __shfl_xor_sync(FULL, M, off));
   // the merge runs in fp64: S - 1 of a peaked row is ~1e-4 and carries the whole entropy
   double S = 0.0, U = 0.0;
 #pragma unroll
@@ -94,7 +100,7 @@ sq_finalize_kernel(const FinalizeParams p) {
     }
   }
 #pragma unroll
-  for (int off = 16; off > 0; off >>= 1) {
+  for (int off = LPR / 2; off > 0; off >>= 1) {
     S += __shfl_xor_sync(FULL, S, off);
     U += __shfl_xor_sync(FULL, U, off);
   }
@@ -127,13 +133,23 @@ sq_finalize_kernel(const FinalizeParams p) {
       if (hv[i] > lv || (hv[i] == lv && hi[i] < li)) { lv = hv[i]; li = hi[i]; }
     float bv = lv; int bi = li;
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
+    for (int off = LPR / 2; off > 0; off >>= 1) {
       const float ov = __shfl_xor_sync(FULL, bv, off);
       const int oi = __shfl_xor_sync(FULL, bi, off);
       if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
     }
     acc += bv;
-    if (lane == j) { my_v = bv; my_i = bi; }
+    if constexpr (LPR == 32) {
+      if (lane == j) { my_v = bv; my_i = bi; }
+    } else if (lane == (j & (LPR - 1)) && live) {   // too few lanes to park k winners: store the j-th right away
+      if (EMIT) {
+        p.out_topv[(size_t)j * p.T + row] = bv;
+        p.out_topi[(size_t)j * p.T + row] = bv > NEG ? bi : -1;
+      } else {
+        if (p.topk_logprob) p.topk_logprob[(size_t)row * p.k + j] = bv - lse;
+        if (p.topk_index) p.topk_index[(size_t)row * p.k + j] = bi;
+      }
+    }
     if (li == bi && lv == bv) {   // vocabulary ids are unique: exactly one list of one lane advances
 #pragma unroll
       for (int i = 0; i < NL; ++i)
@@ -142,11 +158,18 @@ sq_finalize_kernel(const FinalizeParams p) {
   }
   if (EMIT) {
     // the shard's merged state, one chunk: s and u keep their fp64 precision as value + residue (true = s - cs)
-    if (lane < p.cap) {
-      p.out_topv[(size_t)lane * p.T + row] = lane < p.k ? my_v : NEG;
-      p.out_topi[(size_t)lane * p.T + row] = (lane < p.k && my_v > NEG) ? my_i : -1;
+    if constexpr (LPR == 32) {
+      if (lane < p.cap) {
+        p.out_topv[(size_t)lane * p.T + row] = lane < p.k ? my_v : NEG;
+        p.out_topi[(size_t)lane * p.T + row] = (lane < p.k && my_v > NEG) ? my_i : -1;
+      }
+    } else if (live) {
+      for (int j = p.k + lane; j < p.cap; j += LPR) {   // the list slots past k are empty
+        p.out_topv[(size_t)j * p.T + row] = NEG;
+        p.out_topi[(size_t)j * p.T + row] = -1;
+      }
     }
-    if (lane == 0) {
+    if (lane == 0 && live) {
       const float s_hi = (float)S, u_hi = (float)U;
       p.out_m[row] = M;
       p.out_s[row] = s_hi; p.out_cs[row] = (float)((double)s_hi - S);
@@ -155,11 +178,13 @@ sq_finalize_kernel(const FinalizeParams p) {
     }
     return;
   }
-  if (lane < p.k) {
-    if (p.topk_logprob) p.topk_logprob[(size_t)row * p.k + lane] = my_v - lse;
-    if (p.topk_index) p.topk_index[(size_t)row * p.k + lane] = my_i;
+  if constexpr (LPR == 32) {
+    if (lane < p.k) {
+      if (p.topk_logprob) p.topk_logprob[(size_t)row * p.k + lane] = my_v - lse;
+      if (p.topk_index) p.topk_index[(size_t)row * p.k + lane] = my_i;
+    }
   }
-  if (lane == 0) {
+  if (lane == 0 && live) {
     const int tgt = p.targets[row];
     const bool valid = (tgt >= 0) && (tgt < p.V);
     size_t zo = row;

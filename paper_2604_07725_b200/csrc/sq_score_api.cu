@@ -566,7 +566,14 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
     fin.chunks_per_rank = pl.num_chunks; fin.rank_stride = 0; fin.num_ranks = 1;
     const dim3 fgrid((unsigned)cdiv64(T, sq::FIN_WARPS)), fblock(sq::FIN_WARPS * 32);
-    if (shard_state) {   // vocab-parallel shard: the merged state goes out in the packed exchange layout
+    const dim3 fgrid8((unsigned)cdiv64(T, sq::FIN_WARPS * 4));   // 8 lanes per row: four rows per warp
+    const bool lpr8 = pl.num_chunks <= 8 && !(ctx->debug_flags & 128);
+    if (shard_state && lpr8) {
+      set_state_pointers(fin, shard_state, T, pl.topk_cap, /*as_output=*/true);
+      SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, true, 8>, fgrid8, fblock, 0, st, fin));
+    } else if (!shard_state && lpr8) {
+      SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, false, 8>, fgrid8, fblock, 0, st, fin));
+    } else if (shard_state) {   // vocab-parallel shard: the merged state goes out in the packed exchange layout
       set_state_pointers(fin, shard_state, T, pl.topk_cap, /*as_output=*/true);
       if (pl.num_chunks <= 32) SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, true>, fgrid, fblock, 0, st, fin));
       else SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<sq::FIN_MAX_NL, true>, fgrid, fblock, 0, st, fin));
@@ -691,7 +698,10 @@ extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int 
     set_state_pointers(fin, const_cast<float*>(static_cast<const float*>(states)), T, cap, /*as_output=*/false);
     fin.lse = lse; fin.target_logprob = lp; fin.entropy = ent; fin.conf = conf;
     fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
-    SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, false>, dim3((unsigned)cdiv64(T, sq::FIN_WARPS)), dim3(sq::FIN_WARPS * 32), 0, st, fin));
+    if (num_shards <= 8)
+      SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, false, 8>, dim3((unsigned)cdiv64(T, sq::FIN_WARPS * 4)), dim3(sq::FIN_WARPS * 32), 0, st, fin));
+    else
+      SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, false>, dim3((unsigned)cdiv64(T, sq::FIN_WARPS)), dim3(sq::FIN_WARPS * 32), 0, st, fin));
     ctx->launches += 1;
     SQ_CUDA(ctx, cudaGetLastError());
   }
