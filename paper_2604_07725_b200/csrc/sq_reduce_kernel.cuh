@@ -5,8 +5,9 @@
 //   seq_mean_conf     = C(tau) = (1/|tau|) sum_i c(i)                       (Eq. 4)
 //   seq_min_window_conf = min_j (1/w') sum_{i=j}^{j+w'-1} c(i),  w' = min(w, L), stride 1
 //
-// HBM-bound (12 B/token).  Three launches, the 2nd and 3rd with programmatic stream serialization so that
-// their launch latency overlaps the kernel before them:
+// HBM-bound (12 B/token).  Large inputs take three launches, each with programmatic stream serialization so that its
+// launch latency overlaps the kernel before it; small ones (the scoring pipeline) a single launch that does the same
+// work per tile (sq_reduce_fused_kernel, at the end of this file):
 //   tile_scan : tile i of a sequence covers the block of TILE = 8192 tokens that starts at (s0 & ~3) + i*TILE of the
 //               packed arrays (s0 = the sequence's first token), so every tile's 16-byte vectors are aligned and only
 //               a sequence's last tile is ragged.  Exclusive scan of the tiles per sequence -> tile_base[B+1],

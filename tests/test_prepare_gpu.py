@@ -36,7 +36,7 @@ def check_prepared(H_gpu, h64):
     assert diff.mean() < 1e-3
 
 
-@pytest.mark.parametrize("d,N,T", [(64, 50, 37), (200, 300, 300), (4096, 700, 513), (5120, 64, 200), (8, 5, 9)])
+@pytest.mark.parametrize("d,N,T", [(64, 50, 37), (200, 300, 300), (4096, 700, 513), (5120, 64, 200), (8, 5, 9), (8192, 40, 33)])
 def test_prepare_matches_oracle(d, N, T):
     sq = _sq()
     gen = torch.Generator().manual_seed(d + N)
