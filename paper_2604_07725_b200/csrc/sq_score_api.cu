@@ -514,7 +514,9 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fp.num_chunks = pl.num_chunks; fp.m_tiles = pl.m_tiles; fp.group_m = pl.group_m;
     fp.num_gangs = pl.num_gangs; fp.num_gang_units = pl.num_gang_units; fp.gang_ctr = ctx->gang_ctr;
     fp.m_split = pl.m_split; fp.gang_b_size = pl.gang_b_size; fp.num_gang_units_b = pl.num_gang_units_b;
-    SQ_CUDA(ctx, cudaMemsetAsync(ctx->gang_ctr, 0, 256 * sizeof(unsigned int), st));
+    // the gang barrier counters only matter when some gang has more than one member (not in decode-shaped plans)
+    if (pl.group_m > 1 || (pl.num_gang_units_b > 0 && pl.gang_b_size > 1))
+      SQ_CUDA(ctx, cudaMemsetAsync(ctx->gang_ctr, 0, 256 * sizeof(unsigned int), st));
     fp.targets = targets;
     fp.part_m = ctx->part_m; fp.part_s = ctx->part_s; fp.part_u = ctx->part_u;
     fp.part_cs = ctx->part_cs; fp.part_cu = ctx->part_cu;
