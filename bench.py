@@ -358,10 +358,31 @@ def run_ours(args):
             d1.record(stream)
             stream.synchronize()
         d_ms = d0.elapsed_time(d1) / 20
+        # the same step captured once into a CUDA graph (the library enqueues only stream work) and replayed
+        g_ms = None
+        try:
+            with torch.cuda.stream(stream):
+                gr = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gr, stream=stream):
+                    eng3.run(Hd, W, tgd, cud, wl.k, 16, stream=stream, out=od)
+                for _ in range(3):
+                    gr.replay()
+                g0 = torch.cuda.Event(enable_timing=True); g1 = torch.cuda.Event(enable_timing=True)
+                g0.record(stream)
+                for _ in range(20):
+                    gr.replay()
+                g1.record(stream)
+                stream.synchronize()
+            g_ms = g0.elapsed_time(g1) / 20
+            del gr
+        except Exception as exc:   # reported, never fatal for the headline line
+            g_ms = None
+            sys.stderr.write("decode graph leg skipped: %r\n" % (exc,))
         d_bytes = 2.0 * V * d + 2.0 * Td * d + Td * (4 + 16 + 8 * wl.k)
         line["decode_standalone"] = {"bound": "hbm", "achieved": d_bytes / (d_ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                                      "unit": "GB/s", "frac": d_bytes / (d_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "ms": d_ms,
                                      "rows": Td, "tokens_per_s": Td / (d_ms * 1e-3), "algorithmic_bytes": d_bytes,
+                                     "cuda_graph_ms": g_ms, "cuda_graph_frac": (d_bytes / (g_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]) if g_ms else None,
                                      "plan": sq.plan(d, V, Td, wl.k, num_sms=torch.cuda.get_device_properties(dev).multi_processor_count),
                                      "note": "whole path (3 launches) on a decode batch of 64 rows; W (%.0f MB) exceeds L2 and is "
                                              "streamed once per pass" % (V * d * 2 / 1e6)}
