@@ -32,7 +32,7 @@ import math
 import numpy as np
 import torch
 
-ORACLE_VERSION = 4
+ORACLE_VERSION = 5
 
 
 def widen(x_bf16: torch.Tensor) -> torch.Tensor:
@@ -117,7 +117,7 @@ def score(H: torch.Tensor, W: torch.Tensor, targets, cu_seqlens, k: int, window:
     W64 = widen(W)
     T = H.shape[0]
     tg = np.asarray(targets, dtype=np.int64)
-    keys = ("lse", "target_logprob", "target_valid", "entropy", "topk_logprob", "topk_index", "conf")
+    keys = ("lse", "target_logprob", "target_valid", "entropy", "topk_logprob", "topk_index", "conf", "logp")
     parts = {key: [] for key in keys}
     for r0 in range(0, T, row_batch):
         r = token_scores(H[r0:r0 + row_batch], W64, tg[r0:r0 + row_batch], k)
@@ -126,7 +126,7 @@ def score(H: torch.Tensor, W: torch.Tensor, targets, cu_seqlens, k: int, window:
     V = W.shape[0]
     kk = min(V, k + 1)
     tok = {key: (np.concatenate(parts[key]) if T > 0 else
-                 np.zeros((0, kk) if key.startswith("topk") else (0,)))
+                 np.zeros((0, kk) if key.startswith("topk") else ((0, V) if key == "logp" else (0,))))
            for key in keys}
     seq = sequence_scores(tok["target_logprob"], tok["entropy"], tok["conf"], cu_seqlens, window,
                           tok["target_valid"])
@@ -164,7 +164,9 @@ def route(seq_conf, group_members, group_offsets, p: float, lite_mask=None) -> d
     """Per problem q (groups [off[q], off[q+1])): F(g) = GC(g); theta_q over the non-lite groups
     (Eq. 6); mu(g,q) = Model 1 if GC(g) > theta_q ("easy", strict) else Model 2 (Eq. 7).
     Codes: 0 = B_lite (given by `lite_mask`; the consensus test itself is on answer strings and is
-    out of scope), 1 = Model 1, 2 = Model 2."""
+    out of scope), 1 = Model 1, 2 = Model 2, 3 = fitness undefined: a group whose GC is not finite
+    (it holds an empty trajectory, whose C(tau) is NaN) takes no part in the percentile and is left
+    to the caller (reading #24; the paper never scores an empty trajectory)."""
     gc = group_confidence(seq_conf, group_members)
     off = np.asarray(group_offsets, dtype=np.int64)
     G = len(gc)
@@ -173,43 +175,13 @@ def route(seq_conf, group_members, group_offsets, p: float, lite_mask=None) -> d
     code = np.zeros(G, dtype=np.int32)
     for q in range(len(off) - 1):
         idx = np.arange(off[q], off[q + 1])
-        live = idx[~lite[idx]]
+        undefined = idx[~lite[idx] & ~np.isfinite(gc[idx])]
+        code[undefined] = 3
+        live = idx[~lite[idx] & np.isfinite(gc[idx])]
         theta[q] = percentile_threshold(gc[live], p)
         for g in live:
             code[g] = 1 if gc[g] > theta[q] else 2
     return {"group_fitness": gc, "theta": theta, "route": code}
-
-
-def route_decisions_fp32(seq_conf_f32, group_members, group_offsets, p: float, lite_mask=None) -> np.ndarray:
-    """The routing decision taken in the kernel's precision (fp32, same operation order: members
-    summed left to right then divided by K; theta = v[lo] + frac * (v[hi] - v[lo]) with separate
-    roundings).  A floating-point comparison decides an integer here, so the parity test compares
-    the GPU's codes with this, and GC / theta with the fp64 definitions above."""
-    f = np.float32
-    c = np.asarray(seq_conf_f32, dtype=np.float32)
-    gm = np.asarray(group_members, dtype=np.int64)
-    K = gm.shape[1]
-    gc = np.zeros(gm.shape[0], dtype=np.float32)
-    for j in range(K):
-        gc = (gc + c[gm[:, j]]).astype(np.float32)
-    gc = (gc / f(K)).astype(np.float32)
-    off = np.asarray(group_offsets, dtype=np.int64)
-    lite = np.zeros(len(gc), dtype=bool) if lite_mask is None else np.asarray(lite_mask, dtype=bool)
-    code = np.zeros(len(gc), dtype=np.int32)
-    for q in range(len(off) - 1):
-        idx = np.arange(off[q], off[q + 1])
-        live = idx[~lite[idx]]
-        if len(live) == 0:
-            continue
-        v = np.sort(gc[live])
-        n = len(v)
-        pos = f(f(p) / f(100.0)) * f(n - 1)
-        lo = int(np.floor(pos))
-        hi = min(lo + 1, n - 1)
-        frac = f(pos - f(lo))
-        theta = f(v[lo] + f(frac * f(v[hi] - v[lo])))
-        code[live] = np.where(gc[live] > theta, 1, 2)
-    return code
 
 
 def selection_probabilities(fitness, pop_offsets, zeta: float) -> np.ndarray:
@@ -274,10 +246,13 @@ def bf16_half_ulp(h64: np.ndarray) -> np.ndarray:
 
 
 # ------------------------------------------------------------------------------------------------
-# Next row (SURVEY section 8(f)-4, FP8 variant): e4m3 quantisation with per-row / per-tensor scales.
-# The codes are a quantised representation decided by floating point, so the decision is taken in the
-# kernel's precision (fp32) and operation order: inv = 448 / amax; y = x * inv; clamp; round to nearest
-# even e4m3.  Everything after it (the scoring of the dequantised operands) is the fp64 path above.
+# Next row (SURVEY section 8(f)-4, FP8 variant): e4m3 quantisation with per-row / per-tensor scales,
+# by its definition in fp64: scale = amax / 448, code = the e4m3 value nearest to x / scale (ties to the
+# even mantissa).  The codes are a quantised representation decided by floating point; the CUDA path
+# takes that decision in fp32, so the parity test accepts a code that is a correct rounding of a value
+# within a stated fp32 slack of x / scale and demands the code below except within that slack of a
+# rounding boundary (reading #23).  Everything after it (the scoring of the dequantised
+# operands) is the fp64 path above.
 # ------------------------------------------------------------------------------------------------
 E4M3_MAX = 448.0
 
@@ -313,16 +288,23 @@ def round_to_e4m3(y: np.ndarray) -> np.ndarray:
 
 
 def quantize_fp8(X: torch.Tensor, per_tensor: bool):
-    """(codes uint8 [rows, d], scales float32 [rows] or [1]) with x ~= e4m3_values()[code] * scale."""
-    x = X.to(torch.float32).numpy()
+    """(codes uint8 [rows, d], scales fp64 [rows] or [1], y fp64 [rows, d]) with scale = amax / 448 (1 where
+    amax = 0), y = x / scale the exact scaled values and codes = round_to_e4m3(y), so that
+    x ~= e4m3_values()[code] * scale.  amax is taken per row, or over the whole tensor."""
+    x = widen(X).numpy()
     amax = np.abs(x).max() if per_tensor else np.abs(x).max(axis=1)
-    amax = np.asarray(amax, dtype=np.float32).reshape(-1)
-    ok = amax > 0
-    scale = np.where(ok, (amax / np.float32(E4M3_MAX)).astype(np.float32), np.float32(1)).astype(np.float32)
-    inv = np.where(ok, (np.float32(E4M3_MAX) / np.where(ok, amax, np.float32(1))).astype(np.float32), np.float32(1)).astype(np.float32)
-    y = (x * (inv[0] if per_tensor else inv[:, None])).astype(np.float32)
-    y = np.clip(y, -E4M3_MAX, E4M3_MAX)
-    return round_to_e4m3(y), scale
+    amax = np.asarray(amax, dtype=np.float64).reshape(-1)
+    scale = np.where(amax > 0, amax / E4M3_MAX, 1.0)
+    y = x / (scale[0] if per_tensor else scale[:, None])
+    return round_to_e4m3(y), scale, y
+
+
+def e4m3_half_ulp(y: np.ndarray) -> np.ndarray:
+    """Half the spacing of the e4m3 code points around |y| <= 448: 3 mantissa bits, spacing 2^(e-3) in the
+    binade [2^e, 2^(e+1)), e >= -6; below the first normal (2^-6) the subnormal spacing 2^-9."""
+    a = np.abs(np.asarray(y, dtype=np.float64))
+    e = np.floor(np.log2(np.maximum(a, 2.0 ** -6)))
+    return 0.5 * 2.0 ** (np.minimum(e, 8.0) - 3)
 
 
 def dequantize_fp8(codes: np.ndarray, scale: np.ndarray) -> torch.Tensor:

@@ -1,6 +1,15 @@
-"""GPU parity of the FP8 variant: sq_score_quantize_fp8 is byte-exact against the oracle's fp32-mirrored
-e4m3 quantisation, and sq_score_run_fp8 meets the path's tolerances against the fp64 oracle evaluated ON THE QUANTISED
-OPERANDS (codes * scales, exact in fp64).  The distance to the bf16 scores -- what the quantisation itself costs -- is
+"""GPU parity of the FP8 variant.
+
+sq_score_quantize_fp8 against the oracle's fp64 DEFINITION (scale = amax / 448, code = e4m3 nearest to x / scale).  The
+code is an integer decided by floating point, and the kernel decides in fp32: inv = fl(448 / amax), y = fl(x * inv) --
+two roundings, so its y is within 2 * 2^-24 (+ second order) of the exact x / scale.  With FP32_SLACK = 4 * 2^-24:
+  * the scale must be the exact quotient rounded once to fp32 (<= 2^-24 relative);
+  * every byte must decode to a correct rounding of SOME value within FP32_SLACK of the exact y:
+        |decode(byte) - y| <= half the e4m3 spacing at y + FP32_SLACK * |y|;
+  * and it must EQUAL the oracle's code except where y sits within that slack of a rounding boundary (a midpoint between
+    two code points) -- a tiny fraction of the elements.
+sq_score_run_fp8 meets the path's tolerances against the fp64 oracle evaluated ON THE QUANTISED OPERANDS (the GPU's codes
+times the GPU's scales, exact in fp64).  The distance to the bf16 scores -- what the quantisation itself costs -- is
 measured and bounded loosely; it is far outside the bf16 tolerances by construction."""
 import numpy as np
 import pytest
@@ -19,23 +28,38 @@ def _sq():
     return sq
 
 
+FP32_SLACK = 4 * 2.0 ** -24
+
+
+def check_codes(got, scale_gpu, ref_codes, ref_scale, y):
+    np.testing.assert_allclose(scale_gpu.astype(np.float64), ref_scale, rtol=2.0 ** -24, atol=0)
+    table = O.e4m3_values()
+    assert not np.isnan(table[got]).any(), "NaN code emitted"
+    v = table[got]
+    lim = O.e4m3_half_ulp(np.abs(y) * (1 + FP32_SLACK)) + FP32_SLACK * np.abs(y)
+    err = np.abs(v - y)
+    assert (err <= lim).all(), "worst excess %g at %s" % ((err - lim).max(), np.unravel_index((err - lim).argmax(), err.shape))
+    diff = v != table[ref_codes]                       # +0 and -0 are the same value
+    if diff.any():                                     # only where y is within the fp32 slack of a rounding boundary
+        near = np.abs(np.abs(y - table[ref_codes]) - O.e4m3_half_ulp(y)) <= 2 * FP32_SLACK * np.abs(y) + 1e-300
+        assert near[diff].all(), np.argwhere(diff & ~near)[:5]
+    assert diff.mean() < 5e-3      # bf16 x and amax have 8-bit significands: x / amax is often a small rational and y an EXACT midpoint
+
+
 @pytest.mark.parametrize("rows,d", [(5, 16), (33, 200), (300, 4096), (64, 2880), (2000, 5120), (9, 8192)])
-def test_quantize_bytes_match_oracle(rows, d):
+def test_quantize_codes_against_the_fp64_definition(rows, d):
     sq = _sq()
     gen = torch.Generator().manual_seed(rows + d)
     X = (torch.randn(rows, d, generator=gen) * torch.exp(torch.rand(rows, 1, generator=gen) * 6 - 4)).to(torch.bfloat16)
     X[rows // 2] = 0                                   # an all-zero row
     X[0, 0] = 3.0e4; X[1, :] = X[1, :].abs()           # a large outlier, a non-negative row
+    X[2, : min(d, 16)] = X[2].abs().max() * torch.tensor([m / 16.0 + 1 / 32.0 for m in range(min(d, 16))]).to(torch.bfloat16)   # values near midpoints
     eng = sq.SqScore(d, 1000, max_tokens=rows, max_seqs=1)
     for per_tensor in (False, True):
         q, s = eng.quantize_fp8(X.to(DEV), per_tensor)
         torch.cuda.synchronize()
-        qr, sr = O.quantize_fp8(X, per_tensor)
-        np.testing.assert_array_equal(s.cpu().numpy(), sr)
-        got = q.cpu().numpy()
-        same = got == qr
-        # +0 and -0 are the same value; everything else must be the same byte
-        assert np.all(same | ((got & 0x7F) == 0) & ((qr & 0x7F) == 0)), np.argwhere(~same)[:5]
+        qr, sr, y = O.quantize_fp8(X, per_tensor)
+        check_codes(q.cpu().numpy(), s.cpu().numpy(), qr, sr, y)
     eng.close()
 
 

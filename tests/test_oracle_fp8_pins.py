@@ -49,20 +49,35 @@ def test_quantize_scales_and_error_bound():
     gen = torch.Generator().manual_seed(8)
     X = (torch.randn(12, 64, generator=gen) * torch.exp(torch.rand(12, 1, generator=gen) * 4 - 2)).to(torch.bfloat16)
     X[3] = 0
-    q, s = O.quantize_fp8(X, per_tensor=False)
-    amax = X.float().abs().amax(dim=1).numpy()
-    assert q.dtype == np.uint8 and q.shape == (12, 64) and s.shape == (12,)
+    q, s, y = O.quantize_fp8(X, per_tensor=False)
+    amax = X.double().abs().amax(dim=1).numpy()
+    assert q.dtype == np.uint8 and q.shape == (12, 64) and s.shape == (12,) and y.shape == (12, 64)
     assert s[3] == 1.0 and not q[3].any()                                         # all-zero row
-    np.testing.assert_array_equal(s[amax > 0], (amax[amax > 0] / np.float32(448)).astype(np.float32))
+    np.testing.assert_array_equal(s[amax > 0], amax[amax > 0] / 448.0)            # scale = amax / 448 by definition
+    np.testing.assert_allclose(y * s[:, None], X.double().numpy(), rtol=1e-15)    # y = x / scale
     v = np.abs(O.e4m3_values()[q])
     assert np.all(v.max(axis=1)[amax > 0] == 448.0)                               # the row maximum lands on the largest code
+    assert np.abs(y).max() <= 448.0
     deq = O.dequantize_fp8(q, s).numpy()
     x = X.double().numpy()
     # nearest e4m3: relative error <= 2^-4 for normals, absolute <= 2^-10 * scale below the first normal
     assert np.all(np.abs(deq - x) <= np.maximum(2.0 ** -4 * np.abs(x), 2.0 ** -10 * s[:, None]) * (1 + 1e-6))
-    qt, st = O.quantize_fp8(X, per_tensor=True)
-    assert st.shape == (1,) and st[0] == np.float32(amax.max()) / np.float32(448)
+    # the codes are the nearest code points of y (brute force over the table), within half a spacing
+    pts = O.e4m3_values()[:127]
+    nearest = np.abs(np.abs(y)[:, :, None] - pts[None, None, :]).min(axis=2)
+    np.testing.assert_array_equal(np.abs(np.abs(O.e4m3_values()[q]) - np.abs(y)), nearest)
+    assert np.all(nearest <= O.e4m3_half_ulp(y))
+    qt, st, yt = O.quantize_fp8(X, per_tensor=True)
+    assert st.shape == (1,) and st[0] == amax.max() / 448.0
     assert np.abs(O.e4m3_values()[qt]).max() == 448.0
     # a power-of-two rescaling of the input changes the scale, not the codes
-    q2, s2 = O.quantize_fp8((X.float() * 4).to(torch.bfloat16), per_tensor=False)
+    q2, s2, _ = O.quantize_fp8((X.float() * 4).to(torch.bfloat16), per_tensor=False)
     assert np.array_equal(q2, q) and np.array_equal(s2[amax > 0], s[amax > 0] * 4)
+
+
+def test_e4m3_half_ulp_is_half_the_code_point_spacing():
+    pts = O.e4m3_values()[:127]
+    gaps = np.diff(pts)
+    mid = 0.5 * (pts[:-1] + pts[1:])
+    np.testing.assert_array_equal(O.e4m3_half_ulp(mid), 0.5 * gaps)               # every interval between code points
+    assert O.e4m3_half_ulp(0.0) == 2.0 ** -10 and O.e4m3_half_ulp(1.0) == 2.0 ** -4 and O.e4m3_half_ulp(-300.0) == 16.0

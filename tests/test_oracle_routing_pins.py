@@ -81,15 +81,20 @@ def test_routing_fraction_tracks_the_percentile():
     assert (r0["route"] == r1["route"]).all() and r1["theta"][0] == pytest.approx(r0["theta"][0] + 100.0)
 
 
-def test_fp32_decision_mirror_agrees_with_fp64_away_from_the_threshold():
-    rng = np.random.default_rng(3)
-    c = rng.uniform(3, 12, size=64).astype(np.float32)
-    gm = rng.integers(0, 64, size=(48, 4))
-    off = [0, 16, 48]
-    r64 = O.route(c, gm, off, 60.0)
-    d32 = O.route_decisions_fp32(c, gm, off, 60.0)
-    far = np.abs(r64["group_fitness"] - np.repeat(r64["theta"], [16, 32])) > 1e-4
-    assert far.sum() >= 40 and (d32[far] == r64["route"][far]).all()
+def test_group_with_an_empty_trajectory_is_left_out_of_the_percentile():
+    # C(tau) of an empty trajectory is NaN (reading #9); its group has no fitness: code 3, and theta is the
+    # percentile of the remaining groups (reading #24)
+    c = np.array([6.0, np.nan, 2.0, 4.0, 8.0])
+    gm = [[0, 2], [1, 3], [3, 4], [2, 3]]          # GC = 4, NaN, 6, 3
+    r = O.route(c, gm, [0, 4], 50.0)
+    assert np.isnan(r["group_fitness"][1]) and r["group_fitness"][[0, 2, 3]].tolist() == [4.0, 6.0, 3.0]
+    assert r["theta"][0] == 4.0                    # median of {4, 6, 3}
+    assert r["route"].tolist() == [2, 3, 1, 2]
+    same = O.route(c[[0, 2, 3, 4]], [[0, 1], [2, 3], [1, 2]], [0, 3], 50.0)       # the problem without that group
+    assert same["theta"][0] == r["theta"][0] and same["route"].tolist() == [2, 1, 2]
+    # a lite group stays lite even if its fitness is undefined; only undefined groups -> NaN threshold
+    r2 = O.route(c, [[1, 1], [1, 0]], [0, 2], 50.0, [1, 0])
+    assert r2["route"].tolist() == [0, 3] and math.isnan(r2["theta"][0])
 
 
 def test_selection_probabilities():
