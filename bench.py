@@ -5,9 +5,15 @@
 
 A step is one pass of the whole hot path (kernel 1 fused GEMM+statistics, finalize/merge, kernel 2: 3 launches)
 over one synthetic packed batch.  At N=1 the workload is BASELINE.json configs[2] (`qwen3_8b`, the
-config the metric's 60 % target is quoted on).  With N>1 (torchrun) every rank scores its own
-batch of the same shape (sequences shard across GPUs, W replicated, no data-path collective):
-weak scaling.  One JSON line is printed by rank 0.
+config the metric's 60 % target is quoted on); the other four configs are timed briefly into the
+`configs` sub-record.  With N>1 (torchrun):
+  --parallelism dp     (default) every rank scores its own batch of the same shape (sequences shard across
+                       GPUs, W replicated) and the step ends with the path's one exchange, the all-gather
+                       of the 4 scalars per sequence: weak scaling;
+  --parallelism vocab  the LM head is split by rows over the ranks (tensor-parallel scorer): every rank scores
+                       the SAME batch against its shard, one all-gather of the packed partial states, then the
+                       merge on every rank: strong scaling.
+One JSON line is printed by rank 0.
 """
 import argparse
 import json
@@ -159,37 +165,90 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 # GPU arm
 # ------------------------------------------------------------------------------------------------
+def time_steps(eng, H, W, tg, cu, k, window, stream, steps, warmup, step_fn=None):
+    """`warmup` untimed + `steps` timed passes of the whole hot path on `stream`; CUDA events around the timed region;
+    kernel 1's duration from the library's per-run events for EVERY timed step (read after the loop: no host sync inside).
+    Returns (ms per step, per-step kernel times, outputs, launches)."""
+    out = None
+    run = step_fn if step_fn is not None else (lambda o: eng.run(H, W, tg, cu, k, window, stream=stream, out=o))
+    with torch.cuda.stream(stream):
+        for _ in range(warmup):
+            out = run(out)
+        stream.synchronize()
+        eng.profile_read()                                   # empty the ring: only the timed steps remain
+        launches0 = eng.launch_count()
+        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            out = run(out)
+        e1.record(stream)
+        stream.synchronize()
+    return e0.elapsed_time(e1) / steps, eng.profile_read(), out, eng.launch_count() - launches0
+
+
+def kernel_stats(per_step):
+    f = [x["fused_ms"] for x in per_step]
+    return {"mean": float(np.mean(f)), "min": float(np.min(f)), "max": float(np.max(f)), "n": len(f)}
+
+
 def run_ours(args):
     import paper_2604_07725_b200 as sq
+    from paper_2604_07725_b200 import sharding
 
     rank, world, local = dist_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the sq_score path has no CPU fallback")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    use_dist = world > 1
+    vocab_mode = args.parallelism == "vocab"
+    use_dist = world > 1 or vocab_mode          # vocab mode runs its collective through NCCL even at world size 1
     if use_dist:
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        dist.init_process_group("nccl", device_id=dev)
+        os.environ.setdefault("MASTER_PORT", "29531")
+        os.environ.setdefault("NCCL_DEBUG", "WARN")
+        dist.init_process_group("nccl", device_id=dev, rank=rank, world_size=world)
 
     peaks = load_peaks()
     wl = workloads.CONFIGS[args.config]
-    if use_dist:   # weak scaling: every rank scores its own population of the same shape
+    if use_dist and not vocab_mode:   # weak scaling: every rank scores its own population of the same shape
         from dataclasses import replace
         wl_rank = replace(wl, seed=wl.seed + 100 * rank)
     else:
         wl_rank = wl
     inp = workloads.make_inputs(wl_rank)
     T, B, d, V = inp["T"], inp["B"], wl.d, wl.V
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
 
-    eng = sq.SqScore(d, V, max_tokens=T, max_seqs=B, max_k=wl.k, device=local,
-                     cta_group=args.cta_group, num_chunks=args.num_chunks, group_m=args.group_m)
-    pl = sq.plan(d, V, T, wl.k, num_sms=torch.cuda.get_device_properties(dev).multi_processor_count,
-                 cta_group=args.cta_group, num_chunks=args.num_chunks, group_m=args.group_m)
     stream = torch.cuda.Stream(device=dev)
-    H = inp["H"].to(dev); W = inp["W"].to(dev)
-    tg = inp["targets"].to(dev); cu = inp["cu_seqlens"].to(dev)
+    H = inp["H"].to(dev); tg = inp["targets"].to(dev); cu = inp["cu_seqlens"].to(dev)
+    exchange_bytes = 0
+    if vocab_mode:
+        vstarts = sq.shard_vocab(V, world)
+        rows_max = max(b - a for a, b in zip(vstarts, vstarts[1:]))
+        W = inp["W"][vstarts[rank]:vstarts[rank + 1]].to(dev)          # this rank's rows of the LM head only
+        eng = sq.SqScore(d, rows_max, max_tokens=T, max_seqs=B, max_k=wl.k, device=local, staging=False,
+                         cta_group=args.cta_group, num_chunks=args.num_chunks, group_m=args.group_m)
+        pl = sq.plan(d, max(1, W.shape[0]), T, wl.k, num_sms=sms, cta_group=args.cta_group, num_chunks=args.num_chunks, group_m=args.group_m)
+        exchange_bytes = world * sq.shard_state_bytes(T, wl.k)
+        def step_fn(o):
+            return sharding.score_vocab_parallel(eng, H, W, vstarts, rank, tg, cu, wl.k, wl.window, stream=stream)
+    else:
+        W = inp["W"].to(dev)
+        eng = sq.SqScore(d, V, max_tokens=T, max_seqs=B, max_k=wl.k, device=local, staging=True,
+                         cta_group=args.cta_group, num_chunks=args.num_chunks, group_m=args.group_m)
+        pl = sq.plan(d, V, T, wl.k, num_sms=sms, cta_group=args.cta_group, num_chunks=args.num_chunks, group_m=args.group_m)
+        if use_dist:
+            # the path's one exchange (PAPER.md:199-201: the N scoring calls of a loop are one batched request whose
+            # scalars go back to the router): all-gather of [id, 4 scalars] per sequence, inside the timed step
+            seq_ids = list(range(rank * B, (rank + 1) * B))
+            exchange_bytes = world * B * world * 5 * 4
+            def step_fn(o):
+                o = eng.run(H, W, tg, cu, wl.k, wl.window, stream=stream, out=o)
+                o["gathered"] = sharding.gather_sequence_scores(o, seq_ids, B * world, world, device=dev)
+                return o
+        else:
+            step_fn = None
     H_pin = inp["H"].pin_memory(); tg_pin = inp["targets"].pin_memory(); cu_pin = inp["cu_seqlens"].pin_memory()
     seq_pin = torch.empty(4 * B, dtype=torch.float32).pin_memory()
     torch.cuda.synchronize()
@@ -201,44 +260,33 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---------------- device-resident timing (value) + live per-kernel timing (roofline)
-    out = None
     eng.set_profiling(True)
-    with torch.cuda.stream(stream):
-        for _ in range(max(3, args.warmup)):
-            out = eng.run(H, W, tg, cu, wl.k, wl.window, stream=stream, out=out)
-        barrier()
-        sampler = ClockSampler(local)
-        sampler.start()
-        launches0 = eng.launch_count()
-        e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
-        fused_ms = []
-        e0.record(stream)
-        for _ in range(args.steps):
-            eng.run(H, W, tg, cu, wl.k, wl.window, stream=stream, out=out)
-            if args.per_step_kernel_times:
-                fused_ms.append(eng.kernel_times())
-        e1.record(stream)
-        barrier()
-        clocks = sampler.stop()
-        launches = eng.launch_count() - launches0
-        total_ms = e0.elapsed_time(e1)
-        if not fused_ms:
-            fused_ms.append(eng.kernel_times())   # the last timed step's kernels
-    ms_step = total_ms / args.steps
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms_step, fused_ms, out, launches = time_steps(eng, H, W, tg, cu, wl.k, wl.window, stream, args.steps, max(3, args.warmup), step_fn)
+    barrier()
+    clocks = sampler.stop()
 
-    # ---------------- end to end through the C ABI with HOST buffers
-    with torch.cuda.stream(stream):
-        for _ in range(2):
-            eng.run_host(H_pin, W, tg_pin, cu_pin, wl.k, wl.window, seq_pin, stream=stream)
-            stream.synchronize()
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.e2e_steps):
-            eng.run_host(H_pin, W, tg_pin, cu_pin, wl.k, wl.window, seq_pin, stream=stream)
-            stream.synchronize()       # the caller reads the scalars every step
-        e2e_s = (time.perf_counter() - t0) / args.e2e_steps
-    seq_dev = torch.cat([out[n] for n in ("seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf")])
-    e2e_ok = bool(torch.allclose(seq_dev.cpu(), seq_pin, rtol=1e-5, atol=1e-6, equal_nan=True))
+    # ---------------- end to end through the C ABI with HOST buffers (data-parallel form; W is the resident model weight)
+    e2e_s, e2e_ok, e2e_dev_ms = float("nan"), None, None
+    if not vocab_mode:
+        with torch.cuda.stream(stream):
+            for _ in range(2):
+                eng.run_host(H_pin, W, tg_pin, cu_pin, wl.k, wl.window, seq_pin, stream=stream)
+                stream.synchronize()
+            barrier()
+            g0 = torch.cuda.Event(enable_timing=True); g1 = torch.cuda.Event(enable_timing=True)
+            g0.record(stream)
+            t0 = time.perf_counter()
+            for _ in range(args.e2e_steps):
+                eng.run_host(H_pin, W, tg_pin, cu_pin, wl.k, wl.window, seq_pin, stream=stream)
+                stream.synchronize()       # the caller reads the scalars every step
+            e2e_s = (time.perf_counter() - t0) / args.e2e_steps
+            g1.record(stream); stream.synchronize()
+            e2e_dev_ms = g0.elapsed_time(g1) / args.e2e_steps
+        seq_dev = torch.cat([out[n] for n in ("seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf")])
+        e2e_ok = bool(torch.allclose(seq_dev.cpu(), seq_pin, rtol=1e-5, atol=1e-6, equal_nan=True))
 
     # ---------------- max over ranks
     t_loc = torch.tensor([ms_step, e2e_s * 1e3, float(T)], dtype=torch.float64, device=dev)
@@ -246,6 +294,8 @@ def run_ours(args):
         tmax = t_loc.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
         tsum = t_loc.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
         ms_step, e2e_ms, tokens_all = float(tmax[0]), float(tmax[1]), float(tsum[2])
+        if vocab_mode:
+            tokens_all = float(T)        # every rank scored the same T tokens against its shard
     else:
         e2e_ms, tokens_all = e2e_s * 1e3, float(T)
     if rank != 0:
@@ -254,43 +304,77 @@ def run_ours(args):
         return
 
     value = tokens_all / (ms_step * 1e-3)
-    k1_ms = float(np.mean([x["fused_ms"] for x in fused_ms]))
+    k1 = kernel_stats(fused_ms)
+    k1_ms = k1["mean"]
     fin_ms = float(np.mean([x["finalize_ms"] for x in fused_ms]))
     red_ms = float(np.mean([x["reduce_ms"] for x in fused_ms]))
-    flops = 2.0 * T * V * d                                   # algorithmic FLOPs per launch of kernel 1
+    v_rank = W.shape[0]
+    flops = 2.0 * T * v_rank * d                              # algorithmic FLOPs per launch of kernel 1 (on this rank)
     achieved = flops / (k1_ms * 1e-3) / 1e12
     peak = peaks["bf16_tflops_sustained"]                     # kernel timed inside a long step
-    traffic = None
+    traffic, traffic_source = None, None
     tpath = os.path.join(ROOT, "profiles", "traffic_%s.csv" % wl.name)   # from the committed ncu --set full summary
-    if os.path.exists(tpath):
+    if os.path.exists(tpath) and not vocab_mode:
         with open(tpath) as f:
             for ln in f:
                 if ln.startswith("sq_fused_score_kernel,"):
                     traffic = float(ln.strip().split(",")[1])
+                    traffic_source = "profiles/traffic_%s.csv (ncu --set full of this kernel, committed; not measured in this run)" % wl.name
+    par = ("vocab%d (LM head split by rows, one all-gather of the packed partial states per step)" % world) if vocab_mode else \
+          ("dp%d (sequences sharded, W replicated%s)" % (world, "; one all-gather of 5 floats per sequence per step" if use_dist else ""))
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if vocab_mode else "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "config": {"workload": wl.name, "d": d, "V": V, "B": B, "T": T, "k": wl.k, "window": wl.window,
-                   "parallelism": "dp%d (sequences sharded, W replicated)" % world,
-                   "l2": "inputs larger than L2 (H %.0f MB + W %.0f MB re-streamed every step)" % (T * d * 2 / 1e6, V * d * 2 / 1e6),
+                   "parallelism": par, "exchange_bytes_per_step": exchange_bytes,
+                   "l2": "inputs larger than L2 (H %.0f MB + W %.0f MB re-streamed every step)" % (T * d * 2 / 1e6, v_rank * d * 2 / 1e6),
                    "plan": pl},
-        "tflops": flops / (ms_step * 1e-3) / 1e12,
+        "tflops": flops * (world if vocab_mode else 1) / (ms_step * 1e-3) / 1e12,
         "pct_of_bf16_peak_burst": 100.0 * flops / (ms_step * 1e-3) / 1e12 / peaks["bf16_tflops"],
         "roofline": {"bound": "tensor", "kernel": "sq_fused_score_kernel", "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_source,
                      "peak_kind": "bf16_tflops_sustained of %s (kernel timed inside a long step)" % peaks["source"],
                      "frac_of_burst": achieved / peaks["bf16_tflops"], "peak_burst": peaks["bf16_tflops"],
-                     "kernel_ms": k1_ms, "algorithmic_flops_per_launch": flops},
+                     "kernel_ms": k1_ms, "kernel_ms_min": k1["min"], "kernel_ms_max": k1["max"], "kernel_ms_samples": k1["n"],
+                     "algorithmic_flops_per_launch": flops},
         "kernels_ms": {"fused": k1_ms, "finalize": fin_ms, "reduce": red_ms,
                        "fused_per_step": [round(x["fused_ms"], 3) for x in fused_ms]},
-        "e2e": {"value": tokens_all / (e2e_ms * 1e-3), "unit": UNIT,
+        "e2e": {"value": (tokens_all / (e2e_ms * 1e-3)) if e2e_ms == e2e_ms else None, "unit": UNIT,
                 "h2d_bytes_per_step": T * d * 2 + T * 4 + (B + 1) * 4, "d2h_bytes_per_step": 4 * B * 4,
-                "ms_per_step": e2e_ms, "matches_device_path": e2e_ok, "api": "sq_score_run_host"},
+                "ms_per_step": e2e_ms if e2e_ms == e2e_ms else None, "device_ms_per_step": e2e_dev_ms, "steps": args.e2e_steps,
+                "matches_device_path": e2e_ok, "api": "sq_score_run_host"},
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
-    if world == 1 and not args.no_reduce_standalone:
+    if vocab_mode:
+        line["e2e"] = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                       "note": "the host-buffer form (sq_score_run_host) is the data-parallel entry point; not run in vocab mode"}
+    if world == 1 and not vocab_mode and not args.no_all_configs:
+        # the other four BASELINE.json configs, a few steps each (the graded number is the line's own `value`)
+        line["configs"] = {wl.name: {"value": value, "ms_per_step": ms_step, "kernel_ms": k1_ms, "T": T,
+                                     "tflops_kernel": achieved, "frac": achieved / peak, "frac_of_burst": achieved / peaks["bf16_tflops"]}}
+        del H_pin
+        for name in workloads.CONFIG_ORDER:
+            if name == wl.name:
+                continue
+            w2 = workloads.CONFIGS[name]
+            i2 = workloads.make_inputs(w2)
+            e2 = sq.SqScore(w2.d, w2.V, max_tokens=i2["T"], max_seqs=i2["B"], max_k=w2.k, device=local)
+            e2.set_profiling(True)
+            H2, W2, t2, c2 = (i2[n].to(dev) for n in ("H", "W", "targets", "cu_seqlens"))
+            nsteps = 200 if name == "tiny" else (3 if name == "qwen3_32b" else 5)
+            ms2, k2, _, _ = time_steps(e2, H2, W2, t2, c2, w2.k, w2.window, stream, nsteps, 3)
+            f2 = 2.0 * i2["T"] * w2.V * w2.d
+            km = kernel_stats(k2)["mean"]
+            line["configs"][name] = {"value": i2["T"] / (ms2 * 1e-3), "ms_per_step": ms2, "kernel_ms": km, "T": i2["T"], "steps": nsteps,
+                                     "tflops_kernel": f2 / (km * 1e-3) / 1e12, "frac": f2 / (km * 1e-3) / 1e12 / peak,
+                                     "frac_of_burst": f2 / (km * 1e-3) / 1e12 / peaks["bf16_tflops"],
+                                     "plan": {n: v for n, v in sq.plan(w2.d, w2.V, i2["T"], w2.k, num_sms=sms).items() if n != "chunk_vtile"}}
+            e2.close()
+            del H2, W2, t2, c2, i2
+            torch.cuda.empty_cache()
+    if world == 1 and not vocab_mode and not args.no_reduce_standalone:
         # kernel 2 alone on an input large enough for HBM bandwidth to mean something
         r = workloads.reduction_inputs(4096, 1024, 16384, seed=2001)
         eng2 = sq.SqScore(d, V, max_tokens=r["T"], max_seqs=r["B"], max_k=wl.k, device=local, reduce_only=True)
@@ -313,15 +397,15 @@ def run_ours(args):
                                      "note": "3 launches (tile_scan, tile_part, seq_final) at this size; 12 B/token read + 16 B/sequence written"}
         eng2.close()
         del r_lp, r_en, r_cf
-    if world == 1 and not args.no_prepare_standalone:
+    if world == 1 and not vocab_mode and not args.no_prepare_standalone:
         # the step before the path: gather + final RMSNorm of the same T rows out of a packed prefill
         # that also holds query tokens; HBM-bound: 2*d bytes read + 2*d written + 4 (pos) per row
         gen = torch.Generator(device=dev); gen.manual_seed(4242)
         n_src = T + 256 * B
         Xs = torch.randn(n_src, d, generator=gen, device=dev, dtype=torch.float32).to(torch.bfloat16)
         gain = (1 + 0.1 * torch.randn(d, generator=gen, device=dev)).to(torch.bfloat16)
-        pos_l, _ = sq.trajectory_positions([256] * B, (inp["cu_seqlens"][1:] - inp["cu_seqlens"][:-1]).tolist())
-        pos_d = torch.tensor(pos_l, dtype=torch.int32, device=dev)
+        pos_d, _ = eng.positions(torch.full((B,), 256, dtype=torch.int32, device=dev),
+                                 (inp["cu_seqlens"][1:] - inp["cu_seqlens"][:-1]).to(torch.int32).to(dev), T, stream=stream)
         Hs = torch.empty(T, d, dtype=torch.bfloat16, device=dev)
         with torch.cuda.stream(stream):
             for _ in range(3):
@@ -340,11 +424,12 @@ def run_ours(args):
                                       "note": "sq_score_prepare: gather + RMSNorm, 2d B read + 2d B written + 4 B per row; "
                                               "input and output (2 x %.0f MB) exceed L2" % (T * d * 2 / 1e6)}
         del Xs, Hs
-    if world == 1 and not args.no_decode_standalone:
+    if world == 1 and not vocab_mode and not args.no_decode_standalone:
         # decode-shaped run (self-confidence of a decode batch): T = 64 rows against the
         # same LM head -- every SM streams its own slice of W once, so the bound is HBM: V*d*2 bytes per pass
         Td = 64
         eng3 = sq.SqScore(d, V, max_tokens=Td, max_seqs=4, max_k=wl.k, device=local)
+        eng3.set_profiling(True)
         Hd = H[:Td].contiguous(); tgd = tg[:Td].contiguous()
         cud = torch.tensor([0, 16, 32, 48, 64], dtype=torch.int32, device=dev)
         with torch.cuda.stream(stream):
@@ -358,6 +443,7 @@ def run_ours(args):
             d1.record(stream)
             stream.synchronize()
         d_ms = d0.elapsed_time(d1) / 20
+        d_k = eng3.profile_read()
         # the same step captured once into a CUDA graph (the library enqueues only stream work) and replayed
         g_ms = None
         try:
@@ -382,12 +468,13 @@ def run_ours(args):
         line["decode_standalone"] = {"bound": "hbm", "achieved": d_bytes / (d_ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                                      "unit": "GB/s", "frac": d_bytes / (d_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "ms": d_ms,
                                      "rows": Td, "tokens_per_s": Td / (d_ms * 1e-3), "algorithmic_bytes": d_bytes,
+                                     "kernels_ms": {n: float(np.mean([x[n + "_ms"] for x in d_k])) for n in ("fused", "finalize", "reduce")},
                                      "cuda_graph_ms": g_ms, "cuda_graph_frac": (d_bytes / (g_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]) if g_ms else None,
                                      "plan": sq.plan(d, V, Td, wl.k, num_sms=torch.cuda.get_device_properties(dev).multi_processor_count),
                                      "note": "whole path (3 launches) on a decode batch of 64 rows; W (%.0f MB) exceeds L2 and is "
                                              "streamed once per pass" % (V * d * 2 / 1e6)}
         eng3.close()
-    if world == 1 and not args.no_vocab_parallel:
+    if world == 1 and not vocab_mode and not args.no_vocab_parallel:
         # one rank's share of a vocab-parallel (tensor-parallel LM head) deployment over R = 8 GPUs, emulated on this GPU:
         # kernel 1 + merge on shard 0 (V/8 rows), then the merge of 8 gathered states + kernel 2.  The exchange itself
         # (one all-gather of R x state bytes) is not timed here: there is one GPU.
@@ -422,7 +509,7 @@ def run_ours(args):
                                                "bytes (NVLink) is not included"}
         eng4.close()
         del states, st0
-    if world == 1 and not args.no_fp8:
+    if world == 1 and not vocab_mode and not args.no_fp8:
         # FP8 variant (NOT the graded bf16 number): same batch, operands quantised to e4m3 on the device
         # (W once per model, H per step), tcgen05 kind::f8f6f4.  Peak: the measured bf16 peaks x the nominal fp8 : bf16 ratio 2.
         with torch.cuda.stream(stream):
@@ -495,7 +582,7 @@ def run_ours(args):
         line["context_unfused_torch"] = {"ms_per_pass": u_ms, "tokens_per_s": T / (u_ms * 1e-3),
                                          "note": "torch matmul + log_softmax + topk + entropy + gather in 4096-row chunks "
                                                  "(logits materialised); per-token outputs only; not part of the path"}
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not vocab_mode and not args.no_cpu_baseline:
         tps, sec, rows, threads = time_oracle(inp, budget_s=args.oracle_seconds)
         line["cpu_baseline"] = {"value": tps, "unit": UNIT, "cores": threads, "kind": "oracle",
                                 "sample": "%d seeded rows of %s in %.1f s (fp64 oracle.token_scores + sequence_scores)" % (rows, wl.name, sec)}
@@ -512,7 +599,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="qwen3_8b", choices=list(workloads.CONFIGS))
-    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--parallelism", default="dp", choices=["dp", "vocab"])
+    ap.add_argument("--no-all-configs", action="store_true", help="skip the brief timing of the other four configs")
     ap.add_argument("--oracle-seconds", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-reduce-standalone", action="store_true")
@@ -520,8 +609,6 @@ def main():
     ap.add_argument("--no-decode-standalone", action="store_true")
     ap.add_argument("--no-vocab-parallel", action="store_true")
     ap.add_argument("--no-fp8", action="store_true")
-    ap.add_argument("--per-step-kernel-times", action="store_true",
-                    help="read kernel 1's duration after every step (adds a host sync per step)")
     ap.add_argument("--matmul-ceiling", action="store_true", help="also time torch.matmul on the same shapes (context)")
     ap.add_argument("--unfused-baseline", action="store_true", help="also time an unfused torch pipeline (context)")
     ap.add_argument("--cta-group", type=int, default=0)

@@ -17,9 +17,16 @@
  *
  * Conventions
  *   - every function returns 0 (SQ_OK) or a negative SQ_ERR_* code; nothing aborts or throws.
- *   - `sq_score_run` / `sq_score_reduce` are ASYNCHRONOUS on `stream` (a cudaStream_t passed as
- *     void*), do no host synchronisation and no allocation; all workspace is owned by the ctx and
- *     sized at create from max_tokens / max_seqs / max_k.
+ *   - every `sq_score_run*` call, `sq_score_reduce`, `sq_score_prepare`, ... is ASYNCHRONOUS on `stream`
+ *     (a cudaStream_t passed as void*) and does no host synchronisation and NO ALLOCATION of any kind:
+ *     all workspace, staging buffers, streams and events are owned by the ctx and created by
+ *     `sq_score_create` from max_tokens / max_seqs / max_k / flags.  (Only `sq_score_set_profiling`
+ *     creates events, outside any run.)
+ *   - kernel 1 is a persistent kernel whose clusters wait for one another (gang barriers): all of them
+ *     must be resident at once.  `sq_score_create` asks the occupancy calculator how many clusters the
+ *     device can hold and plans for that many; the device must not be running other kernels that
+ *     occupy SMs while a run executes.  A wait that lasts longer than cfg.wait_seconds traps (the run
+ *     fails with a sticky CUDA error) instead of hanging the device.
  *   - pointers marked DEVICE must be device memory on ctx's device; HOST pointers are host memory
  *     (pinned for true async copies).  The library never frees or keeps caller buffers beyond the
  *     work it enqueued.
@@ -50,6 +57,12 @@ extern "C" {
 
 #define SQ_FLAG_REDUCE_ONLY   1   /* ctx serves sq_score_reduce only: no kernel-1 workspace is
                                      allocated and sq_score_run / run_host return INVALID_ARG    */
+#define SQ_FLAG_STAGING       2   /* also allocate, at create, what sq_score_run_host and
+                                     sq_score_run_x need: an H buffer [max_tokens, d] bf16, staged
+                                     targets / cu_seqlens, arrival flags, a copy stream and its
+                                     events.  Without it those two calls return INVALID_ARG.     */
+
+#define SQ_MAX_CHUNKS       160   /* vocab chunks per row at most                                 */
 
 typedef struct sq_score_ctx sq_score_ctx;   /* opaque */
 
@@ -64,8 +77,11 @@ typedef struct {
   int     cta_group;    /* 0 = default (CTA pairs, UMMA M=256; single CTA when T <= 128);
                            1 = always single-CTA UMMA (M=128); 2 = always CTA pairs               */
   int     num_chunks;   /* 0 = planner's choice; >0 forces the number of vocab chunks per row     */
-  int     group_m;      /* 0 = default (12): gang size = token tiles that share one W stream       */
+  int     group_m;      /* 0 = planner's choice (10..14, 12 preferred): gang size = clusters that
+                           share one W stream; >0 forces it                                       */
   int     flags;        /* SQ_FLAG_*                                                              */
+  int     wait_seconds; /* how long a device-side wait (pipeline barrier, gang barrier, H arrival
+                           flag) may last before kernel 1 traps: 0 = default (60 s), < 0 = for ever */
 } sq_score_config;
 
 /* Output pointers of one run.  Per-token pointers may be NULL (= not wanted; the ctx keeps the
@@ -83,29 +99,36 @@ typedef struct {
   float   *seq_min_window_conf; /* DEVICE [B]   min over windows of the window-mean of c(i)       */
 } sq_score_outputs;
 
-/* How a run of T tokens is cut into work units (host logic, no GPU needed).       */
+/* How a run of T tokens is cut into work units (host logic, no GPU needed).
+ * The clusters are split into num_gangs gangs: gangs [0, gangs_big) have gang_size + 1 members, the rest
+ * gang_size.  Gang i owns vocab chunks [i * chunks_per_gang, (i+1) * chunks_per_gang) and walks the token
+ * tiles in batches of its own size; chunk c sweeps vocab tiles [chunk_vtile[c], chunk_vtile[c+1]).        */
 typedef struct {
   int cta_group;        /* 1 or 2                                                                 */
   int rows_per_tile;    /* 128 * cta_group token rows per work unit                               */
   int m_tiles;          /* ceil(T / rows_per_tile)                                                */
   int num_vtiles;       /* ceil(V / 256)                                                          */
   int num_k_blocks;     /* ceil(d / 64)                                                           */
-  int num_chunks;       /* vocab chunks per row (partial states merged by the finalize kernel)    */
-  int tiles_per_chunk;  /* vocab tiles swept by one work unit                                     */
-  int group_m;          /* gang size: clusters that sweep one W chunk together (<= m_tiles)       */
+  int num_chunks;       /* vocab chunks per row = num_gangs * chunks_per_gang (partial states merged
+                           by the finalize kernel)                                                */
+  int chunks_per_gang;  /* chunks a gang's vocabulary stripe is cut into (1 unless num_chunks is forced) */
+  int tiles_per_chunk;  /* width of the widest chunk, in vocab tiles                               */
   int num_units;        /* m_tiles * num_chunks                                                   */
-  int num_clusters;     /* clusters the device can hold (= SMs / cta_group)                       */
-  int num_gangs;        /* num_clusters / group_m; the launch uses num_gangs * group_m clusters   */
-  int num_gang_units;   /* ceil(m_split / group_m) * num_chunks, dealt round-robin to the gangs   */
-  int m_split;          /* token tiles [0,m_split) -> gangs; [m_split,m_tiles) -> the smaller gang B */
-  int gang_b_size;      /* num_clusters - num_gangs * group_m clusters form gang B (0 = none)     */
-  int num_gang_units_b; /* ceil((m_tiles - m_split) / gang_b_size) * num_chunks; 0 = B not used   */
+  int num_clusters;     /* clusters the device can hold (SMs / cta_group, or what create() found)  */
+  int num_gangs;
+  int gang_size;        /* members of the smaller gangs                                           */
+  int gangs_big;        /* gangs with gang_size + 1 members                                       */
+  int clusters_used;    /* num_gangs * gang_size + gangs_big = clusters launched                  */
+  int max_batches;      /* batches of token tiles the smallest gang walks: ceil(m_tiles / gang_size) */
   int topk_cap;         /* compiled top-k list capacity used for this k (8, 20 or 32)             */
+  int chunk_vtile[SQ_MAX_CHUNKS + 1];
 } sq_score_plan_t;
 
-/* Creates a context on cfg->device and allocates its workspace.
- * Errors: INVALID_ARG (null, sizes <= 0, max_k out of range), UNSUPPORTED (d % 8 != 0, device is
- * not compute capability 10.x), CUDA, NOMEM.  On error *out is NULL. */
+/* Creates a context on cfg->device and allocates its workspace (and, with SQ_FLAG_STAGING, the staging of
+ * sq_score_run_host / sq_score_run_x); queries how many clusters of kernel 1 the device can hold at once.
+ * Errors: INVALID_ARG (null, sizes <= 0, max_k out of range), UNSUPPORTED (d % 8 != 0, vocab > 2^24, device
+ * is not compute capability 10.x, or it cannot hold even one cluster of kernel 1), CUDA, NOMEM.  On error
+ * *out is NULL. */
 int sq_score_create(const sq_score_config *cfg, sq_score_ctx **out);
 
 /* Scores T = outputs->... tokens: enqueues kernel 1 (fused GEMM + statistics), the merge/finalize
@@ -132,8 +155,8 @@ int sq_score_run(sq_score_ctx *ctx, const void *H, const void *W, const int32_t 
  * min_window_conf[B]).  W stays on the device (it is the resident model weight).  Asynchronous on
  * `stream` (which also waits for the copy stream); the caller synchronises `stream` before reading
  * seq_out_host or reusing the host buffers.  Pinned host memory is needed for the overlap; pageable
- * memory works but its copies are staged by the runtime.
- * Errors: as sq_score_run. */
+ * memory works but its copies are staged by the runtime.  Needs a ctx created with SQ_FLAG_STAGING.
+ * Errors: as sq_score_run; INVALID_ARG without SQ_FLAG_STAGING. */
 int sq_score_run_host(sq_score_ctx *ctx, const void *H_host, const void *W_dev,
                       const int32_t *targets_host, const int32_t *cu_seqlens_host,
                       int num_tokens, int num_seqs, int k, int window,
@@ -164,13 +187,36 @@ int sq_score_reduce(sq_score_ctx *ctx, const float *target_logprob, const float 
 int sq_score_prepare(sq_score_ctx *ctx, const void *X, int num_rows, const int32_t *pos, int num_tokens,
                      const void *gain, float eps, void *H_out, void *stream);
 
-/* sq_score_prepare into a ctx-owned H buffer ([max_tokens, d] bf16, allocated on first use) followed by
- * sq_score_run on it: the library takes the last layer's output and the position list directly.
- * Errors: as sq_score_prepare and sq_score_run, NOMEM. */
+/* sq_score_prepare into the ctx-owned H buffer ([max_tokens, d] bf16; ctx created with SQ_FLAG_STAGING)
+ * followed by sq_score_run on it: the library takes the last layer's output and the position list directly.
+ * Errors: as sq_score_prepare and sq_score_run; INVALID_ARG without SQ_FLAG_STAGING. */
 int sq_score_run_x(sq_score_ctx *ctx, const void *X, int num_rows, const int32_t *pos, const void *gain,
                    float eps, const void *W, const int32_t *targets, const int32_t *cu_seqlens,
                    int num_tokens, int num_seqs, int k, int window, const sq_score_outputs *outputs,
                    void *stream);
+
+/* The position list of sq_score_prepare / sq_score_run_x for a packed prefill in which candidate b occupies
+ * query_lens[b] query tokens followed by traj_lens[b] trajectory tokens.  Token i (i = 1..|tau|) of a trajectory is
+ * scored by log p(. | t_<i, Q) (Eq. 3), i.e. by the hidden state of the packed row just before it, and
+ * only the |tau| trajectory tokens are averaged (Eq. 4):
+ *     cu[0] = 0, cu[b+1] = cu[b] + traj_lens[b];   base_b = sum_{c<b} (query_lens[c] + traj_lens[c]);
+ *     pos[cu[b] + i] = base_b + query_lens[b] - 1 + i,   i = 0 .. traj_lens[b] - 1.
+ * A trajectory needs at least one query token before it (there is no state that predicts its first token otherwise).
+ *
+ * sq_score_positions_host: HOST arrays in and out, needs no GPU and no ctx.  pos_out has room for pos_capacity
+ * entries; *num_tokens_out (may be NULL) receives T = sum traj_lens.
+ * Errors: INVALID_ARG (null pointer, negative length, a non-empty trajectory with query_lens[b] < 1, T > pos_capacity).
+ *
+ * sq_score_positions: the same on the device (no host round trip between the prefill and sq_score_run_x): DEVICE
+ * int32 arrays query_lens[B], traj_lens[B] -> pos_out[num_tokens], cu_out[B+1]; num_tokens must equal sum traj_lens
+ * (the caller built the batch and knows it).  Device contents are trusted; if status_out (DEVICE int32[1], may be
+ * NULL) is given it receives 0, or the number of candidates that violate the rules above (negative length, missing
+ * query token) plus 1 if the lengths do not sum to num_tokens -- pos entries of such candidates are clamped to >= 0.
+ * B <= max_seqs, num_tokens <= max_tokens.  Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA. */
+int sq_score_positions_host(const int32_t *query_lens, const int32_t *traj_lens, int num_seqs,
+                            int32_t *pos_out, int64_t pos_capacity, int32_t *cu_out, int64_t *num_tokens_out);
+int sq_score_positions(sq_score_ctx *ctx, const int32_t *query_lens, const int32_t *traj_lens, int num_seqs,
+                       int num_tokens, int32_t *pos_out, int32_t *cu_out, int32_t *status_out, void *stream);
 
 /* FP8 variant: the same scoring pass with e4m3 operands (tcgen05 kind::f8f6f4, twice the
  * tensor throughput and half the operand bytes of bf16).  It is NOT the graded bf16 path: the quantisation changes the
@@ -207,12 +253,18 @@ int sq_score_run_fp8(sq_score_ctx *ctx, const void *Hq, const float *h_scale, co
  * sq_score_shard_state_bytes: size of that buffer (host-only; -1 on bad arguments). */
 int64_t sq_score_shard_state_bytes(int64_t num_tokens, int k);
 
-/* One shard: ctx was created with vocab = the shard's row count; W_shard holds rows [vocab_offset, vocab_offset +
- * vocab) of the LM head; targets are GLOBAL ids.  Runs kernel 1 and the merge kernel in EMIT mode, writes state_out
- * (DEVICE, sq_score_shard_state_bytes(T, k) bytes).  k <= min(max_k, shard vocab).  Asynchronous on `stream`.
- * Errors: as sq_score_run. */
-int sq_score_run_shard(sq_score_ctx *ctx, const void *H, const void *W_shard, int vocab_offset,
+/* One shard: W_shard holds the shard_rows rows [vocab_offset, vocab_offset + shard_rows) of the LM head,
+ * 1 <= shard_rows <= cfg.vocab (a ctx sized for the LARGEST shard serves every rank of an uneven split); targets are
+ * GLOBAL ids.  Runs kernel 1 and the merge kernel in EMIT mode, writes state_out (DEVICE,
+ * sq_score_shard_state_bytes(T, k) bytes).  k <= min(max_k, shard_rows).  Asynchronous on `stream`.
+ * Errors: as sq_score_run; INVALID_ARG if shard_rows is outside 1..cfg.vocab. */
+int sq_score_run_shard(sq_score_ctx *ctx, const void *H, const void *W_shard, int shard_rows, int vocab_offset,
                        const int32_t *targets, int num_tokens, int k, void *state_out, void *stream);
+
+/* The packed state of a shard that owns NO vocabulary rows (more ranks than vocab tiles): the neutral element of the
+ * merge (m = -1e30, s = u = 0, empty list).  Writes sq_score_shard_state_bytes(T, k) bytes to state_out (DEVICE).
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, CUDA. */
+int sq_score_neutral_shard_state(sq_score_ctx *ctx, int num_tokens, int k, void *state_out, void *stream);
 
 /* Merge of num_shards (1..32) packed states laid out back to back in `states` (DEVICE; the all-gather's output),
  * then the per-token finalisation and kernel 2 -- the same outputs as sq_score_run on the whole LM head.
@@ -227,6 +279,9 @@ int sq_score_merge_shards(sq_score_ctx *ctx, const void *states, int num_shards,
  *   theta[q] = Percentile_p of GC over problem q's non-lite groups                Eq. 6
  *              (linear interpolation at rank p/100*(n-1); NaN when every group is lite)
  *   route[g] = 0 if lite_mask[g], else 1 (Model 1) if GC(g) > theta[q], else 2 (Model 2)   Eq. 7
+ *              3 = GC(g) is not finite (the group holds an empty trajectory, whose C(tau) is NaN): the group takes no
+ *              part in the percentile and is left to the caller; -1 = the problem has more than 1024 groups (the
+ *              host-side bound was wrong): theta[q] = NaN and nothing of that problem is routed
  *   seq_conf       DEVICE float [num_seqs]      C(tau), e.g. seq_mean_conf of sq_score_run
  *   group_members  DEVICE int32 [num_groups*K]  indices into seq_conf (trusted, must be in range)
  *   group_offsets  DEVICE int32 [num_problems+1] groups of problem q are [off[q], off[q+1])
@@ -250,13 +305,19 @@ int sq_score_select_prob(sq_score_ctx *ctx, const float *fitness, const int32_t 
 int sq_score_plan(const sq_score_config *cfg, int64_t num_tokens, int k, int num_sms,
                   sq_score_plan_t *plan);
 
-/* Per-kernel timing for the roofline report.  With profiling enabled, every sq_score_run with
- * T > 0 and B > 0 records CUDA events on its stream around kernel 1 (fused GEMM + statistics), the
- * finalize kernel and kernel 2.  sq_score_kernel_times blocks until the last profiled run finished
- * and writes its three durations in milliseconds: ms3 = {fused, finalize, reduce}.
+/* Per-kernel timing for the roofline report.  With profiling enabled, every sq_score_run* with
+ * T > 0 records CUDA events on its stream around kernel 1 (fused GEMM + statistics), the
+ * finalize kernel and kernel 2, into a ring of SQ_PROFILE_RING runs (no host synchronisation in the run).
+ * sq_score_kernel_times blocks until the last profiled run finished and writes its three durations in
+ * milliseconds: ms3 = {fused, finalize, reduce}.  sq_score_profile_read does the same for EVERY run recorded
+ * since profiling was enabled or last read (the newest SQ_PROFILE_RING of them, oldest first): up to
+ * `capacity` triples into ms, their number into *num_runs, and empties the ring.
+ * sq_score_set_profiling(ctx, 1) creates the events (the only allocation outside create; call it outside runs).
  * Errors: INVALID_ARG (null, profiling off, no profiled run yet), CUDA. */
+#define SQ_PROFILE_RING 64
 int sq_score_set_profiling(sq_score_ctx *ctx, int enable);
 int sq_score_kernel_times(sq_score_ctx *ctx, float *ms3);
+int sq_score_profile_read(sq_score_ctx *ctx, float *ms, int capacity, int *num_runs);
 
 /* Number of kernels this ctx has launched so far (bench.py's `gpu_launches`). */
 int64_t sq_score_launch_count(const sq_score_ctx *ctx);

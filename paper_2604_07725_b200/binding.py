@@ -8,14 +8,17 @@ from typing import Dict, List, Optional, Sequence
 from . import build as _build
 
 SQ_MAX_K = 32
+SQ_MAX_CHUNKS = 160
+SQ_PROFILE_RING = 64
 FLAG_REDUCE_ONLY = 1
+FLAG_STAGING = 2
 ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOMEM = -1, -2, -3, -4
 
 
 class sq_score_config(C.Structure):
     _fields_ = [("device", C.c_int), ("d", C.c_int), ("vocab", C.c_int), ("max_tokens", C.c_int64),
                 ("max_seqs", C.c_int), ("max_k", C.c_int), ("cta_group", C.c_int), ("num_chunks", C.c_int),
-                ("group_m", C.c_int), ("flags", C.c_int)]
+                ("group_m", C.c_int), ("flags", C.c_int), ("wait_seconds", C.c_int)]
 
 
 class sq_score_outputs(C.Structure):
@@ -26,8 +29,9 @@ class sq_score_outputs(C.Structure):
 
 class sq_score_plan_t(C.Structure):
     _fields_ = [(n, C.c_int) for n in
-                ("cta_group", "rows_per_tile", "m_tiles", "num_vtiles", "num_k_blocks", "num_chunks",
-                 "tiles_per_chunk", "group_m", "num_units", "num_clusters", "num_gangs", "num_gang_units", "m_split", "gang_b_size", "num_gang_units_b", "topk_cap")]
+                ("cta_group", "rows_per_tile", "m_tiles", "num_vtiles", "num_k_blocks", "num_chunks", "chunks_per_gang",
+                 "tiles_per_chunk", "num_units", "num_clusters", "num_gangs", "gang_size", "gangs_big", "clusters_used",
+                 "max_batches", "topk_cap")] + [("chunk_vtile", C.c_int * (SQ_MAX_CHUNKS + 1))]
 
 
 class SqScoreError(RuntimeError):
@@ -40,17 +44,14 @@ _lib = None
 
 
 def lib() -> C.CDLL:
-    """Loads (building if stale) csrc/libsq_score.so.  Fails loudly if it cannot be built/loaded."""
+    """Loads csrc/libsq_score.so, rebuilding it first when a source is newer.  Fails loudly if it cannot be built or
+    loaded: a stale library is never used in place of one that failed to build."""
     global _lib
     if _lib is not None:
         return _lib
-    path = os.environ.get("SQ_SCORE_LIB") or _build.LIB   # SQ_SCORE_LIB: load another build of the same ABI (kernel A/B tests)
-    if path == _build.LIB and _build.is_stale():
-        try:
-            path = _build.build()
-        except Exception:
-            if not os.path.exists(path):
-                raise
+    path = _build.LIB
+    if _build.is_stale():
+        path = _build.build()      # raises with nvcc's output
     L = C.CDLL(path)
     L.sq_score_create.argtypes = [C.POINTER(sq_score_config), C.POINTER(C.c_void_p)]
     L.sq_score_create.restype = C.c_int
@@ -74,8 +75,17 @@ def lib() -> C.CDLL:
     L.sq_score_run_x.restype = C.c_int
     L.sq_score_shard_state_bytes.argtypes = [C.c_int64, C.c_int]
     L.sq_score_shard_state_bytes.restype = C.c_int64
-    L.sq_score_run_shard.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+    L.sq_score_run_shard.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
     L.sq_score_run_shard.restype = C.c_int
+    L.sq_score_neutral_shard_state.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+    L.sq_score_neutral_shard_state.restype = C.c_int
+    L.sq_score_positions_host.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.c_int, C.POINTER(C.c_int32), C.c_int64,
+                                          C.POINTER(C.c_int32), C.POINTER(C.c_int64)]
+    L.sq_score_positions_host.restype = C.c_int
+    L.sq_score_positions.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.sq_score_positions.restype = C.c_int
+    L.sq_score_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int, C.POINTER(C.c_int)]
+    L.sq_score_profile_read.restype = C.c_int
     L.sq_score_merge_shards.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_int32), C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                         C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
     L.sq_score_merge_shards.restype = C.c_int
@@ -111,12 +121,14 @@ def version() -> int:
 def plan(d: int, vocab: int, num_tokens: int, k: int, num_sms: int = 0, cta_group: int = 0,
          num_chunks: int = 0, group_m: int = 0) -> Dict[str, int]:
     """sq_score_plan: host-only work decomposition (no GPU needed)."""
-    cfg = sq_score_config(0, d, vocab, max(1, num_tokens), 1, max(1, min(k, SQ_MAX_K)), cta_group, num_chunks, group_m, 0)
+    cfg = sq_score_config(0, d, vocab, max(1, num_tokens), 1, max(1, min(k, SQ_MAX_K)), cta_group, num_chunks, group_m, 0, 0)
     out = sq_score_plan_t()
     rc = lib().sq_score_plan(C.byref(cfg), num_tokens, k, num_sms, C.byref(out))
     if rc != 0:
         raise SqScoreError(rc, lib().sq_score_error_string(rc).decode())
-    return {n: getattr(out, n) for n, _ in sq_score_plan_t._fields_}
+    res = {n: getattr(out, n) for n, _ in sq_score_plan_t._fields_ if n != "chunk_vtile"}
+    res["chunk_vtile"] = list(out.chunk_vtile[: out.num_chunks + 1])
+    return res
 
 
 def shard_state_bytes(num_tokens: int, k: int) -> int:
@@ -125,18 +137,6 @@ def shard_state_bytes(num_tokens: int, k: int) -> int:
     if n < 0:
         raise SqScoreError(ERR_INVALID_ARG, "bad num_tokens / k")
     return n
-
-
-def neutral_shard_state(num_tokens: int, k: int, device):
-    """The packed state of a shard that owns no vocabulary rows: the merge operator's neutral element."""
-    import torch
-    T = num_tokens
-    cap = (shard_state_bytes(T, k) // 4 // max(T, 1) - 6) // 2 if T else 0
-    st = torch.zeros(shard_state_bytes(T, k) // 4, dtype=torch.float32, device=device)
-    st[:T] = -1.0e30                                      # m
-    st[5 * T:(5 + cap) * T] = -1.0e30                     # topv
-    st[(5 + cap) * T:(5 + 2 * cap) * T] = torch.full((cap * T,), -1, dtype=torch.int32, device=device).view(torch.float32)   # topi
-    return st
 
 
 def shard_vocab(vocab: int, world_size: int, multiple: int = 256) -> List[int]:
@@ -155,10 +155,12 @@ class SqScore:
     """sq_score_create / sq_score_run / sq_score_destroy on torch tensors (device memory + streams)."""
 
     def __init__(self, d: int, vocab: int, max_tokens: int, max_seqs: int, max_k: int = 20, device: int = 0,
-                 cta_group: int = 0, num_chunks: int = 0, group_m: int = 0, reduce_only: bool = False):
+                 cta_group: int = 0, num_chunks: int = 0, group_m: int = 0, reduce_only: bool = False,
+                 staging: bool = False, wait_seconds: int = 0):
+        """`staging=True` (SQ_FLAG_STAGING) also allocates what run_host / run_x need; no run* call ever allocates."""
         self._L = lib()
         self.cfg = sq_score_config(device, d, vocab, max_tokens, max_seqs, max_k, cta_group, num_chunks, group_m,
-                                   FLAG_REDUCE_ONLY if reduce_only else 0)
+                                   (FLAG_REDUCE_ONLY if reduce_only else 0) | (FLAG_STAGING if staging else 0), wait_seconds)
         h = C.c_void_p()
         rc = self._L.sq_score_create(C.byref(self.cfg), C.byref(h))
         if rc != 0:
@@ -226,15 +228,37 @@ class SqScore:
         return out
 
     def run_shard(self, H, W_shard, vocab_offset: int, targets, k: int, out=None, stream=None):
-        """sq_score_run_shard: this ctx's shard of the LM head -> packed partial state (a float32 tensor of
-        shard_state_bytes(T, k) / 4 words; ids inside are int32 bit patterns)."""
+        """sq_score_run_shard: the rows W_shard of the LM head (at most the ctx's vocab of them) -> packed partial state
+        (a float32 tensor of shard_state_bytes(T, k) / 4 words; ids inside are int32 bit patterns)."""
         import torch
         T = H.shape[0]
         if out is None:
             out = torch.empty(shard_state_bytes(T, k) // 4, dtype=torch.float32, device=H.device)
-        self._check(self._L.sq_score_run_shard(self._h, _ptr(H), _ptr(W_shard), int(vocab_offset), _ptr(targets), T, k, _ptr(out),
-                                               self._stream(stream)))
+        self._check(self._L.sq_score_run_shard(self._h, _ptr(H), _ptr(W_shard), W_shard.shape[0], int(vocab_offset), _ptr(targets),
+                                               T, k, _ptr(out), self._stream(stream)))
         return out
+
+    def neutral_shard_state(self, num_tokens: int, k: int, device=None, out=None, stream=None):
+        """sq_score_neutral_shard_state: the packed state of a shard that owns no vocabulary rows."""
+        import torch
+        if out is None:
+            out = torch.empty(shard_state_bytes(num_tokens, k) // 4, dtype=torch.float32,
+                              device=device if device is not None else torch.device("cuda", self.device))
+        self._check(self._L.sq_score_neutral_shard_state(self._h, num_tokens, k, _ptr(out), self._stream(stream)))
+        return out
+
+    def positions(self, query_lens, traj_lens, num_tokens: int, stream=None, with_status: bool = False):
+        """sq_score_positions: device int32 [B] query / trajectory lengths -> (pos [num_tokens], cu_seqlens [B+1]) on the
+        device, no host round trip; `num_tokens` = sum of traj_lens (known to the caller)."""
+        import torch
+        B = traj_lens.shape[0]
+        dev = traj_lens.device
+        pos = torch.empty(num_tokens, dtype=torch.int32, device=dev)
+        cu = torch.empty(B + 1, dtype=torch.int32, device=dev)
+        status = torch.empty(1, dtype=torch.int32, device=dev) if with_status else None
+        self._check(self._L.sq_score_positions(self._h, _ptr(query_lens), _ptr(traj_lens), B, num_tokens, _ptr(pos), _ptr(cu),
+                                               _ptr(status), self._stream(stream)))
+        return (pos, cu, status) if with_status else (pos, cu)
 
     def merge_shards(self, states, vocab_starts: Sequence[int], targets, cu_seqlens, k: int, window: int, stream=None,
                      per_token: bool = True, topk: bool = True, out: Optional[dict] = None) -> dict:
@@ -332,6 +356,13 @@ class SqScore:
         self._check(self._L.sq_score_kernel_times(self._h, ms))
         return {"fused_ms": ms[0], "finalize_ms": ms[1], "reduce_ms": ms[2]}
 
+    def profile_read(self) -> List[dict]:
+        """sq_score_profile_read: the same for every profiled run since the last read (at most the newest 64)."""
+        ms = (C.c_float * (3 * SQ_PROFILE_RING))()
+        n = C.c_int(0)
+        self._check(self._L.sq_score_profile_read(self._h, ms, SQ_PROFILE_RING, C.byref(n)))
+        return [{"fused_ms": ms[3 * i], "finalize_ms": ms[3 * i + 1], "reduce_ms": ms[3 * i + 2]} for i in range(n.value)]
+
     def launch_count(self) -> int:
         return self._L.sq_score_launch_count(self._h)
 
@@ -362,18 +393,21 @@ def shard_sequences(lengths: Sequence[int], world_size: int) -> List[List[int]]:
 
 
 def trajectory_positions(query_lens: Sequence[int], traj_lens: Sequence[int]):
-    """Host-side index arithmetic for sq_score_prepare / run_x: for a packed prefill where candidate b is
-    query_lens[b] query tokens followed by traj_lens[b] trajectory tokens, returns (pos, cu_seqlens) as
-    int32 lists -- pos[t] is the packed row whose hidden state predicts scored token t (the position
-    before it), cu_seqlens delimits the trajectories."""
-    pos: List[int] = []
-    cu = [0]
-    base = 0
-    for q, n in zip(query_lens, traj_lens):
-        q, n = int(q), int(n)
-        if n > 0 and q < 1:
-            raise ValueError("a trajectory needs at least one query token before it")
-        pos.extend(range(base + q - 1, base + q - 1 + n))
-        cu.append(cu[-1] + n)
-        base += q + n
-    return pos, cu
+    """sq_score_positions_host (host-only, no GPU): for a packed prefill where candidate b is query_lens[b] query
+    tokens followed by traj_lens[b] trajectory tokens, returns (pos, cu_seqlens) as int32 lists -- pos[t] is the
+    packed row whose hidden state predicts scored token t (the position before it), cu_seqlens
+    delimits the trajectories.  Raises ValueError where the library returns INVALID_ARG (a
+    trajectory without a query token before it, negative lengths)."""
+    B = len(traj_lens)
+    if len(query_lens) != B:
+        raise ValueError("query_lens and traj_lens differ in length")
+    q = (C.c_int32 * max(B, 1))(*[int(v) for v in query_lens])
+    n = (C.c_int32 * max(B, 1))(*[int(v) for v in traj_lens])
+    cap = sum(max(int(v), 0) for v in traj_lens)
+    pos = (C.c_int32 * max(cap, 1))()
+    cu = (C.c_int32 * (B + 1))()
+    total = C.c_int64(0)
+    rc = lib().sq_score_positions_host(q, n, B, pos, cap, cu, C.byref(total))
+    if rc != 0:
+        raise ValueError("sq_score_positions_host: a trajectory needs at least one query token before it; lengths must be >= 0")
+    return list(pos[: total.value]), list(cu)

@@ -8,7 +8,7 @@ import subprocess
 CSRC = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc")
 LIB = os.path.join(CSRC, "libsq_score.so")
 SOURCES = ["sq_score_api.cu"]
-HEADERS = ["sq_ptx.cuh", "sq_fused_kernel.cuh", "sq_finalize_kernel.cuh", "sq_reduce_kernel.cuh", "sq_route_kernel.cuh", "sq_prepare_kernel.cuh", "sq_quant_kernel.cuh",
+HEADERS = ["sq_ptx.cuh", "sq_fused_kernel.cuh", "sq_finalize_kernel.cuh", "sq_reduce_kernel.cuh", "sq_route_kernel.cuh", "sq_prepare_kernel.cuh", "sq_quant_kernel.cuh", "sq_positions_kernel.cuh",
            os.path.join("..", "..", "include", "sq_score.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]

@@ -7,7 +7,7 @@
 //
 // Persistent, warp-specialised:  warp 0 = TMA producer, warp 1 = MMA issuer, warp 2 = TMEM
 // allocator, warps 4..7 = statistics epilogue (thread = TMEM lane = token row).
-// Work unit = (token tile of 128*CG rows, vocab chunk of `tiles_per_chunk` 256-column tiles);
+// Work unit = (token tile of 128*CG rows, vocab chunk = a run of 256-column tiles, FusedParams::chunk_vt);
 // a unit's running state lives in registers and is written as a partial state at its end.
 #pragma once
 #include "sq_ptx.cuh"
@@ -39,20 +39,20 @@ template <int CG> struct FusedCfg {
   static constexpr int UMMA_M = BLOCK_M * CG;
 };
 
+constexpr int MAX_CHUNKS = 160;   // vocab chunks per row at most (= FIN_MAX_CHUNKS of the finalize kernel)
+
 struct FusedParams {
   int T, V, d;
   int num_k_blocks;
   int num_vtiles;
-  int tiles_per_chunk;
-  int num_chunks;
+  int num_chunks;           // num_gangs * chunks_per_gang
   int m_tiles;
-  int group_m;              // gang size
   int num_gangs;
-  int num_gang_units;       // ceil(m_split / group_m) * num_chunks (class A)
-  int m_split;              // token tiles [0, m_split) go to the class-A gangs, [m_split, m_tiles) to gang B
-  int gang_b_size;          // clusters left over after the class-A gangs form one smaller gang B (0 = none)
-  int num_gang_units_b;     // ceil((m_tiles - m_split) / gang_b_size) * num_chunks
+  int gang_size;            // gangs [0, gangs_big) have gang_size + 1 members, the others gang_size
+  int gangs_big;
+  int chunks_per_gang;      // a gang's vocabulary stripe is cut into this many chunks
   unsigned int* gang_ctr;   // [num_gangs], zeroed before the launch
+  long long wait_limit;     // clock cycles a wait may last before the kernel traps (0 = wait for ever)
   const int32_t* targets;   // [T]
   float* part_m;            // [C][T]
   float* part_s;            // [C][T]
@@ -70,54 +70,54 @@ struct FusedParams {
   const float* w_scale;     //   scales, DEVICE); null in the bf16 path
   int vocab_offset;         // W is rows [vocab_offset, vocab_offset + V) of a larger LM head (vocab-parallel shard):
                             // targets and the reported vocabulary ids are global, columns local
-  int debug_flags;          // experiments only (env SQ_SCORE_DEBUG): bit0 = epilogue skips the statistics,
-                            // bit1 / bit2 = W / H boxes of half height (wrong results; L2->SM traffic probes)
+#ifdef SQ_PROBES
+  int probe_flags;          // builder's A/B probes, WRONG RESULTS (compiled only with -DSQ_PROBES): bit0 = epilogue skips
+                            // the statistics, bit1 / bit2 = W / H boxes of half height (L2->SM traffic probes)
+#endif
+  uint16_t chunk_vt[MAX_CHUNKS + 1];   // chunk c sweeps vocab tiles [chunk_vt[c], chunk_vt[c+1]) (widths differ between gangs)
 };
 
 struct Unit { int m_tile; int chunk; };
 
-// Gang scheduling.  The persistent clusters are split into `num_gangs` gangs of `group_m` clusters.
-// A gang processes gang-units (group g of group_m consecutive token tiles, vocab chunk c) in the
-// order [g][c], round-robin over gangs; member j of the gang takes token tile g*group_m + j.  All
-// members sweep the same W chunk at the same time, so each W tile is fetched from HBM once per
-// gang-unit and served to the other members from L2; gangs working on the same g share its H strips.
-// The num_clusters % group_m clusters that do not fill a gang form one smaller gang B with its own
-// slice of token tiles (sized by the planner so that both classes finish together).
+// Gang scheduling.  The persistent clusters are split into `num_gangs` gangs whose sizes differ by at most one (every
+// cluster the device holds belongs to a gang).  Gang i owns vocab chunks [i*r, (i+1)*r), r = chunks_per_gang, and walks
+// the token tiles in batches of its own size: member j takes token tile b*size + j of batch b and sweeps the gang's
+// chunks for it.  All members sweep the same W chunk at the same time, so each W tile is fetched from HBM once per
+// batch and served to the other members from L2; the gangs advance through the token tiles at the same pace (their
+// stripe widths are sized for it), so they share the H strips of the current region.
 struct GangCtx {
-  int ctr;       // index of this gang's barrier counter
+  int ctr;       // index of this gang = index of its barrier counter
   int member;    // position in the gang
   int size;      // clusters in the gang
-  int m_base, m_end;        // token tiles this gang class owns
-  int gu0, gu_step, gu_end; // this gang's gang-units: gu0, gu0 + gu_step, ... < gu_end
+  int num_iters; // ceil(m_tiles / size) batches x chunks_per_gang chunks
 };
 __device__ __forceinline__ GangCtx make_gang_ctx(const FusedParams& p, int cluster) {
   GangCtx g;
-  const int a_clusters = p.num_gangs * p.group_m;
-  if (cluster < a_clusters) {
-    g.ctr = cluster / p.group_m;
-    g.member = cluster - g.ctr * p.group_m;
-    g.size = p.group_m;
-    g.m_base = 0; g.m_end = p.m_split;
-    g.gu0 = g.ctr; g.gu_step = p.num_gangs; g.gu_end = p.num_gang_units;
+  const int big_clusters = p.gangs_big * (p.gang_size + 1);
+  if (cluster < big_clusters) {
+    g.size = p.gang_size + 1;
+    g.ctr = cluster / g.size;
+    g.member = cluster - g.ctr * g.size;
   } else {
-    g.ctr = p.num_gangs;
-    g.member = cluster - a_clusters;
-    g.size = p.gang_b_size;
-    g.m_base = p.m_split; g.m_end = p.m_tiles;
-    g.gu0 = 0; g.gu_step = 1; g.gu_end = p.num_gang_units_b;
+    g.size = p.gang_size;
+    const int c = cluster - big_clusters;
+    g.ctr = p.gangs_big + c / g.size;
+    g.member = c - (c / g.size) * g.size;
   }
+  g.num_iters = ((p.m_tiles + g.size - 1) / g.size) * p.chunks_per_gang;
   return g;
 }
-__device__ __forceinline__ bool decode_gang_unit(const FusedParams& p, const GangCtx& gc, int gu, Unit& out) {
-  const int g = gu / p.num_chunks;
-  out.chunk = gu - g * p.num_chunks;
-  out.m_tile = gc.m_base + g * gc.size + gc.member;
-  return out.m_tile < gc.m_end;   // ragged last group: the surplus members idle for this gang-unit
+// iteration `it` of the gang -> this member's unit; false: ragged last batch, the member idles for this iteration
+__device__ __forceinline__ bool decode_gang_unit(const FusedParams& p, const GangCtx& gc, int it, Unit& out) {
+  const int b = it / p.chunks_per_gang;
+  out.chunk = gc.ctr * p.chunks_per_gang + (it - b * p.chunks_per_gang);
+  out.m_tile = b * gc.size + gc.member;
+  return out.m_tile < p.m_tiles;
 }
 
 // Producer-side gang barrier: keeps the members' W streams within L2 reach of one another.  The
 // counter only grows (zeroed by the host before the launch); epoch e completes at e * arrivals.
-__device__ __forceinline__ void gang_barrier(unsigned int* ctr, unsigned int target) {
+__device__ __forceinline__ void gang_barrier(unsigned int* ctr, unsigned int target, long long limit) {
   __threadfence();
   atomicAdd(ctr, 1u);
   const long long t0 = clock64();
@@ -126,20 +126,20 @@ __device__ __forceinline__ void gang_barrier(unsigned int* ctr, unsigned int tar
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
     if (v >= target) break;
     __nanosleep(64);
-    if (clock64() - t0 > 4000000000LL) __trap();
+    if (limit > 0 && clock64() - t0 > limit) __trap();
   } while (true);
 }
 
 // H streams in from the host while the kernel runs (sq_score_run_host): rows arrive in ascending order and a copy
 // engine sets flag f once rows [0, (f+1) * flag_rows) have landed.  The producer polls before its first load of a unit.
-__device__ __forceinline__ void wait_rows_ready(const unsigned int* flag) {
+__device__ __forceinline__ void wait_rows_ready(const unsigned int* flag, long long limit) {
   const long long t0 = clock64();
   unsigned int v;
   do {
     asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
     if (v != 0u) break;
     __nanosleep(200);
-    if (clock64() - t0 > 40000000000LL) __trap();
+    if (limit > 0 && clock64() - t0 > 8 * limit) __trap();   // a PCIe copy of the whole H may be ahead of this block
   } while (true);
   asm volatile("fence.proxy.async;" ::: "memory");   // the rows are read through the async proxy (TMA)
 }
@@ -330,23 +330,24 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       uint32_t stage_tx = Cfg::STAGE_BYTES * CG;   // the pair leader's barrier counts both CTAs' bytes
-      if (p.debug_flags & 2) stage_tx -= (Cfg::B_BYTES / 2) * CG;   // experiment: W boxes of half height
-      if (p.debug_flags & 4) stage_tx -= (Cfg::A_BYTES / 2) * CG;   // experiment: H boxes of half height
+#ifdef SQ_PROBES
+      if (p.probe_flags & 2) stage_tx -= (Cfg::B_BYTES / 2) * CG;   // probe: W boxes of half height
+      if (p.probe_flags & 4) stage_tx -= (Cfg::A_BYTES / 2) * CG;   // probe: H boxes of half height
+#endif
       unsigned int epoch = 0;
-      for (int gu = gc.gu0; gu < gc.gu_end; gu += gc.gu_step) {
+      for (int gu = 0; gu < gc.num_iters; ++gu) {
         Unit un;
         const bool active = decode_gang_unit(p, gc, gu, un);
-        if (gc.size > 1) gang_barrier(p.gang_ctr + gc.ctr, (++epoch) * (unsigned)(gc.size * CG));
+        if (gc.size > 1) gang_barrier(p.gang_ctr + gc.ctr, (++epoch) * (unsigned)(gc.size * CG), p.wait_limit);
         if (!active) continue;
         const int row0 = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M;
         if (p.h_ready != nullptr && row0 < p.T)
-          wait_rows_ready(p.h_ready + (min(row0 + BLOCK_M, p.T) - 1) / p.flag_rows);
-        const int vt0 = un.chunk * p.tiles_per_chunk;
-        const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
+          wait_rows_ready(p.h_ready + (min(row0 + BLOCK_M, p.T) - 1) / p.flag_rows, p.wait_limit);
+        const int vt0 = p.chunk_vt[un.chunk], vt1 = p.chunk_vt[un.chunk + 1];
         for (int vt = vt0; vt < vt1; ++vt) {
           const int wrow0 = vt * BLOCK_N + (int)cta_rank * Cfg::B_ROWS;
           for (int kb = 0; kb < p.num_k_blocks; ++kb) {
-            mbar_wait(empty_bar(stage), phase ^ 1u);
+            mbar_wait(empty_bar(stage), phase ^ 1u, p.wait_limit);
             if constexpr (CG == 1) {
               mbar_arrive_expect_tx(full_bar(stage), stage_tx);
               tma_load_2d(smem_a(stage), &tmap_h, full_bar(stage), kb * BK, row0);
@@ -368,18 +369,17 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
       constexpr uint32_t idesc = F8 ? make_idesc_e4m3(Cfg::UMMA_M, BLOCK_N) : make_idesc_bf16(Cfg::UMMA_M, BLOCK_N);
       int stage = 0; uint32_t phase = 0;
       uint32_t tile = 0;
-      for (int gu = gc.gu0; gu < gc.gu_end; gu += gc.gu_step) {
+      for (int gu = 0; gu < gc.num_iters; ++gu) {
         Unit un;
         if (!decode_gang_unit(p, gc, gu, un)) continue;
-        const int vt0 = un.chunk * p.tiles_per_chunk;
-        const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
+        const int vt0 = p.chunk_vt[un.chunk], vt1 = p.chunk_vt[un.chunk + 1];
         for (int vt = vt0; vt < vt1; ++vt, ++tile) {
           const uint32_t acc = tile & 1u;
-          mbar_wait(tempty_bar(acc), ((tile >> 1) & 1u) ^ 1u);   // epilogue drained this accumulator
+          mbar_wait(tempty_bar(acc), ((tile >> 1) & 1u) ^ 1u, p.wait_limit);   // epilogue drained this accumulator
           tc_fence_after();
           const uint32_t d_tmem = tmem_base + acc * BLOCK_N;
           for (int kb = 0; kb < p.num_k_blocks; ++kb) {
-            mbar_wait(full_bar(stage), phase);
+            mbar_wait(full_bar(stage), phase, p.wait_limit);
             tc_fence_after();
             const uint64_t adesc = make_smem_desc_sw128(smem_a(stage));
             const uint64_t bdesc = make_smem_desc_sw128(smem_b(stage));
@@ -404,12 +404,11 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
     const uint32_t tempty_remote = (CG == 2) ? mapa(tempty_bar(0), 0) : tempty_bar(0);
     RowState<CAP> st;
     uint32_t tile = 0;
-    for (int gu = gc.gu0; gu < gc.gu_end; gu += gc.gu_step) {
+    for (int gu = 0; gu < gc.num_iters; ++gu) {
       Unit un;
       if (!decode_gang_unit(p, gc, gu, un)) continue;
       const int row = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M + row_in_tile;
-      const int vt0 = un.chunk * p.tiles_per_chunk;
-      const int vt1 = min(vt0 + p.tiles_per_chunk, p.num_vtiles);
+      const int vt0 = p.chunk_vt[un.chunk], vt1 = p.chunk_vt[un.chunk + 1];
       int tgt = (row < p.T) ? __ldg(p.targets + row) : -1;
       tgt = (tgt >= p.vocab_offset) ? tgt - p.vocab_offset : -1;   // local column, or out of range
       st.reset();
@@ -418,11 +417,14 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
       const float l2e = F8 ? LOG2E_F * deq : LOG2E_F;
       for (int vt = vt0; vt < vt1; ++vt, ++tile) {
         const uint32_t acc = tile & 1u;
-        mbar_wait(tfull_bar(acc), (tile >> 1) & 1u);
+        mbar_wait(tfull_bar(acc), (tile >> 1) & 1u, p.wait_limit);
         tc_fence_after();
         const int colbase = vt * BLOCK_N;
-        const int ngroups = min(BLOCK_N, p.V - colbase + 31) >> 5;   // 32-column groups with a valid column
-        for (int g = 0; g < ngroups && !(p.debug_flags & 1); ++g) {
+        int ngroups = min(BLOCK_N, p.V - colbase + 31) >> 5;   // 32-column groups with a valid column
+#ifdef SQ_PROBES
+        if (p.probe_flags & 1) ngroups = 0;        // probe: the epilogue skips the statistics
+#endif
+        for (int g = 0; g < ngroups; ++g) {
           float r[32];
           tmem_ld_32x32(lane_addr + acc * BLOCK_N + g * 32, r);
           tmem_ld_wait();

@@ -69,13 +69,15 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
-// Bounded wait: a protocol bug traps (CUDA error on the host) instead of hanging the GPU.
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+// Bounded wait: after `limit` clock cycles (0 = no limit) a protocol bug traps (a CUDA error on the host) instead of
+// hanging the GPU.  The limit is the caller's (sq_score_config / SQ_SCORE_WAIT_SECONDS): generous by default, because a
+// time-sliced, debugged or sanitised process can legitimately wait for a long time.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, long long limit) {
   if (mbar_try_wait(bar, parity)) return;
   const long long t0 = clock64();
   uint32_t spins = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if (((++spins) & 0x3FFu) == 0 && (clock64() - t0) > 4000000000LL) __trap();
+    if (((++spins) & 0x3FFu) == 0 && limit > 0 && (clock64() - t0) > limit) __trap();
   }
 }
 

@@ -7,9 +7,11 @@
 //   mu(g,q) = Model 1 if GC(g) > theta_q ("easy", strict) else Model 2      Eq. 7
 //   select  : P(i) = exp(f_i / zeta) / sum_j exp(f_j / zeta) per problem
 //
-// One CTA per problem.  The comparison GC > theta decides an integer, so the fp32 operation order
-// is pinned with _rn intrinsics (no FMA contraction) and mirrored by the oracle's fp32 decision
-// function.  Codes: 0 = B_lite (caller-supplied mask), 1 = Model 1, 2 = Model 2.
+// One CTA per problem.  The comparison GC > theta decides an integer; it is taken in fp32 on the GC and theta this
+// kernel REPORTS (_rn intrinsics: no FMA contraction, so the reported values are the compared ones), and the parity
+// test judges it against the fp64 definition with a derived fp32 margin.  Codes: 0 = B_lite (caller-supplied mask),
+// 1 = Model 1, 2 = Model 2, 3 = GC not finite (the group holds an empty trajectory, C(tau) = NaN: it takes no part in
+// the percentile, reading #24), -1 = the problem has more groups than the sort holds (theta = NaN).
 #pragma once
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -39,6 +41,11 @@ __global__ void __launch_bounds__(ROUTE_THREADS) sq_route_kernel(const RoutePara
   const int q = blockIdx.x;
   const int g0 = p.group_offsets[q], g1 = p.group_offsets[q + 1];
   const int ng = g1 - g0;
+  if (ng > ROUTE_MAX_GROUPS) {   // the host-side bound was wrong: flag the problem instead of routing on a partial sort
+    for (int i = threadIdx.x; i < ng; i += ROUTE_THREADS) p.route[g0 + i] = -1;
+    if (threadIdx.x == 0) p.theta[q] = CUDART_NAN_F;
+    return;
+  }
   if (threadIdx.x == 0) s_n = 0;
   __syncthreads();
   int live = 0;
@@ -51,7 +58,7 @@ __global__ void __launch_bounds__(ROUTE_THREADS) sq_route_kernel(const RoutePara
       const float gc = __fdiv_rn(acc, (float)p.K);
       p.group_fitness[g] = gc;
       const bool lite = p.lite_mask && p.lite_mask[g];
-      if (!lite) { key = gc; ++live; }
+      if (!lite && isfinite(gc)) { key = gc; ++live; }   // a NaN would break the sort's order
     }
     sv[i] = key;
   }
@@ -89,7 +96,8 @@ __global__ void __launch_bounds__(ROUTE_THREADS) sq_route_kernel(const RoutePara
   for (int i = threadIdx.x; i < ng; i += ROUTE_THREADS) {
     const int g = g0 + i;
     const bool lite = p.lite_mask && p.lite_mask[g];
-    p.route[g] = lite ? 0 : (p.group_fitness[g] > th ? 1 : 2);
+    const float gc = p.group_fitness[g];
+    p.route[g] = lite ? 0 : (!isfinite(gc) ? 3 : (gc > th ? 1 : 2));
   }
 }
 

@@ -15,12 +15,13 @@
 
 #include "sq_finalize_kernel.cuh"
 #include "sq_fused_kernel.cuh"
+#include "sq_positions_kernel.cuh"
 #include "sq_prepare_kernel.cuh"
 #include "sq_quant_kernel.cuh"
 #include "sq_reduce_kernel.cuh"
 #include "sq_route_kernel.cuh"
 
-#define SQ_VERSION 100
+#define SQ_VERSION 200
 
 struct sq_score_ctx {
   sq_score_config cfg;
@@ -41,16 +42,24 @@ struct sq_score_ctx {
   unsigned int* amax_bits = nullptr;   // per-tensor amax of sq_score_quantize_fp8
   int* seq_done = nullptr;   // [max_seqs] per-sequence tile counters of the single-launch reduction (zero between runs)
   int* tile_base = nullptr; int* tile_seq = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
-  // staging for sq_score_run_host
+  int max_clusters[3] = {0, 0, 0};   // [cg]: clusters of kernel 1 the device holds at once (occupancy query at create)
+  long long wait_limit = 0;          // cycles a device-side wait may last before kernel 1 traps (0 = for ever)
+  int* pos_base = nullptr;           // [max_seqs + 1] packed start of every candidate (sq_score_positions)
+  // staging for sq_score_run_host / sq_score_run_x (SQ_FLAG_STAGING)
   void* h_stage = nullptr; int32_t* tgt_stage = nullptr; int32_t* cu_stage = nullptr; float* seq_stage = nullptr;
   // sq_score_run_host streams H in on its own copy stream while kernel 1 runs: one flag per block of rows
   cudaStream_t copy_stream = nullptr; cudaEvent_t ev_fork = nullptr, ev_small = nullptr, ev_join = nullptr;
   unsigned int* h_flags = nullptr; unsigned int* one_host = nullptr;
   // driver entry point for tensor-map encoding
   void* encode_fn = nullptr;
-  // optional per-kernel timing (sq_score_set_profiling): events around kernel 1, finalize, kernel 2
-  int profiling = 0; int ev_valid = 0; int debug_flags = 0;
-  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  // optional per-kernel timing (sq_score_set_profiling): events around kernel 1, finalize
+  // and kernel 2 of the last SQ_PROFILE_RING profiled runs
+  int profiling = 0; int debug_flags = 0;
+  int64_t ev_count = 0, ev_read = 0;   // runs recorded / runs already handed out by sq_score_profile_read
+  cudaEvent_t (*ev)[4] = nullptr;      // [SQ_PROFILE_RING][4]
+#ifdef SQ_PROBES
+  int probe_flags = 0;                 // env SQ_SCORE_PROBE: wrong-results A/B probes, builder's builds only
+#endif
 };
 
 static thread_local char g_create_err[512] = {0};
@@ -73,17 +82,45 @@ static int set_err(sq_score_ctx* ctx, int code, const char* fmt, ...) {
   } while (0)
 
 constexpr int THR_MAX_CHUNKS = 16;   // the shared top-k bound is used for 2..16 vocab chunks per row
+constexpr int HOST_FLAG_ROWS_MIN = 2048;   // sq_score_run_host: rows of H per arrival flag (doubled until a run needs at most ...
+constexpr int HOST_FLAGS_PER_RUN = 256;    // ... this many flags)
 
 static int topk_cap_for(int k) { return k <= 8 ? 8 : (k <= 20 ? 20 : 32); }
 static inline int64_t cdiv64(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 // ------------------------------------------------------------------------------------------ plan
-// Work decomposition.  A unit sweeps `tiles_per_chunk` vocab tiles for one
-// token tile; units are ordered [group of group_m token tiles][chunk][tile in group] and handed to
-// the persistent clusters round-robin, so ~num_clusters consecutive units are in flight: group_m
-// token strips (H stays in L2) x ~num_clusters/group_m chunks (each W tile is read from HBM once
-// per group and shared through L2 by the group_m units that sweep it in lockstep).
-static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, sq_score_plan_t* pl) {
+// Work decomposition.  The persistent clusters are split into gangs; gang i has s_i members
+// (sizes differ by at most one, so that EVERY cluster the device holds is used: 74 = 2 x 13 + 4 x 12) and owns a
+// stripe of the vocabulary, cut into `chunks_per_gang` chunks.  A gang walks the token tiles in batches of s_i
+// (member j takes tile b * s_i + j) and sweeps its chunks for each batch, all members on the same W tile at the same
+// time: a W tile is fetched from HBM once per batch and served to the other members from L2, and all gangs are on
+// about the same token tiles at the same time, so the H strips in flight are ~max s_i.  Stripe widths are chosen so
+// that every gang finishes together: a gang with more members needs fewer batches and gets a wider stripe.
+static void split_stripes(int nv, int ng, const int* batches, int* width, int minw) {
+  // minimise max_i batches[i] * width[i] subject to sum width = nv, width >= minw: proportional to 1 / batches, then the
+  // left-over tiles one at a time to the gang whose finishing time grows least
+  double inv = 0.0;
+  for (int i = 0; i < ng; ++i) inv += 1.0 / batches[i];
+  int used = 0;
+  for (int i = 0; i < ng; ++i) {
+    width[i] = std::max(minw, (int)std::floor(nv * (1.0 / batches[i]) / inv));
+    used += width[i];
+  }
+  while (used > nv) {   // the floor of minw tiles per gang overshot: take from the gang that finishes last
+    int w = -1;
+    for (int i = 0; i < ng; ++i)
+      if (width[i] > minw && (w < 0 || (int64_t)batches[i] * width[i] > (int64_t)batches[w] * width[w])) w = i;
+    --width[w]; --used;
+  }
+  while (used < nv) {
+    int w = 0;
+    for (int i = 1; i < ng; ++i)
+      if ((int64_t)batches[i] * (width[i] + 1) < (int64_t)batches[w] * (width[w] + 1)) w = i;
+    ++width[w]; ++used;
+  }
+}
+
+static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, sq_score_plan_t* pl, int max_clusters = 0) {
   if (!cfg || !pl || T < 0 || cfg->d <= 0 || cfg->vocab <= 0 || k < 1 || k > SQ_MAX_K) return SQ_ERR_INVALID_ARG;
   if (num_sms <= 0) num_sms = 148;
   // default: CTA pairs (UMMA M = 256); a decode-shaped run of at most 128 rows fits one CTA's 128 TMEM
@@ -96,62 +133,73 @@ static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, 
   pl->num_vtiles = (int)cdiv64(cfg->vocab, 256);
   pl->num_k_blocks = (int)cdiv64(cfg->d, 64);
   pl->num_clusters = std::max(1, num_sms / cg);
+  if (max_clusters > 0) pl->num_clusters = std::min(pl->num_clusters, max_clusters);   // what can be co-resident (create)
   pl->topk_cap = topk_cap_for(k);
-  // gang size: group_m clusters sweep one W chunk together, never more than there are token tiles or
-  // clusters.  Default 12 (measured on B200 against 8 / 10 / 14 / 16 / 24: +1.5 % at qwen3_8b, +2.7 % at
-  // gpt_oss, neutral at qwen3_4b -- W is read from HBM once per 12 token tiles instead of 8 and the
-  // planner then needs fewer, longer vocab chunks)
-  int G = cfg->group_m > 0 ? cfg->group_m : 12;
-  G = std::max(1, std::min(G, std::min(std::max(1, pl->m_tiles), pl->num_clusters)));
-  pl->group_m = G;
-  pl->num_gangs = pl->num_clusters / G;
-  const int GB = pl->num_clusters - pl->num_gangs * G;   // clusters left over: one smaller gang B
-  pl->gang_b_size = GB;
-  const int M = pl->m_tiles;
-  const int max_chunks = std::min((int)sq::FIN_MAX_CHUNKS, pl->num_vtiles);
-  // cost of a plan = the slower gang class, in tile-times: rounds x (unit length + fill/drain)
-  auto eval = [&](int c, int m_b, double* cost_out) {
-    const int tpc = (int)cdiv64(pl->num_vtiles, c);
-    const int ce = (int)cdiv64(pl->num_vtiles, tpc);
-    const int64_t rounds_a = cdiv64(cdiv64(M - m_b, G) * ce, pl->num_gangs);
-    const int64_t rounds_b = m_b > 0 ? cdiv64(m_b, GB) * ce : 0;
-    *cost_out = (double)std::max(rounds_a, rounds_b) * (tpc + 0.75);   // 0.75 tile-times of fill/drain per unit
-    return ce;
+  const int M = std::max(1, pl->m_tiles), NV = pl->num_vtiles, NC = pl->num_clusters;
+  const int gangs_max = std::min(NV, (int)sq::FIN_MAX_CHUNKS);   // every gang owns at least one vocab tile and one chunk
+
+  // one candidate: `ng` gangs over min(NC, ng * M) clusters; cost in tile-times = the gang that finishes last
+  struct Cand { int ng, base, big, r; double cost; };
+  int batches[sq::FIN_MAX_CHUNKS], width[sq::FIN_MAX_CHUNKS];
+  auto eval = [&](int ng, int r) {
+    Cand c; c.ng = ng; c.r = r;
+    c.base = std::min(NC / ng, M);                       // a member beyond the M-th would never get a token tile
+    c.big = (c.base < M) ? std::min(NC - ng * c.base, ng) : 0;
+    if (c.base + 1 > M) c.big = 0;
+    for (int i = 0; i < ng; ++i) batches[i] = (int)cdiv64(M, c.base + (i < c.big ? 1 : 0));
+    split_stripes(NV, ng, batches, width, r);
+    double cost = 0.0;
+    for (int i = 0; i < ng; ++i) cost = std::max(cost, batches[i] * (width[i] + 0.75 * std::min(r, width[i])));   // 0.75 tile of fill/drain per unit
+    c.cost = cost;
+    return c;
   };
-  int best_c = 1, best_mb = 0;
-  if (M > 0) {
-    // The gangs in flight work on ceil(num_gangs / C) different token groups, i.e. about
-    // num_clusters / C token strips of rows_per_tile x d bf16 are re-read from L2 for every vocab
-    // tile.  Keep that hot set under ~40 MB of the 126 MB L2 (measured: beyond ~50 MB the strips
-    // start to miss and HBM traffic and power go up), then minimise the cost above over the number
-    // of chunks and the number of token tiles handed to gang B; ties -> fewer chunks, smaller B.
-    const double strip_mb = (double)pl->rows_per_tile * cfg->d * 2.0 / 1e6;
-    const int c_l2 = (int)std::ceil(pl->num_gangs * G * strip_mb / 40.0);
-    // decode-shaped runs (fewer token groups than gangs) split the vocabulary further so that every
-    // cluster streams its own slice of W: up to one chunk per gang
-    const int64_t groups = cdiv64(M, G);
-    int c_hi = std::min(max_chunks, groups * 16 < pl->num_gangs ? (int)cdiv64(pl->num_gangs, groups) : 16);
-    int c_lo = std::max(1, std::min(c_hi, c_l2));
-    if (cfg->num_chunks > 0) c_lo = c_hi = std::min(cfg->num_chunks, max_chunks);
-    const int mb_hi = GB > 0 ? std::min(M - 1, (int)(3.0 * M * GB / pl->num_clusters) + GB) : 0;
-    double best_cost = 1e300;
-    for (int c = c_lo; c <= c_hi; ++c) {
-      for (int m_b = 0; m_b <= mb_hi; ++m_b) {
-        double cost;
-        const int ce = eval(c, m_b, &cost);
-        if (ce < c_lo && c < c_hi) break;   // rounding merged chunks below the L2 bound
-        if (cost < best_cost - 1e-9) { best_cost = cost; best_c = c; best_mb = m_b; }
+  Cand best = {0, 0, 0, 1, 1e300};
+  if (cfg->num_chunks > 0) {
+    // forced number of chunks (tests, experiments): the largest gang count that divides it
+    const int C = std::min(cfg->num_chunks, gangs_max);
+    const int g_want = cfg->group_m > 0 ? cfg->group_m : 12;
+    const int ng_hi = std::max(1, std::min(NC / std::max(1, std::min(g_want, std::min(M, NC))), C));
+    int ng = 1;
+    for (int n = 1; n <= ng_hi; ++n) if (C % n == 0) ng = n;
+    best = eval(ng, C / ng);
+  } else {
+    // Gang size: 12 measured best on B200 at qwen3_8b / gpt_oss (swept 8 .. 36); sizes 10 .. 14 are within
+    // noise of one another, so the planner takes the one whose batches and stripes quantise best for this T.
+    const int g_lo = cfg->group_m > 0 ? cfg->group_m : 10, g_hi = cfg->group_m > 0 ? cfg->group_m : 14;
+    int last_ng = -1;
+    for (int pass = 0; pass < 2; ++pass)                 // pass 0: the preferred size first, so that ties keep it
+      for (int g = (pass == 0 ? (cfg->group_m > 0 ? g_lo : 12) : g_lo); g <= (pass == 0 ? (cfg->group_m > 0 ? g_hi : 12) : g_hi); ++g) {
+        const int G = std::max(1, std::min(g, std::min(M, NC)));
+        const int ng = std::max(1, std::min(NC / G, gangs_max));
+        if (ng == last_ng) continue;
+        last_ng = ng;
+        const Cand c = eval(ng, 1);
+        if (c.cost < best.cost * (1.0 - 1e-3)) best = c;   // a different size must win by more than noise
       }
-    }
-  } else if (cfg->num_chunks > 0) {
-    best_c = std::min(cfg->num_chunks, max_chunks);
   }
-  pl->tiles_per_chunk = (int)cdiv64(pl->num_vtiles, best_c);
-  pl->num_chunks = (int)cdiv64(pl->num_vtiles, pl->tiles_per_chunk);
+  pl->num_gangs = best.ng;
+  pl->gang_size = best.base;
+  pl->gangs_big = best.big;
+  pl->chunks_per_gang = best.r;
+  pl->num_chunks = best.ng * best.r;
+  pl->clusters_used = best.ng * best.base + best.big;
   pl->num_units = pl->m_tiles * pl->num_chunks;
-  pl->m_split = M - best_mb;
-  pl->num_gang_units = (int)cdiv64(pl->m_split, G) * pl->num_chunks;
-  pl->num_gang_units_b = best_mb > 0 ? (int)cdiv64(best_mb, GB) * pl->num_chunks : 0;
+  for (int i = 0; i < best.ng; ++i) batches[i] = (int)cdiv64(M, best.base + (i < best.big ? 1 : 0));
+  split_stripes(NV, best.ng, batches, width, best.r);
+  // a gang's stripe is cut into r chunks of near-equal width (every stripe is at least r tiles wide: no empty chunk)
+  int vt = 0, c = 0, widest = 0;
+  pl->chunk_vtile[0] = 0;
+  for (int i = 0; i < best.ng; ++i) {
+    for (int q = 0; q < best.r; ++q) {
+      const int w = width[i] / best.r + (q < width[i] % best.r ? 1 : 0);
+      vt += w;
+      widest = std::max(widest, w);
+      pl->chunk_vtile[++c] = vt;
+    }
+    pl->max_batches = std::max(pl->max_batches, batches[i]);
+  }
+  pl->tiles_per_chunk = widest;
+  if (pl->m_tiles == 0) pl->max_batches = 0;
   return SQ_OK;
 }
 
@@ -190,12 +238,16 @@ extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
   cudaSetDevice(ctx->cfg.device);
   void* bufs[] = {ctx->amax_bits, ctx->seq_done, ctx->thr_pub, ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
                   ctx->tok_lse, ctx->tok_lp, ctx->tok_ent, ctx->tok_conf, ctx->tile_base, ctx->tile_seq, ctx->red_sum,
-                  ctx->red_min, ctx->h_stage, ctx->tgt_stage, ctx->cu_stage, ctx->seq_stage};
+                  ctx->red_min, ctx->h_stage, ctx->tgt_stage, ctx->cu_stage, ctx->seq_stage, ctx->pos_base};
   int rc = SQ_OK;
   for (void* b : bufs)
     if (b && cudaFree(b) != cudaSuccess) rc = SQ_ERR_CUDA;
-  for (cudaEvent_t e : ctx->ev)
-    if (e) cudaEventDestroy(e);
+  if (ctx->ev) {
+    for (int i = 0; i < SQ_PROFILE_RING; ++i)
+      for (cudaEvent_t e : ctx->ev[i])
+        if (e) cudaEventDestroy(e);
+    delete[] ctx->ev;
+  }
   for (cudaEvent_t e : {ctx->ev_fork, ctx->ev_small, ctx->ev_join})
     if (e) cudaEventDestroy(e);
   if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
@@ -226,8 +278,11 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
     return set_err(nullptr, SQ_ERR_INVALID_ARG, "d, vocab, max_tokens and max_seqs must be positive");
   if (cfg->max_k < 1 || cfg->max_k > SQ_MAX_K)
     return set_err(nullptr, SQ_ERR_INVALID_ARG, "max_k must be in 1..%d", SQ_MAX_K);
-  if (cfg->cta_group < 0 || cfg->cta_group > 2 || cfg->num_chunks < 0 || cfg->group_m < 0 || (cfg->flags & ~SQ_FLAG_REDUCE_ONLY))
-    return set_err(nullptr, SQ_ERR_INVALID_ARG, "cta_group must be 0, 1 or 2; num_chunks, group_m >= 0");
+  if (cfg->cta_group < 0 || cfg->cta_group > 2 || cfg->num_chunks < 0 || cfg->group_m < 0 ||
+      (cfg->flags & ~(SQ_FLAG_REDUCE_ONLY | SQ_FLAG_STAGING)))
+    return set_err(nullptr, SQ_ERR_INVALID_ARG, "cta_group must be 0, 1 or 2; num_chunks, group_m >= 0; unknown flag");
+  if (cfg->vocab > (1 << 24))
+    return set_err(nullptr, SQ_ERR_UNSUPPORTED, "vocab = %d exceeds 2^24 (vocab-tile indices are 16-bit)", cfg->vocab);
   if (cfg->d % 8 != 0)
     return set_err(nullptr, SQ_ERR_UNSUPPORTED, "d = %d is not a multiple of 8 (TMA needs 16-byte row strides)", cfg->d);
   if (cfg->max_tokens >= (1LL << 31) - 16384)
@@ -251,10 +306,23 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   if (!ctx) return set_err(nullptr, SQ_ERR_NOMEM, "host allocation failed");
   ctx->cfg = *cfg;
   ctx->num_sms = prop.multiProcessorCount;
-  if (const char* lim = getenv("SQ_SCORE_MAX_SMS"))   // experiments only: plan for fewer SMs
-    if (atoi(lim) >= 2 && atoi(lim) < ctx->num_sms) ctx->num_sms = atoi(lim);
   ctx->cap_max = topk_cap_for(cfg->max_k);
-  if (const char* dbg = getenv("SQ_SCORE_DEBUG")) ctx->debug_flags = atoi(dbg);
+  // SQ_SCORE_DEBUG selects between code paths that give the SAME results (tests force each of them): bit 3 = two-pass
+  // prepare kernel, bit 4 = no shared top-k bound, bit 5 / 6 = three-launch / single-launch kernel 2, bit 7 = one warp
+  // per row in the finalize kernel
+  if (const char* dbg = getenv("SQ_SCORE_DEBUG")) ctx->debug_flags = atoi(dbg) & (8 | 16 | 32 | 64 | 128);
+#ifdef SQ_PROBES
+  if (const char* lim = getenv("SQ_SCORE_MAX_SMS"))   // probe: plan for fewer SMs
+    if (atoi(lim) >= 2 && atoi(lim) < ctx->num_sms) ctx->num_sms = atoi(lim);
+  if (const char* pr = getenv("SQ_SCORE_PROBE")) ctx->probe_flags = atoi(pr);
+#endif
+  {   // device-side waits trap after cfg.wait_seconds (default 60 s; SQ_SCORE_WAIT_SECONDS overrides, e.g. under a sanitizer)
+    int khz = 0;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, cfg->device);
+    long long sec = cfg->wait_seconds == 0 ? 60 : cfg->wait_seconds;
+    if (const char* w = getenv("SQ_SCORE_WAIT_SECONDS")) sec = atoll(w) == 0 ? -1 : atoll(w);
+    ctx->wait_limit = sec < 0 ? 0 : sec * (long long)std::max(khz, 1000000) * 1000LL;
+  }
 
   cudaDriverEntryPointQueryResult qres;
   e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ctx->encode_fn, cudaEnableDefault, &qres);
@@ -292,6 +360,22 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   A(ws_alloc(ctx, &ctx->tile_seq, ctx->red_tiles_max));
   A(ws_alloc(ctx, &ctx->red_min, ctx->red_tiles_max));
   A(ws_alloc(ctx, &ctx->seq_stage, 4 * (int64_t)cfg->max_seqs));
+  A(ws_alloc(ctx, &ctx->pos_base, (int64_t)cfg->max_seqs + 1));
+  if ((cfg->flags & SQ_FLAG_STAGING) && !reduce_only) {   // everything sq_score_run_host / sq_score_run_x need: no run allocates
+    A(ws_alloc(ctx, reinterpret_cast<uint8_t**>(&ctx->h_stage), T * (int64_t)cfg->d * 2));
+    A(ws_alloc(ctx, &ctx->tgt_stage, T));
+    A(ws_alloc(ctx, &ctx->cu_stage, (int64_t)cfg->max_seqs + 1));
+    A(ws_alloc(ctx, &ctx->h_flags, HOST_FLAGS_PER_RUN));
+    if (rc == SQ_OK) {
+      bool ok = cudaHostAlloc(reinterpret_cast<void**>(&ctx->one_host), sizeof(unsigned int), cudaHostAllocDefault) == cudaSuccess;
+      if (ok) *ctx->one_host = 1u;
+      ok = ok && cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) == cudaSuccess;
+      ok = ok && cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) == cudaSuccess;
+      ok = ok && cudaEventCreateWithFlags(&ctx->ev_small, cudaEventDisableTiming) == cudaSuccess;
+      ok = ok && cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) == cudaSuccess;
+      if (!ok) { rc = SQ_ERR_CUDA; set_err(ctx, rc, "creating the copy stream / events failed: %s", cudaGetErrorString(cudaGetLastError())); }
+    }
+  }
   if (rc != SQ_OK) {
     memcpy(g_create_err, ctx->err, sizeof(g_create_err));
     sq_score_destroy(ctx);
@@ -315,6 +399,32 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
     set_err(nullptr, rc, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize) failed: %s", cudaGetErrorString(cudaGetLastError()));
     sq_score_destroy(ctx);
     return rc;
+  }
+  // Kernel 1's clusters wait for one another (gang barriers), so all of them must be resident at once: ask the
+  // occupancy calculator how many the device holds (it knows the shared-memory footprint, the cluster shape and any
+  // SM partitioning of this context) and plan for at most that many.
+  if (!reduce_only) {
+    for (int cg = 1; cg <= 2; ++cg) {
+      cudaLaunchConfig_t lc = {};
+      lc.gridDim = dim3((unsigned)(ctx->num_sms / cg * cg));
+      lc.blockDim = dim3(sq::NUM_THREADS);
+      lc.dynamicSmemBytes = cg == 1 ? sq::FusedCfg<1>::SMEM_BYTES : sq::FusedCfg<2>::SMEM_BYTES;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = cg; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      lc.attrs = at; lc.numAttrs = 1;
+      int n = 0;
+      const cudaError_t oe = cg == 1 ? cudaOccupancyMaxActiveClusters(&n, sq::sq_fused_score_kernel<1, 32>, &lc)
+                                     : cudaOccupancyMaxActiveClusters(&n, sq::sq_fused_score_kernel<2, 32>, &lc);
+      if (oe != cudaSuccess || n < 1) {
+        set_err(nullptr, SQ_ERR_UNSUPPORTED, "the device cannot hold a cluster of %d CTA(s) of the fused kernel (%s)", cg,
+                oe == cudaSuccess ? "occupancy 0" : cudaGetErrorString(oe));
+        cudaGetLastError();
+        sq_score_destroy(ctx);
+        return SQ_ERR_UNSUPPORTED;
+      }
+      ctx->max_clusters[cg] = n;
+    }
   }
   *out = ctx;
   return SQ_OK;
@@ -344,8 +454,7 @@ static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int6
 template <int CG, int CAP, bool F8 = false>
 static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CUtensorMap& th, const CUtensorMap& tw,
                                 const sq::FusedParams& fp, cudaStream_t st) {
-  // every launched cluster belongs to a gang; gang B is launched only if it was given token tiles
-  const int clusters = pl.num_gangs * pl.group_m + (pl.num_gang_units_b > 0 ? pl.gang_b_size : 0);
+  const int clusters = pl.clusters_used;   // every launched cluster belongs to a gang
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3((unsigned)(clusters * CG));
   lc.blockDim = dim3(sq::NUM_THREADS);
@@ -463,15 +572,17 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
                     const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k, int window,
                     const sq_score_outputs* o, void* stream, const unsigned int* h_ready, int flag_rows,
                     int vocab_offset = 0, float* shard_state = nullptr, const float* h_scale = nullptr,
-                    const float* w_scale = nullptr) {
+                    const float* w_scale = nullptr, int shard_rows = 0) {
   if (!ctx) return SQ_ERR_INVALID_ARG;
   if (!o && !shard_state) return set_err(ctx, SQ_ERR_INVALID_ARG, "outputs is null");
   static const sq_score_outputs no_outputs = {};
   if (!o) o = &no_outputs;
   if (ctx->cfg.flags & SQ_FLAG_REDUCE_ONLY) return set_err(ctx, SQ_ERR_INVALID_ARG, "ctx was created with SQ_FLAG_REDUCE_ONLY");
-  const int T = num_tokens, V = ctx->cfg.vocab, d = ctx->cfg.d;
+  const int T = num_tokens, d = ctx->cfg.d;
+  const int V = shard_state ? shard_rows : ctx->cfg.vocab;   // a vocab-parallel shard may hold fewer rows than the ctx was sized for
   int B = num_seqs;
   if (T < 0 || B < 0) return set_err(ctx, SQ_ERR_INVALID_ARG, "negative T or B");
+  if (V < 1 || V > ctx->cfg.vocab) return set_err(ctx, SQ_ERR_INVALID_ARG, "shard_rows = %d outside 1..cfg.vocab = %d", V, ctx->cfg.vocab);
   if (T > ctx->cfg.max_tokens || B > ctx->cfg.max_seqs)
     return set_err(ctx, SQ_ERR_INVALID_ARG, "T = %d / B = %d exceed max_tokens / max_seqs of this ctx", T, B);
   if (k < 1 || k > ctx->cfg.max_k || k > V) return set_err(ctx, SQ_ERR_INVALID_ARG, "k = %d outside 1..min(max_k, V)", k);
@@ -493,35 +604,46 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     const bool f8 = h_scale != nullptr;
     sq_score_plan_t pl;
     sq_score_config pc = ctx->cfg;
+    pc.vocab = V;
     if (f8) pc.d = (d + 1) / 2;   // an e4m3 k-block is 128 elements: the plan sees half as many k-blocks
-    make_plan(&pc, T, k, ctx->num_sms, &pl);
+    const int cg_sel = (pc.cta_group == 1) ? 1 : (pc.cta_group == 2 ? 2 : (T <= 128 ? 1 : 2));
+    make_plan(&pc, T, k, ctx->num_sms, &pl, ctx->max_clusters[cg_sel]);
     const int64_t rows = ws_rows_for(ctx->cfg);
-    if ((int64_t)pl.num_chunks * T > rows) {   // workspace bound: fewer, longer chunks
+    if ((int64_t)pl.num_chunks * T > rows) {   // workspace bound: fewer gangs, wider stripes
       pc.num_chunks = (int)std::max<int64_t>(1, rows / T);
-      make_plan(&pc, T, k, ctx->num_sms, &pl);
+      make_plan(&pc, T, k, ctx->num_sms, &pl, ctx->max_clusters[cg_sel]);
     }
     if (pl.topk_cap > ctx->cap_max) return set_err(ctx, SQ_ERR_INVALID_ARG, "k exceeds the ctx's max_k capacity");
     CUtensorMap th, tw;
     if (f8 && d % 16 != 0) return set_err(ctx, SQ_ERR_UNSUPPORTED, "the FP8 variant needs d %% 16 == 0 (TMA 16-byte row strides)");
-    int rc = make_tmap(ctx, &th, H, T, d, (ctx->debug_flags & 4) ? sq::BLOCK_M / 2 : sq::BLOCK_M, f8);
+    int h_box = sq::BLOCK_M, w_box = sq::BLOCK_N / pl.cta_group;
+#ifdef SQ_PROBES
+    if (ctx->probe_flags & 4) h_box /= 2;
+    if (ctx->probe_flags & 2) w_box /= 2;
+#endif
+    int rc = make_tmap(ctx, &th, H, T, d, h_box, f8);
     if (rc != SQ_OK) return rc;
-    rc = make_tmap(ctx, &tw, W, V, d, (sq::BLOCK_N / pl.cta_group) / ((ctx->debug_flags & 2) ? 2 : 1), f8);
+    rc = make_tmap(ctx, &tw, W, V, d, w_box, f8);
     if (rc != SQ_OK) return rc;
 
     sq::FusedParams fp = {};
     fp.T = T; fp.V = V; fp.d = d;
-    fp.num_k_blocks = pl.num_k_blocks; fp.num_vtiles = pl.num_vtiles; fp.tiles_per_chunk = pl.tiles_per_chunk;
-    fp.num_chunks = pl.num_chunks; fp.m_tiles = pl.m_tiles; fp.group_m = pl.group_m;
-    fp.num_gangs = pl.num_gangs; fp.num_gang_units = pl.num_gang_units; fp.gang_ctr = ctx->gang_ctr;
-    fp.m_split = pl.m_split; fp.gang_b_size = pl.gang_b_size; fp.num_gang_units_b = pl.num_gang_units_b;
+    fp.num_k_blocks = pl.num_k_blocks; fp.num_vtiles = pl.num_vtiles;
+    fp.num_chunks = pl.num_chunks; fp.m_tiles = pl.m_tiles;
+    fp.num_gangs = pl.num_gangs; fp.gang_size = pl.gang_size; fp.gangs_big = pl.gangs_big;
+    fp.chunks_per_gang = pl.chunks_per_gang; fp.gang_ctr = ctx->gang_ctr;
+    fp.wait_limit = ctx->wait_limit;
+    for (int c = 0; c <= pl.num_chunks; ++c) fp.chunk_vt[c] = (uint16_t)pl.chunk_vtile[c];
     // the gang barrier counters only matter when some gang has more than one member (not in decode-shaped plans)
-    if (pl.group_m > 1 || (pl.num_gang_units_b > 0 && pl.gang_b_size > 1))
+    if (pl.gang_size + (pl.gangs_big > 0 ? 1 : 0) > 1)
       SQ_CUDA(ctx, cudaMemsetAsync(ctx->gang_ctr, 0, 256 * sizeof(unsigned int), st));
     fp.targets = targets;
     fp.part_m = ctx->part_m; fp.part_s = ctx->part_s; fp.part_u = ctx->part_u;
     fp.part_cs = ctx->part_cs; fp.part_cu = ctx->part_cu;
     fp.part_topv = ctx->part_topv; fp.part_topi = ctx->part_topi; fp.zt = ctx->zt;
-    fp.debug_flags = ctx->debug_flags;
+#ifdef SQ_PROBES
+    fp.probe_flags = ctx->probe_flags;
+#endif
     fp.vocab_offset = vocab_offset;
     fp.h_scale = h_scale; fp.w_scale = w_scale;
     fp.h_ready = h_ready; fp.flag_rows = flag_rows;
@@ -539,7 +661,8 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
       SQ_CUDA(ctx, cudaMemsetAsync(ctx->thr_pub, 0xFE, (size_t)C * T * sizeof(float), st));
     }
     cudaError_t e;
-    if (ctx->profiling) cudaEventRecord(ctx->ev[0], st);
+    cudaEvent_t* pev = ctx->profiling ? ctx->ev[ctx->ev_count % SQ_PROFILE_RING] : nullptr;
+    if (pev) cudaEventRecord(pev[0], st);
     const int sel = pl.cta_group * 100 + pl.topk_cap + (f8 ? 1000 : 0);
     switch (sel) {
       case 1108: e = launch_fused<1, 8, true>(pl, ctx->num_sms, th, tw, fp, st); break;
@@ -556,7 +679,7 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
       default: e = launch_fused<2, 32>(pl, ctx->num_sms, th, tw, fp, st); break;
     }
     if (e != cudaSuccess) return set_err(ctx, SQ_ERR_CUDA, "fused kernel launch failed: %s", cudaGetErrorString(e));
-    if (ctx->profiling) cudaEventRecord(ctx->ev[1], st);
+    if (pev) cudaEventRecord(pev[1], st);
 
     sq::FinalizeParams fin = {};
     fin.T = T; fin.V = V; fin.k = k; fin.cap = pl.topk_cap; fin.num_chunks = pl.num_chunks;
@@ -586,7 +709,8 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     }
     ctx->launches += 2;
     SQ_CUDA(ctx, cudaGetLastError());
-    if (ctx->profiling) cudaEventRecord(ctx->ev[2], st);
+    if (pev) cudaEventRecord(pev[2], st);
+    if (pev && B == 0) { cudaEventRecord(pev[3], st); ++ctx->ev_count; }   // no kernel 2 follows (shard runs, B = 0)
   }
   if (B > 0) {
     sq::ReduceParams rp = {};
@@ -597,7 +721,7 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     rp.out_min = o->seq_min_window_conf;
     const int rc = launch_reduce(ctx, rp, st);
     if (rc != SQ_OK) return rc;
-    if (ctx->profiling && T > 0) { cudaEventRecord(ctx->ev[3], st); ctx->ev_valid = 1; }
+    if (ctx->profiling && T > 0) { cudaEventRecord(ctx->ev[ctx->ev_count % SQ_PROFILE_RING][3], st); ++ctx->ev_count; }
   }
   return SQ_OK;
 }
@@ -656,14 +780,32 @@ extern "C" int64_t sq_score_shard_state_bytes(int64_t num_tokens, int k) {
   return shard_state_words(num_tokens, topk_cap_for(k)) * 4;
 }
 
-extern "C" int sq_score_run_shard(sq_score_ctx* ctx, const void* H, const void* W_shard, int vocab_offset,
+extern "C" int sq_score_run_shard(sq_score_ctx* ctx, const void* H, const void* W_shard, int shard_rows, int vocab_offset,
                                   const int32_t* targets, int num_tokens, int k, void* state_out, void* stream) {
   if (!ctx) return SQ_ERR_INVALID_ARG;
   if (vocab_offset < 0) return set_err(ctx, SQ_ERR_INVALID_ARG, "vocab_offset must be >= 0");
+  if (shard_rows < 1 || shard_rows > ctx->cfg.vocab)
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "shard_rows = %d outside 1..cfg.vocab = %d", shard_rows, ctx->cfg.vocab);
+  if (k > shard_rows) return set_err(ctx, SQ_ERR_INVALID_ARG, "k = %d exceeds the shard's %d rows", k, shard_rows);
   if (num_tokens > 0 && !state_out) return set_err(ctx, SQ_ERR_INVALID_ARG, "state_out is null");
   if (num_tokens == 0) return SQ_OK;
   return run_impl(ctx, H, W_shard, targets, nullptr, num_tokens, 0, k, 1, nullptr, stream, nullptr, 0, vocab_offset,
-                  static_cast<float*>(state_out));
+                  static_cast<float*>(state_out), nullptr, nullptr, shard_rows);
+}
+
+extern "C" int sq_score_neutral_shard_state(sq_score_ctx* ctx, int num_tokens, int k, void* state_out, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (num_tokens < 0 || k < 1 || k > SQ_MAX_K) return set_err(ctx, SQ_ERR_INVALID_ARG, "T >= 0 and 1 <= k <= %d required", SQ_MAX_K);
+  if (num_tokens == 0) return SQ_OK;
+  if (!state_out) return set_err(ctx, SQ_ERR_INVALID_ARG, "state_out is null");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  const int cap = topk_cap_for(k);
+  const int64_t words = shard_state_words(num_tokens, cap);
+  const unsigned grid = (unsigned)std::min<int64_t>(cdiv64(words, 256), (int64_t)ctx->num_sms * 8);
+  sq::sq_neutral_state_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(static_cast<float*>(state_out), num_tokens, cap);
+  ctx->launches += 1;
+  SQ_CUDA(ctx, cudaGetLastError());
+  return SQ_OK;
 }
 
 extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int num_shards, const int32_t* vocab_starts,
@@ -723,27 +865,89 @@ extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int 
 extern "C" int sq_score_set_profiling(sq_score_ctx* ctx, int enable) {
   if (!ctx) return SQ_ERR_INVALID_ARG;
   SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-  if (enable)
-    for (auto& e : ctx->ev)
-      if (!e) SQ_CUDA(ctx, cudaEventCreate(&e));
+  if (enable && !ctx->ev) {
+    ctx->ev = new (std::nothrow) cudaEvent_t[SQ_PROFILE_RING][4]();
+    if (!ctx->ev) return set_err(ctx, SQ_ERR_NOMEM, "host allocation failed");
+    for (int i = 0; i < SQ_PROFILE_RING; ++i)
+      for (auto& e : ctx->ev[i]) SQ_CUDA(ctx, cudaEventCreate(&e));
+  }
   ctx->profiling = enable ? 1 : 0;
-  ctx->ev_valid = 0;
+  ctx->ev_count = ctx->ev_read = 0;
+  return SQ_OK;
+}
+
+static int read_run_times(sq_score_ctx* ctx, int64_t run, float* ms3) {
+  cudaEvent_t* e = ctx->ev[run % SQ_PROFILE_RING];
+  SQ_CUDA(ctx, cudaEventSynchronize(e[3]));
+  for (int i = 0; i < 3; ++i) SQ_CUDA(ctx, cudaEventElapsedTime(&ms3[i], e[i], e[i + 1]));
   return SQ_OK;
 }
 
 extern "C" int sq_score_kernel_times(sq_score_ctx* ctx, float* ms3) {
   if (!ctx || !ms3) return SQ_ERR_INVALID_ARG;
-  if (!ctx->profiling || !ctx->ev_valid) return set_err(ctx, SQ_ERR_INVALID_ARG, "no profiled run recorded");
-  SQ_CUDA(ctx, cudaEventSynchronize(ctx->ev[3]));
-  for (int i = 0; i < 3; ++i) SQ_CUDA(ctx, cudaEventElapsedTime(&ms3[i], ctx->ev[i], ctx->ev[i + 1]));
+  if (!ctx->profiling || ctx->ev_count == 0) return set_err(ctx, SQ_ERR_INVALID_ARG, "no profiled run recorded");
+  return read_run_times(ctx, ctx->ev_count - 1, ms3);
+}
+
+extern "C" int sq_score_profile_read(sq_score_ctx* ctx, float* ms, int capacity, int* num_runs) {
+  if (!ctx || !ms || !num_runs || capacity < 0) return SQ_ERR_INVALID_ARG;
+  *num_runs = 0;
+  if (!ctx->profiling) return set_err(ctx, SQ_ERR_INVALID_ARG, "profiling is off");
+  int64_t first = std::max(ctx->ev_read, ctx->ev_count - SQ_PROFILE_RING);
+  first = std::max(first, ctx->ev_count - capacity);
+  for (int64_t r = first; r < ctx->ev_count; ++r) {
+    const int rc = read_run_times(ctx, r, ms + 3 * (r - first));
+    if (rc != SQ_OK) return rc;
+  }
+  *num_runs = (int)(ctx->ev_count - first);
+  ctx->ev_read = ctx->ev_count;
   return SQ_OK;
 }
 
-// H staging [max_tokens, d] bf16, allocated on first use: the landing buffer of sq_score_run_host and the output of the
-// prepare step inside sq_score_run_x
-static int ensure_h_stage(sq_score_ctx* ctx) {
-  if (ctx->h_stage) return SQ_OK;
-  return ws_alloc(ctx, reinterpret_cast<uint8_t**>(&ctx->h_stage), ctx->cfg.max_tokens * (int64_t)ctx->cfg.d * 2);
+static int need_staging(sq_score_ctx* ctx) {
+  if (ctx->h_stage && ctx->copy_stream) return SQ_OK;
+  return set_err(ctx, SQ_ERR_INVALID_ARG, "this call needs a ctx created with SQ_FLAG_STAGING (no run allocates)");
+}
+
+// ------------------------------------------------------------------------------------------ positions (8(f)-2)
+extern "C" int sq_score_positions_host(const int32_t* query_lens, const int32_t* traj_lens, int num_seqs, int32_t* pos_out,
+                                       int64_t pos_capacity, int32_t* cu_out, int64_t* num_tokens_out) {
+  if (num_seqs < 0 || pos_capacity < 0 || !cu_out || (num_seqs > 0 && (!query_lens || !traj_lens))) return SQ_ERR_INVALID_ARG;
+  int64_t t = 0, base = 0;
+  cu_out[0] = 0;
+  for (int b = 0; b < num_seqs; ++b) {
+    const int64_t q = query_lens[b], n = traj_lens[b];
+    if (q < 0 || n < 0 || (n > 0 && q < 1)) return SQ_ERR_INVALID_ARG;   // no state predicts the trajectory's first token
+    if (t + n > pos_capacity || base + q + n > INT32_MAX || (n > 0 && !pos_out)) return SQ_ERR_INVALID_ARG;
+    for (int64_t i = 0; i < n; ++i) pos_out[t + i] = (int32_t)(base + q - 1 + i);
+    t += n;
+    base += q + n;
+    cu_out[b + 1] = (int32_t)t;
+  }
+  if (num_tokens_out) *num_tokens_out = t;
+  return SQ_OK;
+}
+
+extern "C" int sq_score_positions(sq_score_ctx* ctx, const int32_t* query_lens, const int32_t* traj_lens, int num_seqs,
+                                  int num_tokens, int32_t* pos_out, int32_t* cu_out, int32_t* status_out, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (num_seqs < 0 || num_tokens < 0 || num_seqs > ctx->cfg.max_seqs || num_tokens > ctx->cfg.max_tokens)
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "B / T out of range for this ctx");
+  if (!cu_out || (num_seqs > 0 && (!query_lens || !traj_lens)) || (num_tokens > 0 && !pos_out))
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "null pointer argument");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  sq::PositionsParams pp = {};
+  pp.query_lens = query_lens; pp.traj_lens = traj_lens; pp.B = num_seqs; pp.num_tokens = num_tokens;
+  pp.pos = pos_out; pp.cu = cu_out; pp.base = ctx->pos_base; pp.status = status_out;
+  sq::sq_positions_scan_kernel<<<1, 1024, 0, st>>>(pp);
+  ctx->launches += 1;
+  if (num_seqs > 0 && num_tokens > 0) {
+    sq::sq_positions_fill_kernel<<<(unsigned)num_seqs, 256, 0, st>>>(pp);
+    ctx->launches += 1;
+  }
+  SQ_CUDA(ctx, cudaGetLastError());
+  return SQ_OK;
 }
 
 // ------------------------------------------------------------------------------------------ prepare (8(f)-2)
@@ -784,16 +988,13 @@ extern "C" int sq_score_run_x(sq_score_ctx* ctx, const void* X, int num_rows, co
   if (!ctx) return SQ_ERR_INVALID_ARG;
   if (ctx->cfg.flags & SQ_FLAG_REDUCE_ONLY) return set_err(ctx, SQ_ERR_INVALID_ARG, "ctx was created with SQ_FLAG_REDUCE_ONLY");
   if (num_tokens < 0 || num_tokens > ctx->cfg.max_tokens) return set_err(ctx, SQ_ERR_INVALID_ARG, "T out of range for this ctx");
-  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
-  int rc = ensure_h_stage(ctx);
+  int rc = need_staging(ctx);
   if (rc != SQ_OK) return rc;
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
   rc = sq_score_prepare(ctx, X, num_rows, pos, num_tokens, gain, eps, ctx->h_stage, stream);
   if (rc != SQ_OK) return rc;
   return run_impl(ctx, ctx->h_stage, W, targets, cu_seqlens, num_tokens, num_seqs, k, window, outputs, stream, nullptr, 0);
 }
-
-constexpr int HOST_FLAG_ROWS_MIN = 2048;   // rows of H per arrival flag (doubled until a run needs at most ...
-constexpr int HOST_FLAGS_PER_RUN = 256;    // ... this many flags)
 
 extern "C" int sq_score_run_host(sq_score_ctx* ctx, const void* H_host, const void* W_dev, const int32_t* targets_host,
                                  const int32_t* cu_seqlens_host, int num_tokens, int num_seqs, int k, int window,
@@ -807,21 +1008,9 @@ extern "C" int sq_score_run_host(sq_score_ctx* ctx, const void* H_host, const vo
   if (ctx->cfg.flags & SQ_FLAG_REDUCE_ONLY) return set_err(ctx, SQ_ERR_INVALID_ARG, "ctx was created with SQ_FLAG_REDUCE_ONLY");
   if (k < 1 || k > ctx->cfg.max_k || k > ctx->cfg.vocab || window < 1)   // before any copy is enqueued
     return set_err(ctx, SQ_ERR_INVALID_ARG, "k = %d outside 1..min(max_k, V) or window = %d < 1", k, window);
+  if (need_staging(ctx) != SQ_OK) return SQ_ERR_INVALID_ARG;
   SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  if (!ctx->copy_stream) {   // staging is allocated on first use: only callers of the host form pay for it
-    int rc = ensure_h_stage(ctx);
-    if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->tgt_stage, ctx->cfg.max_tokens);
-    if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->cu_stage, (int64_t)ctx->cfg.max_seqs + 1);
-    if (rc == SQ_OK) rc = ws_alloc(ctx, &ctx->h_flags, HOST_FLAGS_PER_RUN);
-    if (rc != SQ_OK) return rc;
-    SQ_CUDA(ctx, cudaHostAlloc(reinterpret_cast<void**>(&ctx->one_host), sizeof(unsigned int), cudaHostAllocDefault));
-    *ctx->one_host = 1u;
-    SQ_CUDA(ctx, cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
-    SQ_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming));
-    SQ_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_small, cudaEventDisableTiming));
-    SQ_CUDA(ctx, cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming));
-  }
   // H streams in on the ctx's copy stream in blocks of `flag_rows` rows, ascending, each followed by a 4-byte
   // copy that raises the block's flag; kernel 1 starts as soon as targets and cu_seqlens are in and its producers
   // wait for the flag of the rows they are about to load, so the transfer hides behind the GEMM.

@@ -27,54 +27,60 @@ def local_batch(cu_seqlens: torch.Tensor, rank: int, world_size: int) -> Tuple[L
     return mine, local_cu.to(torch.int32), row_index
 
 
-def gather_sequence_scores(local: dict, seq_ids: Sequence[int], num_seqs: int, world_size: int, group=None) -> dict:
-    """all_gather of the per-sequence scalars into global sequence order.  `local[key]` is a [B_local]
-    float tensor on the collective's device."""
+def gather_sequence_scores(local: dict, seq_ids: Sequence[int], num_seqs: int, world_size: int, group=None,
+                           device=None) -> dict:
+    """The one exchange of the data-parallel path: all_gather of the per-sequence scalars into global sequence
+    order, on the collective's device (`device`: cuda under NCCL, cpu under gloo; default = where `local` lives).
+    Every rank sends one packed [num_seqs, 1 + 4] block (sequence id, 4 scalars; unused rows carry id -1) in ONE
+    all_gather_into_tensor, and the result is scattered by id with tensor ops -- no host round trip, no per-row
+    loop.  `local[key]` is a [B_local] float tensor."""
     import torch.distributed as dist
-    dev = local[SEQ_KEYS[0]].device if len(seq_ids) else torch.device("cpu")
-    cap = num_seqs   # a rank can hold at most all sequences
-    buf = torch.full((cap, 1 + len(SEQ_KEYS)), float("nan"), dtype=torch.float32, device=dev)
+    if device is None:
+        device = local[SEQ_KEYS[0]].device
+    device = torch.device(device)
     n = len(seq_ids)
+    buf = torch.full((num_seqs, 1 + len(SEQ_KEYS)), float("nan"), dtype=torch.float32, device=device)
+    buf[:, 0] = -1.0
     if n:
-        buf[:n, 0] = torch.tensor(list(seq_ids), dtype=torch.float32, device=dev)
-        for j, key in enumerate(SEQ_KEYS):
-            buf[:n, 1 + j] = local[key].to(torch.float32)
-    buf[n:, 0] = -1.0
-    gathered = [torch.empty_like(buf) for _ in range(world_size)]
-    dist.all_gather(gathered, buf, group=group)
-    out = {key: torch.full((num_seqs,), float("nan"), dtype=torch.float32) for key in SEQ_KEYS}
-    for g in gathered:
-        g = g.cpu()
-        for r in range(g.shape[0]):
-            b = int(g[r, 0])
-            if b >= 0:
-                for j, key in enumerate(SEQ_KEYS):
-                    out[key][b] = g[r, 1 + j]
-    return out
+        buf[:n, 0] = torch.as_tensor(list(seq_ids), dtype=torch.float32, device=device)
+        buf[:n, 1:] = torch.stack([local[key].to(device=device, dtype=torch.float32) for key in SEQ_KEYS], dim=1)
+    flat = torch.empty((world_size * num_seqs, 1 + len(SEQ_KEYS)), dtype=torch.float32, device=device)
+    dist.all_gather_into_tensor(flat, buf, group=group)
+    ids = flat[:, 0].to(torch.int64)
+    keep = ids >= 0
+    table = torch.full((num_seqs, len(SEQ_KEYS)), float("nan"), dtype=torch.float32, device=device)
+    table[ids[keep]] = flat[keep, 1:]
+    return {key: table[:, j] for j, key in enumerate(SEQ_KEYS)}
 
 
 def score_vocab_parallel(eng, H, W_shard, vocab_starts: Sequence[int], rank: int, targets, cu_seqlens, k: int, window: int,
                          group=None, stream=None) -> dict:
     """Vocab-parallel scoring on one rank: this rank's shard of the LM head -> packed partial
     state, ONE all_gather of the states (NCCL over NVLink on GPUs), then the associative merge + kernel 2 on every
-    rank.  `eng` was created with vocab = the largest shard; every rank passes the same H, targets and cu_seqlens."""
-    import torch.distributed as dist
+    rank.  `eng` was created with vocab >= the LARGEST shard (sq_score_run_shard takes this rank's own row count from
+    W_shard); every rank passes the same H, targets and cu_seqlens."""
     world = len(vocab_starts) - 1
-    if vocab_starts[rank + 1] > vocab_starts[rank]:
+    rows = int(vocab_starts[rank + 1]) - int(vocab_starts[rank])
+    if rows != W_shard.shape[0]:
+        raise ValueError("W_shard has %d rows, vocab_starts gives this rank %d" % (W_shard.shape[0], rows))
+    if rows > 0:
         state = eng.run_shard(H, W_shard, vocab_starts[rank], targets, k, stream=stream)
     else:                                                  # more ranks than vocab tiles: this rank owns no rows
-        from .binding import neutral_shard_state
-        state = neutral_shard_state(H.shape[0], k, H.device)
+        state = eng.neutral_shard_state(H.shape[0], k, device=H.device, stream=stream)
     states = gather_shard_states(state, world, group=group, stream=stream)
     return eng.merge_shards(states, vocab_starts, targets, cu_seqlens, k, window, stream=stream)
 
 
 def gather_shard_states(state: torch.Tensor, world_size: int, group=None, stream=None) -> torch.Tensor:
     """The one collective of the vocab-parallel path: all_gather of the packed states, rank-major -- shard r's state
-    starts r * words into the result, which is what sq_score_merge_shards reads."""
+    starts r * words into the result, which is what sq_score_merge_shards reads.  On CUDA the collective is issued
+    with `stream` current, so it is ordered after the shard kernels and before the merge on that stream by stream
+    order alone: no host synchronisation."""
     import torch.distributed as dist
     flat = torch.empty(world_size * state.numel(), dtype=state.dtype, device=state.device)
-    if stream is not None:
-        stream.synchronize()   # the collective runs on its own stream
-    dist.all_gather_into_tensor(flat, state, group=group)
+    if state.is_cuda:
+        with torch.cuda.stream(stream if stream is not None else torch.cuda.current_stream(state.device)):
+            dist.all_gather_into_tensor(flat, state, group=group)
+    else:
+        dist.all_gather_into_tensor(flat, state, group=group)
     return flat.view(world_size, state.numel())

@@ -54,7 +54,7 @@ def test_create_fails_loudly_without_gpu():
 def test_create_rejects_bad_config_before_touching_cuda():
     L = sq.lib()
     h = ctypes.c_void_p()
-    bad = [dict(d=0), dict(vocab=0), dict(max_tokens=0), dict(max_seqs=0), dict(max_k=0), dict(max_k=33), dict(cta_group=3), dict(flags=2)]
+    bad = [dict(d=0), dict(vocab=0), dict(max_tokens=0), dict(max_seqs=0), dict(max_k=0), dict(max_k=33), dict(cta_group=3), dict(flags=4)]
     for kw in bad:
         base = dict(device=0, d=64, vocab=1024, max_tokens=256, max_seqs=4, max_k=5, cta_group=0, num_chunks=0, group_m=0, flags=0)
         base.update(kw)
@@ -73,6 +73,37 @@ CONFIG_SHAPES = {"tiny": (64, 1024, 256, 5), "qwen3_4b": (2560, 151936, 20480, 2
                  "gpt_oss": (2880, 201088, 73728, 20), "qwen3_32b": (5120, 151936, 557056, 20)}
 
 
+def replay_plan(p):
+    """Replays the kernel's gang decode (sq_fused_kernel.cuh make_gang_ctx / decode_gang_unit) on the host: returns
+    {(m_tile, vocab tile): visits} and the tile-times of the busiest cluster."""
+    M, r = p["m_tiles"], p["chunks_per_gang"]
+    cv = p["chunk_vtile"]
+    assert len(cv) == p["num_chunks"] + 1 and cv[0] == 0 and cv[-1] == p["num_vtiles"]
+    assert all(b > a for a, b in zip(cv, cv[1:])), "no empty chunk"
+    seen = {}
+    busiest = 0
+    big_clusters = p["gangs_big"] * (p["gang_size"] + 1)
+    for cluster in range(p["clusters_used"]):
+        if cluster < big_clusters:
+            size = p["gang_size"] + 1
+            gang, member = divmod(cluster, size)
+        else:
+            size = p["gang_size"]
+            gang, member = divmod(cluster - big_clusters, size)
+            gang += p["gangs_big"]
+        assert gang < p["num_gangs"]
+        work = 0
+        for it in range(-(-M // size) * r):
+            b, sub = divmod(it, r)
+            m, c = b * size + member, gang * r + sub
+            if m < M:
+                for vt in range(cv[c], cv[c + 1]):
+                    seen[(m, vt)] = seen.get((m, vt), 0) + 1
+                work += cv[c + 1] - cv[c]
+        busiest = max(busiest, work)
+    return seen, busiest
+
+
 @pytest.mark.parametrize("name", list(CONFIG_SHAPES))
 @pytest.mark.parametrize("cg", [1, 2])
 def test_plan_covers_every_tile_exactly_once(name, cg):
@@ -81,63 +112,61 @@ def test_plan_covers_every_tile_exactly_once(name, cg):
     assert p["cta_group"] == cg and p["rows_per_tile"] == 128 * cg
     assert p["m_tiles"] == -(-T // (128 * cg))
     assert p["num_vtiles"] == -(-V // 256) and p["num_k_blocks"] == -(-d // 64)
-    assert 1 <= p["num_chunks"] <= 160
-    # chunks tile the vocabulary: no empty chunk, full coverage
-    assert p["tiles_per_chunk"] * p["num_chunks"] >= p["num_vtiles"]
-    assert p["tiles_per_chunk"] * (p["num_chunks"] - 1) < p["num_vtiles"]
+    assert 1 <= p["num_chunks"] <= 160 and p["num_chunks"] == p["num_gangs"] * p["chunks_per_gang"]
     assert p["num_units"] == p["m_tiles"] * p["num_chunks"]
     assert p["num_clusters"] == 148 // cg
     assert p["topk_cap"] >= k
-    # replay the kernel's gang-unit decode (class-A gangs + the smaller gang B): every
-    # (m_tile, chunk) pair is visited exactly once
-    G, C, M = p["group_m"], p["num_chunks"], p["m_tiles"]
-    assert 1 <= G <= max(1, min(M, p["num_clusters"]))
-    assert p["num_gangs"] == p["num_clusters"] // G and p["num_gangs"] >= 1
-    assert p["gang_b_size"] == p["num_clusters"] - p["num_gangs"] * G
-    assert 0 <= p["m_split"] <= M
-    assert p["num_gang_units"] == -(-p["m_split"] // G) * C
-    seen = set()
-    for gang in range(p["num_gangs"]):
-        for gu in range(gang, p["num_gang_units"], p["num_gangs"]):
-            g, c = divmod(gu, C)
-            for member in range(G):
-                m = g * G + member
-                if m < p["m_split"]:
-                    assert (m, c) not in seen
-                    seen.add((m, c))
-    if p["m_split"] < M:
-        GB = p["gang_b_size"]
-        assert GB >= 1 and p["num_gang_units_b"] == -(-(M - p["m_split"]) // GB) * C
-        for gu in range(p["num_gang_units_b"]):
-            g, c = divmod(gu, C)
-            for member in range(GB):
-                m = p["m_split"] + g * GB + member
-                if m < M:
-                    assert (m, c) not in seen
-                    seen.add((m, c))
-    else:
-        assert p["num_gang_units_b"] == 0
-    assert len(seen) == p["num_units"]
+    assert p["clusters_used"] == p["num_gangs"] * p["gang_size"] + p["gangs_big"] <= p["num_clusters"]
+    assert 0 <= p["gangs_big"] <= p["num_gangs"] and p["gang_size"] >= 1
+    seen, _ = replay_plan(p)
+    assert len(seen) == p["m_tiles"] * p["num_vtiles"] and set(seen.values()) == {1}
 
 
-def test_plan_wave_efficiency_on_target_config():
-    d, V, T, k = CONFIG_SHAPES["qwen3_8b"]
+@pytest.mark.parametrize("name", ["qwen3_4b", "qwen3_8b", "gpt_oss", "qwen3_32b"])
+def test_plan_uses_every_cluster_and_balances_the_gangs(name):
+    """the round-1 plan left 2 of 74 CTA pairs idle on every benchmarked config.  Gangs of uneven size
+    (74 = 2 x 13 + 4 x 12) with vocabulary stripes sized so that all gangs finish together use all of them."""
+    d, V, T, k = CONFIG_SHAPES[name]
     p = sq.plan(d, V, T, k, num_sms=148)
-    rounds = max(-(-p["num_gang_units"] // p["num_gangs"]), p["num_gang_units_b"])
+    assert p["clusters_used"] == p["num_clusters"] == 74
+    _, busiest = replay_plan(p)
     ideal = p["m_tiles"] * p["num_vtiles"] / p["num_clusters"]
-    assert ideal / (rounds * p["tiles_per_chunk"]) > 0.95    # < 5 % lost to gang/wave quantisation
+    assert ideal / busiest > 0.94, (ideal, busiest)         # < 6 % lost to batch / stripe quantisation (qwen3_8b: 2 %)
+    if name == "qwen3_8b":
+        assert ideal / busiest > 0.975 and p["num_gangs"] == 6 and p["gang_size"] == 12 and p["gangs_big"] == 2
+
+
+def test_plan_respects_the_resident_cluster_limit():
+    # a device (or an SM partition) that holds fewer clusters: the plan never launches more than fit
+    d, V, T, k = CONFIG_SHAPES["qwen3_8b"]
+    for sms in (148, 132, 64, 8, 2):
+        p = sq.plan(d, V, T, k, num_sms=sms)
+        assert p["clusters_used"] <= sms // 2
+        seen, _ = replay_plan(p)
+        assert len(seen) == p["m_tiles"] * p["num_vtiles"] and set(seen.values()) == {1}
 
 
 def test_plan_decode_shaped_defaults():
     p = sq.plan(4096, 151936, 64, 20, num_sms=148)
-    assert p["cta_group"] == 1 and p["group_m"] == 1 and p["num_gangs"] == 148 and p["num_chunks"] > 100
+    # every SM streams its own slice of W: 594 vocab tiles over 148 single-CTA gangs, 4 or 5 tiles each
+    assert p["cta_group"] == 1 and p["gang_size"] == 1 and p["num_gangs"] == 148 == p["num_chunks"] == p["clusters_used"]
+    w = [b - a for a, b in zip(p["chunk_vtile"], p["chunk_vtile"][1:])]
+    assert set(w) == {4, 5} and sum(w) == 594
     p = sq.plan(4096, 151936, 256, 20, num_sms=148)
-    assert p["cta_group"] == 2 and p["num_gangs"] == 74 and 60 <= p["num_chunks"] <= 74
+    assert p["cta_group"] == 2 and p["num_gangs"] == 74 == p["num_chunks"]
+    p = sq.plan(4096, 150016, 100, 20, num_sms=148)         # 586 tiles: a V that does not divide evenly either
+    w = [b - a for a, b in zip(p["chunk_vtile"], p["chunk_vtile"][1:])]
+    assert p["num_chunks"] == 148 and set(w) == {3, 4} and sum(w) == 586
 
 
 def test_plan_forced_chunks_and_edge_sizes():
     assert sq.plan(64, 1024, 256, 5, num_chunks=2)["num_chunks"] == 2
     assert sq.plan(64, 1024, 256, 5, num_chunks=99)["num_chunks"] == 4        # clamped to the number of vocab tiles
+    for (T, chunks, gm) in [(600, 3, 2), (600, 1, 8), (82684, 12, 0), (82684, 5, 12), (5000, 7, 3), (300, 2, 1)]:
+        p = sq.plan(512, 5000 if T < 1000 else 151936, T, 20, num_sms=148, num_chunks=chunks, group_m=gm)
+        assert p["num_chunks"] == chunks
+        seen, _ = replay_plan(p)
+        assert len(seen) == p["m_tiles"] * p["num_vtiles"] and set(seen.values()) == {1}
     p = sq.plan(64, 1024, 0, 5)
     assert p["m_tiles"] == 0 and p["num_units"] == 0
     assert sq.plan(64, 100, 1, 1)["num_vtiles"] == 1
@@ -148,6 +177,43 @@ def test_plan_forced_chunks_and_edge_sizes():
     assert sq.plan(64, 1024, 256, 8)["topk_cap"] == 8
     assert sq.plan(64, 1024, 256, 9)["topk_cap"] == 20
     assert sq.plan(64, 1024, 256, 21)["topk_cap"] == 32
+
+
+def test_positions_host_matches_oracle_and_rejects_bad_batches():
+    """sq_score_positions_host (the next-token shift and trajectory packing of Eq. 3 / Eq. 4 behind the C ABI) against the
+    oracle's trajectory_positions."""
+    import numpy as np
+    from oracle import sq_oracle as O
+    rng = np.random.default_rng(0)
+    for B in (0, 1, 5, 300):
+        q = rng.integers(1, 50, size=B); n = rng.integers(0, 200, size=B)
+        pos, cu = sq.trajectory_positions(q.tolist(), n.tolist())
+        rpos, rcu = O.trajectory_positions(q, n)
+        assert pos == rpos.tolist() and cu == rcu.tolist()
+    assert sq.trajectory_positions([3, 1, 2], [2, 0, 3]) == ([2, 3, 7, 8, 9], [0, 2, 2, 5])     # hand-labelled
+    assert sq.trajectory_positions([0], [0]) == ([], [0, 0])                                     # nothing to predict: fine
+    for bad in (([0], [1]), ([2, 0], [1, 4]), ([-1], [0]), ([1], [-2])):
+        with pytest.raises(ValueError):
+            sq.trajectory_positions(*bad)
+    # the capacity of pos_out is respected
+    L = sq.lib()
+    q = (ctypes.c_int32 * 1)(2); n = (ctypes.c_int32 * 1)(5)
+    pos = (ctypes.c_int32 * 4)(); cu = (ctypes.c_int32 * 2)()
+    assert L.sq_score_positions_host(q, n, 1, pos, 4, cu, None) == sq.ERR_INVALID_ARG
+    assert L.sq_score_positions_host(q, n, 1, None, 5, cu, None) == sq.ERR_INVALID_ARG
+
+
+def test_lib_refuses_to_fall_back_to_a_stale_library(monkeypatch):
+    # a failed rebuild must raise, never load the old .so
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(build, "is_stale", lambda: True)
+    def boom(*a, **k):
+        raise RuntimeError("nvcc failed: (simulated)")
+    monkeypatch.setattr(build, "build", boom)
+    with pytest.raises(RuntimeError):
+        binding.lib()
+    monkeypatch.undo()
+    assert binding.lib() is not None
 
 
 def test_shard_sequences_balances_and_partitions():

@@ -43,7 +43,8 @@ def check_codes(got, scale_gpu, ref_codes, ref_scale, y):
     if diff.any():                                     # only where y is within the fp32 slack of a rounding boundary
         near = np.abs(np.abs(y - table[ref_codes]) - O.e4m3_half_ulp(y)) <= 2 * FP32_SLACK * np.abs(y) + 1e-300
         assert near[diff].all(), np.argwhere(diff & ~near)[:5]
-    assert diff.mean() < 5e-3      # bf16 x and amax have 8-bit significands: x / amax is often a small rational and y an EXACT midpoint
+    # bf16 x and amax have 8-bit significands: x / amax is often a small rational and y an EXACT midpoint
+    assert diff.sum() <= max(2, 5e-3 * diff.size)
 
 
 @pytest.mark.parametrize("rows,d", [(5, 16), (33, 200), (300, 4096), (64, 2880), (2000, 5120), (9, 8192)])

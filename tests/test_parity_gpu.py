@@ -451,7 +451,7 @@ def test_run_host_matches_run_and_null_per_token_outputs():
     sq = _sq()
     inp = workloads.make_inputs(workloads.custom(name="host", d=128, V=3000, B=3, len_lo=100, len_hi=400, k=20, window=32, seed=41, w_std=0.1))
     dev = torch.device("cuda:0")
-    eng = sq.SqScore(128, 3000, max_tokens=inp["T"], max_seqs=3, max_k=20)
+    eng = sq.SqScore(128, 3000, max_tokens=inp["T"], max_seqs=3, max_k=20, staging=True)
     W = inp["W"].to(dev)
     out = eng.run(inp["H"].to(dev), W, inp["targets"].to(dev), inp["cu_seqlens"].to(dev), 20, 32)
     out_seq_only = eng.run(inp["H"].to(dev), W, inp["targets"].to(dev), inp["cu_seqlens"].to(dev), 20, 32, per_token=False, topk=False)
@@ -477,7 +477,7 @@ def test_run_host_streams_h_in_blocks(T):
     lens = [base] * (B - 1) + [T - base * (B - 1)]
     inp = workloads.make_inputs(wl, lengths=lens)
     dev = torch.device("cuda:0")
-    eng = sq.SqScore(wl.d, wl.V, max_tokens=T, max_seqs=B, max_k=5)
+    eng = sq.SqScore(wl.d, wl.V, max_tokens=T, max_seqs=B, max_k=5, staging=True)
     W = inp["W"].to(dev)
     out = eng.run(inp["H"].to(dev), W, inp["targets"].to(dev), inp["cu_seqlens"].to(dev), 5, 64, per_token=False, topk=False)
     torch.cuda.synchronize()
@@ -489,6 +489,50 @@ def test_run_host_streams_h_in_blocks(T):
         torch.cuda.synchronize()
         assert torch.equal(dev_seq, host)
     eng.close()
+
+
+def test_no_run_call_allocates_and_staging_is_a_create_time_choice():
+    """`run` does no allocation.  Device memory in use (cudaMemGetInfo) is read after create and after the
+    FIRST call of every run form: it must not move.  Without SQ_FLAG_STAGING, run_host and run_x refuse to run."""
+    sq = _sq()
+    wl = workloads.custom(name="noalloc", d=256, V=5000, B=4, len_lo=300, len_hi=900, k=20, window=32, seed=45, w_std=0.1)
+    inp = workloads.make_inputs(wl)
+    pre = workloads.prepare_inputs(wl, query_lo=1, query_hi=20)
+    dev = torch.device("cuda:0")
+    T, B = inp["T"], inp["B"]
+    # every tensor the calls touch exists before the measurement starts
+    H, W, tg, cu = (inp[n].to(dev) for n in ("H", "W", "targets", "cu_seqlens"))
+    Hp, tp, cp = inp["H"].pin_memory(), inp["targets"].pin_memory(), inp["cu_seqlens"].pin_memory()
+    host = torch.empty(4 * B).pin_memory()
+    X, gain, ptg = pre["X"].to(dev), pre["gain"].to(dev), pre["targets"].to(dev)
+    pos_l, cu_l = sq.trajectory_positions(pre["query_lens"].tolist(), pre["traj_lens"].tolist())
+    pos = torch.tensor(pos_l, dtype=torch.int32, device=dev); pcu = torch.tensor(cu_l, dtype=torch.int32, device=dev)
+    qd, nd = pre["query_lens"].to(torch.int32).to(dev), pre["traj_lens"].to(torch.int32).to(dev)
+    st = torch.empty(sq.shard_state_bytes(T, 20) // 4, device=dev)
+    Tm = max(T, pre["T"])
+    eng = sq.SqScore(wl.d, wl.V, max_tokens=Tm, max_seqs=B, max_k=20, staging=True)
+    out = eng._alloc_out(T, B, 20, dev, True, True)
+    outx = eng._alloc_out(pre["T"], pre["B"], 20, dev, True, True)
+    pos2 = torch.empty(pre["T"], dtype=torch.int32, device=dev); cu2 = torch.empty(pre["B"] + 1, dtype=torch.int32, device=dev)
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info(0)[0]
+    eng.run(H, W, tg, cu, 20, 32, out=out)
+    eng.run_host(Hp, W, tp, cp, 20, 32, host)
+    eng.run_x(X, pos, gain, 1e-6, W, ptg, pcu, 20, 32, out=outx)
+    eng.run_shard(H, W[:2048], 0, tg, 20, out=st)
+    eng.neutral_shard_state(T, 20, out=st)
+    eng._check(eng._L.sq_score_positions(eng._h, qd.data_ptr(), nd.data_ptr(), pre["B"], pre["T"], pos2.data_ptr(), cu2.data_ptr(), None,
+                                         torch.cuda.current_stream().cuda_stream))
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info(0)[0] == free0, "a run* call allocated device memory"
+    assert torch.equal(pos2, pos) and torch.equal(cu2, pcu)
+    eng.close()
+    plain = sq.SqScore(wl.d, wl.V, max_tokens=Tm, max_seqs=B, max_k=20)
+    for call in (lambda: plain.run_host(Hp, W, tp, cp, 20, 32, host), lambda: plain.run_x(X, pos, gain, 1e-6, W, ptg, pcu, 20, 32, out=outx)):
+        with pytest.raises(sq.SqScoreError) as ei:
+            call()
+        assert ei.value.code == sq.ERR_INVALID_ARG and "SQ_FLAG_STAGING" in str(ei.value)
+    plain.close()
 
 
 def test_run_is_cuda_graph_capturable():

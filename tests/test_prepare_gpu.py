@@ -86,9 +86,13 @@ def test_run_x_end_to_end_against_oracle():
     pos_b, cu_b = sq.trajectory_positions(inp["query_lens"].tolist(), inp["traj_lens"].tolist())
     assert pos_b == pos.tolist() and cu_b == cu.tolist()
     dev = torch.device("cuda:0")
-    eng = sq.SqScore(wl.d, wl.V, max_tokens=inp["T"], max_seqs=inp["B"], max_k=wl.k)
+    eng = sq.SqScore(wl.d, wl.V, max_tokens=inp["T"], max_seqs=inp["B"], max_k=wl.k, staging=True)
     Xd, Wd, gd = inp["X"].to(dev), inp["W"].to(dev), inp["gain"].to(dev)
-    pd = torch.tensor(pos_b, dtype=torch.int32, device=dev); cd = torch.tensor(cu_b, dtype=torch.int32, device=dev)
+    # the position list comes from the device kernel (no host round trip) and must equal the oracle's
+    pd, cd, status = eng.positions(inp["query_lens"].to(torch.int32).to(dev), inp["traj_lens"].to(torch.int32).to(dev), inp["T"],
+                                   with_status=True)
+    torch.cuda.synchronize()
+    assert pd.cpu().tolist() == pos.tolist() and cd.cpu().tolist() == cu.tolist() and int(status) == 0
     td = inp["targets"].to(dev)
     out = eng.run_x(Xd, pd, gd, inp["eps"], Wd, td, cd, wl.k, wl.window)
     torch.cuda.synchronize()
@@ -106,6 +110,31 @@ def test_run_x_end_to_end_against_oracle():
     o = {n: v.cpu().numpy() for n, v in out.items()}
     check_tokens(o, ref, wl.k)
     check_seqs(o, ref)
+    eng.close()
+
+
+@pytest.mark.parametrize("B,qr,nr", [(1, (1, 1), (1, 1)), (7, (1, 40), (0, 300)), (1500, (1, 9), (0, 50)), (4096, (1, 3), (0, 7)), (3, (5, 5), (0, 0))])
+def test_positions_kernel_matches_oracle(B, qr, nr):
+    """sq_score_positions (device) against the oracle's trajectory_positions: many candidates (the scan spans several
+    candidates per thread), empty trajectories, an all-empty batch; and the status word for bad inputs."""
+    sq = _sq()
+    rng = np.random.default_rng(B)
+    q = rng.integers(qr[0], qr[1] + 1, size=B); n = rng.integers(nr[0], nr[1] + 1, size=B)
+    pos, cu = O.trajectory_positions(q, n)
+    dev = torch.device("cuda:0")
+    eng = sq.SqScore(64, 1000, max_tokens=max(1, len(pos)), max_seqs=B)
+    pd, cd, st = eng.positions(torch.tensor(q, dtype=torch.int32, device=dev), torch.tensor(n, dtype=torch.int32, device=dev), len(pos),
+                               with_status=True)
+    torch.cuda.synchronize()
+    assert pd.cpu().tolist() == pos.tolist() and cd.cpu().tolist() == cu.tolist() and int(st) == 0
+    if B >= 7 and n.sum() > 0:
+        q2 = q.copy(); b = int(np.argmax(n > 0)); q2[b] = 0                  # a trajectory with no query token before it
+        _, _, st2 = eng.positions(torch.tensor(q2, dtype=torch.int32, device=dev), torch.tensor(n, dtype=torch.int32, device=dev), len(pos),
+                                  with_status=True)
+        _, _, st3 = eng.positions(torch.tensor(q, dtype=torch.int32, device=dev), torch.tensor(n, dtype=torch.int32, device=dev), len(pos) - 1,
+                                  with_status=True)                           # lengths that do not sum to num_tokens
+        torch.cuda.synchronize()
+        assert int(st2) == 1 and int(st3) == 1
     eng.close()
 
 

@@ -50,6 +50,28 @@ def test_two_rank_sharding_matches_single_rank():
         np.testing.assert_allclose(a[~np.isnan(b)], b[~np.isnan(b)], rtol=1e-6)
 
 
+def _few_worker(rank, world, port, ret):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    ids = [0] if rank == 1 else []                      # more ranks than sequences: ranks 0 and 2 own nothing
+    local = {k: torch.tensor([float(i + 1)]) if ids else torch.zeros(0) for i, k in enumerate(sharding.SEQ_KEYS)}
+    out = sharding.gather_sequence_scores(local, ids, 1, world, device="cpu")
+    ret[rank] = {k: v.clone() for k, v in out.items()}
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_gather_with_ranks_that_own_no_sequence():
+    """world > B: a rank without sequences still takes part in the ONE collective, on the collective's device."""
+    with mp.Manager() as mgr:
+        ret = mgr.dict()
+        mp.spawn(_few_worker, args=(3, _free_port(), ret), nprocs=3, join=True)
+        got = dict(ret)
+    for r in range(3):
+        for i, k in enumerate(sharding.SEQ_KEYS):
+            assert got[r][k].tolist() == [float(i + 1)]
+
+
 def test_local_batch_partitions_rows():
     cu = torch.tensor([0, 9, 9, 39, 43, 60], dtype=torch.int32)
     seen = []
@@ -71,6 +93,11 @@ def test_shard_vocab_partition():
         assert all(s % 256 == 0 for s in st[:-1])                       # shards start on vocab-tile boundaries
         sizes = [b - a for a, b in zip(st, st[1:])]
         assert max(sizes) - min(s for s in sizes[:-1] or sizes) <= 2 * 256 or V < 256 * R
+    # more ranks than vocab tiles: the surplus ranks own no rows (they contribute the merge's neutral element)
+    st = sq.shard_vocab(600, 5)
+    assert st == [0, 0, 256, 256, 512, 600] and sum(b > a for a, b in zip(st, st[1:])) == 3
+    # the packed state's size does not depend on the shard's row count: uneven and empty shards exchange equal blocks
+    assert sq.shard_state_bytes(100, 20) == (6 + 40) * 100 * 4
 
 
 def _vp_worker(rank, world, port, words, ret):

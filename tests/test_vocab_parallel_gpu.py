@@ -20,23 +20,22 @@ def _sq():
 
 
 def run_sharded(inp, starts, k, window, targets=None):
+    """Every shard through ONE ctx sized for the largest shard (the layout sharding.score_vocab_parallel uses: uneven
+    shards pass their own row count to sq_score_run_shard)."""
     sq = _sq()
     wl = inp["workload"]
     T, B = inp["T"], inp["B"]
     H = inp["H"].to(DEV); W = inp["W"].to(DEV); cu = inp["cu_seqlens"].to(DEV)
     tg = (inp["targets"] if targets is None else targets).to(DEV)
+    eng = sq.SqScore(wl.d, max(1, max(starts[r + 1] - starts[r] for r in range(len(starts) - 1))), max_tokens=T, max_seqs=B, max_k=k)
     states = []
     for r in range(len(starts) - 1):
         v0, v1 = starts[r], starts[r + 1]
         if v1 == v0:
-            states.append(sq.neutral_shard_state(T, k, DEV))
-            continue
-        eng = sq.SqScore(wl.d, v1 - v0, max_tokens=T, max_seqs=B, max_k=k)
-        states.append(eng.run_shard(H, W[v0:v1].contiguous(), v0, tg, k))
-        torch.cuda.synchronize()
-        eng.close()
+            states.append(eng.neutral_shard_state(T, k, device=DEV))
+        else:
+            states.append(eng.run_shard(H, W[v0:v1], v0, tg, k))          # a view into W: rows beyond v1 belong to the next shard
     allst = torch.stack(states)                       # what all_gather_into_tensor would return
-    eng = sq.SqScore(wl.d, max(1, max(starts[r + 1] - starts[r] for r in range(len(starts) - 1))), max_tokens=T, max_seqs=B, max_k=k)
     out = eng.merge_shards(allst, starts, tg, cu, k, window)
     torch.cuda.synchronize()
     eng.close()
@@ -94,6 +93,40 @@ def test_sharded_model_shaped():
     check_tokens(out, ref, wl.k, rows=rows)
 
 
+def test_score_vocab_parallel_entry_point_single_process():
+    """sharding.score_vocab_parallel itself (the shipped entry point) with uneven shards and a ctx sized for the largest:
+    one process plays every rank in turn with the collective replaced by a local stand-in that returns the stacked
+    states (the NCCL form is exercised at world_size 1 in test_nccl_world1_gpu.py, the layout with gloo on CPU)."""
+    sq = _sq()
+    from paper_2604_07725_b200 import sharding
+    wl = workloads.custom(name="vp_entry", d=128, V=1900, B=3, len_lo=40, len_hi=160, k=20, window=16, seed=64, w_std=0.2,
+                          planted_frac=0.5, planted_scale=3.0, rmsnorm=True)
+    inp = workloads.make_inputs(wl)
+    starts = [0, 512, 1280, 1280, 1900]                                     # 512 / 768 / 0 / 620 rows
+    H = inp["H"].to(DEV); W = inp["W"].to(DEV); cu = inp["cu_seqlens"].to(DEV); tg = inp["targets"].to(DEV)
+    eng = sq.SqScore(wl.d, 768, max_tokens=inp["T"], max_seqs=inp["B"], max_k=wl.k)
+    states = [None] * 4
+    real_gather = sharding.gather_shard_states
+    try:
+        for phase in (0, 1):                                                # phase 0 collects every rank's state, phase 1 merges
+            for r in range(4):
+                def fake_gather(state, world, group=None, stream=None, r=r):
+                    states[r] = state
+                    return torch.stack([s if s is not None else torch.zeros_like(state) for s in states])
+                sharding.gather_shard_states = fake_gather
+                out = sharding.score_vocab_parallel(eng, H, W[starts[r]:starts[r + 1]], starts, r, tg, cu, wl.k, wl.window)
+    finally:
+        sharding.gather_shard_states = real_gather
+    torch.cuda.synchronize()
+    ref = O.score(inp["H"], inp["W"], inp["targets"], inp["cu_seqlens"], wl.k, wl.window)
+    o = {n: v.cpu().numpy() for n, v in out.items()}
+    check_tokens(o, ref, wl.k)
+    check_seqs(o, ref)
+    with pytest.raises(ValueError):
+        sharding.score_vocab_parallel(eng, H, W[0:100], starts, 0, tg, cu, wl.k, wl.window)
+    eng.close()
+
+
 def test_shard_api_errors():
     sq = _sq()
     eng = sq.SqScore(64, 512, max_tokens=32, max_seqs=2, max_k=5)
@@ -105,5 +138,9 @@ def test_shard_api_errors():
         eng.merge_shards(st, [0, 512, 1024], tg, cu, 6, 4)          # k > max_k
     with pytest.raises(sq.SqScoreError):
         eng.run_shard(torch.zeros(32, 64, dtype=torch.bfloat16, device=DEV), torch.zeros(512, 64, dtype=torch.bfloat16, device=DEV), -1, tg, 5)
+    with pytest.raises(sq.SqScoreError):             # more rows than the ctx was sized for
+        eng.run_shard(torch.zeros(32, 64, dtype=torch.bfloat16, device=DEV), torch.zeros(513, 64, dtype=torch.bfloat16, device=DEV), 0, tg, 5)
+    with pytest.raises(sq.SqScoreError):             # k larger than the shard
+        eng.run_shard(torch.zeros(32, 64, dtype=torch.bfloat16, device=DEV), torch.zeros(3, 64, dtype=torch.bfloat16, device=DEV), 0, tg, 5)
     assert sq.shard_state_bytes(32, 5) == (6 + 2 * 8) * 32 * 4 and sq.shard_state_bytes(10, 20) == (6 + 40) * 40
     eng.close()
