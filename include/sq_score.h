@@ -319,6 +319,12 @@ int sq_score_set_profiling(sq_score_ctx *ctx, int enable);
 int sq_score_kernel_times(sq_score_ctx *ctx, float *ms3);
 int sq_score_profile_read(sq_score_ctx *ctx, float *ms, int capacity, int *num_runs);
 
+/* Test hook (tests/test_memory_safety_gpu.py): fills every ctx-owned workspace and staging buffer with the byte
+ * `value` (0xFF = NaN floats / -1 ints) on `stream`, then restores the two invariants the kernels rely on (zeroed
+ * per-sequence counters of kernel 2).  A run after it must give the same results: no kernel may read workspace it
+ * did not write in the same run.  Changes no result.  Errors: INVALID_ARG, CUDA. */
+int sq_score_debug_fill_workspace(sq_score_ctx *ctx, int value, void *stream);
+
 /* Number of kernels this ctx has launched so far (bench.py's `gpu_launches`). */
 int64_t sq_score_launch_count(const sq_score_ctx *ctx);
 

@@ -84,6 +84,8 @@ def lib() -> C.CDLL:
     L.sq_score_positions_host.restype = C.c_int
     L.sq_score_positions.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     L.sq_score_positions.restype = C.c_int
+    L.sq_score_debug_fill_workspace.argtypes = [C.c_void_p, C.c_int, C.c_void_p]
+    L.sq_score_debug_fill_workspace.restype = C.c_int
     L.sq_score_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.c_int, C.POINTER(C.c_int)]
     L.sq_score_profile_read.restype = C.c_int
     L.sq_score_merge_shards.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_int32), C.c_void_p, C.c_void_p, C.c_int, C.c_int,
@@ -346,6 +348,10 @@ class SqScore:
         self._check(self._L.sq_score_select_prob(self._h, _ptr(fitness), _ptr(pop_offsets), pop_offsets.shape[0] - 1,
                                                  float(zeta), _ptr(prob), self._stream(stream)))
         return prob
+
+    def debug_fill_workspace(self, value: int = 0xFF, stream=None):
+        """sq_score_debug_fill_workspace (test hook): poison every ctx-owned buffer with a byte pattern."""
+        self._check(self._L.sq_score_debug_fill_workspace(self._h, int(value), self._stream(stream)))
 
     def set_profiling(self, enable: bool):
         self._check(self._L.sq_score_set_profiling(self._h, 1 if enable else 0))

@@ -23,6 +23,7 @@ struct FinalizeParams {
   long long rank_stride;
   int num_ranks;
   int vstart[33];           // ranks > 1: rank r owns vocabulary ids [vstart[r], vstart[r+1]) -- whose zt is the target's
+  int vocab_offset;         // EMIT mode: this shard's columns are global ids [vocab_offset, vocab_offset + V)
   // EMIT mode (sq_score_run_shard): instead of finalising, write the merged state as ONE chunk in the same format
   float* out_m; float* out_s; float* out_u; float* out_cs; float* out_cu;   // [T]
   float* out_topv; int32_t* out_topi;                                        // [cap][T]
@@ -174,7 +175,9 @@ sq_finalize_kernel(const FinalizeParams p) {
       p.out_m[row] = M;
       p.out_s[row] = s_hi; p.out_cs[row] = (float)((double)s_hi - S);
       p.out_u[row] = u_hi; p.out_cu[row] = (float)((double)u_hi - U);
-      p.out_zt[row] = p.zt[row];                 // meaningful only on the shard that owns the target's column
+      // the target's logit exists only on the shard that owns its column (kernel 1 writes zt[row] only there)
+      const int tl = p.targets[row] - p.vocab_offset;
+      p.out_zt[row] = (tl >= 0 && tl < p.V) ? p.zt[row] : 0.f;
     }
     return;
   }

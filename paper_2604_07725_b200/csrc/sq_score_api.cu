@@ -690,6 +690,7 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fin.lse = lse; fin.target_logprob = lp; fin.entropy = ent; fin.conf = conf;
     fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
     fin.chunks_per_rank = pl.num_chunks; fin.rank_stride = 0; fin.num_ranks = 1;
+    fin.vocab_offset = vocab_offset;
     const dim3 fgrid((unsigned)cdiv64(T, sq::FIN_WARPS)), fblock(sq::FIN_WARPS * 32);
     const dim3 fgrid8((unsigned)cdiv64(T, sq::FIN_WARPS * 4));   // 8 lanes per row: four rows per warp
     const bool lpr8 = pl.num_chunks <= 8 && !(ctx->debug_flags & 128);
@@ -859,6 +860,30 @@ extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int 
     const int rc = launch_reduce(ctx, rp, st);
     if (rc != SQ_OK) return rc;
   }
+  return SQ_OK;
+}
+
+extern "C" int sq_score_debug_fill_workspace(sq_score_ctx* ctx, int value, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const sq_score_config& c = ctx->cfg;
+  const bool ro = (c.flags & SQ_FLAG_REDUCE_ONLY) != 0;
+  const int64_t rows = ro ? 1 : ws_rows_for(c), T = c.max_tokens;
+  struct Buf { void* p; int64_t bytes; };
+  const Buf bufs[] = {
+      {ctx->part_m, rows * 4}, {ctx->part_s, rows * 4}, {ctx->part_u, rows * 4}, {ctx->part_cs, rows * 4}, {ctx->part_cu, rows * 4},
+      {ctx->part_topv, rows * ctx->cap_max * 4}, {ctx->part_topi, rows * ctx->cap_max * 4}, {ctx->zt, (ro ? 1 : T) * 4},
+      {ctx->gang_ctr, 256 * 4}, {ctx->thr_pub, (ro ? 1 : (int64_t)THR_MAX_CHUNKS * T) * 4},
+      {ctx->tok_lse, (ro ? 1 : T) * 4}, {ctx->tok_lp, (ro ? 1 : T) * 4}, {ctx->tok_ent, (ro ? 1 : T) * 4}, {ctx->tok_conf, (ro ? 1 : T) * 4},
+      {ctx->tile_base, ((int64_t)c.max_seqs + 1) * 4}, {ctx->amax_bits, 4}, {ctx->red_sum, ctx->red_tiles_max * 16},
+      {ctx->tile_seq, ctx->red_tiles_max * 4}, {ctx->red_min, ctx->red_tiles_max * 4}, {ctx->seq_stage, 4 * (int64_t)c.max_seqs * 4},
+      {ctx->pos_base, ((int64_t)c.max_seqs + 1) * 4},
+      {ctx->h_stage, ctx->h_stage ? T * (int64_t)c.d * 2 : 0}, {ctx->tgt_stage, ctx->tgt_stage ? T * 4 : 0},
+      {ctx->cu_stage, ctx->cu_stage ? ((int64_t)c.max_seqs + 1) * 4 : 0}, {ctx->h_flags, ctx->h_flags ? HOST_FLAGS_PER_RUN * 4 : 0}};
+  for (const Buf& b : bufs)
+    if (b.p && b.bytes > 0) SQ_CUDA(ctx, cudaMemsetAsync(b.p, value, (size_t)b.bytes, st));
+  SQ_CUDA(ctx, cudaMemsetAsync(ctx->seq_done, 0, (size_t)c.max_seqs * sizeof(int), st));   // invariant: zero between runs
   return SQ_OK;
 }
 

@@ -373,7 +373,7 @@ def _reduce_both_forms(sq, make_engine, call):
     return outs[0]
 
 
-@pytest.mark.parametrize("window", [1, 2, 16, 511, 512, 513, 2048, 4096, 4097, 100000])
+@pytest.mark.parametrize("window", [1, 2, 3, 16, 511, 512, 513, 2048, 4096, 4097, 8191, 8192, 8193, 8195, 12290, 100000])
 def test_reduce_kernel_alone(window):
     sq = _sq()
     lens = [1, 2, 511, 512, 513, 0, 4095, 4096, 4097, 8192, 9000, 20000, 3, 1025]
