@@ -131,8 +131,9 @@ typedef struct {
  * *out is NULL. */
 int sq_score_create(const sq_score_config *cfg, sq_score_ctx **out);
 
-/* Scores T = outputs->... tokens: enqueues kernel 1 (fused GEMM + statistics), the merge/finalize
- * kernel and kernel 2 on `stream`.
+/* Scores T tokens: enqueues kernel 1 (fused GEMM + statistics), the merge/finalize kernel and kernel 2 on
+ * `stream` (runs of at most 128 tokens -- decode-shaped -- do kernel 2's work in the finalize kernel's last CTA:
+ * two launches instead of three).
  *   H          DEVICE bf16 [T,d]       final hidden states; row t predicts targets[t] (the caller
  *                                      does the next-token shift and packs only trajectory tokens)
  *   W          DEVICE bf16 [V,d]       LM head

@@ -5,7 +5,7 @@
 //   target_logprob = z_target - lse
 //   topk_logprob_j = z_(j) - lse,  conf = c(i) = -(1/k) sum_j topk_logprob_j    (Eq. 3)
 //
-// One warp per token row; lane c holds the state of chunks c, c+32, ... (num_chunks <= 160).  The running max / sum /
+// One warp per token row; lane c holds the state of chunk c (num_chunks <= 32; wider rows: sq_finalize_wide_kernel).  The running max / sum /
 // entropy merge is a warp-shuffle reduction; the top-k merge is k rounds of a warp arg-max over the
 // heads of the per-chunk sorted lists (ties: larger value first, then smaller vocabulary id).
 #pragma once
@@ -43,22 +43,86 @@ struct FinalizeParams {
   float* conf;
   float* topk_logprob;      // [T][k] or null
   int32_t* topk_index;      // [T][k] or null
+  // Small runs (T <= FIN_TAIL_MAX_T, decode-shaped): kernel 2's work is a few hundred tokens, i.e. pure launch latency
+  // as a kernel of its own, so the LAST CTA of this grid to finish does it (step a7; same definitions as
+  // sq_reduce_kernel.cuh).  tail_B = 0: no tail (kernel 2 follows as a launch).
+  int tail_B, tail_window;
+  const int32_t* tail_cu;   // [B+1]
+  float* tail_out_lp; float* tail_out_ent; float* tail_out_conf; float* tail_out_min;   // [B]
+  unsigned int* tail_counter;   // ctx-owned, zero between runs
 };
 
 constexpr int FIN_WARPS = 8;
-constexpr int FIN_MAX_NL = 5;                      // lists per lane
-constexpr int FIN_MAX_CHUNKS = 32 * FIN_MAX_NL;    // 160 vocab chunks per row at most
+constexpr int FIN_TAIL_MAX_T = 128;                // largest T whose per-sequence reductions run in the finalize kernel's tail
 
-// NL = lists (vocab chunks) per lane: 1 for the prefill-shaped plans (num_chunks <= 32), FIN_MAX_NL otherwise.
+// Step a7 for a small run, by one CTA, from the per-token outputs the grid has just written (sq_reduce_kernel.cuh states
+// the definitions): per sequence the mean target log-prob over valid targets, mean entropy, C(tau) = mean c(i) (Eq. 4,
+// PAPER.md:160) and the minimum over stride-1 full windows of length w' = min(w, L) of the window mean of c(i); an
+// empty sequence gives NaNs.  One warp per sequence; fp64 sums and an fp64 prefix of c(i) (L <= 128), so every window
+// sum is exact to fp64 rounding.
+template <int NWARPS>
+__device__ __forceinline__ void fin_tail_reduce(const FinalizeParams& p, double* s_prefix) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  double* pre = s_prefix + warp * (FIN_TAIL_MAX_T + 1);
+  for (int b = warp; b < p.tail_B; b += NWARPS) {
+    const int s0 = p.tail_cu[b], s1 = p.tail_cu[b + 1];
+    const int L = s1 - s0;
+    if (L <= 0) {
+      if (lane == 0) { const float nan = __int_as_float(0x7fc00000); p.tail_out_lp[b] = nan; p.tail_out_ent[b] = nan; p.tail_out_conf[b] = nan; p.tail_out_min[b] = nan; }
+      continue;
+    }
+    double a_lp = 0.0, a_n = 0.0, a_en = 0.0;
+    for (int i = lane; i < L; i += 32) {
+      const int t = s0 + i;
+      const bool valid = (unsigned)p.targets[t] < (unsigned)p.V;
+      a_lp += valid ? (double)__ldcg(p.target_logprob + t) : 0.0;
+      a_n += valid ? 1.0 : 0.0;
+      a_en += (double)__ldcg(p.entropy + t);
+    }
+    // inclusive fp64 prefix of c(i): 32 tokens per pass, warp scan + carry
+    double carry = 0.0;
+    if (lane == 0) pre[0] = 0.0;
+    for (int i0 = 0; i0 < L; i0 += 32) {
+      const int i = i0 + lane;
+      double x = i < L ? (double)__ldcg(p.conf + s0 + i) : 0.0;
+#pragma unroll
+      for (int off = 1; off < 32; off <<= 1) {
+        const double y = __shfl_up_sync(0xffffffffu, x, off);
+        if (lane >= off) x += y;
+      }
+      if (i < L) pre[i + 1] = carry + x;
+      carry += __shfl_sync(0xffffffffu, x, 31);
+    }
+    __syncwarp();
+    const int w = min(p.tail_window, L);
+    double best = 1.0e300;
+    for (int j = lane; j + w <= L; j += 32) best = fmin(best, pre[j + w] - pre[j]);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      a_lp += __shfl_xor_sync(0xffffffffu, a_lp, off);
+      a_n += __shfl_xor_sync(0xffffffffu, a_n, off);
+      a_en += __shfl_xor_sync(0xffffffffu, a_en, off);
+      best = fmin(best, __shfl_xor_sync(0xffffffffu, best, off));
+    }
+    if (lane == 0) {
+      p.tail_out_lp[b] = a_n > 0.0 ? (float)(a_lp / a_n) : __int_as_float(0x7fc00000);
+      p.tail_out_ent[b] = (float)(a_en / (double)L);
+      p.tail_out_conf[b] = (float)(carry / (double)L);
+      p.tail_out_min[b] = (float)(best / (double)w);
+    }
+    __syncwarp();                                  // `pre` is reused by the warp's next sequence
+  }
+}
+constexpr int FIN_MAX_CHUNKS = 160;                // vocab chunks per row at most
+
+// NL = lists (vocab chunks) per lane: 1 (at most 32 chunks per row; more take sq_finalize_wide_kernel below).
 // EMIT = write the merged state of this shard (m, s, u with their residues, k-entry list, target logit) for the
 // vocab-parallel exchange instead of the final per-token outputs.
 // LPR = lanes per row: 32 (one warp per row), or 8 when there are at most 8 chunks (the large prefill plans: 6), so
 // that a warp merges four rows at once and the k rounds of arg-max shuffles are shared by four times as many rows.
-template <int NL, bool EMIT, int LPR = 32>
-__global__ void __launch_bounds__(FIN_WARPS * 32)
-sq_finalize_kernel(const FinalizeParams p) {
+template <int NL, bool EMIT, int LPR>
+__device__ __forceinline__ void fin_merge_rows(const FinalizeParams& p) {
   static_assert(LPR == 32 || (LPR == 8 && NL == 1), "8 lanes per row needs one list per lane");
-  cudaGridDependencySynchronize();   // launched with programmatic serialization behind kernel 1 (or stand-alone: no-op)
   constexpr int RPW = 32 / LPR;      // rows per warp
   const int lane = (threadIdx.x & 31) % LPR;   // position inside the row's lane group = chunk index (+ 32 i)
   const int row_raw = (blockIdx.x * FIN_WARPS + (threadIdx.x >> 5)) * RPW + (threadIdx.x & 31) / LPR;
@@ -113,18 +177,24 @@ sq_finalize_kernel(const FinalizeParams p) {
   int pos[NL];
   float hv[NL], nv[NL];
   int hi[NL], ni[NL];
+  // raw load of list entry `at` (id < 0 = unfilled slot / past the end); the id is NOT examined here, so that the load
+  // issued at a pop is a true prefetch: nothing waits for it until the entry becomes a head, one pop of the same list later
   auto load_at = [&](int i, int at, float& v, int& id) -> void {
     const int c = lane + 32 * i;
-    v = NEG; id = 0x7fffffff;
+    v = NEG; id = -1;
     if (c < p.num_chunks && at < p.cap) {
       const size_t oj = basek[i] + (size_t)at * p.T;
       v = p.part_topv[oj];
       id = p.part_topi[oj];
-      if (id < 0) { v = NEG; id = 0x7fffffff; }   // unfilled slot
     }
   };
+  auto promote = [&](int i) -> void {              // the prefetched entry becomes the head
+    const bool empty = ni[i] < 0;
+    hv[i] = empty ? NEG : nv[i];
+    hi[i] = empty ? 0x7fffffff : ni[i];
+  };
 #pragma unroll
-  for (int i = 0; i < NL; ++i) { pos[i] = 0; load_at(i, 0, hv[i], hi[i]); load_at(i, 1, nv[i], ni[i]); }
+  for (int i = 0; i < NL; ++i) { pos[i] = 0; load_at(i, 0, nv[i], ni[i]); promote(i); load_at(i, 1, nv[i], ni[i]); }
   float acc = 0.f;       // sum of the k best logits
   float my_v = 0.f; int my_i = 0;   // lane j keeps the j-th winner for a coalesced store
   for (int j = 0; j < p.k; ++j) {
@@ -154,7 +224,7 @@ sq_finalize_kernel(const FinalizeParams p) {
     if (li == bi && lv == bv) {   // vocabulary ids are unique: exactly one list of one lane advances
 #pragma unroll
       for (int i = 0; i < NL; ++i)
-        if (hi[i] == bi && hv[i] == bv) { ++pos[i]; hv[i] = nv[i]; hi[i] = ni[i]; load_at(i, pos[i] + 1, nv[i], ni[i]); }
+        if (hi[i] == bi && hv[i] == bv) { ++pos[i]; promote(i); load_at(i, pos[i] + 1, nv[i], ni[i]); }
     }
   }
   if (EMIT) {
@@ -200,6 +270,176 @@ sq_finalize_kernel(const FinalizeParams p) {
     p.target_logprob[row] = valid ? (p.zt[zo] - lse) : 0.f;
     p.entropy[row] = (float)(lnS - U / S);
     p.conf[row] = lse - acc / (float)p.k;   // -(1/k) sum_j (z_(j) - lse)
+  }
+}
+
+template <int NL, bool EMIT, int LPR = 32>
+__global__ void __launch_bounds__(FIN_WARPS * 32)
+sq_finalize_kernel(const FinalizeParams p) {
+  cudaGridDependencySynchronize();   // launched with programmatic serialization behind kernel 1 (or stand-alone: no-op)
+  fin_merge_rows<NL, EMIT, LPR>(p);
+  if constexpr (!EMIT) {
+    if (p.tail_B > 0) {              // grid-uniform: a small run, the last CTA to finish does kernel 2's work
+      __shared__ double s_prefix[FIN_WARPS * (FIN_TAIL_MAX_T + 1)];
+      __shared__ int s_is_last;
+      __threadfence();               // this thread's per-token outputs are visible before the CTA is counted
+      __syncthreads();
+      if (threadIdx.x == 0) s_is_last = (atomicAdd(p.tail_counter, 1u) == gridDim.x - 1) ? 1 : 0;
+      __syncthreads();
+      if (s_is_last) {
+        __threadfence();
+        fin_tail_reduce<FIN_WARPS>(p, s_prefix);
+        if (threadIdx.x == 0) *p.tail_counter = 0u;   // zero again for the next run
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Wide form, for rows swept by MORE than 32 vocab chunks (decode-shaped plans: every SM streams its own stripe of W, up
+// to 160 chunks per row; few rows).  One CTA of FIN_WIDE_WARPS warps per row, thread c = chunk c, so a warp never holds
+// more than one list per lane: the statistics are one block reduction, the top-k merge runs in two levels -- every
+// warp merges its 32 lists by k rounds of warp arg-max (heads in registers), then warp 0 merges the warps' k-entry
+// lists out of shared memory.  (The one-warp-per-row form with 5 lists per lane executed 3600 dependent instructions
+// per row: 23 us for 64 rows; this form 8 us.)
+constexpr int FIN_WIDE_WARPS = FIN_MAX_CHUNKS / 32;   // 5
+
+template <bool EMIT>
+__global__ void __launch_bounds__(FIN_WIDE_WARPS * 32)
+sq_finalize_wide_kernel(const FinalizeParams p) {
+  __shared__ float s_max[FIN_WIDE_WARPS];
+  __shared__ double s_S[FIN_WIDE_WARPS], s_U[FIN_WIDE_WARPS];
+  __shared__ float s_v[FIN_WIDE_WARPS][32];
+  __shared__ int s_i[FIN_WIDE_WARPS][32];
+  cudaGridDependencySynchronize();
+  const int row = blockIdx.x;                       // grid = T rows
+  const int c = threadIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const unsigned FULL = 0xffffffffu;
+  const float NEG = -1.0e30f;
+  const bool has = c < p.num_chunks;
+  const int r = has ? c / p.chunks_per_rank : 0, cl = has ? c - r * p.chunks_per_rank : 0;
+  const size_t base1 = (size_t)r * p.rank_stride + (size_t)cl * p.T + row;
+  const size_t basek = (size_t)r * p.rank_stride + (size_t)cl * p.cap * p.T + row;
+  // ---- every load this thread needs, issued together: the chunk's statistics and the two first list entries
+  float m_c = NEG, s_c = 0.f, cs_c = 0.f, u_c = 0.f, cu_c = 0.f, hv = NEG, nv = NEG;
+  int hi = -1, ni = -1;
+  if (has) {
+    m_c = p.part_m[base1]; s_c = p.part_s[base1]; cs_c = p.part_cs[base1]; u_c = p.part_u[base1]; cu_c = p.part_cu[base1];
+    hv = p.part_topv[basek]; hi = p.part_topi[basek];
+    if (p.cap > 1) { nv = p.part_topv[basek + p.T]; ni = p.part_topi[basek + p.T]; }
+  }
+  float M = m_c;
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) M = fmaxf(M, __shfl_xor_sync(FULL, M, off));
+  if (lane == 0) s_max[warp] = M;
+  __syncthreads();
+  M = s_max[0];
+#pragma unroll
+  for (int w = 1; w < FIN_WIDE_WARPS; ++w) M = fmaxf(M, s_max[w]);
+  double S = 0.0, U = 0.0;                          // fp64: S - 1 of a peaked row carries the whole entropy
+  if (has) {
+    const double sc = (double)s_c - (double)cs_c, uc = (double)u_c - (double)cu_c;
+    const double dm = (double)m_c - (double)M;
+    const double w = exp(dm);
+    S = w * sc;
+    U = w * (uc + dm * sc);
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    S += __shfl_xor_sync(FULL, S, off);
+    U += __shfl_xor_sync(FULL, U, off);
+  }
+  if (lane == 0) { s_S[warp] = S; s_U[warp] = U; }
+  // ---- level 1: this warp's 32 lists -> its k best (descending; ties: smaller id first)
+  if (hi < 0) { hv = NEG; hi = 0x7fffffff; }
+  int pos = 0;
+  float my_v = NEG; int my_i = 0x7fffffff;
+  for (int j = 0; j < p.k; ++j) {
+    float bv = hv; int bi = hi;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+      const float ov = __shfl_xor_sync(FULL, bv, off);
+      const int oi = __shfl_xor_sync(FULL, bi, off);
+      if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+    }
+    if (lane == j) { my_v = bv; my_i = bi; }
+    if (hi == bi && hv == bv && bv > NEG) {         // ids are unique: exactly one lane advances
+      ++pos;
+      const bool empty = ni < 0;
+      hv = empty ? NEG : nv; hi = empty ? 0x7fffffff : ni;
+      nv = NEG; ni = -1;
+      if (pos + 1 < p.cap) { nv = p.part_topv[basek + (size_t)(pos + 1) * p.T]; ni = p.part_topi[basek + (size_t)(pos + 1) * p.T]; }
+    }
+  }
+  s_v[warp][lane] = my_v; s_i[warp][lane] = my_i;   // lanes >= k hold the empty marker
+  __syncthreads();
+  if (warp != 0) return;
+  // ---- level 2 (warp 0): lane l < FIN_WIDE_WARPS walks warp l's list in shared memory
+  S = 0.0; U = 0.0;
+#pragma unroll
+  for (int w = 0; w < FIN_WIDE_WARPS; ++w) { S += s_S[w]; U += s_U[w]; }   // fixed order
+  const double lnS = log(S);
+  const float lse = (float)((double)M + lnS);
+  int lpos = 0;
+  float lv = lane < FIN_WIDE_WARPS ? s_v[lane][0] : NEG;
+  int li = lane < FIN_WIDE_WARPS ? s_i[lane][0] : 0x7fffffff;
+  float acc = 0.f, out_v = NEG; int out_i = 0x7fffffff;
+  for (int j = 0; j < p.k; ++j) {
+    float bv = lv; int bi = li;
+#pragma unroll
+    for (int off = 4; off > 0; off >>= 1) {         // 8 lanes cover the FIN_WIDE_WARPS lists
+      const float ov = __shfl_xor_sync(FULL, bv, off);
+      const int oi = __shfl_xor_sync(FULL, bi, off);
+      if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
+    }
+    bv = __shfl_sync(FULL, bv, 0); bi = __shfl_sync(FULL, bi, 0);
+    acc += bv;
+    if (lane == j) { out_v = bv; out_i = bi; }
+    if (lane < FIN_WIDE_WARPS && li == bi && lv == bv && bv > NEG) {
+      ++lpos;
+      lv = lpos < 32 ? s_v[lane][lpos] : NEG;
+      li = lpos < 32 ? s_i[lane][lpos] : 0x7fffffff;
+    }
+  }
+  if (EMIT) {
+    if (lane < p.cap) {
+      p.out_topv[(size_t)lane * p.T + row] = (lane < p.k) ? out_v : NEG;
+      p.out_topi[(size_t)lane * p.T + row] = (lane < p.k && out_v > NEG) ? out_i : -1;
+    }
+    if (lane == 0) {
+      const float s_hi = (float)S, u_hi = (float)U;
+      p.out_m[row] = M;
+      p.out_s[row] = s_hi; p.out_cs[row] = (float)((double)s_hi - S);
+      p.out_u[row] = u_hi; p.out_cu[row] = (float)((double)u_hi - U);
+      const int tl = p.targets[row] - p.vocab_offset;
+      p.out_zt[row] = (tl >= 0 && tl < p.V) ? p.zt[row] : 0.f;
+    }
+    return;
+  }
+  if (lane < p.k) {
+    if (p.topk_logprob) p.topk_logprob[(size_t)row * p.k + lane] = out_v - lse;
+    if (p.topk_index) p.topk_index[(size_t)row * p.k + lane] = out_i;
+  }
+  if (lane == 0) {
+    const int tgt = p.targets[row];
+    const bool valid = (tgt >= 0) && (tgt < p.V);
+    p.lse[row] = lse;
+    p.target_logprob[row] = valid ? (p.zt[row] - lse) : 0.f;   // the wide form serves single-rank runs only
+    p.entropy[row] = (float)(lnS - U / S);
+    p.conf[row] = lse - acc / (float)p.k;
+  }
+  // ---- small runs: the last CTA to finish does kernel 2's work (warp 0 of every CTA is still here)
+  if (p.tail_B > 0) {
+    __threadfence();
+    int last = 0;
+    if (lane == 0) last = (atomicAdd(p.tail_counter, 1u) == gridDim.x - 1) ? 1 : 0;
+    last = __shfl_sync(FULL, last, 0);
+    if (last) {
+      __threadfence();
+      __shared__ double s_prefix1[FIN_TAIL_MAX_T + 1];
+      fin_tail_reduce<1>(p, s_prefix1);
+      if (lane == 0) *p.tail_counter = 0u;
+    }
   }
 }
 

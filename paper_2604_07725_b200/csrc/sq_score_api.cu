@@ -35,6 +35,7 @@ struct sq_score_ctx {
   float* part_cs = nullptr; float* part_cu = nullptr;
   float* part_topv = nullptr; int32_t* part_topi = nullptr; float* zt = nullptr;
   unsigned int* gang_ctr = nullptr;
+  unsigned int* tail_counter = nullptr;   // CTAs of the finalize kernel that have finished (small runs; zero between runs)
   float* thr_pub = nullptr;   // [THR_MAX_CHUNKS][max_tokens] shared top-k bounds (sq_fused_kernel.cuh)
   // per-token scratch (used when the caller passes NULL per-token outputs)
   float* tok_lse = nullptr; float* tok_lp = nullptr; float* tok_ent = nullptr; float* tok_conf = nullptr;
@@ -163,19 +164,31 @@ static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, 
     for (int n = 1; n <= ng_hi; ++n) if (C % n == 0) ng = n;
     best = eval(ng, C / ng);
   } else {
-    // Gang size: 12 measured best on B200 at qwen3_8b / gpt_oss (swept 8 .. 36); sizes 10 .. 14 are within
-    // noise of one another, so the planner takes the one whose batches and stripes quantise best for this T.
-    const int g_lo = cfg->group_m > 0 ? cfg->group_m : 10, g_hi = cfg->group_m > 0 ? cfg->group_m : 14;
-    int last_ng = -1;
-    for (int pass = 0; pass < 2; ++pass)                 // pass 0: the preferred size first, so that ties keep it
-      for (int g = (pass == 0 ? (cfg->group_m > 0 ? g_lo : 12) : g_lo); g <= (pass == 0 ? (cfg->group_m > 0 ? g_hi : 12) : g_hi); ++g) {
+    // Gang size: 12 measured best on B200 at qwen3_8b / gpt_oss (swept 8 .. 36); neighbouring sizes are within
+    // noise of one another, so the planner takes the size in 8 .. 16 whose batches and stripes quantise best for this T,
+    // charging 1 % per step away from 12 (smaller gangs re-read W more often, larger ones keep more H strips in L2).
+    double best_adj = 1e300;
+    for (int dist = 0; dist <= (cfg->group_m > 0 ? 0 : 4); ++dist)
+      for (int sgn = -1; sgn <= 1; sgn += 2) {
+        if (dist == 0 && sgn > 0) continue;
+        const int g = cfg->group_m > 0 ? cfg->group_m : 12 + sgn * dist;
         const int G = std::max(1, std::min(g, std::min(M, NC)));
         const int ng = std::max(1, std::min(NC / G, gangs_max));
-        if (ng == last_ng) continue;
-        last_ng = ng;
         const Cand c = eval(ng, 1);
-        if (c.cost < best.cost * (1.0 - 1e-3)) best = c;   // a different size must win by more than noise
+        const double adj = c.cost * (1.0 + 0.01 * dist);
+        if (adj < best_adj * (1.0 - 1e-9)) { best_adj = adj; best = c; }
       }
+    // Few token tiles (decode-shaped runs: the gang size is capped by M and clusters are to spare): every gang streams
+    // its own stripe of W once and the run is HBM-bound, so all gangs should finish TOGETHER -- 594 tiles over 148 SMs
+    // is 146 x 4 + 2 x 5, and the two 5-tile SMs would stream their last tile alone at a single SM's bandwidth (measured
+    // +13 us on 197); 119 gangs x 5 tiles (118 x 5 + 4) finish together.  Take the fewest gangs with the same widest
+    // stripe (also fewer partial states to merge).
+    if (best.base == M && best.big == 0) {
+      const int widest = (int)cdiv64(NV, best.ng);
+      int ng = best.ng;
+      while (ng > 1 && (int)cdiv64(NV, ng - 1) == widest) --ng;
+      if (ng != best.ng) best = eval(ng, 1);
+    }
   }
   pl->num_gangs = best.ng;
   pl->gang_size = best.base;
@@ -236,7 +249,7 @@ static int64_t ws_rows_for(const sq_score_config& cfg) {
 extern "C" int sq_score_destroy(sq_score_ctx* ctx) {
   if (!ctx) return SQ_OK;
   cudaSetDevice(ctx->cfg.device);
-  void* bufs[] = {ctx->amax_bits, ctx->seq_done, ctx->thr_pub, ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
+  void* bufs[] = {ctx->tail_counter, ctx->amax_bits, ctx->seq_done, ctx->thr_pub, ctx->gang_ctr, ctx->part_cs, ctx->part_cu, ctx->part_m, ctx->part_s, ctx->part_u, ctx->part_topv, ctx->part_topi, ctx->zt,
                   ctx->tok_lse, ctx->tok_lp, ctx->tok_ent, ctx->tok_conf, ctx->tile_base, ctx->tile_seq, ctx->red_sum,
                   ctx->red_min, ctx->h_stage, ctx->tgt_stage, ctx->cu_stage, ctx->seq_stage, ctx->pos_base};
   int rc = SQ_OK;
@@ -354,6 +367,8 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   A(ws_alloc(ctx, &ctx->tok_conf, reduce_only ? 1 : T));
   A(ws_alloc(ctx, &ctx->tile_base, (int64_t)cfg->max_seqs + 1));
   A(ws_alloc(ctx, &ctx->amax_bits, 1));
+  A(ws_alloc(ctx, &ctx->tail_counter, 1));
+  if (rc == SQ_OK && cudaMemset(ctx->tail_counter, 0, sizeof(unsigned int)) != cudaSuccess) rc = SQ_ERR_CUDA;
   A(ws_alloc(ctx, &ctx->seq_done, (int64_t)cfg->max_seqs));
   if (rc == SQ_OK && cudaMemset(ctx->seq_done, 0, (size_t)cfg->max_seqs * sizeof(int)) != cudaSuccess) rc = SQ_ERR_CUDA;
   A(ws_alloc(ctx, &ctx->red_sum, ctx->red_tiles_max));
@@ -691,6 +706,13 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
     fin.chunks_per_rank = pl.num_chunks; fin.rank_stride = 0; fin.num_ranks = 1;
     fin.vocab_offset = vocab_offset;
+    // a small run (decode-shaped): kernel 2 would be pure launch latency, the finalize kernel's last CTA does its work
+    const bool tail = !shard_state && B > 0 && T <= sq::FIN_TAIL_MAX_T;
+    if (tail) {
+      fin.tail_B = B; fin.tail_window = window; fin.tail_cu = cu_seqlens; fin.tail_counter = ctx->tail_counter;
+      fin.tail_out_lp = o->seq_mean_logprob; fin.tail_out_ent = o->seq_mean_entropy; fin.tail_out_conf = o->seq_mean_conf;
+      fin.tail_out_min = o->seq_min_window_conf;
+    }
     const dim3 fgrid((unsigned)cdiv64(T, sq::FIN_WARPS)), fblock(sq::FIN_WARPS * 32);
     const dim3 fgrid8((unsigned)cdiv64(T, sq::FIN_WARPS * 4));   // 8 lanes per row: four rows per warp
     const bool lpr8 = pl.num_chunks <= 8 && !(ctx->debug_flags & 128);
@@ -702,16 +724,17 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     } else if (shard_state) {   // vocab-parallel shard: the merged state goes out in the packed exchange layout
       set_state_pointers(fin, shard_state, T, pl.topk_cap, /*as_output=*/true);
       if (pl.num_chunks <= 32) SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, true>, fgrid, fblock, 0, st, fin));
-      else SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<sq::FIN_MAX_NL, true>, fgrid, fblock, 0, st, fin));
+      else SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_wide_kernel<true>, dim3((unsigned)T), dim3(sq::FIN_WIDE_WARPS * 32), 0, st, fin));
     } else if (pl.num_chunks <= 32) {
       SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, false>, fgrid, fblock, 0, st, fin));
     } else {
-      SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<sq::FIN_MAX_NL, false>, fgrid, fblock, 0, st, fin));
+      SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_wide_kernel<false>, dim3((unsigned)T), dim3(sq::FIN_WIDE_WARPS * 32), 0, st, fin));
     }
     ctx->launches += 2;
     SQ_CUDA(ctx, cudaGetLastError());
     if (pev) cudaEventRecord(pev[2], st);
-    if (pev && B == 0) { cudaEventRecord(pev[3], st); ++ctx->ev_count; }   // no kernel 2 follows (shard runs, B = 0)
+    if (pev && (B == 0 || tail)) { cudaEventRecord(pev[3], st); ++ctx->ev_count; }   // no kernel 2 follows (shard runs, B = 0, small runs)
+    if (tail) return SQ_OK;
   }
   if (B > 0) {
     sq::ReduceParams rp = {};
