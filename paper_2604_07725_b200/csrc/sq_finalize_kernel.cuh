@@ -175,8 +175,8 @@ __device__ __forceinline__ void fin_merge_rows(const FinalizeParams& p) {
   // ---- top-k merge: the lane walks its chunks' descending lists; hv/hi[i] = head of list i, nv/ni[i] = the entry
   // behind it, loaded one pop ahead so that its latency hides behind the next round's shuffles
   int pos[NL];
-  float hv[NL], nv[NL];
-  int hi[NL], ni[NL];
+  float hv[NL] = {}, nv[NL] = {};
+  int hi[NL] = {}, ni[NL] = {};
   // raw load of list entry `at` (id < 0 = unfilled slot / past the end); the id is NOT examined here, so that the load
   // issued at a pop is a true prefetch: nothing waits for it until the entry becomes a head, one pop of the same list later
   auto load_at = [&](int i, int at, float& v, int& id) -> void {
