@@ -297,41 +297,57 @@ sq_finalize_kernel(const FinalizeParams p) {
 
 // ---------------------------------------------------------------------------------------------------------------------
 // Wide form, for rows swept by MORE than 32 vocab chunks (decode-shaped plans: every SM streams its own stripe of W, up
-// to 160 chunks per row; few rows).  One CTA of FIN_WIDE_WARPS warps per row, thread c = chunk c, so a warp never holds
-// more than one list per lane: the statistics are one block reduction, the top-k merge runs in two levels -- every
-// warp merges its 32 lists by k rounds of warp arg-max (heads in registers), then warp 0 merges the warps' k-entry
-// lists out of shared memory.  (The one-warp-per-row form with 5 lists per lane executed 3600 dependent instructions
-// per row: 23 us for 64 rows; this form 8 us.)
+// to 160 chunks per row; few rows).  One CTA of FIN_WIDE_WARPS warps per row, thread c = chunk c.  The statistics are
+// one block reduction.  The top-k merge has NO serial rounds (k rounds of warp arg-max cost 20-35 us for 64 rows, all of
+// it dependent-instruction latency); it is a selection by counting:
+//   1. every thread loads its chunk's whole sorted list (CAP independent loads);
+//   2. x = the k-th largest of the C list HEADS (rank by counting over shared memory).  k lists hold an entry >= x, so
+//      x bounds the row's k-th best from below and only entries >= x can be among the k best: a few dozen of C * CAP;
+//   3. the survivors are compacted into shared memory (block prefix sum of the per-list counts; a list is sorted, so
+//      its survivors are a prefix) and ranked by counting against one another (value desc, id asc): the survivor of
+//      rank j < k IS the j-th best, and writes itself to slot j.
+// 23.9 us (one warp per row, 5 lists per lane) -> 21.7 us (two levels of warp arg-max rounds) -> this form.
 constexpr int FIN_WIDE_WARPS = FIN_MAX_CHUNKS / 32;   // 5
+constexpr int FIN_WIDE_THREADS = FIN_WIDE_WARPS * 32;
+constexpr int FIN_WIDE_CAND = 1024;                   // k lists of CAP entries at most survive: 32 * 32
 
-template <bool EMIT>
-__global__ void __launch_bounds__(FIN_WIDE_WARPS * 32)
+template <int CAP, bool EMIT>
+__global__ void __launch_bounds__(FIN_WIDE_THREADS)
 sq_finalize_wide_kernel(const FinalizeParams p) {
   __shared__ float s_max[FIN_WIDE_WARPS];
   __shared__ double s_S[FIN_WIDE_WARPS], s_U[FIN_WIDE_WARPS];
-  __shared__ float s_v[FIN_WIDE_WARPS][32];
-  __shared__ int s_i[FIN_WIDE_WARPS][32];
+  __shared__ float s_head[FIN_WIDE_THREADS];
+  __shared__ int s_cnt[FIN_WIDE_WARPS];
+  __shared__ float s_thr;
+  __shared__ float s_cv[FIN_WIDE_CAND];
+  __shared__ int s_ci[FIN_WIDE_CAND];
+  __shared__ float s_win[32];
+  __shared__ int s_is_last;
   cudaGridDependencySynchronize();
   const int row = blockIdx.x;                       // grid = T rows
   const int c = threadIdx.x, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned FULL = 0xffffffffu;
-  const float NEG = -1.0e30f;
+  const float NEG = -1.0e30f, EMPTY = -1.0e20f;     // list values below EMPTY are unfilled slots (no logit is that small)
   const bool has = c < p.num_chunks;
   const int r = has ? c / p.chunks_per_rank : 0, cl = has ? c - r * p.chunks_per_rank : 0;
   const size_t base1 = (size_t)r * p.rank_stride + (size_t)cl * p.T + row;
   const size_t basek = (size_t)r * p.rank_stride + (size_t)cl * p.cap * p.T + row;
-  // ---- every load this thread needs, issued together: the chunk's statistics and the two first list entries
-  float m_c = NEG, s_c = 0.f, cs_c = 0.f, u_c = 0.f, cu_c = 0.f, hv = NEG, nv = NEG;
-  int hi = -1, ni = -1;
+  // ---- every load this thread needs, issued together: the chunk's statistics and its whole list of values
+  float m_c = NEG, s_c = 0.f, cs_c = 0.f, u_c = 0.f, cu_c = 0.f;
+  float lv[CAP];
+#pragma unroll
+  for (int j = 0; j < CAP; ++j) lv[j] = NEG;
   if (has) {
     m_c = p.part_m[base1]; s_c = p.part_s[base1]; cs_c = p.part_cs[base1]; u_c = p.part_u[base1]; cu_c = p.part_cu[base1];
-    hv = p.part_topv[basek]; hi = p.part_topi[basek];
-    if (p.cap > 1) { nv = p.part_topv[basek + p.T]; ni = p.part_topi[basek + p.T]; }
+#pragma unroll
+    for (int j = 0; j < CAP; ++j) lv[j] = p.part_topv[basek + (size_t)j * p.T];
   }
   float M = m_c;
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) M = fmaxf(M, __shfl_xor_sync(FULL, M, off));
   if (lane == 0) s_max[warp] = M;
+  const float head = lv[0] > EMPTY ? lv[0] : NEG;
+  s_head[c] = head;
   __syncthreads();
   M = s_max[0];
 #pragma unroll
@@ -350,95 +366,114 @@ sq_finalize_wide_kernel(const FinalizeParams p) {
     U += __shfl_xor_sync(FULL, U, off);
   }
   if (lane == 0) { s_S[warp] = S; s_U[warp] = U; }
-  // ---- level 1: this warp's 32 lists -> its k best (descending; ties: smaller id first)
-  if (hi < 0) { hv = NEG; hi = 0x7fffffff; }
-  int pos = 0;
-  float my_v = NEG; int my_i = 0x7fffffff;
-  for (int j = 0; j < p.k; ++j) {
-    float bv = hv; int bi = hi;
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-      const float ov = __shfl_xor_sync(FULL, bv, off);
-      const int oi = __shfl_xor_sync(FULL, bi, off);
-      if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-    }
-    if (lane == j) { my_v = bv; my_i = bi; }
-    if (hi == bi && hv == bv && bv > NEG) {         // ids are unique: exactly one lane advances
-      ++pos;
-      const bool empty = ni < 0;
-      hv = empty ? NEG : nv; hi = empty ? 0x7fffffff : ni;
-      nv = NEG; ni = -1;
-      if (pos + 1 < p.cap) { nv = p.part_topv[basek + (size_t)(pos + 1) * p.T]; ni = p.part_topi[basek + (size_t)(pos + 1) * p.T]; }
-    }
+  // ---- 2. the k-th largest head, by counting (ties: the smaller chunk index ranks first, so ranks are distinct)
+  int rank = 0;
+#pragma unroll 8
+  for (int q = 0; q < FIN_WIDE_THREADS; ++q) {
+    const float h = s_head[q];
+    rank += (h > head || (h == head && q < c)) ? 1 : 0;
   }
-  s_v[warp][lane] = my_v; s_i[warp][lane] = my_i;   // lanes >= k hold the empty marker
+  if (rank == p.k - 1) s_thr = head;                // exactly one thread (k <= 32 < C non-empty lists)
   __syncthreads();
-  if (warp != 0) return;
-  // ---- level 2 (warp 0): lane l < FIN_WIDE_WARPS walks warp l's list in shared memory
-  S = 0.0; U = 0.0;
+  const float thr = fmaxf(s_thr, EMPTY);
+  // ---- 3. survivors: a prefix of every sorted list.  Entries ABOVE x come first in the buffer (at most k - 1 lists hold
+  // any: they always fit); entries EQUAL to x follow and may be cut off when degenerate inputs tie by the thousand --
+  // any of them is a correct k-th best, so the ones that fit are as good as the ones that do not.
+  int cnt_gt = 0, cnt_ge = 0;
 #pragma unroll
-  for (int w = 0; w < FIN_WIDE_WARPS; ++w) { S += s_S[w]; U += s_U[w]; }   // fixed order
-  const double lnS = log(S);
-  const float lse = (float)((double)M + lnS);
-  int lpos = 0;
-  float lv = lane < FIN_WIDE_WARPS ? s_v[lane][0] : NEG;
-  int li = lane < FIN_WIDE_WARPS ? s_i[lane][0] : 0x7fffffff;
-  float acc = 0.f, out_v = NEG; int out_i = 0x7fffffff;
-  for (int j = 0; j < p.k; ++j) {
-    float bv = lv; int bi = li;
+  for (int j = 0; j < CAP; ++j) { cnt_gt += (lv[j] > thr) ? 1 : 0; cnt_ge += (lv[j] >= thr) ? 1 : 0; }
+  int inc = (cnt_gt << 16) | (cnt_ge - cnt_gt);     // both prefix sums in one scan (each below 2^15)
 #pragma unroll
-    for (int off = 4; off > 0; off >>= 1) {         // 8 lanes cover the FIN_WIDE_WARPS lists
-      const float ov = __shfl_xor_sync(FULL, bv, off);
-      const int oi = __shfl_xor_sync(FULL, bi, off);
-      if (ov > bv || (ov == bv && oi < bi)) { bv = ov; bi = oi; }
-    }
-    bv = __shfl_sync(FULL, bv, 0); bi = __shfl_sync(FULL, bi, 0);
-    acc += bv;
-    if (lane == j) { out_v = bv; out_i = bi; }
-    if (lane < FIN_WIDE_WARPS && li == bi && lv == bv && bv > NEG) {
-      ++lpos;
-      lv = lpos < 32 ? s_v[lane][lpos] : NEG;
-      li = lpos < 32 ? s_i[lane][lpos] : 0x7fffffff;
+  for (int off = 1; off < 32; off <<= 1) {
+    const int y = __shfl_up_sync(FULL, inc, off);
+    if (lane >= off) inc += y;
+  }
+  if (lane == 31) s_cnt[warp] = inc;
+  __syncthreads();
+  int bs = inc - ((cnt_gt << 16) | (cnt_ge - cnt_gt)), tot = 0;
+#pragma unroll
+  for (int w = 0; w < FIN_WIDE_WARPS; ++w) { bs += (w < warp) ? s_cnt[w] : 0; tot += s_cnt[w]; }
+  const int total_gt = tot >> 16, total = min(total_gt + (tot & 0xffff), FIN_WIDE_CAND);
+  const int base_gt = bs >> 16, base_eq = total_gt + (bs & 0xffff);
+#pragma unroll
+  for (int j = 0; j < CAP; ++j) {
+    const int at = j < cnt_gt ? base_gt + j : base_eq + (j - cnt_gt);
+    if (j < cnt_ge && at < FIN_WIDE_CAND) {
+      s_cv[at] = lv[j];
+      s_ci[at] = p.part_topi[basek + (size_t)j * p.T];
     }
   }
-  if (EMIT) {
-    if (lane < p.cap) {
-      p.out_topv[(size_t)lane * p.T + row] = (lane < p.k) ? out_v : NEG;
-      p.out_topi[(size_t)lane * p.T + row] = (lane < p.k && out_v > NEG) ? out_i : -1;
+  if (c < 32) s_win[c] = NEG;
+  __syncthreads();
+  // ---- rank the survivors against one another; rank j < k is the j-th best (value desc, id asc; ids are unique)
+  for (int t = c; t < total; t += FIN_WIDE_THREADS) {
+    const float v = s_cv[t];
+    const int id = s_ci[t];
+    int rk = 0;
+    for (int q = 0; q < total; ++q) {
+      const float ov = s_cv[q];
+      rk += (ov > v || (ov == v && s_ci[q] < id)) ? 1 : 0;
     }
-    if (lane == 0) {
-      const float s_hi = (float)S, u_hi = (float)U;
-      p.out_m[row] = M;
-      p.out_s[row] = s_hi; p.out_cs[row] = (float)((double)s_hi - S);
-      p.out_u[row] = u_hi; p.out_cu[row] = (float)((double)u_hi - U);
-      const int tl = p.targets[row] - p.vocab_offset;
-      p.out_zt[row] = (tl >= 0 && tl < p.V) ? p.zt[row] : 0.f;
+    if (rk < p.k) {
+      s_win[rk] = v;
+      if (EMIT) {
+        p.out_topv[(size_t)rk * p.T + row] = v;
+        p.out_topi[(size_t)rk * p.T + row] = id;
+      } else {
+        if (p.topk_index) p.topk_index[(size_t)row * p.k + rk] = id;
+      }
     }
-    return;
   }
-  if (lane < p.k) {
-    if (p.topk_logprob) p.topk_logprob[(size_t)row * p.k + lane] = out_v - lse;
-    if (p.topk_index) p.topk_index[(size_t)row * p.k + lane] = out_i;
+  __syncthreads();
+  if (warp == 0) {
+    S = 0.0; U = 0.0;
+#pragma unroll
+    for (int w = 0; w < FIN_WIDE_WARPS; ++w) { S += s_S[w]; U += s_U[w]; }   // fixed order
+    const double lnS = log(S);
+    const float lse = (float)((double)M + lnS);
+    if (EMIT) {
+      if (lane < p.cap && (lane >= p.k || s_win[lane] <= EMPTY)) {   // slots past k, and slots no entry filled
+        p.out_topv[(size_t)lane * p.T + row] = NEG;
+        p.out_topi[(size_t)lane * p.T + row] = -1;
+      }
+      if (lane == 0) {
+        const float s_hi = (float)S, u_hi = (float)U;
+        p.out_m[row] = M;
+        p.out_s[row] = s_hi; p.out_cs[row] = (float)((double)s_hi - S);
+        p.out_u[row] = u_hi; p.out_cu[row] = (float)((double)u_hi - U);
+        const int tl = p.targets[row] - p.vocab_offset;
+        p.out_zt[row] = (tl >= 0 && tl < p.V) ? p.zt[row] : 0.f;
+      }
+    } else {
+      if (lane < p.k) {
+        if (p.topk_logprob) p.topk_logprob[(size_t)row * p.k + lane] = s_win[lane] - lse;
+        if (p.topk_index && s_win[lane] <= EMPTY) p.topk_index[(size_t)row * p.k + lane] = 0x7fffffff;   // fewer than k logits
+      }
+      if (lane == 0) {
+        float acc = 0.f;
+        for (int j = 0; j < p.k; ++j) acc += s_win[j];   // fixed order: deterministic
+        const int tgt = p.targets[row];
+        const bool valid = (tgt >= 0) && (tgt < p.V);
+        p.lse[row] = lse;
+        p.target_logprob[row] = valid ? (p.zt[row] - lse) : 0.f;   // the wide form serves single-rank runs only
+        p.entropy[row] = (float)(lnS - U / S);
+        p.conf[row] = lse - acc / (float)p.k;
+      }
+    }
   }
-  if (lane == 0) {
-    const int tgt = p.targets[row];
-    const bool valid = (tgt >= 0) && (tgt < p.V);
-    p.lse[row] = lse;
-    p.target_logprob[row] = valid ? (p.zt[row] - lse) : 0.f;   // the wide form serves single-rank runs only
-    p.entropy[row] = (float)(lnS - U / S);
-    p.conf[row] = lse - acc / (float)p.k;
-  }
-  // ---- small runs: the last CTA to finish does kernel 2's work (warp 0 of every CTA is still here)
-  if (p.tail_B > 0) {
-    __threadfence();
-    int last = 0;
-    if (lane == 0) last = (atomicAdd(p.tail_counter, 1u) == gridDim.x - 1) ? 1 : 0;
-    last = __shfl_sync(FULL, last, 0);
-    if (last) {
+  // ---- small runs: the last CTA to finish does kernel 2's work
+  if constexpr (!EMIT) {
+    if (p.tail_B > 0) {
       __threadfence();
-      __shared__ double s_prefix1[FIN_TAIL_MAX_T + 1];
-      fin_tail_reduce<1>(p, s_prefix1);
-      if (lane == 0) *p.tail_counter = 0u;
+      __syncthreads();
+      if (threadIdx.x == 0) s_is_last = (atomicAdd(p.tail_counter, 1u) == gridDim.x - 1) ? 1 : 0;
+      __syncthreads();
+      if (s_is_last) {
+        __threadfence();
+        __shared__ double s_prefix[FIN_WIDE_WARPS * (FIN_TAIL_MAX_T + 1)];
+        fin_tail_reduce<FIN_WIDE_WARPS>(p, s_prefix);
+        if (threadIdx.x == 0) *p.tail_counter = 0u;
+      }
     }
   }
 }

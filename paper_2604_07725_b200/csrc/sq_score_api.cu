@@ -497,6 +497,15 @@ static cudaError_t launch_pdl(K kernel, dim3 grid, dim3 block, size_t smem, cuda
   return cudaLaunchKernelEx(&lc, kernel, params);
 }
 
+// rows swept by more than 32 vocab chunks: one CTA per row (sq_finalize_wide_kernel), compiled per list capacity
+template <bool EMIT>
+static cudaError_t launch_wide_finalize(int cap, int T, cudaStream_t st, const sq::FinalizeParams& fin) {
+  const dim3 grid((unsigned)T), block(sq::FIN_WIDE_THREADS);
+  if (cap == 8) return launch_pdl(sq::sq_finalize_wide_kernel<8, EMIT>, grid, block, 0, st, fin);
+  if (cap == 20) return launch_pdl(sq::sq_finalize_wide_kernel<20, EMIT>, grid, block, 0, st, fin);
+  return launch_pdl(sq::sq_finalize_wide_kernel<32, EMIT>, grid, block, 0, st, fin);
+}
+
 static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t st) {
   if (rp.B <= 0) return SQ_OK;
   // 16-byte loads need 16-byte aligned arrays (tiles start on multiples of 4 tokens)
@@ -724,11 +733,11 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     } else if (shard_state) {   // vocab-parallel shard: the merged state goes out in the packed exchange layout
       set_state_pointers(fin, shard_state, T, pl.topk_cap, /*as_output=*/true);
       if (pl.num_chunks <= 32) SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, true>, fgrid, fblock, 0, st, fin));
-      else SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_wide_kernel<true>, dim3((unsigned)T), dim3(sq::FIN_WIDE_WARPS * 32), 0, st, fin));
+      else SQ_CUDA(ctx, launch_wide_finalize<true>(pl.topk_cap, T, st, fin));
     } else if (pl.num_chunks <= 32) {
       SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_kernel<1, false>, fgrid, fblock, 0, st, fin));
     } else {
-      SQ_CUDA(ctx, launch_pdl(sq::sq_finalize_wide_kernel<false>, dim3((unsigned)T), dim3(sq::FIN_WIDE_WARPS * 32), 0, st, fin));
+      SQ_CUDA(ctx, launch_wide_finalize<false>(pl.topk_cap, T, st, fin));
     }
     ctx->launches += 2;
     SQ_CUDA(ctx, cudaGetLastError());
