@@ -312,3 +312,44 @@ def dequantize_fp8(codes: np.ndarray, scale: np.ndarray) -> torch.Tensor:
     v = e4m3_values()[codes]
     s = np.asarray(scale, dtype=np.float64)
     return torch.from_numpy(v * (s[0] if s.size == 1 else s[:, None]))
+
+
+# ------------------------------------------------------------------------------------------------
+# Next widening (block-scaled variant): MX-style e4m3 with one power-of-two scale per
+# block of 32 consecutive elements of a row (the format tcgen05.mma.kind::mxf8f6f4.block_scale consumes:
+# e4m3 elements, UE8M0 scales = 2^(code - 127)).  By definition, in exact arithmetic (reading #26):
+#   e_blk  = the smallest integer e with amax_blk <= 448 * 2^e   (no element saturates; amax = 0: e = -127)
+#   code   = the e4m3 value nearest to x / 2^e_blk (ties to the even mantissa)
+#   x     ~= e4m3_values()[code] * 2^e_blk
+# Scaling by a power of two is exact, so the CUDA path must reproduce codes and exponents bit for bit.
+# ------------------------------------------------------------------------------------------------
+MX_BLOCK = 32
+
+
+def quantize_mx(X: torch.Tensor):
+    """(codes uint8 [rows, d], exps int32 [rows, ceil(d / 32)]) -- see the definition above.  A ragged last block
+    (d % 32 != 0) is scaled by the maximum of the elements it has."""
+    x = widen(X).numpy()
+    rows, d = x.shape
+    nb = -(-d // MX_BLOCK)
+    xp = np.zeros((rows, nb * MX_BLOCK))
+    xp[:, :d] = x
+    blk = xp.reshape(rows, nb, MX_BLOCK)
+    amax = np.abs(blk).max(axis=2)
+    m, ex = np.frexp(amax / E4M3_MAX)              # amax / 448 = m * 2^ex, m in [0.5, 1): exact (a division by 7 * 2^6 ...
+    # ... is not exact in general, so decide by the exact comparison amax <= 448 * 2^e instead of trusting m)
+    e = ex.astype(np.int64)                        # candidate: 2^ex > amax / 448 always holds (m < 1)
+    ok_lower = amax <= E4M3_MAX * np.exp2((e - 1).astype(np.float64))   # 448 * 2^(e-1) is exact in fp64
+    e = np.where(ok_lower, e - 1, e)
+    e = np.where(amax > 0, np.clip(e, -127, 127), -127).astype(np.int32)
+    y = blk / np.exp2(e.astype(np.float64))[:, :, None]
+    codes = round_to_e4m3(y).reshape(rows, nb * MX_BLOCK)[:, :d]
+    return np.ascontiguousarray(codes), e
+
+
+def dequantize_mx(codes: np.ndarray, exps: np.ndarray) -> torch.Tensor:
+    """fp64 tensor e4m3_values()[code] * 2^exp of the element's block (exact)."""
+    v = e4m3_values()[codes]
+    rows, d = v.shape
+    s = np.repeat(np.exp2(exps.astype(np.float64)), MX_BLOCK, axis=1)[:, :d]
+    return torch.from_numpy(v * s)
