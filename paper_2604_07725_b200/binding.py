@@ -104,6 +104,8 @@ def lib() -> C.CDLL:
     L.sq_score_kernel_times.restype = C.c_int
     L.sq_score_launch_count.argtypes = [C.c_void_p]
     L.sq_score_launch_count.restype = C.c_int64
+    L.sq_score_reduce_form.argtypes = [C.c_void_p]
+    L.sq_score_reduce_form.restype = C.c_int
     L.sq_score_destroy.argtypes = [C.c_void_p]
     L.sq_score_destroy.restype = C.c_int
     L.sq_score_last_error.argtypes = [C.c_void_p]
@@ -371,6 +373,10 @@ class SqScore:
 
     def launch_count(self) -> int:
         return self._L.sq_score_launch_count(self._h)
+
+    def reduce_form(self) -> str:
+        """Form of kernel 2 the last call used (sq_score_reduce_form): 'fused', 'tiles', 'stream', 'tail' or 'none'."""
+        return ("none", "fused", "tiles", "stream", "tail")[self._L.sq_score_reduce_form(self._h)]
 
     def close(self):
         if getattr(self, "_h", None):

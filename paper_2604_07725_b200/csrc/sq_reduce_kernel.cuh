@@ -391,4 +391,311 @@ __global__ void __launch_bounds__(RED_THREADS) sq_reduce_fused_kernel(const Redu
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Streaming form (large inputs; window <= RS_WMAX; 16-byte aligned arrays): three launches, the first one tiny and
+// hidden under the second.
+//
+// The tile forms above cut tiles at sequence starts, so a CTA must know its sequence before it can load anything
+// (table lookup or search -> loads -> arithmetic, every step a dependent round trip through a saturated memory system),
+// and a CTA's lifetime is mostly latency.  Here CTA x owns the FIXED block [x * RS_TB, (x+1) * RS_TB) of the packed
+// arrays, whatever sequences lie in it, and nothing on its critical path depends on a search:
+//   index  : one warp per block finds the first sequence that reaches into the block (32-ary search over cu_seqlens,
+//            3 probes) and writes it with the next 33 boundaries to a table.  It triggers its dependent launch at once,
+//            so it runs underneath the first wave of the stream kernel.
+//   stream : 1. every thread issues all its 16-byte loads first (lp, ent, conf, targets of its 8 tokens + one vector of
+//               the look-ahead range [block end, block end + w)), then its two table entries (after the grid dependency
+//               wait, which only the first wave ever waits in): one round trip in total;
+//            2. exclusive prefix sums P of conf over the block + look-ahead: in registers (per vector, per warp by
+//               shuffles), one barrier for the 32 warp totals, then P goes to shared memory;
+//            3. window sums S(j) = P[j + w] - P[j] straight from shared memory (unit-stride lanes: conflict-free); the
+//               prefix restarts in every block, so fp32 error does not grow with the sequence;
+//            4. per (warp range of 256 tokens, sequence) piece: masked sums + minimum window sum by shuffles -> one
+//               record in slot (range index + sequence index), strictly increasing along the pieces: no atomics.
+//               A range that holds more sequences than the table lists walks cu_seqlens itself (search + batches).
+//   fold   : one warp per sequence folds the records of its ranges -- slots [r_first + b, r_last + b] -- in fixed
+//            order with fp64 accumulators; empty sequences get NaNs.  Sequences shorter than the window have one
+//            window, the whole sequence: min = mean conf.
+// The stream kernel reads lp / ent / conf BEFORE its grid dependency wait.  That is safe because its predecessor, the
+// index kernel, triggers only after its own wait, i.e. after whatever produced those arrays has completed and flushed.
+constexpr int RS_TB = 4096;         // tokens per CTA
+constexpr int RS_THREADS = 512;
+constexpr int RS_WARPS = RS_THREADS / 32;
+constexpr int RS_R = 256;           // tokens per warp = per record
+constexpr int RS_WMAX = 2048;       // widest window: the look-ahead is one 16-byte vector per thread
+constexpr int RS_IDX = 36;          // table row: first sequence, 34 boundaries cu[i0 .. i0+33] (clamped to cu[B]), pad
+
+__device__ __forceinline__ float4 rs_load4(const float* a, long long e, long long T) {
+  if (e + 4 <= T) return __ldg(reinterpret_cast<const float4*>(a + e));
+  float4 v;
+  v.x = e < T ? __ldg(a + e) : 0.f;         v.y = e + 1 < T ? __ldg(a + e + 1) : 0.f;
+  v.z = e + 2 < T ? __ldg(a + e + 2) : 0.f; v.w = e + 3 < T ? __ldg(a + e + 3) : 0.f;
+  return v;
+}
+__device__ __forceinline__ int4 rs_load4i(const int32_t* a, long long e, long long T) {
+  if (e + 4 <= T) return __ldg(reinterpret_cast<const int4*>(a + e));
+  int4 v;
+  v.x = e < T ? __ldg(a + e) : -1;         v.y = e + 1 < T ? __ldg(a + e + 1) : -1;
+  v.z = e + 2 < T ? __ldg(a + e + 2) : -1; v.w = e + 3 < T ? __ldg(a + e + 3) : -1;
+  return v;
+}
+// inclusive scan over the lanes of a warp
+__device__ __forceinline__ float rs_warp_incl(float x, int lane) {
+#pragma unroll
+  for (int off = 1; off < 32; off <<= 1) {
+    const float y = __shfl_up_sync(0xffffffffu, x, off);
+    if (lane >= off) x += y;
+  }
+  return x;
+}
+// the smallest b in [0, B) with cu[b+1] > pos (exists when pos < cu[B]); whole warp, 32 probes per round
+__device__ __forceinline__ int rs_first_seq(const int32_t* cu, int B, long long pos, int lane) {
+  int lo = 0, n = B;                                         // candidates [lo, lo + n)
+  while (n > 1) {
+    const int stride = (n + 31) >> 5;
+    const int probe = lo + min(n - 1, (lane + 1) * stride - 1);
+    const bool hit = (long long)__ldg(cu + probe + 1) > pos;
+    const unsigned m = __ballot_sync(0xffffffffu, hit);      // monotone in the lane; the last candidate always hits
+    const int f = __ffs(m) - 1;
+    const int nlo = lo + f * stride;
+    n = min(stride, lo + n - nlo);
+    lo = nlo;
+  }
+  return lo;
+}
+
+__global__ void __launch_bounds__(256) sq_reduce_stream_index_kernel(const ReduceParams p) {
+  cudaGridDependencySynchronize();
+  cudaTriggerProgrammaticLaunchCompletion();   // the stream kernel may start: it waits for this table only when it needs it
+  const int x = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  const long long pos = (long long)x * RS_TB;
+  if (pos >= p.T) return;
+  const int i0 = rs_first_seq(p.cu, p.B, pos, lane);
+  int* row = p.tile_seq + (size_t)x * RS_IDX;
+  if (lane == 0) row[0] = i0;
+  row[1 + lane] = __ldg(p.cu + min(i0 + lane, p.B));
+  if (lane < 2) row[33 + lane] = __ldg(p.cu + min(i0 + 32 + lane, p.B));
+}
+
+// minimum over the warp in one instruction (sm_100a: redux.sync on f32; the inputs are finite or +inf)
+__device__ __forceinline__ float rs_warp_min(float v) {
+  float r;
+  asm volatile("redux.sync.min.f32 %0, %1, 0xffffffff;" : "=f"(r) : "f"(v));
+  return r;
+}
+// Sums of four values over the warp in 6 shuffles instead of 20: lanes trade halves of the value set while they fold
+// (xor 16: keep two of four, xor 8: keep one of two, then three plain steps).  Returns the total of a in lanes 0..7,
+// of b in lanes 8..15, of c in lanes 16..23, of d in lanes 24..31.
+__device__ __forceinline__ float rs_warp_sum4(float a, float b, float c, float d, int lane) {
+  const bool hi = lane & 16;
+  const float k0 = hi ? c : a, k1 = hi ? d : b;              // kept
+  const float g0 = hi ? a : c, g1 = hi ? b : d;              // given away
+  const float x0 = k0 + __shfl_xor_sync(0xffffffffu, g0, 16);
+  const float x1 = k1 + __shfl_xor_sync(0xffffffffu, g1, 16);
+  const bool h8 = lane & 8;
+  float y = (h8 ? x1 : x0) + __shfl_xor_sync(0xffffffffu, h8 ? x0 : x1, 8);
+  y += __shfl_xor_sync(0xffffffffu, y, 4);
+  y += __shfl_xor_sync(0xffffffffu, y, 2);
+  y += __shfl_xor_sync(0xffffffffu, y, 1);
+  return y;
+}
+
+template <bool HAS_TG>
+__global__ void __launch_bounds__(RS_THREADS, 2) sq_reduce_stream_kernel(const ReduceParams p) {
+  __shared__ __align__(16) float s_P[RS_TB + RS_WMAX + 4];   // exclusive prefix of conf over block + look-ahead
+  __shared__ float s_tot[32];                                // totals: 16 warp ranges, then 16 look-ahead runs of 128
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long T = p.T;
+  const long long blk0 = (long long)blockIdx.x * RS_TB;
+  const long long rs = blk0 + warp * RS_R;                   // this warp's range [rs, re)
+  const int w = p.window;
+
+  // 1. every load first (see the note on the grid dependency above)
+  float4 vl[2], ve[2], vc[2];
+  int4 vt[2];
+  float4 la = make_float4(0.f, 0.f, 0.f, 0.f);
+  if (blk0 + RS_TB + RS_WMAX <= T) {                         // CTA-uniform: no vector crosses the end of the arrays
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const long long e = rs + k * 128 + 4 * lane;
+      vl[k] = __ldg(reinterpret_cast<const float4*>(p.lp + e));
+      ve[k] = __ldg(reinterpret_cast<const float4*>(p.ent + e));
+      vc[k] = __ldg(reinterpret_cast<const float4*>(p.conf + e));
+      if (HAS_TG) vt[k] = __ldg(reinterpret_cast<const int4*>(p.targets + e));
+    }
+    if (4 * (int)threadIdx.x < w) la = __ldg(reinterpret_cast<const float4*>(p.conf + blk0 + RS_TB + 4 * threadIdx.x));
+  } else {
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const long long e = rs + k * 128 + 4 * lane;
+      vl[k] = rs_load4(p.lp, e, T);
+      ve[k] = rs_load4(p.ent, e, T);
+      vc[k] = rs_load4(p.conf, e, T);
+      if (HAS_TG) vt[k] = rs_load4i(p.targets, e, T);
+    }
+    if (4 * (int)threadIdx.x < w) la = rs_load4(p.conf, blk0 + RS_TB + 4 * threadIdx.x, T);
+  }
+  cudaGridDependencySynchronize();
+  const int* row = p.tile_seq + (size_t)blockIdx.x * RS_IDX;
+  const int i0 = __ldcg(row);
+  int s0l = __ldcg(row + 1 + lane), s1l = __ldcg(row + 2 + lane);
+
+  // 2. prefix sums of conf: per vector, per warp, per block
+  const float t0 = (vc[0].x + vc[0].y) + (vc[0].z + vc[0].w);
+  const float t1 = (vc[1].x + vc[1].y) + (vc[1].z + vc[1].w);
+  float own_excl[2];
+  {
+    const float i0s = rs_warp_incl(t0, lane), i1s = rs_warp_incl(t1, lane);
+    const float half = __shfl_sync(0xffffffffu, i0s, 31);
+    own_excl[0] = i0s - t0;
+    own_excl[1] = half + (i1s - t1);
+    const float la_t = (la.x + la.y) + (la.z + la.w);
+    const float la_incl = rs_warp_incl(la_t, lane);
+    if (lane == 31) { s_tot[warp] = half + i1s; s_tot[RS_WARPS + warp] = la_incl; }
+    la.w = la_incl - la_t;                                   // la.w is not needed below: the slot carries the exclusive prefix
+  }
+  __syncthreads();
+  {
+    const float t = s_tot[lane];
+    const float ex = rs_warp_incl(t, lane) - t;
+    const float off_own = __shfl_sync(0xffffffffu, ex, warp);
+    const float off_la = __shfl_sync(0xffffffffu, ex, RS_WARPS + warp);
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const float b0 = off_own + own_excl[k];
+      float4 o;
+      o.x = b0; o.y = b0 + vc[k].x; o.z = o.y + vc[k].y; o.w = o.z + vc[k].z;
+      *reinterpret_cast<float4*>(s_P + warp * RS_R + k * 128 + 4 * lane) = o;
+    }
+    const float b0 = off_la + la.w;
+    float4 o;
+    o.x = b0; o.y = b0 + la.x; o.z = o.y + la.y; o.w = o.z + la.z;
+    *reinterpret_cast<float4*>(s_P + RS_TB + 4 * threadIdx.x) = o;
+  }
+  __syncthreads();
+  if (rs >= T) return;
+
+  // 3 + 4. the pieces of this range.  Lane l owns tokens rs + 4l .. + 3 and rs + 128 + 4l .. + 3 (as loaded).
+  const int rs_i = (int)rs, re_i = (int)min(rs + RS_R, T);
+  const int range = blockIdx.x * RS_WARPS + warp;
+  const float* Pl = s_P + (rs_i - (int)blk0) + 4 * lane;
+  // one batch: lane l holds sequence base + l = [s0b, s1b); returns the lanes whose sequence starts before the range ends
+  auto batch = [&](int base, int s0b, int s1b) -> unsigned {
+    const unsigned reach = __ballot_sync(0xffffffffu, s0b < re_i);      // a prefix of the lanes: cu is non-decreasing
+    unsigned pieces = reach & __ballot_sync(0xffffffffu, s1b > s0b && s1b > rs_i);   // non-empty and overlapping
+    while (pieces) {
+      const int src = __ffs(pieces) - 1;
+      pieces &= pieces - 1;
+      const int b = base + src;
+      const int s0 = __shfl_sync(0xffffffffu, s0b, src), s1 = __shfl_sync(0xffffffffu, s1b, src);
+      const int g0 = max(s0, rs_i), g1 = min(s1, re_i);
+      const int j1 = (s1 - s0 >= w) ? min(g1, s1 - w + 1) : g0;   // window starts of this piece: [g0, j1)
+      float a_lp, a_n, a_en, a_cf, mn = CUDART_INF_F;
+      if (g0 == rs_i && g1 == rs_i + RS_R) {                 // the range lies inside the sequence: no masks
+        a_en = ((ve[0].x + ve[0].y) + (ve[0].z + ve[0].w)) + ((ve[1].x + ve[1].y) + (ve[1].z + ve[1].w));
+        a_cf = t0 + t1;
+        if (HAS_TG) {
+          a_lp = 0.f; a_n = 0.f;
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            const bool k0 = (unsigned)vt[k].x < (unsigned)p.V, k1 = (unsigned)vt[k].y < (unsigned)p.V;
+            const bool k2 = (unsigned)vt[k].z < (unsigned)p.V, k3 = (unsigned)vt[k].w < (unsigned)p.V;
+            a_lp += ((k0 ? vl[k].x : 0.f) + (k1 ? vl[k].y : 0.f)) + ((k2 ? vl[k].z : 0.f) + (k3 ? vl[k].w : 0.f));
+            a_n += (float)((int)k0 + (int)k1 + (int)k2 + (int)k3);
+          }
+        } else {
+          a_lp = ((vl[0].x + vl[0].y) + (vl[0].z + vl[0].w)) + ((vl[1].x + vl[1].y) + (vl[1].z + vl[1].w));
+          a_n = 8.f;
+        }
+        if (j1 == g1 && (w & 3) == 0) {                      // every token starts a window; 16-byte shared loads line up
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            const float4 lo = *reinterpret_cast<const float4*>(Pl + 128 * k);
+            const float4 hi = *reinterpret_cast<const float4*>(Pl + 128 * k + w);
+            mn = fminf(mn, fminf(fminf(hi.x - lo.x, hi.y - lo.y), fminf(hi.z - lo.z, hi.w - lo.w)));
+          }
+        }
+      } else {
+        a_lp = 0.f; a_n = 0.f; a_en = 0.f; a_cf = 0.f;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          const int e = rs_i + k * 128 + 4 * lane;
+          const float xl[4] = {vl[k].x, vl[k].y, vl[k].z, vl[k].w};
+          const float xe[4] = {ve[k].x, ve[k].y, ve[k].z, ve[k].w};
+          const float xc[4] = {vc[k].x, vc[k].y, vc[k].z, vc[k].w};
+          const int xt[4] = {HAS_TG ? vt[k].x : 0, HAS_TG ? vt[k].y : 0, HAS_TG ? vt[k].z : 0, HAS_TG ? vt[k].w : 0};
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const bool in = (e + i >= g0 && e + i < g1);
+            const bool valid = in && (!HAS_TG || (unsigned)xt[i] < (unsigned)p.V);
+            a_en += in ? xe[i] : 0.f;
+            a_cf += in ? xc[i] : 0.f;
+            a_lp += valid ? xl[i] : 0.f;
+            a_n += valid ? 1.f : 0.f;
+          }
+        }
+      }
+      if (mn == CUDART_INF_F && j1 > g0) {                   // warp-uniform: the fast path above did not apply
+#pragma unroll
+        for (int k = 0; k < 2; ++k)
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int j = rs_i + k * 128 + 4 * lane + i;
+            if (j >= g0 && j < j1) mn = fminf(mn, Pl[128 * k + i + w] - Pl[128 * k + i]);
+          }
+      }
+      const float tot = rs_warp_sum4(a_lp, a_n, a_en, a_cf, lane);
+      mn = rs_warp_min(mn);
+      if ((lane & 7) == 0) reinterpret_cast<float*>(p.part_sum + range + b)[lane >> 3] = tot;
+      if (lane == 0) p.part_min[range + b] = mn;
+    }
+    return reach;
+  };
+  if (__ballot_sync(0xffffffffu, s0l < re_i) != 0xffffffffu) {
+    batch(i0, s0l, s1l);                                     // the table lists every sequence of this range
+  } else {
+    // more sequences than the table lists (33rd boundary still inside the range): walk cu_seqlens from the range's own start
+    for (int base = rs_first_seq(p.cu, p.B, rs, lane); base < p.B; base += 32) {
+      const int bl = base + lane;
+      s0l = bl < p.B ? __ldg(p.cu + bl) : 0x7fffffff;
+      s1l = bl < p.B ? __ldg(p.cu + bl + 1) : 0x7fffffff;
+      if (batch(base, s0l, s1l) != 0xffffffffu) break;       // the next sequence starts at or past the range's end
+    }
+  }
+}
+
+__global__ void __launch_bounds__(128) sq_reduce_stream_fold_kernel(const ReduceParams p) {
+  cudaGridDependencySynchronize();
+  const int b = blockIdx.x * 4 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (b >= p.B) return;
+  const int s0 = __ldg(p.cu + b), s1 = __ldg(p.cu + b + 1);
+  const int L = s1 - s0;
+  if (L <= 0) {
+    if (lane == 0) { const float nan = CUDART_NAN_F; p.out_lp[b] = nan; p.out_ent[b] = nan; p.out_conf[b] = nan; p.out_min[b] = nan; }
+    return;
+  }
+  const int t0 = s0 / RS_R + b, t1 = (s1 - 1) / RS_R + b + 1;
+  double s_lp = 0.0, s_n = 0.0, s_en = 0.0, s_cf = 0.0;
+  float best = CUDART_INF_F;
+  for (int t = t0 + lane; t < t1; t += 32) {
+    const float4 v = __ldcg(p.part_sum + t);
+    s_lp += v.x; s_n += v.y; s_en += v.z; s_cf += v.w;
+    best = fminf(best, __ldcg(p.part_min + t));
+  }
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) {
+    s_lp += __shfl_xor_sync(0xffffffffu, s_lp, off);
+    s_n += __shfl_xor_sync(0xffffffffu, s_n, off);
+    s_en += __shfl_xor_sync(0xffffffffu, s_en, off);
+    s_cf += __shfl_xor_sync(0xffffffffu, s_cf, off);
+    best = fminf(best, __shfl_xor_sync(0xffffffffu, best, off));
+  }
+  if (lane == 0) {
+    p.out_lp[b] = (s_n > 0.0) ? (float)(s_lp / s_n) : CUDART_NAN_F;
+    p.out_ent[b] = (float)(s_en / (double)L);
+    p.out_conf[b] = (float)(s_cf / (double)L);
+    p.out_min[b] = (L >= p.window) ? best / (float)p.window : (float)(s_cf / (double)L);
+  }
+}
+
 }  // namespace sq

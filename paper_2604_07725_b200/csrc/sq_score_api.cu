@@ -55,7 +55,7 @@ struct sq_score_ctx {
   void* encode_fn = nullptr;
   // optional per-kernel timing (sq_score_set_profiling): events around kernel 1, finalize
   // and kernel 2 of the last SQ_PROFILE_RING profiled runs
-  int profiling = 0; int debug_flags = 0;
+  int profiling = 0; int debug_flags = 0; int reduce_form = 0;
   int64_t ev_count = 0, ev_read = 0;   // runs recorded / runs already handed out by sq_score_profile_read
   cudaEvent_t (*ev)[4] = nullptr;      // [SQ_PROFILE_RING][4]
 #ifdef SQ_PROBES
@@ -237,6 +237,7 @@ extern "C" const char* sq_score_error_string(int code) {
 extern "C" const char* sq_score_last_error(const sq_score_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
 
 extern "C" int64_t sq_score_launch_count(const sq_score_ctx* ctx) { return ctx ? ctx->launches : 0; }
+extern "C" int sq_score_reduce_form(const sq_score_ctx* ctx) { return ctx ? ctx->reduce_form : 0; }
 
 // ------------------------------------------------------------------------------------------ create / destroy
 static int64_t ws_rows_for(const sq_score_config& cfg) {
@@ -323,7 +324,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   // SQ_SCORE_DEBUG selects between code paths that give the SAME results (tests force each of them): bit 3 = two-pass
   // prepare kernel, bit 4 = no shared top-k bound, bit 5 / 6 = three-launch / single-launch kernel 2, bit 7 = one warp
   // per row in the finalize kernel
-  if (const char* dbg = getenv("SQ_SCORE_DEBUG")) ctx->debug_flags = atoi(dbg) & (8 | 16 | 32 | 64 | 128);
+  if (const char* dbg = getenv("SQ_SCORE_DEBUG")) ctx->debug_flags = atoi(dbg) & (8 | 16 | 32 | 64 | 128 | 256);
 #ifdef SQ_PROBES
   if (const char* lim = getenv("SQ_SCORE_MAX_SMS"))   // probe: plan for fewer SMs
     if (atoi(lim) >= 2 && atoi(lim) < ctx->num_sms) ctx->num_sms = atoi(lim);
@@ -348,7 +349,9 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   const bool reduce_only = (cfg->flags & SQ_FLAG_REDUCE_ONLY) != 0;
   const int64_t rows = reduce_only ? 1 : ws_rows_for(*cfg);
   const int64_t T = cfg->max_tokens;
-  ctx->red_tiles_max = cdiv64(T, sq::RED_TILE) + 2 * (int64_t)cfg->max_seqs + 1;
+  // kernel 2's partial records: tile forms (one per 8192-token tile) or streaming form (one per 256-token range and sequence)
+  ctx->red_tiles_max = std::max<int64_t>(cdiv64(T, sq::RED_TILE) + 2 * (int64_t)cfg->max_seqs + 1,
+                                         cdiv64(T, sq::RS_TB) * sq::RS_IDX + (int64_t)cfg->max_seqs + 1);   // RS_IDX > RS_WARPS: tile_seq holds the index table
   int rc = SQ_OK;
   auto A = [&](int r) { if (rc == SQ_OK && r != SQ_OK) rc = r; };
   A(ws_alloc(ctx, &ctx->part_m, rows));
@@ -518,16 +521,31 @@ static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t s
   const size_t fused_smem = sq::RED_SMEM_BYTES + (size_t)(rp.B + 1) * sizeof(int);
   const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(6, (size_t)(220 * 1024) / (fused_smem + 1024)));
   const bool one_wave = tiles <= (int64_t)ctx->num_sms * per_sm && rp.B <= 2048;
-  if (rp.B <= sq::RED_FUSED_MAX_SEQS && !(ctx->debug_flags & 32) && (one_wave || (ctx->debug_flags & 64))) {
+  if (rp.B <= sq::RED_FUSED_MAX_SEQS && !(ctx->debug_flags & (32 | 256)) && (one_wave || (ctx->debug_flags & 64))) {
     rp.seq_done = ctx->seq_done;
     const size_t smem = fused_smem;
     const dim3 grid((unsigned)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)ctx->num_sms * per_sm)));
     if (rp.targets) SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_fused_kernel<true>, grid, dim3(sq::RED_THREADS), smem, st, rp));
     else SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_fused_kernel<false>, grid, dim3(sq::RED_THREADS), smem, st, rp));
     ctx->launches += 1;
+    ctx->reduce_form = SQ_REDUCE_FORM_FUSED;
     SQ_CUDA(ctx, cudaGetLastError());
     return SQ_OK;
   }
+  // Streaming form (three launches, the first hidden under the second; sq_reduce_kernel.cuh): fixed 4096-token blocks, loads issued before anything depends on
+  // cu_seqlens.  Needs 16-byte aligned arrays and window <= RS_WMAX; SQ_SCORE_DEBUG bit 8 forces it on small inputs (tests).
+  if (rp.vec && rp.window <= sq::RS_WMAX && rp.T > 0 && !(ctx->debug_flags & (32 | 64))) {
+    const dim3 grid((unsigned)cdiv64(rp.T, sq::RS_TB));
+    SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_index_kernel, dim3((grid.x + 7) / 8), dim3(256), 0, st, rp));
+    if (rp.targets) SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_kernel<true>, grid, dim3(sq::RS_THREADS), 0, st, rp));
+    else SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_kernel<false>, grid, dim3(sq::RS_THREADS), 0, st, rp));
+    SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_fold_kernel, dim3((unsigned)cdiv64(rp.B, 4)), dim3(128), 0, st, rp));
+    ctx->launches += 3;
+    ctx->reduce_form = SQ_REDUCE_FORM_STREAM;
+    SQ_CUDA(ctx, cudaGetLastError());
+    return SQ_OK;
+  }
+  ctx->reduce_form = SQ_REDUCE_FORM_TILES;
   SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_tile_scan_kernel, dim3(1), dim3(1024), 0, st, rp));
   ctx->launches += 1;
   if (rp.T > 0) {
@@ -743,7 +761,7 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     SQ_CUDA(ctx, cudaGetLastError());
     if (pev) cudaEventRecord(pev[2], st);
     if (pev && (B == 0 || tail)) { cudaEventRecord(pev[3], st); ++ctx->ev_count; }   // no kernel 2 follows (shard runs, B = 0, small runs)
-    if (tail) return SQ_OK;
+    if (tail) { ctx->reduce_form = SQ_REDUCE_FORM_TAIL; return SQ_OK; }
   }
   if (B > 0) {
     sq::ReduceParams rp = {};

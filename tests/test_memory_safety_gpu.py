@@ -171,7 +171,8 @@ def test_host_form_shard_merge_fp8_and_run_x_on_poisoned_workspace():
 
 
 @pytest.mark.parametrize("window", [1, 5, 2048, 8193])
-def test_reduce_alone_guarded_arrays_and_poisoned_workspace(window):
+@pytest.mark.parametrize("dbg", [None, "256"], ids=["default", "streaming"])
+def test_reduce_alone_guarded_arrays_and_poisoned_workspace(window, dbg):
     """Kernel 2 reads ahead of the current token (window look-ahead, 16-byte vectors): the per-token arrays end exactly
     where their guard band begins and have a length that is not a multiple of 4."""
     sq = _sq()
@@ -185,7 +186,13 @@ def test_reduce_alone_guarded_arrays_and_poisoned_workspace(window):
     # NaN guards right behind the arrays: a read past the end would poison the window sums
     for gd in G.values():
         gd.raw[GUARD + gd.n:].view(torch.float32)[:] = float("nan")
-    eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
+    import os
+    if dbg:
+        os.environ["SQ_SCORE_DEBUG"] = dbg                # bit 8: kernel 2's streaming form (fixed blocks, look-ahead past the block)
+    try:
+        eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
+    finally:
+        os.environ.pop("SQ_SCORE_DEBUG", None)
     eng.debug_fill_workspace(0xFF)
     out = eng.reduce(G["lp"].t, G["en"].t, G["cf"].t, cu.to(DEV), window)
     torch.cuda.synchronize()

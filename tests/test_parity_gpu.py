@@ -384,12 +384,14 @@ def test_full_size_config_sampled_rows_and_all_sequences(name):
 
 
 # ------------------------------------------------------------------------------------------ kernel 2 alone
-def _reduce_both_forms(sq, make_engine, call):
-    """Kernel 2 forced into its single-launch form (SQ_SCORE_DEBUG bit 6) and into its three-launch form (bit 5): the
-    two must agree bit for bit; returns the single-launch outputs."""
+def _reduce_all_forms(sq, make_engine, call, stream_form="stream"):
+    """Kernel 2 forced into its single-launch form (SQ_SCORE_DEBUG bit 6), its three-launch tile form (bit 5) and its
+    streaming form (bit 8; `stream_form` = "tiles" where the window is too wide for it and the tile form takes over).  The
+    two tile forms must agree bit for bit; returns (single-launch outputs, streaming outputs) -- the caller checks both
+    against the oracle."""
     import os
     outs = []
-    for dbg in ("64", "32"):
+    for dbg in ("64", "32", "256"):
         os.environ["SQ_SCORE_DEBUG"] = dbg
         try:
             eng = make_engine()
@@ -398,16 +400,17 @@ def _reduce_both_forms(sq, make_engine, call):
         n0 = eng.launch_count()
         o = call(eng)
         torch.cuda.synchronize()
-        assert eng.launch_count() - n0 == (1 if dbg == "64" else 3)
+        assert eng.launch_count() - n0 == {"64": 1, "32": 3, "256": 3}[dbg]
+        assert eng.reduce_form() == {"64": "fused", "32": "tiles", "256": stream_form}[dbg]
         outs.append({n: v.cpu().numpy() for n, v in o.items()})
-        o2 = call(eng)                                   # a second run on the same ctx: the per-sequence counters were reset
+        o2 = call(eng)                                   # a second run on the same ctx: nothing is left over from the first
         torch.cuda.synchronize()
         for n in o:
             np.testing.assert_array_equal(outs[-1][n], o2[n].cpu().numpy())
         eng.close()
     for n in outs[0]:
         np.testing.assert_array_equal(outs[0][n], outs[1][n])
-    return outs[0]
+    return outs[0], outs[2]
 
 
 @pytest.mark.parametrize("window", [1, 2, 3, 16, 511, 512, 513, 2048, 4096, 4097, 8191, 8192, 8193, 8195, 12290, 100000])
@@ -421,15 +424,18 @@ def test_reduce_kernel_alone(window):
     cf[30000:30040] = 0.5                      # a dip the minimum window must find
     dev = torch.device("cuda:0")
     a = [x.to(dev) for x in (lp, en, cf, cu)]
-    out = _reduce_both_forms(sq, lambda: sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True),
-                             lambda eng: eng.reduce(a[0], a[1], a[2], a[3], window))
+    out, out_s = _reduce_all_forms(sq, lambda: sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True),
+                                   lambda eng: eng.reduce(a[0], a[1], a[2], a[3], window),
+                                   stream_form="stream" if window <= 2048 else "tiles")
     ref = O.sequence_scores(lp.numpy(), en.numpy(), cf.numpy(), cu.numpy(), window)
     check_seqs(out, ref)
+    check_seqs(out_s, ref)
 
 
 @pytest.mark.parametrize("offset", [0, 1, 3])
 @pytest.mark.parametrize("with_targets", [False, True])
-def test_reduce_alignment_targets_and_array_end(offset, with_targets):
+@pytest.mark.parametrize("dbg", [None, "256"], ids=["default", "streaming"])
+def test_reduce_alignment_targets_and_array_end(offset, with_targets, dbg):
     """Kernel 2's 16-byte-load path against its scalar path: arrays that start `offset` floats into an allocation
     (unaligned -> scalar loads), a total length that is not a multiple of 4 (the last vector would cross the end of
     the arrays), sequences that start and end inside a block, windows with every residue mod 4, invalid targets."""
@@ -448,11 +454,18 @@ def test_reduce_alignment_targets_and_array_end(offset, with_targets):
         buf = torch.empty(T + 8, dtype=x.dtype, device=dev)
         buf[offset:offset + T] = x.to(dev)
         return buf[offset:offset + T]
-    eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
+    import os
+    if dbg:
+        os.environ["SQ_SCORE_DEBUG"] = dbg               # bit 8: the streaming form wherever it applies (aligned, window <= 2048)
+    try:
+        eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
+    finally:
+        os.environ.pop("SQ_SCORE_DEBUG", None)
     valid = ((tg >= 0) & (tg < 1000)).numpy() if with_targets else None
-    for window in (1, 6, 2047, 2048, 2049, 2050, 8192, 8195, 30000):
+    for window in (1, 6, 1023, 2047, 2048, 2049, 2050, 8192, 8195, 30000):
         out = eng.reduce(place(lp), place(en), place(cf), cu.to(dev), window, targets=place(tg) if with_targets else None)
         torch.cuda.synchronize()
+        assert eng.reduce_form() == (("stream" if offset == 0 and window <= 2048 else "tiles") if dbg else "fused")
         ref = O.sequence_scores(lp.numpy(), en.numpy(), cf.numpy(), cu.numpy(), window, target_valid=valid)
         check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
     eng.close()
@@ -463,23 +476,60 @@ def test_reduce_many_sequences():
     r = workloads.reduction_inputs(3000, 1, 3000, seed=5)
     dev = torch.device("cuda:0")
     a = [r[n].to(dev) for n in ("target_logprob", "entropy", "conf", "cu_seqlens")]
-    out = _reduce_both_forms(sq, lambda: sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True),
-                             lambda eng: eng.reduce(a[0], a[1], a[2], a[3], 256))
+    out, out_s = _reduce_all_forms(sq, lambda: sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True),
+                                   lambda eng: eng.reduce(a[0], a[1], a[2], a[3], 256))
     ref = O.sequence_scores(r["target_logprob"].numpy(), r["entropy"].numpy(), r["conf"].numpy(), r["cu_seqlens"].numpy(), 256)
     check_seqs(out, ref)
+    check_seqs(out_s, ref)
 
 
-def test_reduce_more_sequences_than_the_single_launch_form_holds():
-    """B = 13 000 > 12 287: the tile table no longer fits in shared memory and the three-launch form runs."""
+@pytest.mark.parametrize("dbg,form", [(None, "stream"), ("32", "tiles")], ids=["streaming", "three-launch"])
+def test_reduce_more_sequences_than_the_single_launch_form_holds(dbg, form):
+    """B = 13 000 > 12 287 short sequences (many per 256-token range, empty ones among them): more than one wave, so the
+    streaming form runs by default; forced off, the tile table no longer fits in shared memory and the three-launch form
+    runs."""
+    import os
     sq = _sq()
     r = workloads.reduction_inputs(13000, 0, 40, seed=6)
     dev = torch.device("cuda:0")
-    eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True)
+    if dbg:
+        os.environ["SQ_SCORE_DEBUG"] = dbg
+    try:
+        eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True)
+    finally:
+        os.environ.pop("SQ_SCORE_DEBUG", None)
     out = eng.reduce(r["target_logprob"].to(dev), r["entropy"].to(dev), r["conf"].to(dev), r["cu_seqlens"].to(dev), 7)
     torch.cuda.synchronize()
-    assert eng.launch_count() == 3
+    assert eng.launch_count() == 3 and eng.reduce_form() == form
     ref = O.sequence_scores(r["target_logprob"].numpy(), r["entropy"].numpy(), r["conf"].numpy(), r["cu_seqlens"].numpy(), 7)
     check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
+    eng.close()
+
+
+def test_reduce_streaming_form_many_sequences_per_range_and_one_long_sequence():
+    """The streaming form's piece walk: more than 32 sequences inside one 256-token range (two batches of the walk),
+    sequences that start exactly on range and block boundaries, empty sequences at position 0, in the middle and at the
+    end, one sequence that spans many blocks, windows of every kind (1, < 256, = range, > range, = RS_WMAX)."""
+    import os
+    sq = _sq()
+    lens = [0, 0] + [1] * 70 + [186, 256, 0, 512, 4096 - 1280 + 256, 0, 4096, 30011] + [3] * 40 + [2, 0, 0]
+    T = sum(lens)
+    g = torch.Generator().manual_seed(79)
+    cu = torch.tensor(np.concatenate([[0], np.cumsum(lens)]), dtype=torch.int32)
+    lp = -(torch.rand(T, generator=g) * 12); en = torch.rand(T, generator=g) * 11; cf = 3 + torch.rand(T, generator=g) * 12
+    cf[20000:20100] = 0.5
+    dev = torch.device("cuda:0")
+    os.environ["SQ_SCORE_DEBUG"] = "256"
+    try:
+        eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
+    finally:
+        os.environ.pop("SQ_SCORE_DEBUG", None)
+    for window in (1, 2, 100, 255, 256, 257, 1000, 2048):
+        out = eng.reduce(lp.to(dev), en.to(dev), cf.to(dev), cu.to(dev), window)
+        torch.cuda.synchronize()
+        assert eng.reduce_form() == "stream"
+        ref = O.sequence_scores(lp.numpy(), en.numpy(), cf.numpy(), cu.numpy(), window)
+        check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
     eng.close()
 
 
