@@ -392,46 +392,42 @@ __global__ void __launch_bounds__(RED_THREADS) sq_reduce_fused_kernel(const Redu
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// Streaming form (large inputs; window <= RS_WMAX; 16-byte aligned arrays): three launches, the first one tiny and
-// hidden under the second.
+// Streaming form (large inputs; window <= RS_WMAX; 16-byte aligned arrays): two launches.
 //
 // The tile forms above cut tiles at sequence starts, so a CTA must know its sequence before it can load anything
 // (table lookup or search -> loads -> arithmetic, every step a dependent round trip through a saturated memory system),
-// and a CTA's lifetime is mostly latency.  Here CTA x owns the FIXED block [x * RS_TB, (x+1) * RS_TB) of the packed
-// arrays, whatever sequences lie in it, and nothing on its critical path depends on a search:
-//   index  : one warp per block finds the first sequence that reaches into the block (32-ary search over cu_seqlens,
-//            3 probes) and writes it with the next 33 boundaries to a table.  It triggers its dependent launch at once,
-//            so it runs underneath the first wave of the stream kernel.
-//   stream : 1. every thread issues all its 16-byte loads first (lp, ent, conf, targets of its 8 tokens + one vector of
-//               the look-ahead range [block end, block end + w)), then its two table entries (after the grid dependency
-//               wait, which only the first wave ever waits in): one round trip in total;
-//            2. exclusive prefix sums P of conf over the block + look-ahead: in registers (per vector, per warp by
+// and a CTA's lifetime is mostly latency.  Here the streaming kernel does not look at cu_seqlens at all:
+//   stream : CTA x owns the FIXED block [x * RS_TB, (x+1) * RS_TB) of the packed arrays, warp q its 256-token range.
+//            1. every thread issues all its 16-byte loads at once (lp, ent, conf, targets of its 8 tokens + one vector
+//               of the look-ahead range [block end, block end + w)): one round trip;
+//            2. exclusive prefix sums P of conf over block + look-ahead: in registers (per vector, per warp by
 //               shuffles), one barrier for the 32 warp totals, then P goes to shared memory;
-//            3. window sums S(j) = P[j + w] - P[j] straight from shared memory (unit-stride lanes: conflict-free); the
-//               prefix restarts in every block, so fp32 error does not grow with the sequence;
-//            4. per (warp range of 256 tokens, sequence) piece: masked sums + minimum window sum by shuffles -> one
-//               record in slot (range index + sequence index), strictly increasing along the pieces: no atomics.
-//               A range that holds more sequences than the table lists walks cu_seqlens itself (search + batches).
-//   fold   : one warp per sequence folds the records of its ranges -- slots [r_first + b, r_last + b] -- in fixed
-//            order with fp64 accumulators; empty sequences get NaNs.  Sequences shorter than the window have one
-//            window, the whole sequence: min = mean conf.
-// The stream kernel reads lp / ent / conf BEFORE its grid dependency wait.  That is safe because its predecessor, the
-// index kernel, triggers only after its own wait, i.e. after whatever produced those arrays has completed and flushed.
+//            3. window sums S(j) = P[j + w] - P[j] straight from shared memory; the prefix restarts in every block, so
+//               fp32 error does not grow with the sequence;
+//            4. one record per range, whatever sequences it touches: the four sums over its 256 tokens, the minimum of
+//               S(j) over its 256 window starts, and S at its first token.
+//   fold   : one warp per sequence.  Ranges that lie inside the sequence contribute their records (sums; the minimum
+//            where all 256 windows end inside the sequence).  What is left is at most one ragged range at each end of
+//            the sequence and of its window starts: those tokens are read again (<= 512 per array and sequence, from
+//            L2), and the window sums of a ragged range are rebuilt from the range's recorded first sum by a scan of
+//            the differences c[m + w] - c[m].  fp64 accumulators, fixed order: deterministic.  Empty sequences get
+//            NaNs; a sequence shorter than the window has one window, itself: min = mean conf.
+// The prefix runs across sequence boundaries inside a block, so a non-finite conf value spoils the window sums of its
+// whole 4096-token block (the tile forms confine it to its sequence); c(i) of Eq. 3 is always finite.
 constexpr int RS_TB = 4096;         // tokens per CTA
 constexpr int RS_THREADS = 512;
 constexpr int RS_WARPS = RS_THREADS / 32;
 constexpr int RS_R = 256;           // tokens per warp = per record
 constexpr int RS_WMAX = 2048;       // widest window: the look-ahead is one 16-byte vector per thread
-constexpr int RS_IDX = 36;          // table row: first sequence, 34 boundaries cu[i0 .. i0+33] (clamped to cu[B]), pad
 
-__device__ __forceinline__ float4 rs_load4(const float* a, long long e, long long T) {
+__device__ __forceinline__ float4 rs_load4(const float* a, int e, int T) {   // elements at or past T read as 0
   if (e + 4 <= T) return __ldg(reinterpret_cast<const float4*>(a + e));
   float4 v;
   v.x = e < T ? __ldg(a + e) : 0.f;         v.y = e + 1 < T ? __ldg(a + e + 1) : 0.f;
   v.z = e + 2 < T ? __ldg(a + e + 2) : 0.f; v.w = e + 3 < T ? __ldg(a + e + 3) : 0.f;
   return v;
 }
-__device__ __forceinline__ int4 rs_load4i(const int32_t* a, long long e, long long T) {
+__device__ __forceinline__ int4 rs_load4i(const int32_t* a, int e, int T) {  // ... as -1
   if (e + 4 <= T) return __ldg(reinterpret_cast<const int4*>(a + e));
   int4 v;
   v.x = e < T ? __ldg(a + e) : -1;         v.y = e + 1 < T ? __ldg(a + e + 1) : -1;
@@ -447,35 +443,6 @@ __device__ __forceinline__ float rs_warp_incl(float x, int lane) {
   }
   return x;
 }
-// the smallest b in [0, B) with cu[b+1] > pos (exists when pos < cu[B]); whole warp, 32 probes per round
-__device__ __forceinline__ int rs_first_seq(const int32_t* cu, int B, long long pos, int lane) {
-  int lo = 0, n = B;                                         // candidates [lo, lo + n)
-  while (n > 1) {
-    const int stride = (n + 31) >> 5;
-    const int probe = lo + min(n - 1, (lane + 1) * stride - 1);
-    const bool hit = (long long)__ldg(cu + probe + 1) > pos;
-    const unsigned m = __ballot_sync(0xffffffffu, hit);      // monotone in the lane; the last candidate always hits
-    const int f = __ffs(m) - 1;
-    const int nlo = lo + f * stride;
-    n = min(stride, lo + n - nlo);
-    lo = nlo;
-  }
-  return lo;
-}
-
-__global__ void __launch_bounds__(256) sq_reduce_stream_index_kernel(const ReduceParams p) {
-  cudaGridDependencySynchronize();
-  cudaTriggerProgrammaticLaunchCompletion();   // the stream kernel may start: it waits for this table only when it needs it
-  const int x = blockIdx.x * 8 + (threadIdx.x >> 5), lane = threadIdx.x & 31;
-  const long long pos = (long long)x * RS_TB;
-  if (pos >= p.T) return;
-  const int i0 = rs_first_seq(p.cu, p.B, pos, lane);
-  int* row = p.tile_seq + (size_t)x * RS_IDX;
-  if (lane == 0) row[0] = i0;
-  row[1 + lane] = __ldg(p.cu + min(i0 + lane, p.B));
-  if (lane < 2) row[33 + lane] = __ldg(p.cu + min(i0 + 32 + lane, p.B));
-}
-
 // minimum over the warp in one instruction (sm_100a: redux.sync on f32; the inputs are finite or +inf)
 __device__ __forceinline__ float rs_warp_min(float v) {
   float r;
@@ -503,41 +470,39 @@ template <bool HAS_TG>
 __global__ void __launch_bounds__(RS_THREADS, 2) sq_reduce_stream_kernel(const ReduceParams p) {
   __shared__ __align__(16) float s_P[RS_TB + RS_WMAX + 4];   // exclusive prefix of conf over block + look-ahead
   __shared__ float s_tot[32];                                // totals: 16 warp ranges, then 16 look-ahead runs of 128
+  cudaGridDependencySynchronize();
+  cudaTriggerProgrammaticLaunchCompletion();                 // the fold kernel may start its record-independent part
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const long long T = p.T;
-  const long long blk0 = (long long)blockIdx.x * RS_TB;
-  const long long rs = blk0 + warp * RS_R;                   // this warp's range [rs, re)
+  const int T = (int)p.T;                                    // the host takes this form only when T + RS_TB + RS_WMAX fits an int
+  const int blk0 = blockIdx.x * RS_TB;
+  const int e0 = blk0 + warp * RS_R + 4 * lane;              // lane l owns tokens e0 .. + 3 and e0 + 128 .. + 3 of the warp's range
+  const int ela = blk0 + RS_TB + 4 * threadIdx.x;
   const int w = p.window;
+  const bool has_la = 4 * (int)threadIdx.x < w;
 
-  // 1. every load first (see the note on the grid dependency above)
+  // 1. every load first
   float4 vl[2], ve[2], vc[2];
   int4 vt[2];
   float4 la = make_float4(0.f, 0.f, 0.f, 0.f);
   if (blk0 + RS_TB + RS_WMAX <= T) {                         // CTA-uniform: no vector crosses the end of the arrays
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
-      const long long e = rs + k * 128 + 4 * lane;
-      vl[k] = __ldg(reinterpret_cast<const float4*>(p.lp + e));
-      ve[k] = __ldg(reinterpret_cast<const float4*>(p.ent + e));
-      vc[k] = __ldg(reinterpret_cast<const float4*>(p.conf + e));
-      if (HAS_TG) vt[k] = __ldg(reinterpret_cast<const int4*>(p.targets + e));
+      vl[k] = __ldg(reinterpret_cast<const float4*>(p.lp + e0 + 128 * k));
+      ve[k] = __ldg(reinterpret_cast<const float4*>(p.ent + e0 + 128 * k));
+      vc[k] = __ldg(reinterpret_cast<const float4*>(p.conf + e0 + 128 * k));
+      if (HAS_TG) vt[k] = __ldg(reinterpret_cast<const int4*>(p.targets + e0 + 128 * k));
     }
-    if (4 * (int)threadIdx.x < w) la = __ldg(reinterpret_cast<const float4*>(p.conf + blk0 + RS_TB + 4 * threadIdx.x));
+    if (has_la) la = __ldg(reinterpret_cast<const float4*>(p.conf + ela));
   } else {
 #pragma unroll
     for (int k = 0; k < 2; ++k) {
-      const long long e = rs + k * 128 + 4 * lane;
-      vl[k] = rs_load4(p.lp, e, T);
-      ve[k] = rs_load4(p.ent, e, T);
-      vc[k] = rs_load4(p.conf, e, T);
-      if (HAS_TG) vt[k] = rs_load4i(p.targets, e, T);
+      vl[k] = rs_load4(p.lp, e0 + 128 * k, T);
+      ve[k] = rs_load4(p.ent, e0 + 128 * k, T);
+      vc[k] = rs_load4(p.conf, e0 + 128 * k, T);
+      if (HAS_TG) vt[k] = rs_load4i(p.targets, e0 + 128 * k, T);
     }
-    if (4 * (int)threadIdx.x < w) la = rs_load4(p.conf, blk0 + RS_TB + 4 * threadIdx.x, T);
+    if (has_la) la = rs_load4(p.conf, ela, T);
   }
-  cudaGridDependencySynchronize();
-  const int* row = p.tile_seq + (size_t)blockIdx.x * RS_IDX;
-  const int i0 = __ldcg(row);
-  int s0l = __ldcg(row + 1 + lane), s1l = __ldcg(row + 2 + lane);
 
   // 2. prefix sums of conf: per vector, per warp, per block
   const float t0 = (vc[0].x + vc[0].y) + (vc[0].z + vc[0].w);
@@ -571,117 +536,145 @@ __global__ void __launch_bounds__(RS_THREADS, 2) sq_reduce_stream_kernel(const R
     o.x = b0; o.y = b0 + la.x; o.z = o.y + la.y; o.w = o.z + la.z;
     *reinterpret_cast<float4*>(s_P + RS_TB + 4 * threadIdx.x) = o;
   }
-  __syncthreads();
-  if (rs >= T) return;
-
-  // 3 + 4. the pieces of this range.  Lane l owns tokens rs + 4l .. + 3 and rs + 128 + 4l .. + 3 (as loaded).
-  const int rs_i = (int)rs, re_i = (int)min(rs + RS_R, T);
-  const int range = blockIdx.x * RS_WARPS + warp;
-  const float* Pl = s_P + (rs_i - (int)blk0) + 4 * lane;
-  // one batch: lane l holds sequence base + l = [s0b, s1b); returns the lanes whose sequence starts before the range ends
-  auto batch = [&](int base, int s0b, int s1b) -> unsigned {
-    const unsigned reach = __ballot_sync(0xffffffffu, s0b < re_i);      // a prefix of the lanes: cu is non-decreasing
-    unsigned pieces = reach & __ballot_sync(0xffffffffu, s1b > s0b && s1b > rs_i);   // non-empty and overlapping
-    while (pieces) {
-      const int src = __ffs(pieces) - 1;
-      pieces &= pieces - 1;
-      const int b = base + src;
-      const int s0 = __shfl_sync(0xffffffffu, s0b, src), s1 = __shfl_sync(0xffffffffu, s1b, src);
-      const int g0 = max(s0, rs_i), g1 = min(s1, re_i);
-      const int j1 = (s1 - s0 >= w) ? min(g1, s1 - w + 1) : g0;   // window starts of this piece: [g0, j1)
-      float a_lp, a_n, a_en, a_cf, mn = CUDART_INF_F;
-      if (g0 == rs_i && g1 == rs_i + RS_R) {                 // the range lies inside the sequence: no masks
-        a_en = ((ve[0].x + ve[0].y) + (ve[0].z + ve[0].w)) + ((ve[1].x + ve[1].y) + (ve[1].z + ve[1].w));
-        a_cf = t0 + t1;
-        if (HAS_TG) {
-          a_lp = 0.f; a_n = 0.f;
+  // the lane's sums, while the barrier fills
+  const float a_en = ((ve[0].x + ve[0].y) + (ve[0].z + ve[0].w)) + ((ve[1].x + ve[1].y) + (ve[1].z + ve[1].w));
+  float a_lp, a_n;
+  if (HAS_TG) {
+    a_lp = 0.f; a_n = 0.f;
 #pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            const bool k0 = (unsigned)vt[k].x < (unsigned)p.V, k1 = (unsigned)vt[k].y < (unsigned)p.V;
-            const bool k2 = (unsigned)vt[k].z < (unsigned)p.V, k3 = (unsigned)vt[k].w < (unsigned)p.V;
-            a_lp += ((k0 ? vl[k].x : 0.f) + (k1 ? vl[k].y : 0.f)) + ((k2 ? vl[k].z : 0.f) + (k3 ? vl[k].w : 0.f));
-            a_n += (float)((int)k0 + (int)k1 + (int)k2 + (int)k3);
-          }
-        } else {
-          a_lp = ((vl[0].x + vl[0].y) + (vl[0].z + vl[0].w)) + ((vl[1].x + vl[1].y) + (vl[1].z + vl[1].w));
-          a_n = 8.f;
-        }
-        if (j1 == g1 && (w & 3) == 0) {                      // every token starts a window; 16-byte shared loads line up
-#pragma unroll
-          for (int k = 0; k < 2; ++k) {
-            const float4 lo = *reinterpret_cast<const float4*>(Pl + 128 * k);
-            const float4 hi = *reinterpret_cast<const float4*>(Pl + 128 * k + w);
-            mn = fminf(mn, fminf(fminf(hi.x - lo.x, hi.y - lo.y), fminf(hi.z - lo.z, hi.w - lo.w)));
-          }
-        }
-      } else {
-        a_lp = 0.f; a_n = 0.f; a_en = 0.f; a_cf = 0.f;
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-          const int e = rs_i + k * 128 + 4 * lane;
-          const float xl[4] = {vl[k].x, vl[k].y, vl[k].z, vl[k].w};
-          const float xe[4] = {ve[k].x, ve[k].y, ve[k].z, ve[k].w};
-          const float xc[4] = {vc[k].x, vc[k].y, vc[k].z, vc[k].w};
-          const int xt[4] = {HAS_TG ? vt[k].x : 0, HAS_TG ? vt[k].y : 0, HAS_TG ? vt[k].z : 0, HAS_TG ? vt[k].w : 0};
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const bool in = (e + i >= g0 && e + i < g1);
-            const bool valid = in && (!HAS_TG || (unsigned)xt[i] < (unsigned)p.V);
-            a_en += in ? xe[i] : 0.f;
-            a_cf += in ? xc[i] : 0.f;
-            a_lp += valid ? xl[i] : 0.f;
-            a_n += valid ? 1.f : 0.f;
-          }
-        }
-      }
-      if (mn == CUDART_INF_F && j1 > g0) {                   // warp-uniform: the fast path above did not apply
-#pragma unroll
-        for (int k = 0; k < 2; ++k)
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int j = rs_i + k * 128 + 4 * lane + i;
-            if (j >= g0 && j < j1) mn = fminf(mn, Pl[128 * k + i + w] - Pl[128 * k + i]);
-          }
-      }
-      const float tot = rs_warp_sum4(a_lp, a_n, a_en, a_cf, lane);
-      mn = rs_warp_min(mn);
-      if ((lane & 7) == 0) reinterpret_cast<float*>(p.part_sum + range + b)[lane >> 3] = tot;
-      if (lane == 0) p.part_min[range + b] = mn;
+    for (int k = 0; k < 2; ++k) {
+      const bool k0 = (unsigned)vt[k].x < (unsigned)p.V, k1 = (unsigned)vt[k].y < (unsigned)p.V;
+      const bool k2 = (unsigned)vt[k].z < (unsigned)p.V, k3 = (unsigned)vt[k].w < (unsigned)p.V;
+      a_lp += ((k0 ? vl[k].x : 0.f) + (k1 ? vl[k].y : 0.f)) + ((k2 ? vl[k].z : 0.f) + (k3 ? vl[k].w : 0.f));
+      a_n += (float)((int)k0 + (int)k1 + (int)k2 + (int)k3);
     }
-    return reach;
-  };
-  if (__ballot_sync(0xffffffffu, s0l < re_i) != 0xffffffffu) {
-    batch(i0, s0l, s1l);                                     // the table lists every sequence of this range
   } else {
-    // more sequences than the table lists (33rd boundary still inside the range): walk cu_seqlens from the range's own start
-    for (int base = rs_first_seq(p.cu, p.B, rs, lane); base < p.B; base += 32) {
-      const int bl = base + lane;
-      s0l = bl < p.B ? __ldg(p.cu + bl) : 0x7fffffff;
-      s1l = bl < p.B ? __ldg(p.cu + bl + 1) : 0x7fffffff;
-      if (batch(base, s0l, s1l) != 0xffffffffu) break;       // the next sequence starts at or past the range's end
-    }
+    a_lp = ((vl[0].x + vl[0].y) + (vl[0].z + vl[0].w)) + ((vl[1].x + vl[1].y) + (vl[1].z + vl[1].w));
+    a_n = 8.f;
   }
+  const float tot = rs_warp_sum4(a_lp, a_n, a_en, t0 + t1, lane);
+  __syncthreads();
+
+  // 3. the 256 window sums that start in this range
+  const float* Pl = s_P + warp * RS_R + 4 * lane;
+  float mn = CUDART_INF_F, s_first = 0.f;
+  if ((w & 3) == 0) {                                        // 16-byte shared loads line up
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const float4 lo = *reinterpret_cast<const float4*>(Pl + 128 * k);
+      const float4 hi = *reinterpret_cast<const float4*>(Pl + 128 * k + w);
+      if (k == 0) s_first = hi.x - lo.x;
+      mn = fminf(mn, fminf(fminf(hi.x - lo.x, hi.y - lo.y), fminf(hi.z - lo.z, hi.w - lo.w)));
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < 2; ++k)
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const float sj = Pl[128 * k + i + w] - Pl[128 * k + i];
+        if (k == 0 && i == 0) s_first = sj;
+        mn = fminf(mn, sj);
+      }
+  }
+  mn = rs_warp_min(mn);
+  // 4. the record of this range
+  const int range = blockIdx.x * RS_WARPS + warp;
+  if ((lane & 7) == 0) reinterpret_cast<float*>(p.part_sum + range)[lane >> 3] = tot;
+  if (lane == 0) reinterpret_cast<float2*>(p.part_min)[range] = make_float2(mn, s_first);
 }
 
+// Window sums of a ragged range r (tokens [256 r, 256 r + 256)) are rebuilt from its recorded first sum S(256 r):
+// S(j + 1) = S(j) + c[j + w] - c[j].  Lane l rebuilds the starts 256 r + 8l .. + 7; only starts in [lo, hi) count.
+struct RsRagged {
+  float d[8];     // d[i] = S(m0 + i + 1) - S(m0 + i)
+  float excl;     // S(m0) - S(256 r)
+  int m0, lo, hi; // lo >= hi: nothing to do
+};
+__device__ __forceinline__ void rs_ragged_load(RsRagged& g, const ReduceParams& p, int r, int lo, int hi, int w, int lane) {
+  g.m0 = r * RS_R + 8 * lane; g.lo = lo; g.hi = hi;
+  float run = 0.f;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {                              // only differences below the last start matter
+    const int m = g.m0 + i;
+    g.d[i] = (m + 1 < hi) ? __ldg(p.conf + m + w) - __ldg(p.conf + m) : 0.f;   // m + w < hi + w - 1 <= s1 - 1: inside the arrays
+    run += g.d[i];
+  }
+  g.excl = rs_warp_incl(run, lane) - run;
+}
+__device__ __forceinline__ float rs_ragged_min(const RsRagged& g, float s_range_first) {
+  float s = s_range_first + g.excl, best = CUDART_INF_F;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    if (g.m0 + i >= g.lo && g.m0 + i < g.hi) best = fminf(best, s);
+    s += g.d[i];
+  }
+  return best;
+}
+
+// One warp per sequence.  Everything that does not depend on the stream kernel's records -- cu_seqlens, the ragged
+// ends of the sequence, the differences of the ragged window ranges -- is read BEFORE the grid dependency wait, i.e.
+// underneath the stream kernel's last wave (the stream kernel triggers this launch early; it does so after its own
+// dependency wait, so whatever produced lp / ent / conf has completed by the time this kernel can start).
 __global__ void __launch_bounds__(128) sq_reduce_stream_fold_kernel(const ReduceParams p) {
-  cudaGridDependencySynchronize();
   const int b = blockIdx.x * 4 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   if (b >= p.B) return;
   const int s0 = __ldg(p.cu + b), s1 = __ldg(p.cu + b + 1);
-  const int L = s1 - s0;
+  const int L = s1 - s0, w = p.window;
   if (L <= 0) {
     if (lane == 0) { const float nan = CUDART_NAN_F; p.out_lp[b] = nan; p.out_ent[b] = nan; p.out_conf[b] = nan; p.out_min[b] = nan; }
     return;
   }
-  const int t0 = s0 / RS_R + b, t1 = (s1 - 1) / RS_R + b + 1;
+  // sums: the ranges [r_a, r_b) lie inside the sequence; what is left of it are the tokens [s0, h1) and [t0, s1)
+  const int r_a = (s0 + RS_R - 1) / RS_R, r_b = s1 / RS_R;
+  const int h1 = r_a < r_b ? r_a * RS_R : s1, t0 = r_a < r_b ? r_b * RS_R : s1;
   double s_lp = 0.0, s_n = 0.0, s_en = 0.0, s_cf = 0.0;
-  float best = CUDART_INF_F;
-  for (int t = t0 + lane; t < t1; t += 32) {
-    const float4 v = __ldcg(p.part_sum + t);
+  // the ragged ends, at most 255 tokens each (511 when no range lies inside the sequence): every load of a pass at once
+  auto raw = [&](int e_lo, int e_hi) {
+    for (int base = e_lo; base < e_hi; base += 256) {
+      float xl[8], xe[8], xc[8];
+      int xt[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const int e = base + lane + 32 * i;
+        const bool in = e < e_hi;
+        xl[i] = in ? __ldg(p.lp + e) : 0.f;
+        xe[i] = in ? __ldg(p.ent + e) : 0.f;
+        xc[i] = in ? __ldg(p.conf + e) : 0.f;
+        xt[i] = in ? (p.targets ? __ldg(p.targets + e) : 0) : -1;
+      }
+      float f_lp = 0.f, f_n = 0.f, f_en = 0.f, f_cf = 0.f;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        const bool valid = (unsigned)xt[i] < (unsigned)p.V;
+        f_lp += valid ? xl[i] : 0.f;
+        f_n += valid ? 1.f : 0.f;
+        f_en += xe[i];
+        f_cf += xc[i];
+      }
+      s_lp += f_lp; s_n += f_n; s_en += f_en; s_cf += f_cf;
+    }
+  };
+  raw(s0, h1);
+  raw(t0, s1);
+  // window starts [s0, jl]: the ranges [r_a, r_c) hold only valid starts; a ragged range at each end
+  const int jl = s1 - w;
+  const int r_c = (L >= w) ? (jl + 1) / RS_R : r_a;
+  const int r_t = max(r_c, r_a);
+  RsRagged gh, gt;
+  gh.lo = gh.hi = gt.lo = gt.hi = 0;
+  if (L >= w && (s0 % RS_R)) rs_ragged_load(gh, p, s0 / RS_R, s0, min(jl + 1, r_a * RS_R), w, lane);
+  if (L >= w && r_t * RS_R <= jl) rs_ragged_load(gt, p, r_t, r_t * RS_R, jl + 1, w, lane);
+
+  cudaGridDependencySynchronize();                           // the records
+  for (int r = r_a + lane; r < r_b; r += 32) {
+    const float4 v = __ldcg(p.part_sum + r);
     s_lp += v.x; s_n += v.y; s_en += v.z; s_cf += v.w;
-    best = fminf(best, __ldcg(p.part_min + t));
   }
+  float best = CUDART_INF_F;
+  for (int r = r_a + lane; r < r_c; r += 32) best = fminf(best, __ldcg(p.part_min + 2 * r));
+  if (gh.lo < gh.hi) best = fminf(best, rs_ragged_min(gh, __ldcg(p.part_min + 2 * (s0 / RS_R) + 1)));
+  if (gt.lo < gt.hi) best = fminf(best, rs_ragged_min(gt, __ldcg(p.part_min + 2 * r_t + 1)));
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {
     s_lp += __shfl_xor_sync(0xffffffffu, s_lp, off);
@@ -694,7 +687,7 @@ __global__ void __launch_bounds__(128) sq_reduce_stream_fold_kernel(const Reduce
     p.out_lp[b] = (s_n > 0.0) ? (float)(s_lp / s_n) : CUDART_NAN_F;
     p.out_ent[b] = (float)(s_en / (double)L);
     p.out_conf[b] = (float)(s_cf / (double)L);
-    p.out_min[b] = (L >= p.window) ? best / (float)p.window : (float)(s_cf / (double)L);
+    p.out_min[b] = (L >= w) ? best / (float)w : (float)(s_cf / (double)L);
   }
 }
 

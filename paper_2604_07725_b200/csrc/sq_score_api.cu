@@ -351,7 +351,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   const int64_t T = cfg->max_tokens;
   // kernel 2's partial records: tile forms (one per 8192-token tile) or streaming form (one per 256-token range and sequence)
   ctx->red_tiles_max = std::max<int64_t>(cdiv64(T, sq::RED_TILE) + 2 * (int64_t)cfg->max_seqs + 1,
-                                         cdiv64(T, sq::RS_TB) * sq::RS_IDX + (int64_t)cfg->max_seqs + 1);   // RS_IDX > RS_WARPS: tile_seq holds the index table
+                                         2 * cdiv64(T, sq::RS_TB) * sq::RS_WARPS + 2);   // (red_min: two floats per range)
   int rc = SQ_OK;
   auto A = [&](int r) { if (rc == SQ_OK && r != SQ_OK) rc = r; };
   A(ws_alloc(ctx, &ctx->part_m, rows));
@@ -532,15 +532,16 @@ static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t s
     SQ_CUDA(ctx, cudaGetLastError());
     return SQ_OK;
   }
-  // Streaming form (three launches, the first hidden under the second; sq_reduce_kernel.cuh): fixed 4096-token blocks, loads issued before anything depends on
-  // cu_seqlens.  Needs 16-byte aligned arrays and window <= RS_WMAX; SQ_SCORE_DEBUG bit 8 forces it on small inputs (tests).
-  if (rp.vec && rp.window <= sq::RS_WMAX && rp.T > 0 && !(ctx->debug_flags & (32 | 64))) {
+  // Streaming form (two launches, sq_reduce_kernel.cuh): fixed 4096-token blocks whose loads depend on nothing, every
+  // sequence boundary handled in the fold.  Needs 16-byte aligned arrays and window <= RS_WMAX; SQ_SCORE_DEBUG bit 8 forces
+  // it on small inputs (tests).
+  if (rp.vec && rp.window <= sq::RS_WMAX && rp.T > 0 && rp.T <= (int64_t)INT32_MAX - 2 * (sq::RS_TB + sq::RS_WMAX) &&
+      !(ctx->debug_flags & (32 | 64))) {
     const dim3 grid((unsigned)cdiv64(rp.T, sq::RS_TB));
-    SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_index_kernel, dim3((grid.x + 7) / 8), dim3(256), 0, st, rp));
     if (rp.targets) SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_kernel<true>, grid, dim3(sq::RS_THREADS), 0, st, rp));
     else SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_kernel<false>, grid, dim3(sq::RS_THREADS), 0, st, rp));
     SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_fold_kernel, dim3((unsigned)cdiv64(rp.B, 4)), dim3(128), 0, st, rp));
-    ctx->launches += 3;
+    ctx->launches += 2;
     ctx->reduce_form = SQ_REDUCE_FORM_STREAM;
     SQ_CUDA(ctx, cudaGetLastError());
     return SQ_OK;

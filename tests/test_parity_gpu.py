@@ -400,7 +400,7 @@ def _reduce_all_forms(sq, make_engine, call, stream_form="stream"):
         n0 = eng.launch_count()
         o = call(eng)
         torch.cuda.synchronize()
-        assert eng.launch_count() - n0 == {"64": 1, "32": 3, "256": 3}[dbg]
+        assert eng.launch_count() - n0 == {"64": 1, "32": 3, "256": 2 if stream_form == "stream" else 3}[dbg]
         assert eng.reduce_form() == {"64": "fused", "32": "tiles", "256": stream_form}[dbg]
         outs.append({n: v.cpu().numpy() for n, v in o.items()})
         o2 = call(eng)                                   # a second run on the same ctx: nothing is left over from the first
@@ -500,7 +500,7 @@ def test_reduce_more_sequences_than_the_single_launch_form_holds(dbg, form):
         os.environ.pop("SQ_SCORE_DEBUG", None)
     out = eng.reduce(r["target_logprob"].to(dev), r["entropy"].to(dev), r["conf"].to(dev), r["cu_seqlens"].to(dev), 7)
     torch.cuda.synchronize()
-    assert eng.launch_count() == 3 and eng.reduce_form() == form
+    assert eng.launch_count() == (2 if form == "stream" else 3) and eng.reduce_form() == form
     ref = O.sequence_scores(r["target_logprob"].numpy(), r["entropy"].numpy(), r["conf"].numpy(), r["cu_seqlens"].numpy(), 7)
     check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
     eng.close()
