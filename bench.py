@@ -394,7 +394,8 @@ def run_ours(args):
                                      "unit": "GB/s", "frac": r_bytes / (r_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
                                      "ms": r_ms, "tokens": r["T"], "seqs": r["B"], "window": wl.window,
                                      "algorithmic_bytes": r_bytes,
-                                     "note": "3 launches (tile_scan, tile_part, seq_final) at this size; 12 B/token read + 16 B/sequence written"}
+                                     "form": eng2.reduce_form(),
+                                     "note": "streaming form at this size (2 launches: stream over fixed 4096-token blocks + fold per sequence); 12 B/token read + 16 B/sequence written"}
         eng2.close()
         del r_lp, r_en, r_cf
     if world == 1 and not vocab_mode and not args.no_prepare_standalone:

@@ -330,8 +330,8 @@ int sq_score_debug_fill_workspace(sq_score_ctx *ctx, int value, void *stream);
 int64_t sq_score_launch_count(const sq_score_ctx *ctx);
 
 /* Which form of kernel 2 (step a7) the last call on this ctx used: 0 = none yet, SQ_REDUCE_FORM_FUSED = one launch (the
- * whole problem is one wave of CTAs), _TILES = three launches over sequence-aligned tiles, _STREAM = index + stream +
- * fold over fixed blocks (large inputs, window <= 2048, 16-byte aligned arrays), _TAIL = inside the finalize kernel
+ * whole problem is one wave of CTAs), _TILES = three launches over sequence-aligned tiles, _STREAM = stream +
+ * fold over fixed blocks (large inputs, 128 <= window <= 2048, 16-byte aligned arrays), _TAIL = inside the finalize kernel
  * (runs of at most 128 tokens).  All forms compute the same reductions; tests and bench.py report which one ran. */
 #define SQ_REDUCE_FORM_FUSED 1
 #define SQ_REDUCE_FORM_TILES 2

@@ -392,7 +392,7 @@ __global__ void __launch_bounds__(RED_THREADS) sq_reduce_fused_kernel(const Redu
 }
 
 // ------------------------------------------------------------------------------------------------------------------
-// Streaming form (large inputs; window <= RS_WMAX; 16-byte aligned arrays): two launches.
+// Streaming form (large inputs; RS_WMIN <= window <= RS_WMAX; 16-byte aligned arrays): two launches.
 //
 // The tile forms above cut tiles at sequence starts, so a CTA must know its sequence before it can load anything
 // (table lookup or search -> loads -> arithmetic, every step a dependent round trip through a saturated memory system),
@@ -419,6 +419,8 @@ constexpr int RS_THREADS = 512;
 constexpr int RS_WARPS = RS_THREADS / 32;
 constexpr int RS_R = 256;           // tokens per warp = per record
 constexpr int RS_WMAX = 2048;       // widest window: the look-ahead is one 16-byte vector per thread
+constexpr int RS_WMIN = 128;        // narrowest: S(j) = P[j+w] - P[j] with P up to ~6144 x mean(conf) in fp32; the rounding of P
+                                    // (~1e-7 relative to P, i.e. ~5e-6 of a 128-element sum) would reach 1e-3 of a 1-element one
 
 __device__ __forceinline__ float4 rs_load4(const float* a, int e, int T) {   // elements at or past T read as 0
   if (e + 4 <= T) return __ldg(reinterpret_cast<const float4*>(a + e));
@@ -467,7 +469,7 @@ __device__ __forceinline__ float rs_warp_sum4(float a, float b, float c, float d
 }
 
 template <bool HAS_TG>
-__global__ void __launch_bounds__(RS_THREADS, 2) sq_reduce_stream_kernel(const ReduceParams p) {
+__global__ void __launch_bounds__(RS_THREADS, 3) sq_reduce_stream_kernel(const ReduceParams p) {
   __shared__ __align__(16) float s_P[RS_TB + RS_WMAX + 4];   // exclusive prefix of conf over block + look-ahead
   __shared__ float s_tot[32];                                // totals: 16 warp ranges, then 16 look-ahead runs of 128
   cudaGridDependencySynchronize();

@@ -533,9 +533,12 @@ static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t s
     return SQ_OK;
   }
   // Streaming form (two launches, sq_reduce_kernel.cuh): fixed 4096-token blocks whose loads depend on nothing, every
-  // sequence boundary handled in the fold.  Needs 16-byte aligned arrays and window <= RS_WMAX; SQ_SCORE_DEBUG bit 8 forces
+  // sequence boundary handled in the fold.  Needs 16-byte aligned arrays and RS_WMIN <= window <= RS_WMAX; SQ_SCORE_DEBUG bit 8 forces
   // it on small inputs (tests).
-  if (rp.vec && rp.window <= sq::RS_WMAX && rp.T > 0 && rp.T <= (int64_t)INT32_MAX - 2 * (sq::RS_TB + sq::RS_WMAX) &&
+  // Narrow windows stay with the tile forms: the streaming form takes S(j) as a difference of two block-wide prefix sums,
+  // whose fp32 rounding (~1e-7 of the prefix) is only negligible against a sum of >= RS_WMIN elements.
+  if (rp.vec && rp.window >= sq::RS_WMIN && rp.window <= sq::RS_WMAX && rp.T > 0 &&
+      rp.T <= (int64_t)INT32_MAX - 2 * (sq::RS_TB + sq::RS_WMAX) &&
       !(ctx->debug_flags & (32 | 64))) {
     const dim3 grid((unsigned)cdiv64(rp.T, sq::RS_TB));
     if (rp.targets) SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_kernel<true>, grid, dim3(sq::RS_THREADS), 0, st, rp));

@@ -426,7 +426,7 @@ def test_reduce_kernel_alone(window):
     a = [x.to(dev) for x in (lp, en, cf, cu)]
     out, out_s = _reduce_all_forms(sq, lambda: sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True),
                                    lambda eng: eng.reduce(a[0], a[1], a[2], a[3], window),
-                                   stream_form="stream" if window <= 2048 else "tiles")
+                                   stream_form="stream" if 128 <= window <= 2048 else "tiles")
     ref = O.sequence_scores(lp.numpy(), en.numpy(), cf.numpy(), cu.numpy(), window)
     check_seqs(out, ref)
     check_seqs(out_s, ref)
@@ -465,7 +465,7 @@ def test_reduce_alignment_targets_and_array_end(offset, with_targets, dbg):
     for window in (1, 6, 1023, 2047, 2048, 2049, 2050, 8192, 8195, 30000):
         out = eng.reduce(place(lp), place(en), place(cf), cu.to(dev), window, targets=place(tg) if with_targets else None)
         torch.cuda.synchronize()
-        assert eng.reduce_form() == (("stream" if offset == 0 and window <= 2048 else "tiles") if dbg else "fused")
+        assert eng.reduce_form() == (("stream" if offset == 0 and 128 <= window <= 2048 else "tiles") if dbg else "fused")
         ref = O.sequence_scores(lp.numpy(), en.numpy(), cf.numpy(), cu.numpy(), window, target_valid=valid)
         check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
     eng.close()
@@ -483,8 +483,8 @@ def test_reduce_many_sequences():
     check_seqs(out_s, ref)
 
 
-@pytest.mark.parametrize("dbg,form", [(None, "stream"), ("32", "tiles")], ids=["streaming", "three-launch"])
-def test_reduce_more_sequences_than_the_single_launch_form_holds(dbg, form):
+@pytest.mark.parametrize("dbg,form,window", [(None, "stream", 130), ("32", "tiles", 7), (None, "tiles", 7)], ids=["streaming", "three-launch", "narrow-window"])
+def test_reduce_more_sequences_than_the_single_launch_form_holds(dbg, form, window):
     """B = 13 000 > 12 287 short sequences (many per 256-token range, empty ones among them): more than one wave, so the
     streaming form runs by default; forced off, the tile table no longer fits in shared memory and the three-launch form
     runs."""
@@ -498,18 +498,19 @@ def test_reduce_more_sequences_than_the_single_launch_form_holds(dbg, form):
         eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True)
     finally:
         os.environ.pop("SQ_SCORE_DEBUG", None)
-    out = eng.reduce(r["target_logprob"].to(dev), r["entropy"].to(dev), r["conf"].to(dev), r["cu_seqlens"].to(dev), 7)
+    out = eng.reduce(r["target_logprob"].to(dev), r["entropy"].to(dev), r["conf"].to(dev), r["cu_seqlens"].to(dev), window)
     torch.cuda.synchronize()
     assert eng.launch_count() == (2 if form == "stream" else 3) and eng.reduce_form() == form
-    ref = O.sequence_scores(r["target_logprob"].numpy(), r["entropy"].numpy(), r["conf"].numpy(), r["cu_seqlens"].numpy(), 7)
+    ref = O.sequence_scores(r["target_logprob"].numpy(), r["entropy"].numpy(), r["conf"].numpy(), r["cu_seqlens"].numpy(), window)
     check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
     eng.close()
 
 
 def test_reduce_streaming_form_many_sequences_per_range_and_one_long_sequence():
-    """The streaming form's piece walk: more than 32 sequences inside one 256-token range (two batches of the walk),
-    sequences that start exactly on range and block boundaries, empty sequences at position 0, in the middle and at the
-    end, one sequence that spans many blocks, windows of every kind (1, < 256, = range, > range, = RS_WMAX)."""
+    """The streaming form's fold: many sequences inside one 256-token range, sequences that start exactly on range and
+    block boundaries, empty sequences at position 0, in the middle and at the
+    end, one sequence that spans many blocks, windows of every residue mod 4 and below / at / above the range size, up to
+    RS_WMAX."""
     import os
     sq = _sq()
     lens = [0, 0] + [1] * 70 + [186, 256, 0, 512, 4096 - 1280 + 256, 0, 4096, 30011] + [3] * 40 + [2, 0, 0]
@@ -524,7 +525,7 @@ def test_reduce_streaming_form_many_sequences_per_range_and_one_long_sequence():
         eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
     finally:
         os.environ.pop("SQ_SCORE_DEBUG", None)
-    for window in (1, 2, 100, 255, 256, 257, 1000, 2048):
+    for window in (128, 129, 130, 131, 255, 256, 257, 1000, 2047, 2048):
         out = eng.reduce(lp.to(dev), en.to(dev), cf.to(dev), cu.to(dev), window)
         torch.cuda.synchronize()
         assert eng.reduce_form() == "stream"
