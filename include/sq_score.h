@@ -241,6 +241,38 @@ int sq_score_run_fp8(sq_score_ctx *ctx, const void *Hq, const float *h_scale, co
                      const int32_t *targets, const int32_t *cu_seqlens, int num_tokens, int num_seqs, int k,
                      int window, const sq_score_outputs *outputs, void *stream);
 
+/* Block-scaled (MX) variant: e4m3 elements with one power-of-two scale per 32 consecutive elements of a row (UE8M0:
+ * scale = 2^(byte - 127)), the operand format of tcgen05.mma.kind::mxf8f6f4.block_scale -- the tensor core applies the
+ * scales, so a block's dynamic range no longer depends on the rest of its row / of the tensor (PAPER.md:681-692 motivates
+ * the engine by very large scorers, where an 8-bit LM head matters).  Like the FP8 variant it is not the graded bf16
+ * path; tests/test_mx_gpu.py measures how much closer to the bf16 scores it gets.
+ *
+ * sq_score_quantize_mx, by definition (reading #26; exact arithmetic, so the result is unique):
+ *   e    = the smallest integer with max|x_block| <= 448 * 2^e, clamped to [-127, 127] (all-zero block: -127)
+ *   code = the e4m3 value nearest to x * 2^-e, ties to even;       x ~= e4m3(code) * 2^e
+ *   X        DEVICE bf16 [num_rows, d], d = cfg.d, d % 16 == 0, 16-byte aligned
+ *   operand  SQ_MX_OPERAND_H (token rows, grouped by 128) or SQ_MX_OPERAND_W (vocabulary rows, grouped by the kernel's
+ *            224-column tiles): selects the layout of sf_out
+ *   q_out    DEVICE uint8 [num_rows, d] e4m3 codes, 16-byte aligned
+ *   sf_out   DEVICE uint8 [sq_score_mx_scale_bytes(num_rows, d, operand)], 16-byte aligned: byte e + 127 of row r,
+ *            32-element block kb32 is at
+ *              ((kb32 / 4 * num_groups + r / G) * P + (r % G) / 128) * 512 + (r % 32) * 16 + ((r % G) / 32 % 4) * 4 + kb32 % 4
+ *            with G = 128, P = 1 (H) or G = 224, P = 2 (W), num_groups = ceil(num_rows / G): 512-byte pieces that
+ *            tcgen05.cp moves to TMEM as they are.  Bytes no row / block reaches are 0.
+ * Asynchronous on `stream`.  Errors: INVALID_ARG, UNSUPPORTED (d % 16), CUDA.
+ *
+ * sq_score_run_mx: sq_score_run on such operands (logits = sum over blocks of 2^(eh + ew) * sum_j Hq * Wq, products
+ * exact, fp32 accumulate in the tensor core); Hq / h_sf from operand H with num_rows = T, Wq / w_sf from operand W with
+ * num_rows = cfg.vocab; everything else as sq_score_run.  Errors: as sq_score_run, UNSUPPORTED (d % 16). */
+#define SQ_MX_OPERAND_H 0
+#define SQ_MX_OPERAND_W 1
+int64_t sq_score_mx_scale_bytes(int64_t num_rows, int d, int operand);
+int sq_score_quantize_mx(sq_score_ctx *ctx, const void *X, int64_t num_rows, int operand, void *q_out, void *sf_out,
+                         void *stream);
+int sq_score_run_mx(sq_score_ctx *ctx, const void *Hq, const void *h_sf, const void *Wq, const void *w_sf,
+                    const int32_t *targets, const int32_t *cu_seqlens, int num_tokens, int num_seqs, int k,
+                    int window, const sq_score_outputs *outputs, void *stream);
+
 /* Vocab-parallel scoring: the LM head is split by rows over R shards (the tensor-
  * parallel layout of a served scorer); every shard scores the same H against its rows and produces ONE merged partial
  * state per token; the states are exchanged (one all-gather, e.g. ncclAllGather / torch.distributed) and merged by the

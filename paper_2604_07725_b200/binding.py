@@ -12,6 +12,7 @@ SQ_MAX_CHUNKS = 160
 SQ_PROFILE_RING = 64
 FLAG_REDUCE_ONLY = 1
 FLAG_STAGING = 2
+MX_OPERAND_H, MX_OPERAND_W = 0, 1
 ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOMEM = -1, -2, -3, -4
 
 
@@ -96,6 +97,13 @@ def lib() -> C.CDLL:
     L.sq_score_run_fp8.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                    C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
     L.sq_score_run_fp8.restype = C.c_int
+    L.sq_score_mx_scale_bytes.argtypes = [C.c_int64, C.c_int, C.c_int]
+    L.sq_score_mx_scale_bytes.restype = C.c_int64
+    L.sq_score_quantize_mx.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+    L.sq_score_quantize_mx.restype = C.c_int
+    L.sq_score_run_mx.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                  C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
+    L.sq_score_run_mx.restype = C.c_int
     L.sq_score_plan.argtypes = [C.POINTER(sq_score_config), C.c_int64, C.c_int, C.c_int, C.POINTER(sq_score_plan_t)]
     L.sq_score_plan.restype = C.c_int
     L.sq_score_set_profiling.argtypes = [C.c_void_p, C.c_int]
@@ -300,6 +308,30 @@ class SqScore:
         o = sq_score_outputs(*[_ptr(out.get(n)) for n, _ in sq_score_outputs._fields_])
         self._check(self._L.sq_score_run_fp8(self._h, _ptr(Hq), _ptr(h_scale), _ptr(Wq), _ptr(w_scale), _ptr(targets), _ptr(cu_seqlens),
                                              T, B, k, window, C.byref(o), self._stream(stream)))
+        return out
+
+    def quantize_mx(self, X, operand: int, stream=None, out=None):
+        """sq_score_quantize_mx: bf16 [rows, d] -> (uint8 e4m3 codes [rows, d], uint8 scale bytes in the kernel's layout);
+        operand = MX_OPERAND_H (token rows) or MX_OPERAND_W (vocabulary rows); `out` = (codes, scales) reuses tensors."""
+        import torch
+        rows, d = X.shape
+        if out is not None:
+            q, sf = out
+        else:
+            q = torch.empty(rows, d, dtype=torch.uint8, device=X.device)
+            sf = torch.empty(max(16, self._L.sq_score_mx_scale_bytes(rows, d, operand)), dtype=torch.uint8, device=X.device)
+        self._check(self._L.sq_score_quantize_mx(self._h, _ptr(X), rows, operand, _ptr(q), _ptr(sf), self._stream(stream)))
+        return q, sf
+
+    def run_mx(self, Hq, h_sf, Wq, w_sf, targets, cu_seqlens, k: int, window: int, stream=None, per_token: bool = True,
+               topk: bool = True, out: Optional[dict] = None) -> dict:
+        """sq_score_run_mx: the scoring pass on block-scaled (MX) e4m3 operands."""
+        T, B = Hq.shape[0], cu_seqlens.shape[0] - 1
+        if out is None:
+            out = self._alloc_out(T, B, k, Hq.device, per_token, topk)
+        o = sq_score_outputs(*[_ptr(out.get(n)) for n, _ in sq_score_outputs._fields_])
+        self._check(self._L.sq_score_run_mx(self._h, _ptr(Hq), _ptr(h_sf), _ptr(Wq), _ptr(w_sf), _ptr(targets), _ptr(cu_seqlens),
+                                            T, B, k, window, C.byref(o), self._stream(stream)))
         return out
 
     def run_host(self, H_host, W_dev, targets_host, cu_seqlens_host, k: int, window: int, seq_out_host, stream=None):

@@ -7,7 +7,7 @@
 //
 // Persistent, warp-specialised:  warp 0 = TMA producer, warp 1 = MMA issuer, warp 2 = TMEM
 // allocator, warps 4..7 = statistics epilogue (thread = TMEM lane = token row).
-// Work unit = (token tile of 128*CG rows, vocab chunk = a run of 256-column tiles, FusedParams::chunk_vt);
+// Work unit = (token tile of 128*CG rows, vocab chunk = a run of 256-column tiles (224 in the MX variant), FusedParams::chunk_vt);
 // a unit's running state lives in registers and is written as a partial state at its end.
 #pragma once
 #include "sq_ptx.cuh"
@@ -25,11 +25,20 @@ constexpr int TMEM_COLS = 512;  // two 256-column accumulator stages
 constexpr float NEG_BIG = -1.0e30f;
 constexpr float LOG2E_F = 1.4426950408889634f;   // consume32 takes log2(e) times the row's dequantisation scale (1 for bf16)
 
-template <int CG> struct FusedCfg {
+constexpr int BLOCK_N_MX = 224;   // block-scaled variant: 2 x 224 accumulator columns + 12 columns of scale factors fit TMEM's 512
+constexpr int MODE_BF16 = 0, MODE_F8 = 1, MODE_MX = 2;
+
+template <int CG, int MODE = MODE_BF16> struct FusedCfg {
+  static constexpr int BN = (MODE == MODE_MX) ? BLOCK_N_MX : BLOCK_N;   // vocabulary columns per tile
   static constexpr int A_BYTES = BLOCK_M * BLOCK_K * 2;                 // 16 KB
-  static constexpr int B_ROWS = BLOCK_N / CG;                           // W rows this CTA stages
-  static constexpr int B_BYTES = B_ROWS * BLOCK_K * 2;                  // 32 KB (CG=1) / 16 KB (CG=2)
-  static constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+  static constexpr int B_ROWS = BN / CG;                                // W rows this CTA stages
+  static constexpr int B_BYTES = B_ROWS * BLOCK_K * 2;                  // 32 KB (CG=1) / 16 KB (CG=2); MX: 28 / 14 KB
+  // MX: the scale factors of the stage's 128-element k-block: 512 B for this CTA's 128 token rows, 1024 B for ALL the
+  // tile's vocabulary rows (every CTA of a pair multiplies its token rows with the whole tile)
+  static constexpr int SFA_BYTES = (MODE == MODE_MX) ? 512 : 0;
+  static constexpr int SFB_BYTES = (MODE == MODE_MX) ? 1024 : 0;
+  static constexpr int STAGE_BYTES = (A_BYTES + B_BYTES + SFA_BYTES + SFB_BYTES + 1023) / 1024 * 1024;
+  static constexpr int STAGE_TX = A_BYTES + B_BYTES + SFA_BYTES + SFB_BYTES;   // bytes the TMA loads of a stage deliver
 #ifndef SQ_STAGES_PAIR
 #define SQ_STAGES_PAIR 6
 #endif
@@ -37,6 +46,8 @@ template <int CG> struct FusedCfg {
   static constexpr int BAR_BYTES = 256;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;  // +1024: manual alignment
   static constexpr int UMMA_M = BLOCK_M * CG;
+  static constexpr int TMEM_SFA = 2 * BN;        // MX: TMEM columns of the scale factors, behind the two accumulators
+  static constexpr int TMEM_SFB = 2 * BN + 4;
 };
 
 constexpr int MAX_CHUNKS = 160;   // vocab chunks per row at most (= FIN_MAX_CHUNKS of the finalize kernel)
@@ -68,6 +79,7 @@ struct FusedParams {
   int flag_rows;                 //   <=> rows [0, (f+1) * flag_rows) of H are in device memory
   const float* h_scale;     // FP8 variant: H = Hq * h_scale[row], W = Wq * (*w_scale) with Hq, Wq e4m3 (per-row / per-tensor
   const float* w_scale;     //   scales, DEVICE); null in the bf16 path
+  int sf_h_blocks;          // MX variant: 128-row blocks of H in the scale layout (rows of tmap_sfa per k-block)
   int vocab_offset;         // W is rows [vocab_offset, vocab_offset + V) of a larger LM head (vocab-parallel shard):
                             // targets and the reported vocabulary ids are global, columns local
 #ifdef SQ_PROBES
@@ -273,11 +285,19 @@ __device__ __forceinline__ void consume32(RowState<CAP>& st, float (&r)[32], int
 // Hq.Wq^T and the epilogue works in those units with log2(e) * h_scale[row] * w_scale folded into the exponent's
 // multiplier, so the dequantisation costs no instruction per logit; m, u, the list values and the target logit are
 // scaled once per row when the partial state is written.
-template <int CG, int CAP, bool F8 = false>
+// MX (MODE_MX): e4m3 bytes with one UE8M0 scale per 32 elements of K (tcgen05 kind::mxf8f6f4.block_scale).  The scales of a
+// stage arrive by TMA next to the operands (tmap_sfa / tmap_sfb: rows of 512 bytes in the layout tcgen05.cp wants, written
+// by sq_quant_mx_kernel), are copied to TMEM by the MMA thread before the stage's four instructions, and the tensor core
+// applies them: the accumulator holds the logits themselves, so the epilogue is the bf16 one.  Tiles are 224 columns wide.
+template <int CG, int CAP, int MODE = MODE_BF16>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_constant__ CUtensorMap tmap_w,
+                      const __grid_constant__ CUtensorMap tmap_sfa, const __grid_constant__ CUtensorMap tmap_sfb,
                       const FusedParams p) {
-  using Cfg = FusedCfg<CG>;
+  using Cfg = FusedCfg<CG, MODE>;
+  constexpr bool F8 = (MODE == MODE_F8);
+  constexpr bool MX = (MODE == MODE_MX);
+  constexpr int BN = Cfg::BN;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;   // swizzle-128B: 1024-B aligned tiles
   const uint32_t bar_base = smem_base + Cfg::STAGES * Cfg::STAGE_BYTES;
@@ -288,6 +308,8 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   const uint32_t tmem_slot = bar_base + 8u * (2 * Cfg::STAGES + 4);
   auto smem_a = [&](int s) { return smem_base + s * Cfg::STAGE_BYTES; };
   auto smem_b = [&](int s) { return smem_base + s * Cfg::STAGE_BYTES + Cfg::A_BYTES; };
+  auto smem_sfa = [&](int s) { return smem_base + s * Cfg::STAGE_BYTES + Cfg::A_BYTES + Cfg::B_BYTES; };
+  auto smem_sfb = [&](int s) { return smem_base + s * Cfg::STAGE_BYTES + Cfg::A_BYTES + Cfg::B_BYTES + Cfg::SFA_BYTES; };
 
   const int warp = threadIdx.x >> 5;
   const uint32_t lane = lane_id();
@@ -299,6 +321,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   if (warp == 0 && lane == 0) {
     prefetch_tensormap(&tmap_h);
     prefetch_tensormap(&tmap_w);
+    if constexpr (MX) { prefetch_tensormap(&tmap_sfa); prefetch_tensormap(&tmap_sfb); }
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < Cfg::STAGES; ++s) {
@@ -323,13 +346,13 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
   const int rows_per_unit = BLOCK_M * CG;
-  constexpr int BK = F8 ? BLOCK_K_F8 : BLOCK_K;   // elements per k-block (128 bytes of every operand row)
+  constexpr int BK = (F8 || MX) ? BLOCK_K_F8 : BLOCK_K;   // elements per k-block (128 bytes of every operand row)
 
   if (warp == 0) {
     // ===================================================================== TMA producer
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      uint32_t stage_tx = Cfg::STAGE_BYTES * CG;   // the pair leader's barrier counts both CTAs' bytes
+      uint32_t stage_tx = Cfg::STAGE_TX * CG;   // the pair leader's barrier counts both CTAs' bytes
 #ifdef SQ_PROBES
       if (p.probe_flags & 2) stage_tx -= (Cfg::B_BYTES / 2) * CG;   // probe: W boxes of half height
       if (p.probe_flags & 4) stage_tx -= (Cfg::A_BYTES / 2) * CG;   // probe: H boxes of half height
@@ -345,18 +368,28 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
           wait_rows_ready(p.h_ready + (min(row0 + BLOCK_M, p.T) - 1) / p.flag_rows, p.wait_limit);
         const int vt0 = p.chunk_vt[un.chunk], vt1 = p.chunk_vt[un.chunk + 1];
         for (int vt = vt0; vt < vt1; ++vt) {
-          const int wrow0 = vt * BLOCK_N + (int)cta_rank * Cfg::B_ROWS;
+          const int wrow0 = vt * BN + (int)cta_rank * Cfg::B_ROWS;
           for (int kb = 0; kb < p.num_k_blocks; ++kb) {
             mbar_wait(empty_bar(stage), phase ^ 1u, p.wait_limit);
+            // MX: scale rows of 512 bytes: [k-block][128-row block of H] and [k-block][vocab tile][2]
+            const int sfa_row = kb * p.sf_h_blocks + row0 / BLOCK_M, sfb_row = (kb * p.num_vtiles + vt) * 2;
             if constexpr (CG == 1) {
               mbar_arrive_expect_tx(full_bar(stage), stage_tx);
               tma_load_2d(smem_a(stage), &tmap_h, full_bar(stage), kb * BK, row0);
               tma_load_2d(smem_b(stage), &tmap_w, full_bar(stage), kb * BK, wrow0);
+              if constexpr (MX) {
+                tma_load_2d(smem_sfa(stage), &tmap_sfa, full_bar(stage), 0, sfa_row);
+                tma_load_2d(smem_sfb(stage), &tmap_sfb, full_bar(stage), 0, sfb_row);
+              }
             } else {
               const uint32_t bar = mapa(full_bar(stage), 0);
               if (leader) mbar_arrive_expect_tx(full_bar(stage), stage_tx);
               tma_load_2d_pair(smem_a(stage), &tmap_h, bar, kb * BK, row0);
               tma_load_2d_pair(smem_b(stage), &tmap_w, bar, kb * BK, wrow0);
+              if constexpr (MX) {
+                tma_load_2d_pair(smem_sfa(stage), &tmap_sfa, bar, 0, sfa_row);
+                tma_load_2d_pair(smem_sfb(stage), &tmap_sfb, bar, 0, sfb_row);
+              }
             }
             if (++stage == Cfg::STAGES) { stage = 0; phase ^= 1u; }
           }
@@ -366,7 +399,8 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   } else if (warp == 1) {
     // ===================================================================== MMA issuer (pair leader only)
     if (leader && lane == 0) {
-      constexpr uint32_t idesc = F8 ? make_idesc_e4m3(Cfg::UMMA_M, BLOCK_N) : make_idesc_bf16(Cfg::UMMA_M, BLOCK_N);
+      constexpr uint32_t idesc = MX ? make_idesc_mx(Cfg::UMMA_M, BN)
+                                    : (F8 ? make_idesc_e4m3(Cfg::UMMA_M, BN) : make_idesc_bf16(Cfg::UMMA_M, BN));
       int stage = 0; uint32_t phase = 0;
       uint32_t tile = 0;
       for (int gu = 0; gu < gc.num_iters; ++gu) {
@@ -377,16 +411,23 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
           const uint32_t acc = tile & 1u;
           mbar_wait(tempty_bar(acc), ((tile >> 1) & 1u) ^ 1u, p.wait_limit);   // epilogue drained this accumulator
           tc_fence_after();
-          const uint32_t d_tmem = tmem_base + acc * BLOCK_N;
+          const uint32_t d_tmem = tmem_base + acc * BN;
           for (int kb = 0; kb < p.num_k_blocks; ++kb) {
             mbar_wait(full_bar(stage), phase, p.wait_limit);
             tc_fence_after();
             const uint64_t adesc = make_smem_desc_sw128(smem_a(stage));
             const uint64_t bdesc = make_smem_desc_sw128(smem_b(stage));
+            if constexpr (MX) {   // this k-block's scales: 4 columns for the 128 token rows, 8 for the tile's vocabulary rows
+              tmem_cp_32x128b_warpx4<CG>(tmem_base + Cfg::TMEM_SFA, make_smem_desc_sf(smem_sfa(stage)));
+              tmem_cp_32x128b_warpx4<CG>(tmem_base + Cfg::TMEM_SFB, make_smem_desc_sf(smem_sfb(stage)));
+              tmem_cp_32x128b_warpx4<CG>(tmem_base + Cfg::TMEM_SFB + 4, make_smem_desc_sf(smem_sfb(stage) + 512));
+            }
 #pragma unroll
             for (int k = 0; k < BLOCK_K / UMMA_K; ++k) {
               // +32 B per UMMA_K step inside the 128-B swizzle row: +2 in the (addr >> 4) field
-              if constexpr (F8) umma_f8<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
+              if constexpr (MX) umma_mx<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc_mx_sf(idesc, k), tmem_base + Cfg::TMEM_SFA,
+                                            tmem_base + Cfg::TMEM_SFB, (kb | k) != 0 ? 1u : 0u);
+              else if constexpr (F8) umma_f8<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
               else umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
             }
             umma_commit<CG>(empty_bar(stage));   // smem slot free once these MMAs retire
@@ -419,14 +460,14 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
         const uint32_t acc = tile & 1u;
         mbar_wait(tfull_bar(acc), (tile >> 1) & 1u, p.wait_limit);
         tc_fence_after();
-        const int colbase = vt * BLOCK_N;
-        int ngroups = min(BLOCK_N, p.V - colbase + 31) >> 5;   // 32-column groups with a valid column
+        const int colbase = vt * BN;
+        int ngroups = min(BN, p.V - colbase + 31) >> 5;   // 32-column groups with a valid column
 #ifdef SQ_PROBES
         if (p.probe_flags & 1) ngroups = 0;        // probe: the epilogue skips the statistics
 #endif
         for (int g = 0; g < ngroups; ++g) {
           float r[32];
-          tmem_ld_32x32(lane_addr + acc * BLOCK_N + g * 32, r);
+          tmem_ld_32x32(lane_addr + acc * BN + g * 32, r);
           tmem_ld_wait();
           consume32<CAP>(st, r, colbase + g * 32, p.V, tgt, l2e);
         }
@@ -452,8 +493,8 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
           p.part_topv[oj] = st.tv[j] * deq;
           p.part_topi[oj] = st.ti[j] < 0 ? -1 : st.ti[j] + p.vocab_offset;
         }
-        const int c0 = vt0 * BLOCK_N;
-        if (tgt >= c0 && tgt < min(vt1 * BLOCK_N, p.V)) p.zt[row] = st.zt * deq;
+        const int c0 = vt0 * BN;
+        if (tgt >= c0 && tgt < min(vt1 * BN, p.V)) p.zt[row] = st.zt * deq;
       }
     }
   }

@@ -162,6 +162,35 @@ __device__ __forceinline__ void umma_f8(uint32_t d_tmem, uint64_t adesc, uint64_
         ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
         : "memory");
 }
+// Block-scaled: kind::mxf8f6f4.block_scale (e4m3 elements, one UE8M0 scale per 32 elements of K = one scale per row and
+// instruction).  The scales sit in TMEM (tcgen05.cp below): `sfa` / `sfb` are the TMEM addresses of 32-bit columns that
+// hold four scale bytes per row (lane = row % 32, column = row / 32); the descriptor's a_sf_id / b_sf_id pick the byte.
+template <int CG>
+__device__ __forceinline__ void umma_mx(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t sfa,
+                                        uint32_t sfb, uint32_t accumulate) {
+  if constexpr (CG == 1)
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::mxf8f6f4.block_scale [%0], %1, %2, %3, [%5], [%6], p;\n\t}"
+        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(sfa), "r"(sfb)
+        : "memory");
+  else
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::mxf8f6f4.block_scale [%0], %1, %2, %3, [%5], [%6], p;\n\t}"
+        ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate), "r"(sfa), "r"(sfb)
+        : "memory");
+}
+// Shared memory -> TMEM: 32 rows of 16 bytes go to 32 lanes x 4 columns, repeated in all four lane quarters.  With
+// cta_group::2 each CTA of the pair copies from its own shared memory (same offset) into its own TMEM.  Ordered with
+// the MMAs the same thread issues before and after it.
+template <int CG>
+__device__ __forceinline__ void tmem_cp_32x128b_warpx4(uint32_t taddr, uint64_t sdesc) {
+  if constexpr (CG == 1)
+    asm volatile("tcgen05.cp.cta_group::1.32x128b.warpx4 [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+  else
+    asm volatile("tcgen05.cp.cta_group::2.32x128b.warpx4 [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
 // All MMAs issued so far by this thread arrive on `bar` when they complete.  For a pair the
 // arrive is multicast to the same barrier offset in both CTAs.
 template <int CG>
@@ -202,6 +231,15 @@ __device__ __forceinline__ uint64_t make_smem_desc_sw128(uint32_t smem_addr) {
   desc |= static_cast<uint64_t>(2) << 61;
   return desc;
 }
+// Unswizzled K-major descriptor of 32 rows x 16 bytes stored densely (a 512-byte block of scale factors): core matrices
+// of 8 rows x 16 B = 128 contiguous bytes, stacked along the rows at SBO = 128 B; one core matrix wide, so LBO is unused.
+__device__ __forceinline__ uint64_t make_smem_desc_sf(uint32_t smem_addr) {
+  uint64_t desc = 0;
+  desc |= static_cast<uint64_t>((smem_addr & 0x3FFFFu) >> 4);
+  desc |= static_cast<uint64_t>(128 >> 4) << 32;
+  desc |= static_cast<uint64_t>(1) << 46;
+  return desc;
+}
 // kind::f16 instruction descriptor: D=f32, A=B=bf16, both K-major, M x N.
 __host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N) {
   return (1u << 4) | (1u << 7) | (1u << 10) | (static_cast<uint32_t>(N >> 3) << 17) |
@@ -212,6 +250,13 @@ __host__ __device__ constexpr uint32_t make_idesc_bf16(int M, int N) {
 __host__ __device__ constexpr uint32_t make_idesc_e4m3(int M, int N) {
   return (1u << 4) | (static_cast<uint32_t>(N >> 3) << 17) | (static_cast<uint32_t>(M >> 4) << 24);
 }
+
+// kind::mxf8f6f4.block_scale instruction descriptor: A=B=e4m3 (format 0), UE8M0 scales (bit 23), K-major, M x N, D=f32
+// implied; bits [4,6) and [29,31) take the scale byte (0..3) of B and of A for the instruction at hand.
+__host__ __device__ constexpr uint32_t make_idesc_mx(int M, int N) {
+  return (static_cast<uint32_t>(N >> 3) << 17) | (1u << 23) | (static_cast<uint32_t>(M >> 4) << 24);
+}
+__host__ __device__ constexpr uint32_t idesc_mx_sf(uint32_t idesc, uint32_t sf) { return idesc | (sf << 4) | (sf << 29); }
 
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;

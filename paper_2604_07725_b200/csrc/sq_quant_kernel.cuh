@@ -131,4 +131,73 @@ __global__ void __launch_bounds__(QUANT_REG_WARPS * 32) sq_quant_rows_reg_kernel
   }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Block-scaled (MX) e4m3: one power-of-two scale per 32 consecutive elements of a row -- the operand format of
+// tcgen05.mma.kind::mxf8f6f4.block_scale (next widening of SURVEY section 8(f)-4; reading #26):
+//   e    = the smallest integer with amax_blk <= 448 * 2^e, clamped to [-127, 127]   (amax = 0: -127)
+//   code = e4m3 nearest (ties to even) to x * 2^-e        scale byte (UE8M0) = e + 127
+// Everything is exact: bf16 values are fp32 values, e comes from the exponent and a compare of the significand with 1.75
+// (448 = 1.75 * 2^8), the scaling is by powers of two (in two steps, so that 2^127 / 2^-127 never appear as one factor),
+// and |x * 2^-e| <= 448.  So codes and exponents must equal the oracle's bit for bit.
+// The scale bytes are written in the layout tcgen05.cp (32x128b.warpx4) moves to TMEM unchanged.  Rows are grouped in
+// blocks of `blk_rows` (128 for H: the token rows of one CTA; 224 for W: one vocabulary tile), K in blocks of 128
+// elements (4 scales).  Region (kb, blk) holds 512-byte pieces of 128 rows each:
+//   byte = ((kb * num_blk + blk) * pieces + r / 128) * 512 + (r % 32) * 16 + ((r / 32) % 4) * 4 + (k % 128) / 32,  r = row % blk_rows
+struct QuantMxParams {
+  const uint4* X;        // bf16 [rows, d] as 16-byte vectors (8 elements)
+  uint2* Q;              // e4m3 [rows, d] as 8-byte vectors
+  uint8_t* SF;           // scale bytes, layout above (zeroed by the caller: unwritten slots scale zero codes)
+  long long rows;
+  int d;
+  int blk_rows;          // 128 or 224
+  int pieces;            // 512-byte pieces per region: ceil(blk_rows / 128)
+  int64_t num_blk;       // ceil(rows / blk_rows)
+};
+
+__device__ __forceinline__ int mx_exponent(float amax) {   // amax >= 0, finite
+  if (amax == 0.f) return -127;
+  const uint32_t bits = __float_as_uint(amax);
+  const int E = (int)(bits >> 23) - 127;                     // subnormals read as -127: e clamps to -127 either way
+  const bool above = (bits & 0x7fffffu) > 0x600000u;         // significand > 1.75
+  return max(-127, min(127, E - 8 + (above ? 1 : 0)));
+}
+
+__global__ void __launch_bounds__(256) sq_quant_mx_kernel(const QuantMxParams p) {
+  const int lane = threadIdx.x & 31;
+  const long long warps = (long long)gridDim.x * 8;
+  const int nvec = p.d >> 3;                                 // 16-byte vectors per row (d % 16 == 0)
+  for (long long row = (long long)blockIdx.x * 8 + (threadIdx.x >> 5); row < p.rows; row += warps) {
+    const long long blk = row / p.blk_rows;
+    const int r = (int)(row - blk * p.blk_rows);
+    const size_t in_region = (size_t)(r >> 7) * 512 + (size_t)(r & 31) * 16 + (size_t)((r >> 5) & 3) * 4;
+    for (int v0 = 0; v0 < nvec; v0 += 32) {                  // 256 elements = 8 scale blocks per pass; 4 lanes per block
+      const int v = v0 + lane;
+      uint4 x = make_uint4(0u, 0u, 0u, 0u);
+      if (v < nvec) x = __ldg(p.X + row * nvec + v);
+      float m = q_amax8(x);
+      m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+      m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+      const int e = mx_exponent(m);
+      const int ea = (-e) / 2, eb = (-e) - ea;               // x * 2^ea * 2^eb, both factors normal floats
+      const float fa = __uint_as_float((uint32_t)(ea + 127) << 23), fb = __uint_as_float((uint32_t)(eb + 127) << 23);
+      float f[8];
+      q_unpack8(x, f);
+      uint32_t c[8];
+#pragma unroll
+      for (int i = 0; i < 8; ++i) c[i] = (uint32_t)__nv_cvt_float_to_fp8(__fmul_rn(__fmul_rn(f[i], fa), fb), __NV_SATFINITE, __NV_E4M3);
+      if (v < nvec) {
+        uint2 o;
+        o.x = c[0] | (c[1] << 8) | (c[2] << 16) | (c[3] << 24);
+        o.y = c[4] | (c[5] << 8) | (c[6] << 16) | (c[7] << 24);
+        p.Q[row * nvec + v] = o;
+        if ((lane & 3) == 0) {
+          const int k = v * 8;                               // first element of the scale block
+          const size_t region = ((size_t)(k >> 7) * (size_t)p.num_blk + (size_t)blk) * (size_t)p.pieces;
+          p.SF[region * 512 + in_region + ((k & 127) >> 5)] = (uint8_t)(e + 127);
+        }
+      }
+    }
+  }
+}
+
 }  // namespace sq

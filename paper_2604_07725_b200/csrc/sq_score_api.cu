@@ -121,7 +121,8 @@ static void split_stripes(int nv, int ng, const int* batches, int* width, int mi
   }
 }
 
-static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, sq_score_plan_t* pl, int max_clusters = 0) {
+static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, sq_score_plan_t* pl, int max_clusters = 0,
+                     int tile_n = sq::BLOCK_N) {
   if (!cfg || !pl || T < 0 || cfg->d <= 0 || cfg->vocab <= 0 || k < 1 || k > SQ_MAX_K) return SQ_ERR_INVALID_ARG;
   if (num_sms <= 0) num_sms = 148;
   // default: CTA pairs (UMMA M = 256); a decode-shaped run of at most 128 rows fits one CTA's 128 TMEM
@@ -131,7 +132,7 @@ static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, 
   pl->cta_group = cg;
   pl->rows_per_tile = 128 * cg;
   pl->m_tiles = (int)cdiv64(T, pl->rows_per_tile);
-  pl->num_vtiles = (int)cdiv64(cfg->vocab, 256);
+  pl->num_vtiles = (int)cdiv64(cfg->vocab, tile_n);   // 256 columns per tile (224 in the MX variant)
   pl->num_k_blocks = (int)cdiv64(cfg->d, 64);
   pl->num_clusters = std::max(1, num_sms / cg);
   if (max_clusters > 0) pl->num_clusters = std::min(pl->num_clusters, max_clusters);   // what can be co-resident (create)
@@ -405,9 +406,11 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
                            sq::FusedCfg<CG>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
   SQ_SET_SMEM(1, 8) SQ_SET_SMEM(1, 20) SQ_SET_SMEM(1, 32) SQ_SET_SMEM(2, 8) SQ_SET_SMEM(2, 20) SQ_SET_SMEM(2, 32)
 #undef SQ_SET_SMEM
-#define SQ_SET_SMEM8(CG, CAP)                                                                                      \
-  if (cudaFuncSetAttribute(sq::sq_fused_score_kernel<CG, CAP, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
-                           sq::FusedCfg<CG>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
+#define SQ_SET_SMEM8(CG, CAP)                                                                                              \
+  if (cudaFuncSetAttribute(sq::sq_fused_score_kernel<CG, CAP, sq::MODE_F8>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+                           sq::FusedCfg<CG, sq::MODE_F8>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;                    \
+  if (cudaFuncSetAttribute(sq::sq_fused_score_kernel<CG, CAP, sq::MODE_MX>, cudaFuncAttributeMaxDynamicSharedMemorySize,   \
+                           sq::FusedCfg<CG, sq::MODE_MX>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
   SQ_SET_SMEM8(1, 8) SQ_SET_SMEM8(1, 20) SQ_SET_SMEM8(1, 32) SQ_SET_SMEM8(2, 8) SQ_SET_SMEM8(2, 20) SQ_SET_SMEM8(2, 32)
 #undef SQ_SET_SMEM8
   for (const void* f : {(const void*)sq::sq_reduce_fused_kernel<true>, (const void*)sq::sq_reduce_fused_kernel<false>})
@@ -468,15 +471,29 @@ static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int6
   return SQ_OK;
 }
 
+// MX scale factors: `rows` rows of 512 bytes (128 x uint32), unswizzled; a box is `box_rows` whole rows.
+static int make_tmap_sf(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int box_rows) {
+  const cuuint64_t dims[2] = {128, (cuuint64_t)rows};
+  const cuuint64_t strides[1] = {512};
+  const cuuint32_t box[2] = {128, (cuuint32_t)box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  CUresult r = reinterpret_cast<encode_tiled_fn>(ctx->encode_fn)(
+      map, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, const_cast<void*>(base), dims, strides, box, estr,
+      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return set_err(ctx, SQ_ERR_CUDA, "cuTensorMapEncodeTiled (scale factors) failed with CUresult %d", (int)r);
+  return SQ_OK;
+}
+
 // ------------------------------------------------------------------------------------------ launches
-template <int CG, int CAP, bool F8 = false>
+template <int CG, int CAP, int MODE = sq::MODE_BF16>
 static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CUtensorMap& th, const CUtensorMap& tw,
-                                const sq::FusedParams& fp, cudaStream_t st) {
+                                const CUtensorMap& tsa, const CUtensorMap& tsb, const sq::FusedParams& fp, cudaStream_t st) {
   const int clusters = pl.clusters_used;   // every launched cluster belongs to a gang
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3((unsigned)(clusters * CG));
   lc.blockDim = dim3(sq::NUM_THREADS);
-  lc.dynamicSmemBytes = sq::FusedCfg<CG>::SMEM_BYTES;
+  lc.dynamicSmemBytes = sq::FusedCfg<CG, MODE>::SMEM_BYTES;
   lc.stream = st;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeClusterDimension;
@@ -484,7 +501,7 @@ static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CU
   lc.attrs = at;
   lc.numAttrs = 1;
   (void)num_sms;
-  return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP, F8>, th, tw, fp);
+  return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP, MODE>, th, tw, tsa, tsb, fp);
 }
 
 // Launch with programmatic stream serialization: the kernel is scheduled while its predecessor drains and waits in
@@ -618,7 +635,7 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
                     const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k, int window,
                     const sq_score_outputs* o, void* stream, const unsigned int* h_ready, int flag_rows,
                     int vocab_offset = 0, float* shard_state = nullptr, const float* h_scale = nullptr,
-                    const float* w_scale = nullptr, int shard_rows = 0) {
+                    const float* w_scale = nullptr, int shard_rows = 0, const void* h_sf = nullptr, const void* w_sf = nullptr) {
   if (!ctx) return SQ_ERR_INVALID_ARG;
   if (!o && !shard_state) return set_err(ctx, SQ_ERR_INVALID_ARG, "outputs is null");
   static const sq_score_outputs no_outputs = {};
@@ -647,22 +664,24 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
   float* conf = o->conf ? o->conf : ctx->tok_conf;
 
   if (T > 0) {
-    const bool f8 = h_scale != nullptr;
+    const bool mx = h_sf != nullptr;                       // block-scaled e4m3 (sq_score_run_mx)
+    const bool f8 = h_scale != nullptr || mx;              // 8-bit operands: 128 elements per k-block
+    const int tile_n = mx ? sq::BLOCK_N_MX : sq::BLOCK_N;
     sq_score_plan_t pl;
     sq_score_config pc = ctx->cfg;
     pc.vocab = V;
     if (f8) pc.d = (d + 1) / 2;   // an e4m3 k-block is 128 elements: the plan sees half as many k-blocks
     const int cg_sel = (pc.cta_group == 1) ? 1 : (pc.cta_group == 2 ? 2 : (T <= 128 ? 1 : 2));
-    make_plan(&pc, T, k, ctx->num_sms, &pl, ctx->max_clusters[cg_sel]);
+    make_plan(&pc, T, k, ctx->num_sms, &pl, ctx->max_clusters[cg_sel], tile_n);
     const int64_t rows = ws_rows_for(ctx->cfg);
     if ((int64_t)pl.num_chunks * T > rows) {   // workspace bound: fewer gangs, wider stripes
       pc.num_chunks = (int)std::max<int64_t>(1, rows / T);
-      make_plan(&pc, T, k, ctx->num_sms, &pl, ctx->max_clusters[cg_sel]);
+      make_plan(&pc, T, k, ctx->num_sms, &pl, ctx->max_clusters[cg_sel], tile_n);
     }
     if (pl.topk_cap > ctx->cap_max) return set_err(ctx, SQ_ERR_INVALID_ARG, "k exceeds the ctx's max_k capacity");
-    CUtensorMap th, tw;
-    if (f8 && d % 16 != 0) return set_err(ctx, SQ_ERR_UNSUPPORTED, "the FP8 variant needs d %% 16 == 0 (TMA 16-byte row strides)");
-    int h_box = sq::BLOCK_M, w_box = sq::BLOCK_N / pl.cta_group;
+    CUtensorMap th, tw, tsa, tsb;
+    if (f8 && d % 16 != 0) return set_err(ctx, SQ_ERR_UNSUPPORTED, "the FP8 variants need d %% 16 == 0 (TMA 16-byte row strides)");
+    int h_box = sq::BLOCK_M, w_box = tile_n / pl.cta_group;
 #ifdef SQ_PROBES
     if (ctx->probe_flags & 4) h_box /= 2;
     if (ctx->probe_flags & 2) w_box /= 2;
@@ -671,6 +690,14 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     if (rc != SQ_OK) return rc;
     rc = make_tmap(ctx, &tw, W, V, d, w_box, f8);
     if (rc != SQ_OK) return rc;
+    tsa = th; tsb = tw;                                    // unused outside the MX variant
+    const int64_t sf_h_blocks = cdiv64(T, sq::BLOCK_M);
+    if (mx) {   // rows of 512 scale bytes: [k-block][128-row block of H], [k-block][vocab tile][2]  (sq_quant_mx_kernel)
+      rc = make_tmap_sf(ctx, &tsa, h_sf, (int64_t)pl.num_k_blocks * sf_h_blocks, 1);
+      if (rc != SQ_OK) return rc;
+      rc = make_tmap_sf(ctx, &tsb, w_sf, (int64_t)pl.num_k_blocks * pl.num_vtiles * 2, 2);
+      if (rc != SQ_OK) return rc;
+    }
 
     sq::FusedParams fp = {};
     fp.T = T; fp.V = V; fp.d = d;
@@ -691,7 +718,7 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fp.probe_flags = ctx->probe_flags;
 #endif
     fp.vocab_offset = vocab_offset;
-    fp.h_scale = h_scale; fp.w_scale = w_scale;
+    fp.h_scale = h_scale; fp.w_scale = w_scale; fp.sf_h_blocks = (int)sf_h_blocks;
     fp.h_ready = h_ready; fp.flag_rows = flag_rows;
     if (pl.num_chunks >= 2 && pl.num_chunks <= THR_MAX_CHUNKS && !(ctx->debug_flags & 16)) {
       // every chunk publishes its j-th best, j one of cap/4, cap/2, cap (compile-time list slots); r = ceil(k / j)
@@ -709,21 +736,29 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     cudaError_t e;
     cudaEvent_t* pev = ctx->profiling ? ctx->ev[ctx->ev_count % SQ_PROFILE_RING] : nullptr;
     if (pev) cudaEventRecord(pev[0], st);
-    const int sel = pl.cta_group * 100 + pl.topk_cap + (f8 ? 1000 : 0);
+    const int sel = pl.cta_group * 100 + pl.topk_cap + (mx ? 2000 : (f8 ? 1000 : 0));
+#define SQ_LAUNCH(CG, CAP, MODE) e = launch_fused<CG, CAP, MODE>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break
     switch (sel) {
-      case 1108: e = launch_fused<1, 8, true>(pl, ctx->num_sms, th, tw, fp, st); break;
-      case 1120: e = launch_fused<1, 20, true>(pl, ctx->num_sms, th, tw, fp, st); break;
-      case 1132: e = launch_fused<1, 32, true>(pl, ctx->num_sms, th, tw, fp, st); break;
-      case 1208: e = launch_fused<2, 8, true>(pl, ctx->num_sms, th, tw, fp, st); break;
-      case 1220: e = launch_fused<2, 20, true>(pl, ctx->num_sms, th, tw, fp, st); break;
-      case 1232: e = launch_fused<2, 32, true>(pl, ctx->num_sms, th, tw, fp, st); break;
-      case 108: e = launch_fused<1, 8>(pl, ctx->num_sms, th, tw, fp, st); break;
-      case 120: e = launch_fused<1, 20>(pl, ctx->num_sms, th, tw, fp, st); break;
-      case 132: e = launch_fused<1, 32>(pl, ctx->num_sms, th, tw, fp, st); break;
-      case 208: e = launch_fused<2, 8>(pl, ctx->num_sms, th, tw, fp, st); break;
-      case 220: e = launch_fused<2, 20>(pl, ctx->num_sms, th, tw, fp, st); break;
-      default: e = launch_fused<2, 32>(pl, ctx->num_sms, th, tw, fp, st); break;
+      case 2108: SQ_LAUNCH(1, 8, sq::MODE_MX);
+      case 2120: SQ_LAUNCH(1, 20, sq::MODE_MX);
+      case 2132: SQ_LAUNCH(1, 32, sq::MODE_MX);
+      case 2208: SQ_LAUNCH(2, 8, sq::MODE_MX);
+      case 2220: SQ_LAUNCH(2, 20, sq::MODE_MX);
+      case 2232: SQ_LAUNCH(2, 32, sq::MODE_MX);
+      case 1108: SQ_LAUNCH(1, 8, sq::MODE_F8);
+      case 1120: SQ_LAUNCH(1, 20, sq::MODE_F8);
+      case 1132: SQ_LAUNCH(1, 32, sq::MODE_F8);
+      case 1208: SQ_LAUNCH(2, 8, sq::MODE_F8);
+      case 1220: SQ_LAUNCH(2, 20, sq::MODE_F8);
+      case 1232: SQ_LAUNCH(2, 32, sq::MODE_F8);
+      case 108: SQ_LAUNCH(1, 8, sq::MODE_BF16);
+      case 120: SQ_LAUNCH(1, 20, sq::MODE_BF16);
+      case 132: SQ_LAUNCH(1, 32, sq::MODE_BF16);
+      case 208: SQ_LAUNCH(2, 8, sq::MODE_BF16);
+      case 220: SQ_LAUNCH(2, 20, sq::MODE_BF16);
+      default: SQ_LAUNCH(2, 32, sq::MODE_BF16);
     }
+#undef SQ_LAUNCH
     if (e != cudaSuccess) return set_err(ctx, SQ_ERR_CUDA, "fused kernel launch failed: %s", cudaGetErrorString(e));
     if (pev) cudaEventRecord(pev[1], st);
 
@@ -827,6 +862,56 @@ extern "C" int sq_score_run_fp8(sq_score_ctx* ctx, const void* Hq, const float* 
   if (num_tokens > 0 && (!h_scale || !w_scale)) return set_err(ctx, SQ_ERR_INVALID_ARG, "h_scale and w_scale are required");
   return run_impl(ctx, Hq, Wq, targets, cu_seqlens, num_tokens, num_seqs, k, window, outputs, stream, nullptr, 0, 0, nullptr,
                   h_scale, w_scale);
+}
+
+// ------------------------------------------------------------------------------------------ block-scaled (MX) variant
+static void mx_geometry(int64_t rows, int d, int operand, int* blk_rows, int* pieces, int64_t* num_blk, int64_t* kblocks) {
+  *blk_rows = operand == SQ_MX_OPERAND_W ? sq::BLOCK_N_MX : sq::BLOCK_M;
+  *pieces = (*blk_rows + 127) / 128;
+  *num_blk = cdiv64(rows, *blk_rows);
+  *kblocks = cdiv64(d, sq::BLOCK_K_F8);
+}
+
+extern "C" int64_t sq_score_mx_scale_bytes(int64_t num_rows, int d, int operand) {
+  if (num_rows < 0 || d < 1 || (operand != SQ_MX_OPERAND_H && operand != SQ_MX_OPERAND_W)) return -1;
+  int blk_rows, pieces; int64_t num_blk, kblocks;
+  mx_geometry(num_rows, d, operand, &blk_rows, &pieces, &num_blk, &kblocks);
+  return kblocks * num_blk * pieces * 512;
+}
+
+extern "C" int sq_score_quantize_mx(sq_score_ctx* ctx, const void* X, int64_t num_rows, int operand, void* q_out, void* sf_out,
+                                    void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (num_rows < 0 || (operand != SQ_MX_OPERAND_H && operand != SQ_MX_OPERAND_W)) return set_err(ctx, SQ_ERR_INVALID_ARG, "bad row count or operand");
+  if (num_rows == 0) return SQ_OK;
+  if (!X || !q_out || !sf_out) return set_err(ctx, SQ_ERR_INVALID_ARG, "null pointer argument");
+  if (ctx->cfg.d % 16 != 0) return set_err(ctx, SQ_ERR_UNSUPPORTED, "the MX variant needs d %% 16 == 0 (TMA 16-byte row strides)");
+  if (((uintptr_t)X & 15) || ((uintptr_t)q_out & 15) || ((uintptr_t)sf_out & 15))
+    return set_err(ctx, SQ_ERR_INVALID_ARG, "X, q_out and sf_out must be 16-byte aligned");
+  SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  sq::QuantMxParams qp = {};
+  int64_t kblocks;
+  mx_geometry(num_rows, ctx->cfg.d, operand, &qp.blk_rows, &qp.pieces, &qp.num_blk, &kblocks);
+  qp.X = static_cast<const uint4*>(X); qp.Q = static_cast<uint2*>(q_out); qp.SF = static_cast<uint8_t*>(sf_out);
+  qp.rows = num_rows; qp.d = ctx->cfg.d;
+  // slots no row or k-block reaches (ragged last blocks) scale zero-filled codes: any value but NaN (0xFF) would do
+  SQ_CUDA(ctx, cudaMemsetAsync(sf_out, 0, (size_t)(kblocks * qp.num_blk * qp.pieces * 512), st));
+  const unsigned ctas = (unsigned)std::min<int64_t>(cdiv64(num_rows, 8), (int64_t)ctx->num_sms * 8);
+  sq::sq_quant_mx_kernel<<<ctas, 256, 0, st>>>(qp);
+  ctx->launches += 1;
+  SQ_CUDA(ctx, cudaGetLastError());
+  return SQ_OK;
+}
+
+extern "C" int sq_score_run_mx(sq_score_ctx* ctx, const void* Hq, const void* h_sf, const void* Wq, const void* w_sf,
+                               const int32_t* targets, const int32_t* cu_seqlens, int num_tokens, int num_seqs, int k,
+                               int window, const sq_score_outputs* outputs, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (num_tokens > 0 && (!h_sf || !w_sf)) return set_err(ctx, SQ_ERR_INVALID_ARG, "h_sf and w_sf are required");
+  if (num_tokens > 0 && (((uintptr_t)h_sf & 15) || ((uintptr_t)w_sf & 15))) return set_err(ctx, SQ_ERR_INVALID_ARG, "h_sf and w_sf must be 16-byte aligned");
+  return run_impl(ctx, Hq, Wq, targets, cu_seqlens, num_tokens, num_seqs, k, window, outputs, stream, nullptr, 0, 0, nullptr,
+                  nullptr, nullptr, 0, h_sf, w_sf);
 }
 
 // ------------------------------------------------------------------------------------------ vocab-parallel (8(f)-4)
