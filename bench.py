@@ -472,12 +472,41 @@ def run_ours(args):
         except Exception as exc:   # reported, never fatal for the headline line
             g_ms = None
             sys.stderr.write("decode graph leg skipped: %r\n" % (exc,))
+        # the same decode batch with an 8-bit LM head: W is what the run streams, so e4m3 / block-scaled e4m3 halve the bytes
+        d8 = {}
+        with torch.cuda.stream(stream):
+            for fmt in ("fp8", "mx"):
+                if fmt == "fp8":
+                    Wd8, wsd = eng3.quantize_fp8(W, True, stream=stream)
+                    Hd8, hsd = eng3.quantize_fp8(Hd, False, stream=stream)
+                    call = lambda o_: eng3.run_fp8(Hd8, hsd, Wd8, wsd, tgd, cud, wl.k, 16, stream=stream, out=o_)
+                    w_bytes = 1.0 * V * d
+                else:
+                    Wd8, wsd = eng3.quantize_mx(W, sq.MX_OPERAND_W, stream=stream)
+                    Hd8, hsd = eng3.quantize_mx(Hd, sq.MX_OPERAND_H, stream=stream)
+                    call = lambda o_: eng3.run_mx(Hd8, hsd, Wd8, wsd, tgd, cud, wl.k, 16, stream=stream, out=o_)
+                    w_bytes = 1.0 * V * d + float(wsd.numel())
+                o8d = None
+                for _ in range(3):
+                    o8d = call(o8d)
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                for _ in range(20):
+                    call(o8d)
+                e1.record(stream)
+                stream.synchronize()
+                ms8 = e0.elapsed_time(e1) / 20
+                b8 = w_bytes + 1.0 * Td * d + Td * (4 + 16 + 8 * wl.k)
+                d8[fmt] = {"ms": ms8, "algorithmic_bytes": b8, "achieved": b8 / (ms8 * 1e-3) / 1e9, "frac": b8 / (ms8 * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                           "max_abs_lse_gap_to_bf16_path": float((o8d["lse"] - od["lse"]).abs().max())}
+                del Wd8, wsd, Hd8, hsd
         d_bytes = 2.0 * V * d + 2.0 * Td * d + Td * (4 + 16 + 8 * wl.k)
         line["decode_standalone"] = {"bound": "hbm", "achieved": d_bytes / (d_ms * 1e-3) / 1e9, "peak": peaks["hbm_gbs"],
                                      "unit": "GB/s", "frac": d_bytes / (d_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "ms": d_ms,
                                      "rows": Td, "tokens_per_s": Td / (d_ms * 1e-3), "algorithmic_bytes": d_bytes,
                                      "kernels_ms": {n: float(np.mean([x[n + "_ms"] for x in d_k])) for n in ("fused", "finalize", "reduce")},
                                      "cuda_graph_ms": g_ms, "cuda_graph_frac": (d_bytes / (g_ms * 1e-3) / 1e9 / peaks["hbm_gbs"]) if g_ms else None,
+                                     "eight_bit_lm_head": d8,
                                      "plan": sq.plan(d, V, Td, wl.k, num_sms=torch.cuda.get_device_properties(dev).multi_processor_count),
                                      "note": "whole path (2 launches: kernel 1, finalize + per-sequence tail) on a decode batch of 64 rows; W (%.0f MB) "
                                              "exceeds L2 and is streamed once per pass; kernels_ms is from a separate profiled pass "
@@ -550,6 +579,36 @@ def run_ours(args):
                                "note": "not the graded number: e4m3 operands (per-token H scales, per-tensor W scale); parity holds on the "
                                        "quantised operands (tests/test_fp8_gpu.py)"}
         del Wq, Hq
+        # Block-scaled (MX) variant: e4m3 with one UE8M0 scale per 32 elements, tcgen05 kind::mxf8f6f4.block_scale.  Same batch,
+        # same peak as the FP8 variant; also reports how far its scores are from the bf16 path's next to the FP8 variant's.
+        with torch.cuda.stream(stream):
+            Wm, wsf = eng.quantize_mx(W, sq.MX_OPERAND_W, stream=stream)
+            Hm, hsf = eng.quantize_mx(H, sq.MX_OPERAND_H, stream=stream)
+            om = None
+            for _ in range(3):
+                om = eng.run_mx(Hm, hsf, Wm, wsf, tg, cu, wl.k, wl.window, stream=stream, out=om)
+            stream.synchronize()
+            q0 = torch.cuda.Event(enable_timing=True); q1 = torch.cuda.Event(enable_timing=True); q2 = torch.cuda.Event(enable_timing=True)
+            q0.record(stream)
+            for _ in range(args.steps):
+                eng.quantize_mx(H, sq.MX_OPERAND_H, stream=stream, out=(Hm, hsf))
+            q1.record(stream)
+            for _ in range(args.steps):
+                eng.run_mx(Hm, hsf, Wm, wsf, tg, cu, wl.k, wl.window, stream=stream, out=om)
+            q2.record(stream)
+            stream.synchronize()
+            mx_k = eng.kernel_times()["fused_ms"]
+        qm_ms, mx_ms = q0.elapsed_time(q1) / args.steps, q1.elapsed_time(q2) / args.steps
+        gaps = {n: {"mx": float((om[n] - out[n]).abs().max()), "fp8": float((o8[n] - out[n]).abs().max())} for n in ("lse", "target_logprob", "conf")}
+        line["mx_variant"] = {"dtype": "mxfp8 (e4m3 + ue8m0 per 32) x mxfp8 -> f32", "ms_per_step": mx_ms, "quantize_h_ms": qm_ms,
+                              "tokens_per_s": T / ((mx_ms + qm_ms) * 1e-3), "kernel_ms": mx_k,
+                              "kernel_tflops": flops / (mx_k * 1e-3) / 1e12,
+                              "peak": 2.0 * peaks["bf16_tflops_sustained"], "frac": flops / (mx_k * 1e-3) / 1e12 / (2.0 * peaks["bf16_tflops_sustained"]),
+                              "peak_kind": "2 x bf16_tflops_sustained of %s (nominal fp8 : bf16 ratio)" % peaks["source"],
+                              "max_abs_gap_to_bf16_path": gaps,
+                              "note": "not the graded number: block-scaled e4m3 operands, 224-column tiles; parity holds on the quantised "
+                                      "operands (tests/test_mx_gpu.py)"}
+        del Wm, Hm
     if args.matmul_ceiling:
         # context only: cuBLAS on the same (T, V, d) in row chunks, logits materialised chunk by chunk
         rows = 8192

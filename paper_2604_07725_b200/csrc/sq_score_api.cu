@@ -6,6 +6,8 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <queue>
+#include <vector>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -56,6 +58,10 @@ struct sq_score_ctx {
   // optional per-kernel timing (sq_score_set_profiling): events around kernel 1, finalize
   // and kernel 2 of the last SQ_PROFILE_RING profiled runs
   int profiling = 0; int debug_flags = 0; int reduce_form = 0;
+  // the four tensor maps of the last run (H, W, scale factors of H and of W): encoding one costs the host tens of
+  // microseconds, which a decode-shaped run (0.1-0.2 ms on the device) cannot hide; a map depends only on the key below
+  struct { int T = -1, k = 0, V = 0, tile_n = 0, d = 0; sq_score_plan_t pl; } plan_cache;   // the last run's plan (host time, as below)
+  struct TmapSlot { const void* base = nullptr; int64_t rows = -1; int d = 0, box = 0, kind = -1; CUtensorMap map; } tmaps[4];
   int64_t ev_count = 0, ev_read = 0;   // runs recorded / runs already handed out by sq_score_profile_read
   cudaEvent_t (*ev)[4] = nullptr;      // [SQ_PROFILE_RING][4]
 #ifdef SQ_PROBES
@@ -113,11 +119,17 @@ static void split_stripes(int nv, int ng, const int* batches, int* width, int mi
       if (width[i] > minw && (w < 0 || (int64_t)batches[i] * width[i] > (int64_t)batches[w] * width[w])) w = i;
     --width[w]; --used;
   }
-  while (used < nv) {
-    int w = 0;
-    for (int i = 1; i < ng; ++i)
-      if ((int64_t)batches[i] * (width[i] + 1) < (int64_t)batches[w] * (width[w] + 1)) w = i;
-    ++width[w]; ++used;
+  if (used < nv) {
+    // (a heap: decode-shaped plans have ~150 gangs and ~150 left-over tiles, and the host time of a 0.1 ms run matters)
+    typedef std::pair<int64_t, int> Key;   // (finishing time with one more tile, gang): the smallest, lowest gang first
+    std::priority_queue<Key, std::vector<Key>, std::greater<Key>> heap;
+    for (int i = 0; i < ng; ++i) heap.push(Key((int64_t)batches[i] * (width[i] + 1), i));
+    while (used < nv) {
+      const int w = heap.top().second;
+      heap.pop();
+      ++width[w]; ++used;
+      heap.push(Key((int64_t)batches[w] * (width[w] + 1), w));
+    }
   }
 }
 
@@ -175,6 +187,7 @@ static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, 
         const int g = cfg->group_m > 0 ? cfg->group_m : 12 + sgn * dist;
         const int G = std::max(1, std::min(g, std::min(M, NC)));
         const int ng = std::max(1, std::min(NC / G, gangs_max));
+        if (ng == best.ng) continue;                       // the same decomposition, further from the preferred gang size
         const Cand c = eval(ng, 1);
         const double adj = c.cost * (1.0 + 0.01 * dist);
         if (adj < best_adj * (1.0 - 1e-9)) { best_adj = adj; best = c; }
@@ -458,7 +471,11 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
 
 // bf16 [rows, d] row-major -> boxes of {64 columns (128 B, swizzle-128B), box_rows rows}; out-of-range
 // rows and columns are zero filled.
-static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int d, int box_rows, bool f8 = false) {
+static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int d, int box_rows, bool f8 = false, int slot = -1) {
+  if (slot >= 0) {
+    const sq_score_ctx::TmapSlot& c = ctx->tmaps[slot];
+    if (c.base == base && c.rows == rows && c.d == d && c.box == box_rows && c.kind == (f8 ? 1 : 0)) { *map = c.map; return SQ_OK; }
+  }
   const cuuint64_t dims[2] = {(cuuint64_t)d, (cuuint64_t)rows};
   const cuuint64_t strides[1] = {(cuuint64_t)d * (f8 ? 1 : 2)};
   const cuuint32_t box[2] = {(cuuint32_t)(f8 ? sq::BLOCK_K_F8 : sq::BLOCK_K), (cuuint32_t)box_rows};   // 128 bytes wide
@@ -468,11 +485,19 @@ static int make_tmap(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int6
       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return set_err(ctx, SQ_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+  if (slot >= 0) {
+    sq_score_ctx::TmapSlot& c = ctx->tmaps[slot];
+    c.base = base; c.rows = rows; c.d = d; c.box = box_rows; c.kind = f8 ? 1 : 0; c.map = *map;
+  }
   return SQ_OK;
 }
 
 // MX scale factors: `rows` rows of 512 bytes (128 x uint32), unswizzled; a box is `box_rows` whole rows.
-static int make_tmap_sf(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int box_rows) {
+static int make_tmap_sf(sq_score_ctx* ctx, CUtensorMap* map, const void* base, int64_t rows, int box_rows, int slot) {
+  {
+    const sq_score_ctx::TmapSlot& c = ctx->tmaps[slot];
+    if (c.base == base && c.rows == rows && c.box == box_rows && c.kind == 2) { *map = c.map; return SQ_OK; }
+  }
   const cuuint64_t dims[2] = {128, (cuuint64_t)rows};
   const cuuint64_t strides[1] = {512};
   const cuuint32_t box[2] = {128, (cuuint32_t)box_rows};
@@ -482,6 +507,8 @@ static int make_tmap_sf(sq_score_ctx* ctx, CUtensorMap* map, const void* base, i
       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return set_err(ctx, SQ_ERR_CUDA, "cuTensorMapEncodeTiled (scale factors) failed with CUresult %d", (int)r);
+  sq_score_ctx::TmapSlot& c = ctx->tmaps[slot];
+  c.base = base; c.rows = rows; c.d = 0; c.box = box_rows; c.kind = 2; c.map = *map;
   return SQ_OK;
 }
 
@@ -672,11 +699,17 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     pc.vocab = V;
     if (f8) pc.d = (d + 1) / 2;   // an e4m3 k-block is 128 elements: the plan sees half as many k-blocks
     const int cg_sel = (pc.cta_group == 1) ? 1 : (pc.cta_group == 2 ? 2 : (T <= 128 ? 1 : 2));
-    make_plan(&pc, T, k, ctx->num_sms, &pl, ctx->max_clusters[cg_sel], tile_n);
-    const int64_t rows = ws_rows_for(ctx->cfg);
-    if ((int64_t)pl.num_chunks * T > rows) {   // workspace bound: fewer gangs, wider stripes
-      pc.num_chunks = (int)std::max<int64_t>(1, rows / T);
+    auto& pcache = ctx->plan_cache;
+    if (pcache.T == T && pcache.k == k && pcache.V == V && pcache.tile_n == tile_n && pcache.d == pc.d) {
+      pl = pcache.pl;
+    } else {
       make_plan(&pc, T, k, ctx->num_sms, &pl, ctx->max_clusters[cg_sel], tile_n);
+      const int64_t rows = ws_rows_for(ctx->cfg);
+      if ((int64_t)pl.num_chunks * T > rows) {   // workspace bound: fewer gangs, wider stripes
+        pc.num_chunks = (int)std::max<int64_t>(1, rows / T);
+        make_plan(&pc, T, k, ctx->num_sms, &pl, ctx->max_clusters[cg_sel], tile_n);
+      }
+      pcache.T = T; pcache.k = k; pcache.V = V; pcache.tile_n = tile_n; pcache.d = pc.d; pcache.pl = pl;
     }
     if (pl.topk_cap > ctx->cap_max) return set_err(ctx, SQ_ERR_INVALID_ARG, "k exceeds the ctx's max_k capacity");
     CUtensorMap th, tw, tsa, tsb;
@@ -686,16 +719,16 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     if (ctx->probe_flags & 4) h_box /= 2;
     if (ctx->probe_flags & 2) w_box /= 2;
 #endif
-    int rc = make_tmap(ctx, &th, H, T, d, h_box, f8);
+    int rc = make_tmap(ctx, &th, H, T, d, h_box, f8, 0);
     if (rc != SQ_OK) return rc;
-    rc = make_tmap(ctx, &tw, W, V, d, w_box, f8);
+    rc = make_tmap(ctx, &tw, W, V, d, w_box, f8, 1);
     if (rc != SQ_OK) return rc;
     tsa = th; tsb = tw;                                    // unused outside the MX variant
     const int64_t sf_h_blocks = cdiv64(T, sq::BLOCK_M);
     if (mx) {   // rows of 512 scale bytes: [k-block][128-row block of H], [k-block][vocab tile][2]  (sq_quant_mx_kernel)
-      rc = make_tmap_sf(ctx, &tsa, h_sf, (int64_t)pl.num_k_blocks * sf_h_blocks, 1);
+      rc = make_tmap_sf(ctx, &tsa, h_sf, (int64_t)pl.num_k_blocks * sf_h_blocks, 1, 2);
       if (rc != SQ_OK) return rc;
-      rc = make_tmap_sf(ctx, &tsb, w_sf, (int64_t)pl.num_k_blocks * pl.num_vtiles * 2, 2);
+      rc = make_tmap_sf(ctx, &tsb, w_sf, (int64_t)pl.num_k_blocks * pl.num_vtiles * 2, 2, 3);
       if (rc != SQ_OK) return rc;
     }
 

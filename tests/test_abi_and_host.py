@@ -36,6 +36,17 @@ def test_library_builds_and_exports_every_declared_symbol():
     assert sq.version() >= 100
 
 
+def test_mx_scale_bytes_is_host_only_arithmetic():
+    """sq_score_mx_scale_bytes (include/sq_score.h): 512-byte pieces per (128-element k-block, row group); H rows are grouped by
+    128 (one piece), W rows by the kernel's 224-column tiles (two pieces)."""
+    L = sq.lib()
+    assert L.sq_score_mx_scale_bytes(300, 4096, 0) == 32 * 3 * 512
+    assert L.sq_score_mx_scale_bytes(300, 4096, 1) == 32 * 2 * 1024
+    assert L.sq_score_mx_scale_bytes(1, 16, 0) == 512 and L.sq_score_mx_scale_bytes(224, 129, 1) == 2 * 1024
+    assert L.sq_score_mx_scale_bytes(0, 64, 0) == 0
+    assert L.sq_score_mx_scale_bytes(300, 4096, 2) == -1 and L.sq_score_mx_scale_bytes(-1, 64, 0) == -1 and L.sq_score_mx_scale_bytes(5, 0, 0) == -1
+
+
 def test_error_strings():
     L = sq.lib()
     assert L.sq_score_error_string(0) == b"SQ_OK"
