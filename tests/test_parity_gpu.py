@@ -534,6 +534,36 @@ def test_reduce_streaming_form_many_sequences_per_range_and_one_long_sequence():
     eng.close()
 
 
+def test_scoring_pipeline_takes_the_streaming_form_for_many_sequences():
+    """sq_score_run on a population of 2 300 candidates (more than one wave of kernel-2 tiles): kernel 1 -> finalize ->
+    streaming form of kernel 2, chained by programmatic dependent launches.  The per-sequence outputs against oracle-B
+    (fp64 reductions of the GPU's own per-token outputs), invalid targets included, and a sample of rows against oracle-A."""
+    sq = _sq()
+    wl = workloads.custom(name="many", d=64, V=512, B=2300, len_lo=90, len_hi=420, k=5, window=128, seed=88, w_std=0.05,
+                          planted_frac=0.5, planted_scale=3.0, rmsnorm=True)
+    inp = workloads.make_inputs(wl)
+    tg = inp["targets"].clone()
+    tg[torch.rand(inp["T"], generator=torch.Generator().manual_seed(3)) < 0.1] = -1
+    dev = torch.device("cuda:0")
+    eng = sq.SqScore(wl.d, wl.V, max_tokens=inp["T"], max_seqs=inp["B"], max_k=wl.k)
+    out = eng.run(inp["H"].to(dev), inp["W"].to(dev), tg.to(dev), inp["cu_seqlens"].to(dev), wl.k, wl.window)
+    torch.cuda.synchronize()
+    assert eng.reduce_form() == "stream"
+    out2 = eng.run(inp["H"].to(dev), inp["W"].to(dev), tg.to(dev), inp["cu_seqlens"].to(dev), wl.k, wl.window)
+    torch.cuda.synchronize()
+    for n in SEQ_KEYS:
+        assert torch.equal(out[n], out2[n], ) or (torch.isnan(out[n]) == torch.isnan(out2[n])).all()
+    eng.close()
+    out = {n: v.cpu().numpy() for n, v in out.items()}
+    valid = ((tg >= 0) & (tg < wl.V)).numpy()
+    seq_ref = O.sequence_scores(out["target_logprob"], out["entropy"], out["conf"], inp["cu_seqlens"].numpy(), wl.window, target_valid=valid)
+    check_seqs(out, seq_ref)
+    rows = np.unique(np.random.default_rng(8).integers(0, inp["T"], 300))
+    rows = rows[valid[rows]]
+    ref = O.token_scores(inp["H"][rows], O.widen(inp["W"]), tg.numpy()[rows], wl.k)
+    check_tokens(out, ref, wl.k, rows=rows)
+
+
 # ------------------------------------------------------------------------------------------ API behaviour
 def test_run_host_matches_run_and_null_per_token_outputs():
     sq = _sq()
