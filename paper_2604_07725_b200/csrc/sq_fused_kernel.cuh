@@ -63,6 +63,9 @@ struct FusedParams {
   int gangs_big;
   int chunks_per_gang;      // a gang's vocabulary stripe is cut into this many chunks
   unsigned int* gang_ctr;   // [num_gangs], zeroed before the launch
+  unsigned int* region_ctr; // one more counter, zeroed with them: clusters that have finished a region of token tiles
+  int region_tiles;         // 0, or: no cluster starts token tile region_tiles * r before every cluster has finished the tiles
+  int region_arrivals;      //   below it (r = 1, 2, ...); CTAs that arrive per region (a multiple of every gang size in tiles)
   long long wait_limit;     // clock cycles a wait may last before the kernel traps (0 = wait for ever)
   const int32_t* targets;   // [T]
   float* part_m;            // [C][T]
@@ -361,6 +364,15 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
       for (int gu = 0; gu < gc.num_iters; ++gu) {
         Unit un;
         const bool active = decode_gang_unit(p, gc, gu, un);
+        if (p.region_tiles > 0 && gu > 0 && gu % p.chunks_per_gang == 0) {
+          // Gangs of different size or stripe width walk the token tiles at slightly different paces.  Over thousands of
+          // tiles they drift apart, the H strips they were sharing stop being shared, and the live set outgrows the L2
+          // (qwen3_32b: 1.31 TB of DRAM reads per launch, 70 % L2 hits, the clock down to 1.05 GHz under the power cap).
+          // A barrier across ALL clusters every region_tiles token tiles bounds the drift to one region's mismatch.
+          const int t0 = (gu / p.chunks_per_gang) * gc.size;   // first token tile of this batch
+          if (t0 % p.region_tiles == 0)
+            gang_barrier(p.region_ctr, (unsigned)(t0 / p.region_tiles) * (unsigned)p.region_arrivals, p.wait_limit);
+        }
         if (gc.size > 1) gang_barrier(p.gang_ctr + gc.ctr, (++epoch) * (unsigned)(gc.size * CG), p.wait_limit);
         if (!active) continue;
         const int row0 = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M;

@@ -46,6 +46,7 @@ struct sq_score_ctx {
   int* seq_done = nullptr;   // [max_seqs] per-sequence tile counters of the single-launch reduction (zero between runs)
   int* tile_base = nullptr; int* tile_seq = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
   int max_clusters[3] = {0, 0, 0};   // [cg]: clusters of kernel 1 the device holds at once (occupancy query at create)
+  int region_mult = 0;               // region barrier of kernel 1: regions of region_mult x (a common multiple of the gang sizes) token tiles; < 0: off
   long long wait_limit = 0;          // cycles a device-side wait may last before kernel 1 traps (0 = for ever)
   int* pos_base = nullptr;           // [max_seqs + 1] packed start of every candidate (sq_score_positions)
   // staging for sq_score_run_host / sq_score_run_x (SQ_FLAG_STAGING)
@@ -348,6 +349,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
     int khz = 0;
     cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, cfg->device);
     long long sec = cfg->wait_seconds == 0 ? 60 : cfg->wait_seconds;
+    if (const char* rm = getenv("SQ_SCORE_REGION_MULT")) ctx->region_mult = atoi(rm);   // experiment knob (same results): -1 = no region barrier
     if (const char* w = getenv("SQ_SCORE_WAIT_SECONDS")) sec = atoll(w) == 0 ? -1 : atoll(w);
     ctx->wait_limit = sec < 0 ? 0 : sec * (long long)std::max(khz, 1000000) * 1000LL;
   }
@@ -739,6 +741,13 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fp.num_gangs = pl.num_gangs; fp.gang_size = pl.gang_size; fp.gangs_big = pl.gangs_big;
     fp.chunks_per_gang = pl.chunks_per_gang; fp.gang_ctr = ctx->gang_ctr;
     fp.wait_limit = ctx->wait_limit;
+    // region barrier (sq_fused_kernel.cuh): a region is a number of token tiles that every gang covers in whole batches
+    fp.region_ctr = ctx->gang_ctr + 255; fp.region_tiles = 0; fp.region_arrivals = pl.clusters_used * pl.cta_group;
+    if (pl.num_gangs > 1 && pl.gang_size + (pl.gangs_big > 0 ? 1 : 0) > 1) {
+      const int unit = pl.gangs_big > 0 && pl.gangs_big < pl.num_gangs ? pl.gang_size * (pl.gang_size + 1) : pl.gang_size + (pl.gangs_big > 0 ? 1 : 0);
+      const int mult = ctx->region_mult > 0 ? ctx->region_mult : std::max(1, 160 / unit);   // default: regions of ~160 token tiles
+      if (ctx->region_mult >= 0 && unit * mult < pl.m_tiles) fp.region_tiles = unit * mult;
+    }
     for (int c = 0; c <= pl.num_chunks; ++c) fp.chunk_vt[c] = (uint16_t)pl.chunk_vtile[c];
     // the gang barrier counters only matter when some gang has more than one member (not in decode-shaped plans)
     if (pl.gang_size + (pl.gangs_big > 0 ? 1 : 0) > 1)
