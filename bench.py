@@ -10,7 +10,8 @@ config the metric's 60 % target is quoted on); the other four configs are timed 
   --parallelism dp     (default) every rank scores its own batch of the same shape (sequences shard across
                        GPUs, W replicated) and the step ends with the path's one exchange, the all-gather
                        of the 4 scalars per sequence: weak scaling;
-  --parallelism vocab  the LM head is split by rows over the ranks (tensor-parallel scorer): every rank scores
+  --parallelism vocab  (or vocab-peer: the same without the all-gather, peers' states read in place over NVLink)
+                       the LM head is split by rows over the ranks (tensor-parallel scorer): every rank scores
                        the SAME batch against its shard, one all-gather of the packed partial states, then the
                        merge on every rank: strong scaling.
 One JSON line is printed by rank 0.
@@ -200,7 +201,8 @@ def run_ours(args):
         raise SystemExit("bench.py: no CUDA device; the sq_score path has no CPU fallback")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    vocab_mode = args.parallelism == "vocab"
+    vocab_mode = args.parallelism in ("vocab", "vocab-peer")
+    peer_mode = args.parallelism == "vocab-peer"
     use_dist = world > 1 or vocab_mode          # vocab mode runs its collective through NCCL even at world size 1
     if use_dist:
         import torch.distributed as dist
@@ -231,8 +233,17 @@ def run_ours(args):
                          cta_group=args.cta_group, num_chunks=args.num_chunks, group_m=args.group_m)
         pl = sq.plan(d, max(1, W.shape[0]), T, wl.k, num_sms=sms, cta_group=args.cta_group, num_chunks=args.num_chunks, group_m=args.group_m)
         exchange_bytes = world * sq.shard_state_bytes(T, wl.k)
-        def step_fn(o):
-            return sharding.score_vocab_parallel(eng, H, W, vstarts, rank, tg, cu, wl.k, wl.window, stream=stream)
+        if peer_mode:
+            # no all-gather: every rank's state stays in its own buffer, opened once by the peers (CUDA IPC over NVLink); the merge
+            # kernel reads the R states in place; two 4-byte all-reduces per step order writers and readers on the stream
+            exchange_bytes = (world - 1) * sq.shard_state_bytes(T, wl.k)
+            my_state = torch.empty(sq.shard_state_bytes(T, wl.k) // 4, dtype=torch.float32, device=dev)
+            peers = sharding.PeerStates(my_state, rank, world)
+            def step_fn(o):
+                return sharding.score_vocab_parallel_peer(eng, peers, H, W, vstarts, tg, cu, wl.k, wl.window, stream=stream)
+        else:
+            def step_fn(o):
+                return sharding.score_vocab_parallel(eng, H, W, vstarts, rank, tg, cu, wl.k, wl.window, stream=stream)
     else:
         W = inp["W"].to(dev)
         eng = sq.SqScore(d, V, max_tokens=T, max_seqs=B, max_k=wl.k, device=local, staging=True,
@@ -320,7 +331,8 @@ def run_ours(args):
                 if ln.startswith("sq_fused_score_kernel,"):
                     traffic = float(ln.strip().split(",")[1])
                     traffic_source = "profiles/traffic_%s.csv (ncu --set full of this kernel, committed; not measured in this run)" % wl.name
-    par = ("vocab%d (LM head split by rows, one all-gather of the packed partial states per step)" % world) if vocab_mode else \
+    par = ("vocab%d (LM head split by rows, %s)" % (world, "peers' partial states read in place by the merge kernel, two 4-byte all-reduces per step"
+                                                    if peer_mode else "one all-gather of the packed partial states per step")) if vocab_mode else \
           ("dp%d (sequences sharded, W replicated%s)" % (world, "; one all-gather of 5 floats per sequence per step" if use_dist else ""))
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
@@ -668,7 +680,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="qwen3_8b", choices=list(workloads.CONFIGS))
     ap.add_argument("--e2e-steps", type=int, default=10)
-    ap.add_argument("--parallelism", default="dp", choices=["dp", "vocab"])
+    ap.add_argument("--parallelism", default="dp", choices=["dp", "vocab", "vocab-peer"])
     ap.add_argument("--no-all-configs", action="store_true", help="skip the brief timing of the other four configs")
     ap.add_argument("--oracle-seconds", type=float, default=None)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -307,6 +307,18 @@ int sq_score_merge_shards(sq_score_ctx *ctx, const void *states, int num_shards,
                           const int32_t *targets, const int32_t *cu_seqlens, int num_tokens, int num_seqs,
                           int k, int window, const sq_score_outputs *outputs, void *stream);
 
+/* The same merge WITHOUT the all-gather: state_ptrs (HOST array of num_shards DEVICE pointers) names one packed state per
+ * shard wherever it lives in the unified address space -- this GPU's own buffer and the peers' buffers mapped over
+ * NVLink (cudaIpcOpenMemHandle / peer access).  The merge kernel reads every shard's state in place, lane r = shard r, so
+ * the transfer is the merge's own loads: no staging copy of R x state bytes, and the exchange overlaps the merge row by
+ * row.  The caller orders the run: every shard's sq_score_run_shard must have completed before this call's kernels start
+ * (paper_2604_07725_b200/sharding.py: a 4-byte all-reduce on the stream), and a state must not be overwritten while a peer
+ * may still read it.  Pointers must be 4-byte aligned.  Errors: INVALID_ARG, CUDA. */
+int sq_score_merge_shards_peer(sq_score_ctx *ctx, const void *const *state_ptrs, int num_shards,
+                               const int32_t *vocab_starts, const int32_t *targets, const int32_t *cu_seqlens,
+                               int num_tokens, int num_seqs, int k, int window, const sq_score_outputs *outputs,
+                               void *stream);
+
 /* Group fitness and routing on the device, one problem per CTA:
  *   group_fitness[g] = GC(g) = (1/K) * sum_{j<K} seq_conf[group_members[g*K+j]]   Eq. 4 right
  *   theta[q] = Percentile_p of GC over problem q's non-lite groups                Eq. 6

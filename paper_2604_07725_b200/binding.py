@@ -94,6 +94,9 @@ def lib() -> C.CDLL:
     L.sq_score_merge_shards.restype = C.c_int
     L.sq_score_quantize_fp8.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
     L.sq_score_quantize_fp8.restype = C.c_int
+    L.sq_score_merge_shards_peer.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
+                                             C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
+    L.sq_score_merge_shards_peer.restype = C.c_int
     L.sq_score_run_fp8.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int,
                                    C.c_int, C.c_int, C.POINTER(sq_score_outputs), C.c_void_p]
     L.sq_score_run_fp8.restype = C.c_int
@@ -283,6 +286,23 @@ class SqScore:
         vs = (C.c_int32 * (R + 1))(*[int(v) for v in vocab_starts])
         self._check(self._L.sq_score_merge_shards(self._h, _ptr(states), R, vs, _ptr(targets), _ptr(cu_seqlens), T, B, k, window,
                                                   C.byref(o), self._stream(stream)))
+        return out
+
+    def merge_shards_peer(self, states: Sequence, vocab_starts: Sequence[int], targets, cu_seqlens, k: int, window: int, stream=None,
+                          per_token: bool = True, topk: bool = True, out: Optional[dict] = None) -> dict:
+        """sq_score_merge_shards_peer: `states` is a list of R tensors (or raw device addresses), one packed state per
+        shard, read in place -- peers' buffers included."""
+        R = len(vocab_starts) - 1
+        if len(states) != R:
+            raise ValueError("%d states for %d shards" % (len(states), R))
+        T, B = targets.shape[0], cu_seqlens.shape[0] - 1
+        if out is None:
+            out = self._alloc_out(T, B, k, targets.device, per_token, topk)
+        o = sq_score_outputs(*[_ptr(out.get(n)) for n, _ in sq_score_outputs._fields_])
+        vs = (C.c_int32 * (R + 1))(*[int(v) for v in vocab_starts])
+        ptrs = (C.c_void_p * R)(*[(st if isinstance(st, int) else st.data_ptr()) for st in states])
+        self._check(self._L.sq_score_merge_shards_peer(self._h, ptrs, R, vs, _ptr(targets), _ptr(cu_seqlens), T, B, k, window,
+                                                       C.byref(o), self._stream(stream)))
         return out
 
     def quantize_fp8(self, X, per_tensor: bool, stream=None, out=None):

@@ -17,11 +17,13 @@ namespace sq {
 struct FinalizeParams {
   int T, V, k, cap, num_chunks;
   // Partial states may come from several vocab-parallel shards ("ranks"): chunk c lives in rank c / chunks_per_rank,
-  // whose arrays start rank_stride 4-byte words after the previous rank's (one packed state buffer per rank, gathered
-  // back to back).  One rank: chunks_per_rank = num_chunks, rank_stride = 0.
+  // whose arrays start rank_off[r] 4-byte words after rank 0's: r * (words of a packed state) when the states were
+  // gathered back to back (sq_score_merge_shards), or the distance between two buffers anywhere in the unified address
+  // space -- the peers' own state buffers, read in place over NVLink (sq_score_merge_shards_peer).  One rank:
+  // chunks_per_rank = num_chunks, rank_off[0] = 0.
   int chunks_per_rank;
-  long long rank_stride;
   int num_ranks;
+  long long rank_off[32];
   int vstart[33];           // ranks > 1: rank r owns vocabulary ids [vstart[r], vstart[r+1]) -- whose zt is the target's
   int vocab_offset;         // EMIT mode: this shard's columns are global ids [vocab_offset, vocab_offset + V)
   // EMIT mode (sq_score_run_shard): instead of finalising, write the merged state as ONE chunk in the same format
@@ -133,13 +135,13 @@ __device__ __forceinline__ void fin_merge_rows(const FinalizeParams& p) {
   const float NEG = -1.0e30f;
   // lane owns chunks lane, lane + 32, ... (one per lane in the prefill-shaped plans, up to
   // NL in the decode-shaped ones where every SM sweeps its own slice of the vocabulary)
-  size_t base1[NL], basek[NL];   // word offsets of this lane's chunks: scalar arrays / first list entry
+  long long base1[NL], basek[NL];   // word offsets of this lane's chunks (signed: a peer's buffer may lie below rank 0's)
 #pragma unroll
   for (int i = 0; i < NL; ++i) {
     const int c = lane + 32 * i;
     const int r = c / p.chunks_per_rank, cl = c - r * p.chunks_per_rank;
-    base1[i] = (size_t)r * p.rank_stride + (size_t)cl * p.T + row;
-    basek[i] = (size_t)r * p.rank_stride + (size_t)cl * p.cap * p.T + row;
+    base1[i] = (long long)p.rank_off[r & 31] + (long long)cl * p.T + row;
+    basek[i] = (long long)p.rank_off[r & 31] + (long long)cl * p.cap * p.T + row;
   }
   float M = NEG;
 #pragma unroll
@@ -155,7 +157,7 @@ __device__ __forceinline__ void fin_merge_rows(const FinalizeParams& p) {
   for (int i = 0; i < NL; ++i) {
     const int c = lane + 32 * i;
     if (c < p.num_chunks) {
-      const size_t o = base1[i];
+      const long long o = base1[i];
       const double s_c = (double)p.part_s[o] - (double)p.part_cs[o];
       const double u_c = (double)p.part_u[o] - (double)p.part_cu[o];
       const double dm = (double)p.part_m[o] - (double)M;
@@ -183,7 +185,7 @@ __device__ __forceinline__ void fin_merge_rows(const FinalizeParams& p) {
     const int c = lane + 32 * i;
     v = NEG; id = -1;
     if (c < p.num_chunks && at < p.cap) {
-      const size_t oj = basek[i] + (size_t)at * p.T;
+      const long long oj = basek[i] + (long long)at * p.T;
       v = p.part_topv[oj];
       id = p.part_topi[oj];
     }
@@ -260,11 +262,11 @@ __device__ __forceinline__ void fin_merge_rows(const FinalizeParams& p) {
   if (lane == 0 && live) {
     const int tgt = p.targets[row];
     const bool valid = (tgt >= 0) && (tgt < p.V);
-    size_t zo = row;
+    long long zo = row;
     if (p.num_ranks > 1 && valid) {
       int r = 0;
       while (r + 1 < p.num_ranks && tgt >= p.vstart[r + 1]) ++r;
-      zo += (size_t)r * p.rank_stride;
+      zo += p.rank_off[r];
     }
     p.lse[row] = lse;
     p.target_logprob[row] = valid ? (p.zt[zo] - lse) : 0.f;
@@ -330,8 +332,8 @@ sq_finalize_wide_kernel(const FinalizeParams p) {
   const float NEG = -1.0e30f, EMPTY = -1.0e20f;     // list values below EMPTY are unfilled slots (no logit is that small)
   const bool has = c < p.num_chunks;
   const int r = has ? c / p.chunks_per_rank : 0, cl = has ? c - r * p.chunks_per_rank : 0;
-  const size_t base1 = (size_t)r * p.rank_stride + (size_t)cl * p.T + row;
-  const size_t basek = (size_t)r * p.rank_stride + (size_t)cl * p.cap * p.T + row;
+  const long long base1 = p.rank_off[r & 31] + (long long)cl * p.T + row;
+  const long long basek = p.rank_off[r & 31] + (long long)cl * p.cap * p.T + row;
   // ---- every load this thread needs, issued together: the chunk's statistics and its whole list of values
   float m_c = NEG, s_c = 0.f, cs_c = 0.f, u_c = 0.f, cu_c = 0.f;
   float lv[CAP];
@@ -340,7 +342,7 @@ sq_finalize_wide_kernel(const FinalizeParams p) {
   if (has) {
     m_c = p.part_m[base1]; s_c = p.part_s[base1]; cs_c = p.part_cs[base1]; u_c = p.part_u[base1]; cu_c = p.part_cu[base1];
 #pragma unroll
-    for (int j = 0; j < CAP; ++j) lv[j] = p.part_topv[basek + (size_t)j * p.T];
+    for (int j = 0; j < CAP; ++j) lv[j] = p.part_topv[basek + (long long)j * p.T];
   }
   float M = m_c;
 #pragma unroll
@@ -400,7 +402,7 @@ sq_finalize_wide_kernel(const FinalizeParams p) {
     const int at = j < cnt_gt ? base_gt + j : base_eq + (j - cnt_gt);
     if (j < cnt_ge && at < FIN_WIDE_CAND) {
       s_cv[at] = lv[j];
-      s_ci[at] = p.part_topi[basek + (size_t)j * p.T];
+      s_ci[at] = p.part_topi[basek + (long long)j * p.T];
     }
   }
   if (c < 32) s_win[c] = NEG;

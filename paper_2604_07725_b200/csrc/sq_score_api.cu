@@ -812,7 +812,7 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fin.part_topv = ctx->part_topv; fin.part_topi = ctx->part_topi; fin.zt = ctx->zt;
     fin.lse = lse; fin.target_logprob = lp; fin.entropy = ent; fin.conf = conf;
     fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
-    fin.chunks_per_rank = pl.num_chunks; fin.rank_stride = 0; fin.num_ranks = 1;
+    fin.chunks_per_rank = pl.num_chunks; fin.num_ranks = 1;   // (rank_off[0] = 0)
     fin.vocab_offset = vocab_offset;
     // a small run (decode-shaped): kernel 2 would be pure launch latency, the finalize kernel's last CTA does its work
     const bool tail = !shard_state && B > 0 && T <= sq::FIN_TAIL_MAX_T;
@@ -990,9 +990,10 @@ extern "C" int sq_score_neutral_shard_state(sq_score_ctx* ctx, int num_tokens, i
   return SQ_OK;
 }
 
-extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int num_shards, const int32_t* vocab_starts,
-                                     const int32_t* targets, const int32_t* cu_seqlens, int num_tokens, int num_seqs,
-                                     int k, int window, const sq_score_outputs* o, void* stream) {
+// `states`: the R packed states back to back, or null with `peers`: R pointers to one packed state each (HOST array)
+static int merge_impl(sq_score_ctx* ctx, const void* states, const void* const* peers, int num_shards, const int32_t* vocab_starts,
+                      const int32_t* targets, const int32_t* cu_seqlens, int num_tokens, int num_seqs,
+                      int k, int window, const sq_score_outputs* o, void* stream) {
   if (!ctx) return SQ_ERR_INVALID_ARG;
   if (!o) return set_err(ctx, SQ_ERR_INVALID_ARG, "outputs is null");
   if (ctx->cfg.flags & SQ_FLAG_REDUCE_ONLY) return set_err(ctx, SQ_ERR_INVALID_ARG, "ctx was created with SQ_FLAG_REDUCE_ONLY");
@@ -1007,7 +1008,10 @@ extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int 
   if (window < 1) return set_err(ctx, SQ_ERR_INVALID_ARG, "window must be >= 1");
   if (B > 0 && (!cu_seqlens || !o->seq_mean_logprob || !o->seq_mean_entropy || !o->seq_mean_conf || !o->seq_min_window_conf))
     return set_err(ctx, SQ_ERR_INVALID_ARG, "cu_seqlens and the four per-sequence outputs are required");
-  if (T > 0 && (!states || !targets)) return set_err(ctx, SQ_ERR_INVALID_ARG, "states and targets are required");
+  if (T > 0 && ((!states && !peers) || !targets)) return set_err(ctx, SQ_ERR_INVALID_ARG, "states and targets are required");
+  if (T > 0 && peers)
+    for (int r = 0; r < num_shards; ++r)
+      if (!peers[r] || ((uintptr_t)peers[r] & 3)) return set_err(ctx, SQ_ERR_INVALID_ARG, "state pointer %d is null or not 4-byte aligned", r);
   SQ_CUDA(ctx, cudaSetDevice(ctx->cfg.device));
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   float* lse = o->lse ? o->lse : ctx->tok_lse;
@@ -1018,10 +1022,13 @@ extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int 
     const int cap = topk_cap_for(k);
     sq::FinalizeParams fin = {};
     fin.T = T; fin.V = Vg; fin.k = k; fin.cap = cap; fin.num_chunks = num_shards;
-    fin.chunks_per_rank = 1; fin.rank_stride = shard_state_words(T, cap); fin.num_ranks = num_shards;
+    fin.chunks_per_rank = 1; fin.num_ranks = num_shards;
+    const void* base = peers ? peers[0] : states;
+    for (int r = 0; r < num_shards; ++r)   // distance of rank r's state from rank 0's, in words (any sign)
+      fin.rank_off[r] = peers ? (long long)((intptr_t)peers[r] - (intptr_t)base) / 4 : (long long)r * shard_state_words(T, cap);
     for (int r = 0; r <= num_shards; ++r) fin.vstart[r] = vocab_starts[r];
     fin.targets = targets;
-    set_state_pointers(fin, const_cast<float*>(static_cast<const float*>(states)), T, cap, /*as_output=*/false);
+    set_state_pointers(fin, const_cast<float*>(static_cast<const float*>(base)), T, cap, /*as_output=*/false);
     fin.lse = lse; fin.target_logprob = lp; fin.entropy = ent; fin.conf = conf;
     fin.topk_logprob = o->topk_logprob; fin.topk_index = o->topk_index;
     if (num_shards <= 8)
@@ -1042,6 +1049,20 @@ extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int 
     if (rc != SQ_OK) return rc;
   }
   return SQ_OK;
+}
+
+extern "C" int sq_score_merge_shards(sq_score_ctx* ctx, const void* states, int num_shards, const int32_t* vocab_starts,
+                                     const int32_t* targets, const int32_t* cu_seqlens, int num_tokens, int num_seqs,
+                                     int k, int window, const sq_score_outputs* o, void* stream) {
+  return merge_impl(ctx, states, nullptr, num_shards, vocab_starts, targets, cu_seqlens, num_tokens, num_seqs, k, window, o, stream);
+}
+
+extern "C" int sq_score_merge_shards_peer(sq_score_ctx* ctx, const void* const* state_ptrs, int num_shards,
+                                          const int32_t* vocab_starts, const int32_t* targets, const int32_t* cu_seqlens,
+                                          int num_tokens, int num_seqs, int k, int window, const sq_score_outputs* o, void* stream) {
+  if (!ctx) return SQ_ERR_INVALID_ARG;
+  if (!state_ptrs) return set_err(ctx, SQ_ERR_INVALID_ARG, "state_ptrs is null");
+  return merge_impl(ctx, nullptr, state_ptrs, num_shards, vocab_starts, targets, cu_seqlens, num_tokens, num_seqs, k, window, o, stream);
 }
 
 extern "C" int sq_score_debug_fill_workspace(sq_score_ctx* ctx, int value, void* stream) {

@@ -71,6 +71,73 @@ def score_vocab_parallel(eng, H, W_shard, vocab_starts: Sequence[int], rank: int
     return eng.merge_shards(states, vocab_starts, targets, cu_seqlens, k, window, stream=stream)
 
 
+class PeerStates:
+    """The vocab-parallel exchange WITHOUT an all-gather: every rank keeps its packed state in
+    a buffer of its own, the ranks open one another's buffers once (CUDA IPC; over NVLink a peer's buffer is ordinary
+    device memory to a kernel), and sq_score_merge_shards_peer reads all R states in place -- the transfer is the merge
+    kernel's own loads.  Per step the ranks only have to agree on WHEN: `ready()` after the shard kernels (nobody reads a
+    state before it is written) and `release()` after the merge (nobody overwrites a state a peer may still be reading).
+    Under NCCL both are a 4-byte all-reduce enqueued on the compute stream -- ordered by the stream, no host
+    synchronisation; under gloo (CPU-side groups, the one-GPU test) the stream is synchronised and the ranks meet at a
+    host barrier."""
+
+    def __init__(self, state: torch.Tensor, rank: int, world_size: int, group=None):
+        import torch.distributed as dist
+        from torch.multiprocessing.reductions import reduce_tensor
+        self.rank, self.world, self.group = rank, world_size, group
+        self.state = state                                   # this rank's buffer: sq_score_run_shard writes into it every step
+        self._nccl = dist.get_backend(group) == "nccl"
+        self._flag = torch.zeros(1, dtype=torch.int32, device=state.device)
+        handles = [None] * world_size
+        dist.all_gather_object(handles, reduce_tensor(state), group=group)
+        self.views = []
+        for r, (rebuild, args) in enumerate(handles):
+            if r == rank:
+                self.views.append(state)
+                continue
+            v = rebuild(*args)                               # maps the peer's allocation into this process
+            if v.device != state.device:                     # another GPU: one element through torch's P2P path enables peer access
+                torch.empty(1, dtype=v.dtype, device=state.device).copy_(v[:1])
+            self.views.append(v)
+
+    def _meet(self, stream):
+        import torch.distributed as dist
+        if self._nccl:
+            with torch.cuda.stream(stream if stream is not None else torch.cuda.current_stream(self.state.device)):
+                dist.all_reduce(self._flag, group=self.group)
+        else:
+            (stream if stream is not None else torch.cuda.current_stream(self.state.device)).synchronize()
+            dist.barrier(group=self.group)
+
+    def close(self):
+        """Drops the mappings of the peers' buffers (call on every rank before the buffers are freed)."""
+        self.views = []
+
+    def ready(self, stream=None):
+        self._meet(stream)
+
+    def release(self, stream=None):
+        self._meet(stream)
+
+
+def score_vocab_parallel_peer(eng, peers: PeerStates, H, W_shard, vocab_starts: Sequence[int], targets, cu_seqlens, k: int,
+                              window: int, stream=None) -> dict:
+    """score_vocab_parallel with the peers' states read in place (PeerStates) instead of gathered: shard kernels ->
+    ready() -> merge over peer memory + kernel 2 -> release()."""
+    rank = peers.rank
+    rows = int(vocab_starts[rank + 1]) - int(vocab_starts[rank])
+    if rows != W_shard.shape[0]:
+        raise ValueError("W_shard has %d rows, vocab_starts gives this rank %d" % (W_shard.shape[0], rows))
+    if rows > 0:
+        eng.run_shard(H, W_shard, vocab_starts[rank], targets, k, out=peers.state, stream=stream)
+    else:
+        eng.neutral_shard_state(H.shape[0], k, device=H.device, stream=stream, out=peers.state)
+    peers.ready(stream)
+    out = eng.merge_shards_peer(peers.views, vocab_starts, targets, cu_seqlens, k, window, stream=stream)
+    peers.release(stream)
+    return out
+
+
 def gather_shard_states(state: torch.Tensor, world_size: int, group=None, stream=None) -> torch.Tensor:
     """The one collective of the vocab-parallel path: all_gather of the packed states, rank-major -- shard r's state
     starts r * words into the result, which is what sq_score_merge_shards reads.  On CUDA the collective is issued

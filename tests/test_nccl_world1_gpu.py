@@ -46,7 +46,13 @@ def test_nccl_world_size_one_runs_both_exchanges():
             got = sharding.gather_sequence_scores(local, perm, inp["B"], 1, device=dev)
             # vocab-parallel with one rank that owns every row
             out_v = sharding.score_vocab_parallel(eng, H, W, [0, wl.V], 0, tg, cu, wl.k, wl.window, stream=st)
+            # the same with the states read in place: ready() / release() are 4-byte NCCL all-reduces on this stream
+            state = torch.empty(sq.shard_state_bytes(inp["T"], wl.k) // 4, dtype=torch.float32, device=dev)
+            peers = sharding.PeerStates(state, 0, 1)
+            out_p = sharding.score_vocab_parallel_peer(eng, peers, H, W, [0, wl.V], tg, cu, wl.k, wl.window, stream=st)
         st.synchronize()
+        for n in ("lse", "conf", "topk_index", "seq_min_window_conf"):             # (the empty sequence's NaN equals itself here)
+            assert torch.equal(torch.nan_to_num(out_p[n].float(), nan=-7.0), torch.nan_to_num(out_v[n].float(), nan=-7.0)), n
         assert got["seq_mean_conf"].is_cuda
         check_seqs({n: v.cpu().numpy() for n, v in got.items()}, ref)
         o = {n: v.cpu().numpy() for n, v in out_v.items()}

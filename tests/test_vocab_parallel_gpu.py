@@ -37,7 +37,16 @@ def run_sharded(inp, starts, k, window, targets=None):
             states.append(eng.run_shard(H, W[v0:v1], v0, tg, k))          # a view into W: rows beyond v1 belong to the next shard
     allst = torch.stack(states)                       # what all_gather_into_tensor would return
     out = eng.merge_shards(allst, starts, tg, cu, k, window)
+    # the same merge reading every state where it lies (sq_score_merge_shards_peer): separate allocations in no particular
+    # address order -- what the peers' buffers are to the merge kernel -- must give the same bits
+    pad = [torch.empty(1000 * (r + 1), device=DEV) for r in range(len(states))]
+    scattered = [st.clone() for st in reversed(states)][::-1]
+    outp = eng.merge_shards_peer(scattered, starts, tg, cu, k, window)
     torch.cuda.synchronize()
+    for n in out:
+        a, b = out[n], outp[n]
+        assert torch.equal(a, b) or torch.equal(torch.isnan(a), torch.isnan(b)) and torch.equal(a[~torch.isnan(a)], b[~torch.isnan(b)]), n
+    del pad
     eng.close()
     return {n: v.cpu().numpy() for n, v in out.items()}
 
@@ -144,3 +153,18 @@ def test_shard_api_errors():
         eng.run_shard(torch.zeros(32, 64, dtype=torch.bfloat16, device=DEV), torch.zeros(3, 64, dtype=torch.bfloat16, device=DEV), 0, tg, 5)
     assert sq.shard_state_bytes(32, 5) == (6 + 2 * 8) * 32 * 4 and sq.shard_state_bytes(10, 20) == (6 + 40) * 40
     eng.close()
+
+
+def test_peer_exchange_two_processes_on_one_gpu(tmp_path):
+    """sharding.PeerStates + score_vocab_parallel_peer end to end: two processes (gloo for the host-side meeting points)
+    open each other's state buffer through CUDA IPC and every one merges both states in place; each checks its result
+    against the fp64 oracle.  On one GPU the peer's buffer is local memory -- the code path (handles, views, the pointer
+    table of sq_score_merge_shards_peer, ready / release) is the one a multi-GPU node runs; no kernel waits on another."""
+    import os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", PYTHONPATH=root + os.pathsep + os.path.join(root, "tests"))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", "29731", os.path.join(root, "tests", "peer_worker.py")]
+    res = subprocess.run(cmd, env=env, capture_output=True, text=True, timeout=600, cwd=root)
+    assert res.returncode == 0, res.stdout[-3000:] + res.stderr[-3000:]
+    assert res.stdout.count("peer exchange OK") == 2, res.stdout[-2000:]
