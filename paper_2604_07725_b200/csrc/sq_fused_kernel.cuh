@@ -292,7 +292,17 @@ __device__ __forceinline__ void consume32(RowState<CAP>& st, float (&r)[32], int
 // stage arrive by TMA next to the operands (tmap_sfa / tmap_sfb: rows of 512 bytes in the layout tcgen05.cp wants, written
 // by sq_quant_mx_kernel), are copied to TMEM by the MMA thread before the stage's four instructions, and the tensor core
 // applies them: the accumulator holds the logits themselves, so the epilogue is the bf16 one.  Tiles are 224 columns wide.
-template <int CG, int CAP, int MODE = MODE_BF16>
+// CL = 4: "quad" scheduling (CTA pairs, not for the MX variant).  Four consecutive CTAs -- a quad -- take one 512-row token
+// tile, 128 rows each, and sweep the same vocabulary chunk.  The launch asks for clusters of 4 with clusters of 2 as the
+// fallback (cudaLaunchAttributePreferredClusterDimension): this part places 33 clusters of 4, and the 16 SMs they cannot
+// cover (one TPC per GPC) run the other 4 quads as two independent pairs each.  Which quad got which shape is only known
+// at run time (%cluster_nctarank); the work of a CTA does not depend on it, only how W reaches it does:
+//   cluster of 4: both pairs are on the SAME W tile at the same time, and every W box is fetched from L2 once for the two
+//     pairs -- CTA r loads 64 of the 128 W rows that the CTAs r and r ^ 2 need and multicasts them to both.  L2 -> SM
+//     operand traffic per k-block and SM falls from 16 KB (H) + 16 KB (W) to 16 + 8 KB.  A stage is free again when
+//     BOTH pairs' MMAs have retired (the commit goes to all four CTAs, the empty barriers count two arrivals).
+//   cluster of 2: the pair loads its own 2 x 64 W rows, as in the plain pair kernel.
+template <int CG, int CAP, int MODE = MODE_BF16, int CL = CG>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_constant__ CUtensorMap tmap_w,
                       const __grid_constant__ CUtensorMap tmap_sfa, const __grid_constant__ CUtensorMap tmap_sfb,
@@ -316,9 +326,14 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
 
   const int warp = threadIdx.x >> 5;
   const uint32_t lane = lane_id();
-  const uint32_t cta_rank = (CG == 2) ? cluster_ctarank() : 0u;
+  static_assert(CL == CG || (CL == 4 && CG == 2 && MODE != MODE_MX), "quads are two CTA pairs");
+  const uint32_t cl_rank = (CL > 1) ? cluster_ctarank() : 0u;   // rank in the cluster
+  const bool mcast = (CL == 4) && cluster_nctarank() == 4;      // this quad is ONE cluster: W boxes are multicast
+  const uint32_t unit_rank = (CL == 4) ? (blockIdx.x & 3u) : cl_rank;   // position in the quad / pair: rows 128 * unit_rank of the token tile
+  const uint32_t cta_rank = cl_rank & (CG - 1);                 // rank in the CTA pair
+  const uint32_t pair_leader = cl_rank & ~1u;                   // cluster rank of this pair's even CTA
   const bool leader = (cta_rank == 0);
-  const int cluster = (CG == 2) ? (int)cluster_id_x() : (int)blockIdx.x;
+  const int cluster = (CL == 4) ? (int)(blockIdx.x >> 2) : ((CL > 1) ? (int)cluster_id_x() : (int)blockIdx.x);
   const GangCtx gc = make_gang_ctx(p, cluster);
 
   if (warp == 0 && lane == 0) {
@@ -329,7 +344,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < Cfg::STAGES; ++s) {
       mbar_init(full_bar(s), 1);
-      mbar_init(empty_bar(s), 1);
+      mbar_init(empty_bar(s), mcast ? 2 : 1);
     }
     for (int a = 0; a < 2; ++a) {
       mbar_init(tfull_bar(a), 1);
@@ -343,12 +358,12 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   }
   __syncwarp();
   tc_fence_before();
-  if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
+  if constexpr (CL > 1) cluster_sync_all(); else __syncthreads();
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
-  const int rows_per_unit = BLOCK_M * CG;
+  const int rows_per_unit = BLOCK_M * CL;
   constexpr int BK = (F8 || MX) ? BLOCK_K_F8 : BLOCK_K;   // elements per k-block (128 bytes of every operand row)
 
   if (warp == 0) {
@@ -373,9 +388,9 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
           if (t0 % p.region_tiles == 0)
             gang_barrier(p.region_ctr, (unsigned)(t0 / p.region_tiles) * (unsigned)p.region_arrivals, p.wait_limit);
         }
-        if (gc.size > 1) gang_barrier(p.gang_ctr + gc.ctr, (++epoch) * (unsigned)(gc.size * CG), p.wait_limit);
+        if (gc.size > 1) gang_barrier(p.gang_ctr + gc.ctr, (++epoch) * (unsigned)(gc.size * CL), p.wait_limit);
         if (!active) continue;
-        const int row0 = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M;
+        const int row0 = un.m_tile * rows_per_unit + (int)unit_rank * BLOCK_M;
         if (p.h_ready != nullptr && row0 < p.T)
           wait_rows_ready(p.h_ready + (min(row0 + BLOCK_M, p.T) - 1) / p.flag_rows, p.wait_limit);
         const int vt0 = p.chunk_vt[un.chunk], vt1 = p.chunk_vt[un.chunk + 1];
@@ -394,10 +409,22 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
                 tma_load_2d(smem_sfb(stage), &tmap_sfb, full_bar(stage), 0, sfb_row);
               }
             } else {
-              const uint32_t bar = mapa(full_bar(stage), 0);
+              const uint32_t bar = mapa(full_bar(stage), pair_leader);
               if (leader) mbar_arrive_expect_tx(full_bar(stage), stage_tx);
               tma_load_2d_pair(smem_a(stage), &tmap_h, bar, kb * BK, row0);
-              tma_load_2d_pair(smem_b(stage), &tmap_w, bar, kb * BK, wrow0);
+              if constexpr (CL == 4) {   // (tmap_w's boxes are 64 rows high)
+                constexpr int HB = Cfg::B_ROWS / 2;
+                if (mcast) {             // half of this CTA's W rows, to this CTA and to its counterpart in the other pair
+                  const int half = (int)(cl_rank >> 1) * HB;
+                  tma_load_2d_pair_mcast(smem_b(stage) + (uint32_t)half * 128u, &tmap_w, full_bar(stage),
+                                         (uint16_t)(0x5u << cta_rank), kb * BK, wrow0 + half);
+                } else {
+                  tma_load_2d_pair(smem_b(stage), &tmap_w, bar, kb * BK, wrow0);
+                  tma_load_2d_pair(smem_b(stage) + (uint32_t)HB * 128u, &tmap_w, bar, kb * BK, wrow0 + HB);
+                }
+              } else {
+                tma_load_2d_pair(smem_b(stage), &tmap_w, bar, kb * BK, wrow0);
+              }
               if constexpr (MX) {
                 tma_load_2d_pair(smem_sfa(stage), &tmap_sfa, bar, 0, sfa_row);
                 tma_load_2d_pair(smem_sfb(stage), &tmap_sfb, bar, 0, sfb_row);
@@ -445,10 +472,10 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
               else if constexpr (F8) umma_f8<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
               else umma_bf16<CG>(d_tmem, adesc + 2u * k, bdesc + 2u * k, idesc, (kb | k) != 0 ? 1u : 0u);
             }
-            umma_commit<CG>(empty_bar(stage));   // smem slot free once these MMAs retire
+            umma_commit<CG>(empty_bar(stage), mcast ? (uint16_t)0xF : (uint16_t)0x3);   // smem slot free once these MMAs retire
             if (++stage == Cfg::STAGES) { stage = 0; phase ^= 1u; }
           }
-          umma_commit<CG>(tfull_bar(acc));       // accumulator ready for the epilogue
+          umma_commit<CG>(tfull_bar(acc), (uint16_t)(0x3u << pair_leader));   // accumulator ready for the epilogue (this pair's)
         }
       }
     }
@@ -457,13 +484,13 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
     const int q = warp & 3;                       // TMEM lane quarter this warp may read
     const int row_in_tile = q * 32 + (int)lane;
     const uint32_t lane_addr = tmem_base + (static_cast<uint32_t>(q * 32) << 16);
-    const uint32_t tempty_remote = (CG == 2) ? mapa(tempty_bar(0), 0) : tempty_bar(0);
+    const uint32_t tempty_remote = (CG == 2) ? mapa(tempty_bar(0), pair_leader) : tempty_bar(0);
     RowState<CAP> st;
     uint32_t tile = 0;
     for (int gu = 0; gu < gc.num_iters; ++gu) {
       Unit un;
       if (!decode_gang_unit(p, gc, gu, un)) continue;
-      const int row = un.m_tile * rows_per_unit + (int)cta_rank * BLOCK_M + row_in_tile;
+      const int row = un.m_tile * rows_per_unit + (int)unit_rank * BLOCK_M + row_in_tile;
       const int vt0 = p.chunk_vt[un.chunk], vt1 = p.chunk_vt[un.chunk + 1];
       int tgt = (row < p.T) ? __ldg(p.targets + row) : -1;
       tgt = (tgt >= p.vocab_offset) ? tgt - p.vocab_offset : -1;   // local column, or out of range
@@ -517,7 +544,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
   // ----------------------------------------------------------------------- teardown
   __syncwarp();
   tc_fence_before();
-  if constexpr (CG == 2) cluster_sync_all(); else __syncthreads();
+  if constexpr (CL > 1) cluster_sync_all(); else __syncthreads();
   if (warp == 2) {
     tc_fence_after();
     tmem_dealloc<CG>(tmem_base, TMEM_COLS);

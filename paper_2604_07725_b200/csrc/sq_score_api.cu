@@ -45,7 +45,8 @@ struct sq_score_ctx {
   unsigned int* amax_bits = nullptr;   // per-tensor amax of sq_score_quantize_fp8
   int* seq_done = nullptr;   // [max_seqs] per-sequence tile counters of the single-launch reduction (zero between runs)
   int* tile_base = nullptr; int* tile_seq = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
-  int max_clusters[3] = {0, 0, 0};   // [cg]: clusters of kernel 1 the device holds at once (occupancy query at create)
+  int cluster4 = 0;                  // experiment (SQ_SCORE_CLUSTER4=1): large bf16 runs in clusters of 4 CTAs with W multicast
+  int max_clusters[5] = {0, 0, 0, 0, 0};   // [cg]: clusters of kernel 1 the device holds at once (occupancy query at create)
   int region_mult = 0;               // region barrier of kernel 1: regions of region_mult x (a common multiple of the gang sizes) token tiles; < 0: off
   long long wait_limit = 0;          // cycles a device-side wait may last before kernel 1 traps (0 = for ever)
   int* pos_base = nullptr;           // [max_seqs + 1] packed start of every candidate (sq_score_positions)
@@ -140,7 +141,7 @@ static int make_plan(const sq_score_config* cfg, int64_t T, int k, int num_sms, 
   if (num_sms <= 0) num_sms = 148;
   // default: CTA pairs (UMMA M = 256); a decode-shaped run of at most 128 rows fits one CTA's 128 TMEM
   // lanes, so single-CTA UMMA (M = 128) halves the wasted MMA rows and lets all 148 SMs stream W
-  const int cg = (cfg->cta_group == 1) ? 1 : (cfg->cta_group == 2 ? 2 : ((T > 0 && T <= 128) ? 1 : 2));
+  const int cg = (cfg->cta_group == 4) ? 4 : (cfg->cta_group == 1) ? 1 : (cfg->cta_group == 2 ? 2 : ((T > 0 && T <= 128) ? 1 : 2));
   memset(pl, 0, sizeof(*pl));
   pl->cta_group = cg;
   pl->rows_per_tile = 128 * cg;
@@ -428,6 +429,10 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
                            sq::FusedCfg<CG, sq::MODE_MX>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
   SQ_SET_SMEM8(1, 8) SQ_SET_SMEM8(1, 20) SQ_SET_SMEM8(1, 32) SQ_SET_SMEM8(2, 8) SQ_SET_SMEM8(2, 20) SQ_SET_SMEM8(2, 32)
 #undef SQ_SET_SMEM8
+  for (const void* f : {(const void*)sq::sq_fused_score_kernel<2, 8, sq::MODE_BF16, 4>, (const void*)sq::sq_fused_score_kernel<2, 20, sq::MODE_BF16, 4>,
+                        (const void*)sq::sq_fused_score_kernel<2, 32, sq::MODE_BF16, 4>, (const void*)sq::sq_fused_score_kernel<2, 8, sq::MODE_F8, 4>,
+                        (const void*)sq::sq_fused_score_kernel<2, 20, sq::MODE_F8, 4>, (const void*)sq::sq_fused_score_kernel<2, 32, sq::MODE_F8, 4>})
+    if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, sq::FusedCfg<2>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
   for (const void* f : {(const void*)sq::sq_reduce_fused_kernel<true>, (const void*)sq::sq_reduce_fused_kernel<false>})
     if (cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              sq::RED_SMEM_BYTES + (sq::RED_FUSED_MAX_SEQS + 1) * (int)sizeof(int)) != cudaSuccess) rc = SQ_ERR_CUDA;
@@ -461,6 +466,8 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
       }
       ctx->max_clusters[cg] = n;
     }
+    if (const char* c4 = getenv("SQ_SCORE_CLUSTER4")) ctx->cluster4 = atoi(c4);
+    if (ctx->cluster4) ctx->max_clusters[4] = ctx->max_clusters[2] / 2;   // quads: 4 consecutive CTAs, placed as one cluster of 4 or two of 2
   }
   *out = ctx;
   return SQ_OK;
@@ -515,22 +522,27 @@ static int make_tmap_sf(sq_score_ctx* ctx, CUtensorMap* map, const void* base, i
 }
 
 // ------------------------------------------------------------------------------------------ launches
-template <int CG, int CAP, int MODE = sq::MODE_BF16>
+template <int CG, int CAP, int MODE = sq::MODE_BF16, int CL = CG>
 static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CUtensorMap& th, const CUtensorMap& tw,
                                 const CUtensorMap& tsa, const CUtensorMap& tsb, const sq::FusedParams& fp, cudaStream_t st) {
   const int clusters = pl.clusters_used;   // every launched cluster belongs to a gang
   cudaLaunchConfig_t lc = {};
-  lc.gridDim = dim3((unsigned)(clusters * CG));
+  lc.gridDim = dim3((unsigned)(clusters * CL));
   lc.blockDim = dim3(sq::NUM_THREADS);
   lc.dynamicSmemBytes = sq::FusedCfg<CG, MODE>::SMEM_BYTES;
   lc.stream = st;
-  cudaLaunchAttribute at[1];
+  cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeClusterDimension;
   at[0].val.clusterDim.x = CG; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
   lc.attrs = at;
   lc.numAttrs = 1;
+  if (CL == 4) {   // quads: clusters of 4 where the device can place them, pairs elsewhere (sq_fused_kernel.cuh)
+    at[1].id = cudaLaunchAttributePreferredClusterDimension;
+    at[1].val.preferredClusterDim.x = 4; at[1].val.preferredClusterDim.y = 1; at[1].val.preferredClusterDim.z = 1;
+    lc.numAttrs = 2;
+  }
   (void)num_sms;
-  return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP, MODE>, th, tw, tsa, tsb, fp);
+  return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP, MODE, CL>, th, tw, tsa, tsb, fp);
 }
 
 // Launch with programmatic stream serialization: the kernel is scheduled while its predecessor drains and waits in
@@ -700,7 +712,8 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     sq_score_config pc = ctx->cfg;
     pc.vocab = V;
     if (f8) pc.d = (d + 1) / 2;   // an e4m3 k-block is 128 elements: the plan sees half as many k-blocks
-    const int cg_sel = (pc.cta_group == 1) ? 1 : (pc.cta_group == 2 ? 2 : (T <= 128 ? 1 : 2));
+    int cg_sel = (pc.cta_group == 1) ? 1 : (pc.cta_group == 2 ? 2 : (T <= 128 ? 1 : 2));
+    if (ctx->cluster4 && cg_sel == 2 && !mx && T > 4096 && ctx->max_clusters[4] > 0) { cg_sel = 4; pc.cta_group = 4; }
     auto& pcache = ctx->plan_cache;
     if (pcache.T == T && pcache.k == k && pcache.V == V && pcache.tile_n == tile_n && pcache.d == pc.d) {
       pl = pcache.pl;
@@ -796,6 +809,12 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
       case 108: SQ_LAUNCH(1, 8, sq::MODE_BF16);
       case 120: SQ_LAUNCH(1, 20, sq::MODE_BF16);
       case 132: SQ_LAUNCH(1, 32, sq::MODE_BF16);
+      case 1408: e = launch_fused<2, 8, sq::MODE_F8, 4>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break;
+      case 1420: e = launch_fused<2, 20, sq::MODE_F8, 4>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break;
+      case 1432: e = launch_fused<2, 32, sq::MODE_F8, 4>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break;
+      case 408: e = launch_fused<2, 8, sq::MODE_BF16, 4>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break;
+      case 420: e = launch_fused<2, 20, sq::MODE_BF16, 4>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break;
+      case 432: e = launch_fused<2, 32, sq::MODE_BF16, 4>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break;
       case 208: SQ_LAUNCH(2, 8, sq::MODE_BF16);
       case 220: SQ_LAUNCH(2, 20, sq::MODE_BF16);
       default: SQ_LAUNCH(2, 32, sq::MODE_BF16);

@@ -564,6 +564,40 @@ def test_scoring_pipeline_takes_the_streaming_form_for_many_sequences():
     check_tokens(out, ref, wl.k, rows=rows)
 
 
+@pytest.mark.parametrize("d,V,B,lo,hi,gm", [(256, 3000, 6, 700, 1100, 0), (200, 1003, 9, 500, 900, 3), (512, 5000, 4, 1500, 2500, 6)])
+def test_quad_scheduling_with_w_multicast(d, V, B, lo, hi, gm):
+    """SQ_SCORE_CLUSTER4=1 (opt-in): runs of more than 4096 tokens are scheduled in quads of four CTAs that
+    the device places as clusters of 4 (W boxes multicast to both CTA pairs) or, where it cannot, as two pairs; 512-row
+    token tiles, ragged T, d and V.  Same tolerances against the oracle; bf16 and the FP8 variant."""
+    import os
+    sq = _sq()
+    wl = workloads.custom(name="quad", d=d, V=V, B=B, len_lo=lo, len_hi=hi, k=20, window=64, seed=d + V, w_std=0.05,
+                          planted_frac=0.5, planted_scale=3.0, rmsnorm=True)
+    inp = workloads.make_inputs(wl)
+    assert inp["T"] > 4096
+    dev = torch.device("cuda:0")
+    os.environ["SQ_SCORE_CLUSTER4"] = "1"
+    try:
+        eng = sq.SqScore(d, V, max_tokens=inp["T"], max_seqs=B, max_k=20, group_m=gm)
+    finally:
+        os.environ.pop("SQ_SCORE_CLUSTER4", None)
+    H, W, tg, cu = (inp[n].to(dev) for n in ("H", "W", "targets", "cu_seqlens"))
+    out = eng.run(H, W, tg, cu, 20, 64)
+    torch.cuda.synchronize()
+    o = {n: v.cpu().numpy() for n, v in out.items()}
+    ref = O.score(inp["H"], inp["W"], inp["targets"], inp["cu_seqlens"], 20, 64)
+    check_tokens(o, ref, 20); check_seqs(o, ref)
+    if d % 16 == 0:
+        Hq, hs = eng.quantize_fp8(H, False); Wq, ws = eng.quantize_fp8(W, True)
+        o8 = eng.run_fp8(Hq, hs, Wq, ws, tg, cu, 20, 64)
+        torch.cuda.synchronize()
+        ref8 = O.score(O.dequantize_fp8(Hq.cpu().numpy(), hs.cpu().numpy()), O.dequantize_fp8(Wq.cpu().numpy(), ws.cpu().numpy()),
+                       inp["targets"], inp["cu_seqlens"], 20, 64)
+        o8 = {n: v.cpu().numpy() for n, v in o8.items()}
+        check_tokens(o8, ref8, 20); check_seqs(o8, ref8)
+    eng.close()
+
+
 # ------------------------------------------------------------------------------------------ API behaviour
 def test_run_host_matches_run_and_null_per_token_outputs():
     sq = _sq()
