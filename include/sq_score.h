@@ -132,7 +132,7 @@ typedef struct {
 int sq_score_create(const sq_score_config *cfg, sq_score_ctx **out);
 
 /* Scores T tokens: enqueues kernel 1 (fused GEMM + statistics), the merge/finalize kernel and kernel 2 on
- * `stream` (runs of at most 128 tokens -- decode-shaped -- do kernel 2's work in the finalize kernel's last CTA:
+ * `stream` (runs of at most 256 tokens -- decode-shaped -- do kernel 2's work in the finalize kernel's last CTA:
  * two launches instead of three).
  *   H          DEVICE bf16 [T,d]       final hidden states; row t predicts targets[t] (the caller
  *                                      does the next-token shift and packs only trajectory tokens)
@@ -376,7 +376,7 @@ int64_t sq_score_launch_count(const sq_score_ctx *ctx);
 /* Which form of kernel 2 (step a7) the last call on this ctx used: 0 = none yet, SQ_REDUCE_FORM_FUSED = one launch (the
  * whole problem is one wave of CTAs), _TILES = three launches over sequence-aligned tiles, _STREAM = stream +
  * fold over fixed blocks (large inputs, 128 <= window <= 2048, 16-byte aligned arrays), _TAIL = inside the finalize kernel
- * (runs of at most 128 tokens).  All forms compute the same reductions; tests and bench.py report which one ran. */
+ * (runs of at most 256 tokens).  All forms compute the same reductions; tests and bench.py report which one ran. */
 #define SQ_REDUCE_FORM_FUSED 1
 #define SQ_REDUCE_FORM_TILES 2
 #define SQ_REDUCE_FORM_STREAM 3

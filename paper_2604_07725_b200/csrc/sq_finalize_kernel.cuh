@@ -55,12 +55,12 @@ struct FinalizeParams {
 };
 
 constexpr int FIN_WARPS = 8;
-constexpr int FIN_TAIL_MAX_T = 128;                // largest T whose per-sequence reductions run in the finalize kernel's tail
+constexpr int FIN_TAIL_MAX_T = 256;                // largest T whose per-sequence reductions run in the finalize kernel's tail
 
 // Step a7 for a small run, by one CTA, from the per-token outputs the grid has just written (sq_reduce_kernel.cuh states
 // the definitions): per sequence the mean target log-prob over valid targets, mean entropy, C(tau) = mean c(i) (Eq. 4,
 // PAPER.md:160) and the minimum over stride-1 full windows of length w' = min(w, L) of the window mean of c(i); an
-// empty sequence gives NaNs.  One warp per sequence; fp64 sums and an fp64 prefix of c(i) (L <= 128), so every window
+// empty sequence gives NaNs.  One warp per sequence; fp64 sums and an fp64 prefix of c(i) (L <= 256), so every window
 // sum is exact to fp64 rounding.
 template <int NWARPS>
 __device__ __forceinline__ void fin_tail_reduce(const FinalizeParams& p, double* s_prefix) {

@@ -173,18 +173,18 @@ def test_empty_short_and_single_token_sequences():
 
 @pytest.mark.parametrize("window", [1, 3, 16, 17, 40, 1000])
 def test_small_run_sequences_reduced_in_the_finalize_tail(window):
-    """Runs of at most 128 tokens (decode-shaped) do kernel 2's work in the finalize kernel's last CTA (two launches):
+    """Runs of at most 256 tokens (decode-shaped) do kernel 2's work in the finalize kernel's last CTA (two launches):
     empty, L = 1, L < w, L = w, L = w + 1 sequences, invalid targets, a sequence without any valid target; twice on
     one ctx (the CTA counter must be back to zero)."""
     sq = _sq()
     wl = workloads.custom(name="tail", d=64, V=3000, B=8, k=20, window=window, seed=36, w_std=0.2,
                           planted_frac=0.5, planted_scale=3.0, rmsnorm=True)
-    inp = workloads.make_inputs(wl, lengths=[0, 1, 15, 16, 17, 0, 40, 39])      # T = 128
+    inp = workloads.make_inputs(wl, lengths=[128, 0, 1, 15, 16, 17, 0, 40, 39])   # T = 256
     tg = inp["targets"].clone()
     tg[1:16:2] = -1
     tg[-39:] = wl.V + 7                                                           # the last sequence has no valid target
     dev = torch.device("cuda:0")
-    eng = sq.SqScore(wl.d, wl.V, max_tokens=128, max_seqs=8, max_k=20)
+    eng = sq.SqScore(wl.d, wl.V, max_tokens=256, max_seqs=9, max_k=20)
     H, W, cu = inp["H"].to(dev), inp["W"].to(dev), inp["cu_seqlens"].to(dev)
     ref = oracle_full(inp, targets=tg.numpy(), window=window)
     for rep in range(2):
@@ -195,10 +195,10 @@ def test_small_run_sequences_reduced_in_the_finalize_tail(window):
         o = {n: v.cpu().numpy() for n, v in out.items()}
         check_tokens(o, ref, 20)
         check_seqs(o, ref)
-        assert np.isnan(o["seq_mean_logprob"][[0, 5, 7]]).all() and np.isfinite(o["seq_mean_entropy"][7])
+        assert np.isnan(o["seq_mean_logprob"][[1, 6, 8]]).all() and np.isfinite(o["seq_mean_entropy"][8])
     # one more token and kernel 2 is a launch of its own again; the results agree
-    eng2 = sq.SqScore(wl.d, wl.V, max_tokens=129, max_seqs=8, max_k=20)
-    inp3 = workloads.make_inputs(wl, lengths=[0, 1, 15, 16, 17, 0, 40, 40])
+    eng2 = sq.SqScore(wl.d, wl.V, max_tokens=257, max_seqs=9, max_k=20)
+    inp3 = workloads.make_inputs(wl, lengths=[128, 0, 1, 15, 16, 17, 0, 40, 40])
     n0 = eng2.launch_count()
     out3 = eng2.run(inp3["H"].to(dev), W, inp3["targets"].to(dev), inp3["cu_seqlens"].to(dev), 20, window)
     torch.cuda.synchronize()
