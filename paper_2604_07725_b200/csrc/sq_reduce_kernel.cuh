@@ -469,7 +469,7 @@ __device__ __forceinline__ float rs_warp_sum4(float a, float b, float c, float d
 }
 
 template <bool HAS_TG>
-__global__ void __launch_bounds__(RS_THREADS, 3) sq_reduce_stream_kernel(const ReduceParams p) {
+__global__ void __launch_bounds__(RS_THREADS, HAS_TG ? 2 : 3) sq_reduce_stream_kernel(const ReduceParams p) {
   __shared__ __align__(16) float s_P[RS_TB + RS_WMAX + 4];   // exclusive prefix of conf over block + look-ahead
   __shared__ float s_tot[32];                                // totals: 16 warp ranges, then 16 look-ahead runs of 128
   cudaGridDependencySynchronize();
