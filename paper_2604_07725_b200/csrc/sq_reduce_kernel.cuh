@@ -397,7 +397,7 @@ __global__ void __launch_bounds__(RED_THREADS) sq_reduce_fused_kernel(const Redu
 // The tile forms above cut tiles at sequence starts, so a CTA must know its sequence before it can load anything
 // (table lookup or search -> loads -> arithmetic, every step a dependent round trip through a saturated memory system),
 // and a CTA's lifetime is mostly latency.  Here the streaming kernel does not look at cu_seqlens at all:
-//   stream : CTA x owns the FIXED block [x * RS_TB, (x+1) * RS_TB) of the packed arrays, warp q its 256-token range.
+//   stream : CTA x owns the FIXED block [x * TB, (x+1) * TB) of the packed arrays (TB = 4096 or 6144), warp q its range of R = TB / 16 tokens.
 //            1. every thread issues all its 16-byte loads at once (lp, ent, conf, targets of its 8 tokens + one vector
 //               of the look-ahead range [block end, block end + w)): one round trip;
 //            2. exclusive prefix sums P of conf over block + look-ahead: in registers (per vector, per warp by
@@ -414,10 +414,8 @@ __global__ void __launch_bounds__(RED_THREADS) sq_reduce_fused_kernel(const Redu
 //            NaNs; a sequence shorter than the window has one window, itself: min = mean conf.
 // The prefix runs across sequence boundaries inside a block, so a non-finite conf value spoils the window sums of its
 // whole 4096-token block (the tile forms confine it to its sequence); c(i) of Eq. 3 is always finite.
-constexpr int RS_TB = 4096;         // tokens per CTA
 constexpr int RS_THREADS = 512;
 constexpr int RS_WARPS = RS_THREADS / 32;
-constexpr int RS_R = 256;           // tokens per warp = per record
 constexpr int RS_WMAX = 2048;       // widest window: the look-ahead is one 16-byte vector per thread
 constexpr int RS_WMIN = 128;        // narrowest: S(j) = P[j+w] - P[j] with P up to ~6144 x mean(conf) in fp32; the rounding of P
                                     // (~1e-7 relative to P, i.e. ~5e-6 of a 128-element sum) would reach 1e-3 of a 1-element one
@@ -468,27 +466,36 @@ __device__ __forceinline__ float rs_warp_sum4(float a, float b, float c, float d
   return y;
 }
 
-template <bool HAS_TG>
-__global__ void __launch_bounds__(RS_THREADS, HAS_TG ? 2 : 3) sq_reduce_stream_kernel(const ReduceParams p) {
-  __shared__ __align__(16) float s_P[RS_TB + RS_WMAX + 4];   // exclusive prefix of conf over block + look-ahead
+// NV = 16-byte vectors per lane and array: a warp's range is R = 128 NV tokens, a CTA's block 16 R.  More bytes per thread
+// in flight beat more threads: with targets (four arrays) NV = 2 at two CTAs per SM streams at 0.96 of the copy peak, without
+// them NV = 3 at two CTAs (NV = 2 at three CTAs: 0.91).
+template <int NV> struct RsCfg {
+  static constexpr int R = 128 * NV;           // tokens per warp = per record
+  static constexpr int TB = RS_WARPS * R;      // tokens per CTA
+};
+
+template <bool HAS_TG, int NV>
+__global__ void __launch_bounds__(RS_THREADS, 2) sq_reduce_stream_kernel(const ReduceParams p) {
+  constexpr int R = RsCfg<NV>::R, TB = RsCfg<NV>::TB;
+  __shared__ __align__(16) float s_P[TB + RS_WMAX + 4];      // exclusive prefix of conf over block + look-ahead
   __shared__ float s_tot[32];                                // totals: 16 warp ranges, then 16 look-ahead runs of 128
   cudaGridDependencySynchronize();
   cudaTriggerProgrammaticLaunchCompletion();                 // the fold kernel may start its record-independent part
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int T = (int)p.T;                                    // the host takes this form only when T + RS_TB + RS_WMAX fits an int
-  const int blk0 = blockIdx.x * RS_TB;
-  const int e0 = blk0 + warp * RS_R + 4 * lane;              // lane l owns tokens e0 .. + 3 and e0 + 128 .. + 3 of the warp's range
-  const int ela = blk0 + RS_TB + 4 * threadIdx.x;
+  const int T = (int)p.T;                                    // the host takes this form only when T + TB + RS_WMAX fits an int
+  const int blk0 = blockIdx.x * TB;
+  const int e0 = blk0 + warp * R + 4 * lane;                 // lane l owns tokens e0 + 128 k .. + 3, k < NV, of the warp's range
+  const int ela = blk0 + TB + 4 * threadIdx.x;
   const int w = p.window;
   const bool has_la = 4 * (int)threadIdx.x < w;
 
   // 1. every load first
-  float4 vl[2], ve[2], vc[2];
-  int4 vt[2];
+  float4 vl[NV], ve[NV], vc[NV];
+  int4 vt[NV];
   float4 la = make_float4(0.f, 0.f, 0.f, 0.f);
-  if (blk0 + RS_TB + RS_WMAX <= T) {                         // CTA-uniform: no vector crosses the end of the arrays
+  if (blk0 + TB + RS_WMAX <= T) {                            // CTA-uniform: no vector crosses the end of the arrays
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < NV; ++k) {
       vl[k] = __ldg(reinterpret_cast<const float4*>(p.lp + e0 + 128 * k));
       ve[k] = __ldg(reinterpret_cast<const float4*>(p.ent + e0 + 128 * k));
       vc[k] = __ldg(reinterpret_cast<const float4*>(p.conf + e0 + 128 * k));
@@ -497,7 +504,7 @@ __global__ void __launch_bounds__(RS_THREADS, HAS_TG ? 2 : 3) sq_reduce_stream_k
     if (has_la) la = __ldg(reinterpret_cast<const float4*>(p.conf + ela));
   } else {
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < NV; ++k) {
       vl[k] = rs_load4(p.lp, e0 + 128 * k, T);
       ve[k] = rs_load4(p.ent, e0 + 128 * k, T);
       vc[k] = rs_load4(p.conf, e0 + 128 * k, T);
@@ -507,17 +514,20 @@ __global__ void __launch_bounds__(RS_THREADS, HAS_TG ? 2 : 3) sq_reduce_stream_k
   }
 
   // 2. prefix sums of conf: per vector, per warp, per block
-  const float t0 = (vc[0].x + vc[0].y) + (vc[0].z + vc[0].w);
-  const float t1 = (vc[1].x + vc[1].y) + (vc[1].z + vc[1].w);
-  float own_excl[2];
+  float own_excl[NV], t_cf = 0.f;
   {
-    const float i0s = rs_warp_incl(t0, lane), i1s = rs_warp_incl(t1, lane);
-    const float half = __shfl_sync(0xffffffffu, i0s, 31);
-    own_excl[0] = i0s - t0;
-    own_excl[1] = half + (i1s - t1);
+    float before = 0.f;                                      // sum of the vectors k' < k of this warp's range
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+      const float t = (vc[k].x + vc[k].y) + (vc[k].z + vc[k].w);
+      const float inc = rs_warp_incl(t, lane);
+      own_excl[k] = before + (inc - t);
+      before += __shfl_sync(0xffffffffu, inc, 31);
+      t_cf += t;
+    }
     const float la_t = (la.x + la.y) + (la.z + la.w);
     const float la_incl = rs_warp_incl(la_t, lane);
-    if (lane == 31) { s_tot[warp] = half + i1s; s_tot[RS_WARPS + warp] = la_incl; }
+    if (lane == 31) { s_tot[warp] = before; s_tot[RS_WARPS + warp] = la_incl; }
     la.w = la_incl - la_t;                                   // la.w is not needed below: the slot carries the exclusive prefix
   }
   __syncthreads();
@@ -527,42 +537,41 @@ __global__ void __launch_bounds__(RS_THREADS, HAS_TG ? 2 : 3) sq_reduce_stream_k
     const float off_own = __shfl_sync(0xffffffffu, ex, warp);
     const float off_la = __shfl_sync(0xffffffffu, ex, RS_WARPS + warp);
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < NV; ++k) {
       const float b0 = off_own + own_excl[k];
       float4 o;
       o.x = b0; o.y = b0 + vc[k].x; o.z = o.y + vc[k].y; o.w = o.z + vc[k].z;
-      *reinterpret_cast<float4*>(s_P + warp * RS_R + k * 128 + 4 * lane) = o;
+      *reinterpret_cast<float4*>(s_P + warp * R + k * 128 + 4 * lane) = o;
     }
     const float b0 = off_la + la.w;
     float4 o;
     o.x = b0; o.y = b0 + la.x; o.z = o.y + la.y; o.w = o.z + la.z;
-    *reinterpret_cast<float4*>(s_P + RS_TB + 4 * threadIdx.x) = o;
+    *reinterpret_cast<float4*>(s_P + TB + 4 * threadIdx.x) = o;
   }
   // the lane's sums, while the barrier fills
-  const float a_en = ((ve[0].x + ve[0].y) + (ve[0].z + ve[0].w)) + ((ve[1].x + ve[1].y) + (ve[1].z + ve[1].w));
-  float a_lp, a_n;
-  if (HAS_TG) {
-    a_lp = 0.f; a_n = 0.f;
+  float a_en = 0.f, a_lp = 0.f, a_n = 0.f;
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
+  for (int k = 0; k < NV; ++k) {
+    a_en += (ve[k].x + ve[k].y) + (ve[k].z + ve[k].w);
+    if (HAS_TG) {
       const bool k0 = (unsigned)vt[k].x < (unsigned)p.V, k1 = (unsigned)vt[k].y < (unsigned)p.V;
       const bool k2 = (unsigned)vt[k].z < (unsigned)p.V, k3 = (unsigned)vt[k].w < (unsigned)p.V;
       a_lp += ((k0 ? vl[k].x : 0.f) + (k1 ? vl[k].y : 0.f)) + ((k2 ? vl[k].z : 0.f) + (k3 ? vl[k].w : 0.f));
       a_n += (float)((int)k0 + (int)k1 + (int)k2 + (int)k3);
+    } else {
+      a_lp += (vl[k].x + vl[k].y) + (vl[k].z + vl[k].w);
+      a_n += 4.f;
     }
-  } else {
-    a_lp = ((vl[0].x + vl[0].y) + (vl[0].z + vl[0].w)) + ((vl[1].x + vl[1].y) + (vl[1].z + vl[1].w));
-    a_n = 8.f;
   }
-  const float tot = rs_warp_sum4(a_lp, a_n, a_en, t0 + t1, lane);
+  const float tot = rs_warp_sum4(a_lp, a_n, a_en, t_cf, lane);
   __syncthreads();
 
-  // 3. the 256 window sums that start in this range
-  const float* Pl = s_P + warp * RS_R + 4 * lane;
+  // 3. the R window sums that start in this range
+  const float* Pl = s_P + warp * R + 4 * lane;
   float mn = CUDART_INF_F, s_first = 0.f;
   if ((w & 3) == 0) {                                        // 16-byte shared loads line up
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
+    for (int k = 0; k < NV; ++k) {
       const float4 lo = *reinterpret_cast<const float4*>(Pl + 128 * k);
       const float4 hi = *reinterpret_cast<const float4*>(Pl + 128 * k + w);
       if (k == 0) s_first = hi.x - lo.x;
@@ -570,7 +579,7 @@ __global__ void __launch_bounds__(RS_THREADS, HAS_TG ? 2 : 3) sq_reduce_stream_k
     }
   } else {
 #pragma unroll
-    for (int k = 0; k < 2; ++k)
+    for (int k = 0; k < NV; ++k)
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
         const float sj = Pl[128 * k + i + w] - Pl[128 * k + i];
@@ -585,28 +594,30 @@ __global__ void __launch_bounds__(RS_THREADS, HAS_TG ? 2 : 3) sq_reduce_stream_k
   if (lane == 0) reinterpret_cast<float2*>(p.part_min)[range] = make_float2(mn, s_first);
 }
 
-// Window sums of a ragged range r (tokens [256 r, 256 r + 256)) are rebuilt from its recorded first sum S(256 r):
-// S(j + 1) = S(j) + c[j + w] - c[j].  Lane l rebuilds the starts 256 r + 8l .. + 7; only starts in [lo, hi) count.
-struct RsRagged {
-  float d[8];     // d[i] = S(m0 + i + 1) - S(m0 + i)
-  float excl;     // S(m0) - S(256 r)
+// Window sums of a ragged range r (tokens [R r, R r + R)) are rebuilt from its recorded first sum S(R r):
+// S(j + 1) = S(j) + c[j + w] - c[j].  Lane l rebuilds the starts R r + PL l .. + PL - 1 (PL = R / 32); only starts in [lo, hi) count.
+template <int PL> struct RsRagged {
+  float d[PL];    // d[i] = S(m0 + i + 1) - S(m0 + i)
+  float excl;     // S(m0) - S(R r)
   int m0, lo, hi; // lo >= hi: nothing to do
 };
-__device__ __forceinline__ void rs_ragged_load(RsRagged& g, const ReduceParams& p, int r, int lo, int hi, int w, int lane) {
-  g.m0 = r * RS_R + 8 * lane; g.lo = lo; g.hi = hi;
+template <int PL>
+__device__ __forceinline__ void rs_ragged_load(RsRagged<PL>& g, const ReduceParams& p, int r, int lo, int hi, int w, int lane) {
+  g.m0 = r * (32 * PL) + PL * lane; g.lo = lo; g.hi = hi;
   float run = 0.f;
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {                              // only differences below the last start matter
+  for (int i = 0; i < PL; ++i) {                             // only differences below the last start matter
     const int m = g.m0 + i;
     g.d[i] = (m + 1 < hi) ? __ldg(p.conf + m + w) - __ldg(p.conf + m) : 0.f;   // m + w < hi + w - 1 <= s1 - 1: inside the arrays
     run += g.d[i];
   }
   g.excl = rs_warp_incl(run, lane) - run;
 }
-__device__ __forceinline__ float rs_ragged_min(const RsRagged& g, float s_range_first) {
+template <int PL>
+__device__ __forceinline__ float rs_ragged_min(const RsRagged<PL>& g, float s_range_first) {
   float s = s_range_first + g.excl, best = CUDART_INF_F;
 #pragma unroll
-  for (int i = 0; i < 8; ++i) {
+  for (int i = 0; i < PL; ++i) {
     if (g.m0 + i >= g.lo && g.m0 + i < g.hi) best = fminf(best, s);
     s += g.d[i];
   }
@@ -617,7 +628,9 @@ __device__ __forceinline__ float rs_ragged_min(const RsRagged& g, float s_range_
 // ends of the sequence, the differences of the ragged window ranges -- is read BEFORE the grid dependency wait, i.e.
 // underneath the stream kernel's last wave (the stream kernel triggers this launch early; it does so after its own
 // dependency wait, so whatever produced lp / ent / conf has completed by the time this kernel can start).
+template <int NV>
 __global__ void __launch_bounds__(128) sq_reduce_stream_fold_kernel(const ReduceParams p) {
+  constexpr int R = RsCfg<NV>::R, PL = R / 32;
   const int b = blockIdx.x * 4 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   if (b >= p.B) return;
@@ -628,10 +641,10 @@ __global__ void __launch_bounds__(128) sq_reduce_stream_fold_kernel(const Reduce
     return;
   }
   // sums: the ranges [r_a, r_b) lie inside the sequence; what is left of it are the tokens [s0, h1) and [t0, s1)
-  const int r_a = (s0 + RS_R - 1) / RS_R, r_b = s1 / RS_R;
-  const int h1 = r_a < r_b ? r_a * RS_R : s1, t0 = r_a < r_b ? r_b * RS_R : s1;
+  const int r_a = (s0 + R - 1) / R, r_b = s1 / R;
+  const int h1 = r_a < r_b ? r_a * R : s1, t0 = r_a < r_b ? r_b * R : s1;
   double s_lp = 0.0, s_n = 0.0, s_en = 0.0, s_cf = 0.0;
-  // the ragged ends, at most 255 tokens each (511 when no range lies inside the sequence): every load of a pass at once
+  // the ragged ends, fewer than R tokens each (2 R when no range lies inside the sequence): every load of a pass at once
   auto raw = [&](int e_lo, int e_hi) {
     for (int base = e_lo; base < e_hi; base += 256) {
       float xl[8], xe[8], xc[8];
@@ -661,12 +674,12 @@ __global__ void __launch_bounds__(128) sq_reduce_stream_fold_kernel(const Reduce
   raw(t0, s1);
   // window starts [s0, jl]: the ranges [r_a, r_c) hold only valid starts; a ragged range at each end
   const int jl = s1 - w;
-  const int r_c = (L >= w) ? (jl + 1) / RS_R : r_a;
+  const int r_c = (L >= w) ? (jl + 1) / R : r_a;
   const int r_t = max(r_c, r_a);
-  RsRagged gh, gt;
+  RsRagged<PL> gh, gt;
   gh.lo = gh.hi = gt.lo = gt.hi = 0;
-  if (L >= w && (s0 % RS_R)) rs_ragged_load(gh, p, s0 / RS_R, s0, min(jl + 1, r_a * RS_R), w, lane);
-  if (L >= w && r_t * RS_R <= jl) rs_ragged_load(gt, p, r_t, r_t * RS_R, jl + 1, w, lane);
+  if (L >= w && (s0 % R)) rs_ragged_load(gh, p, s0 / R, s0, min(jl + 1, r_a * R), w, lane);
+  if (L >= w && r_t * R <= jl) rs_ragged_load(gt, p, r_t, r_t * R, jl + 1, w, lane);
 
   cudaGridDependencySynchronize();                           // the records
   for (int r = r_a + lane; r < r_b; r += 32) {
@@ -675,7 +688,7 @@ __global__ void __launch_bounds__(128) sq_reduce_stream_fold_kernel(const Reduce
   }
   float best = CUDART_INF_F;
   for (int r = r_a + lane; r < r_c; r += 32) best = fminf(best, __ldcg(p.part_min + 2 * r));
-  if (gh.lo < gh.hi) best = fminf(best, rs_ragged_min(gh, __ldcg(p.part_min + 2 * (s0 / RS_R) + 1)));
+  if (gh.lo < gh.hi) best = fminf(best, rs_ragged_min(gh, __ldcg(p.part_min + 2 * (s0 / R) + 1)));
   if (gt.lo < gt.hi) best = fminf(best, rs_ragged_min(gt, __ldcg(p.part_min + 2 * r_t + 1)));
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) {

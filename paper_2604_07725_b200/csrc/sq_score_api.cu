@@ -368,7 +368,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   const int64_t T = cfg->max_tokens;
   // kernel 2's partial records: tile forms (one per 8192-token tile) or streaming form (one per 256-token range and sequence)
   ctx->red_tiles_max = std::max<int64_t>(cdiv64(T, sq::RED_TILE) + 2 * (int64_t)cfg->max_seqs + 1,
-                                         2 * cdiv64(T, sq::RS_TB) * sq::RS_WARPS + 2);   // (red_min: two floats per range)
+                                         2 * cdiv64(T, sq::RsCfg<2>::TB) * sq::RS_WARPS + 2);   // (red_min: two floats per range; the smaller ranges)
   int rc = SQ_OK;
   auto A = [&](int r) { if (rc == SQ_OK && r != SQ_OK) rc = r; };
   A(ws_alloc(ctx, &ctx->part_m, rows));
@@ -567,6 +567,9 @@ static cudaError_t launch_wide_finalize(int cap, int T, cudaStream_t st, const s
   return launch_pdl(sq::sq_finalize_wide_kernel<32, EMIT>, grid, block, 0, st, fin);
 }
 
+#ifndef SQ_RS_NV_NOTG
+#define SQ_RS_NV_NOTG 3
+#endif
 static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t st) {
   if (rp.B <= 0) return SQ_OK;
   // 16-byte loads need 16-byte aligned arrays (tiles start on multiples of 4 tokens)
@@ -596,12 +599,16 @@ static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t s
   // Narrow windows stay with the tile forms: the streaming form takes S(j) as a difference of two block-wide prefix sums,
   // whose fp32 rounding (~1e-7 of the prefix) is only negligible against a sum of >= RS_WMIN elements.
   if (rp.vec && rp.window >= sq::RS_WMIN && rp.window <= sq::RS_WMAX && rp.T > 0 &&
-      rp.T <= (int64_t)INT32_MAX - 2 * (sq::RS_TB + sq::RS_WMAX) &&
+      rp.T <= (int64_t)INT32_MAX - 2 * (sq::RsCfg<3>::TB + sq::RS_WMAX) &&
       !(ctx->debug_flags & (32 | 64))) {
-    const dim3 grid((unsigned)cdiv64(rp.T, sq::RS_TB));
-    if (rp.targets) SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_kernel<true>, grid, dim3(sq::RS_THREADS), 0, st, rp));
-    else SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_kernel<false>, grid, dim3(sq::RS_THREADS), 0, st, rp));
-    SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_fold_kernel, dim3((unsigned)cdiv64(rp.B, 4)), dim3(128), 0, st, rp));
+    const dim3 fgrid((unsigned)cdiv64(rp.B, 4));
+    if (rp.targets) {   // four arrays: two vectors per lane and array; three arrays: three (sq_reduce_kernel.cuh)
+      SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_kernel<true, 2>, dim3((unsigned)cdiv64(rp.T, sq::RsCfg<2>::TB)), dim3(sq::RS_THREADS), 0, st, rp));
+      SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_fold_kernel<2>, fgrid, dim3(128), 0, st, rp));
+    } else {
+      SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_kernel<false, SQ_RS_NV_NOTG>, dim3((unsigned)cdiv64(rp.T, sq::RsCfg<SQ_RS_NV_NOTG>::TB)), dim3(sq::RS_THREADS), 0, st, rp));
+      SQ_CUDA(ctx, launch_pdl(sq::sq_reduce_stream_fold_kernel<SQ_RS_NV_NOTG>, fgrid, dim3(128), 0, st, rp));
+    }
     ctx->launches += 2;
     ctx->reduce_form = SQ_REDUCE_FORM_STREAM;
     SQ_CUDA(ctx, cudaGetLastError());
