@@ -28,9 +28,12 @@ constexpr float LOG2E_F = 1.4426950408889634f;   // consume32 takes log2(e) time
 constexpr int BLOCK_N_MX = 224;   // block-scaled variant: 2 x 224 accumulator columns + 12 columns of scale factors fit TMEM's 512
 constexpr int MODE_BF16 = 0, MODE_F8 = 1, MODE_MX = 2;
 
-template <int CG, int MODE = MODE_BF16> struct FusedCfg {
+// AROWS: token rows a stage holds (128; 64 for decode-shaped runs of at most 64 rows, single CTA only: the MMA still reads 128
+// rows -- the second half is the first rows of the W tile behind it, finite values whose accumulator rows nobody looks at --
+// and the 8 KB saved per stage buy a FIFTH stage: an HBM-bound run lives on the W bytes it has in flight).
+template <int CG, int MODE = MODE_BF16, int AROWS = 128> struct FusedCfg {
   static constexpr int BN = (MODE == MODE_MX) ? BLOCK_N_MX : BLOCK_N;   // vocabulary columns per tile
-  static constexpr int A_BYTES = BLOCK_M * BLOCK_K * 2;                 // 16 KB
+  static constexpr int A_BYTES = AROWS * BLOCK_K * 2;                   // 16 KB (8 KB)
   static constexpr int B_ROWS = BN / CG;                                // W rows this CTA stages
   static constexpr int B_BYTES = B_ROWS * BLOCK_K * 2;                  // 32 KB (CG=1) / 16 KB (CG=2); MX: 28 / 14 KB
   // MX: the scale factors of the stage's 128-element k-block: 512 B for this CTA's 128 token rows, 1024 B for ALL the
@@ -42,7 +45,7 @@ template <int CG, int MODE = MODE_BF16> struct FusedCfg {
 #ifndef SQ_STAGES_PAIR
 #define SQ_STAGES_PAIR 6
 #endif
-  static constexpr int STAGES = (CG == 1) ? 4 : SQ_STAGES_PAIR;
+  static constexpr int STAGES = (CG == 1) ? (AROWS == 64 ? 5 : 4) : SQ_STAGES_PAIR;
   static constexpr int BAR_BYTES = 256;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;  // +1024: manual alignment
   static constexpr int UMMA_M = BLOCK_M * CG;
@@ -302,12 +305,13 @@ __device__ __forceinline__ void consume32(RowState<CAP>& st, float (&r)[32], int
 //     operand traffic per k-block and SM falls from 16 KB (H) + 16 KB (W) to 16 + 8 KB.  A stage is free again when
 //     BOTH pairs' MMAs have retired (the commit goes to all four CTAs, the empty barriers count two arrivals).
 //   cluster of 2: the pair loads its own 2 x 64 W rows, as in the plain pair kernel.
-template <int CG, int CAP, int MODE = MODE_BF16, int CL = CG>
+template <int CG, int CAP, int MODE = MODE_BF16, int CL = CG, int AROWS = 128>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_constant__ CUtensorMap tmap_w,
                       const __grid_constant__ CUtensorMap tmap_sfa, const __grid_constant__ CUtensorMap tmap_sfb,
                       const FusedParams p) {
-  using Cfg = FusedCfg<CG, MODE>;
+  using Cfg = FusedCfg<CG, MODE, AROWS>;
+  static_assert(AROWS == 128 || (AROWS == 64 && CG == 1), "half-height token tiles are for single-CTA (decode-shaped) runs");
   constexpr bool F8 = (MODE == MODE_F8);
   constexpr bool MX = (MODE == MODE_MX);
   constexpr int BN = Cfg::BN;
@@ -504,6 +508,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
         tc_fence_after();
         const int colbase = vt * BN;
         int ngroups = min(BN, p.V - colbase + 31) >> 5;   // 32-column groups with a valid column
+        if (AROWS < BLOCK_M && q * 32 >= AROWS) ngroups = 0;   // this warp's TMEM lanes hold no token rows
 #ifdef SQ_PROBES
         if (p.probe_flags & 1) ngroups = 0;        // probe: the epilogue skips the statistics
 #endif

@@ -429,6 +429,13 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
                            sq::FusedCfg<CG, sq::MODE_MX>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
   SQ_SET_SMEM8(1, 8) SQ_SET_SMEM8(1, 20) SQ_SET_SMEM8(1, 32) SQ_SET_SMEM8(2, 8) SQ_SET_SMEM8(2, 20) SQ_SET_SMEM8(2, 32)
 #undef SQ_SET_SMEM8
+#define SQ_SET_SMEM_H(CAP, MODE)                                                                                                 \
+  if (cudaFuncSetAttribute(sq::sq_fused_score_kernel<1, CAP, MODE, 1, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize,         \
+                           sq::FusedCfg<1, MODE, 64>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
+  SQ_SET_SMEM_H(8, sq::MODE_BF16) SQ_SET_SMEM_H(20, sq::MODE_BF16) SQ_SET_SMEM_H(32, sq::MODE_BF16)
+  SQ_SET_SMEM_H(8, sq::MODE_F8) SQ_SET_SMEM_H(20, sq::MODE_F8) SQ_SET_SMEM_H(32, sq::MODE_F8)
+  SQ_SET_SMEM_H(8, sq::MODE_MX) SQ_SET_SMEM_H(20, sq::MODE_MX) SQ_SET_SMEM_H(32, sq::MODE_MX)
+#undef SQ_SET_SMEM_H
   for (const void* f : {(const void*)sq::sq_fused_score_kernel<2, 8, sq::MODE_BF16, 4>, (const void*)sq::sq_fused_score_kernel<2, 20, sq::MODE_BF16, 4>,
                         (const void*)sq::sq_fused_score_kernel<2, 32, sq::MODE_BF16, 4>, (const void*)sq::sq_fused_score_kernel<2, 8, sq::MODE_F8, 4>,
                         (const void*)sq::sq_fused_score_kernel<2, 20, sq::MODE_F8, 4>, (const void*)sq::sq_fused_score_kernel<2, 32, sq::MODE_F8, 4>})
@@ -522,14 +529,14 @@ static int make_tmap_sf(sq_score_ctx* ctx, CUtensorMap* map, const void* base, i
 }
 
 // ------------------------------------------------------------------------------------------ launches
-template <int CG, int CAP, int MODE = sq::MODE_BF16, int CL = CG>
+template <int CG, int CAP, int MODE = sq::MODE_BF16, int CL = CG, int AROWS = 128>
 static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CUtensorMap& th, const CUtensorMap& tw,
                                 const CUtensorMap& tsa, const CUtensorMap& tsb, const sq::FusedParams& fp, cudaStream_t st) {
   const int clusters = pl.clusters_used;   // every launched cluster belongs to a gang
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3((unsigned)(clusters * CL));
   lc.blockDim = dim3(sq::NUM_THREADS);
-  lc.dynamicSmemBytes = sq::FusedCfg<CG, MODE>::SMEM_BYTES;
+  lc.dynamicSmemBytes = sq::FusedCfg<CG, MODE, AROWS>::SMEM_BYTES;
   lc.stream = st;
   cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeClusterDimension;
@@ -542,7 +549,7 @@ static cudaError_t launch_fused(const sq_score_plan_t& pl, int num_sms, const CU
     lc.numAttrs = 2;
   }
   (void)num_sms;
-  return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP, MODE, CL>, th, tw, tsa, tsb, fp);
+  return cudaLaunchKernelEx(&lc, sq::sq_fused_score_kernel<CG, CAP, MODE, CL, AROWS>, th, tw, tsa, tsb, fp);
 }
 
 // Launch with programmatic stream serialization: the kernel is scheduled while its predecessor drains and waits in
@@ -736,7 +743,8 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     if (pl.topk_cap > ctx->cap_max) return set_err(ctx, SQ_ERR_INVALID_ARG, "k exceeds the ctx's max_k capacity");
     CUtensorMap th, tw, tsa, tsb;
     if (f8 && d % 16 != 0) return set_err(ctx, SQ_ERR_UNSUPPORTED, "the FP8 variants need d %% 16 == 0 (TMA 16-byte row strides)");
-    int h_box = sq::BLOCK_M, w_box = tile_n / pl.cta_group;
+    const bool half_a = pl.cta_group == 1 && T <= 64;     // decode-shaped, at most 64 rows: 64-row H boxes, five stages
+    int h_box = half_a ? 64 : sq::BLOCK_M, w_box = tile_n / pl.cta_group;
 #ifdef SQ_PROBES
     if (ctx->probe_flags & 4) h_box /= 2;
     if (ctx->probe_flags & 2) w_box /= 2;
@@ -798,9 +806,20 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     cudaError_t e;
     cudaEvent_t* pev = ctx->profiling ? ctx->ev[ctx->ev_count % SQ_PROFILE_RING] : nullptr;
     if (pev) cudaEventRecord(pev[0], st);
-    const int sel = pl.cta_group * 100 + pl.topk_cap + (mx ? 2000 : (f8 ? 1000 : 0));
+    const int sel = pl.cta_group * 100 + pl.topk_cap + (mx ? 2000 : (f8 ? 1000 : 0)) + (half_a ? 10000 : 0);
 #define SQ_LAUNCH(CG, CAP, MODE) e = launch_fused<CG, CAP, MODE>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break
     switch (sel) {
+#define SQ_LAUNCH_H(CAP, MODE) e = launch_fused<1, CAP, MODE, 1, 64>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break
+      case 12108: SQ_LAUNCH_H(8, sq::MODE_MX);
+      case 12120: SQ_LAUNCH_H(20, sq::MODE_MX);
+      case 12132: SQ_LAUNCH_H(32, sq::MODE_MX);
+      case 11108: SQ_LAUNCH_H(8, sq::MODE_F8);
+      case 11120: SQ_LAUNCH_H(20, sq::MODE_F8);
+      case 11132: SQ_LAUNCH_H(32, sq::MODE_F8);
+      case 10108: SQ_LAUNCH_H(8, sq::MODE_BF16);
+      case 10120: SQ_LAUNCH_H(20, sq::MODE_BF16);
+      case 10132: SQ_LAUNCH_H(32, sq::MODE_BF16);
+#undef SQ_LAUNCH_H
       case 2108: SQ_LAUNCH(1, 8, sq::MODE_MX);
       case 2120: SQ_LAUNCH(1, 20, sq::MODE_MX);
       case 2132: SQ_LAUNCH(1, 32, sq::MODE_MX);
