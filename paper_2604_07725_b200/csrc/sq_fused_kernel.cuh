@@ -28,9 +28,9 @@ constexpr float LOG2E_F = 1.4426950408889634f;   // consume32 takes log2(e) time
 constexpr int BLOCK_N_MX = 224;   // block-scaled variant: 2 x 224 accumulator columns + 12 columns of scale factors fit TMEM's 512
 constexpr int MODE_BF16 = 0, MODE_F8 = 1, MODE_MX = 2;
 
-// AROWS: token rows a stage holds (128; 64 for decode-shaped runs of at most 64 rows, single CTA only: the MMA still reads 128
+// AROWS: token rows a stage holds (128; 64 / 32 for decode-shaped runs of at most 64 / 32 rows, single CTA only: the MMA still reads 128
 // rows -- the second half is the first rows of the W tile behind it, finite values whose accumulator rows nobody looks at --
-// and the 8 KB saved per stage buy a FIFTH stage: an HBM-bound run lives on the W bytes it has in flight).
+// and the 8 / 12 KB saved per stage buy a fifth / sixth stage: an HBM-bound run lives on the W bytes it has in flight).
 template <int CG, int MODE = MODE_BF16, int AROWS = 128> struct FusedCfg {
   static constexpr int BN = (MODE == MODE_MX) ? BLOCK_N_MX : BLOCK_N;   // vocabulary columns per tile
   static constexpr int A_BYTES = AROWS * BLOCK_K * 2;                   // 16 KB (8 KB)
@@ -45,7 +45,7 @@ template <int CG, int MODE = MODE_BF16, int AROWS = 128> struct FusedCfg {
 #ifndef SQ_STAGES_PAIR
 #define SQ_STAGES_PAIR 6
 #endif
-  static constexpr int STAGES = (CG == 1) ? (AROWS == 64 ? 5 : 4) : SQ_STAGES_PAIR;
+  static constexpr int STAGES = (CG == 1) ? (AROWS == 32 ? 6 : (AROWS == 64 ? 5 : 4)) : SQ_STAGES_PAIR;
   static constexpr int BAR_BYTES = 256;
   static constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + BAR_BYTES + 1024;  // +1024: manual alignment
   static constexpr int UMMA_M = BLOCK_M * CG;
@@ -311,7 +311,7 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
                       const __grid_constant__ CUtensorMap tmap_sfa, const __grid_constant__ CUtensorMap tmap_sfb,
                       const FusedParams p) {
   using Cfg = FusedCfg<CG, MODE, AROWS>;
-  static_assert(AROWS == 128 || (AROWS == 64 && CG == 1), "half-height token tiles are for single-CTA (decode-shaped) runs");
+  static_assert(AROWS == 128 || ((AROWS == 64 || AROWS == 32) && CG == 1), "short token tiles are for single-CTA (decode-shaped) runs");
   constexpr bool F8 = (MODE == MODE_F8);
   constexpr bool MX = (MODE == MODE_MX);
   constexpr int BN = Cfg::BN;

@@ -431,7 +431,9 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
 #undef SQ_SET_SMEM8
 #define SQ_SET_SMEM_H(CAP, MODE)                                                                                                 \
   if (cudaFuncSetAttribute(sq::sq_fused_score_kernel<1, CAP, MODE, 1, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize,         \
-                           sq::FusedCfg<1, MODE, 64>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
+                           sq::FusedCfg<1, MODE, 64>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;                              \
+  if (cudaFuncSetAttribute(sq::sq_fused_score_kernel<1, CAP, MODE, 1, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize,         \
+                           sq::FusedCfg<1, MODE, 32>::SMEM_BYTES) != cudaSuccess) rc = SQ_ERR_CUDA;
   SQ_SET_SMEM_H(8, sq::MODE_BF16) SQ_SET_SMEM_H(20, sq::MODE_BF16) SQ_SET_SMEM_H(32, sq::MODE_BF16)
   SQ_SET_SMEM_H(8, sq::MODE_F8) SQ_SET_SMEM_H(20, sq::MODE_F8) SQ_SET_SMEM_H(32, sq::MODE_F8)
   SQ_SET_SMEM_H(8, sq::MODE_MX) SQ_SET_SMEM_H(20, sq::MODE_MX) SQ_SET_SMEM_H(32, sq::MODE_MX)
@@ -743,8 +745,9 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     if (pl.topk_cap > ctx->cap_max) return set_err(ctx, SQ_ERR_INVALID_ARG, "k exceeds the ctx's max_k capacity");
     CUtensorMap th, tw, tsa, tsb;
     if (f8 && d % 16 != 0) return set_err(ctx, SQ_ERR_UNSUPPORTED, "the FP8 variants need d %% 16 == 0 (TMA 16-byte row strides)");
-    const bool half_a = pl.cta_group == 1 && T <= 64;     // decode-shaped, at most 64 rows: 64-row H boxes, five stages
-    int h_box = half_a ? 64 : sq::BLOCK_M, w_box = tile_n / pl.cta_group;
+    // decode-shaped, at most 64 / 32 rows: 64- / 32-row H boxes, five / six stages
+    const int a_rows = (pl.cta_group == 1 && T <= 32) ? 32 : ((pl.cta_group == 1 && T <= 64) ? 64 : sq::BLOCK_M);
+    int h_box = a_rows, w_box = tile_n / pl.cta_group;
 #ifdef SQ_PROBES
     if (ctx->probe_flags & 4) h_box /= 2;
     if (ctx->probe_flags & 2) w_box /= 2;
@@ -806,9 +809,20 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     cudaError_t e;
     cudaEvent_t* pev = ctx->profiling ? ctx->ev[ctx->ev_count % SQ_PROFILE_RING] : nullptr;
     if (pev) cudaEventRecord(pev[0], st);
-    const int sel = pl.cta_group * 100 + pl.topk_cap + (mx ? 2000 : (f8 ? 1000 : 0)) + (half_a ? 10000 : 0);
+    const int sel = pl.cta_group * 100 + pl.topk_cap + (mx ? 2000 : (f8 ? 1000 : 0)) + (a_rows == 64 ? 10000 : (a_rows == 32 ? 20000 : 0));
 #define SQ_LAUNCH(CG, CAP, MODE) e = launch_fused<CG, CAP, MODE>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break
     switch (sel) {
+#define SQ_LAUNCH_Q(CAP, MODE) e = launch_fused<1, CAP, MODE, 1, 32>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break
+      case 22108: SQ_LAUNCH_Q(8, sq::MODE_MX);
+      case 22120: SQ_LAUNCH_Q(20, sq::MODE_MX);
+      case 22132: SQ_LAUNCH_Q(32, sq::MODE_MX);
+      case 21108: SQ_LAUNCH_Q(8, sq::MODE_F8);
+      case 21120: SQ_LAUNCH_Q(20, sq::MODE_F8);
+      case 21132: SQ_LAUNCH_Q(32, sq::MODE_F8);
+      case 20108: SQ_LAUNCH_Q(8, sq::MODE_BF16);
+      case 20120: SQ_LAUNCH_Q(20, sq::MODE_BF16);
+      case 20132: SQ_LAUNCH_Q(32, sq::MODE_BF16);
+#undef SQ_LAUNCH_Q
 #define SQ_LAUNCH_H(CAP, MODE) e = launch_fused<1, CAP, MODE, 1, 64>(pl, ctx->num_sms, th, tw, tsa, tsb, fp, st); break
       case 12108: SQ_LAUNCH_H(8, sq::MODE_MX);
       case 12120: SQ_LAUNCH_H(20, sq::MODE_MX);
