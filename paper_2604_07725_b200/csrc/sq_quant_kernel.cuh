@@ -170,30 +170,40 @@ __global__ void __launch_bounds__(256) sq_quant_mx_kernel(const QuantMxParams p)
     const long long blk = row / p.blk_rows;
     const int r = (int)(row - blk * p.blk_rows);
     const size_t in_region = (size_t)(r >> 7) * 512 + (size_t)(r & 31) * 16 + (size_t)((r >> 5) & 3) * 4;
-    for (int v0 = 0; v0 < nvec; v0 += 32) {                  // 256 elements = 8 scale blocks per pass; 4 lanes per block
-      const int v = v0 + lane;
-      uint4 x = make_uint4(0u, 0u, 0u, 0u);
-      if (v < nvec) x = __ldg(p.X + row * nvec + v);
-      float m = q_amax8(x);
-      m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
-      m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
-      const int e = mx_exponent(m);
-      const int ea = (-e) / 2, eb = (-e) - ea;               // x * 2^ea * 2^eb, both factors normal floats
-      const float fa = __uint_as_float((uint32_t)(ea + 127) << 23), fb = __uint_as_float((uint32_t)(eb + 127) << 23);
-      float f[8];
-      q_unpack8(x, f);
-      uint32_t c[8];
+    constexpr int U = 4;                                     // passes whose loads are issued together (HBM-bound: bytes in flight)
+    for (int v0 = 0; v0 < nvec; v0 += 32 * U) {              // a pass: 256 elements = 8 scale blocks; 4 lanes per block
+      uint4 xs[U];
 #pragma unroll
-      for (int i = 0; i < 8; ++i) c[i] = (uint32_t)__nv_cvt_float_to_fp8(__fmul_rn(__fmul_rn(f[i], fa), fb), __NV_SATFINITE, __NV_E4M3);
-      if (v < nvec) {
-        uint2 o;
-        o.x = c[0] | (c[1] << 8) | (c[2] << 16) | (c[3] << 24);
-        o.y = c[4] | (c[5] << 8) | (c[6] << 16) | (c[7] << 24);
-        p.Q[row * nvec + v] = o;
-        if ((lane & 3) == 0) {
-          const int k = v * 8;                               // first element of the scale block
-          const size_t region = ((size_t)(k >> 7) * (size_t)p.num_blk + (size_t)blk) * (size_t)p.pieces;
-          p.SF[region * 512 + in_region + ((k & 127) >> 5)] = (uint8_t)(e + 127);
+      for (int u = 0; u < U; ++u) {
+        const int v = v0 + 32 * u + lane;
+        xs[u] = make_uint4(0u, 0u, 0u, 0u);
+        if (v < nvec) xs[u] = __ldg(p.X + row * nvec + v);
+      }
+#pragma unroll
+      for (int u = 0; u < U; ++u) {
+        const int v = v0 + 32 * u + lane;
+        const uint4 x = xs[u];
+        float m = q_amax8(x);
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 1));
+        m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, 2));
+        const int e = mx_exponent(m);
+        const int ea = (-e) / 2, eb = (-e) - ea;             // x * 2^ea * 2^eb, both factors normal floats
+        const float fa = __uint_as_float((uint32_t)(ea + 127) << 23), fb = __uint_as_float((uint32_t)(eb + 127) << 23);
+        float f[8];
+        q_unpack8(x, f);
+        uint32_t c[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) c[i] = (uint32_t)__nv_cvt_float_to_fp8(__fmul_rn(__fmul_rn(f[i], fa), fb), __NV_SATFINITE, __NV_E4M3);
+        if (v < nvec) {
+          uint2 o;
+          o.x = c[0] | (c[1] << 8) | (c[2] << 16) | (c[3] << 24);
+          o.y = c[4] | (c[5] << 8) | (c[6] << 16) | (c[7] << 24);
+          p.Q[row * nvec + v] = o;
+          if ((lane & 3) == 0) {
+            const int k = v * 8;                             // first element of the scale block
+            const size_t region = ((size_t)(k >> 7) * (size_t)p.num_blk + (size_t)blk) * (size_t)p.pieces;
+            p.SF[region * 512 + in_region + ((k & 127) >> 5)] = (uint8_t)(e + 127);
+          }
         }
       }
     }
