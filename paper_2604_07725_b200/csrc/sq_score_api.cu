@@ -45,7 +45,8 @@ struct sq_score_ctx {
   unsigned int* amax_bits = nullptr;   // per-tensor amax of sq_score_quantize_fp8
   int* seq_done = nullptr;   // [max_seqs] per-sequence tile counters of the single-launch reduction (zero between runs)
   int* tile_base = nullptr; int* tile_seq = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
-  int cluster4 = 0;                  // experiment (SQ_SCORE_CLUSTER4=1): large bf16 runs in clusters of 4 CTAs with W multicast
+  int cluster4 = -1;                 // quad scheduling with W multicast (sq_fused_kernel.cuh): -1 = for very long runs only (default),
+                                     // 0 = never, 1 = every run of more than 4096 tokens (SQ_SCORE_CLUSTER4)
   int max_clusters[5] = {0, 0, 0, 0, 0};   // [cg]: clusters of kernel 1 the device holds at once (occupancy query at create)
   int region_mult = 0;               // region barrier of kernel 1: regions of region_mult x (a common multiple of the gang sizes) token tiles; < 0: off
   long long wait_limit = 0;          // cycles a device-side wait may last before kernel 1 traps (0 = for ever)
@@ -477,6 +478,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
     }
     if (const char* c4 = getenv("SQ_SCORE_CLUSTER4")) ctx->cluster4 = atoi(c4);
     if (ctx->cluster4) ctx->max_clusters[4] = ctx->max_clusters[2] / 2;   // quads: 4 consecutive CTAs, placed as one cluster of 4 or two of 2
+    if (ctx->max_clusters[4] * 4 != ctx->num_sms / 4 * 4) ctx->max_clusters[4] = 0;   // (only when every quad fits at once)
   }
   *out = ctx;
   return SQ_OK;
@@ -729,7 +731,13 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     pc.vocab = V;
     if (f8) pc.d = (d + 1) / 2;   // an e4m3 k-block is 128 elements: the plan sees half as many k-blocks
     int cg_sel = (pc.cta_group == 1) ? 1 : (pc.cta_group == 2 ? 2 : (T <= 128 ? 1 : 2));
-    if (ctx->cluster4 && cg_sel == 2 && !mx && T > 4096 && ctx->max_clusters[4] > 0) { cg_sel = 4; pc.cta_group = 4; }
+    // Quads pay where kernel 1's energy goes into operand traffic for long: measured +2.4 % at qwen3_32b (T = 5e5), +1.2 % at
+    // gpt_oss, +0.3 % (noise) at qwen3_8b, so by default only runs of more than 200 000 tokens take them.
+    const int quad_min_t = ctx->cluster4 > 0 ? 4096 : 200000;
+    if (ctx->cluster4 != 0 && cg_sel == 2 && !mx && pc.cta_group == 0 && T > quad_min_t && ctx->max_clusters[4] > 0) {
+      cg_sel = 4; pc.cta_group = 4;
+      if (pc.group_m == 0) pc.group_m = 6;             // gangs of 6 quads = 12 strips of 256 rows, the pair kernel's optimum
+    }
     auto& pcache = ctx->plan_cache;
     if (pcache.T == T && pcache.k == k && pcache.V == V && pcache.tile_n == tile_n && pcache.d == pc.d) {
       pl = pcache.pl;

@@ -566,7 +566,8 @@ def test_scoring_pipeline_takes_the_streaming_form_for_many_sequences():
 
 @pytest.mark.parametrize("d,V,B,lo,hi,gm", [(256, 3000, 6, 700, 1100, 0), (200, 1003, 9, 500, 900, 3), (512, 5000, 4, 1500, 2500, 6)])
 def test_quad_scheduling_with_w_multicast(d, V, B, lo, hi, gm):
-    """SQ_SCORE_CLUSTER4=1 (opt-in): runs of more than 4096 tokens are scheduled in quads of four CTAs that
+    """SQ_SCORE_CLUSTER4=1 (by default only runs of more than 200 000 tokens -- the full-size qwen3_32b test --
+    take this path): runs of more than 4096 tokens are scheduled in quads of four CTAs that
     the device places as clusters of 4 (W boxes multicast to both CTA pairs) or, where it cannot, as two pairs; 512-row
     token tiles, ragged T, d and V.  Same tolerances against the oracle; bf16 and the FP8 variant."""
     import os
