@@ -174,6 +174,44 @@ int sq_score_reduce(sq_score_ctx *ctx, const float *target_logprob, const float 
                     float *seq_mean_logprob, float *seq_mean_entropy, float *seq_mean_conf,
                     float *seq_min_window_conf, void *stream);
 
+/* Kernel 2 for callers that cannot allocate device memory -- and therefore cannot call sq_score_create, which
+ * cudaMallocs the workspace.  Two kinds of caller are meant:
+ *   - a plug-in inside a serving engine that has already handed (nearly) all free HBM to its own pool (KV cache,
+ *     activation arena): a cudaMalloc from a library fails there, or eats into a budget the engine believes it owns;
+ *   - code on a latency-critical path (a decode loop, a scheduler callback): cudaMalloc and cudaFree may synchronise
+ *     the whole device, so one allocation stalls every stream of the process.
+ * This call needs NO ctx and calls no cudaMalloc, cudaFree or allocating library routine, neither on its first call nor
+ * later.  It computes what sq_score_reduce computes (same kernel body, the single-launch form; the same bits), with the
+ * tile partials and per-sequence counters the kernel needs kept in a fixed array inside the library's device image
+ * instead of a ctx workspace.  That array costs about 186 KB of HBM on every GPU that loads libsq_score.so, from load to
+ * process exit, whether or not this call is ever made; in exchange the sizes are capped:
+ *     num_tokens <= SQ_STATIC_MAX_TOKENS,   num_seqs <= SQ_STATIC_MAX_SEQS
+ * and anything larger is refused with SQ_ERR_INVALID_ARG (message via sq_score_last_error(NULL)); nothing is launched.
+ *
+ * It runs on the calling thread's CURRENT device (cudaSetDevice is the caller's business; all pointers DEVICE memory of
+ * that device), asynchronously on `stream`: one 4*num_seqs-byte cudaMemsetAsync (the counters must start at zero, and a
+ * call that died half way may have left some behind) and one kernel launch.
+ *   target_logprob, entropy, conf  DEVICE float [num_tokens]
+ *   targets      DEVICE int32 [num_tokens] or NULL (NULL = every target valid)
+ *   cu_seqlens   DEVICE int32 [num_seqs+1]
+ *   vocab        targets outside [0, vocab) are "no target" (sq_score_reduce takes this from its ctx); ignored when
+ *                targets == NULL
+ *   seq_*        DEVICE float [num_seqs], written by this call; the caller owns every buffer it passes
+ * First call on each device: looks up the device address of the array and the SM count and raises the kernel's
+ * dynamic-shared-memory limit (host-side driver calls, no allocation).  Make that first call early, at start-up and
+ * before any stream capture begins; later calls only enqueue work.
+ * One array per device, shared by every call in the process and keeping what the last call left: two calls whose
+ * kernels may overlap on the GPU (different streams with no ordering between them, several host threads) RACE on it
+ * and give wrong results.  Put every call on one stream, or order the streams with events.
+ * Errors: INVALID_ARG (null pointer, negative size, window < 1, vocab < 1 with targets, a size beyond the maximum),
+ * CUDA (no device, not an sm_100 device, a runtime call failed).  Messages: sq_score_last_error(NULL), per thread. */
+#define SQ_STATIC_MAX_TOKENS 4194304   /* 2^22 tokens per call                                    */
+#define SQ_STATIC_MAX_SEQS      4096   /* sequences per call                                      */
+int sq_score_reduce_static(const float *target_logprob, const float *entropy, const float *conf,
+                           const int32_t *targets, const int32_t *cu_seqlens, int64_t num_tokens, int num_seqs,
+                           int vocab, int window, float *seq_mean_logprob, float *seq_mean_entropy,
+                           float *seq_mean_conf, float *seq_min_window_conf, void *stream);
+
 /* The step before the path: gathers the hidden states that predict the scored
  * tokens and applies the scorer's final RMSNorm,
  *     H_out[t,:] = bf16( x / sqrt(mean_j x_j^2 + eps) * gain ),  x = X[pos[t],:]
@@ -387,7 +425,7 @@ int sq_score_reduce_form(const sq_score_ctx *ctx);
 int sq_score_destroy(sq_score_ctx *ctx);
 
 /* Message of the last error on this ctx (ctx-owned, valid until the next call on ctx); with
- * ctx == NULL, the message of the last failed sq_score_create on this thread. */
+ * ctx == NULL, the message of the last failed sq_score_create or sq_score_reduce_static on this thread. */
 const char *sq_score_last_error(const sq_score_ctx *ctx);
 
 /* Static name of an SQ_ERR_* code. */

@@ -12,6 +12,8 @@ SQ_MAX_CHUNKS = 160
 SQ_PROFILE_RING = 64
 FLAG_REDUCE_ONLY = 1
 FLAG_STAGING = 2
+STATIC_MAX_TOKENS = 1 << 22     # SQ_STATIC_MAX_TOKENS / SQ_STATIC_MAX_SEQS: limits of reduce_static
+STATIC_MAX_SEQS = 4096
 MX_OPERAND_H, MX_OPERAND_W = 0, 1
 ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOMEM = -1, -2, -3, -4
 
@@ -64,6 +66,8 @@ def lib() -> C.CDLL:
     L.sq_score_run_host.restype = C.c_int
     L.sq_score_reduce.argtypes = [C.c_void_p] + [C.c_void_p] * 5 + [C.c_int64, C.c_int, C.c_int] + [C.c_void_p] * 5
     L.sq_score_reduce.restype = C.c_int
+    L.sq_score_reduce_static.argtypes = [C.c_void_p] * 5 + [C.c_int64, C.c_int, C.c_int, C.c_int] + [C.c_void_p] * 5
+    L.sq_score_reduce_static.restype = C.c_int
     L.sq_score_route.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int,
                                  C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     L.sq_score_route.restype = C.c_int
@@ -152,6 +156,31 @@ def shard_state_bytes(num_tokens: int, k: int) -> int:
     if n < 0:
         raise SqScoreError(ERR_INVALID_ARG, "bad num_tokens / k")
     return n
+
+
+def reduce_static(target_logprob, entropy, conf, cu_seqlens, window: int, targets=None, vocab: int = 1,
+                  out: Optional[dict] = None, stream=None) -> dict:
+    """sq_score_reduce_static: kernel 2 without a ctx, for callers that cannot allocate device memory (a plug-in inside a
+    serving engine whose pool already owns the free HBM; a latency-critical loop that cannot afford cudaMalloc's
+    device-wide synchronisation).  The library allocates nothing: its scratch is a fixed array in the device image, so at
+    most STATIC_MAX_TOKENS tokens and STATIC_MAX_SEQS sequences per call, and calls that may overlap on the GPU race on
+    it -- keep them on one stream.  Pass `out` (the four float32 [B] tensors of SqScore.reduce) to keep this wrapper
+    from allocating too; without it the result tensors come from torch's allocator.  Runs on the tensors' device."""
+    import torch
+    B = cu_seqlens.shape[0] - 1
+    if out is None:
+        out = {n: torch.empty(B, dtype=torch.float32, device=conf.device)
+               for n in ("seq_mean_logprob", "seq_mean_entropy", "seq_mean_conf", "seq_min_window_conf")}
+    L = lib()
+    with torch.cuda.device(conf.device):          # the call uses the thread's current device
+        s = stream if stream is not None else torch.cuda.current_stream()
+        rc = L.sq_score_reduce_static(_ptr(target_logprob), _ptr(entropy), _ptr(conf), _ptr(targets), _ptr(cu_seqlens),
+                                      conf.shape[0], B, vocab, window, _ptr(out["seq_mean_logprob"]),
+                                      _ptr(out["seq_mean_entropy"]), _ptr(out["seq_mean_conf"]),
+                                      _ptr(out["seq_min_window_conf"]), s.cuda_stream)
+    if rc != 0:
+        raise SqScoreError(rc, L.sq_score_last_error(None).decode())
+    return out
 
 
 def shard_vocab(vocab: int, world_size: int, multiple: int = 256) -> List[int]:

@@ -13,6 +13,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 #include "sq_finalize_kernel.cuh"
@@ -672,6 +673,95 @@ extern "C" int sq_score_reduce(sq_score_ctx* ctx, const float* target_logprob, c
   rp.tile_base = ctx->tile_base; rp.tile_seq = ctx->tile_seq; rp.part_sum = ctx->red_sum; rp.part_min = ctx->red_min;
   rp.out_lp = seq_mean_logprob; rp.out_ent = seq_mean_entropy; rp.out_conf = seq_mean_conf; rp.out_min = seq_min_window_conf;
   return launch_reduce(ctx, rp, static_cast<cudaStream_t>(stream));
+}
+
+// ------------------------------------------------------------------------------------------ kernel 2 without a ctx
+// sq_score_reduce_static (include/sq_score.h): kernel 2's single-launch form for callers that must not allocate.  What
+// a ctx keeps in cudaMalloc'ed workspace -- one float4 + one float per tile, one counter per sequence -- lives in the
+// array below, which is part of the library's device image: the driver places it when the module is loaded on a device
+// and it stays until the process exits.  Sized for the stated maxima (tiles <= ceil(T / RED_TILE) + 2 B).
+constexpr int64_t STATIC_MAX_TILES = (SQ_STATIC_MAX_TOKENS + sq::RED_TILE - 1) / sq::RED_TILE + 2 * (int64_t)SQ_STATIC_MAX_SEQS;
+constexpr size_t STATIC_OFF_SUM = 0;                                                                  // float4 [tiles]
+constexpr size_t STATIC_OFF_MIN = (STATIC_OFF_SUM + STATIC_MAX_TILES * sizeof(float4) + 255) / 256 * 256;   // float [tiles]
+constexpr size_t STATIC_OFF_DONE = (STATIC_OFF_MIN + STATIC_MAX_TILES * sizeof(float) + 255) / 256 * 256;   // int [seqs]
+constexpr size_t STATIC_BYTES = (STATIC_OFF_DONE + SQ_STATIC_MAX_SEQS * sizeof(int) + 255) / 256 * 256;
+static_assert(SQ_STATIC_MAX_SEQS <= sq::RED_FUSED_MAX_SEQS, "the single-launch form keeps B + 1 ints in shared memory");
+static_assert(STATIC_BYTES <= 256 * 1024, "keep the resident scratch modest: every GPU that loads the library holds it");
+
+static __device__ __align__(256) unsigned char g_static_scratch[STATIC_BYTES];
+
+// In host code `g_static_scratch` is only a handle for the runtime's symbol table, not a device address: the address a
+// kernel may use comes from cudaGetSymbolAddress, per device (every device has its own copy of the array).
+constexpr int STATIC_MAX_DEVICES = 64;
+struct StaticDev { unsigned char* base; int num_sms; };
+static StaticDev g_static_dev[STATIC_MAX_DEVICES] = {};
+static std::mutex g_static_mu;
+
+// Set-up of the calling thread's current device `dev`, once: host-side queries only, nothing is allocated.
+static int static_setup(int dev, StaticDev* out) {
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_dev[dev].base) {
+    int major = 0, sms = 0;
+    SQ_CUDA(nullptr, cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10)
+      return set_err(nullptr, SQ_ERR_CUDA, "device %d is sm_%dx; the kernels are built for sm_100a only", dev, major);
+    SQ_CUDA(nullptr, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    unsigned char* base = nullptr;
+    SQ_CUDA(nullptr, cudaGetSymbolAddress(reinterpret_cast<void**>(&base), g_static_scratch));
+    if (!base || ((uintptr_t)base & 255)) return set_err(nullptr, SQ_ERR_CUDA, "cudaGetSymbolAddress gave %p for the scratch array", (void*)base);
+    // the same limit sq_score_create sets (it is per kernel and device, shared with every ctx: never a smaller one)
+    for (const void* f : {(const void*)sq::sq_reduce_fused_kernel<true>, (const void*)sq::sq_reduce_fused_kernel<false>})
+      SQ_CUDA(nullptr, cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                            sq::RED_SMEM_BYTES + (sq::RED_FUSED_MAX_SEQS + 1) * (int)sizeof(int)));
+    g_static_dev[dev].num_sms = sms;
+    g_static_dev[dev].base = base;
+  }
+  *out = g_static_dev[dev];
+  return SQ_OK;
+}
+
+extern "C" int sq_score_reduce_static(const float* target_logprob, const float* entropy, const float* conf,
+                                      const int32_t* targets, const int32_t* cu_seqlens, int64_t num_tokens, int num_seqs,
+                                      int vocab, int window, float* seq_mean_logprob, float* seq_mean_entropy,
+                                      float* seq_mean_conf, float* seq_min_window_conf, void* stream) {
+  if (num_tokens < 0 || num_seqs < 0 || window < 1)
+    return set_err(nullptr, SQ_ERR_INVALID_ARG, "sq_score_reduce_static: T, B >= 0 and window >= 1 required");
+  if (num_tokens > SQ_STATIC_MAX_TOKENS || num_seqs > SQ_STATIC_MAX_SEQS)
+    return set_err(nullptr, SQ_ERR_INVALID_ARG,
+                   "sq_score_reduce_static: T = %lld / B = %d exceed the fixed scratch (at most %d tokens and %d sequences per "
+                   "call); larger inputs need sq_score_create + sq_score_reduce",
+                   (long long)num_tokens, num_seqs, SQ_STATIC_MAX_TOKENS, SQ_STATIC_MAX_SEQS);
+  if (num_seqs == 0) return SQ_OK;
+  if (!cu_seqlens || !seq_mean_logprob || !seq_mean_entropy || !seq_mean_conf || !seq_min_window_conf ||
+      (num_tokens > 0 && (!target_logprob || !entropy || !conf)))
+    return set_err(nullptr, SQ_ERR_INVALID_ARG, "sq_score_reduce_static: null pointer argument");
+  if (targets && vocab < 1) return set_err(nullptr, SQ_ERR_INVALID_ARG, "sq_score_reduce_static: vocab >= 1 required with targets");
+  int dev = -1;
+  SQ_CUDA(nullptr, cudaGetDevice(&dev));
+  if (dev < 0 || dev >= STATIC_MAX_DEVICES) return set_err(nullptr, SQ_ERR_CUDA, "sq_score_reduce_static: device ordinal %d not supported", dev);
+  StaticDev sd;
+  const int rc = static_setup(dev, &sd);
+  if (rc != SQ_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  sq::ReduceParams rp = {};
+  rp.T = num_tokens; rp.B = num_seqs; rp.V = targets ? vocab : 1; rp.window = window;
+  rp.lp = target_logprob; rp.ent = entropy; rp.conf = conf; rp.targets = targets; rp.cu = cu_seqlens;
+  rp.part_sum = reinterpret_cast<float4*>(sd.base + STATIC_OFF_SUM);
+  rp.part_min = reinterpret_cast<float*>(sd.base + STATIC_OFF_MIN);
+  rp.seq_done = reinterpret_cast<int*>(sd.base + STATIC_OFF_DONE);
+  rp.out_lp = seq_mean_logprob; rp.out_ent = seq_mean_entropy; rp.out_conf = seq_mean_conf; rp.out_min = seq_min_window_conf;
+  rp.vec = ((((uintptr_t)rp.lp | (uintptr_t)rp.ent | (uintptr_t)rp.conf | (uintptr_t)rp.targets) & 15) == 0) ? 1 : 0;
+  // the array keeps the last call's contents: the counters must be zero when the kernel starts
+  SQ_CUDA(nullptr, cudaMemsetAsync(rp.seq_done, 0, (size_t)num_seqs * sizeof(int), st));
+  const int64_t tiles = cdiv64(num_tokens, sq::RED_TILE) + 2 * (int64_t)num_seqs;   // <= STATIC_MAX_TILES by the size check
+  const size_t smem = sq::RED_SMEM_BYTES + (size_t)(num_seqs + 1) * sizeof(int);
+  const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(6, (size_t)(220 * 1024) / (smem + 1024)));
+  const unsigned grid = (unsigned)std::max<int64_t>(1, std::min<int64_t>(tiles, (int64_t)sd.num_sms * per_sm));
+  // a plain launch behind the memset (no programmatic serialization: cudaGridDependencySynchronize() is then a no-op)
+  if (targets) sq::sq_reduce_fused_kernel<true><<<grid, sq::RED_THREADS, smem, st>>>(rp);
+  else sq::sq_reduce_fused_kernel<false><<<grid, sq::RED_THREADS, smem, st>>>(rp);
+  SQ_CUDA(nullptr, cudaGetLastError());
+  return SQ_OK;
 }
 
 // Packed partial state of one vocab-parallel shard, in 4-byte words (the exchange unit of sq_score_run_shard /
