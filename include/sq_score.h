@@ -63,6 +63,8 @@ extern "C" {
                                      events.  Without it those two calls return INVALID_ARG.     */
 
 #define SQ_MAX_CHUNKS       160   /* vocab chunks per row at most                                 */
+#define SQ_MAX_VOCAB   14679840   /* largest V: 65535 vocab tiles (16-bit tile indices) of the narrowest
+                                     tile, the MX variant's 224 columns                           */
 
 typedef struct sq_score_ctx sq_score_ctx;   /* opaque */
 
@@ -81,7 +83,9 @@ typedef struct {
                            share one W stream; >0 forces it                                       */
   int     flags;        /* SQ_FLAG_*                                                              */
   int     wait_seconds; /* how long a device-side wait (pipeline barrier, gang barrier, H arrival
-                           flag) may last before kernel 1 traps: 0 = default (60 s), < 0 = for ever */
+                           flag) may last before kernel 1 traps: 0 = default (60 s), < 0 = for ever.
+                           One limit for every wait: in sq_score_run_host the copy of the whole H must
+                           land within it                                                          */
 } sq_score_config;
 
 /* Output pointers of one run.  Per-token pointers may be NULL (= not wanted; the ctx keeps the
@@ -126,7 +130,7 @@ typedef struct {
 
 /* Creates a context on cfg->device and allocates its workspace (and, with SQ_FLAG_STAGING, the staging of
  * sq_score_run_host / sq_score_run_x); queries how many clusters of kernel 1 the device can hold at once.
- * Errors: INVALID_ARG (null, sizes <= 0, max_k out of range), UNSUPPORTED (d % 8 != 0, vocab > 2^24, device
+ * Errors: INVALID_ARG (null, sizes <= 0, max_k out of range), UNSUPPORTED (d % 8 != 0, vocab > SQ_MAX_VOCAB, device
  * is not compute capability 10.x, or it cannot hold even one cluster of kernel 1), CUDA, NOMEM.  On error
  * *out is NULL. */
 int sq_score_create(const sq_score_config *cfg, sq_score_ctx **out);

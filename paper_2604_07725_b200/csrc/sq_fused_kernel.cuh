@@ -157,7 +157,10 @@ __device__ __forceinline__ void wait_rows_ready(const unsigned int* flag, long l
     asm volatile("ld.acquire.sys.global.u32 %0, [%1];" : "=r"(v) : "l"(flag) : "memory");
     if (v != 0u) break;
     __nanosleep(200);
-    if (limit > 0 && clock64() - t0 > 8 * limit) __trap();   // a PCIe copy of the whole H may be ahead of this block
+    // the same limit as every other wait of the kernel: the consumers of this producer (full_bar, tfull_bar, the
+    // other clusters' gang and region barriers) give up after `limit` anyway, so a longer allowance here could never
+    // take effect -- in sq_score_run_host the whole copy of H must land within cfg.wait_seconds
+    if (limit > 0 && clock64() - t0 > limit) __trap();
   } while (true);
   asm volatile("fence.proxy.async;" ::: "memory");   // the rows are read through the async proxy (TMA)
 }

@@ -313,8 +313,9 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   if (cfg->cta_group < 0 || cfg->cta_group > 2 || cfg->num_chunks < 0 || cfg->group_m < 0 ||
       (cfg->flags & ~(SQ_FLAG_REDUCE_ONLY | SQ_FLAG_STAGING)))
     return set_err(nullptr, SQ_ERR_INVALID_ARG, "cta_group must be 0, 1 or 2; num_chunks, group_m >= 0; unknown flag");
-  if (cfg->vocab > (1 << 24))
-    return set_err(nullptr, SQ_ERR_UNSUPPORTED, "vocab = %d exceeds 2^24 (vocab-tile indices are 16-bit)", cfg->vocab);
+  if (cfg->vocab > SQ_MAX_VOCAB)   // 65535 tiles of the narrowest tile width (224 columns, MX variant)
+    return set_err(nullptr, SQ_ERR_UNSUPPORTED, "vocab = %d exceeds %d (vocab-tile indices are 16-bit: at most 65535 tiles of 224 columns)",
+                   cfg->vocab, SQ_MAX_VOCAB);
   if (cfg->d % 8 != 0)
     return set_err(nullptr, SQ_ERR_UNSUPPORTED, "d = %d is not a multiple of 8 (TMA needs 16-byte row strides)", cfg->d);
   if (cfg->max_tokens >= (1LL << 31) - 16384)
@@ -354,6 +355,7 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
     long long sec = cfg->wait_seconds == 0 ? 60 : cfg->wait_seconds;
     if (const char* rm = getenv("SQ_SCORE_REGION_MULT")) ctx->region_mult = atoi(rm);   // experiment knob (same results): -1 = no region barrier
     if (const char* w = getenv("SQ_SCORE_WAIT_SECONDS")) sec = atoll(w) == 0 ? -1 : atoll(w);
+    sec = std::min<long long>(sec, 1000000000LL);   // keeps the cycle count far inside 63 bits (31 years are for ever too)
     ctx->wait_limit = sec < 0 ? 0 : sec * (long long)std::max(khz, 1000000) * 1000LL;
   }
 
@@ -841,6 +843,8 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
       pcache.T = T; pcache.k = k; pcache.V = V; pcache.tile_n = tile_n; pcache.d = pc.d; pcache.pl = pl;
     }
     if (pl.topk_cap > ctx->cap_max) return set_err(ctx, SQ_ERR_INVALID_ARG, "k exceeds the ctx's max_k capacity");
+    if (pl.num_vtiles > 65535)   // FusedParams::chunk_vt is 16-bit: the last chunk's end would wrap to 0 and the chunk be skipped
+      return set_err(ctx, SQ_ERR_UNSUPPORTED, "%d vocab tiles of %d columns exceed the 16-bit tile index", pl.num_vtiles, tile_n);
     CUtensorMap th, tw, tsa, tsb;
     if (f8 && d % 16 != 0) return set_err(ctx, SQ_ERR_UNSUPPORTED, "the FP8 variants need d %% 16 == 0 (TMA 16-byte row strides)");
     // decode-shaped, at most 64 / 32 rows: 64- / 32-row H boxes, five / six stages

@@ -75,6 +75,13 @@ def test_create_rejects_bad_config_before_touching_cuda():
     cfg = binding.sq_score_config(device=0, d=60, vocab=1024, max_tokens=256, max_seqs=4, max_k=5)
     assert L.sq_score_create(ctypes.byref(cfg), ctypes.byref(h)) == sq.ERR_UNSUPPORTED      # d % 8 != 0
     assert b"multiple of 8" in L.sq_score_last_error(None)
+    # vocab tiles are indexed in 16 bits: 65535 tiles of the narrowest tile (224 columns, MX variant) is the limit --
+    # one row more would make the last chunk's end wrap to 0 in FusedParams::chunk_vt (a skipped chunk, stale results)
+    cfg = binding.sq_score_config(device=0, d=64, vocab=65535 * 224 + 1, max_tokens=256, max_seqs=4, max_k=5)
+    assert L.sq_score_create(ctypes.byref(cfg), ctypes.byref(h)) == sq.ERR_UNSUPPORTED
+    assert b"16-bit" in L.sq_score_last_error(None) and h.value is None
+    for tile_n in (224, 256):          # the largest accepted vocab plans to at most 65535 tiles at either tile width
+        assert -(-(65535 * 224) // tile_n) <= 65535
     assert L.sq_score_create(None, ctypes.byref(h)) == sq.ERR_INVALID_ARG
     assert L.sq_score_destroy(None) == 0
 
