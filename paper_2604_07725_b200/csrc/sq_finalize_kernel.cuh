@@ -67,7 +67,9 @@ __device__ __forceinline__ void fin_tail_reduce(const FinalizeParams& p, double*
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   double* pre = s_prefix + warp * (FIN_TAIL_MAX_T + 1);
   for (int b = warp; b < p.tail_B; b += NWARPS) {
-    const int s0 = p.tail_cu[b], s1 = p.tail_cu[b + 1];
+    // cu_seqlens is device data nobody has checked (sq_score_positions emits an inconsistent one when its status is
+    // non-zero): clamped into [0, T], T <= FIN_TAIL_MAX_T, so that `pre` and the per-token arrays are never overrun
+    const int s0 = min(max(p.tail_cu[b], 0), p.T), s1 = min(max(p.tail_cu[b + 1], s0), p.T);
     const int L = s1 - s0;
     if (L <= 0) {
       if (lane == 0) { const float nan = __int_as_float(0x7fc00000); p.tail_out_lp[b] = nan; p.tail_out_ent[b] = nan; p.tail_out_conf[b] = nan; p.tail_out_min[b] = nan; }

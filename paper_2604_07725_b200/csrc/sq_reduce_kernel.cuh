@@ -633,11 +633,15 @@ __global__ void __launch_bounds__(128) sq_reduce_stream_fold_kernel(const Reduce
   constexpr int R = RsCfg<NV>::R, PL = R / 32;
   const int b = blockIdx.x * 4 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
-  if (b >= p.B) return;
+  // Every warp waits for the stream kernel before it leaves, also those with nothing to fold: a fold grid that finished
+  // without waiting (every sequence empty) would leave "this kernel is complete => the stream kernel is complete" to
+  // unspecified behaviour of programmatic launches, and the stream kernel still writes the ctx's records.
+  if (b >= p.B) { cudaGridDependencySynchronize(); return; }
   const int s0 = __ldg(p.cu + b), s1 = __ldg(p.cu + b + 1);
   const int L = s1 - s0, w = p.window;
   if (L <= 0) {
     if (lane == 0) { const float nan = CUDART_NAN_F; p.out_lp[b] = nan; p.out_ent[b] = nan; p.out_conf[b] = nan; p.out_min[b] = nan; }
+    cudaGridDependencySynchronize();
     return;
   }
   // sums: the ranges [r_a, r_b) lie inside the sequence; what is left of it are the tokens [s0, h1) and [t0, s1)

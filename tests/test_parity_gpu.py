@@ -534,6 +534,58 @@ def test_reduce_streaming_form_many_sequences_per_range_and_one_long_sequence():
     eng.close()
 
 
+def test_reduce_streaming_form_every_sequence_empty_then_a_normal_call():
+    """Every warp of the fold kernel leaves early (all sequences empty although T > 0: a cu_seqlens the caller got wrong):
+    NaNs everywhere, and the next call on the ctx -- whose stream kernel overwrites the same records -- is correct, i.e. the
+    fold grid did not finish ahead of the stream kernel it was launched behind."""
+    import os
+    sq = _sq()
+    r = workloads.reduction_inputs(300, 100, 900, seed=9)
+    dev = torch.device("cuda:0")
+    os.environ["SQ_SCORE_DEBUG"] = "256"
+    try:
+        eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True)
+    finally:
+        os.environ.pop("SQ_SCORE_DEBUG", None)
+    a = [r[n].to(dev) for n in ("target_logprob", "entropy", "conf", "cu_seqlens")]
+    empty = eng.reduce(a[0], a[1], a[2], torch.zeros_like(a[3]), 256)
+    out = eng.reduce(a[0], a[1], a[2], a[3], 256)                 # enqueued right behind it, no host sync between
+    torch.cuda.synchronize()
+    assert eng.reduce_form() == "stream"
+    for n in SEQ_KEYS:
+        assert torch.isnan(empty[n]).all(), n
+    ref = O.sequence_scores(r["target_logprob"].numpy(), r["entropy"].numpy(), r["conf"].numpy(), r["cu_seqlens"].numpy(), 256)
+    check_seqs({n: v.cpu().numpy() for n, v in out.items()}, ref)
+    eng.close()
+
+
+def test_small_run_with_an_inconsistent_cu_seqlens_stays_inside_its_arrays():
+    """cu_seqlens is device data nobody checks (sq_score_positions writes an inconsistent one when its status is non-zero).
+    In a run of at most 256 tokens the finalize tail clamps it into [0, T]: a last entry far beyond T, and a negative
+    one, neither overrun the 257-entry prefix in shared memory nor the per-token arrays; sequences whose bounds are
+    sound keep their values, a clamped one is reduced over the tokens that exist."""
+    sq = _sq()
+    wl = workloads.custom(name="badcu", d=64, V=3000, B=3, k=20, window=16, seed=37, w_std=0.2,
+                          planted_frac=0.5, planted_scale=3.0, rmsnorm=True)
+    inp = workloads.make_inputs(wl, lengths=[100, 60, 96])                        # T = 256
+    dev = torch.device("cuda:0")
+    eng = sq.SqScore(wl.d, wl.V, max_tokens=256, max_seqs=3, max_k=20)
+    H, W, tg = inp["H"].to(dev), inp["W"].to(dev), inp["targets"].to(dev)
+    good = eng.run(H, W, tg, inp["cu_seqlens"].to(dev), 20, 16)
+    torch.cuda.synchronize()
+    assert eng.reduce_form() == "tail"
+    bad = eng.run(H, W, tg, torch.tensor([0, 100, 160, 100000], dtype=torch.int32, device=dev), 20, 16)   # end >> T
+    neg = eng.run(H, W, tg, torch.tensor([-500, 100, 160, 256], dtype=torch.int32, device=dev), 20, 16)   # start < 0
+    torch.cuda.synchronize()
+    again = eng.run(H, W, tg, inp["cu_seqlens"].to(dev), 20, 16)
+    torch.cuda.synchronize()
+    for n in SEQ_KEYS:
+        assert torch.equal(bad[n], good[n]), n            # [160, 100000) clamps to [160, 256): the sequence that exists
+        assert torch.equal(neg[n], good[n]), n            # [-500, 100) clamps to [0, 100)
+        assert torch.equal(again[n], good[n]), n
+    eng.close()
+
+
 def test_scoring_pipeline_takes_the_streaming_form_for_many_sequences():
     """sq_score_run on a population of 2 300 candidates (more than one wave of kernel-2 tiles): kernel 1 -> finalize ->
     streaming form of kernel 2, chained by programmatic dependent launches.  The per-sequence outputs against oracle-B
