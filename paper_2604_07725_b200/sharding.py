@@ -63,12 +63,22 @@ def score_vocab_parallel(eng, H, W_shard, vocab_starts: Sequence[int], rank: int
     rows = int(vocab_starts[rank + 1]) - int(vocab_starts[rank])
     if rows != W_shard.shape[0]:
         raise ValueError("W_shard has %d rows, vocab_starts gives this rank %d" % (W_shard.shape[0], rows))
-    if rows > 0:
-        state = eng.run_shard(H, W_shard, vocab_starts[rank], targets, k, stream=stream)
-    else:                                                  # more ranks than vocab tiles: this rank owns no rows
-        state = eng.neutral_shard_state(H.shape[0], k, device=H.device, stream=stream)
-    states = gather_shard_states(state, world, group=group, stream=stream)
-    return eng.merge_shards(states, vocab_starts, targets, cu_seqlens, k, window, stream=stream)
+
+    def step():
+        if rows > 0:
+            state = eng.run_shard(H, W_shard, vocab_starts[rank], targets, k, stream=stream)
+        else:                                              # more ranks than vocab tiles: this rank owns no rows
+            state = eng.neutral_shard_state(H.shape[0], k, device=H.device, stream=stream)
+        states = gather_shard_states(state, world, group=group, stream=stream)
+        return eng.merge_shards(states, vocab_starts, targets, cu_seqlens, k, window, stream=stream)
+
+    # The packed state, the gathered states and the outputs are allocated here and used by kernels on `stream`: with
+    # `stream` current the caching allocator ties those blocks to it, so a block freed when this function returns is not
+    # handed to another stream's tensor while kernels on `stream` still read or write it.
+    if stream is not None and H.is_cuda:
+        with torch.cuda.stream(stream):
+            return step()
+    return step()
 
 
 class PeerStates:
@@ -144,10 +154,14 @@ def gather_shard_states(state: torch.Tensor, world_size: int, group=None, stream
     with `stream` current, so it is ordered after the shard kernels and before the merge on that stream by stream
     order alone: no host synchronisation."""
     import torch.distributed as dist
-    flat = torch.empty(world_size * state.numel(), dtype=state.dtype, device=state.device)
     if state.is_cuda:
-        with torch.cuda.stream(stream if stream is not None else torch.cuda.current_stream(state.device)):
+        s = stream if stream is not None else torch.cuda.current_stream(state.device)
+        with torch.cuda.stream(s):
+            # allocated with `s` current (see score_vocab_parallel); `state` may come from another stream's pool
+            flat = torch.empty(world_size * state.numel(), dtype=state.dtype, device=state.device)
             dist.all_gather_into_tensor(flat, state, group=group)
+        state.record_stream(s)
     else:
+        flat = torch.empty(world_size * state.numel(), dtype=state.dtype, device=state.device)
         dist.all_gather_into_tensor(flat, state, group=group)
     return flat.view(world_size, state.numel())

@@ -51,6 +51,18 @@ def test_nccl_world_size_one_runs_both_exchanges():
             peers = sharding.PeerStates(state, 0, 1)
             out_p = sharding.score_vocab_parallel_peer(eng, peers, H, W, [0, wl.V], tg, cu, wl.k, wl.window, stream=st)
         st.synchronize()
+        # a stream that is NOT the current one: what the step allocates (packed state, gathered states, outputs) must still
+        # belong to that stream -- default-stream tensors allocated right behind the call must not land on its blocks
+        st2 = torch.cuda.Stream()
+        st2.wait_stream(torch.cuda.current_stream())
+        assert torch.cuda.current_stream() != st2
+        out_s = sharding.score_vocab_parallel(eng, H, W, [0, wl.V], 0, tg, cu, wl.k, wl.window, stream=st2)
+        junk = [torch.full((sq.shard_state_bytes(inp["T"], wl.k) // 4,), float("nan"), device=dev) for _ in range(8)]
+        st2.synchronize()
+        torch.cuda.synchronize()
+        del junk
+        for n in ("lse", "conf", "topk_index", "seq_min_window_conf"):
+            assert torch.equal(torch.nan_to_num(out_s[n].float(), nan=-7.0), torch.nan_to_num(out_v[n].float(), nan=-7.0)), n
         for n in ("lse", "conf", "topk_index", "seq_min_window_conf"):             # (the empty sequence's NaN equals itself here)
             assert torch.equal(torch.nan_to_num(out_p[n].float(), nan=-7.0), torch.nan_to_num(out_v[n].float(), nan=-7.0)), n
         assert got["seq_mean_conf"].is_cuda
