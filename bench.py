@@ -154,9 +154,12 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": tps, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        # the same keys as the GPU arm's config (the workload entries carry the same values; the rest describe this arm)
         "config": {"workload": wl.name, "d": wl.d, "V": wl.V, "B": inp["B"], "T": inp["T"], "k": wl.k,
-                   "window": wl.window, "sample_rows_per_step": rows},
-        "cpu_baseline": {"value": tps, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+                   "window": wl.window, "parallelism": "none (fp64 oracle on the host cores of rank 0)",
+                   "exchange_bytes_per_step": 0, "l2": "n/a (host arm)", "plan": None},
+        "cpu_baseline": {"value": tps, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                         "sample_rows_per_step": rows},
         "e2e": {"value": tps, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -199,17 +202,30 @@ def run_ours(args):
     rank, world, local = dist_env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the sq_score path has no CPU fallback")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
     vocab_mode = args.parallelism in ("vocab", "vocab-peer")
     peer_mode = args.parallelism == "vocab-peer"
+    ndev = torch.cuda.device_count()
+    if args.share_device:
+        # debug: every rank on the visible devices round-robin (two ranks on one GPU).  NCCL refuses two ranks on one
+        # device, so the exchange goes through gloo on host tensors; the ranks' kernels never wait on one another (dp
+        # only: the one collective is a host-side gather after each rank's own step).  Not a measurement.
+        if vocab_mode:
+            raise SystemExit("bench.py: --share-device is a debug mode of the data-parallel path only")
+        local = local % max(1, ndev)
+    elif local >= ndev:
+        raise SystemExit("bench.py: rank %d needs cuda:%d but only %d CUDA device(s) are visible" % (rank, local, ndev))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    coll_dev = torch.device("cpu") if args.share_device else dev     # where the collectives' tensors live
     use_dist = world > 1 or vocab_mode          # vocab mode runs its collective through NCCL even at world size 1
     if use_dist:
         import torch.distributed as dist
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         os.environ.setdefault("MASTER_PORT", "29531")
-        os.environ.setdefault("NCCL_DEBUG", "WARN")
-        dist.init_process_group("nccl", device_id=dev, rank=rank, world_size=world)
+        if args.share_device:
+            dist.init_process_group("gloo", rank=rank, world_size=world)
+        else:                                   # NCCL_DEBUG is left to the environment (INFO shows the NVLS / ring choice)
+            dist.init_process_group("nccl", device_id=dev, rank=rank, world_size=world)
 
     peaks = load_peaks()
     wl = workloads.CONFIGS[args.config]
@@ -256,7 +272,9 @@ def run_ours(args):
             exchange_bytes = world * B * world * 5 * 4
             def step_fn(o):
                 o = eng.run(H, W, tg, cu, wl.k, wl.window, stream=stream, out=o)
-                o["gathered"] = sharding.gather_sequence_scores(o, seq_ids, B * world, world, device=dev)
+                if args.share_device:
+                    stream.synchronize()        # gloo gathers host tensors: the step's scalars must have landed
+                o["gathered"] = sharding.gather_sequence_scores(o, seq_ids, B * world, world, device=coll_dev)
                 return o
         else:
             step_fn = None
@@ -300,7 +318,7 @@ def run_ours(args):
         e2e_ok = bool(torch.allclose(seq_dev.cpu(), seq_pin, rtol=1e-5, atol=1e-6, equal_nan=True))
 
     # ---------------- max over ranks
-    t_loc = torch.tensor([ms_step, e2e_s * 1e3, float(T)], dtype=torch.float64, device=dev)
+    t_loc = torch.tensor([ms_step, e2e_s * 1e3, float(T)], dtype=torch.float64, device=coll_dev)
     if use_dist:
         tmax = t_loc.clone(); dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
         tsum = t_loc.clone(); dist.all_reduce(tsum, op=dist.ReduceOp.SUM)
@@ -672,6 +690,28 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def launch_command(gpus: int, argv, port: int):
+    """The command `python bench.py --gpus N` turns itself into when it was not started by torchrun: one rank per GPU on
+    this node, rendezvous on 127.0.0.1 (the container's hostname may not resolve)."""
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(gpus),
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
+def self_launch(args, argv) -> int:
+    """`--gpus N` with N > 1 outside torchrun (no WORLD_SIZE in the environment): start the N ranks ourselves.  Refuses
+    loudly when the node shows fewer than N devices, unless --share-device (debug) lets ranks share one."""
+    import socket
+    import subprocess
+    ndev = torch.cuda.device_count()
+    if ndev < args.gpus and not args.share_device:
+        raise SystemExit("bench.py: --gpus %d needs %d CUDA devices, %d visible (no silent single-GPU run; "
+                         "--share-device puts the ranks on the devices there are, for debugging only)" % (args.gpus, args.gpus, ndev))
+    if ndev < 1:
+        raise SystemExit("bench.py: no CUDA device; the sq_score path has no CPU fallback")
+    sock = socket.socket(); sock.bind(("127.0.0.1", 0)); port = sock.getsockname()[1]; sock.close()
+    return subprocess.call(launch_command(args.gpus, argv, port))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -694,7 +734,15 @@ def main():
     ap.add_argument("--cta-group", type=int, default=0)
     ap.add_argument("--num-chunks", type=int, default=0)
     ap.add_argument("--group-m", type=int, default=0)
+    ap.add_argument("--share-device", action="store_true",
+                    help="debug: ranks may share a GPU (gloo for the gather instead of NCCL); not a measurement")
     args = ap.parse_args()
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    if "WORLD_SIZE" in os.environ and int(os.environ["WORLD_SIZE"]) != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but the launcher started %s ranks" % (args.gpus, os.environ["WORLD_SIZE"]))
+    if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(self_launch(args, sys.argv[1:]))
     if args.impl == "reference":
         if args.oracle_seconds is None:
             args.oracle_seconds = max(1.0, 90.0 / (args.steps + 1))
