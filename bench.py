@@ -359,7 +359,7 @@ def run_ours(args):
         "config": {"workload": wl.name, "d": d, "V": V, "B": B, "T": T, "k": wl.k, "window": wl.window,
                    "parallelism": par, "exchange_bytes_per_step": exchange_bytes,
                    "l2": "inputs larger than L2 (H %.0f MB + W %.0f MB re-streamed every step)" % (T * d * 2 / 1e6, v_rank * d * 2 / 1e6),
-                   "plan": pl},
+                   "plan": eng.last_plan()},        # what the last run launched (cta_group 4 = quads), not a host-side guess
         "tflops": flops * (world if vocab_mode else 1) / (ms_step * 1e-3) / 1e12,
         "pct_of_bf16_peak_burst": 100.0 * flops / (ms_step * 1e-3) / 1e12 / peaks["bf16_tflops"],
         "roofline": {"bound": "tensor", "kernel": "sq_fused_score_kernel", "achieved": achieved, "peak": peak,
@@ -400,7 +400,7 @@ def run_ours(args):
             line["configs"][name] = {"value": i2["T"] / (ms2 * 1e-3), "ms_per_step": ms2, "kernel_ms": km, "T": i2["T"], "steps": nsteps,
                                      "tflops_kernel": f2 / (km * 1e-3) / 1e12, "frac": f2 / (km * 1e-3) / 1e12 / peak,
                                      "frac_of_burst": f2 / (km * 1e-3) / 1e12 / peaks["bf16_tflops"],
-                                     "plan": {n: v for n, v in sq.plan(w2.d, w2.V, i2["T"], w2.k, num_sms=sms).items() if n != "chunk_vtile"}}
+                                     "plan": {n: v for n, v in e2.last_plan().items() if n != "chunk_vtile"}}   # what ran (qwen3_32b: quads)
             e2.close()
             del H2, W2, t2, c2, i2
             torch.cuda.empty_cache()

@@ -392,6 +392,12 @@ int sq_score_select_prob(sq_score_ctx *ctx, const float *fitness, const int32_t 
 int sq_score_plan(const sq_score_config *cfg, int64_t num_tokens, int k, int num_sms,
                   sq_score_plan_t *plan);
 
+/* The work decomposition the LAST sq_score_run* call on this ctx actually launched kernel 1 with (sq_score_plan answers
+ * for a ctx-less default and always describes CTA pairs or single CTAs).  plan->cta_group is 1, 2, or 4 = quad scheduling
+ * with W multicast, which runs of more than 200 000 tokens take by default: rows_per_tile is then 512 and the cluster
+ * counts are in quads.  Host-only, no synchronisation.  Errors: INVALID_ARG (null, or no run with T > 0 yet). */
+int sq_score_last_plan(const sq_score_ctx *ctx, sq_score_plan_t *plan);
+
 /* Per-kernel timing for the roofline report.  With profiling enabled, every sq_score_run* with
  * T > 0 records CUDA events on its stream around kernel 1 (fused GEMM + statistics), the
  * finalize kernel and kernel 2, into a ring of SQ_PROFILE_RING runs (no host synchronisation in the run).

@@ -119,6 +119,8 @@ def lib() -> C.CDLL:
     L.sq_score_kernel_times.restype = C.c_int
     L.sq_score_launch_count.argtypes = [C.c_void_p]
     L.sq_score_launch_count.restype = C.c_int64
+    L.sq_score_last_plan.argtypes = [C.c_void_p, C.POINTER(sq_score_plan_t)]
+    L.sq_score_last_plan.restype = C.c_int
     L.sq_score_reduce_form.argtypes = [C.c_void_p]
     L.sq_score_reduce_form.restype = C.c_int
     L.sq_score_destroy.argtypes = [C.c_void_p]
@@ -454,6 +456,16 @@ class SqScore:
 
     def launch_count(self) -> int:
         return self._L.sq_score_launch_count(self._h)
+
+    def last_plan(self) -> Dict[str, int]:
+        """sq_score_last_plan: the decomposition the last run launched kernel 1 with (cta_group 4 = quads)."""
+        out = sq_score_plan_t()
+        rc = self._L.sq_score_last_plan(self._h, C.byref(out))
+        if rc != 0:
+            raise SqScoreError(rc, "no run with T > 0 on this ctx yet")
+        res = {n: getattr(out, n) for n, _ in sq_score_plan_t._fields_ if n != "chunk_vtile"}
+        res["chunk_vtile"] = list(out.chunk_vtile[: out.num_chunks + 1])
+        return res
 
     def reduce_form(self) -> str:
         """Form of kernel 2 the last call used (sq_score_reduce_form): 'fused', 'tiles', 'stream', 'tail' or 'none'."""

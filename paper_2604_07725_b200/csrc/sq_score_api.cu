@@ -256,6 +256,11 @@ extern "C" const char* sq_score_last_error(const sq_score_ctx* ctx) { return ctx
 
 extern "C" int64_t sq_score_launch_count(const sq_score_ctx* ctx) { return ctx ? ctx->launches : 0; }
 extern "C" int sq_score_reduce_form(const sq_score_ctx* ctx) { return ctx ? ctx->reduce_form : 0; }
+extern "C" int sq_score_last_plan(const sq_score_ctx* ctx, sq_score_plan_t* plan) {
+  if (!ctx || !plan || ctx->plan_cache.T <= 0) return SQ_ERR_INVALID_ARG;
+  *plan = ctx->plan_cache.pl;
+  return SQ_OK;
+}
 
 // ------------------------------------------------------------------------------------------ create / destroy
 static int64_t ws_rows_for(const sq_score_config& cfg) {
