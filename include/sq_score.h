@@ -62,6 +62,14 @@ extern "C" {
                                      targets / cu_seqlens, arrival flags, a copy stream and its
                                      events.  Without it those two calls return INVALID_ARG.     */
 
+#define SQ_DEBUG_PREPARE_TWO_PASS   8   /* sq_score_prepare: two-pass kernel instead of register-resident rows */
+#define SQ_DEBUG_NO_SHARED_BOUND   16   /* kernel 1: no shared top-k bound between the chunks of a row     */
+#define SQ_DEBUG_REDUCE_TILES      32   /* kernel 2: three-launch tile form                                */
+#define SQ_DEBUG_REDUCE_FUSED      64   /* kernel 2: single-launch form                                    */
+#define SQ_DEBUG_FINALIZE_WARP    128   /* finalize: one warp per row                                      */
+#define SQ_DEBUG_REDUCE_STREAM    256   /* kernel 2: streaming form wherever it applies                    */
+#define SQ_DEBUG_ALL (8 | 16 | 32 | 64 | 128 | 256)
+
 #define SQ_MAX_CHUNKS       160   /* vocab chunks per row at most                                 */
 #define SQ_MAX_VOCAB   14679840   /* largest V: 65535 vocab tiles (16-bit tile indices) of the narrowest
                                      tile, the MX variant's 224 columns                           */
@@ -86,6 +94,14 @@ typedef struct {
                            flag) may last before kernel 1 traps: 0 = default (60 s), < 0 = for ever.
                            One limit for every wait: in sq_score_run_host the copy of the whole H must
                            land within it                                                          */
+  /* The three below select between code paths that give the SAME results; 0 = the library's choice.  Tests force
+     every path through them; a user has no reason to set them. */
+  int     debug_flags;  /* SQ_DEBUG_* bits                                                        */
+  int     cluster4;     /* quad scheduling with W multicast in kernel 1: 0 = runs of more than 200 000
+                           tokens (default), 1 = every run of more than 4096 tokens, -1 = never       */
+  int     region_mult;  /* length of kernel 1's regions (token tiles between barriers across all gangs) in
+                           units of the gang sizes' common multiple: 0 = default (~160 tiles), > 0 forced,
+                           -1 = no region barrier                                                  */
 } sq_score_config;
 
 /* Output pointers of one run.  Per-token pointers may be NULL (= not wanted; the ctx keeps the

@@ -21,7 +21,8 @@ ERR_INVALID_ARG, ERR_UNSUPPORTED, ERR_CUDA, ERR_NOMEM = -1, -2, -3, -4
 class sq_score_config(C.Structure):
     _fields_ = [("device", C.c_int), ("d", C.c_int), ("vocab", C.c_int), ("max_tokens", C.c_int64),
                 ("max_seqs", C.c_int), ("max_k", C.c_int), ("cta_group", C.c_int), ("num_chunks", C.c_int),
-                ("group_m", C.c_int), ("flags", C.c_int), ("wait_seconds", C.c_int)]
+                ("group_m", C.c_int), ("flags", C.c_int), ("wait_seconds", C.c_int),
+                ("debug_flags", C.c_int), ("cluster4", C.c_int), ("region_mult", C.c_int)]
 
 
 class sq_score_outputs(C.Structure):
@@ -202,11 +203,14 @@ class SqScore:
 
     def __init__(self, d: int, vocab: int, max_tokens: int, max_seqs: int, max_k: int = 20, device: int = 0,
                  cta_group: int = 0, num_chunks: int = 0, group_m: int = 0, reduce_only: bool = False,
-                 staging: bool = False, wait_seconds: int = 0):
-        """`staging=True` (SQ_FLAG_STAGING) also allocates what run_host / run_x need; no run* call ever allocates."""
+                 staging: bool = False, wait_seconds: int = 0, debug_flags: int = 0, cluster4: int = 0, region_mult: int = 0):
+        """`staging=True` (SQ_FLAG_STAGING) also allocates what run_host / run_x need; no run* call ever allocates.
+        `debug_flags` (SQ_DEBUG_* bits), `cluster4` and `region_mult` choose between code paths with the same results
+        (include/sq_score.h); tests force each path through them."""
         self._L = lib()
         self.cfg = sq_score_config(device, d, vocab, max_tokens, max_seqs, max_k, cta_group, num_chunks, group_m,
-                                   (FLAG_REDUCE_ONLY if reduce_only else 0) | (FLAG_STAGING if staging else 0), wait_seconds)
+                                   (FLAG_REDUCE_ONLY if reduce_only else 0) | (FLAG_STAGING if staging else 0), wait_seconds,
+                                   int(debug_flags or 0), cluster4, region_mult)
         h = C.c_void_p()
         rc = self._L.sq_score_create(C.byref(self.cfg), C.byref(h))
         if rc != 0:

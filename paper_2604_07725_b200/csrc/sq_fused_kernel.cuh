@@ -88,10 +88,6 @@ struct FusedParams {
   int sf_h_blocks;          // MX variant: 128-row blocks of H in the scale layout (rows of tmap_sfa per k-block)
   int vocab_offset;         // W is rows [vocab_offset, vocab_offset + V) of a larger LM head (vocab-parallel shard):
                             // targets and the reported vocabulary ids are global, columns local
-#ifdef SQ_PROBES
-  int probe_flags;          // builder's A/B probes, WRONG RESULTS (compiled only with -DSQ_PROBES): bit0 = epilogue skips
-                            // the statistics, bit1 / bit2 = W / H boxes of half height (L2->SM traffic probes)
-#endif
   uint16_t chunk_vt[MAX_CHUNKS + 1];   // chunk c sweeps vocab tiles [chunk_vt[c], chunk_vt[c+1]) (widths differ between gangs)
 };
 
@@ -378,10 +374,6 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       uint32_t stage_tx = Cfg::STAGE_TX * CG;   // the pair leader's barrier counts both CTAs' bytes
-#ifdef SQ_PROBES
-      if (p.probe_flags & 2) stage_tx -= (Cfg::B_BYTES / 2) * CG;   // probe: W boxes of half height
-      if (p.probe_flags & 4) stage_tx -= (Cfg::A_BYTES / 2) * CG;   // probe: H boxes of half height
-#endif
       unsigned int epoch = 0;
       for (int gu = 0; gu < gc.num_iters; ++gu) {
         Unit un;
@@ -512,9 +504,6 @@ sq_fused_score_kernel(const __grid_constant__ CUtensorMap tmap_h, const __grid_c
         const int colbase = vt * BN;
         int ngroups = min(BN, p.V - colbase + 31) >> 5;   // 32-column groups with a valid column
         if (AROWS < BLOCK_M && q * 32 >= AROWS) ngroups = 0;   // this warp's TMEM lanes hold no token rows
-#ifdef SQ_PROBES
-        if (p.probe_flags & 1) ngroups = 0;        // probe: the epilogue skips the statistics
-#endif
         for (int g = 0; g < ngroups; ++g) {
           float r[32];
           tmem_ld_32x32(lane_addr + acc * BN + g * 32, r);

@@ -75,7 +75,7 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
   return ok != 0;
 }
 // Bounded wait: after `limit` clock cycles (0 = no limit) a protocol bug traps (a CUDA error on the host) instead of
-// hanging the GPU.  The limit is the caller's (sq_score_config / SQ_SCORE_WAIT_SECONDS): generous by default, because a
+// hanging the GPU.  The limit is the caller's (sq_score_config.wait_seconds): generous by default, because a
 // time-sliced, debugged or sanitised process can legitimately wait for a long time.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity, long long limit) {
   if (mbar_try_wait(bar, parity)) return;

@@ -47,7 +47,7 @@ struct sq_score_ctx {
   int* seq_done = nullptr;   // [max_seqs] per-sequence tile counters of the single-launch reduction (zero between runs)
   int* tile_base = nullptr; int* tile_seq = nullptr; float4* red_sum = nullptr; float* red_min = nullptr; int64_t red_tiles_max = 0;
   int cluster4 = -1;                 // quad scheduling with W multicast (sq_fused_kernel.cuh): -1 = for very long runs only (default),
-                                     // 0 = never, 1 = every run of more than 4096 tokens (SQ_SCORE_CLUSTER4)
+                                     // 0 = never, 1 = every run of more than 4096 tokens (cfg.clusTER4)
   int max_clusters[5] = {0, 0, 0, 0, 0};   // [cg]: clusters of kernel 1 the device holds at once (occupancy query at create)
   int region_mult = 0;               // region barrier of kernel 1: regions of region_mult x (a common multiple of the gang sizes) token tiles; < 0: off
   long long wait_limit = 0;          // cycles a device-side wait may last before kernel 1 traps (0 = for ever)
@@ -68,9 +68,6 @@ struct sq_score_ctx {
   struct TmapSlot { const void* base = nullptr; int64_t rows = -1; int d = 0, box = 0, kind = -1; CUtensorMap map; } tmaps[4];
   int64_t ev_count = 0, ev_read = 0;   // runs recorded / runs already handed out by sq_score_profile_read
   cudaEvent_t (*ev)[4] = nullptr;      // [SQ_PROFILE_RING][4]
-#ifdef SQ_PROBES
-  int probe_flags = 0;                 // env SQ_SCORE_PROBE: wrong-results A/B probes, builder's builds only
-#endif
 };
 
 static thread_local char g_create_err[512] = {0};
@@ -316,8 +313,8 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   if (cfg->max_k < 1 || cfg->max_k > SQ_MAX_K)
     return set_err(nullptr, SQ_ERR_INVALID_ARG, "max_k must be in 1..%d", SQ_MAX_K);
   if (cfg->cta_group < 0 || cfg->cta_group > 2 || cfg->num_chunks < 0 || cfg->group_m < 0 ||
-      (cfg->flags & ~(SQ_FLAG_REDUCE_ONLY | SQ_FLAG_STAGING)))
-    return set_err(nullptr, SQ_ERR_INVALID_ARG, "cta_group must be 0, 1 or 2; num_chunks, group_m >= 0; unknown flag");
+      (cfg->flags & ~(SQ_FLAG_REDUCE_ONLY | SQ_FLAG_STAGING)) || (cfg->debug_flags & ~SQ_DEBUG_ALL) || cfg->region_mult < -1)
+    return set_err(nullptr, SQ_ERR_INVALID_ARG, "cta_group must be 0, 1 or 2; num_chunks, group_m >= 0; region_mult >= -1; unknown flag");
   if (cfg->vocab > SQ_MAX_VOCAB)   // 65535 tiles of the narrowest tile width (224 columns, MX variant)
     return set_err(nullptr, SQ_ERR_UNSUPPORTED, "vocab = %d exceeds %d (vocab-tile indices are 16-bit: at most 65535 tiles of 224 columns)",
                    cfg->vocab, SQ_MAX_VOCAB);
@@ -345,21 +342,16 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
   ctx->cfg = *cfg;
   ctx->num_sms = prop.multiProcessorCount;
   ctx->cap_max = topk_cap_for(cfg->max_k);
-  // SQ_SCORE_DEBUG selects between code paths that give the SAME results (tests force each of them): bit 3 = two-pass
+  // cfg.debug_flags selects between code paths that give the SAME results (tests force each of them): bit 3 = two-pass
   // prepare kernel, bit 4 = no shared top-k bound, bit 5 / 6 = three-launch / single-launch kernel 2, bit 7 = one warp
   // per row in the finalize kernel
-  if (const char* dbg = getenv("SQ_SCORE_DEBUG")) ctx->debug_flags = atoi(dbg) & (8 | 16 | 32 | 64 | 128 | 256);
-#ifdef SQ_PROBES
-  if (const char* lim = getenv("SQ_SCORE_MAX_SMS"))   // probe: plan for fewer SMs
-    if (atoi(lim) >= 2 && atoi(lim) < ctx->num_sms) ctx->num_sms = atoi(lim);
-  if (const char* pr = getenv("SQ_SCORE_PROBE")) ctx->probe_flags = atoi(pr);
-#endif
-  {   // device-side waits trap after cfg.wait_seconds (default 60 s; SQ_SCORE_WAIT_SECONDS overrides, e.g. under a sanitizer)
+  ctx->debug_flags = cfg->debug_flags;
+  ctx->region_mult = cfg->region_mult;                                  // 0 = default, > 0 forced, -1 = no region barrier
+  ctx->cluster4 = cfg->cluster4 == 0 ? -1 : (cfg->cluster4 > 0 ? 1 : 0);   // -1 = long runs only (default), 1 = always, 0 = never
+  {   // device-side waits trap after cfg.wait_seconds (default 60 s; raise it under a sanitizer)
     int khz = 0;
     cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, cfg->device);
     long long sec = cfg->wait_seconds == 0 ? 60 : cfg->wait_seconds;
-    if (const char* rm = getenv("SQ_SCORE_REGION_MULT")) ctx->region_mult = atoi(rm);   // experiment knob (same results): -1 = no region barrier
-    if (const char* w = getenv("SQ_SCORE_WAIT_SECONDS")) sec = atoll(w) == 0 ? -1 : atoll(w);
     sec = std::min<long long>(sec, 1000000000LL);   // keeps the cycle count far inside 63 bits (31 years are for ever too)
     ctx->wait_limit = sec < 0 ? 0 : sec * (long long)std::max(khz, 1000000) * 1000LL;
   }
@@ -484,7 +476,6 @@ extern "C" int sq_score_create(const sq_score_config* cfg, sq_score_ctx** out) {
       }
       ctx->max_clusters[cg] = n;
     }
-    if (const char* c4 = getenv("SQ_SCORE_CLUSTER4")) ctx->cluster4 = atoi(c4);
     if (ctx->cluster4) ctx->max_clusters[4] = ctx->max_clusters[2] / 2;   // quads: 4 consecutive CTAs, placed as one cluster of 4 or two of 2
     if (ctx->max_clusters[4] * 4 != ctx->num_sms / 4 * 4) ctx->max_clusters[4] = 0;   // (only when every quad fits at once)
   }
@@ -597,7 +588,7 @@ static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t s
   // Single launch (sq_reduce_kernel.cuh) when the whole problem is one wave of CTAs -- the scoring pipeline's case, a few
   // dozen tiles, where the three launches are pure latency (20 -> 8 us).  On large inputs the three-launch form is 2x
   // faster (measured 0.099 vs 0.218 ms on 3.6e7 tokens: a persistent CTA pays the fence + atomic + barriers per tile in
-  // series), so it stays.  SQ_SCORE_DEBUG bit 5 / bit 6 force the three-launch / single-launch form (tests).
+  // series), so it stays.  cfg.debug_flags bit 5 / bit 6 force the three-launch / single-launch form (tests).
   const size_t fused_smem = sq::RED_SMEM_BYTES + (size_t)(rp.B + 1) * sizeof(int);
   const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(6, (size_t)(220 * 1024) / (fused_smem + 1024)));
   const bool one_wave = tiles <= (int64_t)ctx->num_sms * per_sm && rp.B <= 2048;
@@ -613,7 +604,7 @@ static int launch_reduce(sq_score_ctx* ctx, sq::ReduceParams& rp, cudaStream_t s
     return SQ_OK;
   }
   // Streaming form (two launches, sq_reduce_kernel.cuh): fixed 4096-token blocks whose loads depend on nothing, every
-  // sequence boundary handled in the fold.  Needs 16-byte aligned arrays and RS_WMIN <= window <= RS_WMAX; SQ_SCORE_DEBUG bit 8 forces
+  // sequence boundary handled in the fold.  Needs 16-byte aligned arrays and RS_WMIN <= window <= RS_WMAX; cfg.debug_flags bit 8 forces
   // it on small inputs (tests).
   // Narrow windows stay with the tile forms: the streaming form takes S(j) as a difference of two block-wide prefix sums,
   // whose fp32 rounding (~1e-7 of the prefix) is only negligible against a sum of >= RS_WMIN elements.
@@ -855,10 +846,6 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     // decode-shaped, at most 64 / 32 rows: 64- / 32-row H boxes, five / six stages
     const int a_rows = (pl.cta_group == 1 && T <= 32) ? 32 : ((pl.cta_group == 1 && T <= 64) ? 64 : sq::BLOCK_M);
     int h_box = a_rows, w_box = tile_n / pl.cta_group;
-#ifdef SQ_PROBES
-    if (ctx->probe_flags & 4) h_box /= 2;
-    if (ctx->probe_flags & 2) w_box /= 2;
-#endif
     int rc = make_tmap(ctx, &th, H, T, d, h_box, f8, 0);
     if (rc != SQ_OK) return rc;
     rc = make_tmap(ctx, &tw, W, V, d, w_box, f8, 1);
@@ -894,9 +881,6 @@ static int run_impl(sq_score_ctx* ctx, const void* H, const void* W, const int32
     fp.part_m = ctx->part_m; fp.part_s = ctx->part_s; fp.part_u = ctx->part_u;
     fp.part_cs = ctx->part_cs; fp.part_cu = ctx->part_cu;
     fp.part_topv = ctx->part_topv; fp.part_topi = ctx->part_topi; fp.zt = ctx->zt;
-#ifdef SQ_PROBES
-    fp.probe_flags = ctx->probe_flags;
-#endif
     fp.vocab_offset = vocab_offset;
     fp.h_scale = h_scale; fp.w_scale = w_scale; fp.sf_h_blocks = (int)sf_h_blocks;
     fp.h_ready = h_ready; fp.flag_rows = flag_rows;

@@ -65,7 +65,8 @@ def test_create_fails_loudly_without_gpu():
 def test_create_rejects_bad_config_before_touching_cuda():
     L = sq.lib()
     h = ctypes.c_void_p()
-    bad = [dict(d=0), dict(vocab=0), dict(max_tokens=0), dict(max_seqs=0), dict(max_k=0), dict(max_k=33), dict(cta_group=3), dict(flags=4)]
+    bad = [dict(d=0), dict(vocab=0), dict(max_tokens=0), dict(max_seqs=0), dict(max_k=0), dict(max_k=33), dict(cta_group=3), dict(flags=4),
+           dict(debug_flags=1), dict(debug_flags=512), dict(region_mult=-2)]
     for kw in bad:
         base = dict(device=0, d=64, vocab=1024, max_tokens=256, max_seqs=4, max_k=5, cta_group=0, num_chunks=0, group_m=0, flags=0)
         base.update(kw)

@@ -110,7 +110,7 @@ def test_eightbit_full_size_qwen3_8b_sampled_rows(variant):
 
 def test_fp8_run_of_more_than_200000_tokens_takes_the_quad_kernel_by_default():
     """No environment switch: T > 200 000 alone selects quad scheduling with W multicast (sq_score_last_plan says so), in
-    FP8 -- launch_fused<2, CAP, MODE_F8, 4>, which the small tests only reach with SQ_SCORE_CLUSTER4=1."""
+    FP8 -- launch_fused<2, CAP, MODE_F8, 4>, which the small tests only reach with sq_score_config.cluster4 = 1."""
     wl = workloads.custom(name="fp8_quad", d=1024, V=50304, B=64, len_lo=2900, len_hi=3700, k=20, window=256, seed=91,
                           w_std=0.03, planted_frac=0.5, planted_scale=3.0, rmsnorm=True)
     inp = workloads.make_inputs(wl)

@@ -187,12 +187,7 @@ def test_reduce_alone_guarded_arrays_and_poisoned_workspace(window, dbg):
     for gd in G.values():
         gd.raw[GUARD + gd.n:].view(torch.float32)[:] = float("nan")
     import os
-    if dbg:
-        os.environ["SQ_SCORE_DEBUG"] = dbg                # bit 8: kernel 2's streaming form (fixed blocks, look-ahead past the block)
-    try:
-        eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
-    finally:
-        os.environ.pop("SQ_SCORE_DEBUG", None)
+    eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True, debug_flags=int(dbg or 0))
     eng.debug_fill_workspace(0xFF)
     out = eng.reduce(G["lp"].t, G["en"].t, G["cf"].t, cu.to(DEV), window)
     torch.cuda.synchronize()

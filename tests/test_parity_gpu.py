@@ -385,18 +385,14 @@ def test_full_size_config_sampled_rows_and_all_sequences(name):
 
 # ------------------------------------------------------------------------------------------ kernel 2 alone
 def _reduce_all_forms(sq, make_engine, call, stream_form="stream"):
-    """Kernel 2 forced into its single-launch form (SQ_SCORE_DEBUG bit 6), its three-launch tile form (bit 5) and its
+    """Kernel 2 forced into its single-launch form (sq_score_config.debug_flags bit 6), its three-launch tile form (bit 5) and its
     streaming form (bit 8; `stream_form` = "tiles" where the window is too wide for it and the tile form takes over).  The
     two tile forms must agree bit for bit; returns (single-launch outputs, streaming outputs) -- the caller checks both
     against the oracle."""
     import os
     outs = []
     for dbg in ("64", "32", "256"):
-        os.environ["SQ_SCORE_DEBUG"] = dbg
-        try:
-            eng = make_engine()
-        finally:
-            os.environ.pop("SQ_SCORE_DEBUG", None)
+        eng = make_engine(int(dbg))
         n0 = eng.launch_count()
         o = call(eng)
         torch.cuda.synchronize()
@@ -424,7 +420,7 @@ def test_reduce_kernel_alone(window):
     cf[30000:30040] = 0.5                      # a dip the minimum window must find
     dev = torch.device("cuda:0")
     a = [x.to(dev) for x in (lp, en, cf, cu)]
-    out, out_s = _reduce_all_forms(sq, lambda: sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True),
+    out, out_s = _reduce_all_forms(sq, lambda dbg: sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True, debug_flags=dbg),
                                    lambda eng: eng.reduce(a[0], a[1], a[2], a[3], window),
                                    stream_form="stream" if 128 <= window <= 2048 else "tiles")
     ref = O.sequence_scores(lp.numpy(), en.numpy(), cf.numpy(), cu.numpy(), window)
@@ -455,12 +451,7 @@ def test_reduce_alignment_targets_and_array_end(offset, with_targets, dbg):
         buf[offset:offset + T] = x.to(dev)
         return buf[offset:offset + T]
     import os
-    if dbg:
-        os.environ["SQ_SCORE_DEBUG"] = dbg               # bit 8: the streaming form wherever it applies (aligned, window <= 2048)
-    try:
-        eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
-    finally:
-        os.environ.pop("SQ_SCORE_DEBUG", None)
+    eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True, debug_flags=int(dbg or 0))
     valid = ((tg >= 0) & (tg < 1000)).numpy() if with_targets else None
     for window in (1, 6, 1023, 2047, 2048, 2049, 2050, 8192, 8195, 30000):
         out = eng.reduce(place(lp), place(en), place(cf), cu.to(dev), window, targets=place(tg) if with_targets else None)
@@ -476,7 +467,7 @@ def test_reduce_many_sequences():
     r = workloads.reduction_inputs(3000, 1, 3000, seed=5)
     dev = torch.device("cuda:0")
     a = [r[n].to(dev) for n in ("target_logprob", "entropy", "conf", "cu_seqlens")]
-    out, out_s = _reduce_all_forms(sq, lambda: sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True),
+    out, out_s = _reduce_all_forms(sq, lambda dbg: sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True, debug_flags=dbg),
                                    lambda eng: eng.reduce(a[0], a[1], a[2], a[3], 256))
     ref = O.sequence_scores(r["target_logprob"].numpy(), r["entropy"].numpy(), r["conf"].numpy(), r["cu_seqlens"].numpy(), 256)
     check_seqs(out, ref)
@@ -492,12 +483,7 @@ def test_reduce_more_sequences_than_the_single_launch_form_holds(dbg, form, wind
     sq = _sq()
     r = workloads.reduction_inputs(13000, 0, 40, seed=6)
     dev = torch.device("cuda:0")
-    if dbg:
-        os.environ["SQ_SCORE_DEBUG"] = dbg
-    try:
-        eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True)
-    finally:
-        os.environ.pop("SQ_SCORE_DEBUG", None)
+    eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True, debug_flags=int(dbg or 0))
     out = eng.reduce(r["target_logprob"].to(dev), r["entropy"].to(dev), r["conf"].to(dev), r["cu_seqlens"].to(dev), window)
     torch.cuda.synchronize()
     assert eng.launch_count() == (2 if form == "stream" else 3) and eng.reduce_form() == form
@@ -520,11 +506,7 @@ def test_reduce_streaming_form_many_sequences_per_range_and_one_long_sequence():
     lp = -(torch.rand(T, generator=g) * 12); en = torch.rand(T, generator=g) * 11; cf = 3 + torch.rand(T, generator=g) * 12
     cf[20000:20100] = 0.5
     dev = torch.device("cuda:0")
-    os.environ["SQ_SCORE_DEBUG"] = "256"
-    try:
-        eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True)
-    finally:
-        os.environ.pop("SQ_SCORE_DEBUG", None)
+    eng = sq.SqScore(64, 1000, max_tokens=T, max_seqs=len(lens), max_k=5, reduce_only=True, debug_flags=int("256" or 0))
     for window in (128, 129, 130, 131, 255, 256, 257, 1000, 2047, 2048):
         out = eng.reduce(lp.to(dev), en.to(dev), cf.to(dev), cu.to(dev), window)
         torch.cuda.synchronize()
@@ -542,11 +524,7 @@ def test_reduce_streaming_form_every_sequence_empty_then_a_normal_call():
     sq = _sq()
     r = workloads.reduction_inputs(300, 100, 900, seed=9)
     dev = torch.device("cuda:0")
-    os.environ["SQ_SCORE_DEBUG"] = "256"
-    try:
-        eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True)
-    finally:
-        os.environ.pop("SQ_SCORE_DEBUG", None)
+    eng = sq.SqScore(64, 1000, max_tokens=r["T"], max_seqs=r["B"], max_k=5, reduce_only=True, debug_flags=int("256" or 0))
     a = [r[n].to(dev) for n in ("target_logprob", "entropy", "conf", "cu_seqlens")]
     empty = eng.reduce(a[0], a[1], a[2], torch.zeros_like(a[3]), 256)
     out = eng.reduce(a[0], a[1], a[2], a[3], 256)                 # enqueued right behind it, no host sync between
@@ -618,7 +596,7 @@ def test_scoring_pipeline_takes_the_streaming_form_for_many_sequences():
 
 @pytest.mark.parametrize("d,V,B,lo,hi,gm", [(256, 3000, 6, 700, 1100, 0), (200, 1003, 9, 500, 900, 3), (512, 5000, 4, 1500, 2500, 6)])
 def test_quad_scheduling_with_w_multicast(d, V, B, lo, hi, gm):
-    """SQ_SCORE_CLUSTER4=1 (by default only runs of more than 200 000 tokens -- the full-size qwen3_32b test --
+    """sq_score_config.cluster4 = 1 (by default only runs of more than 200 000 tokens -- the full-size qwen3_32b test --
     take this path): runs of more than 4096 tokens are scheduled in quads of four CTAs that
     the device places as clusters of 4 (W boxes multicast to both CTA pairs) or, where it cannot, as two pairs; 512-row
     token tiles, ragged T, d and V.  Same tolerances against the oracle; bf16 and the FP8 variant."""
@@ -629,11 +607,7 @@ def test_quad_scheduling_with_w_multicast(d, V, B, lo, hi, gm):
     inp = workloads.make_inputs(wl)
     assert inp["T"] > 4096
     dev = torch.device("cuda:0")
-    os.environ["SQ_SCORE_CLUSTER4"] = "1"
-    try:
-        eng = sq.SqScore(d, V, max_tokens=inp["T"], max_seqs=B, max_k=20, group_m=gm)
-    finally:
-        os.environ.pop("SQ_SCORE_CLUSTER4", None)
+    eng = sq.SqScore(d, V, max_tokens=inp["T"], max_seqs=B, max_k=20, group_m=gm, cluster4=1)
     H, W, tg, cu = (inp[n].to(dev) for n in ("H", "W", "targets", "cu_seqlens"))
     out = eng.run(H, W, tg, cu, 20, 64)
     torch.cuda.synchronize()
